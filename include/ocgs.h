@@ -1,0 +1,190 @@
+/* ocgs.h -- C ABI of libocgs: B200 (sm_100a) tile rasterizer for 2D Gaussian surfels, fused with the background
+ * loss and the occlusion-aware pruning statistics of "Object-Centric 2D Gaussian Splatting" (arXiv 2501.08174).
+ *
+ * Citations are PAPER.md:<line> (the paper) or S<n>/O<n> (readings in DESIGN.md / SURVEY.md 8(c), used where the
+ * paper defers the renderer mathematics to the cited 2DGS/3DGS work).
+ *
+ * Conventions
+ *  - Every function returns 0 (OCGS_OK) or a negative error code.  Nothing throws, nothing prints.
+ *  - "device" pointers are CUDA device memory owned by the caller; "host" pointers are ordinary host memory.
+ *    The library allocates no device memory, keeps no global state and is re-entrant per stream.
+ *  - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream).  No entry point
+ *    synchronises except ocgs_check() and ocgs_step_host().  A step can therefore be captured in a CUDA graph.
+ *  - The data-dependent key count K never travels to the host inside a step: kernels read it from the workspace
+ *    header.  If K exceeds `key_capacity` the header error flag is set, later calls of the step become no-ops, and
+ *    ocgs_check() reports OCGS_ERR_CAPACITY with the needed size.
+ *  - Images are planar [C,H,W] fp32, row-major, origin top-left; integer pixel index (ix,iy) is the pixel centre,
+ *    x_idx = fx X/Z + cx - 1/2 (S2).  Surfel parameters are ACTIVATED values: scale > 0, opacity in (0,1),
+ *    quaternion (w,x,y,z) used through the polynomial R(q) without normalisation (S19).
+ *  - Surfel arrays: pos[N,3], scale[N,2], quat[N,4], opacity[N], sh[N,16,3] fp32 (232 B per surfel).
+ *    quat must be 16-byte aligned, scale 8-byte aligned (torch allocations are).
+ */
+#ifndef OCGS_H
+#define OCGS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define OCGS_OK 0
+#define OCGS_ERR_INVALID_ARG (-1)
+#define OCGS_ERR_CAPACITY (-2)    /* K > key_capacity (see ocgs_check) */
+#define OCGS_ERR_CUDA (-3)        /* a CUDA runtime call failed; ocgs_last_cuda_error() has the cudaError_t */
+#define OCGS_ERR_UNSUPPORTED (-4) /* tile != 16, sh_degree > 3, image or surfel count over the limits */
+
+#define OCGS_MAX_DIM 32768        /* width, height <= this (pixel rects are stored as u16 pairs) */
+
+/* world->camera pinhole camera (poses P_i in SE(3)); S2 */
+typedef struct {
+  float view[16]; /* row-major 4x4, camera looks down +z, x right, y down */
+  float fx, fy;   /* focal lengths in pixels */
+  float cx, cy;   /* principal point, corner-origin continuous coordinates (W/2, H/2 = centred) */
+  int width, height;
+} ocgs_camera;
+
+/* constants of the method; ocgs_default_config() fills the defaults */
+typedef struct {
+  int tile;            /* 16 (S5); only 16 is supported */
+  float near_z;        /* 0.2 (S3): cull centres at z <= near, skip hits at z < near */
+  float alpha_min;     /* 1/255 (S11): pairs below this are skipped (expressed through rho_cut, S6) */
+  float alpha_max;     /* 0.99 (S11): cap; gradient through the cap is zero (S12) */
+  float t_min;         /* 1e-4 (S11): stop BEFORE blending the pair that would leave T(1-alpha) < t_min
+                          ("terminated once ... p reaches a threshold opacity close to 1") */
+  float rho_max;       /* 9 (S6): 3-sigma truncation */
+  float filter_sigma2; /* 0.5 (S8): variance of the screen-space low-pass filter, in px^2 */
+  float bg[3];         /* background colour (S13) */
+  float gamma_bg;      /* 0.5: weight of L_b; render_bwd adds gamma (1-M)/(H W) to dL/dA */
+  float tau_contrib;   /* 0 (S17): prune when contrib_sum <= tau */
+  float min_opacity;   /* 0: prune when opacity < min_opacity */
+  int sh_degree;       /* 0..3 (S14) */
+} ocgs_config;
+
+typedef struct {
+  const float *pos, *scale, *quat, *opacity, *sh; /* device */
+  int n;
+} ocgs_surfels;
+
+typedef struct {
+  float *pos, *scale, *quat, *opacity, *sh; /* device, caller-allocated for `capacity` surfels */
+  int capacity;
+} ocgs_surfels_mut;
+
+/* Byte offsets of the workspace sections (all 256-byte aligned), for inspection by tests and tools.  "by id" =
+ * indexed by surfel id; "by rank" = indexed by position in the (depth bits, id) order of the visible surfels. */
+typedef struct {
+  size_t total_bytes;
+  size_t header;        /* ocgs_header */
+  size_t depth_bits;    /* u32 [N]    by id: IEEE bits of the view-space centre depth (Appendix A step 2) */
+  size_t rect;          /* u16 [N,4]  by id: pixel rect ix0,iy0,ix1,iy1 inclusive; undefined when tiles == 0 */
+  size_t tiles;         /* u32 [N]    by id: tiles touched, 0 = culled */
+  size_t clamp;         /* u8  [N]    by id: bit c set when colour channel c was clamped at 0 */
+  size_t rec_id;        /* f32 [N,20] by id: raster record */
+  size_t id_to_rank;    /* u32 [N]    by id: rank, 0xFFFFFFFF when culled */
+  size_t rank_to_id;    /* u32 [N]    by rank (first n_vis entries) */
+  size_t rec;           /* f32 [N,20] by rank */
+  size_t offsets;       /* u32 [N+1]  by rank: exclusive scan of tiles touched */
+  size_t tile_keys;     /* u32 [key_capacity] tile id of each sorted list entry */
+  size_t tile_vals;     /* u32 [key_capacity] rank of each sorted list entry */
+  size_t ranges;        /* u32 [n_tiles,2] [start,end) of each tile's list */
+  size_t grad_rec;      /* f32 [N,20] by rank: backward accumulators */
+  size_t loss_partial;  /* f32 [n_tiles] */
+  size_t final_T;       /* f32 [H,W] transmittance left after the forward pass (exact, not 1 - alpha) */
+  size_t scratch;       /* sort ping-pong buffers, histograms, scan partials */
+} ocgs_ws_layout;
+
+typedef struct {
+  unsigned long long K; /* number of (tile, surfel) keys of the current view */
+  unsigned int n_vis;   /* surfels that survived culling */
+  unsigned int error;   /* bit 0: K > key_capacity */
+} ocgs_header;
+
+/* ---- host-only helpers ------------------------------------------------------------------------------------------ */
+void ocgs_default_config(ocgs_config* cfg);
+/* Fills `out`; returns OCGS_ERR_UNSUPPORTED when the sizes are over the limits. */
+int ocgs_workspace_layout(int n, int width, int height, size_t key_capacity, ocgs_ws_layout* out);
+size_t ocgs_workspace_bytes(int n, int width, int height, size_t key_capacity);
+int ocgs_last_cuda_error(void);
+/* Synchronises `stream`, copies the header to host.  Returns OCGS_ERR_CAPACITY if the error flag is set
+ * (header_out->K then holds the capacity that was needed). header_out: host, may be NULL. */
+int ocgs_check(const void* ws, void* stream, ocgs_header* header_out);
+
+/* ---- (1) per-surfel preprocessing ------------------------------------------------------------------------------
+ * PAPER.md:119 (4.3): "G_j is projected to the image and rasterized, identifying which pixels it can contribute
+ * to"; a surfel outside the frustum "is disqualified from rendering and not assigned to any pixel".  O1 / Appendix A:
+ * view transform, homography M = K'[s_u R t_u | s_v R t_v | p_c], cut-off rho_cut = min(rho_max, 2 ln(o/alpha_min)),
+ * exact AABB of the projected rho_cut ellipse united with the filter disc, integer pixel rect, tile count,
+ * facing normal, SH colour with clamp mask.  Writes ws sections depth_bits, rect, tiles, clamp, rec_id, id_to_rank
+ * (all surfels) and the header (n_vis).  Integer outputs are bit-exact with the oracle (fp32 op order of Appendix A).
+ * ws: device, ocgs_workspace_bytes() bytes, 256-byte aligned.  surfels/cam/cfg: host structs (device arrays inside). */
+int ocgs_preprocess(const ocgs_surfels* surfels, const ocgs_camera* cam, const ocgs_config* cfg, void* ws,
+                    size_t key_capacity, void* stream);
+
+/* ---- (2) depth-ordered tile binning -----------------------------------------------------------------------------
+ * PAPER.md:39 ("tile-based rasterization"), :119 ("rendered in front-to-back order"); O2/O3, S9.  Result: per-tile
+ * lists ordered by (tile id, centre-depth bits, surfel id) and ranges[t] = [lower_bound(t), lower_bound(t+1)).
+ * Two stable LSD radix sorts: all surfels by depth bits (ties keep id order), then the emitted
+ * (tile, rank) keys by tile id.  Writes rank_to_id, rec, offsets, tile_keys, tile_vals, ranges and header.K.
+ * sorted_ids: device u32 [key_capacity] or NULL; when given, receives the surfel id of each list entry. */
+int ocgs_bin_sort(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
+                  uint32_t* sorted_ids, void* stream);
+
+/* ---- (3) forward raster + background loss + visibility statistics ---------------------------------------------------
+ * per pixel, "all assigned Gaussians are rendered in front-to-back order, accumulating their colors
+ * and opacities"; stop rule S11; O4 ray-splat intersection in the surfel's (u,v) frame with the low-pass filter
+ * rho = min(u^2+v^2, |x-c|^2/sigma_f^2) (S8).  Outputs (device): color[3,H,W] (+ T*bg), alpha[H,W] = 1-T (the
+ * "accumulated alphas" A_i), depth[H,W] = sum w z (S10), normal[3,H,W] = sum w n, n_contrib[H,W] = list
+ * position after the last blended pair; ws.final_T[H,W] = T.  loss_bg (device scalar, nullable; needs mask): Eq. 1, PAPER.md:99,
+ * L_b = 1/(H W) sum A (1-M), deterministic reduction.  vis_count[N] / contrib_sum[N] (device, nullable): ACCUMULATE
+ * (+=) the number of pixels that blended surfel j and sum of alpha*T ("we save which Gaussians are used
+ * during the color accumulation step"; O8).  mask: device u8 [H,W], non-zero = object, nullable (= all background). */
+int ocgs_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
+                    float* color, float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg,
+                    uint32_t* vis_count, float* contrib_sum, void* stream);
+
+/* ---- (4) backward ---------------------------------------------------------------------------------------------------
+ * "Through backpropagation, the position, shape, and appearance of all involved Gaussians are updated";
+ * occluded Gaussians receive no gradient (exact zeros).  O7.  Inputs: the forward's n_contrib (and the
+ * lists, records and final transmittance that ocgs_render_fwd of the SAME view left in ws),
+ * upstream gradients dL_dcolor[3,H,W], dL_dalpha[H,W], dL_ddepth[H,W], dL_dnormal[3,H,W] (device; any may be NULL = 0).
+ * With mask != NULL and cfg->gamma_bg != 0 the gradient of gamma*L_b, gamma (1-M)/(H W), is added to dL/dA.
+ * Outputs (device, OVERWRITTEN, zero for culled surfels): d_pos[N,3], d_scale[N,2], d_quat[N,4], d_opacity[N],
+ * d_sh[N,16,3], d_center2d[N,2] (nullable) = M22 * (dL/dM02, dL/dM12), the gradient w.r.t. the projected centre at
+ * fixed depth (densification statistic).  Uses ws.grad_rec as accumulator. */
+int ocgs_render_bwd(const ocgs_surfels* surfels, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
+                    const uint8_t* mask, const uint32_t* n_contrib, const float* dL_dcolor,
+                    const float* dL_dalpha, const float* dL_ddepth, const float* dL_dnormal, float* d_pos, float* d_scale,
+                    float* d_quat, float* d_opacity, float* d_sh, float* d_center2d, void* stream);
+
+/* ---- (5) prune statistics -> mask -> stream compaction ----------------------------------------------------------------
+ * "We propose to assign both G_j and G_k with false" -- a surfel that was never blended in any render
+ * of the interval is removed whether it was outside the frustum or occluded; PAPER.md:101 (opacity threshold), S17.
+ * prune[j] = (vis_count[j]==0) | (contrib_sum[j] <= tau) | (opacity[j] < min_opacity).  Survivors keep ascending id
+ * order: out[remap[j]] = in[j], remap[j] = -1 when pruned.  prune_mask u8[N], remap i32[N], n_out i32 (device scalar).
+ * `out` may be NULL (mask/remap/count only).  reset_stats != 0 zeroes vis_count / contrib_sum afterwards.
+ * ws: device scratch of at least ocgs_prune_workspace_bytes(n). */
+size_t ocgs_prune_workspace_bytes(int n);
+int ocgs_prune_stats(const ocgs_surfels* in, uint32_t* vis_count, float* contrib_sum, const ocgs_config* cfg,
+                     uint8_t* prune_mask, int32_t* remap, const ocgs_surfels_mut* out, int* n_out, int reset_stats,
+                     void* ws, void* stream);
+
+/* ---- end-to-end step with HOST buffers (bench.py "e2e") ---------------------------------------------------------------
+ * Copies the surfel parameters, mask and upstream colour gradient from (pinned) host memory to the given device
+ * staging buffers, runs (1)-(4) with L_b and statistics on, copies the gradients, the alpha map and loss_bg back and
+ * synchronises.  Every pointer named h_* is host memory, d_* device memory owned by the caller.
+ * h_grads: host [N*58] floats in the order pos(3N) scale(2N) quat(4N) opacity(N) sh(48N).  d_params and d_grads: device
+ * staging of at least 58*N + 16 floats each (sections start on multiples of 4 floats).  key_capacity must be the value
+ * the workspace was sized with (every call of one step passes the same n, image size and key_capacity).
+ * d_images: device [11*H*W] floats (color 3, alpha 1, depth 1, normal 3, dL_dcolor 3) + d_ncontrib u32 [H*W]. */
+int ocgs_step_host(const float* h_pos, const float* h_scale, const float* h_quat, const float* h_opacity,
+                   const float* h_sh, int n, const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask,
+                   const float* h_dL_dcolor, float* h_grads, float* h_alpha, float* h_loss_bg, float* d_params,
+                   uint8_t* d_mask, float* d_images, uint32_t* d_ncontrib, float* d_grads, uint32_t* d_vis_count,
+                   float* d_contrib_sum, float* d_loss_bg, void* ws, size_t key_capacity, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OCGS_H */

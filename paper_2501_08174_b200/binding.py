@@ -1,0 +1,224 @@
+"""Thin ctypes binding over ``csrc/libocgs.so`` (C ABI in ``include/ocgs.h``): argument marshalling only.
+
+Every function has the name of the C entry point it calls; tensors are torch CUDA tensors whose ``data_ptr()`` is
+passed through.  torch is used for device memory and streams, nothing else.  There is no CPU fallback: importing
+this module without the built library, or calling it without a CUDA device, raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "csrc", "libocgs.so")
+
+OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
+EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
+           "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_prune_workspace_bytes",
+           "ocgs_prune_stats", "ocgs_step_host"]
+
+
+class OcgsError(RuntimeError):
+    def __init__(self, fn: str, code: int):
+        names = {-1: "INVALID_ARG", -2: "CAPACITY", -3: "CUDA", -4: "UNSUPPORTED"}
+        extra = f" (cudaError {lib().ocgs_last_cuda_error()})" if code == OCGS_ERR_CUDA else ""
+        super().__init__(f"{fn} failed: OCGS_ERR_{names.get(code, code)}{extra}")
+        self.code = code
+
+
+class ocgs_camera(C.Structure):
+    _fields_ = [("view", C.c_float * 16), ("fx", C.c_float), ("fy", C.c_float), ("cx", C.c_float), ("cy", C.c_float),
+                ("width", C.c_int), ("height", C.c_int)]
+
+
+class ocgs_config(C.Structure):
+    _fields_ = [("tile", C.c_int), ("near_z", C.c_float), ("alpha_min", C.c_float), ("alpha_max", C.c_float),
+                ("t_min", C.c_float), ("rho_max", C.c_float), ("filter_sigma2", C.c_float), ("bg", C.c_float * 3),
+                ("gamma_bg", C.c_float), ("tau_contrib", C.c_float), ("min_opacity", C.c_float), ("sh_degree", C.c_int)]
+
+
+class ocgs_surfels(C.Structure):
+    _fields_ = [("pos", C.c_void_p), ("scale", C.c_void_p), ("quat", C.c_void_p), ("opacity", C.c_void_p), ("sh", C.c_void_p),
+                ("n", C.c_int)]
+
+
+class ocgs_surfels_mut(C.Structure):
+    _fields_ = [("pos", C.c_void_p), ("scale", C.c_void_p), ("quat", C.c_void_p), ("opacity", C.c_void_p), ("sh", C.c_void_p),
+                ("capacity", C.c_int)]
+
+
+_LAYOUT_FIELDS = ["total_bytes", "header", "depth_bits", "rect", "tiles", "clamp", "rec_id", "id_to_rank", "rank_to_id", "rec",
+                  "offsets", "tile_keys", "tile_vals", "ranges", "grad_rec", "loss_partial", "final_T", "scratch"]
+
+
+class ocgs_ws_layout(C.Structure):
+    _fields_ = [(f, C.c_size_t) for f in _LAYOUT_FIELDS]
+
+
+class ocgs_header(C.Structure):
+    _fields_ = [("K", C.c_ulonglong), ("n_vis", C.c_uint), ("error", C.c_uint)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError(f"{_LIB_PATH} is missing: run `python -m paper_2501_08174_b200.build` "
+                               "(or __graft_entry__.build()); there is no CPU fallback")
+        _lib = C.CDLL(_LIB_PATH)
+        _lib.ocgs_workspace_bytes.restype = C.c_size_t
+        _lib.ocgs_prune_workspace_bytes.restype = C.c_size_t
+        for name in EXPORTS:
+            getattr(_lib, name)  # raises AttributeError if a declared symbol is not exported
+    return _lib
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise ValueError("expected a CUDA tensor")
+    if not t.is_contiguous():
+        raise ValueError("expected a contiguous tensor")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _ok(fn: str, code: int):
+    if code != OCGS_OK:
+        raise OcgsError(fn, code)
+
+
+def ocgs_default_config(**kw) -> ocgs_config:
+    c = ocgs_config()
+    lib().ocgs_default_config(C.byref(c))
+    for k, v in kw.items():
+        if k == "bg":
+            c.bg[0], c.bg[1], c.bg[2] = v
+        else:
+            setattr(c, k, v)
+    return c
+
+
+def make_camera(view, fx, fy, cx, cy, width, height) -> ocgs_camera:
+    cam = ocgs_camera()
+    flat = [float(x) for x in (view.reshape(-1).tolist() if hasattr(view, "reshape") else view)]
+    for i in range(16):
+        cam.view[i] = flat[i]
+    cam.fx, cam.fy, cam.cx, cam.cy = float(fx), float(fy), float(cx), float(cy)
+    cam.width, cam.height = int(width), int(height)
+    return cam
+
+
+def camera_from(scene_cam) -> ocgs_camera:
+    return make_camera(scene_cam.view, scene_cam.fx, scene_cam.fy, scene_cam.cx, scene_cam.cy, scene_cam.width, scene_cam.height)
+
+
+def make_surfels(pos, scale, quat, opacity, sh) -> ocgs_surfels:
+    n = int(pos.shape[0])
+    for t, per in ((pos, 3), (scale, 2), (quat, 4), (opacity, 1), (sh, 48)):
+        if t.dtype != torch.float32 or t.numel() != n * per:
+            raise ValueError("surfel arrays must be float32 with shapes [N,3],[N,2],[N,4],[N],[N,16,3]")
+    return ocgs_surfels(_ptr(pos), _ptr(scale), _ptr(quat), _ptr(opacity), _ptr(sh), n)
+
+
+def ocgs_workspace_layout(n: int, width: int, height: int, key_capacity: int) -> ocgs_ws_layout:
+    L = ocgs_ws_layout()
+    _ok("ocgs_workspace_layout", lib().ocgs_workspace_layout(C.c_int(n), C.c_int(width), C.c_int(height), C.c_size_t(key_capacity), C.byref(L)))
+    return L
+
+
+def ocgs_workspace_bytes(n: int, width: int, height: int, key_capacity: int) -> int:
+    return int(lib().ocgs_workspace_bytes(C.c_int(n), C.c_int(width), C.c_int(height), C.c_size_t(key_capacity)))
+
+
+def ocgs_check(ws: torch.Tensor, stream=None, raise_on_error: bool = True) -> ocgs_header:
+    h = ocgs_header()
+    code = lib().ocgs_check(_ptr(ws), _stream(stream), C.byref(h))
+    if code != OCGS_OK and raise_on_error:
+        raise OcgsError("ocgs_check", code)
+    return h
+
+
+def ocgs_preprocess(surfels: ocgs_surfels, cam: ocgs_camera, cfg: ocgs_config, ws: torch.Tensor, key_capacity: int, stream=None):
+    _ok("ocgs_preprocess", lib().ocgs_preprocess(C.byref(surfels), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity), _stream(stream)))
+
+
+def ocgs_bin_sort(n: int, cam: ocgs_camera, cfg: ocgs_config, ws: torch.Tensor, key_capacity: int, sorted_ids=None, stream=None):
+    _ok("ocgs_bin_sort", lib().ocgs_bin_sort(C.c_int(n), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity), _ptr(sorted_ids), _stream(stream)))
+
+
+def ocgs_render_fwd(n, cam, cfg, ws, key_capacity, mask, color, alpha, depth, normal, n_contrib, loss_bg=None, vis_count=None,
+                    contrib_sum=None, stream=None):
+    _ok("ocgs_render_fwd", lib().ocgs_render_fwd(C.c_int(n), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity), _ptr(mask),
+                                                 _ptr(color), _ptr(alpha), _ptr(depth), _ptr(normal), _ptr(n_contrib), _ptr(loss_bg),
+                                                 _ptr(vis_count), _ptr(contrib_sum), _stream(stream)))
+
+
+def ocgs_render_bwd(surfels, cam, cfg, ws, key_capacity, mask, n_contrib, dL_dcolor, dL_dalpha, dL_ddepth, dL_dnormal, d_pos, d_scale,
+                    d_quat, d_opacity, d_sh, d_center2d=None, stream=None):
+    _ok("ocgs_render_bwd", lib().ocgs_render_bwd(C.byref(surfels), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity), _ptr(mask),
+                                                 _ptr(n_contrib), _ptr(dL_dcolor), _ptr(dL_dalpha), _ptr(dL_ddepth), _ptr(dL_dnormal),
+                                                 _ptr(d_pos), _ptr(d_scale), _ptr(d_quat), _ptr(d_opacity), _ptr(d_sh), _ptr(d_center2d),
+                                                 _stream(stream)))
+
+
+def ocgs_prune_workspace_bytes(n: int) -> int:
+    return int(lib().ocgs_prune_workspace_bytes(C.c_int(n)))
+
+
+def ocgs_prune_stats(surfels, vis_count, contrib_sum, cfg, prune_mask, remap, out: Optional[ocgs_surfels_mut], n_out, reset_stats, ws,
+                     stream=None):
+    _ok("ocgs_prune_stats", lib().ocgs_prune_stats(C.byref(surfels), _ptr(vis_count), _ptr(contrib_sum), C.byref(cfg), _ptr(prune_mask),
+                                                   _ptr(remap), C.byref(out) if out is not None else None, _ptr(n_out),
+                                                   C.c_int(int(reset_stats)), _ptr(ws), _stream(stream)))
+
+
+def ocgs_step_host(h_pos, h_scale, h_quat, h_opacity, h_sh, n, cam, cfg, h_mask, h_dL_dcolor, h_grads, h_alpha, h_loss_bg, d_params,
+                   d_mask, d_images, d_ncontrib, d_grads, d_vis_count, d_contrib_sum, d_loss_bg, ws, key_capacity, stream=None):
+    def hp(t):
+        return None if t is None else C.c_void_p(t.data_ptr())
+    _ok("ocgs_step_host", lib().ocgs_step_host(hp(h_pos), hp(h_scale), hp(h_quat), hp(h_opacity), hp(h_sh), C.c_int(n), C.byref(cam),
+                                               C.byref(cfg), hp(h_mask), hp(h_dL_dcolor), hp(h_grads), hp(h_alpha), hp(h_loss_bg),
+                                               _ptr(d_params), _ptr(d_mask), _ptr(d_images), _ptr(d_ncontrib), _ptr(d_grads),
+                                               _ptr(d_vis_count), _ptr(d_contrib_sum), _ptr(d_loss_bg), _ptr(ws),
+                                               C.c_size_t(key_capacity), _stream(stream)))
+
+
+# ---- allocation helpers (device memory only; no arithmetic) --------------------------------------------------------
+
+def alloc_workspace(n: int, width: int, height: int, key_capacity: int, device="cuda") -> torch.Tensor:
+    nbytes = ocgs_workspace_bytes(n, width, height, key_capacity)
+    if nbytes == 0:
+        raise OcgsError("ocgs_workspace_bytes", OCGS_ERR_UNSUPPORTED)
+    return torch.empty(nbytes, dtype=torch.uint8, device=device)
+
+
+def ws_section(ws: torch.Tensor, layout: ocgs_ws_layout, name: str, dtype: torch.dtype, count: int) -> torch.Tensor:
+    """View of a workspace section (see ocgs_ws_layout in include/ocgs.h)."""
+    off = getattr(layout, name)
+    nbytes = count * torch.empty(0, dtype=dtype).element_size()
+    return ws[off:off + nbytes].view(dtype)
+
+
+def alloc_outputs(width: int, height: int, device="cuda") -> Dict[str, torch.Tensor]:
+    f = dict(dtype=torch.float32, device=device)
+    return dict(color=torch.empty((3, height, width), **f), alpha=torch.empty((height, width), **f),
+                depth=torch.empty((height, width), **f), normal=torch.empty((3, height, width), **f),
+                n_contrib=torch.empty((height, width), dtype=torch.int32, device=device), loss_bg=torch.zeros(1, **f))
+
+
+def alloc_grads(n: int, device="cuda") -> Dict[str, torch.Tensor]:
+    f = dict(dtype=torch.float32, device=device)
+    return dict(d_pos=torch.empty((n, 3), **f), d_scale=torch.empty((n, 2), **f), d_quat=torch.empty((n, 4), **f),
+                d_opacity=torch.empty(n, **f), d_sh=torch.empty((n, 16, 3), **f), d_center2d=torch.empty((n, 2), **f))

@@ -1,0 +1,240 @@
+// api.cu -- extern "C" entry points of libocgs (include/ocgs.h): argument checks, workspace carving, stage launches.
+#include <string.h>
+
+#include "common.cuh"
+
+namespace ocgs {
+
+thread_local int g_last_cuda_error = 0;
+
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+bool carve_workspace(void* ws, int n, int width, int height, size_t key_capacity, Workspace* out, ocgs_ws_layout* layout) {
+  if (n < 0 || width <= 0 || height <= 0 || width > OCGS_MAX_DIM || height > OCGS_MAX_DIM) return false;
+  if (key_capacity > 0xFFFFFFF0ull || (size_t)n > 0x7FFFFFF0ull) return false;
+  const int tiles_x = (width + kTile - 1) / kTile, tiles_y = (height + kTile - 1) / kTile;
+  const size_t n_tiles = (size_t)tiles_x * tiles_y;
+  const size_t N = (size_t)n, K = key_capacity;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { const size_t o = off; off = align256(off + bytes); return o; };
+  ocgs_ws_layout L;
+  memset(&L, 0, sizeof(L));
+  L.header = take(256);
+  L.depth_bits = take(N * 4);
+  L.rect = take(N * 8);
+  L.tiles = take(N * 4);
+  L.clamp = take(N);
+  L.rec_id = take(N * kRec * 4);
+  L.id_to_rank = take(N * 4);
+  L.rank_to_id = take(N * 4);
+  L.rec = take(N * kRec * 4);
+  L.offsets = take((N + 1) * 4);
+  L.tile_keys = take(K * 4);
+  L.tile_vals = take(K * 4);
+  L.ranges = take(n_tiles * 8);
+  L.grad_rec = take(N * kRec * 4);
+  L.loss_partial = take(n_tiles * 4);
+  L.final_T = take((size_t)width * height * 4);
+  L.scratch = off;
+  const size_t o_dkeyA = take(N * 4), o_dkeyB = take(N * 4), o_dvalB = take(N * 4);
+  const size_t o_tkeyB = take(K * 4), o_tvalB = take(K * 4);
+  const size_t max_items = N > K ? N : K;
+  const size_t o_hist = take((div_up(max_items, kSortTile) + 1) * kRadix * 4);
+  const size_t o_dtot = take(kRadix * 4);
+  const size_t o_tcount = take(N * 4);
+  const size_t o_bsum = take((div_up(N, 1024) + 2) * 4);
+  L.total_bytes = off;
+  if (layout) *layout = L;
+  if (out) {
+    char* b = (char*)ws;
+    out->header = (ocgs_header*)(b + L.header);
+    out->depth_bits = (uint32_t*)(b + L.depth_bits);
+    out->rect = (ushort4*)(b + L.rect);
+    out->tiles = (uint32_t*)(b + L.tiles);
+    out->clamp = (uint8_t*)(b + L.clamp);
+    out->rec_id = (float*)(b + L.rec_id);
+    out->id_to_rank = (uint32_t*)(b + L.id_to_rank);
+    out->rank_to_id = (uint32_t*)(b + L.rank_to_id);
+    out->rec = (float*)(b + L.rec);
+    out->offsets = (uint32_t*)(b + L.offsets);
+    out->tile_keys = (uint32_t*)(b + L.tile_keys);
+    out->tile_vals = (uint32_t*)(b + L.tile_vals);
+    out->ranges = (uint32_t*)(b + L.ranges);
+    out->grad_rec = (float*)(b + L.grad_rec);
+    out->loss_partial = (float*)(b + L.loss_partial);
+    out->final_T = (float*)(b + L.final_T);
+    out->dkeyA = (uint32_t*)(b + o_dkeyA);
+    out->dkeyB = (uint32_t*)(b + o_dkeyB);
+    out->dvalB = (uint32_t*)(b + o_dvalB);
+    out->tkeyB = (uint32_t*)(b + o_tkeyB);
+    out->tvalB = (uint32_t*)(b + o_tvalB);
+    out->hist = (uint32_t*)(b + o_hist);
+    out->digit_total = (uint32_t*)(b + o_dtot);
+    out->tcount = (uint32_t*)(b + o_tcount);
+    out->blocksum = (uint32_t*)(b + o_bsum);
+    out->n = n; out->width = width; out->height = height;
+    out->tiles_x = tiles_x; out->tiles_y = tiles_y; out->n_tiles = (int)n_tiles;
+    out->key_capacity = key_capacity;
+  }
+  return true;
+}
+
+CamParams make_cam(const ocgs_camera& c) {
+  CamParams p;
+  for (int i = 0; i < 12; ++i) p.V[i] = c.view[i];
+  p.fx = c.fx; p.fy = c.fy;
+  p.ox = c.cx - 0.5f; p.oy = c.cy - 0.5f;
+  // camera position -R^T t (double, rounded once)
+  for (int k = 0; k < 3; ++k)
+    p.campos[k] = (float)(-((double)c.view[k] * c.view[3] + (double)c.view[4 + k] * c.view[7] + (double)c.view[8 + k] * c.view[11]));
+  p.W = c.width; p.H = c.height;
+  p.tiles_x = (c.width + kTile - 1) / kTile;
+  p.tiles_y = (c.height + kTile - 1) / kTile;
+  return p;
+}
+
+static int check_cfg(const ocgs_config* cfg) {
+  if (!cfg) return OCGS_ERR_INVALID_ARG;
+  if (cfg->tile != kTile || cfg->sh_degree < 0 || cfg->sh_degree > 3) return OCGS_ERR_UNSUPPORTED;
+  if (!(cfg->filter_sigma2 > 0.f) || !(cfg->alpha_min > 0.f)) return OCGS_ERR_INVALID_ARG;
+  return OCGS_OK;
+}
+
+}  // namespace ocgs
+
+using namespace ocgs;
+
+extern "C" {
+
+void ocgs_default_config(ocgs_config* c) {
+  c->tile = 16; c->near_z = 0.2f; c->alpha_min = (float)(1.0 / 255.0); c->alpha_max = 0.99f; c->t_min = 1e-4f;
+  c->rho_max = 9.0f; c->filter_sigma2 = 0.5f; c->bg[0] = c->bg[1] = c->bg[2] = 0.f; c->gamma_bg = 0.5f;
+  c->tau_contrib = 0.f; c->min_opacity = 0.f; c->sh_degree = 3;
+}
+
+int ocgs_workspace_layout(int n, int width, int height, size_t key_capacity, ocgs_ws_layout* out) {
+  if (!out) return OCGS_ERR_INVALID_ARG;
+  return carve_workspace(nullptr, n, width, height, key_capacity, nullptr, out) ? OCGS_OK : OCGS_ERR_UNSUPPORTED;
+}
+
+size_t ocgs_workspace_bytes(int n, int width, int height, size_t key_capacity) {
+  ocgs_ws_layout L;
+  return carve_workspace(nullptr, n, width, height, key_capacity, nullptr, &L) ? L.total_bytes : 0;
+}
+
+int ocgs_last_cuda_error(void) { return g_last_cuda_error; }
+
+int ocgs_check(const void* ws, void* stream, ocgs_header* header_out) {
+  if (!ws) return OCGS_ERR_INVALID_ARG;
+  ocgs_header h;
+  OCGS_CUDA_OK(cudaMemcpyAsync(&h, ws, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  OCGS_CUDA_OK(cudaStreamSynchronize((cudaStream_t)stream));
+  if (header_out) *header_out = h;
+  return (h.error & 1u) ? OCGS_ERR_CAPACITY : OCGS_OK;
+}
+
+int ocgs_preprocess(const ocgs_surfels* s, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, void* stream) {
+  if (!s || !cam || !ws) return OCGS_ERR_INVALID_ARG;
+  int rc = check_cfg(cfg);
+  if (rc != OCGS_OK) return rc;
+  if (s->n > 0 && (!s->pos || !s->scale || !s->quat || !s->opacity || !s->sh)) return OCGS_ERR_INVALID_ARG;
+  Workspace w;
+  if (!carve_workspace(ws, s->n, cam->width, cam->height, key_capacity, &w, nullptr)) return OCGS_ERR_UNSUPPORTED;
+  return launch_preprocess(*s, make_cam(*cam), *cfg, w, (cudaStream_t)stream);
+}
+
+int ocgs_bin_sort(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, uint32_t* sorted_ids, void* stream) {
+  if (!cam || !ws) return OCGS_ERR_INVALID_ARG;
+  int rc = check_cfg(cfg);
+  if (rc != OCGS_OK) return rc;
+  Workspace w;
+  if (!carve_workspace(ws, n, cam->width, cam->height, key_capacity, &w, nullptr)) return OCGS_ERR_UNSUPPORTED;
+  return launch_bin_sort(make_cam(*cam), w, sorted_ids, (cudaStream_t)stream);
+}
+
+static int carve_for_render(void* ws, int n, const ocgs_camera* cam, size_t key_capacity, Workspace* w) {
+  return carve_workspace(ws, n, cam->width, cam->height, key_capacity, w, nullptr) ? OCGS_OK : OCGS_ERR_UNSUPPORTED;
+}
+
+int ocgs_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
+                        float* color, float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg,
+                        uint32_t* vis_count, float* contrib_sum, void* stream) {
+  if (!cam || !ws || !color || !alpha || !depth || !normal || !n_contrib) return OCGS_ERR_INVALID_ARG;
+  int rc = check_cfg(cfg);
+  if (rc != OCGS_OK) return rc;
+  if ((vis_count == nullptr) != (contrib_sum == nullptr)) return OCGS_ERR_INVALID_ARG;
+  Workspace w;
+  if ((rc = carve_for_render(ws, n, cam, key_capacity, &w)) != OCGS_OK) return rc;
+  return launch_render_fwd(make_cam(*cam), *cfg, w, mask, color, alpha, depth, normal, n_contrib, loss_bg, vis_count, contrib_sum,
+                           (cudaStream_t)stream);
+}
+
+int ocgs_render_bwd(const ocgs_surfels* s, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
+                        const uint8_t* mask, const uint32_t* n_contrib, const float* gC, const float* gA, const float* gD,
+                        const float* gN, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
+                        float* d_center2d, void* stream) {
+  if (!s || !cam || !ws || !n_contrib) return OCGS_ERR_INVALID_ARG;
+  int rc = check_cfg(cfg);
+  if (rc != OCGS_OK) return rc;
+  if (s->n > 0 && (!d_pos || !d_scale || !d_quat || !d_opacity || !d_sh)) return OCGS_ERR_INVALID_ARG;
+  Workspace w;
+  if ((rc = carve_for_render(ws, s->n, cam, key_capacity, &w)) != OCGS_OK) return rc;
+  return launch_render_bwd(*s, make_cam(*cam), *cfg, w, mask, w.final_T, n_contrib, gC, gA, gD, gN, d_pos, d_scale, d_quat, d_opacity,
+                           d_sh, d_center2d, (cudaStream_t)stream);
+}
+
+size_t ocgs_prune_workspace_bytes(int n) { return (div_up((size_t)(n > 0 ? n : 0), 1024) + 2) * sizeof(uint32_t); }
+
+int ocgs_prune_stats(const ocgs_surfels* in, uint32_t* vis_count, float* contrib_sum, const ocgs_config* cfg, uint8_t* prune_mask,
+                     int32_t* remap, const ocgs_surfels_mut* out, int* n_out, int reset_stats, void* ws, void* stream) {
+  if (!in || !vis_count || !contrib_sum || !cfg || !prune_mask || !remap || !n_out || !ws) return OCGS_ERR_INVALID_ARG;
+  if (out && out->capacity < in->n) return OCGS_ERR_CAPACITY;
+  return launch_prune(*in, vis_count, contrib_sum, *cfg, prune_mask, remap, out, n_out, reset_stats, ws, (cudaStream_t)stream);
+}
+
+int ocgs_step_host(const float* h_pos, const float* h_scale, const float* h_quat, const float* h_opacity, const float* h_sh, int n,
+                   const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask, const float* h_dL_dcolor, float* h_grads,
+                   float* h_alpha, float* h_loss_bg, float* d_params, uint8_t* d_mask, float* d_images, uint32_t* d_ncontrib,
+                   float* d_grads, uint32_t* d_vis_count, float* d_contrib_sum, float* d_loss_bg, void* ws, size_t key_capacity,
+                   void* stream) {
+  if (!cam || !cfg || !ws || !d_params || !d_mask || !d_images || !d_ncontrib || !d_grads || !d_loss_bg) return OCGS_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t N = (size_t)n, HW = (size_t)cam->width * cam->height;
+  float* p_pos = d_params;               // 3N
+  float* p_scale = p_pos + 3 * N;         // 2N   (3N*4 bytes is 8-aligned only when N is even: keep sections 16-B aligned)
+  // section starts rounded up to 4 floats so float2/float4 loads stay aligned
+  auto up4 = [](size_t x) { return (x + 3) & ~(size_t)3; };
+  p_scale = d_params + up4(3 * N);
+  float* p_quat = p_scale + up4(2 * N);
+  float* p_opa = p_quat + 4 * N;
+  float* p_sh = p_opa + up4(N);
+  OCGS_CUDA_OK(cudaMemcpyAsync(p_pos, h_pos, 3 * N * 4, cudaMemcpyHostToDevice, st));
+  OCGS_CUDA_OK(cudaMemcpyAsync(p_scale, h_scale, 2 * N * 4, cudaMemcpyHostToDevice, st));
+  OCGS_CUDA_OK(cudaMemcpyAsync(p_quat, h_quat, 4 * N * 4, cudaMemcpyHostToDevice, st));
+  OCGS_CUDA_OK(cudaMemcpyAsync(p_opa, h_opacity, N * 4, cudaMemcpyHostToDevice, st));
+  OCGS_CUDA_OK(cudaMemcpyAsync(p_sh, h_sh, 48 * N * 4, cudaMemcpyHostToDevice, st));
+  OCGS_CUDA_OK(cudaMemcpyAsync(d_mask, h_mask, HW, cudaMemcpyHostToDevice, st));
+  float* color = d_images; float* alpha = color + 3 * HW; float* depth = alpha + HW; float* normal = depth + HW;
+  float* gC = normal + 3 * HW;
+  OCGS_CUDA_OK(cudaMemcpyAsync(gC, h_dL_dcolor, 3 * HW * 4, cudaMemcpyHostToDevice, st));
+  ocgs_surfels s = {p_pos, p_scale, p_quat, p_opa, p_sh, n};
+  int rc;
+  if ((rc = ocgs_preprocess(&s, cam, cfg, ws, key_capacity, stream)) != OCGS_OK) return rc;
+  if ((rc = ocgs_bin_sort(n, cam, cfg, ws, key_capacity, nullptr, stream)) != OCGS_OK) return rc;
+  if ((rc = ocgs_render_fwd(n, cam, cfg, ws, key_capacity, d_mask, color, alpha, depth, normal, d_ncontrib, d_loss_bg, d_vis_count,
+                            d_contrib_sum, stream)) != OCGS_OK) return rc;
+  float* g_pos = d_grads; float* g_scale = d_grads + up4(3 * N); float* g_quat = g_scale + up4(2 * N); float* g_opa = g_quat + 4 * N;
+  float* g_sh = g_opa + up4(N);
+  if ((rc = ocgs_render_bwd(&s, cam, cfg, ws, key_capacity, d_mask, d_ncontrib, gC, nullptr, nullptr, nullptr, g_pos, g_scale, g_quat,
+                            g_opa, g_sh, nullptr, stream)) != OCGS_OK) return rc;
+  OCGS_CUDA_OK(cudaMemcpyAsync(h_grads, g_pos, 3 * N * 4, cudaMemcpyDeviceToHost, st));
+  OCGS_CUDA_OK(cudaMemcpyAsync(h_grads + 3 * N, g_scale, 2 * N * 4, cudaMemcpyDeviceToHost, st));
+  OCGS_CUDA_OK(cudaMemcpyAsync(h_grads + 5 * N, g_quat, 4 * N * 4, cudaMemcpyDeviceToHost, st));
+  OCGS_CUDA_OK(cudaMemcpyAsync(h_grads + 9 * N, g_opa, N * 4, cudaMemcpyDeviceToHost, st));
+  OCGS_CUDA_OK(cudaMemcpyAsync(h_grads + 10 * N, g_sh, 48 * N * 4, cudaMemcpyDeviceToHost, st));
+  if (h_alpha) OCGS_CUDA_OK(cudaMemcpyAsync(h_alpha, alpha, HW * 4, cudaMemcpyDeviceToHost, st));
+  if (h_loss_bg) OCGS_CUDA_OK(cudaMemcpyAsync(h_loss_bg, d_loss_bg, 4, cudaMemcpyDeviceToHost, st));
+  return ocgs_check(ws, stream, nullptr);
+}
+
+}  // extern "C"

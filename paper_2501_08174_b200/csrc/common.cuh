@@ -1,0 +1,100 @@
+// common.cuh -- shared declarations of libocgs (sm_100a). Internal; the public boundary is include/ocgs.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/ocgs.h"
+
+namespace ocgs {
+
+constexpr int kTile = 16;
+constexpr int kRec = 20;  // floats per raster record (80 B = 5 x float4)
+// record layout: the homography M in a form centred on the projected centre c = c2d
+//   k = (x-cx)*M2 - A0,  l = (y-cy)*M2 - A1   with A0 = M0 - cx*M2, A1 = M1 - cy*M2 (third components are the exact
+//   division residuals r0, r1), so forming k, l has no large-number cancellation.
+enum RecField {
+  R_M20 = 0, R_M21, R_M22, R_A00, R_A01, R_A10, R_A11, R_R0, R_R1, R_CX, R_CY, R_RHOCUT, R_OPA, R_COLR, R_COLG, R_COLB,
+  R_NX, R_NY, R_NZ, R_PAD
+};
+// gradient accumulator layout in ws.grad_rec (by rank), 18 used
+enum GradField {
+  G_M20 = 0, G_M21, G_M22,   // sum (x-cx) gk + (y-cy) gl + (u,v,1) gz
+  G_K0, G_K1, G_K2,          // sum gk   (dL/dM0 = -gk)
+  G_L0, G_L1, G_L2,          // sum gl   (dL/dM1 = -gl)
+  G_CX, G_CY,                // filter term: dL/dc2d
+  G_OPA, G_COLR, G_COLG, G_COLB, G_NX, G_NY, G_NZ, G_PAD0, G_PAD1
+};
+
+constexpr int kSortItems = 16;                       // keys per thread in a radix pass
+constexpr int kSortThreads = 256;
+constexpr int kSortTile = kSortItems * kSortThreads;  // 4096 keys per block
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+
+struct Workspace {
+  ocgs_header* header;
+  uint32_t* depth_bits;
+  ushort4* rect;
+  uint32_t* tiles;
+  uint8_t* clamp;
+  float* rec_id;
+  uint32_t* id_to_rank;
+  uint32_t* rank_to_id;
+  float* rec;
+  uint32_t* offsets;
+  uint32_t* tile_keys;
+  uint32_t* tile_vals;
+  uint32_t* ranges;
+  float* grad_rec;
+  float* loss_partial;
+  float* final_T;
+  // scratch
+  uint32_t* dkeyA; uint32_t* dkeyB; uint32_t* dvalB;  // depth sort ping-pong (dvalA == rank_to_id)
+  uint32_t* tkeyB; uint32_t* tvalB;                   // tile sort ping-pong
+  uint32_t* hist;                                     // [kRadix * max_blocks] digit-major block histograms
+  uint32_t* digit_total;                              // [kRadix]
+  uint32_t* tcount;                                   // [N] tiles touched by rank
+  uint32_t* blocksum;                                 // [ceil(N/1024)+1]
+  int n, width, height, tiles_x, tiles_y, n_tiles;
+  size_t key_capacity;
+};
+
+// host: carve `ws` into sections. Returns false when the sizes are unsupported.
+bool carve_workspace(void* ws, int n, int width, int height, size_t key_capacity, Workspace* out, ocgs_ws_layout* layout);
+
+extern thread_local int g_last_cuda_error;
+inline int cuda_fail(cudaError_t e) { g_last_cuda_error = (int)e; return OCGS_ERR_CUDA; }
+#define OCGS_CUDA_OK(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) return ::ocgs::cuda_fail(_e); } while (0)
+#define OCGS_LAUNCH_OK() do { cudaError_t _e = cudaGetLastError(); if (_e != cudaSuccess) return ::ocgs::cuda_fail(_e); } while (0)
+
+struct CamParams {
+  float V[12];  // rows 0..2 of the view matrix
+  float fx, fy, ox, oy;  // ox = cx - 1/2, oy = cy - 1/2 (Appendix A step 4)
+  float campos[3];
+  int W, H, tiles_x, tiles_y;
+};
+CamParams make_cam(const ocgs_camera& c);
+
+// stage launchers (each returns an OCGS_* code)
+int launch_preprocess(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, cudaStream_t st);
+int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cudaStream_t st);
+int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Workspace& w, const uint8_t* mask, float* color,
+                      float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,
+                      float* contrib_sum, cudaStream_t st);
+int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, const uint8_t* mask,
+                      const float* final_T, const uint32_t* n_contrib, const float* gC, const float* gA, const float* gD,
+                      const float* gN, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
+                      float* d_center2d, cudaStream_t st);
+
+int launch_prune(const ocgs_surfels& in, uint32_t* vis_count, float* contrib_sum, const ocgs_config& cfg, uint8_t* prune_mask,
+                 int32_t* remap, const ocgs_surfels_mut* out, int* n_out, int reset_stats, void* ws, cudaStream_t st);
+
+// stable LSD radix sort of (u32 key, u32 value) pairs on bits [0, key_bits); count is read from the device (*n_ptr, u64 or
+// u32 selected by n_is_u64) and bounded by n_max for grid sizing. Result lands in (keysA, valsA) when the number of
+// passes is even, else in (keysB, valsB); returns that through *result_in_B.
+int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t* valsB, const void* n_ptr, bool n_is_u64,
+                     size_t n_max, int key_bits, uint32_t* hist, uint32_t* digit_total, bool* result_in_B, cudaStream_t st);
+
+__host__ __device__ inline size_t div_up(size_t a, size_t b) { return (a + b - 1) / b; }
+
+}  // namespace ocgs

@@ -1,0 +1,97 @@
+// preprocess.cu -- ocgs_preprocess (O1): one thread per surfel.  HBM-bound: 40 B read per surfel, +192 B SH and ~116 B
+// written per visible surfel.
+#include "projection.cuh"
+
+namespace ocgs {
+
+__global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict__ pos, const float2* __restrict__ scale,
+                                                         const float4* __restrict__ quat, const float* __restrict__ opacity,
+                                                         const float4* __restrict__ sh, int n, CamParams cam, ocgs_config cfg,
+                                                         uint32_t* __restrict__ depth_bits, ushort4* __restrict__ rect,
+                                                         uint32_t* __restrict__ tiles, uint8_t* __restrict__ clamp_bits,
+                                                         float4* __restrict__ rec_id, uint32_t* __restrict__ id_to_rank,
+                                                         uint32_t* __restrict__ sort_key, uint32_t* __restrict__ sort_val,
+                                                         ocgs_header* __restrict__ header) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  bool vis = false;
+  if (j < n) {
+    const float p[3] = {pos[3 * j], pos[3 * j + 1], pos[3 * j + 2]};
+    const float2 s = scale[j];
+    const float4 q = quat[j];
+    const float o = opacity[j];
+    Projected pr;
+    project_surfel(p, s.x, s.y, q, o, cam, cfg, pr);
+    vis = pr.visible;
+    const uint32_t zb = __float_as_uint(pr.pc[2]);
+    depth_bits[j] = zb;
+    sort_key[j] = vis ? zb : 0xFFFFFFFFu;  // culled surfels sort behind every positive depth
+    sort_val[j] = (uint32_t)j;
+    id_to_rank[j] = 0xFFFFFFFFu;
+    uint32_t nt = 0;
+    uint8_t cl = 0;
+    if (vis) {
+      const int tx0 = pr.ix0 >> 4, tx1 = (pr.ix1 >> 4) + 1, ty0 = pr.iy0 >> 4, ty1 = (pr.iy1 >> 4) + 1;
+      nt = (uint32_t)((tx1 - tx0) * (ty1 - ty0));
+      rect[j] = make_ushort4((unsigned short)pr.ix0, (unsigned short)pr.iy0, (unsigned short)pr.ix1, (unsigned short)pr.iy1);
+      // facing normal (view space): n = R_wc t_w, flipped when n . p_c > 0
+      const float w = q.x, x = q.y, y = q.z, z = q.w;
+      const float tw0 = 2.0f * (x * z + w * y), tw1 = 2.0f * (y * z - w * x), tw2 = 1.0f - 2.0f * (x * x + y * y);
+      float nx = cam.V[0] * tw0 + cam.V[1] * tw1 + cam.V[2] * tw2;
+      float ny = cam.V[4] * tw0 + cam.V[5] * tw1 + cam.V[6] * tw2;
+      float nz = cam.V[8] * tw0 + cam.V[9] * tw1 + cam.V[10] * tw2;
+      if (nx * pr.pc[0] + ny * pr.pc[1] + nz * pr.pc[2] > 0.0f) { nx = -nx; ny = -ny; nz = -nz; }
+      // SH colour (S14)
+      float dx = p[0] - cam.campos[0], dy = p[1] - cam.campos[1], dz = p[2] - cam.campos[2];
+      const float inv = rsqrtf(dx * dx + dy * dy + dz * dz);
+      dx *= inv; dy *= inv; dz *= inv;
+      float Y[16];
+      sh_basis(dx, dy, dz, cfg.sh_degree, Y);
+      const int nb = (cfg.sh_degree + 1) * (cfg.sh_degree + 1);
+      float col[3] = {0.5f, 0.5f, 0.5f};
+      const float4* shj = sh + (size_t)j * 12;
+      const int nvec = (3 * nb + 3) / 4;
+      for (int v4 = 0; v4 < nvec; ++v4) {
+        const float4 f = __ldg(shj + v4);
+        const float ff[4] = {f.x, f.y, f.z, f.w};
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const int idx = 4 * v4 + e;
+          if (idx < 3 * nb) {
+            const int k = idx / 3, c = idx - 3 * k;
+            col[c] = fmaf(Y[k], ff[e], col[c]);
+          }
+        }
+      }
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+        if (col[c] < 0.0f) { col[c] = 0.0f; cl |= (uint8_t)(1u << c); }
+      // centred record
+      const float* M = pr.M;
+      const float A00 = __fmaf_rn(-pr.cx, M[6], M[0]), A01 = __fmaf_rn(-pr.cx, M[7], M[1]), r0 = __fmaf_rn(-pr.cx, M[8], M[2]);
+      const float A10 = __fmaf_rn(-pr.cy, M[6], M[3]), A11 = __fmaf_rn(-pr.cy, M[7], M[4]), r1 = __fmaf_rn(-pr.cy, M[8], M[5]);
+      float4* out = rec_id + (size_t)j * 5;
+      out[0] = make_float4(M[6], M[7], M[8], A00);
+      out[1] = make_float4(A01, A10, A11, r0);
+      out[2] = make_float4(r1, pr.cx, pr.cy, pr.rho_cut);
+      out[3] = make_float4(o, col[0], col[1], col[2]);
+      out[4] = make_float4(nx, ny, nz, 0.0f);
+    }
+    tiles[j] = nt;
+    clamp_bits[j] = cl;
+  }
+  const unsigned ball = __ballot_sync(0xFFFFFFFFu, vis);
+  if ((threadIdx.x & 31) == 0 && ball) atomicAdd(&header->n_vis, (unsigned)__popc(ball));
+}
+
+int launch_preprocess(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, cudaStream_t st) {
+  OCGS_CUDA_OK(cudaMemsetAsync(w.header, 0, sizeof(ocgs_header), st));
+  if (s.n == 0) return OCGS_OK;
+  const int blocks = (int)div_up((size_t)s.n, 256);
+  preprocess_kernel<<<blocks, 256, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity, (const float4*)s.sh,
+                                            s.n, cam, cfg, w.depth_bits, w.rect, w.tiles, w.clamp, (float4*)w.rec_id,
+                                            w.id_to_rank, w.dkeyA, w.rank_to_id, w.header);
+  OCGS_LAUNCH_OK();
+  return OCGS_OK;
+}
+
+}  // namespace ocgs

@@ -1,0 +1,325 @@
+// raster_bwd.cu -- ocgs_render_bwd (O7).
+//  (a) render_bwd_kernel: one CTA per tile, one thread per pixel, the tile list walked BACK to FRONT over
+//      [0, max n_contrib); per pair the chain rule through compositing and the ray-splat intersection gives 18 record
+//      gradients, reduced across the warp by a transposing butterfly (16 values, 16+8+4+2+1 shuffles) then combined
+//      across the CTA in shared memory and flushed with one global RED per (tile, entry, field).
+//  (b) project_bwd_kernel: one thread per surfel, record gradients -> (pos, scale, quat, opacity, sh) gradients.
+#include "projection.cuh"
+
+namespace ocgs {
+
+constexpr int kBwdBatch = 64;
+constexpr int kNG = 18;
+
+// sum of v[0..15] over the 32 lanes; afterwards v[0] of lane L holds the total of value index
+// 8*bit4(L) + 4*bit3(L) + 2*bit2(L) + bit1(L)
+__device__ __forceinline__ void warp_transpose_reduce16(float* v, int lane) {
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const bool up = lane & 16;
+    const float send = up ? v[i] : v[i + 8], keep = up ? v[i + 8] : v[i];
+    v[i] = keep + __shfl_xor_sync(0xFFFFFFFFu, send, 16);
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const bool up = lane & 8;
+    const float send = up ? v[i] : v[i + 4], keep = up ? v[i + 4] : v[i];
+    v[i] = keep + __shfl_xor_sync(0xFFFFFFFFu, send, 8);
+  }
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    const bool up = lane & 4;
+    const float send = up ? v[i] : v[i + 2], keep = up ? v[i + 2] : v[i];
+    v[i] = keep + __shfl_xor_sync(0xFFFFFFFFu, send, 4);
+  }
+  {
+    const bool up = lane & 2;
+    const float send = up ? v[0] : v[1], keep = up ? v[1] : v[0];
+    v[0] = keep + __shfl_xor_sync(0xFFFFFFFFu, send, 2);
+  }
+  v[0] += __shfl_xor_sync(0xFFFFFFFFu, v[0], 1);
+}
+
+// order of the 16 transposed values -> GradField
+__constant__ int kFieldOf16[16] = {G_M20, G_M21, G_M22, G_K0, G_K1, G_K2, G_L0, G_L1, G_L2, G_OPA, G_COLR, G_COLG, G_COLB, G_NX, G_NY, G_NZ};
+
+__global__ void __launch_bounds__(256) render_bwd_kernel(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
+                                                         const float4* __restrict__ rec, const uint8_t* __restrict__ mask,
+                                                         const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
+                                                         const float* __restrict__ gC, const float* __restrict__ gA,
+                                                         const float* __restrict__ gD, const float* __restrict__ gN, int W, int H,
+                                                         int tiles_x, ocgs_config cfg, float gamma_over_hw, float* __restrict__ grad_rec) {
+  __shared__ float4 s_rec[kBwdBatch * 5];
+  __shared__ uint32_t s_rank[kBwdBatch];
+  __shared__ float s_acc[kBwdBatch * kNG];
+  __shared__ uint32_t s_max[8];
+
+  const int tile = blockIdx.x;
+  const int tx = tile % tiles_x, ty = tile / tiles_x;
+  const int lx = threadIdx.x & 15, ly = threadIdx.x >> 4;
+  const int ix = tx * kTile + lx, iy = ty * kTile + ly;
+  const bool inside = ix < W && iy < H;
+  const float px = (float)ix, py = (float)iy;
+  const uint32_t start = ranges[2 * tile];
+  const float inv_sigma2 = 1.0f / cfg.filter_sigma2;
+  const int lane = threadIdx.x & 31;
+  const size_t HW = (size_t)W * H, p = inside ? (size_t)iy * W + ix : 0;
+
+  uint32_t last = 0;
+  float Tfin = 1.0f, gc0 = 0.f, gc1 = 0.f, gc2 = 0.f, ga = 0.f, gd = 0.f, gn0 = 0.f, gn1 = 0.f, gn2 = 0.f;
+  if (inside) {
+    last = n_contrib[p];
+    Tfin = final_T[p];
+    if (gC) { gc0 = gC[p]; gc1 = gC[HW + p]; gc2 = gC[2 * HW + p]; }
+    if (gA) ga = gA[p];
+    if (gD) gd = gD[p];
+    if (gN) { gn0 = gN[p]; gn1 = gN[HW + p]; gn2 = gN[2 * HW + p]; }
+    if (mask && mask[p] == 0) ga += gamma_over_hw;  // d(gamma L_b)/dA = gamma (1-M)/(HW), Eq. 1 / Eq. 3
+  }
+  // block max of n_contrib
+  uint32_t mx = last;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
+  if (lane == 0) s_max[threadIdx.x >> 5] = mx;
+  __syncthreads();
+  mx = 0;
+#pragma unroll
+  for (int w2 = 0; w2 < 8; ++w2) mx = max(mx, s_max[w2]);
+  if (mx == 0) return;
+
+  float T = Tfin;
+  float SC0 = Tfin * cfg.bg[0], SC1 = Tfin * cfg.bg[1], SC2 = Tfin * cfg.bg[2], SD = 0.f, SN0 = 0.f, SN1 = 0.f, SN2 = 0.f;
+
+  const int nbatch = (int)((mx + kBwdBatch - 1) / kBwdBatch);
+  for (int bi = nbatch - 1; bi >= 0; --bi) {
+    const uint32_t b0 = (uint32_t)bi * kBwdBatch;
+    const int cnt = (int)min((uint32_t)kBwdBatch, mx - b0);
+    __syncthreads();  // previous batch fully flushed before s_rank / s_acc are reused
+    if ((int)threadIdx.x < cnt) s_rank[threadIdx.x] = list[start + b0 + threadIdx.x];
+    for (int i = threadIdx.x; i < cnt * kNG; i += 256) s_acc[i] = 0.f;
+    __syncthreads();
+    for (int i = threadIdx.x; i < cnt * 5; i += 256) {
+      const int e = i / 5, part = i - 5 * e;
+      s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 5 + part);
+    }
+    __syncthreads();
+    for (int j = cnt - 1; j >= 0; --j) {
+      const uint32_t idx = b0 + (uint32_t)j;
+      const bool act = inside && idx < last;
+      if (!__any_sync(0xFFFFFFFFu, act)) continue;
+      const float4 r0 = s_rec[5 * j], r1 = s_rec[5 * j + 1], r2 = s_rec[5 * j + 2];
+      float v[16];
+#pragma unroll
+      for (int i = 0; i < 16; ++i) v[i] = 0.f;
+      float gcx = 0.f, gcy = 0.f;
+      bool contributes = false;
+      if (act) {
+        const float dx = px - r2.y, dy = py - r2.z;
+        const float k0 = fmaf(dx, r0.x, -r0.w), k1 = fmaf(dx, r0.y, -r1.x), k2 = fmaf(dx, r0.z, -r1.w);
+        const float l0 = fmaf(dy, r0.x, -r1.y), l1 = fmaf(dy, r0.y, -r1.z), l2 = fmaf(dy, r0.z, -r2.x);
+        const float qx = fmaf(k1, l2, -k2 * l1), qy = fmaf(k2, l0, -k0 * l2), qz = fmaf(k0, l1, -k1 * l0);
+        if (qz != 0.0f) {
+          const float inv = __frcp_rn(qz);
+          const float u = qx * inv, vv = qy * inv;
+          const float rho3 = fmaf(u, u, vv * vv);
+          const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
+          const bool surf = rho3 <= rho2;
+          const float rho = surf ? rho3 : rho2;
+          const float z = surf ? fmaf(r0.x, u, fmaf(r0.y, vv, r0.z)) : r0.z;
+          if (!(z < cfg.near_z) && !(rho > r2.w)) {
+            contributes = true;
+            const float4 r3 = s_rec[5 * j + 3], r4 = s_rec[5 * j + 4];
+            const float G = __expf(-0.5f * rho);
+            const float araw = r3.x * G;
+            const bool capped = araw > cfg.alpha_max;
+            const float a = capped ? cfg.alpha_max : araw;
+            const float inv1ma = __frcp_rn(1.0f - a);
+            T *= inv1ma;  // T_i = T_{i+1} / (1 - alpha_i)
+            const float w = a * T;
+            float galpha = ga * Tfin * inv1ma + gd * (z * T - SD * inv1ma);
+            galpha += gc0 * (r3.y * T - SC0 * inv1ma) + gc1 * (r3.z * T - SC1 * inv1ma) + gc2 * (r3.w * T - SC2 * inv1ma);
+            galpha += gn0 * (r4.x * T - SN0 * inv1ma) + gn1 * (r4.y * T - SN1 * inv1ma) + gn2 * (r4.z * T - SN2 * inv1ma);
+            SC0 = fmaf(w, r3.y, SC0); SC1 = fmaf(w, r3.z, SC1); SC2 = fmaf(w, r3.w, SC2);
+            SD = fmaf(w, z, SD);
+            SN0 = fmaf(w, r4.x, SN0); SN1 = fmaf(w, r4.y, SN1); SN2 = fmaf(w, r4.z, SN2);
+            v[10] = w * gc0; v[11] = w * gc1; v[12] = w * gc2;
+            v[13] = w * gn0; v[14] = w * gn1; v[15] = w * gn2;
+            const float gz = w * gd;
+            float grho = 0.f;
+            if (!capped) { v[9] = G * galpha; grho = -0.5f * G * r3.x * galpha; }  // S12: zero through the cap
+            if (surf) {
+              const float gu = fmaf(2.0f * u, grho, r0.x * gz), gv = fmaf(2.0f * vv, grho, r0.y * gz);
+              const float gq0 = gu * inv, gq1 = gv * inv, gq2 = -(gu * u + gv * vv) * inv;
+              // q = k x l: gk = l x gq, gl = gq x k
+              const float gk0 = l1 * gq2 - l2 * gq1, gk1 = l2 * gq0 - l0 * gq2, gk2 = l0 * gq1 - l1 * gq0;
+              const float gl0 = gq1 * k2 - gq2 * k1, gl1 = gq2 * k0 - gq0 * k2, gl2 = gq0 * k1 - gq1 * k0;
+              v[0] = fmaf(dx, gk0, fmaf(dy, gl0, u * gz));
+              v[1] = fmaf(dx, gk1, fmaf(dy, gl1, vv * gz));
+              v[2] = fmaf(dx, gk2, fmaf(dy, gl2, gz));
+              v[3] = gk0; v[4] = gk1; v[5] = gk2;
+              v[6] = gl0; v[7] = gl1; v[8] = gl2;
+            } else {
+              gcx = -2.0f * dx * inv_sigma2 * grho;
+              gcy = -2.0f * dy * inv_sigma2 * grho;
+              v[2] = gz;  // z = z_j = M22
+            }
+          }
+        }
+      }
+      if (!__any_sync(0xFFFFFFFFu, contributes)) continue;
+      warp_transpose_reduce16(v, lane);
+      if ((lane & 1) == 0) atomicAdd(&s_acc[j * kNG + kFieldOf16[lane >> 1]], v[0]);
+      if (__any_sync(0xFFFFFFFFu, gcx != 0.f || gcy != 0.f)) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          gcx += __shfl_xor_sync(0xFFFFFFFFu, gcx, o);
+          gcy += __shfl_xor_sync(0xFFFFFFFFu, gcy, o);
+        }
+        if (lane == 0) { atomicAdd(&s_acc[j * kNG + G_CX], gcx); atomicAdd(&s_acc[j * kNG + G_CY], gcy); }
+      }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < cnt * kNG; i += 256) {
+      const float val = s_acc[i];
+      if (val != 0.f) {
+        const int e = i / kNG, f = i - kNG * e;
+        atomicAdd(grad_rec + (size_t)s_rank[e] * kRec + f, val);
+      }
+    }
+  }
+}
+
+// ---- per-surfel: record gradients -> parameter gradients -------------------------------------------------------
+__global__ void __launch_bounds__(128) project_bwd_kernel(const float* __restrict__ pos, const float2* __restrict__ scale,
+                                                          const float4* __restrict__ quat, const float* __restrict__ opacity,
+                                                          const float4* __restrict__ sh, int n, CamParams cam, ocgs_config cfg,
+                                                          const uint32_t* __restrict__ id_to_rank, const uint8_t* __restrict__ clamp_bits,
+                                                          const float* __restrict__ grad_rec, float* __restrict__ d_pos,
+                                                          float2* __restrict__ d_scale, float4* __restrict__ d_quat,
+                                                          float* __restrict__ d_opacity, float4* __restrict__ d_sh,
+                                                          float2* __restrict__ d_center2d) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n) return;
+  const uint32_t rank = id_to_rank[j];
+  float4* dsh = d_sh + (size_t)j * 12;
+  if (rank == 0xFFFFFFFFu) {
+    d_pos[3 * j] = 0.f; d_pos[3 * j + 1] = 0.f; d_pos[3 * j + 2] = 0.f;
+    d_scale[j] = make_float2(0.f, 0.f);
+    d_quat[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+    d_opacity[j] = 0.f;
+    if (d_center2d) d_center2d[j] = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int i = 0; i < 12; ++i) dsh[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    return;
+  }
+  float g[kRec];
+  const float4* gr = (const float4*)(grad_rec + (size_t)rank * kRec);
+#pragma unroll
+  for (int i = 0; i < 5; ++i) {
+    const float4 t = gr[i];
+    g[4 * i] = t.x; g[4 * i + 1] = t.y; g[4 * i + 2] = t.z; g[4 * i + 3] = t.w;
+  }
+  const float p[3] = {pos[3 * j], pos[3 * j + 1], pos[3 * j + 2]};
+  const float2 s = scale[j];
+  const float4 q = quat[j];
+  Projected pr;
+  project_surfel(p, s.x, s.y, q, opacity[j], cam, cfg, pr);
+  const float M22 = pr.M[8];
+  const float ex = pr.cx - cam.ox, ey = pr.cy - cam.oy;
+  const float f0 = g[G_CX] / M22, f1 = g[G_CY] / M22;
+  const float m0[3] = {-g[G_K0], -g[G_K1], -g[G_K2] + f0};  // dL/dM0
+  const float m1[3] = {-g[G_L0], -g[G_L1], -g[G_L2] + f1};  // dL/dM1
+  float gcol[3][3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    gcol[i][0] = cam.fx * m0[i];
+    gcol[i][1] = cam.fy * m1[i];
+    gcol[i][2] = g[G_M20 + i] - ex * m0[i] - ey * m1[i];  // = ox m0 + oy m1 + dL/dM2 with dL/dM2 = G2 + cx Gk + cy Gl - ...
+  }
+  if (d_center2d) d_center2d[j] = make_float2(M22 * m0[2], M22 * m1[2]);
+  const float* V = cam.V;
+  d_scale[j] = make_float2(gcol[0][0] * pr.vu[0] + gcol[0][1] * pr.vu[1] + gcol[0][2] * pr.vu[2],
+                           gcol[1][0] * pr.vv[0] + gcol[1][1] * pr.vv[1] + gcol[1][2] * pr.vv[2]);
+  float gtu[3], gtv[3], gtw[3], gp[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {  // R_wc^T g
+    gtu[k] = s.x * (V[k] * gcol[0][0] + V[4 + k] * gcol[0][1] + V[8 + k] * gcol[0][2]);
+    gtv[k] = s.y * (V[k] * gcol[1][0] + V[4 + k] * gcol[1][1] + V[8 + k] * gcol[1][2]);
+    gp[k] = V[k] * gcol[2][0] + V[4 + k] * gcol[2][1] + V[8 + k] * gcol[2][2];
+  }
+  const float w = q.x, x = q.y, y = q.z, z = q.w;
+  {
+    const float tw0 = 2.0f * (x * z + w * y), tw1 = 2.0f * (y * z - w * x), tw2 = 1.0f - 2.0f * (x * x + y * y);
+    const float nx = V[0] * tw0 + V[1] * tw1 + V[2] * tw2, ny = V[4] * tw0 + V[5] * tw1 + V[6] * tw2,
+                nz = V[8] * tw0 + V[9] * tw1 + V[10] * tw2;
+    const float sgn = (nx * pr.pc[0] + ny * pr.pc[1] + nz * pr.pc[2] > 0.0f) ? -1.0f : 1.0f;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) gtw[k] = sgn * (V[k] * g[G_NX] + V[4 + k] * g[G_NY] + V[8 + k] * g[G_NZ]);
+  }
+  d_quat[j] = make_float4(
+      2.0f * (z * gtu[1] - y * gtu[2] - z * gtv[0] + x * gtv[2] + y * gtw[0] - x * gtw[1]),
+      2.0f * (y * gtu[1] + z * gtu[2] + y * gtv[0] - 2.0f * x * gtv[1] + w * gtv[2] + z * gtw[0] - w * gtw[1] - 2.0f * x * gtw[2]),
+      2.0f * (-2.0f * y * gtu[0] + x * gtu[1] - w * gtu[2] + x * gtv[0] + z * gtv[2] + w * gtw[0] + z * gtw[1] - 2.0f * y * gtw[2]),
+      2.0f * (-2.0f * z * gtu[0] + w * gtu[1] + x * gtu[2] - w * gtv[0] - 2.0f * z * gtv[1] + y * gtv[2] + x * gtw[0] + y * gtw[1]));
+  d_opacity[j] = g[G_OPA];
+  // colour
+  float dx = p[0] - cam.campos[0], dy = p[1] - cam.campos[1], dz = p[2] - cam.campos[2];
+  const float inv = rsqrtf(dx * dx + dy * dy + dz * dz);
+  dx *= inv; dy *= inv; dz *= inv;
+  float Y[16];
+  sh_basis(dx, dy, dz, cfg.sh_degree, Y);
+  const int nb = (cfg.sh_degree + 1) * (cfg.sh_degree + 1);
+  const uint8_t cl = clamp_bits[j];
+  const float gcolr[3] = {(cl & 1) ? 0.f : g[G_COLR], (cl & 2) ? 0.f : g[G_COLG], (cl & 4) ? 0.f : g[G_COLB]};
+  float a[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) a[k] = 0.f;
+  const float4* shj = sh + (size_t)j * 12;
+#pragma unroll
+  for (int v4 = 0; v4 < 12; ++v4) {
+    float4 out = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (4 * v4 < 3 * nb) {
+      const float4 f = __ldg(shj + v4);
+      const float ff[4] = {f.x, f.y, f.z, f.w};
+      float oo[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int idx = 4 * v4 + e, k = idx / 3, c = idx - 3 * k;
+        oo[e] = 0.f;
+        if (idx < 3 * nb) {
+          oo[e] = Y[k] * gcolr[c];
+          a[k] = fmaf(ff[e], gcolr[c], a[k]);
+        }
+      }
+      out = make_float4(oo[0], oo[1], oo[2], oo[3]);
+    }
+    dsh[v4] = out;
+  }
+  float gdir[3];
+  sh_basis_grad(dx, dy, dz, cfg.sh_degree, a, gdir);
+  const float dd = dx * gdir[0] + dy * gdir[1] + dz * gdir[2];
+  gp[0] += (gdir[0] - dx * dd) * inv; gp[1] += (gdir[1] - dy * dd) * inv; gp[2] += (gdir[2] - dz * dd) * inv;
+  d_pos[3 * j] = gp[0]; d_pos[3 * j + 1] = gp[1]; d_pos[3 * j + 2] = gp[2];
+}
+
+int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, const uint8_t* mask,
+                      const float* final_T, const uint32_t* n_contrib, const float* gC, const float* gA, const float* gD,
+                      const float* gN, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
+                      float* d_center2d, cudaStream_t st) {
+  if (s.n == 0) return OCGS_OK;
+  OCGS_CUDA_OK(cudaMemsetAsync(w.grad_rec, 0, (size_t)s.n * kRec * sizeof(float), st));
+  if (w.n_tiles > 0) {
+    const float goh = mask ? (float)((double)cfg.gamma_bg / ((double)cam.W * (double)cam.H)) : 0.f;
+    render_bwd_kernel<<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, mask, final_T, n_contrib, gC, gA, gD, gN,
+                                                 cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
+    OCGS_LAUNCH_OK();
+  }
+  project_bwd_kernel<<<(unsigned)div_up((size_t)s.n, 128), 128, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity,
+                                                                        (const float4*)s.sh, s.n, cam, cfg, w.id_to_rank, w.clamp,
+                                                                        w.grad_rec, d_pos, (float2*)d_scale, (float4*)d_quat, d_opacity,
+                                                                        (float4*)d_sh, (float2*)d_center2d);
+  OCGS_LAUNCH_OK();
+  return OCGS_OK;
+}
+
+}  // namespace ocgs

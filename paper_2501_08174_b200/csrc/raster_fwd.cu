@@ -1,0 +1,175 @@
+// raster_fwd.cu -- ocgs_render_fwd (O4-O6, O8): one CTA per 16x16 tile, one thread per pixel, the tile's depth-ordered
+// list walked front to back in shared-memory batches of records; early stop per pixel, per warp and per CTA.
+// Fused: background loss L_b (Eq. 1) and the visibility statistics.
+#include "common.cuh"
+
+namespace ocgs {
+
+constexpr int kFwdBatch = 128;                 // list entries staged per batch
+constexpr float kContribFix = 134217728.0f;    // 2^27: alpha*T in fixed point for the warp-wide REDUX sum
+
+// O4 in the centred form: k = dx*M2 - A0, l = dy*M2 - A1, (u,v) = (qx,qy)/qz with q = k x l.
+__device__ __forceinline__ bool eval_pair(const float4 r0, const float4 r1, const float4 r2, float px, float py, float near_z,
+                                          float inv_sigma2, float& rho, float& z, float& u, float& v, bool& surf) {
+  const float dx = px - r2.y, dy = py - r2.z;
+  const float k0 = fmaf(dx, r0.x, -r0.w), k1 = fmaf(dx, r0.y, -r1.x), k2 = fmaf(dx, r0.z, -r1.w);
+  const float l0 = fmaf(dy, r0.x, -r1.y), l1 = fmaf(dy, r0.y, -r1.z), l2 = fmaf(dy, r0.z, -r2.x);
+  const float qx = fmaf(k1, l2, -k2 * l1), qy = fmaf(k2, l0, -k0 * l2), qz = fmaf(k0, l1, -k1 * l0);
+  if (qz == 0.0f) return false;
+  const float inv = __frcp_rn(qz);
+  u = qx * inv; v = qy * inv;
+  const float rho3 = fmaf(u, u, v * v);
+  const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
+  surf = rho3 <= rho2;
+  rho = surf ? rho3 : rho2;
+  z = surf ? fmaf(r0.x, u, fmaf(r0.y, v, r0.z)) : r0.z;
+  if (z < near_z) return false;
+  if (rho > r2.w) return false;
+  return true;
+}
+
+template <bool kStats>
+__global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
+                                                         const float4* __restrict__ rec, const uint32_t* __restrict__ rank_to_id,
+                                                         const uint8_t* __restrict__ mask, int W, int H, int tiles_x,
+                                                         ocgs_config cfg, float* __restrict__ color, float* __restrict__ alpha,
+                                                         float* __restrict__ depth, float* __restrict__ normal,
+                                                         uint32_t* __restrict__ n_contrib, float* __restrict__ final_T, float* __restrict__ loss_partial,
+                                                         uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum) {
+  __shared__ float4 s_rec[kFwdBatch * 5];
+  __shared__ uint32_t s_rank[kFwdBatch];
+  __shared__ uint32_t s_cnt[kStats ? kFwdBatch : 1];
+  __shared__ float s_sum[kStats ? kFwdBatch : 1];
+  __shared__ float s_red[8];
+
+  const int tile = blockIdx.x;
+  const int tx = tile % tiles_x, ty = tile / tiles_x;
+  const int lx = threadIdx.x & 15, ly = threadIdx.x >> 4;
+  const int ix = tx * kTile + lx, iy = ty * kTile + ly;
+  const bool inside = ix < W && iy < H;
+  const float px = (float)ix, py = (float)iy;
+  const uint32_t start = ranges[2 * tile], end = ranges[2 * tile + 1];
+  const float inv_sigma2 = 1.0f / cfg.filter_sigma2;
+  const int lane = threadIdx.x & 31;
+
+  float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f;
+  uint32_t last = 0;
+  bool done = !inside;
+
+  for (uint32_t b0 = start; b0 < end; b0 += kFwdBatch) {
+    const int cnt = (int)min((uint32_t)kFwdBatch, end - b0);
+    if (__syncthreads_and(done)) break;
+    if ((int)threadIdx.x < cnt) s_rank[threadIdx.x] = list[b0 + threadIdx.x];
+    if (kStats && threadIdx.x < kFwdBatch) { s_cnt[threadIdx.x] = 0; s_sum[threadIdx.x] = 0.f; }
+    __syncthreads();
+    for (int i = threadIdx.x; i < cnt * 5; i += 256) {
+      const int e = i / 5, part = i - 5 * e;
+      s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 5 + part);
+    }
+    __syncthreads();
+    for (int j = 0; j < cnt; ++j) {
+      if (__all_sync(0xFFFFFFFFu, done)) break;
+      const float4 r0 = s_rec[5 * j], r1 = s_rec[5 * j + 1], r2 = s_rec[5 * j + 2];
+      float rho, z, u, v;
+      bool surf;
+      bool blend = false;
+      float wgt = 0.f;
+      if (!done && eval_pair(r0, r1, r2, px, py, cfg.near_z, inv_sigma2, rho, z, u, v, surf)) {
+        const float4 r3 = s_rec[5 * j + 3], r4 = s_rec[5 * j + 4];
+        const float a = fminf(cfg.alpha_max, r3.x * __expf(-0.5f * rho));
+        const float Tn = T * (1.0f - a);
+        if (Tn < cfg.t_min) {
+          done = true;  // S11: stop before blending this pair
+        } else {
+          wgt = a * T;
+          C0 = fmaf(wgt, r3.y, C0); C1 = fmaf(wgt, r3.z, C1); C2 = fmaf(wgt, r3.w, C2);
+          D = fmaf(wgt, z, D);
+          N0 = fmaf(wgt, r4.x, N0); N1 = fmaf(wgt, r4.y, N1); N2 = fmaf(wgt, r4.z, N2);
+          T = Tn;
+          last = (b0 - start) + j + 1;
+          blend = true;
+        }
+      }
+      if (kStats) {
+        const unsigned bal = __ballot_sync(0xFFFFFFFFu, blend);
+        if (bal) {
+          const unsigned fix = __reduce_add_sync(0xFFFFFFFFu, (unsigned)__float2uint_rn(wgt * kContribFix));
+          if (lane == 0) {
+            atomicAdd(&s_cnt[j], (uint32_t)__popc(bal));
+            atomicAdd(&s_sum[j], (float)fix * (1.0f / kContribFix));
+          }
+        }
+      }
+    }
+    if (kStats) {
+      __syncthreads();
+      if ((int)threadIdx.x < cnt && s_cnt[threadIdx.x] > 0) {
+        const uint32_t id = rank_to_id[s_rank[threadIdx.x]];
+        atomicAdd(&vis_count[id], s_cnt[threadIdx.x]);
+        atomicAdd(&contrib_sum[id], s_sum[threadIdx.x]);
+      }
+    }
+  }
+
+  const float A = 1.0f - T;
+  if (inside) {
+    const size_t HW = (size_t)W * H, p = (size_t)iy * W + ix;
+    color[p] = fmaf(T, cfg.bg[0], C0); color[HW + p] = fmaf(T, cfg.bg[1], C1); color[2 * HW + p] = fmaf(T, cfg.bg[2], C2);
+    alpha[p] = A;
+    depth[p] = D;
+    normal[p] = N0; normal[HW + p] = N1; normal[2 * HW + p] = N2;
+    n_contrib[p] = last;
+    final_T[p] = T;
+  }
+  if (loss_partial) {  // Eq. 1: A (1 - M), fixed-order reduction -> deterministic
+    float lb = 0.f;
+    if (inside) lb = (mask == nullptr || mask[(size_t)iy * W + ix] == 0) ? A : 0.f;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) lb += __shfl_xor_sync(0xFFFFFFFFu, lb, o);
+    __syncthreads();
+    if (lane == 0) s_red[threadIdx.x >> 5] = lb;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      float s = 0.f;
+#pragma unroll
+      for (int w2 = 0; w2 < 8; ++w2) s += s_red[w2];
+      loss_partial[tile] = s;
+    }
+  }
+}
+
+__global__ void __launch_bounds__(1024) loss_final_kernel(const float* __restrict__ partial, int n_tiles, float inv_hw,
+                                                          float* __restrict__ loss_bg) {
+  __shared__ double s[1024];
+  double acc = 0.0;
+  for (int i = threadIdx.x; i < n_tiles; i += 1024) acc += (double)partial[i];
+  s[threadIdx.x] = acc;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *loss_bg = (float)(s[0] * (double)inv_hw);
+}
+
+int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Workspace& w, const uint8_t* mask, float* color,
+                      float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,
+                      float* contrib_sum, cudaStream_t st) {
+  if (w.n_tiles == 0) return OCGS_OK;
+  const bool stats = vis_count != nullptr && contrib_sum != nullptr;
+  float* lp = loss_bg ? w.loss_partial : nullptr;
+  if (stats)
+    render_fwd_kernel<true><<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, mask, cam.W, cam.H,
+                                                       cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, lp, vis_count, contrib_sum);
+  else
+    render_fwd_kernel<false><<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, mask, cam.W, cam.H,
+                                                        cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, lp, nullptr, nullptr);
+  OCGS_LAUNCH_OK();
+  if (loss_bg) {
+    loss_final_kernel<<<1, 1024, 0, st>>>(w.loss_partial, w.n_tiles, (float)(1.0 / ((double)cam.W * (double)cam.H)), loss_bg);
+    OCGS_LAUNCH_OK();
+  }
+  return OCGS_OK;
+}
+
+}  // namespace ocgs

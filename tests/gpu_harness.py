@@ -1,0 +1,116 @@
+"""Shared helpers of the -m gpu parity tests: run one view through the C ABI (via the thin binding) and through the oracle
+on the same seeded inputs.  No arithmetic of the method lives here."""
+from __future__ import annotations
+
+import numpy as np
+
+
+def gpu_modules():
+    import torch
+    from paper_2501_08174_b200 import binding as B
+    return torch, B
+
+
+class GpuView:
+    """preprocess -> bin_sort -> render_fwd (-> render_bwd) of one view through the C ABI."""
+
+    def __init__(self, scene_arrays, cam_np, cfg_kw, key_capacity=None, ws=None):
+        torch, B = gpu_modules()
+        self.torch, self.B = torch, B
+        pos, scale, quat, opacity, sh = scene_arrays
+        dev = "cuda"
+        self.t = dict(pos=torch.tensor(np.ascontiguousarray(pos, np.float32), device=dev),
+                      scale=torch.tensor(np.ascontiguousarray(scale, np.float32), device=dev),
+                      quat=torch.tensor(np.ascontiguousarray(quat, np.float32), device=dev),
+                      opacity=torch.tensor(np.ascontiguousarray(opacity, np.float32), device=dev),
+                      sh=torch.tensor(np.ascontiguousarray(sh, np.float32), device=dev))
+        self.n = int(pos.shape[0])
+        self.cam = B.camera_from(cam_np)
+        self.W, self.H = cam_np.width, cam_np.height
+        self.cfg = B.ocgs_default_config(**cfg_kw)
+        self.cap = int(key_capacity if key_capacity is not None else max(1 << 16, 64 * self.n))
+        self.layout = B.ocgs_workspace_layout(self.n, self.W, self.H, self.cap)
+        self.ws = ws if ws is not None else B.alloc_workspace(self.n, self.W, self.H, self.cap)
+        self.surfels = B.make_surfels(self.t["pos"], self.t["scale"], self.t["quat"], self.t["opacity"], self.t["sh"])
+        self.out = None
+        self.mask_t = None
+
+    def sec(self, name, dtype, count):
+        return self.B.ws_section(self.ws, self.layout, name, dtype, count).cpu().numpy()
+
+    def preprocess(self):
+        self.B.ocgs_preprocess(self.surfels, self.cam, self.cfg, self.ws, self.cap)
+        torch = self.torch
+        n = self.n
+        return dict(depth_bits=self.sec("depth_bits", torch.int32, n).view(np.uint32),
+                    rect=self.sec("rect", torch.int16, 4 * n).view(np.uint16).reshape(n, 4).astype(np.int32),
+                    tiles=self.sec("tiles", torch.int32, n).view(np.uint32), clamp=self.sec("clamp", torch.uint8, n),
+                    rec_id=self.sec("rec_id", torch.float32, 20 * n).reshape(n, 20))
+
+    def bin_sort(self, want_ids=True):
+        torch = self.torch
+        ids = torch.zeros(self.cap, dtype=torch.int32, device="cuda") if want_ids else None
+        self.B.ocgs_bin_sort(self.n, self.cam, self.cfg, self.ws, self.cap, ids)
+        h = self.B.ocgs_check(self.ws, raise_on_error=False)
+        K = int(h.K)
+        n_tiles = ((self.W + 15) // 16) * ((self.H + 15) // 16)
+        res = dict(K=K, n_vis=int(h.n_vis), error=int(h.error),
+                   ranges=self.sec("ranges", torch.int32, 2 * n_tiles).view(np.uint32).reshape(n_tiles, 2))
+        if want_ids and not h.error:
+            res["ids"] = ids[:K].cpu().numpy().view(np.uint32)
+            res["tile_keys"] = self.sec("tile_keys", torch.int32, max(K, 1)).view(np.uint32)[:K]
+        return res
+
+    def render_fwd(self, mask=None, stats=True, vis_count=None, contrib_sum=None, want_loss=True):
+        torch, B = self.torch, self.B
+        self.out = B.alloc_outputs(self.W, self.H)
+        self.mask_t = None if mask is None else torch.tensor(np.ascontiguousarray(mask, np.uint8), device="cuda")
+        if stats:
+            self.vis = vis_count if vis_count is not None else torch.zeros(self.n, dtype=torch.int32, device="cuda")
+            self.cs = contrib_sum if contrib_sum is not None else torch.zeros(self.n, dtype=torch.float32, device="cuda")
+        else:
+            self.vis = self.cs = None
+        o = self.out
+        B.ocgs_render_fwd(self.n, self.cam, self.cfg, self.ws, self.cap, self.mask_t, o["color"], o["alpha"], o["depth"], o["normal"],
+                          o["n_contrib"], o["loss_bg"] if want_loss else None, self.vis, self.cs)
+        torch.cuda.synchronize()
+        res = {k: v.cpu().numpy() for k, v in o.items()}
+        res["n_contrib"] = res["n_contrib"].view(np.uint32)
+        res["loss_bg"] = float(res["loss_bg"][0])
+        if stats:
+            res["vis_count"] = self.vis.cpu().numpy().view(np.uint32)
+            res["contrib_sum"] = self.cs.cpu().numpy()
+        return res
+
+    def render_bwd(self, gC=None, gA=None, gD=None, gN=None, mask="same"):
+        torch, B = self.torch, self.B
+        g = B.alloc_grads(self.n)
+
+        def dev(a):
+            return None if a is None else torch.tensor(np.ascontiguousarray(a, np.float32), device="cuda")
+        m = self.mask_t if isinstance(mask, str) else (None if mask is None else torch.tensor(np.ascontiguousarray(mask, np.uint8), device="cuda"))
+        B.ocgs_render_bwd(self.surfels, self.cam, self.cfg, self.ws, self.cap, m, self.out["n_contrib"], dev(gC), dev(gA), dev(gD), dev(gN),
+                          g["d_pos"], g["d_scale"], g["d_quat"], g["d_opacity"], g["d_sh"], g["d_center2d"])
+        torch.cuda.synchronize()
+        return {k: v.cpu().numpy() for k, v in g.items()}
+
+
+def oracle_view(scene_arrays, cam_np, cfg_kw, mask=None):
+    import oracle as orc
+    kw = dict(cfg_kw)
+    cfg = orc.default_config(sh_degree=kw.pop("sh_degree", 3), bg=kw.pop("bg", (0.0, 0.0, 0.0)), gamma_bg=kw.pop("gamma_bg", 0.5), **kw)
+    cam = orc.camera_from(cam_np)
+    pre, srt, fwd = orc.forward_view(*scene_arrays, cam, cfg, mask=mask)
+    return orc, cam, cfg, pre, srt, fwd
+
+
+def grad_errors(gpu, ora, floor=1e-6):
+    """max relative error per gradient array over entries with |oracle| > floor (north_star tolerance rule)."""
+    out = {}
+    for k in ora:
+        a, b = gpu[k].astype(np.float64).ravel(), ora[k].ravel()
+        sel = np.abs(b) > floor
+        rel = np.abs(a[sel] - b[sel]) / np.abs(b[sel]) if sel.any() else np.zeros(1)
+        small = np.abs(a[~sel] - b[~sel]).max() if (~sel).any() else 0.0
+        out[k] = (float(rel.max()), float(np.quantile(rel, 0.999)), float(small), int(sel.sum()))
+    return out
