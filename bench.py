@@ -1,0 +1,366 @@
+#!/usr/bin/env python
+"""bench.py -- ms per fwd+bwd raster step on the paper-shaped workload (BASELINE.json configs[2]: 1600x1200, 1 M surfels).
+
+A "step" is one pass of the whole hot path over one view: ocgs_preprocess -> ocgs_bin_sort -> ocgs_render_fwd (background
+loss L_b and visibility statistics on) -> ocgs_masked_l1 (harness photometric gradient, S20) -> ocgs_render_bwd, all
+through the C ABI.  Views rotate over a fixed set; inputs are resident in HBM before the timed region (`value`), or in
+pinned host memory with the copies inside the timed region (`e2e`, through ocgs_step_host).  `--impl reference` times the
+CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "ms per fwd+bwd raster step (1600x1200, 1M surfels)"
+FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 40.0, 22.0, 111.0
+ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 148 SMs x 128 FP32 lanes x 2 (FMA) x max SM clock (B200_PROFILING.md)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="config3")
+    ap.add_argument("--views", type=int, default=4, help="distinct views rotated over per rank")
+    ap.add_argument("--shrink", type=float, default=1.0, help="scale surfel counts (debug only; invalidates the metric)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def make_scene(args):
+    from paper_2501_08174_b200 import scenegen as sg
+    kw = {}
+    if args.shrink != 1.0:
+        import inspect
+        sig = inspect.signature(sg.CONFIGS[args.config]).parameters
+        for k in ("n_obj", "n_bg", "n_shell", "n_in"):
+            if k in sig:
+                kw[k] = max(1, int(sig[k].default * args.shrink))
+    return sg.make_scene(args.config, **kw)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f).get("hbm_gbs", 6650.0), "measured"
+    return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx = float(f[1])
+            except ValueError:
+                continue
+            for nme, val in zip(names, f[2:6]):
+                if val.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# CPU oracle arm (cpu_baseline and --impl reference)
+# ------------------------------------------------------------------------------------------------------------------
+
+def oracle_sample(scene, view, window_frac=0.2):
+    """One bounded sample of the step on the host cores: full preprocess + bin_sort of the view, forward and backward
+    of a centred window of window_frac x window_frac of the image, extrapolated by pixel count.  Returns (ms per step
+    extrapolated, description, cores)."""
+    import oracle as orc
+    cam_np = scene.cameras[view]
+    cam = orc.camera_from(cam_np)
+    cfg = orc.default_config(sh_degree=scene.sh_degree)
+    W, H = cam_np.width, cam_np.height
+    ww, wh = max(16, int(W * window_frac) // 16 * 16), max(16, int(H * window_frac) // 16 * 16)
+    x0, y0 = (W - ww) // 2 // 16 * 16, (H - wh) // 2 // 16 * 16
+    win = (x0, y0, x0 + ww, y0 + wh)
+    mask = scene.mask(view)
+    P = (scene.pos, scene.scale, scene.quat, scene.opacity, scene.sh)
+    t0 = time.perf_counter()
+    pre = orc.preprocess(*P, cam, cfg)
+    srt = orc.bin_sort(pre, cam, cfg)
+    t1 = time.perf_counter()
+    fwd = orc.render_fwd(pre, srt, scene.opacity, cam, cfg, mask=mask, window=win, want_fragile=False)
+    gC = np.where(mask[None] > 0, np.sign(fwd["color"] - 0.5), 0.0) / (3.0 * W * H)
+    orc.render_bwd(*P, pre, srt, cam, cfg, mask=mask, gC=gC, window=win)
+    t2 = time.perf_counter()
+    scale = (W * H) / float(ww * wh)
+    ms = ((t1 - t0) + (t2 - t1) * scale) * 1e3
+    desc = (f"view {view}: preprocess+bin_sort of all {scene.n} surfels ({(t1 - t0):.2f} s) + fwd+bwd of a centred {ww}x{wh} window "
+            f"({(t2 - t1):.2f} s) scaled by {scale:.1f} to {W}x{H}")
+    return ms, desc, orc.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    scene = make_scene(args)
+    cam0 = scene.cameras[0]
+    vals = []
+    desc, cores = "", 0
+    for i in range(args.warmup + args.steps):
+        ms, desc, cores = oracle_sample(scene, i % min(args.views, len(scene.cameras)), window_frac=0.1)
+        if i >= args.warmup:
+            vals.append(ms)
+    v = float(np.mean(vals))
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{scene.name}: {scene.n} surfels, {cam0.width}x{cam0.height}, views rotated"},
+            "cpu_baseline": {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# CUDA arm
+# ------------------------------------------------------------------------------------------------------------------
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2501_08174_b200 import binding as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    B.lib()
+
+    scene = make_scene(args)
+    n, deg = scene.n, scene.sh_degree
+    cams = scene.cameras
+    W, H = cams[0].width, cams[0].height
+    # views are sharded over ranks: rank r owns views r, r+world, ...; no data-path collective
+    my_views = [v for v in range(len(cams)) if v % world == rank][: args.views] or [rank % len(cams)]
+    cfg = B.ocgs_default_config(sh_degree=deg)
+    cap = int(os.environ.get("OCGS_KEY_CAPACITY", 48 * n if n < 2_000_000 else 16 * n))
+
+    def to_dev(a, dt=torch.float32):
+        return torch.tensor(np.ascontiguousarray(a), dtype=dt, device=dev)
+
+    params = dict(pos=to_dev(scene.pos), scale=to_dev(scene.scale), quat=to_dev(scene.quat), opacity=to_dev(scene.opacity), sh=to_dev(scene.sh))
+    surfels = B.make_surfels(params["pos"], params["scale"], params["quat"], params["opacity"], params["sh"])
+    ws = B.alloc_workspace(n, W, H, cap, device=dev)
+    out = B.alloc_outputs(W, H, device=dev)
+    grads = B.alloc_grads(n, device=dev)
+    gC = torch.empty((3, H, W), dtype=torch.float32, device=dev)
+    loss_l1 = torch.zeros(1, dtype=torch.float32, device=dev)
+    vis = torch.zeros(n, dtype=torch.int32, device=dev)
+    cs = torch.zeros(n, dtype=torch.float32, device=dev)
+    cam_c = [B.camera_from(cams[v]) for v in my_views]
+    masks = [to_dev(scene.mask(v), torch.uint8) for v in my_views]
+
+    # targets: forward render of the perturbed copy (Appendix B), once, outside the timed region
+    pert = scene.perturbed()
+    pp = dict(pos=to_dev(pert.pos), scale=params["scale"], quat=params["quat"], opacity=to_dev(pert.opacity), sh=to_dev(pert.sh))
+    psurf = B.make_surfels(pp["pos"], pp["scale"], pp["quat"], pp["opacity"], pp["sh"])
+    targets = []
+    for i in range(len(my_views)):
+        B.ocgs_preprocess(psurf, cam_c[i], cfg, ws, cap)
+        B.ocgs_bin_sort(n, cam_c[i], cfg, ws, cap)
+        B.ocgs_render_fwd(n, cam_c[i], cfg, ws, cap, masks[i], out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"])
+        h = B.ocgs_check(ws)
+        targets.append(out["color"].clone())
+    del pp, psurf
+
+    def step(i, stats=True):
+        c, m = cam_c[i], masks[i]
+        B.ocgs_preprocess(surfels, c, cfg, ws, cap)
+        B.ocgs_bin_sort(n, c, cfg, ws, cap)
+        B.ocgs_render_fwd(n, c, cfg, ws, cap, m, out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"], out["loss_bg"],
+                          vis if stats else None, cs if stats else None)
+        B.ocgs_masked_l1(out["color"], targets[i], m, W, H, gC, loss_l1, ws, n, cap)
+        B.ocgs_render_bwd(surfels, c, cfg, ws, cap, m, out["n_contrib"], gC, None, None, None, grads["d_pos"], grads["d_scale"],
+                          grads["d_quat"], grads["d_opacity"], grads["d_sh"], grads["d_center2d"])
+
+    # warm-up + workload counters (outside the timed region)
+    nv = len(my_views)
+    counters = []
+    for i in range(max(args.warmup, nv)):
+        vis.zero_()
+        step(i % nv)
+        h = B.ocgs_check(ws)
+        if i < nv:
+            counters.append(dict(K=int(h.K), n_vis=int(h.n_vis), E=int(out["n_contrib"].long().sum().item()),
+                                 B=int(vis.long().sum().item()), loss_bg=float(out["loss_bg"].item()), loss_l1=float(loss_l1.item())))
+    vis.zero_(); cs.zero_()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- timed region: K steps, CUDA events on the launching stream, per-launch marks inside ------------------------
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    cap_marks = 64 * args.steps + 8
+    barrier()
+    ev0.record()
+    B.ocgs_profile_begin(cap_marks)
+    for i in range(args.steps):
+        step(i % nv)
+    marks = B.ocgs_profile_end(cap_marks)
+    ev1.record()
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if rank == 0 else None
+    B.ocgs_check(ws)
+    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+
+    # ---- e2e: the same step through ocgs_step_host with pinned host buffers -----------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        hp = {k: torch.tensor(np.ascontiguousarray(getattr(scene, k)), dtype=torch.float32).pin_memory() for k in ("pos", "scale", "quat", "opacity", "sh")}
+        h_masks = [m.cpu().pin_memory() for m in masks]
+        h_targets = [tg.cpu().pin_memory() for tg in targets]
+        h_grads = torch.empty(58 * n, dtype=torch.float32).pin_memory()
+        h_alpha = torch.empty(H * W, dtype=torch.float32).pin_memory()
+        h_loss = torch.empty(1, dtype=torch.float32).pin_memory()
+        d_params = torch.empty(58 * n + 16, dtype=torch.float32, device=dev)
+        d_grads = torch.empty(58 * n + 16, dtype=torch.float32, device=dev)
+        d_images = torch.empty(14 * H * W, dtype=torch.float32, device=dev)
+        d_mask = torch.empty(H * W, dtype=torch.uint8, device=dev)
+        d_nc = torch.empty(H * W, dtype=torch.int32, device=dev)
+        d_lb = torch.zeros(1, dtype=torch.float32, device=dev)
+
+        def e2e_step(i):
+            B.ocgs_step_host(hp["pos"], hp["scale"], hp["quat"], hp["opacity"], hp["sh"], n, cam_c[i], cfg, h_masks[i], h_targets[i],
+                             h_grads, h_alpha, h_loss, d_params, d_mask, d_images, d_nc, d_grads, vis, cs, d_lb, ws, cap)
+        for i in range(2):
+            e2e_step(i % nv)
+        k_e = max(3, min(args.steps, 10))
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(k_e):
+            e2e_step(i % nv)  # synchronises inside (results are on the host when it returns)
+        torch.cuda.synchronize()
+        t_e = (time.perf_counter() - t0) * 1e3
+        te = torch.tensor([t_e], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        h2d = 58 * n * 4 + H * W + 3 * H * W * 4
+        d2h = 58 * n * 4 + H * W * 4 + 4 + 16
+        e2e = {"value": float(te.item()) / (k_e * world), "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": k_e}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- per-kernel breakdown and roofline of the dominant kernel ----------------------------------------------------
+    agg, cnt = {}, {}
+    for name, ms in marks:
+        agg[name] = agg.get(name, 0.0) + ms
+        cnt[name] = cnt.get(name, 0) + 1
+    steps = args.steps
+    kern_total = sum(agg.values())
+    kernels = sorted(({"name": k, "ms_per_step": agg[k] / steps, "launches_per_step": cnt[k] / steps, "share": agg[k] / kern_total}
+                      for k in agg), key=lambda d: -d["ms_per_step"])
+    launches = sum(c for k, c in cnt.items() if not k.startswith("memset"))
+    mean = {k: float(np.mean([c[k] for c in counters])) for k in counters[0]}
+    hbm_peak, peak_src = measured_peaks()
+    dom = kernels[0]
+    avg_launch_s = (agg[dom["name"]] / cnt[dom["name"]]) * 1e-3
+    roof = None
+    if dom["name"] in ("render_bwd_kernel", "render_fwd_kernel"):
+        fl = FLOP_EVAL * mean["E"] + (FLOP_BLEND_BWD if dom["name"] == "render_bwd_kernel" else FLOP_BLEND_FWD) * mean["B"]
+        ach = fl / avg_launch_s / 1e12
+        roof = {"kernel": dom["name"], "bound": "alu", "achieved": ach, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": ach / ALU_PEAK_TFLOPS, "traffic": None,
+                "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                "algorithmic": f"{FLOP_EVAL:.0f} flop x E evaluated pairs + {FLOP_BLEND_BWD if dom['name']=='render_bwd_kernel' else FLOP_BLEND_FWD:.0f} flop x B blended pairs"}
+    else:
+        per_launch = {"radix_scatter_kernel": 16.0 * mean["K"], "radix_hist_kernel": 4.0 * mean["K"], "emit_keys_kernel": 8.0 * mean["K"],
+                      "preprocess_kernel": 61.0 * n + 280.0 * mean["n_vis"], "project_bwd_kernel": 232.0 * n + 312.0 * mean["n_vis"],
+                      "memset_grad_rec": 80.0 * n}.get(dom["name"], 0.0)
+        ach = per_launch / avg_launch_s / 1e9
+        roof = {"kernel": dom["name"], "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                "traffic": None, "peak_source": peak_src}
+
+    ms_per_step = ms_total / (steps * world)
+    line = {"metric": METRIC, "value": ms_per_step, "unit": "ms", "n_gpus": world, "steps": steps, "warmup": max(args.warmup, nv),
+            "ms_per_step": ms_total / steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": f"{scene.name}: {n} surfels, {W}x{H}, SH degree {deg}, {nv} views rotated per rank (views sharded over ranks)",
+                       "l2": "inputs larger than L2: 232 MB of surfel parameters are re-read every step", "key_capacity": cap,
+                       "shrink": args.shrink},
+            "surfels_per_s": n * world / (ms_total / steps * 1e-3), "pixels_per_s": W * H * world / (ms_total / steps * 1e-3),
+            "workload_counters": mean, "gpu_launches": launches, "clocks": clocks, "roofline": roof, "kernels": kernels[:12],
+            "kernel_ms_sum_per_step": kern_total / steps}
+    if e2e:
+        line["e2e"] = e2e
+    if world == 1 and not args.no_cpu_baseline:
+        ms_cpu, desc, cores = oracle_sample(scene, my_views[0], window_frac=0.1)
+        line["cpu_baseline"] = {"value": ms_cpu, "unit": "ms", "cores": cores, "kind": "oracle", "sample": desc}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

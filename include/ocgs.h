@@ -170,17 +170,32 @@ int ocgs_prune_stats(const ocgs_surfels* in, uint32_t* vis_count, float* contrib
                      uint8_t* prune_mask, int32_t* remap, const ocgs_surfels_mut* out, int* n_out, int reset_stats,
                      void* ws, void* stream);
 
+/* ---- harness photometric term (S20; the L1 part of Eq. 2) --------------------------------------------
+ * loss = 1/(3 H W) sum |M (R - I)| (device scalar, nullable), dL_dcolor[3,H,W] = M sign(R - I)/(3 H W).  color, target:
+ * device [3,H,W]; mask device u8 [H,W], nullable (= all ones).  Uses ws.loss_partial as scratch (n, key_capacity: the values
+ * the workspace was sized with). */
+int ocgs_masked_l1(const float* color, const float* target, const uint8_t* mask, int width, int height, float* dL_dcolor,
+                   float* loss, void* ws, int n, size_t key_capacity, void* stream);
+
+/* ---- diagnostics: per-launch device timing ----------------------------------------------------------------------------
+ * Between ocgs_profile_begin and ocgs_profile_end every kernel (and memset) the library enqueues from the calling thread
+ * is followed by a CUDA event; ocgs_profile_end synchronises `stream` and returns, for each launch in order, the
+ * elapsed milliseconds since the previous mark (ms_out[max_out], host) and its name (names_out, host, 32 bytes each).
+ * Thread-local; the only state the library keeps, and only while profiling. */
+int ocgs_profile_begin(int capacity, void* stream);
+int ocgs_profile_end(void* stream, int max_out, float* ms_out, char* names_out, int* count);
+
 /* ---- end-to-end step with HOST buffers (bench.py "e2e") ---------------------------------------------------------------
- * Copies the surfel parameters, mask and upstream colour gradient from (pinned) host memory to the given device
- * staging buffers, runs (1)-(4) with L_b and statistics on, copies the gradients, the alpha map and loss_bg back and
- * synchronises.  Every pointer named h_* is host memory, d_* device memory owned by the caller.
+ * Copies the surfel parameters, mask and target image from (pinned) host memory to the given device staging buffers,
+ * runs (1)-(3) with L_b and statistics on, ocgs_masked_l1, then (4); copies the gradients, the alpha map and loss_bg back
+ * and synchronises.  Every pointer named h_* is host memory, d_* device memory owned by the caller.
  * h_grads: host [N*58] floats in the order pos(3N) scale(2N) quat(4N) opacity(N) sh(48N).  d_params and d_grads: device
  * staging of at least 58*N + 16 floats each (sections start on multiples of 4 floats).  key_capacity must be the value
  * the workspace was sized with (every call of one step passes the same n, image size and key_capacity).
- * d_images: device [11*H*W] floats (color 3, alpha 1, depth 1, normal 3, dL_dcolor 3) + d_ncontrib u32 [H*W]. */
+ * d_images: device [14*H*W] floats (color 3, alpha 1, depth 1, normal 3, target 3, dL_dcolor 3); d_ncontrib u32 [H*W]. */
 int ocgs_step_host(const float* h_pos, const float* h_scale, const float* h_quat, const float* h_opacity,
                    const float* h_sh, int n, const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask,
-                   const float* h_dL_dcolor, float* h_grads, float* h_alpha, float* h_loss_bg, float* d_params,
+                   const float* h_target, float* h_grads, float* h_alpha, float* h_loss_bg, float* d_params,
                    uint8_t* d_mask, float* d_images, uint32_t* d_ncontrib, float* d_grads, uint32_t* d_vis_count,
                    float* d_contrib_sum, float* d_loss_bg, void* ws, size_t key_capacity, void* stream);
 

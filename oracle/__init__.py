@@ -160,6 +160,7 @@ def render_fwd(pre, srt, opacity, cam: OrcCamera, cfg: OrcConfig, mask=None, win
         contrib_sum = np.zeros(n, np.float64)
     fragile = np.zeros((H, W), np.uint8) if want_fragile else None
     ftouch = np.zeros(n, np.uint32) if want_fragile else None
+    cond_rho = np.zeros(n, np.float64) if want_fragile else None
     if margins is None and want_fragile:
         margins = default_margins()
     ids = srt["ids"] if srt["K"] > 0 else np.zeros(1, np.uint32)
@@ -168,8 +169,8 @@ def render_fwd(pre, srt, opacity, cam: OrcCamera, cfg: OrcConfig, mask=None, win
                               _p(pre["M"]), _p(pre["c2d"]), _p(pre["rho_cut"]), _p(opacity), _p(pre["normal"]), _p(pre["rgb"]),
                               _p(ids), _p(srt["ranges"]), _p(m), C.c_int(x0), C.c_int(y0), C.c_int(x1), C.c_int(y1),
                               _p(out["color"]), _p(out["alpha"]), _p(out["depth"]), _p(out["normal"]), _p(out["n_contrib"]),
-                              _p(vis_count), _p(contrib_sum), _p(fragile), _p(ftouch))
-    out.update(loss_bg=float(Lb), vis_count=vis_count, contrib_sum=contrib_sum, fragile=fragile, fragile_touch=ftouch)
+                              _p(vis_count), _p(contrib_sum), _p(fragile), _p(ftouch), _p(cond_rho))
+    out.update(loss_bg=float(Lb), vis_count=vis_count, contrib_sum=contrib_sum, fragile=fragile, fragile_touch=ftouch, cond_rho=cond_rho)
     return out
 
 
@@ -181,6 +182,7 @@ def render_bwd(pos, scale, quat, opacity, sh, pre, srt, cam: OrcCamera, cfg: Orc
     x0, y0, x1, y1 = window if window is not None else (0, 0, W, H)
     out = dict(d_pos=np.zeros((n, 3)), d_scale=np.zeros((n, 2)), d_quat=np.zeros((n, 4)), d_opacity=np.zeros(n),
                d_sh=np.zeros((n, 16, 3)), d_center2d=np.zeros((n, 2)))
+    oabs = np.zeros(n)
     ids = srt["ids"] if srt["K"] > 0 else np.zeros(1, np.uint32)
     m = None if mask is None else np.ascontiguousarray(mask, np.uint8)
     gC, gA, gD, gN = _f64(gC), _f64(gA), _f64(gD), _f64(gN)
@@ -188,7 +190,8 @@ def render_bwd(pos, scale, quat, opacity, sh, pre, srt, cam: OrcCamera, cfg: Orc
                          _p(pre["visible"]), _p(pre["M"]), _p(pre["c2d"]), _p(pre["rho_cut"]), _p(pre["normal"]), _p(pre["rgb"]),
                          _p(pre["clamp"]), _p(ids), _p(srt["ranges"]), _p(m), _p(gC), _p(gA), _p(gD), _p(gN),
                          C.c_int(x0), C.c_int(y0), C.c_int(x1), C.c_int(y1), _p(out["d_pos"]), _p(out["d_scale"]),
-                         _p(out["d_quat"]), _p(out["d_opacity"]), _p(out["d_sh"]), _p(out["d_center2d"]))
+                         _p(out["d_quat"]), _p(out["d_opacity"]), _p(out["d_sh"]), _p(out["d_center2d"]), _p(oabs))
+    out["_d_opacity_abs"] = oabs
     return out
 
 

@@ -276,13 +276,14 @@ struct PairEval {
   bool capped;     // o G > alpha_max
   bool fragile;
   double u, v, qz, k[3], l[3], rho, z, G, alpha, dx, dy;
+  double drho_est; // fp32 forward-error estimate of rho for this pair
   double err_est;  // a-priori bound on |delta alpha| (+ relative depth term) of an fp32 evaluation of this pair
 };
 
 inline PairEval eval_pair(double x, double y, const float* Mf, const float* c2df, float rho_cut_f, float of,
                           const OrcConfig& cfg, const OrcMargins* mg) {
   PairEval e;
-  e.valid = false; e.fragile = false; e.surf = true; e.capped = false; e.err_est = 0.0;
+  e.valid = false; e.fragile = false; e.surf = true; e.capped = false; e.err_est = 0.0; e.drho_est = 0.0;
   double M[9];
   for (int i = 0; i < 9; ++i) M[i] = Mf[i];
   for (int i = 0; i < 3; ++i) { e.k[i] = x * M[6 + i] - M[i]; e.l[i] = y * M[6 + i] - M[3 + i]; }
@@ -337,6 +338,7 @@ inline PairEval eval_pair(double x, double y, const float* Mf, const float* c2df
     } else {
       drho = 4.0 * ep * e.rho;
     }
+    e.drho_est = drho;
     const double dalpha = e.capped ? 0.0 : 0.5 * e.alpha * drho;
     e.err_est = dalpha + e.alpha * dz / std::fmax(1.0, A(e.z));
   }
@@ -431,13 +433,14 @@ int64_t orc_bin_sort(int n, const uint8_t* visible, const uint32_t* depth_bits, 
 // which Gaussians are used during the color accumulation step"; Eq. 1 for L_b.
 // Pixels inside the window [wx0,wx1) x [wy0,wy1) are computed, the rest is left untouched.
 // vis_count / contrib_sum ACCUMULATE (O8).  Returns L_b summed over the window (divided by W*H).
-// fragile (bit 0 = a decision within its margin, bit 1 = ill-conditioned, S22) / fragile_touch may be null.
+// fragile (bit 0 = a decision within its margin, bit 1 = ill-conditioned, S22) / fragile_touch / cond_rho may be null.
+// cond_rho[N] (max-accumulated): largest fp32 error estimate of rho over the blended pairs of each surfel.
 // ------------------------------------------------------------------------------------------------
 double orc_render_fwd(int n, const OrcCamera* cam, const OrcConfig* cfg, const OrcMargins* mg, const float* M, const float* c2d,
                       const float* rho_cut, const float* opacity, const double* normal, const double* rgb, const uint32_t* ids,
                       const uint32_t* ranges, const uint8_t* mask, int wx0, int wy0, int wx1, int wy1, double* color,
                       double* alpha, double* depth, double* nrm, uint32_t* n_contrib, uint32_t* vis_count, double* contrib_sum,
-                      uint8_t* fragile, uint32_t* fragile_touch) {
+                      uint8_t* fragile, uint32_t* fragile_touch, double* cond_rho) {
   (void)n;
   const int W = cam->width, H = cam->height, T = cfg->tile;
   const int tiles_x = (W + T - 1) / T, tiles_y = (H + T - 1) / T;
@@ -463,6 +466,10 @@ double orc_render_fwd(int n, const OrcCamera* cam, const OrcConfig* cfg, const O
           if (Tn < (double)cfg->t_min) break;  // S11: stop before blending this pair
           const double w = e.alpha * Tr;
           cerr += Tr * e.err_est;
+          if (cond_rho && e.drho_est > cond_rho[j]) {  // per-surfel conditioning: worst fp32 rho error among its blended pairs
+#pragma omp critical(condrho)
+            if (e.drho_est > cond_rho[j]) cond_rho[j] = e.drho_est;
+          }
           for (int c = 0; c < 3; ++c) { C[c] += w * rgb[3 * j + c]; N[c] += w * normal[3 * j + c]; }
           D += w * e.z;
           if (vis_count) {
@@ -500,18 +507,20 @@ double orc_render_fwd(int n, const OrcCamera* cam, const OrcConfig* cfg, const O
 // involved Gaussians are updated"; occluded Gaussians "cannot receive gradients".
 // Upstream gradients gC[3HW], gA[HW], gD[HW], gN[3HW] (any may be null = 0); with mask != null and
 // gamma_bg != 0 the background-loss gradient gamma (1-M)/(H W) is added to gA (Eq. 1 / Eq. 3).
-// Outputs are OVERWRITTEN.  d_center2d = M22 * (dL/dM02, dL/dM12) (reading R-c2d).
+// Outputs are OVERWRITTEN.  d_opacity_abs (nullable) = sum over pairs of |term of d_opacity| (summation conditioning).
+// d_center2d = M22 * (dL/dM02, dL/dM12) (reading R-c2d).
 // ------------------------------------------------------------------------------------------------
 void orc_render_bwd(int n, const float* pos, const float* scale, const float* quat, const float* opacity, const float* sh,
                     const OrcCamera* cam, const OrcConfig* cfg, const uint8_t* visible, const float* M, const float* c2d,
                     const float* rho_cut, const double* normal, const double* rgb, const uint8_t* clamp, const uint32_t* ids,
                     const uint32_t* ranges, const uint8_t* mask, const double* gC, const double* gA, const double* gD,
                     const double* gN, int wx0, int wy0, int wx1, int wy1, double* d_pos, double* d_scale, double* d_quat,
-                    double* d_opacity, double* d_sh, double* d_center2d) {
+                    double* d_opacity, double* d_sh, double* d_center2d, double* d_opacity_abs) {
   const int W = cam->width, H = cam->height, T = cfg->tile;
   const int tiles_x = (W + T - 1) / T, tiles_y = (H + T - 1) / T;
   const size_t HW = (size_t)W * H;
   // per-surfel intermediate gradients: gM[9], g_c2d[2], g_o, g_rgb[3], g_n[3]
+  std::vector<double> goabs((size_t)n, 0.0);
   std::vector<double> gM((size_t)n * 9, 0.0), gc2((size_t)n * 2, 0.0), go((size_t)n, 0.0), grgb((size_t)n * 3, 0.0), gn((size_t)n * 3, 0.0);
 
 #pragma omp parallel
@@ -594,6 +603,8 @@ void orc_render_bwd(int n, const float* pos, const float* scale, const float* qu
             if (a_o != 0.0) {
 #pragma omp atomic
               go[j] += a_o;
+#pragma omp atomic
+              goabs[j] += std::fabs(a_o);
             }
             for (int c = 0; c < 3; ++c) {
               if (a_rgb[c] != 0.0) {
@@ -622,6 +633,7 @@ void orc_render_bwd(int n, const float* pos, const float* scale, const float* qu
     for (int k = 0; k < 2; ++k) { d_scale[2 * j + k] = 0; d_center2d[2 * j + k] = 0; }
     for (int k = 0; k < 4; ++k) d_quat[4 * j + k] = 0;
     d_opacity[j] = 0;
+    if (d_opacity_abs) d_opacity_abs[j] = goabs[j];  // sum of |terms|: conditioning of the d_opacity summation
     for (int k = 0; k < 48; ++k) d_sh[48 * (size_t)j + k] = 0;
     if (!visible[j]) continue;
     double g[9];

@@ -18,7 +18,7 @@ _LIB_PATH = os.path.join(_HERE, "csrc", "libocgs.so")
 OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
            "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_prune_workspace_bytes",
-           "ocgs_prune_stats", "ocgs_step_host"]
+           "ocgs_prune_stats", "ocgs_step_host", "ocgs_masked_l1", "ocgs_profile_begin", "ocgs_profile_end"]
 
 
 class OcgsError(RuntimeError):
@@ -184,15 +184,34 @@ def ocgs_prune_stats(surfels, vis_count, contrib_sum, cfg, prune_mask, remap, ou
                                                    C.c_int(int(reset_stats)), _ptr(ws), _stream(stream)))
 
 
-def ocgs_step_host(h_pos, h_scale, h_quat, h_opacity, h_sh, n, cam, cfg, h_mask, h_dL_dcolor, h_grads, h_alpha, h_loss_bg, d_params,
+def ocgs_step_host(h_pos, h_scale, h_quat, h_opacity, h_sh, n, cam, cfg, h_mask, h_target, h_grads, h_alpha, h_loss_bg, d_params,
                    d_mask, d_images, d_ncontrib, d_grads, d_vis_count, d_contrib_sum, d_loss_bg, ws, key_capacity, stream=None):
     def hp(t):
         return None if t is None else C.c_void_p(t.data_ptr())
     _ok("ocgs_step_host", lib().ocgs_step_host(hp(h_pos), hp(h_scale), hp(h_quat), hp(h_opacity), hp(h_sh), C.c_int(n), C.byref(cam),
-                                               C.byref(cfg), hp(h_mask), hp(h_dL_dcolor), hp(h_grads), hp(h_alpha), hp(h_loss_bg),
+                                               C.byref(cfg), hp(h_mask), hp(h_target), hp(h_grads), hp(h_alpha), hp(h_loss_bg),
                                                _ptr(d_params), _ptr(d_mask), _ptr(d_images), _ptr(d_ncontrib), _ptr(d_grads),
                                                _ptr(d_vis_count), _ptr(d_contrib_sum), _ptr(d_loss_bg), _ptr(ws),
                                                C.c_size_t(key_capacity), _stream(stream)))
+
+
+def ocgs_masked_l1(color, target, mask, width, height, dL_dcolor, loss, ws, n, key_capacity, stream=None):
+    _ok("ocgs_masked_l1", lib().ocgs_masked_l1(_ptr(color), _ptr(target), _ptr(mask), C.c_int(width), C.c_int(height), _ptr(dL_dcolor),
+                                               _ptr(loss), _ptr(ws), C.c_int(n), C.c_size_t(key_capacity), _stream(stream)))
+
+
+def ocgs_profile_begin(capacity: int, stream=None):
+    _ok("ocgs_profile_begin", lib().ocgs_profile_begin(C.c_int(capacity), _stream(stream)))
+
+
+def ocgs_profile_end(capacity: int, stream=None):
+    """-> list of (kernel name, milliseconds) in launch order."""
+    ms = (C.c_float * capacity)()
+    names = C.create_string_buffer(capacity * 32)
+    cnt = C.c_int(0)
+    _ok("ocgs_profile_end", lib().ocgs_profile_end(_stream(stream), C.c_int(capacity), ms, names, C.byref(cnt)))
+    raw = names.raw
+    return [(raw[i * 32:(i + 1) * 32].split(b"\0", 1)[0].decode(), float(ms[i])) for i in range(cnt.value)]
 
 
 # ---- allocation helpers (device memory only; no arithmetic) --------------------------------------------------------

@@ -1,11 +1,26 @@
 // api.cu -- extern "C" entry points of libocgs (include/ocgs.h): argument checks, workspace carving, stage launches.
 #include <string.h>
 
+#include <vector>
+
 #include "common.cuh"
 
 namespace ocgs {
 
 thread_local int g_last_cuda_error = 0;
+
+// ---- diagnostic per-launch timing -------------------------------------------------------------------------------
+thread_local bool g_prof_on = false;
+namespace {
+struct Prof { std::vector<cudaEvent_t> ev; std::vector<const char*> names; size_t used = 0; };
+thread_local Prof g_prof;
+}
+void prof_mark(cudaStream_t st, const char* name) {
+  if (g_prof.used >= g_prof.ev.size()) return;
+  cudaEventRecord(g_prof.ev[g_prof.used], st);
+  g_prof.names[g_prof.used] = name;
+  ++g_prof.used;
+}
 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -183,6 +198,43 @@ int ocgs_render_bwd(const ocgs_surfels* s, const ocgs_camera* cam, const ocgs_co
                            d_sh, d_center2d, (cudaStream_t)stream);
 }
 
+int ocgs_masked_l1(const float* color, const float* target, const uint8_t* mask, int width, int height, float* dL_dcolor, float* loss,
+                   void* ws, int n, size_t key_capacity, void* stream) {
+  if (!color || !target || !dL_dcolor || !ws) return OCGS_ERR_INVALID_ARG;
+  Workspace w;
+  if (!carve_workspace(ws, n, width, height, key_capacity, &w, nullptr)) return OCGS_ERR_UNSUPPORTED;
+  return launch_masked_l1(color, target, mask, width, height, dL_dcolor, loss, w.loss_partial, w.n_tiles, (cudaStream_t)stream);
+}
+
+int ocgs_profile_begin(int capacity, void* stream) {
+  if (capacity <= 0) return OCGS_ERR_INVALID_ARG;
+  while ((int)g_prof.ev.size() < capacity + 1) {
+    cudaEvent_t e;
+    OCGS_CUDA_OK(cudaEventCreate(&e));
+    g_prof.ev.push_back(e);
+    g_prof.names.push_back("");
+  }
+  g_prof.used = 0;
+  g_prof_on = true;
+  prof_mark((cudaStream_t)stream, "begin");
+  return OCGS_OK;
+}
+
+int ocgs_profile_end(void* stream, int max_out, float* ms_out, char* names_out, int* count) {
+  g_prof_on = false;
+  OCGS_CUDA_OK(cudaStreamSynchronize((cudaStream_t)stream));
+  int c = 0;
+  for (size_t i = 1; i < g_prof.used && c < max_out; ++i, ++c) {
+    float ms = 0.f;
+    OCGS_CUDA_OK(cudaEventElapsedTime(&ms, g_prof.ev[i - 1], g_prof.ev[i]));
+    ms_out[c] = ms;
+    strncpy(names_out + (size_t)c * 32, g_prof.names[i], 31);
+    names_out[(size_t)c * 32 + 31] = 0;
+  }
+  if (count) *count = c;
+  return OCGS_OK;
+}
+
 size_t ocgs_prune_workspace_bytes(int n) { return (div_up((size_t)(n > 0 ? n : 0), 1024) + 2) * sizeof(uint32_t); }
 
 int ocgs_prune_stats(const ocgs_surfels* in, uint32_t* vis_count, float* contrib_sum, const ocgs_config* cfg, uint8_t* prune_mask,
@@ -193,7 +245,7 @@ int ocgs_prune_stats(const ocgs_surfels* in, uint32_t* vis_count, float* contrib
 }
 
 int ocgs_step_host(const float* h_pos, const float* h_scale, const float* h_quat, const float* h_opacity, const float* h_sh, int n,
-                   const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask, const float* h_dL_dcolor, float* h_grads,
+                   const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask, const float* h_target, float* h_grads,
                    float* h_alpha, float* h_loss_bg, float* d_params, uint8_t* d_mask, float* d_images, uint32_t* d_ncontrib,
                    float* d_grads, uint32_t* d_vis_count, float* d_contrib_sum, float* d_loss_bg, void* ws, size_t key_capacity,
                    void* stream) {
@@ -215,14 +267,16 @@ int ocgs_step_host(const float* h_pos, const float* h_scale, const float* h_quat
   OCGS_CUDA_OK(cudaMemcpyAsync(p_sh, h_sh, 48 * N * 4, cudaMemcpyHostToDevice, st));
   OCGS_CUDA_OK(cudaMemcpyAsync(d_mask, h_mask, HW, cudaMemcpyHostToDevice, st));
   float* color = d_images; float* alpha = color + 3 * HW; float* depth = alpha + HW; float* normal = depth + HW;
-  float* gC = normal + 3 * HW;
-  OCGS_CUDA_OK(cudaMemcpyAsync(gC, h_dL_dcolor, 3 * HW * 4, cudaMemcpyHostToDevice, st));
+  float* target = normal + 3 * HW;
+  float* gC = target + 3 * HW;
+  OCGS_CUDA_OK(cudaMemcpyAsync(target, h_target, 3 * HW * 4, cudaMemcpyHostToDevice, st));
   ocgs_surfels s = {p_pos, p_scale, p_quat, p_opa, p_sh, n};
   int rc;
   if ((rc = ocgs_preprocess(&s, cam, cfg, ws, key_capacity, stream)) != OCGS_OK) return rc;
   if ((rc = ocgs_bin_sort(n, cam, cfg, ws, key_capacity, nullptr, stream)) != OCGS_OK) return rc;
   if ((rc = ocgs_render_fwd(n, cam, cfg, ws, key_capacity, d_mask, color, alpha, depth, normal, d_ncontrib, d_loss_bg, d_vis_count,
                             d_contrib_sum, stream)) != OCGS_OK) return rc;
+  if ((rc = ocgs_masked_l1(color, target, d_mask, cam->width, cam->height, gC, nullptr, ws, n, key_capacity, stream)) != OCGS_OK) return rc;
   float* g_pos = d_grads; float* g_scale = d_grads + up4(3 * N); float* g_quat = g_scale + up4(2 * N); float* g_opa = g_quat + 4 * N;
   float* g_sh = g_opa + up4(N);
   if ((rc = ocgs_render_bwd(&s, cam, cfg, ws, key_capacity, d_mask, d_ncontrib, gC, nullptr, nullptr, nullptr, g_pos, g_scale, g_quat,

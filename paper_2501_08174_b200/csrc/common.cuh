@@ -66,6 +66,10 @@ extern thread_local int g_last_cuda_error;
 inline int cuda_fail(cudaError_t e) { g_last_cuda_error = (int)e; return OCGS_ERR_CUDA; }
 #define OCGS_CUDA_OK(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) return ::ocgs::cuda_fail(_e); } while (0)
 #define OCGS_LAUNCH_OK() do { cudaError_t _e = cudaGetLastError(); if (_e != cudaSuccess) return ::ocgs::cuda_fail(_e); } while (0)
+// diagnostic per-launch timing (ocgs_profile_begin/end): when enabled on this thread, an event is recorded after each launch
+extern thread_local bool g_prof_on;
+void prof_mark(cudaStream_t st, const char* name);
+#define OCGS_LAUNCHED(st, name) do { OCGS_LAUNCH_OK(); if (::ocgs::g_prof_on) ::ocgs::prof_mark(st, name); } while (0)
 
 struct CamParams {
   float V[12];  // rows 0..2 of the view matrix
@@ -88,6 +92,9 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
 
 int launch_prune(const ocgs_surfels& in, uint32_t* vis_count, float* contrib_sum, const ocgs_config& cfg, uint8_t* prune_mask,
                  int32_t* remap, const ocgs_surfels_mut* out, int* n_out, int reset_stats, void* ws, cudaStream_t st);
+
+int launch_masked_l1(const float* color, const float* target, const uint8_t* mask, int W, int H, float* dL_dcolor, float* loss,
+                     float* partial, int n_partial, cudaStream_t st);
 
 // stable LSD radix sort of (u32 key, u32 value) pairs on bits [0, key_bits); count is read from the device (*n_ptr, u64 or
 // u32 selected by n_is_u64) and bounded by n_max for grid sizing. Result lands in (keysA, valsA) when the number of

@@ -85,12 +85,13 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
 
 int launch_preprocess(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, cudaStream_t st) {
   OCGS_CUDA_OK(cudaMemsetAsync(w.header, 0, sizeof(ocgs_header), st));
+  if (g_prof_on) prof_mark(st, "memset_header");
   if (s.n == 0) return OCGS_OK;
   const int blocks = (int)div_up((size_t)s.n, 256);
   preprocess_kernel<<<blocks, 256, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity, (const float4*)s.sh,
                                             s.n, cam, cfg, w.depth_bits, w.rect, w.tiles, w.clamp, (float4*)w.rec_id,
                                             w.id_to_rank, w.dkeyA, w.rank_to_id, w.header);
-  OCGS_LAUNCH_OK();
+  OCGS_LAUNCHED(st, "preprocess_kernel");
   return OCGS_OK;
 }
 

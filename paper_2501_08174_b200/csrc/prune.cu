@@ -106,7 +106,7 @@ static int launch_compact(const float* in, float* out, const int32_t* remap, int
   if (total == 0) return OCGS_OK;
   const unsigned grid = (unsigned)min(div_up(total, 256), (size_t)148 * 64);
   compact_kernel<Vec, VPS><<<grid, 256, 0, st>>>((const Vec*)in, remap, total, (Vec*)out);
-  OCGS_LAUNCH_OK();
+  OCGS_LAUNCHED(st, "compact_kernel");
   return OCGS_OK;
 }
 
@@ -120,11 +120,11 @@ int launch_prune(const ocgs_surfels& in, uint32_t* vis_count, float* contrib_sum
   uint32_t* blocksum = (uint32_t*)ws;
   const int nb = (int)div_up((size_t)n, kPruneBlock);
   prune_flag_kernel<<<nb, kPruneBlock, 0, st>>>(vis_count, contrib_sum, in.opacity, n, cfg.tau_contrib, cfg.min_opacity, prune_mask, blocksum);
-  OCGS_LAUNCH_OK();
+  OCGS_LAUNCHED(st, "prune_flag_kernel");
   prune_scan_kernel<<<1, 1024, 0, st>>>(blocksum, nb, n_out);
-  OCGS_LAUNCH_OK();
+  OCGS_LAUNCHED(st, "prune_scan_kernel");
   prune_remap_kernel<<<nb, kPruneBlock, 0, st>>>(prune_mask, blocksum, n, remap);
-  OCGS_LAUNCH_OK();
+  OCGS_LAUNCHED(st, "prune_remap_kernel");
   if (out) {
     int rc;
     if ((rc = launch_compact<float, 3>(in.pos, out->pos, remap, n, st)) != OCGS_OK) return rc;

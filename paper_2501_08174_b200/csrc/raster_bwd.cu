@@ -308,17 +308,18 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
                       float* d_center2d, cudaStream_t st) {
   if (s.n == 0) return OCGS_OK;
   OCGS_CUDA_OK(cudaMemsetAsync(w.grad_rec, 0, (size_t)s.n * kRec * sizeof(float), st));
+  if (g_prof_on) prof_mark(st, "memset_grad_rec");
   if (w.n_tiles > 0) {
     const float goh = mask ? (float)((double)cfg.gamma_bg / ((double)cam.W * (double)cam.H)) : 0.f;
     render_bwd_kernel<<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, mask, final_T, n_contrib, gC, gA, gD, gN,
                                                  cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
-    OCGS_LAUNCH_OK();
+    OCGS_LAUNCHED(st, "render_bwd_kernel");
   }
   project_bwd_kernel<<<(unsigned)div_up((size_t)s.n, 128), 128, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity,
                                                                         (const float4*)s.sh, s.n, cam, cfg, w.id_to_rank, w.clamp,
                                                                         w.grad_rec, d_pos, (float2*)d_scale, (float4*)d_quat, d_opacity,
                                                                         (float4*)d_sh, (float2*)d_center2d);
-  OCGS_LAUNCH_OK();
+  OCGS_LAUNCHED(st, "project_bwd_kernel");
   return OCGS_OK;
 }
 

@@ -164,10 +164,10 @@ int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Worksp
   else
     render_fwd_kernel<false><<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, mask, cam.W, cam.H,
                                                         cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, lp, nullptr, nullptr);
-  OCGS_LAUNCH_OK();
+  OCGS_LAUNCHED(st, "render_fwd_kernel");
   if (loss_bg) {
     loss_final_kernel<<<1, 1024, 0, st>>>(w.loss_partial, w.n_tiles, (float)(1.0 / ((double)cam.W * (double)cam.H)), loss_bg);
-    OCGS_LAUNCH_OK();
+    OCGS_LAUNCHED(st, "loss_final_kernel");
   }
   return OCGS_OK;
 }

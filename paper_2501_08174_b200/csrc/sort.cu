@@ -170,11 +170,11 @@ int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t
     const int bits = min(kRadixBits, key_bits - shift);
     const uint32_t mask = (1u << bits) - 1u;
     radix_hist_kernel<<<grid, kSortThreads, 0, st>>>(kin, n_ptr, n_is_u64, n_max, shift, mask, hist);
-    OCGS_LAUNCH_OK();
+    OCGS_LAUNCHED(st, "radix_hist_kernel");
     radix_rowscan_kernel<<<kRadix, 1024, 0, st>>>(hist, n_ptr, n_is_u64, n_max, digit_total);
-    OCGS_LAUNCH_OK();
+    OCGS_LAUNCHED(st, "radix_rowscan_kernel");
     radix_scatter_kernel<<<grid, kSortThreads, 0, st>>>(kin, vin, kout, vout, n_ptr, n_is_u64, n_max, shift, mask, hist, digit_total);
-    OCGS_LAUNCH_OK();
+    OCGS_LAUNCHED(st, "radix_scatter_kernel");
     uint32_t* t = kin; kin = kout; kout = t;
     t = vin; vin = vout; vout = t;
   }
@@ -384,19 +384,19 @@ int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cu
   if (n > 0) {
     reorder_kernel<<<nblk, kScanBlock, 0, st>>>(w.rank_to_id, w.header, w.tiles, (const float4*)w.rec_id, w.id_to_rank, (float4*)w.rec,
                                                 w.tcount, w.blocksum);
-    OCGS_LAUNCH_OK();
+    OCGS_LAUNCHED(st, "reorder_kernel");
   }
   scan_blocksums_kernel<<<1, 1024, 0, st>>>(w.blocksum, w.header, w.key_capacity, w.offsets);
-  OCGS_LAUNCH_OK();
+  OCGS_LAUNCHED(st, "scan_blocksums_kernel");
   if (n > 0) {
     scan_apply_kernel<<<nblk, kScanBlock, 0, st>>>(w.tcount, w.blocksum, w.header, w.offsets);
-    OCGS_LAUNCH_OK();
+    OCGS_LAUNCHED(st, "scan_apply_kernel");
   }
   const size_t cap = w.key_capacity;
   if (cap > 0 && n > 0) {
     emit_keys_kernel<<<(unsigned)div_up(cap, kEmitTile), kEmitThreads, 0, st>>>(w.header, w.offsets, w.rank_to_id, w.rect, cam.tiles_x,
                                                                                 w.tile_keys, w.tile_vals);
-    OCGS_LAUNCH_OK();
+    OCGS_LAUNCHED(st, "emit_keys_kernel");
     int bits = 1;
     while ((1 << bits) < w.n_tiles) ++bits;
     bool inB = false;
@@ -406,15 +406,15 @@ int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cu
       const unsigned g = (unsigned)min(div_up(cap, 1024), (size_t)148 * 8);
       copy_u32_kernel<<<g, 1024, 0, st>>>(w.tkeyB, w.tile_keys, w.header);
       copy_u32_kernel<<<g, 1024, 0, st>>>(w.tvalB, w.tile_vals, w.header);
-      OCGS_LAUNCH_OK();
+      OCGS_LAUNCHED(st, "copy_u32_kernel");
     }
   }
   const unsigned rgrid = (unsigned)max(div_up(max(cap, (size_t)1), 256), div_up((size_t)w.n_tiles, 256));
   tile_ranges_kernel<<<rgrid, 256, 0, st>>>(w.header, w.tile_keys, w.n_tiles, w.ranges);
-  OCGS_LAUNCH_OK();
+  OCGS_LAUNCHED(st, "tile_ranges_kernel");
   if (sorted_ids && cap > 0) {
     gather_ids_kernel<<<(unsigned)div_up(cap, 256), 256, 0, st>>>(w.header, w.tile_vals, w.rank_to_id, sorted_ids);
-    OCGS_LAUNCH_OK();
+    OCGS_LAUNCHED(st, "gather_ids_kernel");
   }
   return OCGS_OK;
 }

@@ -382,8 +382,10 @@ def config3(n_obj=300_000, n_bg=700_000, width=1600, height=1200, f=2800.0, n_vi
                                                    (0, 0, 0), 1.0 + 1e-3))
 
 
-def config4(n_shell=250_000, n_in=400_000, n_bg=150_000, res=1024, f=1300.0, n_views=64, seed=3) -> Scene:
-    """Occlusion-heavy pruning workload (configs[3]): near-opaque shell, occluded interior, room shell."""
+def config4(n_shell=250_000, n_in=400_000, n_bg=150_000, res=1024, f=1300.0, n_views=64, seed=3, scale_mul=1.0) -> Scene:
+    """Occlusion-heavy pruning workload (configs[3]): near-opaque shell, occluded interior, room shell.
+    scale_mul > 1 enlarges the SHELL surfels only, to keep the shell's coverage when a test shrinks the surfel counts
+    (coverage ~ n_shell * scale^2)."""
     rng = np.random.Generator(np.random.PCG64(seed))
     p_shell = _normalize(rng.normal(size=(n_shell, 3)))
     q_shell = frames_from_normals(p_shell, rng)
@@ -395,6 +397,7 @@ def config4(n_shell=250_000, n_in=400_000, n_bg=150_000, res=1024, f=1300.0, n_v
     quat = np.concatenate([q_shell, q_in, q_bg])
     n = pos.shape[0]
     scale = log_uniform(rng, 0.003, 0.03, (n, 2))
+    scale[:n_shell] *= scale_mul
     opacity = np.concatenate([sigmoid(rng.normal(3.0, 0.5, n_shell)), sigmoid(rng.normal(0.0, 1.0, n_in + n_bg))])
     sh = make_sh(rng, n, 3)
     cams = sphere_cameras(n_views, 3.0, res, res, f)

@@ -1,0 +1,192 @@
+"""-m gpu: the CUDA path (through the C ABI) against the oracle, element by element, on seeded inputs.
+
+Tolerances (north_star / DESIGN.md "tolerances"): integer outputs bit-exact; images, alpha, depth (relative to
+max(1,|D|)) and L_b to 1e-4 on non-fragile pixels; gradients per check_grads (relative 1e-3 above 1e-6).
+"""
+import numpy as np
+import pytest
+
+from gpu_harness import GpuView, check_grads, oracle_view
+from paper_2501_08174_b200 import scenegen as sg
+
+pytestmark = pytest.mark.gpu
+
+IMG_TOL = 1e-4
+
+
+def arrays(sc):
+    return (sc.pos, sc.scale, sc.quat, sc.opacity, sc.sh)
+
+
+def full_parity(sc, view, cfg_kw, rng_seed=5, max_fragile=2e-3, with_bwd=True):
+    P = arrays(sc)
+    camn = sc.cameras[view]
+    m = sc.mask(view)
+    orc, cam, cfg, pre, srt, fw = oracle_view(P, camn, cfg_kw, mask=m)
+    g = GpuView(P, camn, cfg_kw)
+    # (1) preprocess: integer outputs bit-exact
+    gp = g.preprocess()
+    vis = pre["visible"] == 1
+    assert np.array_equal(gp["tiles"], pre["tiles_touched"])
+    assert np.array_equal(gp["depth_bits"], pre["depth_bits"])
+    assert np.array_equal(gp["rect"][vis], pre["rect"][vis])
+    assert np.array_equal(gp["clamp"][vis], pre["clamp"][vis])
+    rec = gp["rec_id"][vis]
+    assert np.array_equal(rec[:, 0:3], pre["M"][vis][:, 6:9])           # M2 row, bit-exact (Appendix A)
+    assert np.array_equal(rec[:, 9:11], pre["c2d"][vis]) and np.array_equal(rec[:, 11], pre["rho_cut"][vis])
+    assert np.abs(rec[:, 13:16] - pre["rgb"][vis]).max() < 2e-5 if vis.any() else True
+    assert np.abs(rec[:, 16:19] - pre["normal"][vis]).max() < 2e-6 if vis.any() else True
+    # (2) bin_sort: keys, order, ranges bit-exact
+    gs = g.bin_sort()
+    assert gs["error"] == 0 and gs["K"] == srt["K"] and gs["n_vis"] == int(vis.sum())
+    assert np.array_equal(gs["ids"], srt["ids"])
+    assert np.array_equal(gs["tile_keys"], (srt["keys"] >> np.uint64(32)).astype(np.uint32))
+    assert np.array_equal(gs["ranges"], srt["ranges"])
+    # (3) forward
+    gf = g.render_fwd(mask=m)
+    ok = fw["fragile"] == 0
+    assert 1.0 - ok.mean() <= max_fragile, f"fragile fraction {1 - ok.mean()}"
+    for k in ("color", "alpha", "depth", "normal"):
+        scale = np.maximum(1.0, np.abs(fw[k])) if k == "depth" else 1.0
+        err = np.abs(gf[k] - fw[k]) / scale
+        assert (err * ok).max() <= IMG_TOL, (k, (err * ok).max())
+        assert err.max() <= 0.02, (k, "fragile pixel beyond the discontinuity bound", err.max())
+    assert np.array_equal(gf["n_contrib"][ok], fw["n_contrib"][ok])
+    assert abs(gf["loss_bg"] - fw["loss_bg"]) <= IMG_TOL
+    dv = np.abs(gf["vis_count"].astype(np.int64) - fw["vis_count"].astype(np.int64))
+    assert np.all(dv <= fw["fragile_touch"])
+    clean = fw["fragile_touch"] == 0
+    assert np.array_equal(gf["vis_count"][clean], fw["vis_count"][clean])
+    assert np.allclose(gf["contrib_sum"][clean], fw["contrib_sum"][clean], rtol=1e-4, atol=2e-6)
+    rep = None
+    if with_bwd:
+        # (4) backward: seeded N(0,1) upstream on all four maps, zero on fragile pixels (both sides see the same inputs)
+        rng = np.random.default_rng(rng_seed)
+        H, W = camn.height, camn.width
+        okf = ok.astype(np.float64)
+        gC, gA = rng.normal(size=(3, H, W)) * okf, rng.normal(size=(H, W)) * okf
+        gD, gN = rng.normal(size=(H, W)) * okf, rng.normal(size=(3, H, W)) * okf
+        mm = np.where(ok, m, 1).astype(np.uint8)
+        gg = g.render_bwd(gC=gC, gA=gA, gD=gD, gN=gN, mask=mm)
+        og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=gC.astype(np.float32), gA=gA.astype(np.float32),
+                            gD=gD.astype(np.float32), gN=gN.astype(np.float32))
+        rep = check_grads(gg, og)
+        # surfels never blended receive exactly zero gradient
+        never = gf["vis_count"] == 0
+        for k in ("d_pos", "d_scale", "d_quat", "d_opacity", "d_sh"):
+            assert np.all(gg[k][never] == 0.0), k
+    return dict(fragile=float(1 - ok.mean()), grads=rep, K=srt["K"])
+
+
+def test_config1_all_views():
+    sc = sg.make_scene("config1")
+    for v in range(4):
+        full_parity(sc, v, dict(sh_degree=0))
+
+
+def test_random_scenes_ragged_image_sh3_background():
+    # 100x70: partial tiles on both axes; random orientations; coloured background
+    for seed in (3, 4):
+        sc = sg.random_scene(300, 100, 70, 80.0, seed=seed, sh_degree=3)
+        full_parity(sc, 0, dict(sh_degree=3, bg=(0.3, 0.1, 0.2)))
+
+
+def test_subpixel_surfels_filter_branch():
+    sc = sg.random_scene(400, 64, 48, 40.0, seed=9, sh_degree=1, scale_lo=0.005, scale_hi=0.05)
+    full_parity(sc, 0, dict(sh_degree=1))
+
+
+def test_config2_shrunk_two_views():
+    # config 2's geometry and distributions at 1/5 of the surfels: 1 900 tiles, several sort blocks, SH degree 3
+    sc = sg.make_scene("config2", n_obj=20_000, n_bg=20_000)
+    for v in (0, 7):
+        r = full_parity(sc, v, dict(sh_degree=3))
+        assert r["K"] > 4096 * 3
+
+
+def test_sh_degrees():
+    sc = sg.random_scene(120, 48, 48, 40.0, seed=13, sh_degree=3)
+    for deg in (0, 1, 2, 3):
+        full_parity(sc, 0, dict(sh_degree=deg))
+
+
+def test_empty_and_all_culled_and_capacity():
+    import torch
+    from paper_2501_08174_b200 import binding as B
+    sc = sg.random_scene(50, 40, 40, 30.0, seed=2, sh_degree=0)
+    camn = sc.cameras[0]
+    # all culled: everything behind the camera
+    P = list(arrays(sc))
+    P[0] = sc.pos * np.array([1, 1, -1], np.float32)
+    g = GpuView(tuple(P), camn, dict(sh_degree=0, bg=(0.5, 0.25, 0.125)))
+    gp = g.preprocess()
+    assert np.all(gp["tiles"] == 0)
+    gs = g.bin_sort()
+    assert gs["K"] == 0 and gs["n_vis"] == 0 and np.all(gs["ranges"] == 0)
+    gf = g.render_fwd(mask=np.zeros((40, 40), np.uint8))
+    assert np.all(gf["alpha"] == 0) and gf["loss_bg"] == 0.0 and np.all(gf["n_contrib"] == 0)
+    assert np.allclose(gf["color"][0], 0.5) and np.allclose(gf["color"][2], 0.125)
+    gg = g.render_bwd(gC=np.ones((3, 40, 40)))
+    assert all(np.all(v == 0) for v in gg.values())
+    # n = 0
+    z = GpuView(tuple(a[:0] for a in arrays(sc)), camn, dict(sh_degree=0))
+    z.preprocess()
+    zs = z.bin_sort()
+    assert zs["K"] == 0
+    zf = z.render_fwd()
+    assert np.all(zf["alpha"] == 0)
+    # capacity overflow: flagged on the device, reported by ocgs_check, later calls stay safe
+    small = GpuView(arrays(sc), camn, dict(sh_degree=0), key_capacity=8)
+    small.preprocess()
+    s2 = small.bin_sort()
+    assert s2["error"] == 1 and s2["K"] > 8
+    with pytest.raises(B.OcgsError) as e:
+        B.ocgs_check(small.ws)
+    assert e.value.code == B.OCGS_ERR_CAPACITY
+    f2 = small.render_fwd()
+    assert np.all(f2["alpha"] == 0)
+    # unsupported / invalid arguments
+    with pytest.raises(B.OcgsError):
+        B.ocgs_preprocess(small.surfels, small.cam, B.ocgs_default_config(tile=8), small.ws, small.cap)
+    with pytest.raises(B.OcgsError):
+        B.ocgs_preprocess(small.surfels, small.cam, B.ocgs_default_config(sh_degree=4), small.ws, small.cap)
+    torch.cuda.synchronize()
+
+
+def test_masked_l1_and_host_step_match_device_path():
+    import torch
+    from paper_2501_08174_b200 import binding as B
+    sc = sg.make_scene("config2", n_obj=4000, n_bg=4000, width=320, height=240, f=360.0)
+    camn = sc.cameras[1]
+    m = sc.mask(1)
+    g = GpuView(arrays(sc), camn, dict(sh_degree=3))
+    g.preprocess(); g.bin_sort()
+    gf = g.render_fwd(mask=m)
+    rng = np.random.default_rng(0)
+    target = rng.uniform(0, 1, (3, 240, 320)).astype(np.float32)
+    tt = torch.tensor(target, device="cuda")
+    gC = torch.empty_like(tt)
+    loss = torch.zeros(1, device="cuda")
+    B.ocgs_masked_l1(g.out["color"], tt, g.mask_t, 320, 240, gC, loss, g.ws, g.n, g.cap)
+    d = (gf["color"].astype(np.float64) - target) * (m[None] > 0)
+    assert abs(float(loss.item()) - np.abs(d).sum() / (3 * 240 * 320)) < 1e-6
+    assert np.array_equal(gC.cpu().numpy(), (np.sign(d) / np.float32(3 * 240 * 320)).astype(np.float32))
+    gg = g.render_bwd(gC=gC.cpu().numpy())
+    # the same step through ocgs_step_host (host buffers, copies inside)
+    n, H, W = g.n, 240, 320
+    hp = [torch.tensor(np.ascontiguousarray(a, np.float32)).pin_memory() for a in arrays(sc)]
+    h_grads = torch.empty(58 * n).pin_memory(); h_alpha = torch.empty(H * W).pin_memory(); h_loss = torch.empty(1).pin_memory()
+    d_params = torch.empty(58 * n + 16, device="cuda"); d_grads = torch.empty(58 * n + 16, device="cuda")
+    d_images = torch.empty(14 * H * W, device="cuda"); d_mask = torch.empty(H * W, dtype=torch.uint8, device="cuda")
+    d_nc = torch.empty(H * W, dtype=torch.int32, device="cuda"); d_lb = torch.zeros(1, device="cuda")
+    vis = torch.zeros(n, dtype=torch.int32, device="cuda"); cs = torch.zeros(n, device="cuda")
+    B.ocgs_step_host(hp[0], hp[1], hp[2], hp[3], hp[4], n, g.cam, g.cfg, torch.tensor(m).pin_memory(), torch.tensor(target).pin_memory(),
+                     h_grads, h_alpha, h_loss, d_params, d_mask, d_images, d_nc, d_grads, vis, cs, d_lb, g.ws, g.cap)
+    assert np.array_equal(h_alpha.numpy().reshape(H, W), gf["alpha"])
+    assert float(h_loss.item()) == gf["loss_bg"]
+    hg = h_grads.numpy()
+    # float atomics: run-to-run order differs, so compare to tolerance, not bits
+    for name, lo, hi in (("d_pos", 0, 3 * n), ("d_scale", 3 * n, 5 * n), ("d_quat", 5 * n, 9 * n), ("d_opacity", 9 * n, 10 * n), ("d_sh", 10 * n, 58 * n)):
+        a, b = hg[lo:hi], gg[name].ravel()
+        assert np.allclose(a, b, rtol=2e-3, atol=1e-6 + 1e-4 * np.abs(b).max()), name
+    assert np.array_equal(vis.cpu().numpy().view(np.uint32), gf["vis_count"])

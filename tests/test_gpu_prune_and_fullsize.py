@@ -1,0 +1,153 @@
+"""-m gpu: (a) occlusion-aware pruning over many views (config 4's geometry), (b) parity at BASELINE.json's full size
+(config 3: 1 M surfels, 1600x1200) in the launch configuration bench.py times, on sampled windows."""
+import numpy as np
+import pytest
+
+from gpu_harness import GpuView, check_grads, oracle_view
+from paper_2501_08174_b200 import scenegen as sg
+
+pytestmark = pytest.mark.gpu
+
+
+def arrays(sc):
+    return (sc.pos, sc.scale, sc.quat, sc.opacity, sc.sh)
+
+
+def test_prune_stats_config4_shrunk_all_views():
+    """accumulate visibility over all views, remove never-blended surfels, compact."""
+    import torch
+    import oracle as orc
+    from paper_2501_08174_b200 import binding as B
+    sc = sg.make_scene("config4", n_shell=6000, n_in=9000, n_bg=3000, res=256, f=325.0, n_views=12, scale_mul=6.5)
+    P = arrays(sc)
+    n = sc.n
+    cfg_kw = dict(sh_degree=3)
+    vis_o = np.zeros(n, np.uint32); cs_o = np.zeros(n, np.float64); touch = np.zeros(n, np.uint64)
+    g = GpuView(P, sc.cameras[0], cfg_kw)
+    vis_g = torch.zeros(n, dtype=torch.int32, device="cuda"); cs_g = torch.zeros(n, dtype=torch.float32, device="cuda")
+    ocfg = orc.default_config(sh_degree=3)
+    for v in range(len(sc.cameras)):
+        cam = orc.camera_from(sc.cameras[v])
+        pre = orc.preprocess(*P, cam, ocfg)
+        srt = orc.bin_sort(pre, cam, ocfg)
+        fw = orc.render_fwd(pre, srt, sc.opacity, cam, ocfg, mask=None, vis_count=vis_o, contrib_sum=cs_o)
+        touch += fw["fragile_touch"]
+        g.cam = B.camera_from(sc.cameras[v])
+        g.preprocess(); g.bin_sort(want_ids=False)
+        g.render_fwd(mask=None, vis_count=vis_g, contrib_sum=cs_g, want_loss=False)
+    vg = vis_g.cpu().numpy().view(np.uint32)
+    clean = touch == 0
+    assert np.array_equal(vg[clean], vis_o[clean])
+    assert np.all(np.abs(vg.astype(np.int64) - vis_o.astype(np.int64)) <= touch.astype(np.int64))
+    assert np.allclose(cs_g.cpu().numpy()[clean], cs_o[clean], rtol=2e-4, atol=5e-6)
+    # prune + compact on the GPU
+    mask_t = torch.empty(n, dtype=torch.uint8, device="cuda"); remap_t = torch.empty(n, dtype=torch.int32, device="cuda")
+    n_out = torch.zeros(1, dtype=torch.int32, device="cuda")
+    outs = [torch.full_like(t, -7.0) for t in (g.t["pos"], g.t["scale"], g.t["quat"], g.t["opacity"], g.t["sh"])]
+    om = B.ocgs_surfels_mut(*[B._ptr(t) for t in outs], n)
+    pws = torch.empty(B.ocgs_prune_workspace_bytes(n), dtype=torch.uint8, device="cuda")
+    B.ocgs_prune_stats(g.surfels, vis_g, cs_g, g.cfg, mask_t, remap_t, om, n_out, 0, pws)
+    torch.cuda.synchronize()
+    pm = mask_t.cpu().numpy()
+    # bit-exact against the oracle's rule applied to the same statistics ...
+    po = orc.prune(vg, cs_g.cpu().numpy(), sc.opacity)
+    assert np.array_equal(pm, po["prune_mask"]) and np.array_equal(remap_t.cpu().numpy(), po["remap"]) and int(n_out.item()) == po["n_out"]
+    # ... and against the oracle's own statistics wherever no fragile pixel was involved
+    po2 = orc.prune(vis_o, cs_o.astype(np.float32), sc.opacity)
+    assert np.array_equal(pm[clean], po2["prune_mask"][clean])
+    assert (pm != po2["prune_mask"]).sum() <= 2
+    comp = orc.compact(dict(pos=sc.pos, scale=sc.scale, quat=sc.quat, opacity=sc.opacity, sh=sc.sh), pm)
+    k = po["n_out"]
+    for t, name in zip(outs, ("pos", "scale", "quat", "opacity", "sh")):
+        got = t.cpu().numpy()
+        assert np.array_equal(got[:k], comp[name]), name
+        assert np.all(got[k:] == -7.0), name  # nothing written past the survivors
+    # the method's purpose: interior surfels (behind a near-opaque shell in every view) go, the visible shell stays
+    interior, shell = sc.group == 2, sc.group == 0
+    assert pm[interior].mean() > 0.97
+    assert pm[shell].mean() < 0.35
+    # tau / min_opacity extension and reset
+    cfg2 = B.ocgs_default_config(sh_degree=3, tau_contrib=0.5, min_opacity=0.2)
+    B.ocgs_prune_stats(g.surfels, vis_g, cs_g, cfg2, mask_t, remap_t, None, n_out, 1, pws)
+    torch.cuda.synchronize()
+    assert int(vis_g.abs().sum().item()) == 0 and float(cs_g.abs().sum().item()) == 0.0  # reset_stats
+
+
+def test_prune_tau_and_min_opacity_rule():
+    import torch
+    import oracle as orc
+    from paper_2501_08174_b200 import binding as B
+    rng = np.random.default_rng(1)
+    n = 100_003  # not a multiple of the block size
+    vis = rng.integers(0, 3, n).astype(np.uint32)
+    cs = np.where(vis > 0, rng.uniform(0, 1, n), 0).astype(np.float32)
+    sc = sg.random_scene(n, 32, 32, 30.0, seed=1, sh_degree=0)
+    g = GpuView(arrays(sc), sc.cameras[0], dict(sh_degree=0), key_capacity=16)
+    vt = torch.tensor(vis.view(np.int32), device="cuda"); ct = torch.tensor(cs, device="cuda")
+    mask_t = torch.empty(n, dtype=torch.uint8, device="cuda"); remap_t = torch.empty(n, dtype=torch.int32, device="cuda")
+    n_out = torch.zeros(1, dtype=torch.int32, device="cuda")
+    pws = torch.empty(B.ocgs_prune_workspace_bytes(n), dtype=torch.uint8, device="cuda")
+    for tau, omin in ((0.0, 0.0), (0.25, 0.1)):
+        cfg = B.ocgs_default_config(sh_degree=0, tau_contrib=tau, min_opacity=omin)
+        B.ocgs_prune_stats(g.surfels, vt, ct, cfg, mask_t, remap_t, None, n_out, 0, pws)
+        torch.cuda.synchronize()
+        po = orc.prune(vis, cs, sc.opacity, tau=tau, min_opacity=omin)
+        assert np.array_equal(mask_t.cpu().numpy(), po["prune_mask"])
+        assert np.array_equal(remap_t.cpu().numpy(), po["remap"]) and int(n_out.item()) == po["n_out"]
+
+
+def test_config3_full_size_sampled_windows():
+    """BASELINE.json configs[2] at full size, in bench.py's launch configuration: integer outputs compared in full,
+    images and gradients on sampled windows the oracle can compute."""
+    import oracle as orc
+    sc = sg.make_scene("config3")
+    view = 0
+    P = arrays(sc)
+    camn = sc.cameras[view]
+    m = sc.mask(view)
+    cfg_kw = dict(sh_degree=3)
+    cam = orc.camera_from(camn)
+    cfg = orc.default_config(sh_degree=3)
+    pre = orc.preprocess(*P, cam, cfg)
+    srt = orc.bin_sort(pre, cam, cfg)
+    g = GpuView(P, camn, cfg_kw, key_capacity=48 * sc.n)
+    gp = g.preprocess()
+    vis = pre["visible"] == 1
+    assert np.array_equal(gp["tiles"], pre["tiles_touched"]) and np.array_equal(gp["depth_bits"], pre["depth_bits"])
+    assert np.array_equal(gp["rect"][vis], pre["rect"][vis])
+    gs = g.bin_sort()
+    assert gs["K"] == srt["K"] and np.array_equal(gs["ids"], srt["ids"]) and np.array_equal(gs["ranges"], srt["ranges"])
+    gf = g.render_fwd(mask=m)
+    H, W = camn.height, camn.width
+    windows = [(0, 0, 48, 48), (784, 592, 832, 640), (W - 48, H - 48, W, H), (400, 900, 448, 948)]
+    gC = np.zeros((3, H, W)); gA = np.zeros((H, W)); gD = np.zeros((H, W)); gN = np.zeros((3, H, W))
+    mm = m.copy()
+    rng = np.random.default_rng(11)
+    frag_total = 0
+    for (x0, y0, x1, y1) in windows:
+        fw = orc.render_fwd(pre, srt, sc.opacity, cam, cfg, mask=m, window=(x0, y0, x1, y1))
+        ok = fw["fragile"][y0:y1, x0:x1] == 0
+        frag_total += int((~ok).sum())
+        for k in ("color", "alpha", "depth", "normal"):
+            a, b = gf[k][..., y0:y1, x0:x1], fw[k][..., y0:y1, x0:x1]
+            scale = np.maximum(1.0, np.abs(b)) if k == "depth" else 1.0
+            assert ((np.abs(a - b) / scale) * ok).max() <= 1e-4, (k, (x0, y0))
+        assert np.array_equal(gf["n_contrib"][y0:y1, x0:x1][ok], fw["n_contrib"][y0:y1, x0:x1][ok])
+        okf = ok.astype(np.float64)
+        gC[:, y0:y1, x0:x1] = rng.normal(size=(3, y1 - y0, x1 - x0)) * okf
+        gA[y0:y1, x0:x1] = rng.normal(size=ok.shape) * okf
+        gD[y0:y1, x0:x1] = rng.normal(size=ok.shape) * okf
+        gN[:, y0:y1, x0:x1] = rng.normal(size=(3, y1 - y0, x1 - x0)) * okf
+    assert frag_total <= 0.01 * 4 * 48 * 48
+    # gradients: upstream non-zero only inside the windows, so the oracle only has to walk those pixels
+    cfg0 = orc.default_config(sh_degree=3, gamma_bg=0.0)
+    g.cfg.gamma_bg = 0.0
+    gg = g.render_bwd(gC=gC, gA=gA, gD=gD, gN=gN, mask=mm)
+    og = {k: np.zeros_like(v, dtype=np.float64) for k, v in gg.items()}
+    og["_d_opacity_abs"] = np.zeros(sc.n)
+    for w in windows:
+        part = orc.render_bwd(*P, pre, srt, cam, cfg0, mask=mm, gC=gC.astype(np.float32), gA=gA.astype(np.float32),
+                              gD=gD.astype(np.float32), gN=gN.astype(np.float32), window=w)
+        for k in og:
+            og[k] += part[k]
+    check_grads(gg, og)
