@@ -81,15 +81,15 @@ typedef struct {
   size_t rect;          /* u16 [N,4]  by id: pixel rect ix0,iy0,ix1,iy1 inclusive; undefined when tiles == 0 */
   size_t tiles;         /* u32 [N]    by id: tiles touched, 0 = culled */
   size_t clamp;         /* u8  [N]    by id: bit c set when colour channel c was clamped at 0 */
-  size_t rec_id;        /* f32 [N,20] by id: raster record */
+  size_t rec_id;        /* f32 [N,24] by id: raster record */
   size_t id_to_rank;    /* u32 [N]    by id: rank, 0xFFFFFFFF when culled */
   size_t rank_to_id;    /* u32 [N]    by rank (first n_vis entries) */
-  size_t rec;           /* f32 [N,20] by rank */
+  size_t rec;           /* f32 [N,24] by rank */
   size_t offsets;       /* u32 [N+1]  by rank: exclusive scan of tiles touched */
   size_t tile_keys;     /* u32 [key_capacity] tile id of each sorted list entry */
   size_t tile_vals;     /* u32 [key_capacity] rank of each sorted list entry */
   size_t ranges;        /* u32 [n_tiles,2] [start,end) of each tile's list */
-  size_t grad_rec;      /* f32 [N,20] by rank: backward accumulators */
+  size_t grad_rec;      /* f32 [N,24] by rank: backward accumulators (20 used) */
   size_t loss_partial;  /* f32 [n_tiles] */
   size_t final_T;       /* f32 [H,W] transmittance left after the forward pass (exact, not 1 - alpha) */
   size_t scratch;       /* sort ping-pong buffers, histograms, scan partials */

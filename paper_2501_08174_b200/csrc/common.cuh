@@ -8,21 +8,23 @@
 namespace ocgs {
 
 constexpr int kTile = 16;
-constexpr int kRec = 20;  // floats per raster record (80 B = 5 x float4)
-// record layout: the homography M in a form centred on the projected centre c = c2d
-//   k = (x-cx)*M2 - A0,  l = (y-cy)*M2 - A1   with A0 = M0 - cx*M2, A1 = M1 - cy*M2 (third components are the exact
-//   division residuals r0, r1), so forming k, l has no large-number cancellation.
+constexpr int kRec = 24;  // floats per raster record (96 B = 6 x float4)
+// Record layout.  With c = c2d the projected centre, A0 = M0 - cx*M2, A1 = M1 - cy*M2 (third
+// components are the exact division residuals), the pixel ray (x, y) meets the surfel plane at (u,v) = (qx,qy)/qz with
+//   q = (dx*M2 - A0) x (dy*M2 - A1) = R - dx*P - dy*Q,   dx = x - cx, dy = y - cy,
+//   P = M2 x A1,  Q = A0 x M2,  R = A0 x A1,  and the hit depth is z = M2.(u,v,1) = D0/qz with D0 = M2.R
+// (M2.P = M2.Q = 0).  P, Q, R, D0 are formed in fp64 from the fp32 M and rounded once.
+//   f4[0] = (Px, Py, Pz, Qx)  f4[1] = (Qy, Qz, Rx, Ry)  f4[2] = (Rz, D0, cx, cy)
+//   f4[3] = (rho_cut, z_j, bits(ix0 | iy0<<16), bits(ix1 | iy1<<16))  f4[4] = (opacity, r, g, b)  f4[5] = (nx, ny, nz, 0)
 enum RecField {
-  R_M20 = 0, R_M21, R_M22, R_A00, R_A01, R_A10, R_A11, R_R0, R_R1, R_CX, R_CY, R_RHOCUT, R_OPA, R_COLR, R_COLG, R_COLB,
-  R_NX, R_NY, R_NZ, R_PAD
+  R_PX = 0, R_PY, R_PZ, R_QX, R_QY, R_QZ, R_RX, R_RY, R_RZ, R_D0, R_CX, R_CY, R_RHOCUT, R_ZJ, R_RECT0, R_RECT1, R_OPA, R_COLR,
+  R_COLG, R_COLB, R_NX, R_NY, R_NZ, R_PAD
 };
-// gradient accumulator layout in ws.grad_rec (by rank), 18 used
+// gradient accumulator layout in ws.grad_rec (by rank, stride kRec): 16 "main" fields reduced by the transposing
+// butterfly, 4 "extra" fields that are non-zero only with a depth gradient or when the filter term wins
 enum GradField {
-  G_M20 = 0, G_M21, G_M22,   // sum (x-cx) gk + (y-cy) gl + (u,v,1) gz
-  G_K0, G_K1, G_K2,          // sum gk   (dL/dM0 = -gk)
-  G_L0, G_L1, G_L2,          // sum gl   (dL/dM1 = -gl)
-  G_CX, G_CY,                // filter term: dL/dc2d
-  G_OPA, G_COLR, G_COLG, G_COLB, G_NX, G_NY, G_NZ, G_PAD0, G_PAD1
+  G_PX = 0, G_PY, G_PZ, G_QX, G_QY, G_QZ, G_RX, G_RY, G_RZ, G_OPA, G_COLR, G_COLG, G_COLB, G_NX, G_NY, G_NZ,
+  G_D0, G_ZJ, G_CX, G_CY, G_COUNT
 };
 
 constexpr int kSortItems = 16;                       // keys per thread in a radix pass

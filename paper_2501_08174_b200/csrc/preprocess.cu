@@ -65,16 +65,24 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
 #pragma unroll
       for (int c = 0; c < 3; ++c)
         if (col[c] < 0.0f) { col[c] = 0.0f; cl |= (uint8_t)(1u << c); }
-      // centred record
+      // centred record (common.cuh): P, Q, R, D0 in fp64 from the fp32 M, rounded once
       const float* M = pr.M;
-      const float A00 = __fmaf_rn(-pr.cx, M[6], M[0]), A01 = __fmaf_rn(-pr.cx, M[7], M[1]), r0 = __fmaf_rn(-pr.cx, M[8], M[2]);
-      const float A10 = __fmaf_rn(-pr.cy, M[6], M[3]), A11 = __fmaf_rn(-pr.cy, M[7], M[4]), r1 = __fmaf_rn(-pr.cy, M[8], M[5]);
-      float4* out = rec_id + (size_t)j * 5;
-      out[0] = make_float4(M[6], M[7], M[8], A00);
-      out[1] = make_float4(A01, A10, A11, r0);
-      out[2] = make_float4(r1, pr.cx, pr.cy, pr.rho_cut);
-      out[3] = make_float4(o, col[0], col[1], col[2]);
-      out[4] = make_float4(nx, ny, nz, 0.0f);
+      const double cxd = pr.cx, cyd = pr.cy;
+      const double m2[3] = {M[6], M[7], M[8]};
+      const double a0[3] = {M[0] - cxd * m2[0], M[1] - cxd * m2[1], M[2] - cxd * m2[2]};
+      const double a1[3] = {M[3] - cyd * m2[0], M[4] - cyd * m2[1], M[5] - cyd * m2[2]};
+      const double P[3] = {m2[1] * a1[2] - m2[2] * a1[1], m2[2] * a1[0] - m2[0] * a1[2], m2[0] * a1[1] - m2[1] * a1[0]};
+      const double Q[3] = {a0[1] * m2[2] - a0[2] * m2[1], a0[2] * m2[0] - a0[0] * m2[2], a0[0] * m2[1] - a0[1] * m2[0]};
+      const double R[3] = {a0[1] * a1[2] - a0[2] * a1[1], a0[2] * a1[0] - a0[0] * a1[2], a0[0] * a1[1] - a0[1] * a1[0]};
+      const double D0 = m2[0] * R[0] + m2[1] * R[1] + m2[2] * R[2];
+      float4* out = rec_id + (size_t)j * 6;
+      out[0] = make_float4((float)P[0], (float)P[1], (float)P[2], (float)Q[0]);
+      out[1] = make_float4((float)Q[1], (float)Q[2], (float)R[0], (float)R[1]);
+      out[2] = make_float4((float)R[2], (float)D0, pr.cx, pr.cy);
+      out[3] = make_float4(pr.rho_cut, M[8], __uint_as_float((uint32_t)pr.ix0 | ((uint32_t)pr.iy0 << 16)),
+                           __uint_as_float((uint32_t)pr.ix1 | ((uint32_t)pr.iy1 << 16)));
+      out[4] = make_float4(o, col[0], col[1], col[2]);
+      out[5] = make_float4(nx, ny, nz, 0.0f);
     }
     tiles[j] = nt;
     clamp_bits[j] = cl;

@@ -9,10 +9,10 @@
 namespace ocgs {
 
 constexpr int kBwdBatch = 64;
-constexpr int kNG = 18;
+constexpr int kNG = G_COUNT;  // 20 accumulated fields per list entry
 
-// sum of v[0..15] over the 32 lanes; afterwards v[0] of lane L holds the total of value index
-// 8*bit4(L) + 4*bit3(L) + 2*bit2(L) + bit1(L)
+// sum of v[0..15] over the 32 lanes (16 shuffles); afterwards v[0] of lane L holds the total of value index
+// 8*bit4(L) + 4*bit3(L) + 2*bit2(L) + bit1(L), i.e. index L >> 1
 __device__ __forceinline__ void warp_transpose_reduce16(float* v, int lane) {
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
@@ -40,17 +40,39 @@ __device__ __forceinline__ void warp_transpose_reduce16(float* v, int lane) {
   v[0] += __shfl_xor_sync(0xFFFFFFFFu, v[0], 1);
 }
 
-// order of the 16 transposed values -> GradField
-__constant__ int kFieldOf16[16] = {G_M20, G_M21, G_M22, G_K0, G_K1, G_K2, G_L0, G_L1, G_L2, G_OPA, G_COLR, G_COLG, G_COLB, G_NX, G_NY, G_NZ};
+// sum of e[0..3] over the 32 lanes (6 shuffles); afterwards e[0] of lane L holds the total of value index 2*bit4(L) + bit3(L)
+__device__ __forceinline__ void warp_transpose_reduce4(float* e, int lane) {
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    const bool up = lane & 16;
+    const float send = up ? e[i] : e[i + 2], keep = up ? e[i + 2] : e[i];
+    e[i] = keep + __shfl_xor_sync(0xFFFFFFFFu, send, 16);
+  }
+  {
+    const bool up = lane & 8;
+    const float send = up ? e[0] : e[1], keep = up ? e[1] : e[0];
+    e[0] = keep + __shfl_xor_sync(0xFFFFFFFFu, send, 8);
+  }
+  e[0] += __shfl_xor_sync(0xFFFFFFFFu, e[0], 4);
+  e[0] += __shfl_xor_sync(0xFFFFFFFFu, e[0], 2);
+  e[0] += __shfl_xor_sync(0xFFFFFFFFu, e[0], 1);
+}
 
-__global__ void __launch_bounds__(256) render_bwd_kernel(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
-                                                         const float4* __restrict__ rec, const uint8_t* __restrict__ mask,
-                                                         const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
-                                                         const float* __restrict__ gC, const float* __restrict__ gA,
-                                                         const float* __restrict__ gD, const float* __restrict__ gN, int W, int H,
-                                                         int tiles_x, ocgs_config cfg, float gamma_over_hw, float* __restrict__ grad_rec) {
-  __shared__ float4 s_rec[kBwdBatch * 5];
+__device__ __forceinline__ uint32_t strip_mask_bwd(const float4 r3, int tile_y0) {
+  const int iy0 = (int)(__float_as_uint(r3.z) >> 16), iy1 = (int)(__float_as_uint(r3.w) >> 16);
+  const int lo = max(iy0 - tile_y0, 0) >> 1, hi = min(iy1 - tile_y0, 15) >> 1;
+  return hi < lo ? 0u : ((2u << hi) - 1u) & ~((1u << lo) - 1u);
+}
+
+__global__ void __launch_bounds__(256, 3) render_bwd_kernel(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
+                                                            const float4* __restrict__ rec, const uint8_t* __restrict__ mask,
+                                                            const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
+                                                            const float* __restrict__ gC, const float* __restrict__ gA,
+                                                            const float* __restrict__ gD, const float* __restrict__ gN, int W, int H,
+                                                            int tiles_x, ocgs_config cfg, float gamma_over_hw, float* __restrict__ grad_rec) {
+  __shared__ float4 s_rec[kBwdBatch * 6];
   __shared__ uint32_t s_rank[kBwdBatch];
+  __shared__ uint8_t s_mask[kBwdBatch];
   __shared__ float s_acc[kBwdBatch * kNG];
   __shared__ uint32_t s_max[8];
 
@@ -63,6 +85,7 @@ __global__ void __launch_bounds__(256) render_bwd_kernel(const uint32_t* __restr
   const uint32_t start = ranges[2 * tile];
   const float inv_sigma2 = 1.0f / cfg.filter_sigma2;
   const int lane = threadIdx.x & 31;
+  const uint32_t wbit = 1u << (threadIdx.x >> 5);
   const size_t HW = (size_t)W * H, p = inside ? (size_t)iy * W + ix : 0;
 
   uint32_t last = 0;
@@ -88,6 +111,7 @@ __global__ void __launch_bounds__(256) render_bwd_kernel(const uint32_t* __restr
   if (mx == 0) return;
 
   float T = Tfin;
+  const float gaT = ga * Tfin;
   float SC0 = Tfin * cfg.bg[0], SC1 = Tfin * cfg.bg[1], SC2 = Tfin * cfg.bg[2], SD = 0.f, SN0 = 0.f, SN1 = 0.f, SN2 = 0.f;
 
   const int nbatch = (int)((mx + kBwdBatch - 1) / kBwdBatch);
@@ -95,87 +119,85 @@ __global__ void __launch_bounds__(256) render_bwd_kernel(const uint32_t* __restr
     const uint32_t b0 = (uint32_t)bi * kBwdBatch;
     const int cnt = (int)min((uint32_t)kBwdBatch, mx - b0);
     __syncthreads();  // previous batch fully flushed before s_rank / s_acc are reused
-    if ((int)threadIdx.x < cnt) s_rank[threadIdx.x] = list[start + b0 + threadIdx.x];
+    if ((int)threadIdx.x < cnt) {
+      const uint32_t rk = list[start + b0 + threadIdx.x];
+      s_rank[threadIdx.x] = rk;
+      s_mask[threadIdx.x] = (uint8_t)strip_mask_bwd(__ldg(rec + (size_t)rk * 6 + 3), ty * kTile);
+    }
     for (int i = threadIdx.x; i < cnt * kNG; i += 256) s_acc[i] = 0.f;
     __syncthreads();
-    for (int i = threadIdx.x; i < cnt * 5; i += 256) {
-      const int e = i / 5, part = i - 5 * e;
-      s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 5 + part);
+    for (int i = threadIdx.x; i < cnt * 6; i += 256) {
+      const int e = i / 6, part = i - 6 * e;
+      s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
     }
     __syncthreads();
     for (int j = cnt - 1; j >= 0; --j) {
+      if (!(s_mask[j] & wbit)) continue;
       const uint32_t idx = b0 + (uint32_t)j;
       const bool act = inside && idx < last;
       if (!__any_sync(0xFFFFFFFFu, act)) continue;
-      const float4 r0 = s_rec[5 * j], r1 = s_rec[5 * j + 1], r2 = s_rec[5 * j + 2];
+      const float4 r0 = s_rec[6 * j], r1 = s_rec[6 * j + 1], r2 = s_rec[6 * j + 2], r3 = s_rec[6 * j + 3];
       float v[16];
 #pragma unroll
       for (int i = 0; i < 16; ++i) v[i] = 0.f;
-      float gcx = 0.f, gcy = 0.f;
+      float ex[4] = {0.f, 0.f, 0.f, 0.f};  // gD0, gzj, gcx, gcy
       bool contributes = false;
       if (act) {
-        const float dx = px - r2.y, dy = py - r2.z;
-        const float k0 = fmaf(dx, r0.x, -r0.w), k1 = fmaf(dx, r0.y, -r1.x), k2 = fmaf(dx, r0.z, -r1.w);
-        const float l0 = fmaf(dy, r0.x, -r1.y), l1 = fmaf(dy, r0.y, -r1.z), l2 = fmaf(dy, r0.z, -r2.x);
-        const float qx = fmaf(k1, l2, -k2 * l1), qy = fmaf(k2, l0, -k0 * l2), qz = fmaf(k0, l1, -k1 * l0);
+        const float dx = px - r2.z, dy = py - r2.w;
+        const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
+        const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
+        const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
         if (qz != 0.0f) {
-          const float inv = __frcp_rn(qz);
+          const float inv = __fdividef(1.0f, qz);
           const float u = qx * inv, vv = qy * inv;
           const float rho3 = fmaf(u, u, vv * vv);
           const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
           const bool surf = rho3 <= rho2;
           const float rho = surf ? rho3 : rho2;
-          const float z = surf ? fmaf(r0.x, u, fmaf(r0.y, vv, r0.z)) : r0.z;
-          if (!(z < cfg.near_z) && !(rho > r2.w)) {
+          const float z = surf ? r2.y * inv : r3.y;
+          if (!(z < cfg.near_z) && !(rho > r3.x)) {
             contributes = true;
-            const float4 r3 = s_rec[5 * j + 3], r4 = s_rec[5 * j + 4];
+            const float4 r4 = s_rec[6 * j + 4], r5 = s_rec[6 * j + 5];
             const float G = __expf(-0.5f * rho);
-            const float araw = r3.x * G;
+            const float araw = r4.x * G;
             const bool capped = araw > cfg.alpha_max;
             const float a = capped ? cfg.alpha_max : araw;
-            const float inv1ma = __frcp_rn(1.0f - a);
+            const float inv1ma = __fdividef(1.0f, 1.0f - a);
             T *= inv1ma;  // T_i = T_{i+1} / (1 - alpha_i)
             const float w = a * T;
-            float galpha = ga * Tfin * inv1ma + gd * (z * T - SD * inv1ma);
-            galpha += gc0 * (r3.y * T - SC0 * inv1ma) + gc1 * (r3.z * T - SC1 * inv1ma) + gc2 * (r3.w * T - SC2 * inv1ma);
-            galpha += gn0 * (r4.x * T - SN0 * inv1ma) + gn1 * (r4.y * T - SN1 * inv1ma) + gn2 * (r4.z * T - SN2 * inv1ma);
-            SC0 = fmaf(w, r3.y, SC0); SC1 = fmaf(w, r3.z, SC1); SC2 = fmaf(w, r3.w, SC2);
+            float galpha = gaT * inv1ma + gd * (z * T - SD * inv1ma);
+            galpha += gc0 * (r4.y * T - SC0 * inv1ma) + gc1 * (r4.z * T - SC1 * inv1ma) + gc2 * (r4.w * T - SC2 * inv1ma);
+            galpha += gn0 * (r5.x * T - SN0 * inv1ma) + gn1 * (r5.y * T - SN1 * inv1ma) + gn2 * (r5.z * T - SN2 * inv1ma);
+            SC0 = fmaf(w, r4.y, SC0); SC1 = fmaf(w, r4.z, SC1); SC2 = fmaf(w, r4.w, SC2);
             SD = fmaf(w, z, SD);
-            SN0 = fmaf(w, r4.x, SN0); SN1 = fmaf(w, r4.y, SN1); SN2 = fmaf(w, r4.z, SN2);
+            SN0 = fmaf(w, r5.x, SN0); SN1 = fmaf(w, r5.y, SN1); SN2 = fmaf(w, r5.z, SN2);
             v[10] = w * gc0; v[11] = w * gc1; v[12] = w * gc2;
             v[13] = w * gn0; v[14] = w * gn1; v[15] = w * gn2;
             const float gz = w * gd;
             float grho = 0.f;
-            if (!capped) { v[9] = G * galpha; grho = -0.5f * G * r3.x * galpha; }  // S12: zero through the cap
+            if (!capped) { v[9] = G * galpha; grho = -0.5f * G * r4.x * galpha; }  // S12: zero through the cap
             if (surf) {
-              const float gu = fmaf(2.0f * u, grho, r0.x * gz), gv = fmaf(2.0f * vv, grho, r0.y * gz);
-              const float gq0 = gu * inv, gq1 = gv * inv, gq2 = -(gu * u + gv * vv) * inv;
-              // q = k x l: gk = l x gq, gl = gq x k
-              const float gk0 = l1 * gq2 - l2 * gq1, gk1 = l2 * gq0 - l0 * gq2, gk2 = l0 * gq1 - l1 * gq0;
-              const float gl0 = gq1 * k2 - gq2 * k1, gl1 = gq2 * k0 - gq0 * k2, gl2 = gq0 * k1 - gq1 * k0;
-              v[0] = fmaf(dx, gk0, fmaf(dy, gl0, u * gz));
-              v[1] = fmaf(dx, gk1, fmaf(dy, gl1, vv * gz));
-              v[2] = fmaf(dx, gk2, fmaf(dy, gl2, gz));
-              v[3] = gk0; v[4] = gk1; v[5] = gk2;
-              v[6] = gl0; v[7] = gl1; v[8] = gl2;
+              // rho = u^2+v^2, z = D0/qz, (u,v) = (qx,qy)/qz, q = R - dx P - dy Q
+              const float gu = 2.0f * u * grho, gv = 2.0f * vv * grho;
+              const float gq0 = gu * inv, gq1 = gv * inv, gq2 = -(fmaf(gu, u, fmaf(gv, vv, gz * z))) * inv;
+              v[0] = -dx * gq0; v[1] = -dx * gq1; v[2] = -dx * gq2;
+              v[3] = -dy * gq0; v[4] = -dy * gq1; v[5] = -dy * gq2;
+              v[6] = gq0; v[7] = gq1; v[8] = gq2;
+              ex[0] = gz * inv;
             } else {
-              gcx = -2.0f * dx * inv_sigma2 * grho;
-              gcy = -2.0f * dy * inv_sigma2 * grho;
-              v[2] = gz;  // z = z_j = M22
+              ex[1] = gz;  // z = z_j
+              ex[2] = -2.0f * dx * inv_sigma2 * grho;
+              ex[3] = -2.0f * dy * inv_sigma2 * grho;
             }
           }
         }
       }
       if (!__any_sync(0xFFFFFFFFu, contributes)) continue;
       warp_transpose_reduce16(v, lane);
-      if ((lane & 1) == 0) atomicAdd(&s_acc[j * kNG + kFieldOf16[lane >> 1]], v[0]);
-      if (__any_sync(0xFFFFFFFFu, gcx != 0.f || gcy != 0.f)) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-          gcx += __shfl_xor_sync(0xFFFFFFFFu, gcx, o);
-          gcy += __shfl_xor_sync(0xFFFFFFFFu, gcy, o);
-        }
-        if (lane == 0) { atomicAdd(&s_acc[j * kNG + G_CX], gcx); atomicAdd(&s_acc[j * kNG + G_CY], gcy); }
+      if ((lane & 1) == 0) atomicAdd(&s_acc[j * kNG + (lane >> 1)], v[0]);
+      if (__any_sync(0xFFFFFFFFu, (ex[0] != 0.f) | (ex[1] != 0.f) | (ex[2] != 0.f) | (ex[3] != 0.f))) {
+        warp_transpose_reduce4(ex, lane);
+        if ((lane & 7) == 0) atomicAdd(&s_acc[j * kNG + 16 + (lane >> 3)], ex[0]);
       }
     }
     __syncthreads();
@@ -224,17 +246,40 @@ __global__ void __launch_bounds__(128) project_bwd_kernel(const float* __restric
   const float4 q = quat[j];
   Projected pr;
   project_surfel(p, s.x, s.y, q, opacity[j], cam, cfg, pr);
-  const float M22 = pr.M[8];
+  const float* M = pr.M;
+  const float M22 = M[8];
+  // forward quantities of the record (common.cuh): A0, A1, R
+  const float m2[3] = {M[6], M[7], M[8]};
+  const float a0[3] = {fmaf(-pr.cx, m2[0], M[0]), fmaf(-pr.cx, m2[1], M[1]), fmaf(-pr.cx, m2[2], M[2])};
+  const float a1[3] = {fmaf(-pr.cy, m2[0], M[3]), fmaf(-pr.cy, m2[1], M[4]), fmaf(-pr.cy, m2[2], M[5])};
+  const float R[3] = {a0[1] * a1[2] - a0[2] * a1[1], a0[2] * a1[0] - a0[0] * a1[2], a0[0] * a1[1] - a0[1] * a1[0]};
+  const float gP[3] = {g[G_PX], g[G_PY], g[G_PZ]}, gQ[3] = {g[G_QX], g[G_QY], g[G_QZ]};
+  const float gD0 = g[G_D0];
+  const float gR[3] = {g[G_RX] + gD0 * m2[0], g[G_RY] + gD0 * m2[1], g[G_RZ] + gD0 * m2[2]};  // D0 = M2 . R
+  // c = a x b: ga = b x gc, gb = gc x a
+  auto cross = [](const float* a, const float* b, float* o) {
+    o[0] = a[1] * b[2] - a[2] * b[1]; o[1] = a[2] * b[0] - a[0] * b[2]; o[2] = a[0] * b[1] - a[1] * b[0];
+  };
+  float t1[3], t2[3], gA0[3], gA1[3], gM2c[3];
+  cross(m2, gQ, t1); cross(a1, gR, t2);      // Q = A0 x M2, R = A0 x A1
+  for (int i = 0; i < 3; ++i) gA0[i] = t1[i] + t2[i];
+  cross(gP, m2, t1); cross(gR, a0, t2);      // P = M2 x A1
+  for (int i = 0; i < 3; ++i) gA1[i] = t1[i] + t2[i];
+  cross(a1, gP, t1); cross(gQ, a0, t2);      // dL/dM2 through P, Q and D0 (the -c*gA parts are folded in below)
+  for (int i = 0; i < 3; ++i) gM2c[i] = t1[i] + t2[i] + gD0 * R[i];
+  gM2c[2] += g[G_ZJ];                        // z_j = M22
+  // A0 = M0 - cx M2, A1 = M1 - cy M2 (c constant: the intersection does not depend on it) and c2d = (M02, M12)/M22
   const float ex = pr.cx - cam.ox, ey = pr.cy - cam.oy;
   const float f0 = g[G_CX] / M22, f1 = g[G_CY] / M22;
-  const float m0[3] = {-g[G_K0], -g[G_K1], -g[G_K2] + f0};  // dL/dM0
-  const float m1[3] = {-g[G_L0], -g[G_L1], -g[G_L2] + f1};  // dL/dM1
+  const float m0[3] = {gA0[0], gA0[1], gA0[2] + f0};  // dL/dM0
+  const float m1[3] = {gA1[0], gA1[1], gA1[2] + f1};  // dL/dM1
   float gcol[3][3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     gcol[i][0] = cam.fx * m0[i];
     gcol[i][1] = cam.fy * m1[i];
-    gcol[i][2] = g[G_M20 + i] - ex * m0[i] - ey * m1[i];  // = ox m0 + oy m1 + dL/dM2 with dL/dM2 = G2 + cx Gk + cy Gl - ...
+    // ox m0 + oy m1 + dL/dM2 with dL/dM2 = gM2c - cx gA0 - cy gA1 (- (f0 cx + f1 cy) on i = 2), combined to avoid cancellation
+    gcol[i][2] = gM2c[i] - ex * m0[i] - ey * m1[i];
   }
   if (d_center2d) d_center2d[j] = make_float2(M22 * m0[2], M22 * m1[2]);
   const float* V = cam.V;

@@ -8,24 +8,32 @@ namespace ocgs {
 constexpr int kFwdBatch = 128;                 // list entries staged per batch
 constexpr float kContribFix = 134217728.0f;    // 2^27: alpha*T in fixed point for the warp-wide REDUX sum
 
-// O4 in the centred form: k = dx*M2 - A0, l = dy*M2 - A1, (u,v) = (qx,qy)/qz with q = k x l.
-__device__ __forceinline__ bool eval_pair(const float4 r0, const float4 r1, const float4 r2, float px, float py, float near_z,
-                                          float inv_sigma2, float& rho, float& z, float& u, float& v, bool& surf) {
-  const float dx = px - r2.y, dy = py - r2.z;
-  const float k0 = fmaf(dx, r0.x, -r0.w), k1 = fmaf(dx, r0.y, -r1.x), k2 = fmaf(dx, r0.z, -r1.w);
-  const float l0 = fmaf(dy, r0.x, -r1.y), l1 = fmaf(dy, r0.y, -r1.z), l2 = fmaf(dy, r0.z, -r2.x);
-  const float qx = fmaf(k1, l2, -k2 * l1), qy = fmaf(k2, l0, -k0 * l2), qz = fmaf(k0, l1, -k1 * l0);
+// O4 from the record (common.cuh): q = R - dx*P - dy*Q, (u,v) = (qx,qy)/qz, hit depth z = D0/qz.
+__device__ __forceinline__ bool eval_pair(const float4 r0, const float4 r1, const float4 r2, const float4 r3, float px, float py,
+                                          float near_z, float inv_sigma2, float& rho, float& z) {
+  const float dx = px - r2.z, dy = py - r2.w;
+  const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
+  const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
+  const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
   if (qz == 0.0f) return false;
-  const float inv = __frcp_rn(qz);
-  u = qx * inv; v = qy * inv;
+  const float inv = __fdividef(1.0f, qz);
+  const float u = qx * inv, v = qy * inv;
   const float rho3 = fmaf(u, u, v * v);
   const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
-  surf = rho3 <= rho2;
+  const bool surf = rho3 <= rho2;
   rho = surf ? rho3 : rho2;
-  z = surf ? fmaf(r0.x, u, fmaf(r0.y, v, r0.z)) : r0.z;
+  z = surf ? r2.y * inv : r3.y;
   if (z < near_z) return false;
-  if (rho > r2.w) return false;
+  if (rho > r3.x) return false;
   return true;
+}
+
+// bit w of the result: warp w's 16x2 pixel strip of tile row ty intersects the surfel's pixel rect (rows only: the
+// rect always overlaps the tile's columns, it was binned to this tile)
+__device__ __forceinline__ uint32_t strip_mask(const float4 r3, int tile_y0) {
+  const int iy0 = (int)(__float_as_uint(r3.z) >> 16), iy1 = (int)(__float_as_uint(r3.w) >> 16);
+  const int lo = max(iy0 - tile_y0, 0) >> 1, hi = min(iy1 - tile_y0, 15) >> 1;  // strips lo..hi
+  return hi < lo ? 0u : ((2u << hi) - 1u) & ~((1u << lo) - 1u);
 }
 
 template <bool kStats>
@@ -36,8 +44,9 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
                                                          float* __restrict__ depth, float* __restrict__ normal,
                                                          uint32_t* __restrict__ n_contrib, float* __restrict__ final_T, float* __restrict__ loss_partial,
                                                          uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum) {
-  __shared__ float4 s_rec[kFwdBatch * 5];
+  __shared__ float4 s_rec[kFwdBatch * 6];
   __shared__ uint32_t s_rank[kFwdBatch];
+  __shared__ uint8_t s_mask[kFwdBatch];
   __shared__ uint32_t s_cnt[kStats ? kFwdBatch : 1];
   __shared__ float s_sum[kStats ? kFwdBatch : 1];
   __shared__ float s_red[8];
@@ -51,6 +60,7 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
   const uint32_t start = ranges[2 * tile], end = ranges[2 * tile + 1];
   const float inv_sigma2 = 1.0f / cfg.filter_sigma2;
   const int lane = threadIdx.x & 31;
+  const uint32_t wbit = 1u << (threadIdx.x >> 5);
 
   float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f;
   uint32_t last = 0;
@@ -59,32 +69,36 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
   for (uint32_t b0 = start; b0 < end; b0 += kFwdBatch) {
     const int cnt = (int)min((uint32_t)kFwdBatch, end - b0);
     if (__syncthreads_and(done)) break;
-    if ((int)threadIdx.x < cnt) s_rank[threadIdx.x] = list[b0 + threadIdx.x];
+    if ((int)threadIdx.x < cnt) {
+      const uint32_t rk = list[b0 + threadIdx.x];
+      s_rank[threadIdx.x] = rk;
+      s_mask[threadIdx.x] = (uint8_t)strip_mask(__ldg(rec + (size_t)rk * 6 + 3), ty * kTile);
+    }
     if (kStats && threadIdx.x < kFwdBatch) { s_cnt[threadIdx.x] = 0; s_sum[threadIdx.x] = 0.f; }
     __syncthreads();
-    for (int i = threadIdx.x; i < cnt * 5; i += 256) {
-      const int e = i / 5, part = i - 5 * e;
-      s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 5 + part);
+    for (int i = threadIdx.x; i < cnt * 6; i += 256) {
+      const int e = i / 6, part = i - 6 * e;
+      s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
     }
     __syncthreads();
     for (int j = 0; j < cnt; ++j) {
+      if (!(s_mask[j] & wbit)) continue;  // the surfel's rect misses this warp's strip
       if (__all_sync(0xFFFFFFFFu, done)) break;
-      const float4 r0 = s_rec[5 * j], r1 = s_rec[5 * j + 1], r2 = s_rec[5 * j + 2];
-      float rho, z, u, v;
-      bool surf;
+      const float4 r0 = s_rec[6 * j], r1 = s_rec[6 * j + 1], r2 = s_rec[6 * j + 2], r3 = s_rec[6 * j + 3];
+      float rho, z;
       bool blend = false;
       float wgt = 0.f;
-      if (!done && eval_pair(r0, r1, r2, px, py, cfg.near_z, inv_sigma2, rho, z, u, v, surf)) {
-        const float4 r3 = s_rec[5 * j + 3], r4 = s_rec[5 * j + 4];
-        const float a = fminf(cfg.alpha_max, r3.x * __expf(-0.5f * rho));
+      if (!done && eval_pair(r0, r1, r2, r3, px, py, cfg.near_z, inv_sigma2, rho, z)) {
+        const float4 r4 = s_rec[6 * j + 4], r5 = s_rec[6 * j + 5];
+        const float a = fminf(cfg.alpha_max, r4.x * __expf(-0.5f * rho));
         const float Tn = T * (1.0f - a);
         if (Tn < cfg.t_min) {
           done = true;  // S11: stop before blending this pair
         } else {
           wgt = a * T;
-          C0 = fmaf(wgt, r3.y, C0); C1 = fmaf(wgt, r3.z, C1); C2 = fmaf(wgt, r3.w, C2);
+          C0 = fmaf(wgt, r4.y, C0); C1 = fmaf(wgt, r4.z, C1); C2 = fmaf(wgt, r4.w, C2);
           D = fmaf(wgt, z, D);
-          N0 = fmaf(wgt, r4.x, N0); N1 = fmaf(wgt, r4.y, N1); N2 = fmaf(wgt, r4.z, N2);
+          N0 = fmaf(wgt, r5.x, N0); N1 = fmaf(wgt, r5.y, N1); N2 = fmaf(wgt, r5.z, N2);
           T = Tn;
           last = (b0 - start) + j + 1;
           blend = true;

@@ -198,10 +198,10 @@ __global__ void __launch_bounds__(kScanBlock) reorder_kernel(const uint32_t* __r
     id_to_rank[id] = r;
     t = tiles[id];
     tcount[r] = t;
-    const float4* src = rec_id + (size_t)id * 5;
-    float4* dst = rec + (size_t)r * 5;
-    const float4 a = src[0], b = src[1], c = src[2], d = src[3], e = src[4];
-    dst[0] = a; dst[1] = b; dst[2] = c; dst[3] = d; dst[4] = e;
+    const float4* src = rec_id + (size_t)id * 6;
+    float4* dst = rec + (size_t)r * 6;
+    const float4 a = src[0], b = src[1], c = src[2], d = src[3], e = src[4], f = src[5];
+    dst[0] = a; dst[1] = b; dst[2] = c; dst[3] = d; dst[4] = e; dst[5] = f;
   }
   // block sum
   __shared__ uint32_t ws[32];

@@ -45,7 +45,7 @@ class GpuView:
         return dict(depth_bits=self.sec("depth_bits", torch.int32, n).view(np.uint32),
                     rect=self.sec("rect", torch.int16, 4 * n).view(np.uint16).reshape(n, 4).astype(np.int32),
                     tiles=self.sec("tiles", torch.int32, n).view(np.uint32), clamp=self.sec("clamp", torch.uint8, n),
-                    rec_id=self.sec("rec_id", torch.float32, 20 * n).reshape(n, 20))
+                    rec_id=self.sec("rec_id", torch.float32, 24 * n).reshape(n, 24))
 
     def bin_sort(self, want_ids=True):
         torch = self.torch
