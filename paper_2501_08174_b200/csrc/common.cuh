@@ -104,6 +104,13 @@ int launch_masked_l1(const float* color, const float* target, const uint8_t* mas
 int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t* valsB, const void* n_ptr, bool n_is_u64,
                      size_t n_max, int key_bits, uint32_t* hist, uint32_t* digit_total, bool* result_in_B, cudaStream_t st);
 
+#ifdef __CUDACC__
+// MUFU approximations (1-2 ulp, flush-to-zero): enough for the 1e-4 / 1e-3 tolerances, no denormal fix-up code
+__device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float ex2_approx(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+constexpr float kNegHalfLog2e = -0.72134752044448170f;  // exp(-rho/2) = 2^(rho * -0.5 log2 e)
+#endif
+
 __host__ __device__ inline size_t div_up(size_t a, size_t b) { return (a + b - 1) / b; }
 
 }  // namespace ocgs

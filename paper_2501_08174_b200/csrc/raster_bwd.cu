@@ -87,6 +87,7 @@ __global__ void __launch_bounds__(256, 3) render_bwd_kernel(const uint32_t* __re
   const int lane = threadIdx.x & 31;
   const uint32_t wbit = 1u << (threadIdx.x >> 5);
   const size_t HW = (size_t)W * H, p = inside ? (size_t)iy * W + ix : 0;
+  const float near_z = cfg.near_z, alpha_max = cfg.alpha_max;
 
   uint32_t last = 0;
   float Tfin = 1.0f, gc0 = 0.f, gc1 = 0.f, gc2 = 0.f, ga = 0.f, gd = 0.f, gn0 = 0.f, gn1 = 0.f, gn2 = 0.f;
@@ -131,68 +132,63 @@ __global__ void __launch_bounds__(256, 3) render_bwd_kernel(const uint32_t* __re
       s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
     }
     __syncthreads();
-    for (int j = cnt - 1; j >= 0; --j) {
+    const float4* sr = s_rec + 6 * (cnt - 1);
+    for (int j = cnt - 1; j >= 0; --j, sr -= 6) {
       if (!(s_mask[j] & wbit)) continue;
-      const uint32_t idx = b0 + (uint32_t)j;
-      const bool act = inside && idx < last;
+      const bool act = (b0 + (uint32_t)j) < last;  // last == 0 for pixels outside the image
       if (!__any_sync(0xFFFFFFFFu, act)) continue;
-      const float4 r0 = s_rec[6 * j], r1 = s_rec[6 * j + 1], r2 = s_rec[6 * j + 2], r3 = s_rec[6 * j + 3];
+      const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
+      const float dx = px - r2.z, dy = py - r2.w;
+      const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
+      const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
+      const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
+      const float inv = rcp_approx(qz);
+      const float u = qx * inv, vv = qy * inv;
+      const float rho3 = fmaf(u, u, vv * vv);
+      const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
+      const bool surf = rho3 <= rho2;
+      const float rho = surf ? rho3 : rho2;
+      const float z = surf ? r2.y * inv : r3.y;
+      const bool contributes = act && qz != 0.0f && !(z < near_z) && !(rho > r3.x);
+      if (!__any_sync(0xFFFFFFFFu, contributes)) continue;
       float v[16];
 #pragma unroll
       for (int i = 0; i < 16; ++i) v[i] = 0.f;
       float ex[4] = {0.f, 0.f, 0.f, 0.f};  // gD0, gzj, gcx, gcy
-      bool contributes = false;
-      if (act) {
-        const float dx = px - r2.z, dy = py - r2.w;
-        const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
-        const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
-        const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
-        if (qz != 0.0f) {
-          const float inv = __fdividef(1.0f, qz);
-          const float u = qx * inv, vv = qy * inv;
-          const float rho3 = fmaf(u, u, vv * vv);
-          const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
-          const bool surf = rho3 <= rho2;
-          const float rho = surf ? rho3 : rho2;
-          const float z = surf ? r2.y * inv : r3.y;
-          if (!(z < cfg.near_z) && !(rho > r3.x)) {
-            contributes = true;
-            const float4 r4 = s_rec[6 * j + 4], r5 = s_rec[6 * j + 5];
-            const float G = __expf(-0.5f * rho);
-            const float araw = r4.x * G;
-            const bool capped = araw > cfg.alpha_max;
-            const float a = capped ? cfg.alpha_max : araw;
-            const float inv1ma = __fdividef(1.0f, 1.0f - a);
-            T *= inv1ma;  // T_i = T_{i+1} / (1 - alpha_i)
-            const float w = a * T;
-            float galpha = gaT * inv1ma + gd * (z * T - SD * inv1ma);
-            galpha += gc0 * (r4.y * T - SC0 * inv1ma) + gc1 * (r4.z * T - SC1 * inv1ma) + gc2 * (r4.w * T - SC2 * inv1ma);
-            galpha += gn0 * (r5.x * T - SN0 * inv1ma) + gn1 * (r5.y * T - SN1 * inv1ma) + gn2 * (r5.z * T - SN2 * inv1ma);
-            SC0 = fmaf(w, r4.y, SC0); SC1 = fmaf(w, r4.z, SC1); SC2 = fmaf(w, r4.w, SC2);
-            SD = fmaf(w, z, SD);
-            SN0 = fmaf(w, r5.x, SN0); SN1 = fmaf(w, r5.y, SN1); SN2 = fmaf(w, r5.z, SN2);
-            v[10] = w * gc0; v[11] = w * gc1; v[12] = w * gc2;
-            v[13] = w * gn0; v[14] = w * gn1; v[15] = w * gn2;
-            const float gz = w * gd;
-            float grho = 0.f;
-            if (!capped) { v[9] = G * galpha; grho = -0.5f * G * r4.x * galpha; }  // S12: zero through the cap
-            if (surf) {
-              // rho = u^2+v^2, z = D0/qz, (u,v) = (qx,qy)/qz, q = R - dx P - dy Q
-              const float gu = 2.0f * u * grho, gv = 2.0f * vv * grho;
-              const float gq0 = gu * inv, gq1 = gv * inv, gq2 = -(fmaf(gu, u, fmaf(gv, vv, gz * z))) * inv;
-              v[0] = -dx * gq0; v[1] = -dx * gq1; v[2] = -dx * gq2;
-              v[3] = -dy * gq0; v[4] = -dy * gq1; v[5] = -dy * gq2;
-              v[6] = gq0; v[7] = gq1; v[8] = gq2;
-              ex[0] = gz * inv;
-            } else {
-              ex[1] = gz;  // z = z_j
-              ex[2] = -2.0f * dx * inv_sigma2 * grho;
-              ex[3] = -2.0f * dy * inv_sigma2 * grho;
-            }
-          }
+      if (contributes) {
+        const float4 r4 = sr[4], r5 = sr[5];
+        const float G = ex2_approx(rho * kNegHalfLog2e);
+        const float araw = r4.x * G;
+        const bool capped = araw > alpha_max;
+        const float a = capped ? alpha_max : araw;
+        const float inv1ma = rcp_approx(1.0f - a);
+        T *= inv1ma;  // T_i = T_{i+1} / (1 - alpha_i)
+        const float w = a * T;
+        float galpha = gaT * inv1ma + gd * (z * T - SD * inv1ma);
+        galpha += gc0 * (r4.y * T - SC0 * inv1ma) + gc1 * (r4.z * T - SC1 * inv1ma) + gc2 * (r4.w * T - SC2 * inv1ma);
+        galpha += gn0 * (r5.x * T - SN0 * inv1ma) + gn1 * (r5.y * T - SN1 * inv1ma) + gn2 * (r5.z * T - SN2 * inv1ma);
+        SC0 = fmaf(w, r4.y, SC0); SC1 = fmaf(w, r4.z, SC1); SC2 = fmaf(w, r4.w, SC2);
+        SD = fmaf(w, z, SD);
+        SN0 = fmaf(w, r5.x, SN0); SN1 = fmaf(w, r5.y, SN1); SN2 = fmaf(w, r5.z, SN2);
+        v[10] = w * gc0; v[11] = w * gc1; v[12] = w * gc2;
+        v[13] = w * gn0; v[14] = w * gn1; v[15] = w * gn2;
+        const float gz = w * gd;
+        float grho = 0.f;
+        if (!capped) { v[9] = G * galpha; grho = -0.5f * G * r4.x * galpha; }  // S12: zero through the cap
+        if (surf) {
+          // rho = u^2+v^2, z = D0/qz, (u,v) = (qx,qy)/qz, q = R - dx P - dy Q
+          const float gu = 2.0f * u * grho, gv = 2.0f * vv * grho;
+          const float gq0 = gu * inv, gq1 = gv * inv, gq2 = -(fmaf(gu, u, fmaf(gv, vv, gz * z))) * inv;
+          v[0] = -dx * gq0; v[1] = -dx * gq1; v[2] = -dx * gq2;
+          v[3] = -dy * gq0; v[4] = -dy * gq1; v[5] = -dy * gq2;
+          v[6] = gq0; v[7] = gq1; v[8] = gq2;
+          ex[0] = gz * inv;
+        } else {
+          ex[1] = gz;  // z = z_j
+          ex[2] = -2.0f * dx * inv_sigma2 * grho;
+          ex[3] = -2.0f * dy * inv_sigma2 * grho;
         }
       }
-      if (!__any_sync(0xFFFFFFFFu, contributes)) continue;
       warp_transpose_reduce16(v, lane);
       if ((lane & 1) == 0) atomicAdd(&s_acc[j * kNG + (lane >> 1)], v[0]);
       if (__any_sync(0xFFFFFFFFu, (ex[0] != 0.f) | (ex[1] != 0.f) | (ex[2] != 0.f) | (ex[3] != 0.f))) {

@@ -8,26 +8,6 @@ namespace ocgs {
 constexpr int kFwdBatch = 128;                 // list entries staged per batch
 constexpr float kContribFix = 134217728.0f;    // 2^27: alpha*T in fixed point for the warp-wide REDUX sum
 
-// O4 from the record (common.cuh): q = R - dx*P - dy*Q, (u,v) = (qx,qy)/qz, hit depth z = D0/qz.
-__device__ __forceinline__ bool eval_pair(const float4 r0, const float4 r1, const float4 r2, const float4 r3, float px, float py,
-                                          float near_z, float inv_sigma2, float& rho, float& z) {
-  const float dx = px - r2.z, dy = py - r2.w;
-  const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
-  const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
-  const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
-  if (qz == 0.0f) return false;
-  const float inv = __fdividef(1.0f, qz);
-  const float u = qx * inv, v = qy * inv;
-  const float rho3 = fmaf(u, u, v * v);
-  const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
-  const bool surf = rho3 <= rho2;
-  rho = surf ? rho3 : rho2;
-  z = surf ? r2.y * inv : r3.y;
-  if (z < near_z) return false;
-  if (rho > r3.x) return false;
-  return true;
-}
-
 // bit w of the result: warp w's 16x2 pixel strip of tile row ty intersects the surfel's pixel rect (rows only: the
 // rect always overlaps the tile's columns, it was binned to this tile)
 __device__ __forceinline__ uint32_t strip_mask(const float4 r3, int tile_y0) {
@@ -48,7 +28,7 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
   __shared__ uint32_t s_rank[kFwdBatch];
   __shared__ uint8_t s_mask[kFwdBatch];
   __shared__ uint32_t s_cnt[kStats ? kFwdBatch : 1];
-  __shared__ float s_sum[kStats ? kFwdBatch : 1];
+  __shared__ unsigned long long s_fix[kStats ? kFwdBatch : 1];  // sum of alpha*T in 2^-27 fixed point
   __shared__ float s_red[8];
 
   const int tile = blockIdx.x;
@@ -61,6 +41,7 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
   const float inv_sigma2 = 1.0f / cfg.filter_sigma2;
   const int lane = threadIdx.x & 31;
   const uint32_t wbit = 1u << (threadIdx.x >> 5);
+  const float near_z = cfg.near_z, alpha_max = cfg.alpha_max, t_min = cfg.t_min;
 
   float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f;
   uint32_t last = 0;
@@ -74,45 +55,65 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
       s_rank[threadIdx.x] = rk;
       s_mask[threadIdx.x] = (uint8_t)strip_mask(__ldg(rec + (size_t)rk * 6 + 3), ty * kTile);
     }
-    if (kStats && threadIdx.x < kFwdBatch) { s_cnt[threadIdx.x] = 0; s_sum[threadIdx.x] = 0.f; }
+    if (kStats && threadIdx.x < kFwdBatch) { s_cnt[threadIdx.x] = 0; s_fix[threadIdx.x] = 0ull; }
     __syncthreads();
     for (int i = threadIdx.x; i < cnt * 6; i += 256) {
       const int e = i / 6, part = i - 6 * e;
       s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
     }
     __syncthreads();
-    for (int j = 0; j < cnt; ++j) {
-      if (!(s_mask[j] & wbit)) continue;  // the surfel's rect misses this warp's strip
-      if (__all_sync(0xFFFFFFFFu, done)) break;
-      const float4 r0 = s_rec[6 * j], r1 = s_rec[6 * j + 1], r2 = s_rec[6 * j + 2], r3 = s_rec[6 * j + 3];
-      float rho, z;
-      bool blend = false;
-      float wgt = 0.f;
-      if (!done && eval_pair(r0, r1, r2, r3, px, py, cfg.near_z, inv_sigma2, rho, z)) {
-        const float4 r4 = s_rec[6 * j + 4], r5 = s_rec[6 * j + 5];
-        const float a = fminf(cfg.alpha_max, r4.x * __expf(-0.5f * rho));
-        const float Tn = T * (1.0f - a);
-        if (Tn < cfg.t_min) {
-          done = true;  // S11: stop before blending this pair
-        } else {
-          wgt = a * T;
-          C0 = fmaf(wgt, r4.y, C0); C1 = fmaf(wgt, r4.z, C1); C2 = fmaf(wgt, r4.w, C2);
-          D = fmaf(wgt, z, D);
-          N0 = fmaf(wgt, r5.x, N0); N1 = fmaf(wgt, r5.y, N1); N2 = fmaf(wgt, r5.z, N2);
-          T = Tn;
-          last = (b0 - start) + j + 1;
-          blend = true;
-        }
-      }
-      if (kStats) {
-        const unsigned bal = __ballot_sync(0xFFFFFFFFu, blend);
-        if (bal) {
-          const unsigned fix = __reduce_add_sync(0xFFFFFFFFu, (unsigned)__float2uint_rn(wgt * kContribFix));
-          if (lane == 0) {
-            atomicAdd(&s_cnt[j], (uint32_t)__popc(bal));
-            atomicAdd(&s_sum[j], (float)fix * (1.0f / kContribFix));
+    // the batch in chunks of 32 entries: lane jj keeps the statistics of entry c0 + jj in registers
+    bool all_done = false;
+    for (int c0 = 0; c0 < cnt && !all_done; c0 += 32) {
+      uint32_t cntr = 0, fixr = 0;
+      const int ce = min(32, cnt - c0);
+      const float4* sr = s_rec + 6 * c0;
+      for (int jj = 0; jj < ce; ++jj, sr += 6) {
+        if (!(s_mask[c0 + jj] & wbit)) continue;  // the surfel's rect misses this warp's strip
+        if (__all_sync(0xFFFFFFFFu, done)) { all_done = true; break; }
+        const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
+        // O4 from the record: q = R - dx P - dy Q, (u,v) = (qx,qy)/qz, hit depth D0/qz
+        const float dx = px - r2.z, dy = py - r2.w;
+        const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
+        const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
+        const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
+        const float inv = rcp_approx(qz);
+        const float u = qx * inv, v = qy * inv;
+        const float rho3 = fmaf(u, u, v * v);
+        const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
+        const bool surf = rho3 <= rho2;
+        const float rho = surf ? rho3 : rho2;
+        const float z = surf ? r2.y * inv : r3.y;
+        bool blend = false;
+        float wgt = 0.f;
+        if (!done && qz != 0.0f && !(z < near_z) && !(rho > r3.x)) {
+          const float4 r4 = sr[4];
+          const float a = fminf(alpha_max, r4.x * ex2_approx(rho * kNegHalfLog2e));
+          const float Tn = T * (1.0f - a);
+          if (Tn < t_min) {
+            done = true;  // S11: stop before blending this pair
+          } else {
+            const float4 r5 = sr[5];
+            wgt = a * T;
+            C0 = fmaf(wgt, r4.y, C0); C1 = fmaf(wgt, r4.z, C1); C2 = fmaf(wgt, r4.w, C2);
+            D = fmaf(wgt, z, D);
+            N0 = fmaf(wgt, r5.x, N0); N1 = fmaf(wgt, r5.y, N1); N2 = fmaf(wgt, r5.z, N2);
+            T = Tn;
+            last = (b0 - start) + c0 + jj + 1;
+            blend = true;
           }
         }
+        if (kStats) {
+          const unsigned bal = __ballot_sync(0xFFFFFFFFu, blend);
+          if (bal) {
+            const unsigned fix = __reduce_add_sync(0xFFFFFFFFu, (unsigned)__float2uint_rn(wgt * kContribFix));
+            if (lane == jj) { cntr = (uint32_t)__popc(bal); fixr = fix; }
+          }
+        }
+      }
+      if (kStats && cntr) {
+        atomicAdd(&s_cnt[c0 + lane], cntr);
+        atomicAdd(&s_fix[c0 + lane], (unsigned long long)fixr);
       }
     }
     if (kStats) {
@@ -120,7 +121,7 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
       if ((int)threadIdx.x < cnt && s_cnt[threadIdx.x] > 0) {
         const uint32_t id = rank_to_id[s_rank[threadIdx.x]];
         atomicAdd(&vis_count[id], s_cnt[threadIdx.x]);
-        atomicAdd(&contrib_sum[id], s_sum[threadIdx.x]);
+        atomicAdd(&contrib_sum[id], (float)s_fix[threadIdx.x] * (1.0f / kContribFix));
       }
     }
   }
