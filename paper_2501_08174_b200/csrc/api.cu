@@ -53,6 +53,7 @@ bool carve_workspace(void* ws, int n, int width, int height, size_t key_capacity
   L.scratch = off;
   const size_t o_dkeyA = take(N * 4), o_dkeyB = take(N * 4), o_dvalB = take(N * 4);
   const size_t o_tkeyB = take(K * 4), o_tvalB = take(K * 4);
+  const size_t o_hit = take(K);
   const size_t max_items = N > K ? N : K;
   const size_t o_hist = take((div_up(max_items, kSortTile) + 1) * kRadix * 4);
   const size_t o_dtot = take(kRadix * 4);
@@ -83,6 +84,7 @@ bool carve_workspace(void* ws, int n, int width, int height, size_t key_capacity
     out->dvalB = (uint32_t*)(b + o_dvalB);
     out->tkeyB = (uint32_t*)(b + o_tkeyB);
     out->tvalB = (uint32_t*)(b + o_tvalB);
+    out->hit = (uint8_t*)(b + o_hit);
     out->hist = (uint32_t*)(b + o_hist);
     out->digit_total = (uint32_t*)(b + o_dtot);
     out->tcount = (uint32_t*)(b + o_tcount);

@@ -53,6 +53,7 @@ struct Workspace {
   // scratch
   uint32_t* dkeyA; uint32_t* dkeyB; uint32_t* dvalB;  // depth sort ping-pong (dvalA == rank_to_id)
   uint32_t* tkeyB; uint32_t* tvalB;                   // tile sort ping-pong
+  uint8_t* hit;                                       // [key_capacity] per list entry: bit w = warp w of the tile blended it (fwd -> bwd)
   uint32_t* hist;                                     // [kRadix * max_blocks] digit-major block histograms
   uint32_t* digit_total;                              // [kRadix]
   uint32_t* tcount;                                   // [N] tiles touched by rank

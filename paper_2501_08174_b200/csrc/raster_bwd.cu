@@ -58,14 +58,8 @@ __device__ __forceinline__ void warp_transpose_reduce4(float* e, int lane) {
   e[0] += __shfl_xor_sync(0xFFFFFFFFu, e[0], 1);
 }
 
-__device__ __forceinline__ uint32_t strip_mask_bwd(const float4 r3, int tile_y0) {
-  const int iy0 = (int)(__float_as_uint(r3.z) >> 16), iy1 = (int)(__float_as_uint(r3.w) >> 16);
-  const int lo = max(iy0 - tile_y0, 0) >> 1, hi = min(iy1 - tile_y0, 15) >> 1;
-  return hi < lo ? 0u : ((2u << hi) - 1u) & ~((1u << lo) - 1u);
-}
-
 __global__ void __launch_bounds__(256, 3) render_bwd_kernel(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
-                                                            const float4* __restrict__ rec, const uint8_t* __restrict__ mask,
+                                                            const float4* __restrict__ rec, const uint8_t* __restrict__ hit, const uint8_t* __restrict__ mask,
                                                             const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
                                                             const float* __restrict__ gC, const float* __restrict__ gA,
                                                             const float* __restrict__ gD, const float* __restrict__ gN, int W, int H,
@@ -123,7 +117,7 @@ __global__ void __launch_bounds__(256, 3) render_bwd_kernel(const uint32_t* __re
     if ((int)threadIdx.x < cnt) {
       const uint32_t rk = list[start + b0 + threadIdx.x];
       s_rank[threadIdx.x] = rk;
-      s_mask[threadIdx.x] = (uint8_t)strip_mask_bwd(__ldg(rec + (size_t)rk * 6 + 3), ty * kTile);
+      s_mask[threadIdx.x] = hit[start + b0 + threadIdx.x];  // bit w: warp w blended this entry in the forward pass
     }
     for (int i = threadIdx.x; i < cnt * kNG; i += 256) s_acc[i] = 0.f;
     __syncthreads();
@@ -352,7 +346,7 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
   if (g_prof_on) prof_mark(st, "memset_grad_rec");
   if (w.n_tiles > 0) {
     const float goh = mask ? (float)((double)cfg.gamma_bg / ((double)cam.W * (double)cam.H)) : 0.f;
-    render_bwd_kernel<<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, mask, final_T, n_contrib, gC, gA, gD, gN,
+    render_bwd_kernel<<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, w.hit, mask, final_T, n_contrib, gC, gA, gD, gN,
                                                  cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
     OCGS_LAUNCHED(st, "render_bwd_kernel");
   }

@@ -22,11 +22,12 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
                                                          const uint8_t* __restrict__ mask, int W, int H, int tiles_x,
                                                          ocgs_config cfg, float* __restrict__ color, float* __restrict__ alpha,
                                                          float* __restrict__ depth, float* __restrict__ normal,
-                                                         uint32_t* __restrict__ n_contrib, float* __restrict__ final_T, float* __restrict__ loss_partial,
+                                                         uint32_t* __restrict__ n_contrib, float* __restrict__ final_T, uint8_t* __restrict__ hit, float* __restrict__ loss_partial,
                                                          uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum) {
   __shared__ float4 s_rec[kFwdBatch * 6];
   __shared__ uint32_t s_rank[kFwdBatch];
   __shared__ uint8_t s_mask[kFwdBatch];
+  __shared__ uint32_t s_hit[kFwdBatch];  // bit w: warp w blended the entry (read by the backward pass)
   __shared__ uint32_t s_cnt[kStats ? kFwdBatch : 1];
   __shared__ unsigned long long s_fix[kStats ? kFwdBatch : 1];  // sum of alpha*T in 2^-27 fixed point
   __shared__ float s_red[8];
@@ -55,6 +56,7 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
       s_rank[threadIdx.x] = rk;
       s_mask[threadIdx.x] = (uint8_t)strip_mask(__ldg(rec + (size_t)rk * 6 + 3), ty * kTile);
     }
+    if (threadIdx.x < kFwdBatch) s_hit[threadIdx.x] = 0;
     if (kStats && threadIdx.x < kFwdBatch) { s_cnt[threadIdx.x] = 0; s_fix[threadIdx.x] = 0ull; }
     __syncthreads();
     for (int i = threadIdx.x; i < cnt * 6; i += 256) {
@@ -103,21 +105,26 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
             blend = true;
           }
         }
-        if (kStats) {
-          const unsigned bal = __ballot_sync(0xFFFFFFFFu, blend);
-          if (bal) {
+        const unsigned bal = __ballot_sync(0xFFFFFFFFu, blend);
+        if (bal) {
+          if (kStats) {
             const unsigned fix = __reduce_add_sync(0xFFFFFFFFu, (unsigned)__float2uint_rn(wgt * kContribFix));
-            if (lane == jj) { cntr = (uint32_t)__popc(bal); fixr = fix; }
+            if (lane == jj) fixr = fix;
           }
+          if (lane == jj) cntr = (uint32_t)__popc(bal);
         }
       }
-      if (kStats && cntr) {
-        atomicAdd(&s_cnt[c0 + lane], cntr);
-        atomicAdd(&s_fix[c0 + lane], (unsigned long long)fixr);
+      if (cntr) {
+        atomicOr(&s_hit[c0 + lane], wbit);
+        if (kStats) {
+          atomicAdd(&s_cnt[c0 + lane], cntr);
+          atomicAdd(&s_fix[c0 + lane], (unsigned long long)fixr);
+        }
       }
     }
+    __syncthreads();
+    if ((int)threadIdx.x < cnt) hit[b0 + threadIdx.x] = (uint8_t)s_hit[threadIdx.x];
     if (kStats) {
-      __syncthreads();
       if ((int)threadIdx.x < cnt && s_cnt[threadIdx.x] > 0) {
         const uint32_t id = rank_to_id[s_rank[threadIdx.x]];
         atomicAdd(&vis_count[id], s_cnt[threadIdx.x]);
@@ -175,10 +182,10 @@ int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Worksp
   float* lp = loss_bg ? w.loss_partial : nullptr;
   if (stats)
     render_fwd_kernel<true><<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, mask, cam.W, cam.H,
-                                                       cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, lp, vis_count, contrib_sum);
+                                                       cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, w.hit, lp, vis_count, contrib_sum);
   else
     render_fwd_kernel<false><<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, mask, cam.W, cam.H,
-                                                        cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, lp, nullptr, nullptr);
+                                                        cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, w.hit, lp, nullptr, nullptr);
   OCGS_LAUNCHED(st, "render_fwd_kernel");
   if (loss_bg) {
     loss_final_kernel<<<1, 1024, 0, st>>>(w.loss_partial, w.n_tiles, (float)(1.0 / ((double)cam.W * (double)cam.H)), loss_bg);
