@@ -58,7 +58,7 @@ __device__ __forceinline__ void warp_transpose_reduce4(float* e, int lane) {
   e[0] += __shfl_xor_sync(0xFFFFFFFFu, e[0], 1);
 }
 
-__global__ void __launch_bounds__(256, 3) render_bwd_kernel(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
+__global__ void __launch_bounds__(256, 4) render_bwd_kernel(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                             const float4* __restrict__ rec, const uint8_t* __restrict__ hit, const uint8_t* __restrict__ mask,
                                                             const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
                                                             const float* __restrict__ gC, const float* __restrict__ gA,

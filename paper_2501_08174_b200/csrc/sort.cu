@@ -341,21 +341,22 @@ __global__ void __launch_bounds__(kEmitThreads) emit_keys_kernel(const ocgs_head
 __global__ void __launch_bounds__(256) tile_ranges_kernel(const ocgs_header* __restrict__ header, const uint32_t* __restrict__ keys,
                                                           int n_tiles, uint32_t* __restrict__ ranges) {
   const unsigned K = header->error ? 0u : (unsigned)header->K;
-  const size_t k = (size_t)blockIdx.x * 256 + threadIdx.x;
+  const size_t stride = (size_t)gridDim.x * 256;
   if (K == 0) {
-    for (size_t t = k; t < (size_t)n_tiles; t += (size_t)gridDim.x * 256) { ranges[2 * t] = 0; ranges[2 * t + 1] = 0; }
+    for (size_t t = (size_t)blockIdx.x * 256 + threadIdx.x; t < (size_t)n_tiles; t += stride) { ranges[2 * t] = 0; ranges[2 * t + 1] = 0; }
     return;
   }
-  if (k >= K) return;
-  const int cur = (int)keys[k];
-  const int prev = k == 0 ? -1 : (int)keys[k - 1];
-  for (int t = prev + 1; t <= cur; ++t) {  // tiles in (prev, cur] start at k; the tile before each of them ends at k
-    ranges[2 * t] = (uint32_t)k;
-    if (t >= 1) ranges[2 * (t - 1) + 1] = (uint32_t)k;
-  }
-  if (k == K - 1) {
-    for (int t = cur + 1; t < n_tiles; ++t) { ranges[2 * t] = K; ranges[2 * (t - 1) + 1] = K; }
-    ranges[2 * (n_tiles - 1) + 1] = K;
+  for (size_t k = (size_t)blockIdx.x * 256 + threadIdx.x; k < K; k += stride) {
+    const int cur = (int)keys[k];
+    const int prev = k == 0 ? -1 : (int)keys[k - 1];
+    for (int t = prev + 1; t <= cur; ++t) {  // tiles in (prev, cur] start at k; the tile before each of them ends at k
+      ranges[2 * t] = (uint32_t)k;
+      if (t >= 1) ranges[2 * (t - 1) + 1] = (uint32_t)k;
+    }
+    if (k == K - 1) {
+      for (int t = cur + 1; t < n_tiles; ++t) { ranges[2 * t] = K; ranges[2 * (t - 1) + 1] = K; }
+      ranges[2 * (n_tiles - 1) + 1] = K;
+    }
   }
 }
 
@@ -409,7 +410,7 @@ int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cu
       OCGS_LAUNCHED(st, "copy_u32_kernel");
     }
   }
-  const unsigned rgrid = (unsigned)max(div_up(max(cap, (size_t)1), 256), div_up((size_t)w.n_tiles, 256));
+  const unsigned rgrid = (unsigned)min(max(div_up(max(cap, (size_t)1), 256), div_up((size_t)w.n_tiles, 256)), (size_t)148 * 16);
   tile_ranges_kernel<<<rgrid, 256, 0, st>>>(w.header, w.tile_keys, w.n_tiles, w.ranges);
   OCGS_LAUNCHED(st, "tile_ranges_kernel");
   if (sorted_ids && cap > 0) {
