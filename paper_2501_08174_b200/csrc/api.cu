@@ -59,6 +59,7 @@ bool carve_workspace(void* ws, int n, int width, int height, size_t key_capacity
   const size_t o_dtot = take(kRadix * 4);
   const size_t o_tcount = take(N * 4);
   const size_t o_bsum = take((div_up(N, 1024) + 2) * 4);
+  const size_t o_twork = take(n_tiles * 4), o_torder = take(n_tiles * 4);
   L.total_bytes = off;
   if (layout) *layout = L;
   if (out) {
@@ -89,6 +90,8 @@ bool carve_workspace(void* ws, int n, int width, int height, size_t key_capacity
     out->digit_total = (uint32_t*)(b + o_dtot);
     out->tcount = (uint32_t*)(b + o_tcount);
     out->blocksum = (uint32_t*)(b + o_bsum);
+    out->tile_work = (uint32_t*)(b + o_twork);
+    out->tile_order = (uint32_t*)(b + o_torder);
     out->n = n; out->width = width; out->height = height;
     out->tiles_x = tiles_x; out->tiles_y = tiles_y; out->n_tiles = (int)n_tiles;
     out->key_capacity = key_capacity;

@@ -58,6 +58,8 @@ struct Workspace {
   uint32_t* digit_total;                              // [kRadix]
   uint32_t* tcount;                                   // [N] tiles touched by rank
   uint32_t* blocksum;                                 // [ceil(N/1024)+1]
+  uint32_t* tile_work;                                // [n_tiles] forward: list length; backward: max n_contrib of the tile
+  uint32_t* tile_order;                               // [n_tiles] tiles in descending order of work (heavy tiles first)
   int n, width, height, tiles_x, tiles_y, n_tiles;
   size_t key_capacity;
 };
@@ -98,6 +100,9 @@ int launch_prune(const ocgs_surfels& in, uint32_t* vis_count, float* contrib_sum
 
 int launch_masked_l1(const float* color, const float* target, const uint8_t* mask, int W, int H, float* dL_dcolor, float* loss,
                      float* partial, int n_partial, cudaStream_t st);
+
+// tile_order <- tiles sorted by descending tile_work (bucketed; launch order of the raster CTAs)
+int launch_order_tiles(const Workspace& w, bool from_ranges, cudaStream_t st);
 
 // stable LSD radix sort of (u32 key, u32 value) pairs on bits [0, key_bits); count is read from the device (*n_ptr, u64 or
 // u32 selected by n_is_u64) and bounded by n_max for grid sizing. Result lands in (keysA, valsA) when the number of

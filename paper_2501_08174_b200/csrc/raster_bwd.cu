@@ -58,7 +58,75 @@ __device__ __forceinline__ void warp_transpose_reduce4(float* e, int lane) {
   e[0] += __shfl_xor_sync(0xFFFFFFFFu, e[0], 1);
 }
 
-__global__ void __launch_bounds__(256, 4) render_bwd_kernel(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
+// per-pixel state of the back-to-front walk
+struct BwdPixel {
+  float px, py;
+  float T, gaT;                    // running transmittance T_i, gA * T_final
+  float gc0, gc1, gc2, gd, gn0, gn1, gn2;
+  float SC0, SC1, SC2, SD, SN0, SN1, SN2;  // suffix sums behind the current pair
+  uint32_t last;                   // n_contrib (0 for pixels outside the image)
+};
+
+struct BwdConsts { float near_z, alpha_max, inv_sigma2; };
+
+// One (pixel, entry) pair: recompute O4, and if the pair was blended add its 20 record-gradient terms into v / ex.
+__device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4 r0, const float4 r1, const float4 r2, const float4 r3,
+                                         const float4* __restrict__ sr, const BwdConsts& k, float* v, float* ex) {
+  const float dx = s.px - r2.z, dy = s.py - r2.w;
+  const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
+  const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
+  const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
+  const float inv = rcp_approx(qz);
+  const float u = qx * inv, vv = qy * inv;
+  const float rho3 = fmaf(u, u, vv * vv);
+  const float rho2 = fmaf(dx, dx, dy * dy) * k.inv_sigma2;
+  const bool surf = rho3 <= rho2;
+  const float rho = surf ? rho3 : rho2;
+  const float z = surf ? r2.y * inv : r3.y;
+  const bool contributes = idx < s.last && qz != 0.0f && !(z < k.near_z) && !(rho > r3.x);
+  if (contributes) {
+    const float4 r4 = sr[4], r5 = sr[5];
+    const float G = ex2_approx(rho * kNegHalfLog2e);
+    const float araw = r4.x * G;
+    const bool capped = araw > k.alpha_max;
+    const float a = capped ? k.alpha_max : araw;
+    const float inv1ma = rcp_approx(1.0f - a);
+    s.T *= inv1ma;  // T_i = T_{i+1} / (1 - alpha_i)
+    const float T = s.T, w = a * T;
+    float galpha = s.gaT * inv1ma + s.gd * (z * T - s.SD * inv1ma);
+    galpha += s.gc0 * (r4.y * T - s.SC0 * inv1ma) + s.gc1 * (r4.z * T - s.SC1 * inv1ma) + s.gc2 * (r4.w * T - s.SC2 * inv1ma);
+    galpha += s.gn0 * (r5.x * T - s.SN0 * inv1ma) + s.gn1 * (r5.y * T - s.SN1 * inv1ma) + s.gn2 * (r5.z * T - s.SN2 * inv1ma);
+    s.SC0 = fmaf(w, r4.y, s.SC0); s.SC1 = fmaf(w, r4.z, s.SC1); s.SC2 = fmaf(w, r4.w, s.SC2);
+    s.SD = fmaf(w, z, s.SD);
+    s.SN0 = fmaf(w, r5.x, s.SN0); s.SN1 = fmaf(w, r5.y, s.SN1); s.SN2 = fmaf(w, r5.z, s.SN2);
+    v[10] = fmaf(w, s.gc0, v[10]); v[11] = fmaf(w, s.gc1, v[11]); v[12] = fmaf(w, s.gc2, v[12]);
+    v[13] = fmaf(w, s.gn0, v[13]); v[14] = fmaf(w, s.gn1, v[14]); v[15] = fmaf(w, s.gn2, v[15]);
+    const float gz = w * s.gd;
+    float grho = 0.f;
+    if (!capped) { v[9] = fmaf(G, galpha, v[9]); grho = -0.5f * G * r4.x * galpha; }  // S12: zero through the cap
+    if (surf) {
+      // rho = u^2+v^2, z = D0/qz, (u,v) = (qx,qy)/qz, q = R - dx P - dy Q
+      const float gu = 2.0f * u * grho, gv = 2.0f * vv * grho;
+      const float gq0 = gu * inv, gq1 = gv * inv, gq2 = -(fmaf(gu, u, fmaf(gv, vv, gz * z))) * inv;
+      v[0] = fmaf(-dx, gq0, v[0]); v[1] = fmaf(-dx, gq1, v[1]); v[2] = fmaf(-dx, gq2, v[2]);
+      v[3] = fmaf(-dy, gq0, v[3]); v[4] = fmaf(-dy, gq1, v[4]); v[5] = fmaf(-dy, gq2, v[5]);
+      v[6] += gq0; v[7] += gq1; v[8] += gq2;
+      ex[0] = fmaf(gz, inv, ex[0]);
+    } else {
+      ex[1] += gz;  // z = z_j
+      ex[2] = fmaf(-2.0f * dx * k.inv_sigma2, grho, ex[2]);
+      ex[3] = fmaf(-2.0f * dy * k.inv_sigma2, grho, ex[3]);
+    }
+  }
+  return contributes;
+}
+
+// CTA = one 16x16 tile, 128 threads, TWO pixels per thread: warp w owns rows 4w..4w+3, lane l the pixels
+// (l & 15, 4w + (l >> 4)) and (l & 15, 4w + 2 + (l >> 4)), i.e. one pixel in each of the forward kernel's 16x2 strips
+// 2w and 2w+1.  The two pixels' gradient terms are added in registers (free: the adds fold into FMAs) before the
+// 32-lane transposing reduction, which is therefore paid once per 64 pixels.
+__global__ void __launch_bounds__(128, 5) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
+                                                            const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                             const float4* __restrict__ rec, const uint8_t* __restrict__ hit, const uint8_t* __restrict__ mask,
                                                             const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
                                                             const float* __restrict__ gC, const float* __restrict__ gA,
@@ -68,121 +136,69 @@ __global__ void __launch_bounds__(256, 4) render_bwd_kernel(const uint32_t* __re
   __shared__ uint32_t s_rank[kBwdBatch];
   __shared__ uint8_t s_mask[kBwdBatch];
   __shared__ float s_acc[kBwdBatch * kNG];
-  __shared__ uint32_t s_max[8];
-
-  const int tile = blockIdx.x;
-  const int tx = tile % tiles_x, ty = tile / tiles_x;
-  const int lx = threadIdx.x & 15, ly = threadIdx.x >> 4;
-  const int ix = tx * kTile + lx, iy = ty * kTile + ly;
-  const bool inside = ix < W && iy < H;
-  const float px = (float)ix, py = (float)iy;
-  const uint32_t start = ranges[2 * tile];
-  const float inv_sigma2 = 1.0f / cfg.filter_sigma2;
-  const int lane = threadIdx.x & 31;
-  const uint32_t wbit = 1u << (threadIdx.x >> 5);
-  const size_t HW = (size_t)W * H, p = inside ? (size_t)iy * W + ix : 0;
-  const float near_z = cfg.near_z, alpha_max = cfg.alpha_max;
-
-  uint32_t last = 0;
-  float Tfin = 1.0f, gc0 = 0.f, gc1 = 0.f, gc2 = 0.f, ga = 0.f, gd = 0.f, gn0 = 0.f, gn1 = 0.f, gn2 = 0.f;
-  if (inside) {
-    last = n_contrib[p];
-    Tfin = final_T[p];
-    if (gC) { gc0 = gC[p]; gc1 = gC[HW + p]; gc2 = gC[2 * HW + p]; }
-    if (gA) ga = gA[p];
-    if (gD) gd = gD[p];
-    if (gN) { gn0 = gN[p]; gn1 = gN[HW + p]; gn2 = gN[2 * HW + p]; }
-    if (mask && mask[p] == 0) ga += gamma_over_hw;  // d(gamma L_b)/dA = gamma (1-M)/(HW), Eq. 1 / Eq. 3
-  }
-  // block max of n_contrib
-  uint32_t mx = last;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
-  if (lane == 0) s_max[threadIdx.x >> 5] = mx;
-  __syncthreads();
-  mx = 0;
-#pragma unroll
-  for (int w2 = 0; w2 < 8; ++w2) mx = max(mx, s_max[w2]);
+  const int tile = (int)tile_order[blockIdx.x];  // heavy tiles are launched first
+  const uint32_t mx = tile_work[tile];           // max n_contrib of the tile (written by the forward pass)
   if (mx == 0) return;
+  const int tx = tile % tiles_x, ty = tile / tiles_x;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t start = ranges[2 * tile];
+  const uint32_t bit0 = 1u << (2 * warp), bit1 = 2u << (2 * warp);
+  const size_t HW = (size_t)W * H;
+  BwdConsts kc = {cfg.near_z, cfg.alpha_max, 1.0f / cfg.filter_sigma2};
 
-  float T = Tfin;
-  const float gaT = ga * Tfin;
-  float SC0 = Tfin * cfg.bg[0], SC1 = Tfin * cfg.bg[1], SC2 = Tfin * cfg.bg[2], SD = 0.f, SN0 = 0.f, SN1 = 0.f, SN2 = 0.f;
-
+  BwdPixel ps[2];
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+    const int ix = tx * kTile + (lane & 15), iy = ty * kTile + 4 * warp + 2 * q + (lane >> 4);
+    BwdPixel& s = ps[q];
+    s.px = (float)ix; s.py = (float)iy;
+    s.last = 0;
+    float Tfin = 1.0f, ga = 0.f;
+    s.gc0 = s.gc1 = s.gc2 = s.gd = s.gn0 = s.gn1 = s.gn2 = 0.f;
+    if (ix < W && iy < H) {
+      const size_t p = (size_t)iy * W + ix;
+      s.last = n_contrib[p];
+      Tfin = final_T[p];
+      if (gC) { s.gc0 = gC[p]; s.gc1 = gC[HW + p]; s.gc2 = gC[2 * HW + p]; }
+      if (gA) ga = gA[p];
+      if (gD) s.gd = gD[p];
+      if (gN) { s.gn0 = gN[p]; s.gn1 = gN[HW + p]; s.gn2 = gN[2 * HW + p]; }
+      if (mask && mask[p] == 0) ga += gamma_over_hw;  // d(gamma L_b)/dA = gamma (1-M)/(HW), Eq. 1 / Eq. 3
+    }
+    s.T = Tfin; s.gaT = ga * Tfin;
+    s.SC0 = Tfin * cfg.bg[0]; s.SC1 = Tfin * cfg.bg[1]; s.SC2 = Tfin * cfg.bg[2];
+    s.SD = s.SN0 = s.SN1 = s.SN2 = 0.f;
+  }
   const int nbatch = (int)((mx + kBwdBatch - 1) / kBwdBatch);
   for (int bi = nbatch - 1; bi >= 0; --bi) {
     const uint32_t b0 = (uint32_t)bi * kBwdBatch;
     const int cnt = (int)min((uint32_t)kBwdBatch, mx - b0);
     __syncthreads();  // previous batch fully flushed before s_rank / s_acc are reused
     if ((int)threadIdx.x < cnt) {
-      const uint32_t rk = list[start + b0 + threadIdx.x];
-      s_rank[threadIdx.x] = rk;
-      s_mask[threadIdx.x] = hit[start + b0 + threadIdx.x];  // bit w: warp w blended this entry in the forward pass
+      s_rank[threadIdx.x] = list[start + b0 + threadIdx.x];
+      s_mask[threadIdx.x] = hit[start + b0 + threadIdx.x];  // bit s: strip s of the tile blended this entry in the forward pass
     }
-    for (int i = threadIdx.x; i < cnt * kNG; i += 256) s_acc[i] = 0.f;
+    for (int i = threadIdx.x; i < cnt * kNG; i += 128) s_acc[i] = 0.f;
     __syncthreads();
-    for (int i = threadIdx.x; i < cnt * 6; i += 256) {
+    for (int i = threadIdx.x; i < cnt * 6; i += 128) {
       const int e = i / 6, part = i - 6 * e;
       s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
     }
     __syncthreads();
     const float4* sr = s_rec + 6 * (cnt - 1);
     for (int j = cnt - 1; j >= 0; --j, sr -= 6) {
-      if (!(s_mask[j] & wbit)) continue;
-      const bool act = (b0 + (uint32_t)j) < last;  // last == 0 for pixels outside the image
-      if (!__any_sync(0xFFFFFFFFu, act)) continue;
+      const uint32_t m = s_mask[j];
+      if (!(m & (bit0 | bit1))) continue;
+      const uint32_t idx = b0 + (uint32_t)j;
       const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
-      const float dx = px - r2.z, dy = py - r2.w;
-      const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
-      const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
-      const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
-      const float inv = rcp_approx(qz);
-      const float u = qx * inv, vv = qy * inv;
-      const float rho3 = fmaf(u, u, vv * vv);
-      const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
-      const bool surf = rho3 <= rho2;
-      const float rho = surf ? rho3 : rho2;
-      const float z = surf ? r2.y * inv : r3.y;
-      const bool contributes = act && qz != 0.0f && !(z < near_z) && !(rho > r3.x);
-      if (!__any_sync(0xFFFFFFFFu, contributes)) continue;
       float v[16];
 #pragma unroll
       for (int i = 0; i < 16; ++i) v[i] = 0.f;
       float ex[4] = {0.f, 0.f, 0.f, 0.f};  // gD0, gzj, gcx, gcy
-      if (contributes) {
-        const float4 r4 = sr[4], r5 = sr[5];
-        const float G = ex2_approx(rho * kNegHalfLog2e);
-        const float araw = r4.x * G;
-        const bool capped = araw > alpha_max;
-        const float a = capped ? alpha_max : araw;
-        const float inv1ma = rcp_approx(1.0f - a);
-        T *= inv1ma;  // T_i = T_{i+1} / (1 - alpha_i)
-        const float w = a * T;
-        float galpha = gaT * inv1ma + gd * (z * T - SD * inv1ma);
-        galpha += gc0 * (r4.y * T - SC0 * inv1ma) + gc1 * (r4.z * T - SC1 * inv1ma) + gc2 * (r4.w * T - SC2 * inv1ma);
-        galpha += gn0 * (r5.x * T - SN0 * inv1ma) + gn1 * (r5.y * T - SN1 * inv1ma) + gn2 * (r5.z * T - SN2 * inv1ma);
-        SC0 = fmaf(w, r4.y, SC0); SC1 = fmaf(w, r4.z, SC1); SC2 = fmaf(w, r4.w, SC2);
-        SD = fmaf(w, z, SD);
-        SN0 = fmaf(w, r5.x, SN0); SN1 = fmaf(w, r5.y, SN1); SN2 = fmaf(w, r5.z, SN2);
-        v[10] = w * gc0; v[11] = w * gc1; v[12] = w * gc2;
-        v[13] = w * gn0; v[14] = w * gn1; v[15] = w * gn2;
-        const float gz = w * gd;
-        float grho = 0.f;
-        if (!capped) { v[9] = G * galpha; grho = -0.5f * G * r4.x * galpha; }  // S12: zero through the cap
-        if (surf) {
-          // rho = u^2+v^2, z = D0/qz, (u,v) = (qx,qy)/qz, q = R - dx P - dy Q
-          const float gu = 2.0f * u * grho, gv = 2.0f * vv * grho;
-          const float gq0 = gu * inv, gq1 = gv * inv, gq2 = -(fmaf(gu, u, fmaf(gv, vv, gz * z))) * inv;
-          v[0] = -dx * gq0; v[1] = -dx * gq1; v[2] = -dx * gq2;
-          v[3] = -dy * gq0; v[4] = -dy * gq1; v[5] = -dy * gq2;
-          v[6] = gq0; v[7] = gq1; v[8] = gq2;
-          ex[0] = gz * inv;
-        } else {
-          ex[1] = gz;  // z = z_j
-          ex[2] = -2.0f * dx * inv_sigma2 * grho;
-          ex[3] = -2.0f * dy * inv_sigma2 * grho;
-        }
-      }
+      bool any = false;
+      if (m & bit0) any |= bwd_pair(ps[0], idx, r0, r1, r2, r3, sr, kc, v, ex);
+      if (m & bit1) any |= bwd_pair(ps[1], idx, r0, r1, r2, r3, sr, kc, v, ex);
+      if (!__any_sync(0xFFFFFFFFu, any)) continue;
       warp_transpose_reduce16(v, lane);
       if ((lane & 1) == 0) atomicAdd(&s_acc[j * kNG + (lane >> 1)], v[0]);
       if (__any_sync(0xFFFFFFFFu, (ex[0] != 0.f) | (ex[1] != 0.f) | (ex[2] != 0.f) | (ex[3] != 0.f))) {
@@ -191,7 +207,7 @@ __global__ void __launch_bounds__(256, 4) render_bwd_kernel(const uint32_t* __re
       }
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < cnt * kNG; i += 256) {
+    for (int i = threadIdx.x; i < cnt * kNG; i += 128) {
       const float val = s_acc[i];
       if (val != 0.f) {
         const int e = i / kNG, f = i - kNG * e;
@@ -345,8 +361,10 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
   OCGS_CUDA_OK(cudaMemsetAsync(w.grad_rec, 0, (size_t)s.n * kRec * sizeof(float), st));
   if (g_prof_on) prof_mark(st, "memset_grad_rec");
   if (w.n_tiles > 0) {
+    int rc = launch_order_tiles(w, /*from_ranges=*/false, st);  // tile_work = max n_contrib per tile, from the forward pass
+    if (rc != OCGS_OK) return rc;
     const float goh = mask ? (float)((double)cfg.gamma_bg / ((double)cam.W * (double)cam.H)) : 0.f;
-    render_bwd_kernel<<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, w.hit, mask, final_T, n_contrib, gC, gA, gD, gN,
+    render_bwd_kernel<<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.hit, mask, final_T, n_contrib, gC, gA, gD, gN,
                                                  cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
     OCGS_LAUNCHED(st, "render_bwd_kernel");
   }

@@ -17,7 +17,8 @@ __device__ __forceinline__ uint32_t strip_mask(const float4 r3, int tile_y0) {
 }
 
 template <bool kStats>
-__global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
+__global__ void __launch_bounds__(256, 5) render_fwd_kernel(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ tile_work,
+                                                            const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                          const float4* __restrict__ rec, const uint32_t* __restrict__ rank_to_id,
                                                          const uint8_t* __restrict__ mask, int W, int H, int tiles_x,
                                                          ocgs_config cfg, float* __restrict__ color, float* __restrict__ alpha,
@@ -31,8 +32,11 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
   __shared__ uint32_t s_cnt[kStats ? kFwdBatch : 1];
   __shared__ unsigned long long s_fix[kStats ? kFwdBatch : 1];  // sum of alpha*T in 2^-27 fixed point
   __shared__ float s_red[8];
+  __shared__ uint32_t s_maxc;
+  if (threadIdx.x == 0) s_maxc = 0;
+  __syncthreads();
 
-  const int tile = blockIdx.x;
+  const int tile = (int)tile_order[blockIdx.x];  // heavy tiles are launched first
   const int tx = tile % tiles_x, ty = tile / tiles_x;
   const int lx = threadIdx.x & 15, ly = threadIdx.x >> 4;
   const int ix = tx * kTile + lx, iy = ty * kTile + ly;
@@ -143,6 +147,14 @@ __global__ void __launch_bounds__(256) render_fwd_kernel(const uint32_t* __restr
     n_contrib[p] = last;
     final_T[p] = T;
   }
+  {  // per-tile max n_contrib: the backward pass's work estimate and loop bound
+    uint32_t mxl = last;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mxl = max(mxl, __shfl_xor_sync(0xFFFFFFFFu, mxl, o));
+    if (mxl && lane == 0) atomicMax(&s_maxc, mxl);
+    __syncthreads();
+    if (threadIdx.x == 0) tile_work[tile] = s_maxc;
+  }
   if (loss_partial) {  // Eq. 1: A (1 - M), fixed-order reduction -> deterministic
     float lb = 0.f;
     if (inside) lb = (mask == nullptr || mask[(size_t)iy * W + ix] == 0) ? A : 0.f;
@@ -178,13 +190,15 @@ int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Worksp
                       float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,
                       float* contrib_sum, cudaStream_t st) {
   if (w.n_tiles == 0) return OCGS_OK;
+  int rc = launch_order_tiles(w, /*from_ranges=*/true, st);  // launch order: longest lists first
+  if (rc != OCGS_OK) return rc;
   const bool stats = vis_count != nullptr && contrib_sum != nullptr;
   float* lp = loss_bg ? w.loss_partial : nullptr;
   if (stats)
-    render_fwd_kernel<true><<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, mask, cam.W, cam.H,
+    render_fwd_kernel<true><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, mask, cam.W, cam.H,
                                                        cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, w.hit, lp, vis_count, contrib_sum);
   else
-    render_fwd_kernel<false><<<w.n_tiles, 256, 0, st>>>(w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, mask, cam.W, cam.H,
+    render_fwd_kernel<false><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, mask, cam.W, cam.H,
                                                         cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, w.hit, lp, nullptr, nullptr);
   OCGS_LAUNCHED(st, "render_fwd_kernel");
   if (loss_bg) {

@@ -421,3 +421,74 @@ int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cu
 }
 
 }  // namespace ocgs
+
+// ---- launch order of the raster CTAs: heavy tiles first (longest-processing-time-first keeps the tail short) -----------
+namespace ocgs {
+
+__global__ void __launch_bounds__(1024) order_tiles_kernel(const uint32_t* __restrict__ ranges, uint32_t* __restrict__ work, int n_tiles,
+                                                           bool from_ranges, uint32_t* __restrict__ order) {
+  constexpr int kBuckets = 1024;
+  __shared__ uint32_t s_cnt[kBuckets];
+  __shared__ uint32_t s_warp[32];
+  __shared__ uint32_t s_maxw;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  uint32_t mx = 0;
+  for (int t = tid; t < n_tiles; t += 1024) {
+    uint32_t wk = from_ranges ? ranges[2 * t + 1] - ranges[2 * t] : work[t];
+    if (from_ranges) work[t] = wk;
+    mx = max(mx, wk);
+  }
+  s_cnt[tid] = 0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
+  if (lane == 0) s_warp[wid] = mx;
+  __syncthreads();
+  if (tid == 0) {
+    uint32_t m = 0;
+    for (int i = 0; i < 32; ++i) m = max(m, s_warp[i]);
+    s_maxw = m;
+  }
+  __syncthreads();
+  const unsigned long long maxw = (unsigned long long)s_maxw + 1ull;
+  // bucket 0 = heaviest
+  for (int t = tid; t < n_tiles; t += 1024) {
+    const uint32_t b = (kBuckets - 1) - (uint32_t)(((unsigned long long)work[t] * kBuckets) / maxw);
+    atomicAdd(&s_cnt[b], 1u);
+  }
+  __syncthreads();
+  // exclusive scan of the 1024 bucket counts
+  const uint32_t c = s_cnt[tid];
+  uint32_t inc = c;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+    if (lane >= o) inc += x;
+  }
+  if (lane == 31) s_warp[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    uint32_t x = s_warp[lane];
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, x, o);
+      if (lane >= o) x += y;
+    }
+    s_warp[lane] = x;
+  }
+  __syncthreads();
+  s_cnt[tid] = (wid ? s_warp[wid - 1] : 0) + inc - c;
+  __syncthreads();
+  for (int t = tid; t < n_tiles; t += 1024) {
+    const uint32_t b = (kBuckets - 1) - (uint32_t)(((unsigned long long)work[t] * kBuckets) / maxw);
+    order[atomicAdd(&s_cnt[b], 1u)] = (uint32_t)t;
+  }
+}
+
+int launch_order_tiles(const Workspace& w, bool from_ranges, cudaStream_t st) {
+  if (w.n_tiles == 0) return OCGS_OK;
+  order_tiles_kernel<<<1, 1024, 0, st>>>(w.ranges, w.tile_work, w.n_tiles, from_ranges, w.tile_order);
+  OCGS_LAUNCHED(st, "order_tiles_kernel");
+  return OCGS_OK;
+}
+
+}  // namespace ocgs
