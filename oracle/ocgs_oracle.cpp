@@ -127,28 +127,36 @@ Pre preprocess_one(const float* p, const float* s, const float* q, float o, cons
   const double rr = 2.0 * std::log((double)o / (double)cfg.alpha_min);
   const float rc = (float)std::fmin((double)cfg.rho_max, rr);
   r.rho_cut = rc;
-  // step 6: conic tangents (S7)
+  // step 6: conic tangents (S7), in coordinates CENTRED on the projected centre c2d (reading R-bbox).
+  // The roots of a x^2 - 2 b x + c = 0 taken about the image origin (m^2 - c/a with m ~ 500, h ~ 3) cancel
+  // catastrophically in fp32 (half-extent off by 1e-2 px, so the integer rect can MISS a contributing pixel and S7's
+  // "conservative" fails); about c2d the same closed form has m' ~ 0 and -c'/a ~ h^2: no cancellation.
   const float a = std::fmaf(rc, std::fmaf(M[6], M[6], M[7] * M[7]), -(M[8] * M[8]));
   if (!(a < 0.0f)) return r;  // ellipse reaches the eye plane
+  r.c2d[0] = M[2] / M[8];
+  r.c2d[1] = M[5] / M[8];
   float m[2], h[2];
   for (int k = 0; k < 2; ++k) {
     const float* Mr = M + 3 * k;
-    const float b = std::fmaf(rc, std::fmaf(Mr[0], M[6], Mr[1] * M[7]), -(Mr[2] * M[8]));
-    const float cc = std::fmaf(rc, std::fmaf(Mr[0], Mr[0], Mr[1] * Mr[1]), -(Mr[2] * Mr[2]));
+    const float nc = -r.c2d[k];
+    const float A0 = std::fmaf(nc, M[6], Mr[0]), A1 = std::fmaf(nc, M[7], Mr[1]), A2 = std::fmaf(nc, M[8], Mr[2]);  // M_r - c_r M_2
+    const float b = std::fmaf(rc, std::fmaf(A0, M[6], A1 * M[7]), -(A2 * M[8]));
+    const float cc = std::fmaf(rc, std::fmaf(A0, A0, A1 * A1), -(A2 * A2));
     m[k] = b / a;
     h[k] = std::sqrt(std::fmax(0.0f, std::fmaf(m[k], m[k], -(cc / a))));
+    // outward pad (1 + 2^-16) h + 2^-7 px: far above the fp32 error of this sequence, far below a pixel; pixels
+    // inside the pad but outside the ellipse are rejected by the per-pixel rho test (S6), so the image is unchanged
+    h[k] = std::fmaf(h[k], 1.0000152587890625f, 0.0078125f);
   }
-  // step 7: centre and filter disc (S8)
-  r.c2d[0] = M[2] / M[8];
-  r.c2d[1] = M[5] / M[8];
-  const float rf = std::sqrt(cfg.filter_sigma2 * rc);
+  // step 7: filter disc (S8), same absolute pad
+  const float rf = std::sqrt(cfg.filter_sigma2 * rc) + 0.0078125f;
   // step 8: integer bounds
   const float lim = 1073741824.0f;
   const int WH[2] = {cam.width, cam.height};
   int lo[2], hi[2];
   for (int k = 0; k < 2; ++k) {
-    float mn = std::fmin(m[k] - h[k], r.c2d[k] - rf);
-    float mx = std::fmax(m[k] + h[k], r.c2d[k] + rf);
+    float mn = std::fmin(r.c2d[k] + (m[k] - h[k]), r.c2d[k] - rf);
+    float mx = std::fmax(r.c2d[k] + (m[k] + h[k]), r.c2d[k] + rf);
     mn = std::fmax(-lim, std::fmin(lim, mn));
     mx = std::fmax(-lim, std::fmin(lim, mx));
     lo[k] = (int)std::ceil(mn);

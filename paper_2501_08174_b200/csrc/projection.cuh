@@ -59,26 +59,30 @@ __device__ __forceinline__ void project_surfel(const float p[3], float su, float
   r.rho_cut = rc;
   const float a = __fmaf_rn(rc, __fmaf_rn(M[6], M[6], __fmul_rn(M[7], M[7])), -__fmul_rn(M[8], M[8]));
   if (!(a < 0.0f)) return;
+  // conic tangents about the projected centre c2d (reading R-bbox: no cancellation in fp32), padded outwards
+  r.cx = __fdiv_rn(M[2], M[8]);
+  r.cy = __fdiv_rn(M[5], M[8]);
+  const float c2[2] = {r.cx, r.cy};
   float m[2], h[2];
 #pragma unroll
   for (int k = 0; k < 2; ++k) {
     const float* Mr = M + 3 * k;
-    const float b = __fmaf_rn(rc, __fmaf_rn(Mr[0], M[6], __fmul_rn(Mr[1], M[7])), -__fmul_rn(Mr[2], M[8]));
-    const float cc = __fmaf_rn(rc, __fmaf_rn(Mr[0], Mr[0], __fmul_rn(Mr[1], Mr[1])), -__fmul_rn(Mr[2], Mr[2]));
+    const float nc = -c2[k];
+    const float A0 = __fmaf_rn(nc, M[6], Mr[0]), A1 = __fmaf_rn(nc, M[7], Mr[1]), A2 = __fmaf_rn(nc, M[8], Mr[2]);
+    const float b = __fmaf_rn(rc, __fmaf_rn(A0, M[6], __fmul_rn(A1, M[7])), -__fmul_rn(A2, M[8]));
+    const float cc = __fmaf_rn(rc, __fmaf_rn(A0, A0, __fmul_rn(A1, A1)), -__fmul_rn(A2, A2));
     m[k] = __fdiv_rn(b, a);
     h[k] = __fsqrt_rn(fmaxf(0.0f, __fmaf_rn(m[k], m[k], -__fdiv_rn(cc, a))));
+    h[k] = __fmaf_rn(h[k], 1.0000152587890625f, 0.0078125f);
   }
-  r.cx = __fdiv_rn(M[2], M[8]);
-  r.cy = __fdiv_rn(M[5], M[8]);
-  const float rf = __fsqrt_rn(__fmul_rn(cfg.filter_sigma2, rc));
+  const float rf = __fadd_rn(__fsqrt_rn(__fmul_rn(cfg.filter_sigma2, rc)), 0.0078125f);
   const float lim = 1073741824.0f;
-  const float c2[2] = {r.cx, r.cy};
   const int WH[2] = {cam.W, cam.H};
   int lo[2], hi[2];
 #pragma unroll
   for (int k = 0; k < 2; ++k) {
-    float mn = fminf(__fsub_rn(m[k], h[k]), __fsub_rn(c2[k], rf));
-    float mx = fmaxf(__fadd_rn(m[k], h[k]), __fadd_rn(c2[k], rf));
+    float mn = fminf(__fadd_rn(c2[k], __fsub_rn(m[k], h[k])), __fsub_rn(c2[k], rf));
+    float mx = fmaxf(__fadd_rn(c2[k], __fadd_rn(m[k], h[k])), __fadd_rn(c2[k], rf));
     mn = fmaxf(-lim, fminf(lim, mn));
     mx = fmaxf(-lim, fminf(lim, mx));
     lo[k] = (int)ceilf(mn);

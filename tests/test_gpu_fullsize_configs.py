@@ -1,0 +1,148 @@
+"""-m gpu: parity at BASELINE.json's FULL sizes for configs 2, 4 and 5 (config 3 is in test_gpu_prune_and_fullsize.py),
+in the launch configuration bench.py uses.  Integer outputs (tiles, rects, depth bits, order, ranges) are compared in
+full; images and gradients in full where the oracle finishes in seconds (config 2) and on sampled windows otherwise
+(config 5); config 4 accumulates the visibility statistics over all 64 views, prunes and compacts."""
+import numpy as np
+import pytest
+
+from gpu_harness import GpuView, check_grads
+from paper_2501_08174_b200 import scenegen as sg
+from test_gpu_parity import arrays, full_parity
+
+pytestmark = pytest.mark.gpu
+
+
+def test_config2_full_size_full_image():
+    """200 k surfels, 800x600 (DTU's training resolution), SH degree 3: every pixel, every gradient."""
+    sc = sg.make_scene("config2")
+    r = full_parity(sc, 3, dict(sh_degree=3), max_fragile=4e-3)
+    assert r["K"] > 100_000
+
+
+def windows_parity(sc, view, windows, key_capacity, rng_seed=11):
+    """Integer outputs in full; forward maps and gradients on `windows` (x0, y0, x1, y1), upstream gradients non-zero
+    only inside them so that the oracle walks only those pixels."""
+    import oracle as orc
+    P = arrays(sc)
+    camn = sc.cameras[view]
+    m = sc.mask(view)
+    cam = orc.camera_from(camn)
+    cfg = orc.default_config(sh_degree=sc.sh_degree)
+    pre = orc.preprocess(*P, cam, cfg)
+    srt = orc.bin_sort(pre, cam, cfg)
+    g = GpuView(P, camn, dict(sh_degree=sc.sh_degree), key_capacity=key_capacity)
+    gp = g.preprocess()
+    vis = pre["visible"] == 1
+    assert np.array_equal(gp["tiles"], pre["tiles_touched"]) and np.array_equal(gp["depth_bits"], pre["depth_bits"])
+    assert np.array_equal(gp["rect"][vis], pre["rect"][vis]) and np.array_equal(gp["clamp"][vis], pre["clamp"][vis])
+    gs = g.bin_sort()
+    assert gs["error"] == 0 and gs["K"] == srt["K"] and gs["n_vis"] == int(vis.sum())
+    assert np.array_equal(gs["ids"], srt["ids"]) and np.array_equal(gs["ranges"], srt["ranges"])
+    gf = g.render_fwd(mask=m)
+    H, W = camn.height, camn.width
+    gC = np.zeros((3, H, W)); gA = np.zeros((H, W)); gD = np.zeros((H, W)); gN = np.zeros((3, H, W))
+    rng = np.random.default_rng(rng_seed)
+    frag_total = npix = 0
+    for (x0, y0, x1, y1) in windows:
+        fw = orc.render_fwd(pre, srt, sc.opacity, cam, cfg, mask=m, window=(x0, y0, x1, y1))
+        ok = fw["fragile"][y0:y1, x0:x1] == 0
+        frag_total += int((~ok).sum()); npix += ok.size
+        for k in ("color", "alpha", "depth", "normal"):
+            a, b = gf[k][..., y0:y1, x0:x1], fw[k][..., y0:y1, x0:x1]
+            scale = np.maximum(1.0, np.abs(b)) if k == "depth" else 1.0
+            err = np.abs(a - b) / scale
+            assert (err * ok).max() <= 1e-4, (k, (x0, y0), (err * ok).max())
+            assert err.max() <= 0.02, (k, (x0, y0), "fragile pixel beyond the discontinuity bound")
+        assert np.array_equal(gf["n_contrib"][y0:y1, x0:x1][ok], fw["n_contrib"][y0:y1, x0:x1][ok])
+        okf = ok.astype(np.float64)
+        gC[:, y0:y1, x0:x1] = rng.normal(size=(3, y1 - y0, x1 - x0)) * okf
+        gA[y0:y1, x0:x1] = rng.normal(size=ok.shape) * okf
+        gD[y0:y1, x0:x1] = rng.normal(size=ok.shape) * okf
+        gN[:, y0:y1, x0:x1] = rng.normal(size=(3, y1 - y0, x1 - x0)) * okf
+    assert frag_total <= 0.01 * npix
+    cfg0 = orc.default_config(sh_degree=sc.sh_degree, gamma_bg=0.0)
+    g.cfg.gamma_bg = 0.0
+    gg = g.render_bwd(gC=gC, gA=gA, gD=gD, gN=gN, mask=m)
+    og = {k: np.zeros_like(v, dtype=np.float64) for k, v in gg.items()}
+    og["_d_opacity_abs"] = np.zeros(sc.n)
+    for w in windows:
+        part = orc.render_bwd(*P, pre, srt, cam, cfg0, mask=m, gC=gC.astype(np.float32), gA=gA.astype(np.float32),
+                              gD=gD.astype(np.float32), gN=gN.astype(np.float32), window=w)
+        for k in og:
+            og[k] += part[k]
+    rep = check_grads(gg, og)
+    return dict(K=srt["K"], n_vis=int(vis.sum()), grads=rep, ranges=srt["ranges"])
+
+
+def test_config5_full_size_sampled_windows():
+    """4 M surfels, 1920x1080: 1080 = 67.5 x 16, so the last tile row is half empty (ragged tail), tile lists up to
+    ~15 k entries (many 128-entry batches per tile), 4.3 M keys through both radix stages."""
+    sc = sg.make_scene("config5")
+    W, H = 1920, 1080
+    windows = [(0, 0, 48, 48), (936, 516, 984, 564), (W - 48, H - 40, W, H), (608, H - 24, 656, H), (1300, 300, 1332, 332)]
+    r = windows_parity(sc, 0, windows, key_capacity=16 * sc.n)
+    L = r["ranges"][:, 1] - r["ranges"][:, 0]
+    assert r["K"] > 2_000_000 and L.max() > 4096
+
+
+def test_config4_full_size_all_views_prune():
+    """800 k surfels (250 k near-opaque shell, 400 k interior, 150 k background), 64 views at 1024x1024: per-surfel
+    statistics over all views, then the prune mask and the compaction, bit-exact against the oracle's rule; the mask
+    must remove the interior and keep the shell (BASELINE.json configs[3])."""
+    import torch
+    import oracle as orc
+    from paper_2501_08174_b200 import binding as B
+    sc = sg.make_scene("config4")
+    P = arrays(sc)
+    n = sc.n
+    vis_o = np.zeros(n, np.uint32); cs_o = np.zeros(n, np.float64); touch = np.zeros(n, np.uint64)
+    g = GpuView(P, sc.cameras[0], dict(sh_degree=3), key_capacity=24 * n)
+    vis_g = torch.zeros(n, dtype=torch.int32, device="cuda"); cs_g = torch.zeros(n, dtype=torch.float32, device="cuda")
+    ocfg = orc.default_config(sh_degree=3)
+    for v in range(len(sc.cameras)):
+        cam = orc.camera_from(sc.cameras[v])
+        pre = orc.preprocess(*P, cam, ocfg)
+        srt = orc.bin_sort(pre, cam, ocfg)
+        fw = orc.render_fwd(pre, srt, sc.opacity, cam, ocfg, mask=None, vis_count=vis_o, contrib_sum=cs_o)
+        touch += fw["fragile_touch"]
+        g.cam = B.camera_from(sc.cameras[v])
+        g.preprocess()
+        gs = g.bin_sort(want_ids=(v % 16 == 0))
+        assert gs["K"] == srt["K"] and np.array_equal(gs["ranges"], srt["ranges"])
+        if "ids" in gs:
+            assert np.array_equal(gs["ids"], srt["ids"])
+        gf = g.render_fwd(mask=None, vis_count=vis_g, contrib_sum=cs_g, want_loss=False)
+        if v % 16 == 0:
+            ok = fw["fragile"] == 0
+            assert (np.abs(gf["alpha"] - fw["alpha"]) * ok).max() <= 1e-4
+            assert (np.abs(gf["color"] - fw["color"]) * ok).max() <= 1e-4
+    vg = vis_g.cpu().numpy().view(np.uint32)
+    clean = touch == 0
+    assert np.array_equal(vg[clean], vis_o[clean])
+    assert np.all(np.abs(vg.astype(np.int64) - vis_o.astype(np.int64)) <= touch.astype(np.int64))
+    assert np.allclose(cs_g.cpu().numpy()[clean], cs_o[clean], rtol=2e-4, atol=5e-6)
+    mask_t = torch.empty(n, dtype=torch.uint8, device="cuda"); remap_t = torch.empty(n, dtype=torch.int32, device="cuda")
+    n_out = torch.zeros(1, dtype=torch.int32, device="cuda")
+    outs = [torch.full_like(t, -7.0) for t in (g.t["pos"], g.t["scale"], g.t["quat"], g.t["opacity"], g.t["sh"])]
+    om = B.ocgs_surfels_mut(*[B._ptr(t) for t in outs], n)
+    pws = torch.empty(B.ocgs_prune_workspace_bytes(n), dtype=torch.uint8, device="cuda")
+    B.ocgs_prune_stats(g.surfels, vis_g, cs_g, g.cfg, mask_t, remap_t, om, n_out, 0, pws)
+    torch.cuda.synchronize()
+    pm = mask_t.cpu().numpy()
+    po = orc.prune(vg, cs_g.cpu().numpy(), sc.opacity)
+    assert np.array_equal(pm, po["prune_mask"]) and np.array_equal(remap_t.cpu().numpy(), po["remap"]) and int(n_out.item()) == po["n_out"]
+    po2 = orc.prune(vis_o, cs_o.astype(np.float32), sc.opacity)
+    assert np.array_equal(pm[clean], po2["prune_mask"][clean])
+    # surfels whose only blends fell on fragile pixels may legitimately differ (S22); there must be almost none
+    assert (pm != po2["prune_mask"]).sum() <= 8
+    comp = orc.compact(dict(pos=sc.pos, scale=sc.scale, quat=sc.quat, opacity=sc.opacity, sh=sc.sh), pm)
+    k = po["n_out"]
+    for t, name in zip(outs, ("pos", "scale", "quat", "opacity", "sh")):
+        got = t.cpu().numpy()
+        assert np.array_equal(got[:k], comp[name]), name
+        assert np.all(got[k:] == -7.0), name
+    interior, shell = sc.group == 2, sc.group == 0
+    print("config4: pruned interior %.4f, shell %.4f, background %.4f, kept %d of %d" %
+          (pm[interior].mean(), pm[shell].mean(), pm[sc.group == 1].mean(), k, n))
+    assert pm[interior].mean() > 0.97
+    assert pm[shell].mean() < 0.5

@@ -317,6 +317,81 @@ def test_bbox_contains_projected_ellipse_and_is_tight():
     assert checked > 150
 
 
+def test_bbox_fp32_is_conservative_at_config2_scale():
+    """S7 / reading R-bbox at the size where fp32 matters (800x600, f = 900, 140 k visible surfels): the integer rect
+    produced by the fp32 sequence must contain the exact (fp64, from the raw parameters) extent of the rho_cut ellipse
+    and of the filter disc, and exceed it by at most one pixel.  The extent is the closed form of the projected
+    conic's axis-aligned tangents (the formula the sampled-boundary test above pins), evaluated in fp64 where its
+    cancellation is harmless.  Regression: surfel 97584 of config 2 / view 3, whose rect under the uncentred fp32
+    formula started at row 538 although rho(450, 537) = 8.5708 < rho_cut = 8.5892."""
+    sc = sg.make_scene("config2")
+    camn = sc.cameras[3]
+    cam = orc.camera_from(camn)
+    cfg = orc.default_config(sh_degree=3)
+    pre = orc.preprocess(sc.pos, sc.scale, sc.quat, sc.opacity, sc.sh, cam, cfg)
+    vis = pre["visible"] == 1
+    q = sc.quat.astype(np.float64)
+    w, x, y, z = q[:, 0], q[:, 1], q[:, 2], q[:, 3]
+    tu = np.stack([1 - 2 * (y * y + z * z), 2 * (x * y + w * z), 2 * (x * z - w * y)], 1)
+    tv = np.stack([2 * (x * y - w * z), 1 - 2 * (x * x + z * z), 2 * (y * z + w * x)], 1)
+    V = camn.view.astype(np.float64)
+    R, t = V[:3, :3], V[:3, 3]
+    pc = sc.pos.astype(np.float64) @ R.T + t
+    cu = (tu @ R.T) * sc.scale[:, 0:1].astype(np.float64)
+    cv = (tv @ R.T) * sc.scale[:, 1:2].astype(np.float64)
+    o = sc.opacity.astype(np.float64)
+    rc = np.minimum(9.0, 2 * np.log(np.maximum(o, 1e-12) * 255.0))
+    rf = np.sqrt(0.5 * rc)
+    f, off = 900.0, (camn.cx - 0.5, camn.cy - 0.5)
+    lo, hi = np.zeros((sc.n, 2)), np.zeros((sc.n, 2))
+    tt = np.stack([rc, rc, -np.ones_like(rc)], 1)
+    m2 = np.stack([cu[:, 2], cv[:, 2], pc[:, 2]], 1)
+    a = (tt * m2 * m2).sum(1)
+    for r in (0, 1):
+        mr = f * np.stack([cu[:, r], cv[:, r], pc[:, r]], 1)  # pixel coordinates relative to the principal point
+        b, c = (tt * mr * m2).sum(1), (tt * mr * mr).sum(1)
+        ctr = b / a
+        half = np.sqrt(np.maximum(0.0, ctr * ctr - c / a))
+        c2 = f * pc[:, r] / pc[:, 2]
+        lo[:, r] = np.minimum(ctr - half, c2 - rf) + off[r]
+        hi[:, r] = np.maximum(ctr + half, c2 + rf) + off[r]
+    WH = (camn.width, camn.height)
+    sel = vis & (a < 0)
+    assert sel.sum() > 100_000
+    rect = pre["rect"][sel].astype(np.int64)
+    for r in (0, 1):
+        e0 = np.clip(np.ceil(lo[sel, r]), 0, WH[r] - 1)
+        e1 = np.clip(np.floor(hi[sel, r]), 0, WH[r] - 1)
+        assert np.all(rect[:, r] <= e0) and np.all(rect[:, 2 + r] >= e1), "rect misses a pixel of the exact extent"
+        assert np.all(rect[:, r] >= e0 - 1) and np.all(rect[:, 2 + r] <= e1 + 1), "rect more than one pixel loose"
+    # surfels the fp32 path culled must have an exact extent that misses the image or is empty
+    culled = (~vis) & (a < 0) & (pc[:, 2] > 0.2) & (o >= 1 / 255)
+    e0x, e1x = np.ceil(lo[culled, 0]), np.floor(hi[culled, 0])
+    e0y, e1y = np.ceil(lo[culled, 1]), np.floor(hi[culled, 1])
+    assert np.all((e1x < 0) | (e0x > WH[0] - 1) | (e0x > e1x) | (e1y < 0) | (e0y > WH[1] - 1) | (e0y > e1y))
+    assert pre["rect"][97584][1] <= 537 <= pre["rect"][97584][3]
+
+
+def test_bruteforce_equals_tiled_config2_full_size_window():
+    """BF == TILED on a window of the full 200 k-surfel config 2 (view 3) that contains pixel (450, 537), where the
+    uncentred fp32 bbox used to drop a contributing pair (alpha jump 1/255 => 5e-4 in colour)."""
+    sc = sg.make_scene("config2")
+    cam = orc.camera_from(sc.cameras[3])
+    cfg = orc.default_config(sh_degree=3)
+    P = (sc.pos, sc.scale, sc.quat, sc.opacity, sc.sh)
+    win = (448, 528, 464, 544)
+    pre = orc.preprocess(*P, cam, cfg)
+    srt = orc.bin_sort(pre, cam, cfg)
+    fw = orc.render_fwd(pre, srt, sc.opacity, cam, cfg, mask=None, window=win)
+    bf = orc.bf_render(*P, cam, cfg, mask=None, window=win, want_stats=False)
+    x0, y0, x1, y1 = win
+    ok = fw["fragile"][y0:y1, x0:x1] == 0
+    assert ok[537 - y0, 450 - x0]
+    for k in ("color", "alpha", "normal"):
+        err = np.abs(fw[k][..., y0:y1, x0:x1] - bf[k][..., y0:y1, x0:x1])
+        assert (err * ok).max() < 5e-5, (k, (err * ok).max())
+
+
 # ---------------------------------------------------------------------------------------------
 # BF (fp64, explicit ray-plane, exhaustive per-pixel sort, no tiles) == TILED
 # ---------------------------------------------------------------------------------------------
