@@ -61,15 +61,18 @@ __device__ __forceinline__ void warp_transpose_reduce4(float* e, int lane) {
 // per-pixel state of the back-to-front walk
 struct BwdPixel {
   float px, py;
-  float T, gaT;                    // running transmittance T_i, gA * T_final
+  float T;                         // running transmittance T_i
+  float GS;                        // sum_c g_c S_c - gA T_final: upstream gradients dotted with the suffix sums behind the pair
   float gc0, gc1, gc2, gd, gn0, gn1, gn2;
-  float SC0, SC1, SC2, SD, SN0, SN1, SN2;  // suffix sums behind the current pair
   uint32_t last;                   // n_contrib (0 for pixels outside the image)
 };
 
 struct BwdConsts { float near_z, alpha_max, inv_sigma2; };
 
 // One (pixel, entry) pair: recompute O4, and if the pair was blended add its 20 record-gradient terms into v / ex.
+// With Q_c the accumulated maps, q_c this pair's values (rgb, z, n), S_c the suffix sums behind it (O7):
+//   dL/dalpha_i = sum_c g_c (q_c T_i - S_c/(1-alpha_i)) + gA T_final/(1-alpha_i) = T_i (g.q) - (g.S - gA T_final)/(1-alpha_i),
+// and g.S advances by w_i (g.q): one running scalar GS replaces the seven suffix sums.
 __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4 r0, const float4 r1, const float4 r2, const float4 r3,
                                          const float4* __restrict__ sr, const BwdConsts& k, float* v, float* ex) {
   const float dx = s.px - r2.z, dy = s.py - r2.w;
@@ -93,12 +96,11 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
     const float inv1ma = rcp_approx(1.0f - a);
     s.T *= inv1ma;  // T_i = T_{i+1} / (1 - alpha_i)
     const float T = s.T, w = a * T;
-    float galpha = s.gaT * inv1ma + s.gd * (z * T - s.SD * inv1ma);
-    galpha += s.gc0 * (r4.y * T - s.SC0 * inv1ma) + s.gc1 * (r4.z * T - s.SC1 * inv1ma) + s.gc2 * (r4.w * T - s.SC2 * inv1ma);
-    galpha += s.gn0 * (r5.x * T - s.SN0 * inv1ma) + s.gn1 * (r5.y * T - s.SN1 * inv1ma) + s.gn2 * (r5.z * T - s.SN2 * inv1ma);
-    s.SC0 = fmaf(w, r4.y, s.SC0); s.SC1 = fmaf(w, r4.z, s.SC1); s.SC2 = fmaf(w, r4.w, s.SC2);
-    s.SD = fmaf(w, z, s.SD);
-    s.SN0 = fmaf(w, r5.x, s.SN0); s.SN1 = fmaf(w, r5.y, s.SN1); s.SN2 = fmaf(w, r5.z, s.SN2);
+    float gq = s.gd * z;
+    gq = fmaf(s.gc0, r4.y, gq); gq = fmaf(s.gc1, r4.z, gq); gq = fmaf(s.gc2, r4.w, gq);
+    gq = fmaf(s.gn0, r5.x, gq); gq = fmaf(s.gn1, r5.y, gq); gq = fmaf(s.gn2, r5.z, gq);
+    const float galpha = fmaf(T, gq, -s.GS * inv1ma);
+    s.GS = fmaf(w, gq, s.GS);
     v[10] = fmaf(w, s.gc0, v[10]); v[11] = fmaf(w, s.gc1, v[11]); v[12] = fmaf(w, s.gc2, v[12]);
     v[13] = fmaf(w, s.gn0, v[13]); v[14] = fmaf(w, s.gn1, v[14]); v[15] = fmaf(w, s.gn2, v[15]);
     const float gz = w * s.gd;
@@ -124,7 +126,9 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
 // CTA = one 16x16 tile, 128 threads, TWO pixels per thread: warp w owns rows 4w..4w+3, lane l the pixels
 // (l & 15, 4w + (l >> 4)) and (l & 15, 4w + 2 + (l >> 4)), i.e. one pixel in each of the forward kernel's 16x2 strips
 // 2w and 2w+1.  The two pixels' gradient terms are added in registers (free: the adds fold into FMAs) before the
-// 32-lane transposing reduction, which is therefore paid once per 64 pixels.
+// 32-lane transposing reduction, which is therefore paid once per 64 pixels.  Each warp owns a slice of the batch
+// accumulator and visits an entry at most once per batch, so its totals are plain stores (shared float atomics are
+// CAS loops); the flush adds the slices of the warps whose forward `hit` bits are set.
 __global__ void __launch_bounds__(128, 5) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                             const float4* __restrict__ rec, const uint8_t* __restrict__ hit, const uint8_t* __restrict__ mask,
@@ -135,7 +139,8 @@ __global__ void __launch_bounds__(128, 5) render_bwd_kernel(const uint32_t* __re
   __shared__ float4 s_rec[kBwdBatch * 6];
   __shared__ uint32_t s_rank[kBwdBatch];
   __shared__ uint8_t s_mask[kBwdBatch];
-  __shared__ float s_acc[kBwdBatch * kNG];
+  __shared__ float s_acc[4][kBwdBatch * kNG];
+  static_assert(kBwdBatch == 64, "the per-warp entry masks below cover two 32-entry halves");
   const int tile = (int)tile_order[blockIdx.x];  // heavy tiles are launched first
   const uint32_t mx = tile_work[tile];           // max n_contrib of the tile (written by the forward pass)
   if (mx == 0) return;
@@ -145,6 +150,7 @@ __global__ void __launch_bounds__(128, 5) render_bwd_kernel(const uint32_t* __re
   const uint32_t bit0 = 1u << (2 * warp), bit1 = 2u << (2 * warp);
   const size_t HW = (size_t)W * H;
   BwdConsts kc = {cfg.near_z, cfg.alpha_max, 1.0f / cfg.filter_sigma2};
+  float* acc = s_acc[warp];
 
   BwdPixel ps[2];
 #pragma unroll
@@ -165,54 +171,62 @@ __global__ void __launch_bounds__(128, 5) render_bwd_kernel(const uint32_t* __re
       if (gN) { s.gn0 = gN[p]; s.gn1 = gN[HW + p]; s.gn2 = gN[2 * HW + p]; }
       if (mask && mask[p] == 0) ga += gamma_over_hw;  // d(gamma L_b)/dA = gamma (1-M)/(HW), Eq. 1 / Eq. 3
     }
-    s.T = Tfin; s.gaT = ga * Tfin;
-    s.SC0 = Tfin * cfg.bg[0]; s.SC1 = Tfin * cfg.bg[1]; s.SC2 = Tfin * cfg.bg[2];
-    s.SD = s.SN0 = s.SN1 = s.SN2 = 0.f;
+    s.T = Tfin;
+    // behind the last pair only the background term T_final bg_c is left (O5); dA/dalpha_i = T_final/(1-alpha_i)
+    s.GS = Tfin * (fmaf(s.gc0, cfg.bg[0], fmaf(s.gc1, cfg.bg[1], s.gc2 * cfg.bg[2])) - ga);
   }
   const int nbatch = (int)((mx + kBwdBatch - 1) / kBwdBatch);
   for (int bi = nbatch - 1; bi >= 0; --bi) {
     const uint32_t b0 = (uint32_t)bi * kBwdBatch;
     const int cnt = (int)min((uint32_t)kBwdBatch, mx - b0);
-    __syncthreads();  // previous batch fully flushed before s_rank / s_acc are reused
+    __syncthreads();  // previous batch fully flushed before s_rank / s_mask / s_acc are reused
     if ((int)threadIdx.x < cnt) {
       s_rank[threadIdx.x] = list[start + b0 + threadIdx.x];
       s_mask[threadIdx.x] = hit[start + b0 + threadIdx.x];  // bit s: strip s of the tile blended this entry in the forward pass
     }
-    for (int i = threadIdx.x; i < cnt * kNG; i += 128) s_acc[i] = 0.f;
     __syncthreads();
     for (int i = threadIdx.x; i < cnt * 6; i += 128) {
       const int e = i / 6, part = i - 6 * e;
       s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
     }
+    // per warp: which entries of the batch did strips 2w / 2w+1 blend (bit e of lo: entry e, of hi: entry 32 + e)
+    const uint32_t mlo = lane < cnt ? s_mask[lane] : 0u, mhi = lane + 32 < cnt ? s_mask[lane + 32] : 0u;
+    const uint32_t lo0 = __ballot_sync(0xFFFFFFFFu, mlo & bit0), lo1 = __ballot_sync(0xFFFFFFFFu, mlo & bit1);
+    const uint32_t hi0 = __ballot_sync(0xFFFFFFFFu, mhi & bit0), hi1 = __ballot_sync(0xFFFFFFFFu, mhi & bit1);
     __syncthreads();
-    const float4* sr = s_rec + 6 * (cnt - 1);
-    for (int j = cnt - 1; j >= 0; --j, sr -= 6) {
-      const uint32_t m = s_mask[j];
-      if (!(m & (bit0 | bit1))) continue;
-      const uint32_t idx = b0 + (uint32_t)j;
-      const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
-      float v[16];
+#pragma unroll 1
+    for (int half = 1; half >= 0; --half) {
+      const uint32_t m0 = half ? hi0 : lo0, m1 = half ? hi1 : lo1;
+      uint32_t todo = m0 | m1;
+      while (todo) {
+        const int jb = 31 - __clz(todo);  // back to front
+        todo &= ~(1u << jb);
+        const int j = 32 * half + jb;
+        const float4* sr = s_rec + 6 * j;
+        const uint32_t idx = b0 + (uint32_t)j;
+        const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
+        float v[16];
 #pragma unroll
-      for (int i = 0; i < 16; ++i) v[i] = 0.f;
-      float ex[4] = {0.f, 0.f, 0.f, 0.f};  // gD0, gzj, gcx, gcy
-      bool any = false;
-      if (m & bit0) any |= bwd_pair(ps[0], idx, r0, r1, r2, r3, sr, kc, v, ex);
-      if (m & bit1) any |= bwd_pair(ps[1], idx, r0, r1, r2, r3, sr, kc, v, ex);
-      if (!__any_sync(0xFFFFFFFFu, any)) continue;
-      warp_transpose_reduce16(v, lane);
-      if ((lane & 1) == 0) atomicAdd(&s_acc[j * kNG + (lane >> 1)], v[0]);
-      if (__any_sync(0xFFFFFFFFu, (ex[0] != 0.f) | (ex[1] != 0.f) | (ex[2] != 0.f) | (ex[3] != 0.f))) {
-        warp_transpose_reduce4(ex, lane);
-        if ((lane & 7) == 0) atomicAdd(&s_acc[j * kNG + 16 + (lane >> 3)], ex[0]);
+        for (int i = 0; i < 16; ++i) v[i] = 0.f;
+        float ex[4] = {0.f, 0.f, 0.f, 0.f};  // gD0, gzj, gcx, gcy
+        if ((m0 >> jb) & 1u) bwd_pair(ps[0], idx, r0, r1, r2, r3, sr, kc, v, ex);
+        if ((m1 >> jb) & 1u) bwd_pair(ps[1], idx, r0, r1, r2, r3, sr, kc, v, ex);
+        float* dst = acc + j * kNG;
+        warp_transpose_reduce16(v, lane);
+        if ((lane & 1) == 0) dst[lane >> 1] = v[0];
+        if (__any_sync(0xFFFFFFFFu, (ex[0] != 0.f) | (ex[1] != 0.f) | (ex[2] != 0.f) | (ex[3] != 0.f))) warp_transpose_reduce4(ex, lane);
+        if ((lane & 7) == 0) dst[16 + (lane >> 3)] = ex[0];  // without the reduction every lane's ex[0] is zero
       }
     }
     __syncthreads();
     for (int i = threadIdx.x; i < cnt * kNG; i += 128) {
-      const float val = s_acc[i];
-      if (val != 0.f) {
-        const int e = i / kNG, f = i - kNG * e;
-        atomicAdd(grad_rec + (size_t)s_rank[e] * kRec + f, val);
-      }
+      const int e = i / kNG;
+      const uint32_t m = s_mask[e];
+      float val = 0.f;
+#pragma unroll
+      for (int w2 = 0; w2 < 4; ++w2)
+        if (m & (3u << (2 * w2))) val += s_acc[w2][i];
+      if (val != 0.f) atomicAdd(grad_rec + (size_t)s_rank[e] * kRec + (i - kNG * e), val);
     }
   }
 }

@@ -8,12 +8,38 @@ namespace ocgs {
 constexpr int kFwdBatch = 128;                 // list entries staged per batch
 constexpr float kContribFix = 134217728.0f;    // 2^27: alpha*T in fixed point for the warp-wide REDUX sum
 
-// bit w of the result: warp w's 16x2 pixel strip of tile row ty intersects the surfel's pixel rect (rows only: the
-// rect always overlaps the tile's columns, it was binned to this tile)
-__device__ __forceinline__ uint32_t strip_mask(const float4 r3, int tile_y0) {
-  const int iy0 = (int)(__float_as_uint(r3.z) >> 16), iy1 = (int)(__float_as_uint(r3.w) >> 16);
-  const int lo = max(iy0 - tile_y0, 0) >> 1, hi = min(iy1 - tile_y0, 15) >> 1;  // strips lo..hi
-  return hi < lo ? 0u : ((2u << hi) - 1u) & ~((1u << lo) - 1u);
+// Conservative test "can surfel (r0..r3) contribute to any pixel of the 16x2 strip with first pixel (x0, y0)?", run by ONE
+// lane per list entry (32 entries per warp step) so that the pixel-parallel walk below only visits survivors.
+// A pair contributes iff rho = min(rho3, rho2) <= rho_cut (S6).  Per pixel row dy = y - cy:
+//   rho3 <= rc  <=>  F(dx) = |S - dx P|_W^2 <= 0,  S = R - dy Q,  W = diag(1, 1, -rc)   (q = R - dx P - dy Q, rho3 = (qx^2+qy^2)/qz^2)
+//   i.e. A dx^2 - 2 B dx + C <= 0 with A = P.WP, B = S.WP, C = S.WS: real roots (B -+ sqrt(B^2 - AC))/A must overlap the
+//   strip's dx range; rho2 <= rc is a disc of radius sqrt(rc sigma_f^2) about the centre.
+// Every inequality is relaxed (rc by 1e-4 relative + 1e-4, the dx range by 0.01 px, the discriminant by 1e-5 of its
+// term magnitudes), far more than the fp32 error of either this test or the per-pixel evaluation, so a pair the walk
+// would blend is never culled: the images are bit-identical with and without the cull.
+__device__ __forceinline__ bool strip_may_contribute(const float4 r0, const float4 r1, const float4 r2, const float4 r3, int x0, int y0,
+                                                     float inv_sigma2) {
+  const uint32_t b0 = __float_as_uint(r3.z), b1 = __float_as_uint(r3.w);
+  const int ix0 = (int)(b0 & 0xFFFFu), iy0 = (int)(b0 >> 16), ix1 = (int)(b1 & 0xFFFFu), iy1 = (int)(b1 >> 16);
+  if (iy1 < y0 || iy0 > y0 + 1 || ix1 < x0 || ix0 > x0 + 15) return false;  // pixel rect (S7) misses the strip
+  const float rc = fmaf(r3.x, 1.0001f, 1e-4f);
+  const float dxa = ((float)x0 - r2.z) - 0.01f, dxb = ((float)(x0 + 15) - r2.z) + 0.01f;
+  const float dxn = fminf(fmaxf(0.0f, dxa), dxb);  // dx of the range closest to the centre
+  const float Px = r0.x, Py = r0.y, Pz = r0.z, Qx = r0.w, Qy = r1.x, Qz = r1.y, Rx = r1.z, Ry = r1.w, Rz = r2.x;
+  const float Ap = fmaf(Px, Px, Py * Py), An = rc * Pz * Pz, A = Ap - An;
+  bool keep = !(A > 0.0f);  // not an ellipse along x (cannot happen after the a < 0 cull): keep
+#pragma unroll
+  for (int row = 0; row < 2; ++row) {
+    const float dy = (float)(y0 + row) - r2.w;
+    keep |= fmaf(dxn, dxn, dy * dy) * inv_sigma2 <= rc;  // filter disc (S8)
+    const float Sx = fmaf(-dy, Qx, Rx), Sy = fmaf(-dy, Qy, Ry), Sz = fmaf(-dy, Qz, Rz);
+    const float Cp = fmaf(Sx, Sx, Sy * Sy), Cn = rc * Sz * Sz;
+    const float B = fmaf(Sx, Px, fmaf(Sy, Py, -rc * Sz * Pz));
+    const float disc = fmaf(B, B, -A * (Cp - Cn)) + 1e-5f * (Ap + An) * (Cp + Cn);
+    const float sq = sqrtf(fmaxf(disc, 0.0f));
+    keep |= disc >= 0.0f && (B - sq) <= A * dxb && (B + sq) >= A * dxa;
+  }
+  return keep;
 }
 
 template <bool kStats>
@@ -27,7 +53,6 @@ __global__ void __launch_bounds__(256, 5) render_fwd_kernel(const uint32_t* __re
                                                          uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum) {
   __shared__ float4 s_rec[kFwdBatch * 6];
   __shared__ uint32_t s_rank[kFwdBatch];
-  __shared__ uint8_t s_mask[kFwdBatch];
   __shared__ uint32_t s_hit[kFwdBatch];  // bit w: warp w blended the entry (read by the backward pass)
   __shared__ uint32_t s_cnt[kStats ? kFwdBatch : 1];
   __shared__ unsigned long long s_fix[kStats ? kFwdBatch : 1];  // sum of alpha*T in 2^-27 fixed point
@@ -55,11 +80,7 @@ __global__ void __launch_bounds__(256, 5) render_fwd_kernel(const uint32_t* __re
   for (uint32_t b0 = start; b0 < end; b0 += kFwdBatch) {
     const int cnt = (int)min((uint32_t)kFwdBatch, end - b0);
     if (__syncthreads_and(done)) break;
-    if ((int)threadIdx.x < cnt) {
-      const uint32_t rk = list[b0 + threadIdx.x];
-      s_rank[threadIdx.x] = rk;
-      s_mask[threadIdx.x] = (uint8_t)strip_mask(__ldg(rec + (size_t)rk * 6 + 3), ty * kTile);
-    }
+    if ((int)threadIdx.x < cnt) s_rank[threadIdx.x] = list[b0 + threadIdx.x];
     if (threadIdx.x < kFwdBatch) s_hit[threadIdx.x] = 0;
     if (kStats && threadIdx.x < kFwdBatch) { s_cnt[threadIdx.x] = 0; s_fix[threadIdx.x] = 0ull; }
     __syncthreads();
@@ -73,9 +94,17 @@ __global__ void __launch_bounds__(256, 5) render_fwd_kernel(const uint32_t* __re
     for (int c0 = 0; c0 < cnt && !all_done; c0 += 32) {
       uint32_t cntr = 0, fixr = 0;
       const int ce = min(32, cnt - c0);
-      const float4* sr = s_rec + 6 * c0;
-      for (int jj = 0; jj < ce; ++jj, sr += 6) {
-        if (!(s_mask[c0 + jj] & wbit)) continue;  // the surfel's rect misses this warp's strip
+      // entry-parallel cull: lane l tests entry c0 + l against this warp's strip; the walk visits the survivors
+      bool keep = false;
+      if (lane < ce) {
+        const float4* se = s_rec + 6 * (c0 + lane);
+        keep = strip_may_contribute(se[0], se[1], se[2], se[3], tx * kTile, ty * kTile + 2 * (int)(threadIdx.x >> 5), inv_sigma2);
+      }
+      uint32_t todo = __ballot_sync(0xFFFFFFFFu, keep);
+      while (todo) {
+        const int jj = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const float4* sr = s_rec + 6 * (c0 + jj);
         if (__all_sync(0xFFFFFFFFu, done)) { all_done = true; break; }
         const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
         // O4 from the record: q = R - dx P - dy Q, (u,v) = (qx,qy)/qz, hit depth D0/qz
