@@ -55,8 +55,8 @@ bool carve_workspace(void* ws, int n, int width, int height, size_t key_capacity
   const size_t o_tkeyB = take(K * 4), o_tvalB = take(K * 4);
   const size_t o_hit = take(K);
   const size_t max_items = N > K ? N : K;
-  const size_t o_hist = take((div_up(max_items, kSortTile) + 1) * kRadix * 4);
-  const size_t o_dtot = take(kRadix * 4);
+  const size_t o_hist = take((div_up(max_items, kSortTile) + 1) * kRadix * 4 * 4);  // look-back status words, 4 passes
+  const size_t o_dtot = take((4 * kRadix + 4) * 4);  // global digit histograms of 4 passes + 4 tile tickets
   const size_t o_tcount = take(N * 4);
   const size_t o_bsum = take((div_up(N, 1024) + 2) * 4);
   const size_t o_twork = take(n_tiles * 4), o_torder = take(n_tiles * 4);

@@ -54,8 +54,8 @@ struct Workspace {
   uint32_t* dkeyA; uint32_t* dkeyB; uint32_t* dvalB;  // depth sort ping-pong (dvalA == rank_to_id)
   uint32_t* tkeyB; uint32_t* tvalB;                   // tile sort ping-pong
   uint8_t* hit;                                       // [key_capacity] per list entry: bit w = warp w of the tile blended it (fwd -> bwd)
-  uint32_t* hist;                                     // [kRadix * max_blocks] digit-major block histograms
-  uint32_t* digit_total;                              // [kRadix]
+  uint32_t* hist;                                     // [4 passes][max_blocks][kRadix] look-back status words of the radix passes
+  uint32_t* digit_total;                              // [4][kRadix] global digit histograms + [4] tile tickets
   uint32_t* tcount;                                   // [N] tiles touched by rank
   uint32_t* blocksum;                                 // [ceil(N/1024)+1]
   uint32_t* tile_work;                                // [n_tiles] forward: list length; backward: max n_contrib of the tile
@@ -108,7 +108,7 @@ int launch_order_tiles(const Workspace& w, bool from_ranges, cudaStream_t st);
 // u32 selected by n_is_u64) and bounded by n_max for grid sizing. Result lands in (keysA, valsA) when the number of
 // passes is even, else in (keysB, valsB); returns that through *result_in_B.
 int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t* valsB, const void* n_ptr, bool n_is_u64,
-                     size_t n_max, int key_bits, uint32_t* hist, uint32_t* digit_total, bool* result_in_B, cudaStream_t st);
+                     size_t n_max, int key_bits, uint32_t* status, uint32_t* ghist, bool* result_in_B, cudaStream_t st);
 
 #ifdef __CUDACC__
 // MUFU approximations (1-2 ulp, flush-to-zero): enough for the 1e-4 / 1e-3 tolerances, no denormal fix-up code

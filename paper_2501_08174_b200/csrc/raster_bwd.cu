@@ -129,7 +129,10 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
 // 32-lane transposing reduction, which is therefore paid once per 64 pixels.  Each warp owns a slice of the batch
 // accumulator and visits an entry at most once per batch, so its totals are plain stores (shared float atomics are
 // CAS loops); the flush adds the slices of the warps whose forward `hit` bits are set.
-__global__ void __launch_bounds__(128, 5) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
+#ifndef OCGS_BWD_MINB
+#define OCGS_BWD_MINB 5
+#endif
+__global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                             const float4* __restrict__ rec, const uint8_t* __restrict__ hit, const uint8_t* __restrict__ mask,
                                                             const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,

@@ -5,7 +5,10 @@
 
 namespace ocgs {
 
-constexpr int kFwdBatch = 128;                 // list entries staged per batch
+#ifndef OCGS_FWD_BATCH
+#define OCGS_FWD_BATCH 128
+#endif
+constexpr int kFwdBatch = OCGS_FWD_BATCH;     // list entries staged per batch
 constexpr float kContribFix = 134217728.0f;    // 2^27: alpha*T in fixed point for the warp-wide REDUX sum
 
 // Conservative test "can surfel (r0..r3) contribute to any pixel of the 16x2 strip with first pixel (x0, y0)?", run by ONE
@@ -42,8 +45,11 @@ __device__ __forceinline__ bool strip_may_contribute(const float4 r0, const floa
   return keep;
 }
 
+#ifndef OCGS_FWD_MINB
+#define OCGS_FWD_MINB 6
+#endif
 template <bool kStats>
-__global__ void __launch_bounds__(256, 5) render_fwd_kernel(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ tile_work,
+__global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                          const float4* __restrict__ rec, const uint32_t* __restrict__ rank_to_id,
                                                          const uint8_t* __restrict__ mask, int W, int H, int tiles_x,
@@ -101,11 +107,11 @@ __global__ void __launch_bounds__(256, 5) render_fwd_kernel(const uint32_t* __re
         keep = strip_may_contribute(se[0], se[1], se[2], se[3], tx * kTile, ty * kTile + 2 * (int)(threadIdx.x >> 5), inv_sigma2);
       }
       uint32_t todo = __ballot_sync(0xFFFFFFFFu, keep);
+      if (__all_sync(0xFFFFFFFFu, done)) { all_done = true; break; }  // once per 32 entries: finished lanes are predicated off below
       while (todo) {
         const int jj = __ffs(todo) - 1;
         todo &= todo - 1;
         const float4* sr = s_rec + 6 * (c0 + jj);
-        if (__all_sync(0xFFFFFFFFu, done)) { all_done = true; break; }
         const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
         // O4 from the record: q = R - dx P - dy Q, (u,v) = (qx,qy)/qz, hit depth D0/qz
         const float dx = px - r2.z, dy = py - r2.w;

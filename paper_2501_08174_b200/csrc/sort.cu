@@ -16,106 +16,81 @@ __device__ __forceinline__ unsigned long long load_count(const void* n_ptr, bool
   return is_u64 ? *(const unsigned long long*)n_ptr : (unsigned long long)*(const unsigned int*)n_ptr;
 }
 
-// ---- radix pass, kernel 1: per-block digit histogram, stored digit-major: hist[d * nblk + b] ----------------------
-__global__ void __launch_bounds__(kSortThreads) radix_hist_kernel(const uint32_t* __restrict__ keys, const void* n_ptr,
-                                                                  bool n_is_u64, size_t n_cap, int shift, uint32_t mask,
-                                                                  uint32_t* __restrict__ hist) {
+// ---- stable LSD radix sort, onesweep style ------------------------------------------------------------------------
+// One kernel reads the keys once and builds the global digit histograms of ALL passes; then each pass is ONE kernel:
+// a block takes the next 4096-key tile (atomic ticket, so a tile only ever waits on tiles that are already running),
+// ranks its keys, publishes its per-digit counts, finds its global offsets by decoupled look-back over the preceding
+// tiles' status words (thread d owns digit d), reorders the tile by digit in shared memory and writes it out in runs.
+// Status word = 2 flag bits | 30-bit count, so a plain 32-bit store/load carries flag and value together.
+constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kFlagMask = 3u << 30, kValMask = (1u << 30) - 1u;
+constexpr int kMaxPasses = 4;
+
+__global__ void __launch_bounds__(kSortThreads) radix_hist_all_kernel(const uint32_t* __restrict__ keys, const void* n_ptr, bool n_is_u64,
+                                                                      size_t n_cap, int key_bits, int passes, uint32_t* __restrict__ ghist,
+                                                                      uint32_t* __restrict__ status, size_t status_stride) {
   const unsigned long long n = min(load_count(n_ptr, n_is_u64), (unsigned long long)n_cap);
   const unsigned nblk = (unsigned)div_up((size_t)n, kSortTile);
   if (blockIdx.x >= nblk) return;
-  __shared__ uint32_t h[kRadix];
-  for (int i = threadIdx.x; i < kRadix; i += kSortThreads) h[i] = 0;
+  __shared__ uint32_t h[kMaxPasses][kRadix];
+  for (int p = 0; p < passes; ++p) h[p][threadIdx.x] = 0;
   __syncthreads();
-  const size_t base = (size_t)blockIdx.x * kSortTile;
-#pragma unroll
+  const int lane = threadIdx.x & 31;
+  for (unsigned tile = blockIdx.x; tile < nblk; tile += gridDim.x) {
+  for (int p = 0; p < passes; ++p) status[(size_t)p * status_stride + (size_t)tile * kRadix + threadIdx.x] = 0;  // look-back state of the tile
+  const size_t base = (size_t)tile * kSortTile;
+#pragma unroll 4
   for (int r = 0; r < kSortItems; ++r) {
     const size_t i = base + (size_t)r * kSortThreads + threadIdx.x;
     const bool valid = i < n;
-    const uint32_t d = valid ? ((keys[i] >> shift) & mask) : (0x100u + (threadIdx.x & 31));
-    const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
-    if (valid && (threadIdx.x & 31) == (unsigned)(__ffs(peers) - 1)) atomicAdd(&h[d], (uint32_t)__popc(peers));
-  }
-  __syncthreads();
-  for (int i = threadIdx.x; i < kRadix; i += kSortThreads) hist[(size_t)i * nblk + blockIdx.x] = h[i];
-}
-
-// ---- kernel 2: block d scans row d of the histogram in place (exclusive) and writes the digit total --------------
-__global__ void __launch_bounds__(1024) radix_rowscan_kernel(uint32_t* __restrict__ hist, const void* n_ptr, bool n_is_u64,
-                                                             size_t n_cap, uint32_t* __restrict__ digit_total) {
-  const unsigned long long n = min(load_count(n_ptr, n_is_u64), (unsigned long long)n_cap);
-  const unsigned nblk = (unsigned)div_up((size_t)n, kSortTile);
-  uint32_t* row = hist + (size_t)blockIdx.x * nblk;
-  __shared__ uint32_t warp_sums[32];
-  __shared__ uint32_t carry;
-  if (threadIdx.x == 0) carry = 0;
-  __syncthreads();
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  for (unsigned base = 0; base < nblk; base += 1024) {
-    const unsigned i = base + threadIdx.x;
-    const uint32_t v = i < nblk ? row[i] : 0;
-    uint32_t inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
-      if (lane >= o) inc += t;
-    }
-    if (lane == 31) warp_sums[wid] = inc;
-    __syncthreads();
-    if (wid == 0) {
-      uint32_t ws = warp_sums[lane];
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, ws, o);
-        if (lane >= o) ws += t;
+    const uint32_t k = valid ? keys[i] : 0u;
+    for (int p = 0; p < passes; ++p) {
+      const int shift = p * kRadixBits;
+      const uint32_t mask = (1u << min(kRadixBits, key_bits - shift)) - 1u;
+      const uint32_t dg = (k >> shift) & mask;
+      // high digits are nearly constant across a warp (depth exponent, tile row): one add of 32 instead of 32 colliding adds
+      const uint32_t d0 = __shfl_sync(0xFFFFFFFFu, dg, 0);
+      if (__all_sync(0xFFFFFFFFu, valid && dg == d0)) {
+        if (lane == 0) atomicAdd(&h[p][d0], 32u);
+      } else if (valid) {
+        atomicAdd(&h[p][dg], 1u);
       }
-      warp_sums[lane] = ws;  // inclusive
     }
-    __syncthreads();
-    const uint32_t c = carry;
-    const uint32_t wpre = wid ? warp_sums[wid - 1] : 0;
-    if (i < nblk) row[i] = c + wpre + inc - v;
-    __syncthreads();
-    if (threadIdx.x == 0) carry = c + warp_sums[31];
-    __syncthreads();
   }
-  if (threadIdx.x == 0) digit_total[blockIdx.x] = carry;
+  }
+  __syncthreads();
+  for (int p = 0; p < passes; ++p) {
+    const uint32_t c = h[p][threadIdx.x];
+    if (c) atomicAdd(&ghist[p * kRadix + threadIdx.x], c);
+  }
 }
 
-// ---- kernel 3: stable scatter --------------------------------------------------------------------------------------
-// Items of a block are owned warp-by-warp (warp w: items [w*512, w*512+512), round r, lane l -> w*512 + r*32 + l), so
-// the block-local rank of a key is (same digit in earlier warps) + (same digit in this warp, earlier rounds) +
-// (same digit, lower lanes of this round): the order the keys had in memory.
-__global__ void __launch_bounds__(kSortThreads) radix_scatter_kernel(const uint32_t* __restrict__ keys_in,
-                                                                     const uint32_t* __restrict__ vals_in,
-                                                                     uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
-                                                                     const void* n_ptr, bool n_is_u64, size_t n_cap, int shift,
-                                                                     uint32_t mask, const uint32_t* __restrict__ hist,
-                                                                     const uint32_t* __restrict__ digit_total) {
+__global__ void __launch_bounds__(kSortThreads) radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
+                                                                      uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
+                                                                      const void* n_ptr, bool n_is_u64, size_t n_cap, int shift, uint32_t mask,
+                                                                      const uint32_t* __restrict__ ghist, uint32_t* status,
+                                                                      uint32_t* __restrict__ ticket) {
   const unsigned long long n = min(load_count(n_ptr, n_is_u64), (unsigned long long)n_cap);
   const unsigned nblk = (unsigned)div_up((size_t)n, kSortTile);
-  if (blockIdx.x >= nblk) return;
   constexpr int kWarps = kSortThreads / 32;
   __shared__ uint32_t cnt[kWarps][kRadix];
-  __shared__ uint32_t gbase[kRadix];
+  __shared__ uint32_t s_gpos[kRadix];   // global position of smem slot 0 of each digit's run (may wrap below 0: used mod 2^32)
+  __shared__ uint32_t s_keys[kSortTile];
+  __shared__ uint32_t s_vals[kSortTile];
+  __shared__ uint32_t s_warp[kWarps];
+  __shared__ unsigned s_tile;
+  __shared__ uint32_t s_wg[kWarps], s_wt[kWarps];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  // persistent: the grid is a few blocks per SM, each takes tiles until the tickets run out (the key count lives on
+  // the device, so a grid sized by the capacity would mostly launch blocks with nothing to do)
+  while (true) {
+  __syncthreads();  // previous tile fully written out before its shared state is reused
+  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
   for (int i = threadIdx.x; i < kWarps * kRadix; i += kSortThreads) (&cnt[0][0])[i] = 0;
-  // exclusive scan of the 256 digit totals (one warp, 8 per lane)
-  if (wid == 0) {
-    uint32_t loc[8], s = 0;
-#pragma unroll
-    for (int e = 0; e < 8; ++e) { loc[e] = digit_total[lane * 8 + e]; s += loc[e]; }
-    uint32_t inc = s;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
-      if (lane >= o) inc += t;
-    }
-    uint32_t run = inc - s;
-#pragma unroll
-    for (int e = 0; e < 8; ++e) { gbase[lane * 8 + e] = run; run += loc[e]; }
-  }
   __syncthreads();
-  const size_t base = (size_t)blockIdx.x * kSortTile + (size_t)wid * (kSortItems * 32);
+  const unsigned tile = s_tile;
+  if (tile >= nblk) return;
+  // ---- rank: items are owned warp by warp in memory order (warp w: [w*512, w*512+512), round r, lane l) -----------
+  const size_t base = (size_t)tile * kSortTile + (size_t)wid * (kSortItems * 32);
   uint32_t key[kSortItems], val[kSortItems];
   uint16_t rank[kSortItems];
   const unsigned lt = (1u << lane) - 1u;
@@ -125,6 +100,10 @@ __global__ void __launch_bounds__(kSortThreads) radix_scatter_kernel(const uint3
     const bool valid = i < n;
     key[r] = valid ? keys_in[i] : 0xFFFFFFFFu;
     val[r] = valid ? vals_in[i] : 0u;
+  }
+#pragma unroll
+  for (int r = 0; r < kSortItems; ++r) {
+    const bool valid = base + (size_t)r * 32 + lane < n;
     const uint32_t d = valid ? ((key[r] >> shift) & mask) : (0x100u + lane);
     const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
     uint32_t pre = 0;
@@ -135,50 +114,99 @@ __global__ void __launch_bounds__(kSortThreads) radix_scatter_kernel(const uint3
     rank[r] = (uint16_t)(pre + (uint32_t)__popc(peers & lt));
   }
   __syncthreads();
-  // per digit: exclusive prefix over warps, plus this block's global base
-  {
-    const int d = threadIdx.x;  // kSortThreads == kRadix
-    uint32_t run = gbase[d] + hist[(size_t)d * nblk + blockIdx.x];
+  // ---- thread d: tile count of digit d, publish, exclusive prefixes over warps / digits / preceding tiles ---------
+  const int d = threadIdx.x;  // kSortThreads == kRadix
+  uint32_t total = 0;
 #pragma unroll
-    for (int w2 = 0; w2 < kWarps; ++w2) {
-      const uint32_t t = cnt[w2][d];
-      cnt[w2][d] = run;
-      run += t;
-    }
+  for (int w2 = 0; w2 < kWarps; ++w2) {
+    const uint32_t t = cnt[w2][d];
+    cnt[w2][d] = total;  // exclusive over warps
+    total += t;
   }
+  volatile uint32_t* st = status + (size_t)tile * kRadix + d;
+  *st = (tile == 0 ? kFlagIncl : kFlagAgg) | total;
+  // exclusive scan of ghist (global digit start) and of `total` (start of the digit's run inside the sorted tile)
+  uint32_t gin = ghist[d], tin = total;
+  uint32_t gsc = gin, tsc = tin;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, gsc, o), b2 = __shfl_up_sync(0xFFFFFFFFu, tsc, o);
+    if (lane >= o) { gsc += a; tsc += b2; }
+  }
+  if (lane == 31) { s_wg[wid] = gsc; s_wt[wid] = tsc; }
   __syncthreads();
+  uint32_t gpre = 0, tpre = 0;
+#pragma unroll
+  for (int w2 = 0; w2 < kWarps; ++w2)
+    if (w2 < wid) { gpre += s_wg[w2]; tpre += s_wt[w2]; }
+  const uint32_t gstart = gpre + gsc - gin, dstart = tpre + tsc - tin;
+  // make cnt[w][d] the smem slot of warp w's first key of digit d
+#pragma unroll
+  for (int w2 = 0; w2 < kWarps; ++w2) cnt[w2][d] += dstart;
+  __syncthreads();
+  // ---- reorder the tile by digit in shared memory (local work, overlaps the predecessors' progress) ---------------
 #pragma unroll
   for (int r = 0; r < kSortItems; ++r) {
-    const size_t i = base + (size_t)r * 32 + lane;
-    if (i < n) {
-      const uint32_t d = (key[r] >> shift) & mask;
-      const uint32_t p = cnt[wid][d] + rank[r];
-      keys_out[p] = key[r];
-      vals_out[p] = val[r];
+    if (base + (size_t)r * 32 + lane < n) {
+      const uint32_t dd = (key[r] >> shift) & mask;
+      const uint32_t slot = cnt[wid][dd] + rank[r];
+      s_keys[slot] = key[r];
+      s_vals[slot] = val[r];
     }
   }
+  // ---- decoupled look-back: keys of digit d in preceding tiles --------------------------------------------------
+  uint32_t excl = 0;
+  if (tile > 0) {
+    int p = (int)tile - 1;
+    while (true) {
+      const uint32_t sv = *(volatile uint32_t*)(status + (size_t)p * kRadix + d);
+      const uint32_t fl = sv & kFlagMask;
+      if (fl == 0) continue;  // predecessor has not published yet (it is running: tickets are taken in order)
+      excl += sv & kValMask;
+      if (fl == kFlagIncl) break;
+      --p;  // p >= 0 always: tile 0 publishes inclusive
+    }
+    *st = kFlagIncl | (excl + total);
+  }
+  s_gpos[d] = gstart + excl - dstart;
+  __syncthreads();
+  // ---- coalesced write-out: slot i of the sorted tile goes to s_gpos[digit] + i ------------------------------------
+  const unsigned in_tile = (unsigned)min((unsigned long long)kSortTile, n - (unsigned long long)tile * kSortTile);
+#pragma unroll 4
+  for (unsigned i = threadIdx.x; i < in_tile; i += kSortThreads) {
+    const uint32_t k = s_keys[i];
+    const uint32_t pos = s_gpos[(k >> shift) & mask] + i;
+    keys_out[pos] = k;
+    vals_out[pos] = s_vals[i];
+  }
+  }  // next ticket
 }
 
 int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t* valsB, const void* n_ptr, bool n_is_u64,
-                     size_t n_max, int key_bits, uint32_t* hist, uint32_t* digit_total, bool* result_in_B, cudaStream_t st) {
-  static_assert(kSortThreads == kRadix, "scatter kernel maps one thread per digit");
+                     size_t n_max, int key_bits, uint32_t* status, uint32_t* ghist, bool* result_in_B, cudaStream_t st) {
+  static_assert(kSortThreads == kRadix, "one thread per digit");
   const int passes = (key_bits + kRadixBits - 1) / kRadixBits;
-  const unsigned grid = (unsigned)div_up(n_max, kSortTile);
+  const unsigned tiles_max = (unsigned)div_up(n_max, kSortTile);
+  const unsigned grid = min(tiles_max, 148u * 4u);
+  *result_in_B = (passes & 1) != 0;
+  if (grid == 0 || passes == 0) { *result_in_B = false; return OCGS_OK; }
+  if (passes > kMaxPasses || n_max > (size_t)kValMask) return OCGS_ERR_UNSUPPORTED;
+  uint32_t* tickets = ghist + kMaxPasses * kRadix;
+  OCGS_CUDA_OK(cudaMemsetAsync(ghist, 0, (kMaxPasses * kRadix + kMaxPasses) * sizeof(uint32_t), st));
+  const size_t stride = (size_t)tiles_max * kRadix;
+  radix_hist_all_kernel<<<grid, kSortThreads, 0, st>>>(keysA, n_ptr, n_is_u64, n_max, key_bits, passes, ghist, status, stride);
+  OCGS_LAUNCHED(st, "radix_hist_all_kernel");
   uint32_t *kin = keysA, *vin = valsA, *kout = keysB, *vout = valsB;
-  for (int p = 0; p < passes && grid > 0; ++p) {
+  for (int p = 0; p < passes; ++p) {
     const int shift = p * kRadixBits;
     const int bits = min(kRadixBits, key_bits - shift);
     const uint32_t mask = (1u << bits) - 1u;
-    radix_hist_kernel<<<grid, kSortThreads, 0, st>>>(kin, n_ptr, n_is_u64, n_max, shift, mask, hist);
-    OCGS_LAUNCHED(st, "radix_hist_kernel");
-    radix_rowscan_kernel<<<kRadix, 1024, 0, st>>>(hist, n_ptr, n_is_u64, n_max, digit_total);
-    OCGS_LAUNCHED(st, "radix_rowscan_kernel");
-    radix_scatter_kernel<<<grid, kSortThreads, 0, st>>>(kin, vin, kout, vout, n_ptr, n_is_u64, n_max, shift, mask, hist, digit_total);
-    OCGS_LAUNCHED(st, "radix_scatter_kernel");
+    radix_onesweep_kernel<<<min(tiles_max, 148u * 2u), kSortThreads, 0, st>>>(kin, vin, kout, vout, n_ptr, n_is_u64, n_max, shift, mask, ghist + p * kRadix,
+                                                         status + (size_t)p * stride, tickets + p);
+    OCGS_LAUNCHED(st, "radix_onesweep_kernel");
     uint32_t* t = kin; kin = kout; kout = t;
     t = vin; vin = vout; vout = t;
   }
-  *result_in_B = (passes & 1) != 0;
   return OCGS_OK;
 }
 
@@ -304,11 +332,11 @@ __global__ void __launch_bounds__(kEmitThreads) emit_keys_kernel(const ocgs_head
   if (header->error) return;
   const unsigned K = (unsigned)header->K;
   const unsigned n_vis = header->n_vis;
-  const unsigned k0 = blockIdx.x * kEmitTile;
-  if (k0 >= K) return;
-  const unsigned k1 = min(k0 + kEmitTile, K);
   __shared__ uint32_t s_off[kEmitTile + 2];
   __shared__ unsigned s_r0, s_cnt;
+  for (unsigned k0 = blockIdx.x * kEmitTile; k0 < K; k0 += gridDim.x * kEmitTile) {
+  const unsigned k1 = min(k0 + kEmitTile, K);
+  __syncthreads();  // previous tile's s_off fully consumed
   if (threadIdx.x == 0) {
     // r_lo = last rank with offsets[r] <= k0; r_hi = last rank with offsets[r] <= k1-1
     unsigned lo = 0, hi = n_vis;  // offsets has n_vis+1 entries, offsets[n_vis] = K > k0
@@ -334,6 +362,7 @@ __global__ void __launch_bounds__(kEmitThreads) emit_keys_kernel(const ocgs_head
     const unsigned ty = ty0 + local / wdt, tx = tx0 + local % wdt;
     keys[k] = ty * (unsigned)tiles_x + tx;
     vals[k] = r;
+  }
   }
 }
 
@@ -395,7 +424,7 @@ int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cu
   }
   const size_t cap = w.key_capacity;
   if (cap > 0 && n > 0) {
-    emit_keys_kernel<<<(unsigned)div_up(cap, kEmitTile), kEmitThreads, 0, st>>>(w.header, w.offsets, w.rank_to_id, w.rect, cam.tiles_x,
+    emit_keys_kernel<<<(unsigned)min(div_up(cap, kEmitTile), (size_t)148 * 8), kEmitThreads, 0, st>>>(w.header, w.offsets, w.rank_to_id, w.rect, cam.tiles_x,
                                                                                 w.tile_keys, w.tile_vals);
     OCGS_LAUNCHED(st, "emit_keys_kernel");
     int bits = 1;
