@@ -220,16 +220,24 @@ __global__ void __launch_bounds__(kScanBlock) reorder_kernel(const uint32_t* __r
   const unsigned n_vis = header->n_vis;
   const unsigned r = blockIdx.x * kScanBlock + threadIdx.x;
   if (blockIdx.x * kScanBlock >= n_vis) return;
-  uint32_t t = 0;
+  const int lane = threadIdx.x & 31;
+  uint32_t t = 0, id = 0;
   if (r < n_vis) {
-    const uint32_t id = rank_to_id[r];
+    id = rank_to_id[r];
     id_to_rank[id] = r;
     t = tiles[id];
     tcount[r] = t;
-    const float4* src = rec_id + (size_t)id * 6;
-    float4* dst = rec + (size_t)r * 6;
-    const float4 a = src[0], b = src[1], c = src[2], d = src[3], e = src[4], f = src[5];
-    dst[0] = a; dst[1] = b; dst[2] = c; dst[3] = d; dst[4] = e; dst[5] = f;
+  }
+  // the warp copies its 32 records (6 float4 each) together: lane l moves float4 l, l+32, ... of the 192, so the writes
+  // are contiguous and each gathered record is read as one 96-byte run
+  const unsigned r_warp = r - lane;
+#pragma unroll
+  for (int i = 0; i < 6; ++i) {
+    const int f = i * 32 + lane, e = f / 6, part = f - 6 * e;
+    const uint32_t src_id = __shfl_sync(0xFFFFFFFFu, id, e);
+    if (r_warp + e < n_vis) {
+      rec[(size_t)r_warp * 6 + f] = __ldg(rec_id + (size_t)src_id * 6 + part);
+    }
   }
   // block sum
   __shared__ uint32_t ws[32];
@@ -333,22 +341,29 @@ __global__ void __launch_bounds__(kEmitThreads) emit_keys_kernel(const ocgs_head
   const unsigned K = (unsigned)header->K;
   const unsigned n_vis = header->n_vis;
   __shared__ uint32_t s_off[kEmitTile + 2];
-  __shared__ unsigned s_r0, s_cnt;
+  __shared__ unsigned s_r0, s_r1;
   for (unsigned k0 = blockIdx.x * kEmitTile; k0 < K; k0 += gridDim.x * kEmitTile) {
   const unsigned k1 = min(k0 + kEmitTile, K);
   __syncthreads();  // previous tile's s_off fully consumed
-  if (threadIdx.x == 0) {
-    // r_lo = last rank with offsets[r] <= k0; r_hi = last rank with offsets[r] <= k1-1
-    unsigned lo = 0, hi = n_vis;  // offsets has n_vis+1 entries, offsets[n_vis] = K > k0
-    while (hi - lo > 1) { const unsigned mid = (lo + hi) >> 1; if (offsets[mid] <= k0) lo = mid; else hi = mid; }
-    const unsigned r_lo = lo;
-    lo = r_lo; hi = n_vis;
-    while (hi - lo > 1) { const unsigned mid = (lo + hi) >> 1; if (offsets[mid] <= k1 - 1) lo = mid; else hi = mid; }
-    s_r0 = r_lo;
-    s_cnt = lo - r_lo + 1;
+  // r_lo = last rank with offsets[r] <= k0 (warp 0), r_hi = last rank with offsets[r] <= k1-1 (warp 1); offsets has
+  // n_vis+1 strictly increasing entries with offsets[0] = 0 and offsets[n_vis] = K, searched 33-ary: 32 probes per round
+  if (threadIdx.x < 64) {
+    const int lane = threadIdx.x & 31;
+    const unsigned key = (threadIdx.x < 32) ? k0 : k1 - 1;
+    unsigned lo = 0, hi = n_vis;  // offsets[lo] <= key < offsets[hi]
+    while (hi - lo > 1) {
+      const unsigned step = (hi - lo + 32) / 33;
+      const unsigned long long pos = (unsigned long long)lo + (unsigned long long)(lane + 1) * step;
+      const bool le = pos < hi && offsets[pos] <= key;
+      const int c = __popc(__ballot_sync(0xFFFFFFFFu, le));  // probes are increasing, so the true ones are lanes 0..c-1
+      const unsigned nlo = lo + (unsigned)c * step;
+      if (c < 32) hi = (unsigned)min((unsigned long long)hi, (unsigned long long)nlo + step);
+      lo = nlo;
+    }
+    if (lane == 0) { if (threadIdx.x < 32) s_r0 = lo; else s_r1 = lo; }
   }
   __syncthreads();
-  const unsigned r0 = s_r0, cnt = s_cnt;  // surfels r0 .. r0+cnt-1 own the keys of this block (cnt <= kEmitTile)
+  const unsigned r0 = s_r0, cnt = s_r1 - s_r0 + 1;  // surfels r0 .. r0+cnt-1 own the keys of this block (cnt <= kEmitTile)
   for (unsigned i = threadIdx.x; i <= cnt; i += kEmitThreads) s_off[i] = offsets[r0 + i];
   __syncthreads();
   for (unsigned k = k0 + threadIdx.x; k < k1; k += kEmitThreads) {
