@@ -4,6 +4,10 @@
 
 namespace ocgs {
 
+// Two phases per block of 256 surfels.  (1) every thread projects and culls its surfel (Appendix A / R-bbox) and writes
+// the per-id integers; the visible ones (29 % at config 3, scattered) are compacted into a block-local list.  (2) the
+// list is processed densely, one visible surfel per thread: normal, SH colour (192 B read), the 96-byte raster record.
+// Without the compaction every warp runs the long second part with a third of its lanes.
 __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict__ pos, const float2* __restrict__ scale,
                                                          const float4* __restrict__ quat, const float* __restrict__ opacity,
                                                          const float4* __restrict__ sh, int n, CamParams cam, ocgs_config cfg,
@@ -12,15 +16,15 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
                                                          float4* __restrict__ rec_id, uint32_t* __restrict__ id_to_rank,
                                                          uint32_t* __restrict__ sort_key, uint32_t* __restrict__ sort_val,
                                                          ocgs_header* __restrict__ header) {
+  __shared__ uint32_t s_list[256];
+  __shared__ uint32_t s_warp[8];
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   bool vis = false;
   if (j < n) {
     const float p[3] = {pos[3 * j], pos[3 * j + 1], pos[3 * j + 2]};
-    const float2 s = scale[j];
-    const float4 q = quat[j];
-    const float o = opacity[j];
     Projected pr;
-    project_surfel(p, s.x, s.y, q, o, cam, cfg, pr);
+    project_surfel(p, scale[j].x, scale[j].y, quat[j], opacity[j], cam, cfg, pr);
     vis = pr.visible;
     const uint32_t zb = __float_as_uint(pr.pc[2]);
     depth_bits[j] = zb;
@@ -28,11 +32,39 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
     sort_val[j] = (uint32_t)j;
     id_to_rank[j] = 0xFFFFFFFFu;
     uint32_t nt = 0;
-    uint8_t cl = 0;
     if (vis) {
       const int tx0 = pr.ix0 >> 4, tx1 = (pr.ix1 >> 4) + 1, ty0 = pr.iy0 >> 4, ty1 = (pr.iy1 >> 4) + 1;
       nt = (uint32_t)((tx1 - tx0) * (ty1 - ty0));
       rect[j] = make_ushort4((unsigned short)pr.ix0, (unsigned short)pr.iy0, (unsigned short)pr.ix1, (unsigned short)pr.iy1);
+    } else {
+      clamp_bits[j] = 0;
+    }
+    tiles[j] = nt;
+  }
+  // block-local compaction of the visible surfels (order inside the block is irrelevant: every output is indexed by id)
+  const unsigned ball = __ballot_sync(0xFFFFFFFFu, vis);
+  if (lane == 0) s_warp[wid] = (uint32_t)__popc(ball);
+  __syncthreads();
+  uint32_t before = 0, total = 0;
+#pragma unroll
+  for (int w2 = 0; w2 < 8; ++w2) {
+    const uint32_t c = s_warp[w2];
+    if (w2 < wid) before += c;
+    total += c;
+  }
+  if (vis) s_list[before + (uint32_t)__popc(ball & ((1u << lane) - 1u))] = (uint32_t)j;
+  if (threadIdx.x == 0 && total) atomicAdd(&header->n_vis, total);
+  __syncthreads();
+  if (threadIdx.x >= total) return;
+  {
+    const int id = (int)s_list[threadIdx.x];
+    const float p[3] = {pos[3 * id], pos[3 * id + 1], pos[3 * id + 2]};
+    const float4 q = quat[id];
+    const float o = opacity[id];
+    Projected pr;
+    project_surfel(p, scale[id].x, scale[id].y, q, o, cam, cfg, pr);  // same inputs, same fp32 sequence: same result as phase 1
+    uint8_t cl = 0;
+    {
       // facing normal (view space): n = R_wc t_w, flipped when n . p_c > 0
       const float w = q.x, x = q.y, y = q.z, z = q.w;
       const float tw0 = 2.0f * (x * z + w * y), tw1 = 2.0f * (y * z - w * x), tw2 = 1.0f - 2.0f * (x * x + y * y);
@@ -48,9 +80,11 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
       sh_basis(dx, dy, dz, cfg.sh_degree, Y);
       const int nb = (cfg.sh_degree + 1) * (cfg.sh_degree + 1);
       float col[3] = {0.5f, 0.5f, 0.5f};
-      const float4* shj = sh + (size_t)j * 12;
+      const float4* shj = sh + (size_t)id * 12;
       const int nvec = (3 * nb + 3) / 4;
-      for (int v4 = 0; v4 < nvec; ++v4) {
+#pragma unroll
+      for (int v4 = 0; v4 < 12; ++v4) {
+        if (v4 >= nvec) break;
         const float4 f = __ldg(shj + v4);
         const float ff[4] = {f.x, f.y, f.z, f.w};
 #pragma unroll
@@ -75,7 +109,7 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
       const double Q[3] = {a0[1] * m2[2] - a0[2] * m2[1], a0[2] * m2[0] - a0[0] * m2[2], a0[0] * m2[1] - a0[1] * m2[0]};
       const double R[3] = {a0[1] * a1[2] - a0[2] * a1[1], a0[2] * a1[0] - a0[0] * a1[2], a0[0] * a1[1] - a0[1] * a1[0]};
       const double D0 = m2[0] * R[0] + m2[1] * R[1] + m2[2] * R[2];
-      float4* out = rec_id + (size_t)j * 6;
+      float4* out = rec_id + (size_t)id * 6;
       out[0] = make_float4((float)P[0], (float)P[1], (float)P[2], (float)Q[0]);
       out[1] = make_float4((float)Q[1], (float)Q[2], (float)R[0], (float)R[1]);
       out[2] = make_float4((float)R[2], (float)D0, pr.cx, pr.cy);
@@ -84,11 +118,8 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
       out[4] = make_float4(o, col[0], col[1], col[2]);
       out[5] = make_float4(nx, ny, nz, 0.0f);
     }
-    tiles[j] = nt;
-    clamp_bits[j] = cl;
+    clamp_bits[id] = cl;
   }
-  const unsigned ball = __ballot_sync(0xFFFFFFFFu, vis);
-  if ((threadIdx.x & 31) == 0 && ball) atomicAdd(&header->n_vis, (unsigned)__popc(ball));
 }
 
 int launch_preprocess(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, cudaStream_t st) {

@@ -244,25 +244,44 @@ __global__ void __launch_bounds__(256) clear_grad_rec_kernel(const ocgs_header* 
 __global__ void __launch_bounds__(128) project_bwd_kernel(const float* __restrict__ pos, const float2* __restrict__ scale,
                                                           const float4* __restrict__ quat, const float* __restrict__ opacity,
                                                           const float4* __restrict__ sh, int n, CamParams cam, ocgs_config cfg,
-                                                          const uint32_t* __restrict__ id_to_rank, const uint8_t* __restrict__ clamp_bits,
+                                                          const ocgs_header* __restrict__ header, const uint32_t* __restrict__ id_to_rank,
+                                                          const uint32_t* __restrict__ rank_to_id, const uint8_t* __restrict__ clamp_bits,
                                                           const float* __restrict__ grad_rec, float* __restrict__ d_pos,
                                                           float2* __restrict__ d_scale, float4* __restrict__ d_quat,
                                                           float* __restrict__ d_opacity, float4* __restrict__ d_sh,
                                                           float2* __restrict__ d_center2d) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= n) return;
-  const uint32_t rank = id_to_rank[j];
-  float4* dsh = d_sh + (size_t)j * 12;
-  if (rank == 0xFFFFFFFFu) {
-    d_pos[3 * j] = 0.f; d_pos[3 * j + 1] = 0.f; d_pos[3 * j + 2] = 0.f;
-    d_scale[j] = make_float2(0.f, 0.f);
-    d_quat[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-    d_opacity[j] = 0.f;
-    if (d_center2d) d_center2d[j] = make_float2(0.f, 0.f);
+  // (1) by id: zero gradients of the surfels this view culled, written warp-cooperatively so that runs of culled
+  //     surfels become full-line stores (71 % of the surfels at config 3)
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  {
+    const int jw = t - lane;  // first id of this warp
+    const bool culled = t < n && id_to_rank[t] == 0xFFFFFFFFu;
+    const unsigned cm = __ballot_sync(0xFFFFFFFFu, culled);
+    if (cm) {
+      if (culled) {
+        d_scale[t] = make_float2(0.f, 0.f);
+        d_quat[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+        d_opacity[t] = 0.f;
+        if (d_center2d) d_center2d[t] = make_float2(0.f, 0.f);
+      }
 #pragma unroll
-    for (int i = 0; i < 12; ++i) dsh[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    return;
+      for (int i = 0; i < 3; ++i) {
+        const int f = i * 32 + lane;
+        if ((cm >> (f / 3)) & 1u) d_pos[(size_t)jw * 3 + f] = 0.f;
+      }
+#pragma unroll
+      for (int i = 0; i < 12; ++i) {
+        const int f = i * 32 + lane;
+        if ((cm >> (f / 12)) & 1u) d_sh[(size_t)jw * 12 + f] = make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+    }
   }
+  // (2) by depth rank: thread t handles the visible surfel of rank t, so the warps that do the arithmetic are full
+  if ((unsigned)t >= header->n_vis) return;
+  const uint32_t rank = (uint32_t)t;
+  const int j = (int)rank_to_id[rank];
+  float4* dsh = d_sh + (size_t)j * 12;
   float g[kRec];
   const float4* gr = (const float4*)(grad_rec + (size_t)rank * kRec);
 #pragma unroll
@@ -392,7 +411,7 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
     OCGS_LAUNCHED(st, "render_bwd_kernel");
   }
   project_bwd_kernel<<<(unsigned)div_up((size_t)s.n, 128), 128, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity,
-                                                                        (const float4*)s.sh, s.n, cam, cfg, w.id_to_rank, w.clamp,
+                                                                        (const float4*)s.sh, s.n, cam, cfg, w.header, w.id_to_rank, w.rank_to_id, w.clamp,
                                                                         w.grad_rec, d_pos, (float2*)d_scale, (float4*)d_quat, d_opacity,
                                                                         (float4*)d_sh, (float2*)d_center2d);
   OCGS_LAUNCHED(st, "project_bwd_kernel");
