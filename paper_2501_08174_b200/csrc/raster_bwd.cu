@@ -150,7 +150,10 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
   const int tx = tile % tiles_x, ty = tile / tiles_x;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t start = ranges[2 * tile];
-  const uint32_t bit0 = 1u << (2 * warp), bit1 = 2u << (2 * warp);
+  // this warp's two forward blocks: vertically adjacent, block ids differ by the number of blocks per tile row
+  constexpr int kBX = kTile / kSubW;  // forward blocks per tile row
+  const int bcol = warp % kBX, brow = 2 * (warp / kBX);
+  const uint32_t bit0 = 1u << (brow * kBX + bcol), bit1 = bit0 << kBX;
   const size_t HW = (size_t)W * H;
   BwdConsts kc = {cfg.near_z, cfg.alpha_max, 1.0f / cfg.filter_sigma2};
   float* acc = s_acc[warp];
@@ -158,7 +161,7 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
   BwdPixel ps[2];
 #pragma unroll
   for (int q = 0; q < 2; ++q) {
-    const int ix = tx * kTile + (lane & 15), iy = ty * kTile + 4 * warp + 2 * q + (lane >> 4);
+    const int ix = tx * kTile + bcol * kSubW + lane % kSubW, iy = ty * kTile + (brow + q) * kSubH + lane / kSubW;
     BwdPixel& s = ps[q];
     s.px = (float)ix; s.py = (float)iy;
     s.last = 0;
@@ -228,7 +231,7 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
       float val = 0.f;
 #pragma unroll
       for (int w2 = 0; w2 < 4; ++w2)
-        if (m & (3u << (2 * w2))) val += s_acc[w2][i];
+        if (m & (((1u << kBX) | 1u) << ((2 * (w2 / kBX)) * kBX + w2 % kBX))) val += s_acc[w2][i];
       if (val != 0.f) atomicAdd(grad_rec + (size_t)s_rank[e] * kRec + (i - kNG * e), val);
     }
   }

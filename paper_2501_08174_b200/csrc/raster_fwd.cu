@@ -22,17 +22,18 @@ constexpr float kContribFix = 134217728.0f;    // 2^27: alpha*T in fixed point f
 // would blend is never culled: the images are bit-identical with and without the cull.
 __device__ __forceinline__ bool strip_may_contribute(const float4 r0, const float4 r1, const float4 r2, const float4 r3, int x0, int y0,
                                                      float inv_sigma2) {
+  constexpr int kW = kSubW, kH = kSubH;  // the warp's pixel block (common.cuh)
   const uint32_t b0 = __float_as_uint(r3.z), b1 = __float_as_uint(r3.w);
   const int ix0 = (int)(b0 & 0xFFFFu), iy0 = (int)(b0 >> 16), ix1 = (int)(b1 & 0xFFFFu), iy1 = (int)(b1 >> 16);
-  if (iy1 < y0 || iy0 > y0 + 1 || ix1 < x0 || ix0 > x0 + 15) return false;  // pixel rect (S7) misses the strip
+  if (iy1 < y0 || iy0 > y0 + kH - 1 || ix1 < x0 || ix0 > x0 + kW - 1) return false;  // pixel rect (S7) misses the block
   const float rc = fmaf(r3.x, 1.0001f, 1e-4f);
-  const float dxa = ((float)x0 - r2.z) - 0.01f, dxb = ((float)(x0 + 15) - r2.z) + 0.01f;
+  const float dxa = ((float)x0 - r2.z) - 0.01f, dxb = ((float)(x0 + kW - 1) - r2.z) + 0.01f;
   const float dxn = fminf(fmaxf(0.0f, dxa), dxb);  // dx of the range closest to the centre
   const float Px = r0.x, Py = r0.y, Pz = r0.z, Qx = r0.w, Qy = r1.x, Qz = r1.y, Rx = r1.z, Ry = r1.w, Rz = r2.x;
   const float Ap = fmaf(Px, Px, Py * Py), An = rc * Pz * Pz, A = Ap - An;
   bool keep = !(A > 0.0f);  // not an ellipse along x (cannot happen after the a < 0 cull): keep
 #pragma unroll
-  for (int row = 0; row < 2; ++row) {
+  for (int row = 0; row < kH; ++row) {
     const float dy = (float)(y0 + row) - r2.w;
     keep |= fmaf(dxn, dxn, dy * dy) * inv_sigma2 <= rc;  // filter disc (S8)
     const float Sx = fmaf(-dy, Qx, Rx), Sy = fmaf(-dy, Qy, Ry), Sz = fmaf(-dy, Qz, Rz);
@@ -69,7 +70,10 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
 
   const int tile = (int)tile_order[blockIdx.x];  // heavy tiles are launched first
   const int tx = tile % tiles_x, ty = tile / tiles_x;
-  const int lx = threadIdx.x & 15, ly = threadIdx.x >> 4;
+  // warp w owns the kSubW x kSubH pixel block number w of the tile (row-major over blocks), lane l pixel (l % kSubW, l / kSubW)
+  const int sub = threadIdx.x >> 5, sl = threadIdx.x & 31;
+  const int sub_x0 = (sub % (kTile / kSubW)) * kSubW, sub_y0 = (sub / (kTile / kSubW)) * kSubH;
+  const int lx = sub_x0 + sl % kSubW, ly = sub_y0 + sl / kSubW;
   const int ix = tx * kTile + lx, iy = ty * kTile + ly;
   const bool inside = ix < W && iy < H;
   const float px = (float)ix, py = (float)iy;
@@ -104,7 +108,7 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
       bool keep = false;
       if (lane < ce) {
         const float4* se = s_rec + 6 * (c0 + lane);
-        keep = strip_may_contribute(se[0], se[1], se[2], se[3], tx * kTile, ty * kTile + 2 * (int)(threadIdx.x >> 5), inv_sigma2);
+        keep = strip_may_contribute(se[0], se[1], se[2], se[3], tx * kTile + sub_x0, ty * kTile + sub_y0, inv_sigma2);
       }
       uint32_t todo = __ballot_sync(0xFFFFFFFFu, keep);
       if (__all_sync(0xFFFFFFFFu, done)) { all_done = true; break; }  // once per 32 entries: finished lanes are predicated off below
