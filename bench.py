@@ -23,7 +23,11 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "ms per fwd+bwd raster step (1600x1200, 1M surfels)"
-FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 40.0, 22.0, 111.0
+FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 40.0, 22.0, 72.0  # DESIGN.md section 6 "algorithmic work per unit" (FMA = 2)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the raster kernels, from the `ncu --set full` capture of this
+# workload committed as profiles/r01d_raster_kernels_full.md (bytes)
+NCU_TRAFFIC = {"render_bwd_kernel": 95.6e6, "render_fwd_kernel": 85.5e6}
+NCU_TRAFFIC_SOURCE = "profiles/r01d_raster_kernels_full.md"
 ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 148 SMs x 128 FP32 lanes x 2 (FMA) x max SM clock (B200_PROFILING.md)
 
 
@@ -364,23 +368,34 @@ def run_ours(args):
     launches = sum(c for k, c in cnt.items() if not k.startswith("memset"))
     mean = {k: float(np.mean([c[k] for c in counters])) for k in counters[0]}
     hbm_peak, peak_src = measured_peaks()
-    dom = kernels[0]
-    avg_launch_s = (agg[dom["name"]] / cnt[dom["name"]]) * 1e-3
-    roof = None
-    if dom["name"] in ("render_bwd_kernel", "render_fwd_kernel"):
-        fl = FLOP_EVAL * mean["E"] + (FLOP_BLEND_BWD if dom["name"] == "render_bwd_kernel" else FLOP_BLEND_FWD) * mean["B"]
-        ach = fl / avg_launch_s / 1e12
-        roof = {"kernel": dom["name"], "bound": "alu", "achieved": ach, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": ach / ALU_PEAK_TFLOPS, "traffic": None,
-                "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)",
-                "algorithmic": f"{FLOP_EVAL:.0f} flop x E evaluated pairs + {FLOP_BLEND_BWD if dom['name']=='render_bwd_kernel' else FLOP_BLEND_FWD:.0f} flop x B blended pairs"}
-    else:
-        per_launch = {"radix_scatter_kernel": 16.0 * mean["K"], "radix_hist_kernel": 4.0 * mean["K"], "emit_keys_kernel": 8.0 * mean["K"],
-                      "preprocess_kernel": 61.0 * n + 280.0 * mean["n_vis"], "project_bwd_kernel": 232.0 * n + 312.0 * mean["n_vis"],
-                      "memset_grad_rec": 80.0 * n}.get(dom["name"], 0.0)
-        ach = per_launch / avg_launch_s / 1e9
-        roof = {"kernel": dom["name"], "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+
+    def roofline_of(kd):
+        """Roofline entry of one kernel: algorithmic work per launch / average launch duration."""
+        name = kd["name"]
+        avg_s = (agg[name] / cnt[name]) * 1e-3
+        K, nvis, E, Bp = mean["K"], mean["n_vis"], mean["E"], mean["B"]
+        if name in ("render_fwd_kernel", "render_bwd_kernel"):
+            if name == "render_fwd_kernel":
+                fl, what = FLOP_EVAL * E + FLOP_BLEND_FWD * Bp, f"{FLOP_EVAL:.0f} flop x E evaluated pairs + {FLOP_BLEND_FWD:.0f} flop x B blended pairs"
+            else:
+                fl, what = (FLOP_EVAL + FLOP_BLEND_BWD) * Bp, f"({FLOP_EVAL:.0f} + {FLOP_BLEND_BWD:.0f}) flop x B blended pairs"
+            ach = fl / avg_s / 1e12
+            return {"kernel": name, "bound": "alu", "achieved": ach, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / ALU_PEAK_TFLOPS,
+                    "traffic": NCU_TRAFFIC.get(name), "traffic_source": NCU_TRAFFIC_SOURCE,
+                    "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)", "algorithmic": what}
+        per_launch = {"radix_onesweep_kernel": 16.0 * (4 * n + 2 * K) / 6.0,  # 8 B read + 8 B written per key; 4 passes over N, 2 over K
+                      "radix_hist_all_kernel": 4.0 * (n + K) / 2.0, "emit_keys_kernel": 8.0 * K + 12.0 * nvis,
+                      "preprocess_kernel": 61.0 * n + 296.0 * nvis, "project_bwd_kernel": 232.0 * n + 328.0 * nvis,
+                      "reorder_kernel": 208.0 * nvis, "clear_grad_rec_kernel": 96.0 * nvis, "tile_ranges_kernel": 4.0 * K,
+                      "masked_l1_kernel": 25.0 * W * H}.get(name)
+        if per_launch is None:
+            return None
+        ach = per_launch / avg_s / 1e9
+        return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
                 "traffic": None, "peak_source": peak_src}
+
+    rooflines = [r for r in (roofline_of(kd) for kd in kernels) if r is not None]
+    roof = rooflines[0] if rooflines and rooflines[0]["kernel"] == kernels[0]["name"] else roofline_of(kernels[0])
 
     ms_per_step = ms_total / (steps * world)
     line = {"metric": METRIC, "value": ms_per_step, "unit": "ms", "n_gpus": world, "steps": steps, "warmup": max(args.warmup, nv),
@@ -390,7 +405,7 @@ def run_ours(args):
                        "l2": "inputs larger than L2: 232 MB of surfel parameters are re-read every step", "key_capacity": cap,
                        "shrink": args.shrink},
             "surfels_per_s": n * world / (ms_total / steps * 1e-3), "pixels_per_s": W * H * world / (ms_total / steps * 1e-3),
-            "workload_counters": mean, "gpu_launches": launches, "clocks": clocks, "roofline": roof, "kernels": kernels[:12],
+            "workload_counters": mean, "gpu_launches": launches, "clocks": clocks, "roofline": roof, "rooflines": rooflines, "kernels": kernels[:14],
             "kernel_ms_sum_per_step": kern_total / steps,
             "launch": "cuda_graph_replay" if graphs is not None else "direct",
             "kernel_timing": {"how": "second timed region of the same K steps, direct launches, one CUDA event after every launch "

@@ -6,7 +6,7 @@
 namespace ocgs {
 
 #ifndef OCGS_FWD_BATCH
-#define OCGS_FWD_BATCH 128
+#define OCGS_FWD_BATCH 256
 #endif
 constexpr int kFwdBatch = OCGS_FWD_BATCH;     // list entries staged per batch
 constexpr float kContribFix = 134217728.0f;    // 2^27: alpha*T in fixed point for the warp-wide REDUX sum
