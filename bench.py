@@ -316,6 +316,38 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_total = float(t.item())
 
+    # ---- prune pass, timed separately: once per pruning interval, not per step -------------------
+    # statistics of the nv views just rendered -> mask -> scan -> stable compaction of all five parameter arrays
+    prune = None
+    if rank == 0:
+        vis.zero_(); cs.zero_()
+        for i in range(nv):
+            step(i)
+        pm = torch.empty(n, dtype=torch.uint8, device=dev)
+        remap = torch.empty(n, dtype=torch.int32, device=dev)
+        n_out = torch.zeros(1, dtype=torch.int32, device=dev)
+        outs = [torch.empty_like(params[k]) for k in ("pos", "scale", "quat", "opacity", "sh")]
+        om = B.ocgs_surfels_mut(*[B._ptr(t_) for t_ in outs], n)
+        pws = torch.empty(B.ocgs_prune_workspace_bytes(n), dtype=torch.uint8, device=dev)
+        for _ in range(2):
+            B.ocgs_prune_stats(surfels, vis, cs, cfg, pm, remap, om, n_out, 0, pws)
+        pe0, pe1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        reps = 10
+        pe0.record()
+        for _ in range(reps):
+            B.ocgs_prune_stats(surfels, vis, cs, cfg, pm, remap, om, n_out, 0, pws)
+        pe1.record()
+        torch.cuda.synchronize()
+        p_ms = pe0.elapsed_time(pe1) / reps
+        kept = int(n_out.item())
+        p_bytes = n * (8 + 4 + 1 + 4 + 232) + kept * 232  # stats + opacity read, mask + remap written, params read, survivors written
+        hbm_pk, _src = measured_peaks()
+        prune = {"ms": p_ms, "kept": kept, "of": n, "views": nv, "achieved_gbs": p_bytes / (p_ms * 1e-3) / 1e9,
+                 "frac_of_hbm": p_bytes / (p_ms * 1e-3) / 1e9 / hbm_pk, "algorithmic_bytes": p_bytes}
+        del outs, om
+        vis.zero_(); cs.zero_()
+
     # ---- e2e: the same step through ocgs_step_host with pinned host buffers -----------------------------------------
     e2e = None
     if not args.no_e2e:
@@ -411,6 +443,7 @@ def run_ours(args):
             "kernel_timing": {"how": "second timed region of the same K steps, direct launches, one CUDA event after every launch "
                                      "(those events cost idle gaps, so `value` comes from the region without them)",
                               "ms_per_step_with_events": ms_marked / steps}}
+    line["prune"] = prune
     if e2e:
         line["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline:

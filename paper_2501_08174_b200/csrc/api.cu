@@ -53,7 +53,7 @@ bool carve_workspace(void* ws, int n, int width, int height, size_t key_capacity
   L.scratch = off;
   const size_t o_dkeyA = take(N * 4), o_dkeyB = take(N * 4), o_dvalB = take(N * 4);
   const size_t o_tkeyB = take(K * 4), o_tvalB = take(K * 4);
-  const size_t o_hit = take(K);
+  const size_t o_hit = take(K * 8);
   const size_t max_items = N > K ? N : K;
   const size_t o_hist = take((div_up(max_items, kSortTile) + 1) * kRadix * 4 * 4);  // look-back status words, 4 passes
   const size_t o_dtot = take((4 * kRadix + 4) * 4);  // global digit histograms of 4 passes + 4 tile tickets
@@ -85,7 +85,7 @@ bool carve_workspace(void* ws, int n, int width, int height, size_t key_capacity
     out->dvalB = (uint32_t*)(b + o_dvalB);
     out->tkeyB = (uint32_t*)(b + o_tkeyB);
     out->tvalB = (uint32_t*)(b + o_tvalB);
-    out->hit = (uint8_t*)(b + o_hit);
+    out->blist = (uint2*)(b + o_hit);
     out->hist = (uint32_t*)(b + o_hist);
     out->digit_total = (uint32_t*)(b + o_dtot);
     out->tcount = (uint32_t*)(b + o_tcount);
@@ -150,7 +150,7 @@ int ocgs_check(const void* ws, void* stream, ocgs_header* header_out) {
   OCGS_CUDA_OK(cudaMemcpyAsync(&h, ws, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
   OCGS_CUDA_OK(cudaStreamSynchronize((cudaStream_t)stream));
   if (header_out) *header_out = h;
-  return (h.error & 1u) ? OCGS_ERR_CAPACITY : OCGS_OK;
+  return (h.error & 1u) ? OCGS_ERR_CAPACITY : (h.error & 2u) ? OCGS_ERR_UNSUPPORTED : OCGS_OK;
 }
 
 int ocgs_preprocess(const ocgs_surfels* s, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, void* stream) {

@@ -59,12 +59,13 @@ struct Workspace {
   // scratch
   uint32_t* dkeyA; uint32_t* dkeyB; uint32_t* dvalB;  // depth sort ping-pong (dvalA == rank_to_id)
   uint32_t* tkeyB; uint32_t* tvalB;                   // tile sort ping-pong
-  uint8_t* hit;                                       // [key_capacity] per list entry: bit w = warp w of the tile blended it (fwd -> bwd)
+  uint2* blist;                                       // [key_capacity] per tile, at its list offset: the entries some warp blended, in list order:
+                                                      // x = rank, y = (position in the tile list << 8) | bit w: warp block w blended it (fwd -> bwd)
   uint32_t* hist;                                     // [4 passes][max_blocks][kRadix] look-back status words of the radix passes
   uint32_t* digit_total;                              // [4][kRadix] global digit histograms + [4] tile tickets
   uint32_t* tcount;                                   // [N] tiles touched by rank
   uint32_t* blocksum;                                 // [ceil(N/1024)+1]
-  uint32_t* tile_work;                                // [n_tiles] forward: list length; backward: max n_contrib of the tile
+  uint32_t* tile_work;                                // [n_tiles] forward: list length; backward: number of blended entries of the tile
   uint32_t* tile_order;                               // [n_tiles] tiles in descending order of work (heavy tiles first)
   int n, width, height, tiles_x, tiles_y, n_tiles;
   size_t key_capacity;

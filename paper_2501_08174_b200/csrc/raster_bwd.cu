@@ -134,7 +134,7 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
 #endif
 __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
-                                                            const float4* __restrict__ rec, const uint8_t* __restrict__ hit, const uint8_t* __restrict__ mask,
+                                                            const float4* __restrict__ rec, const uint2* __restrict__ blist, const uint8_t* __restrict__ mask,
                                                             const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
                                                             const float* __restrict__ gC, const float* __restrict__ gA,
                                                             const float* __restrict__ gD, const float* __restrict__ gN, int W, int H,
@@ -142,10 +142,11 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
   __shared__ float4 s_rec[kBwdBatch * 6];
   __shared__ uint32_t s_rank[kBwdBatch];
   __shared__ uint8_t s_mask[kBwdBatch];
+  __shared__ uint32_t s_idx[kBwdBatch];   // position of the entry in the tile's full list (n_contrib counts those)
   __shared__ float s_acc[4][kBwdBatch * kNG];
   static_assert(kBwdBatch == 64, "the per-warp entry masks below cover two 32-entry halves");
   const int tile = (int)tile_order[blockIdx.x];  // heavy tiles are launched first
-  const uint32_t mx = tile_work[tile];           // max n_contrib of the tile (written by the forward pass)
+  const uint32_t mx = tile_work[tile];           // length of the tile's blended list (written by the forward pass)
   if (mx == 0) return;
   const int tx = tile % tiles_x, ty = tile / tiles_x;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -187,8 +188,10 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
     const int cnt = (int)min((uint32_t)kBwdBatch, mx - b0);
     __syncthreads();  // previous batch fully flushed before s_rank / s_mask / s_acc are reused
     if ((int)threadIdx.x < cnt) {
-      s_rank[threadIdx.x] = list[start + b0 + threadIdx.x];
-      s_mask[threadIdx.x] = hit[start + b0 + threadIdx.x];  // bit s: strip s of the tile blended this entry in the forward pass
+      const uint2 be = blist[start + b0 + threadIdx.x];
+      s_rank[threadIdx.x] = be.x;
+      s_mask[threadIdx.x] = (uint8_t)(be.y & 0xFFu);  // bit w: warp block w of the tile blended this entry in the forward pass
+      s_idx[threadIdx.x] = be.y >> 8;
     }
     __syncthreads();
     for (int i = threadIdx.x; i < cnt * 6; i += 128) {
@@ -209,7 +212,7 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
         todo &= ~(1u << jb);
         const int j = 32 * half + jb;
         const float4* sr = s_rec + 6 * j;
-        const uint32_t idx = b0 + (uint32_t)j;
+        const uint32_t idx = s_idx[j];
         const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
         float v[16];
 #pragma unroll
@@ -409,7 +412,7 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
     int rc = launch_order_tiles(w, /*from_ranges=*/false, st);  // tile_work = max n_contrib per tile, from the forward pass
     if (rc != OCGS_OK) return rc;
     const float goh = mask ? (float)((double)cfg.gamma_bg / ((double)cam.W * (double)cam.H)) : 0.f;
-    render_bwd_kernel<<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.hit, mask, final_T, n_contrib, gC, gA, gD, gN,
+    render_bwd_kernel<<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN,
                                                  cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
     OCGS_LAUNCHED(st, "render_bwd_kernel");
   }

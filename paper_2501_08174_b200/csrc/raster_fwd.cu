@@ -56,7 +56,7 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
                                                          const uint8_t* __restrict__ mask, int W, int H, int tiles_x,
                                                          ocgs_config cfg, float* __restrict__ color, float* __restrict__ alpha,
                                                          float* __restrict__ depth, float* __restrict__ normal,
-                                                         uint32_t* __restrict__ n_contrib, float* __restrict__ final_T, uint8_t* __restrict__ hit, float* __restrict__ loss_partial,
+                                                         uint32_t* __restrict__ n_contrib, float* __restrict__ final_T, uint2* __restrict__ blist, ocgs_header* __restrict__ header, float* __restrict__ loss_partial,
                                                          uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum) {
   __shared__ float4 s_rec[kFwdBatch * 6];
   __shared__ uint32_t s_rank[kFwdBatch];
@@ -64,9 +64,7 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
   __shared__ uint32_t s_cnt[kStats ? kFwdBatch : 1];
   __shared__ unsigned long long s_fix[kStats ? kFwdBatch : 1];  // sum of alpha*T in 2^-27 fixed point
   __shared__ float s_red[8];
-  __shared__ uint32_t s_maxc;
-  if (threadIdx.x == 0) s_maxc = 0;
-  __syncthreads();
+  __shared__ uint32_t s_wcnt[8];
 
   const int tile = (int)tile_order[blockIdx.x];  // heavy tiles are launched first
   const int tx = tile % tiles_x, ty = tile / tiles_x;
@@ -85,6 +83,7 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
 
   float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f;
   uint32_t last = 0;
+  uint32_t nhit = 0;  // entries of this tile blended so far (uniform across the CTA)
   bool done = !inside;
 
   for (uint32_t b0 = start; b0 < end; b0 += kFwdBatch) {
@@ -166,7 +165,23 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
       }
     }
     __syncthreads();
-    if ((int)threadIdx.x < cnt) hit[b0 + threadIdx.x] = (uint8_t)s_hit[threadIdx.x];
+    {  // append the entries some warp blended to the tile's blended list (walked back to front by render_bwd)
+      const bool hitme = (int)threadIdx.x < cnt && s_hit[threadIdx.x] != 0;
+      const unsigned bal = __ballot_sync(0xFFFFFFFFu, hitme);
+      if (lane == 0) s_wcnt[threadIdx.x >> 5] = (uint32_t)__popc(bal);
+      __syncthreads();
+      uint32_t before = 0, total = 0;
+#pragma unroll
+      for (int w2 = 0; w2 < 8; ++w2) {
+        const uint32_t c = s_wcnt[w2];
+        if (w2 < (int)(threadIdx.x >> 5)) before += c;
+        total += c;
+      }
+      if (hitme)
+        blist[start + nhit + before + (uint32_t)__popc(bal & ((1u << lane) - 1u))] =
+            make_uint2(s_rank[threadIdx.x], (((b0 - start) + threadIdx.x) << 8) | s_hit[threadIdx.x]);
+      nhit += total;
+    }
     if (kStats) {
       if ((int)threadIdx.x < cnt && s_cnt[threadIdx.x] > 0) {
         const uint32_t id = rank_to_id[s_rank[threadIdx.x]];
@@ -186,13 +201,9 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
     n_contrib[p] = last;
     final_T[p] = T;
   }
-  {  // per-tile max n_contrib: the backward pass's work estimate and loop bound
-    uint32_t mxl = last;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) mxl = max(mxl, __shfl_xor_sync(0xFFFFFFFFu, mxl, o));
-    if (mxl && lane == 0) atomicMax(&s_maxc, mxl);
-    __syncthreads();
-    if (threadIdx.x == 0) tile_work[tile] = s_maxc;
+  if (threadIdx.x == 0) {
+    tile_work[tile] = nhit;  // length of the blended list: the backward pass's loop bound and work estimate
+    if (end - start >= (1u << 24)) atomicOr(&header->error, 2u);  // list positions are packed into 24 bits of blist.y
   }
   if (loss_partial) {  // Eq. 1: A (1 - M), fixed-order reduction -> deterministic
     float lb = 0.f;
@@ -235,10 +246,10 @@ int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Worksp
   float* lp = loss_bg ? w.loss_partial : nullptr;
   if (stats)
     render_fwd_kernel<true><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, mask, cam.W, cam.H,
-                                                       cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, w.hit, lp, vis_count, contrib_sum);
+                                                       cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, w.blist, w.header, lp, vis_count, contrib_sum);
   else
     render_fwd_kernel<false><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, mask, cam.W, cam.H,
-                                                        cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, w.hit, lp, nullptr, nullptr);
+                                                        cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib, w.final_T, w.blist, w.header, lp, nullptr, nullptr);
   OCGS_LAUNCHED(st, "render_fwd_kernel");
   if (loss_bg) {
     loss_final_kernel<<<1, 1024, 0, st>>>(w.loss_partial, w.n_tiles, (float)(1.0 / ((double)cam.W * (double)cam.H)), loss_bg);
