@@ -177,6 +177,19 @@ int ocgs_prune_stats(const ocgs_surfels* in, uint32_t* vis_count, float* contrib
 int ocgs_masked_l1(const float* color, const float* target, const uint8_t* mask, int width, int height, float* dL_dcolor,
                    float* loss, void* ws, int n, size_t key_capacity, void* stream);
 
+/* ---- masked photometric loss L_c^M (Eq. 2) ---------------------------------------
+ * L_c^M = L_c(I M, R M) with L_c = (1 - lambda) mean|x - y| + lambda (1 - mean SSIM(x, y)): the loss the paper takes from
+ * "Equation 7 in the 3DGS paper" (reading S20b of DESIGN.md: SSIM of Wang et al. 2004 per channel over an
+ * 11x11 Gaussian window, sigma 1.5, zero padding, C1 = 0.01^2, C2 = 0.03^2, both means over all 3 H W values).
+ * color, target: device f32 [3,H,W]; mask: device u8 [H,W], nullable (= all ones), non-zero = object.
+ * dL_dcolor: device f32 [3,H,W], OVERWRITTEN with dL_c^M/dcolor (zero outside the mask).
+ * loss: device f32[3] or NULL; receives (L_c^M, its L1 term mean|x-y|, its D-SSIM term 1 - mean SSIM), deterministic.
+ * scratch: device memory of at least ocgs_photometric_workspace_bytes(width, height), caller-owned, 256-B aligned.
+ * Asynchronous on `stream`; returns OCGS_ERR_INVALID_ARG on null pointers / non-positive sizes / lambda outside [0,1]. */
+size_t ocgs_photometric_workspace_bytes(int width, int height);
+int ocgs_photometric_loss(const float* color, const float* target, const uint8_t* mask, int width, int height,
+                          float lambda_dssim, float* dL_dcolor, float* loss, void* scratch, void* stream);
+
 /* ---- diagnostics: per-launch device timing ----------------------------------------------------------------------------
  * Between ocgs_profile_begin and ocgs_profile_end every kernel (and memset) the library enqueues from the calling thread
  * is followed by a CUDA event; ocgs_profile_end synchronises `stream` and returns, for each launch in order, the

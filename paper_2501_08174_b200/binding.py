@@ -18,7 +18,8 @@ _LIB_PATH = os.path.join(_HERE, "csrc", "libocgs.so")
 OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
            "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_prune_workspace_bytes",
-           "ocgs_prune_stats", "ocgs_step_host", "ocgs_masked_l1", "ocgs_profile_begin", "ocgs_profile_end"]
+           "ocgs_prune_stats", "ocgs_step_host", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss",
+           "ocgs_profile_begin", "ocgs_profile_end"]
 
 
 class OcgsError(RuntimeError):
@@ -74,6 +75,7 @@ def lib():
         _lib = C.CDLL(_LIB_PATH)
         _lib.ocgs_workspace_bytes.restype = C.c_size_t
         _lib.ocgs_prune_workspace_bytes.restype = C.c_size_t
+        _lib.ocgs_photometric_workspace_bytes.restype = C.c_size_t
         for name in EXPORTS:
             getattr(_lib, name)  # raises AttributeError if a declared symbol is not exported
     return _lib
@@ -198,6 +200,16 @@ def ocgs_step_host(h_pos, h_scale, h_quat, h_opacity, h_sh, n, cam, cfg, h_mask,
 def ocgs_masked_l1(color, target, mask, width, height, dL_dcolor, loss, ws, n, key_capacity, stream=None):
     _ok("ocgs_masked_l1", lib().ocgs_masked_l1(_ptr(color), _ptr(target), _ptr(mask), C.c_int(width), C.c_int(height), _ptr(dL_dcolor),
                                                _ptr(loss), _ptr(ws), C.c_int(n), C.c_size_t(key_capacity), _stream(stream)))
+
+
+def ocgs_photometric_workspace_bytes(width: int, height: int) -> int:
+    return int(lib().ocgs_photometric_workspace_bytes(C.c_int(width), C.c_int(height)))
+
+
+def ocgs_photometric_loss(color, target, mask, width, height, lambda_dssim, dL_dcolor, loss, scratch, stream=None):
+    _ok("ocgs_photometric_loss", lib().ocgs_photometric_loss(_ptr(color), _ptr(target), _ptr(mask), C.c_int(width), C.c_int(height),
+                                                             C.c_float(lambda_dssim), _ptr(dL_dcolor), _ptr(loss), _ptr(scratch),
+                                                             _stream(stream)))
 
 
 def ocgs_profile_begin(capacity: int, stream=None):

@@ -211,6 +211,16 @@ int ocgs_masked_l1(const float* color, const float* target, const uint8_t* mask,
   return launch_masked_l1(color, target, mask, width, height, dL_dcolor, loss, w.loss_partial, w.n_tiles, (cudaStream_t)stream);
 }
 
+size_t ocgs_photometric_workspace_bytes(int width, int height) { return photometric_workspace_bytes(width, height); }
+
+int ocgs_photometric_loss(const float* color, const float* target, const uint8_t* mask, int width, int height, float lambda_dssim,
+                          float* dL_dcolor, float* loss, void* scratch, void* stream) {
+  if (!color || !target || !dL_dcolor || !scratch || width <= 0 || height <= 0) return OCGS_ERR_INVALID_ARG;
+  if (!(lambda_dssim >= 0.f && lambda_dssim <= 1.f)) return OCGS_ERR_INVALID_ARG;
+  if (width > OCGS_MAX_DIM || height > OCGS_MAX_DIM) return OCGS_ERR_UNSUPPORTED;
+  return launch_photometric(color, target, mask, width, height, lambda_dssim, dL_dcolor, loss, scratch, (cudaStream_t)stream);
+}
+
 int ocgs_profile_begin(int capacity, void* stream) {
   if (capacity <= 0) return OCGS_ERR_INVALID_ARG;
   while ((int)g_prof.ev.size() < capacity + 1) {

@@ -108,6 +108,10 @@ int launch_prune(const ocgs_surfels& in, uint32_t* vis_count, float* contrib_sum
 int launch_masked_l1(const float* color, const float* target, const uint8_t* mask, int W, int H, float* dL_dcolor, float* loss,
                      float* partial, int n_partial, cudaStream_t st);
 
+size_t photometric_workspace_bytes(int W, int H);
+int launch_photometric(const float* color, const float* target, const uint8_t* mask, int W, int H, float lam, float* dL_dcolor,
+                       float* loss, void* scratch, cudaStream_t st);
+
 // tile_order <- tiles sorted by descending tile_work (bucketed; launch order of the raster CTAs)
 int launch_order_tiles(const Workspace& w, bool from_ranges, cudaStream_t st);
 
