@@ -43,41 +43,62 @@ __global__ void __launch_bounds__(256) ssim_terms_kernel(const float* __restrict
     s_y[ry][rx] = masked_load(I, mask, x0 + rx - kPH, y0 + ry - kPH, W, H);
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < kPR * kPT; i += 256) {
-    const int ry = i / kPT, ox = i - ry * kPT;
-    float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, a4 = 0.f;
+  // horizontal pass, 8 adjacent outputs per thread: 18 staged values feed 8 x 11 taps (one map at a time)
+  for (int i = threadIdx.x; i < kPR * (kPT / 8); i += 256) {
+    const int ry = i / (kPT / 8), ox0 = (i - ry * (kPT / 8)) * 8;
+    float xs[18], ys[18];
 #pragma unroll
-    for (int t = 0; t < 11; ++t) {
-      const float xv = s_x[ry][ox + t], yv = s_y[ry][ox + t], g = taps.g[t];
-      a0 = fmaf(g, xv, a0); a1 = fmaf(g, yv, a1);
-      a2 = fmaf(g, xv * xv, a2); a3 = fmaf(g, yv * yv, a3); a4 = fmaf(g, xv * yv, a4);
+    for (int t = 0; t < 18; ++t) { xs[t] = s_x[ry][ox0 + t]; ys[t] = s_y[ry][ox0 + t]; }
+#pragma unroll
+    for (int m = 0; m < 5; ++m) {
+      float v[18];
+#pragma unroll
+      for (int t = 0; t < 18; ++t) v[t] = m == 0 ? xs[t] : m == 1 ? ys[t] : m == 2 ? xs[t] * xs[t] : m == 3 ? ys[t] * ys[t] : xs[t] * ys[t];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        float a = 0.f;
+#pragma unroll
+        for (int t = 0; t < 11; ++t) a = fmaf(taps.g[t], v[k + t], a);
+        s_h[m][ry][ox0 + k] = a;
+      }
     }
-    s_h[0][ry][ox] = a0; s_h[1][ry][ox] = a1; s_h[2][ry][ox] = a2; s_h[3][ry][ox] = a3; s_h[4][ry][ox] = a4;
   }
   __syncthreads();
   double l1 = 0.0, ss = 0.0;
-  for (int i = threadIdx.x; i < kPT * kPT; i += 256) {
-    const int oy = i / kPT, ox = i - oy * kPT;
-    const int ix = x0 + ox, iy = y0 + oy;
-    if (ix >= W || iy >= H) continue;
-    float mx = 0.f, my = 0.f, exx = 0.f, eyy = 0.f, exy = 0.f;
+  // vertical pass, 4 vertically adjacent outputs per thread: 14 values per map feed 4 x 11 taps
+  for (int i = threadIdx.x; i < kPT * (kPT / 4); i += 256) {
+    const int ox = i % kPT, oy0 = (i / kPT) * 4;
+    float bl[5][4];
 #pragma unroll
-    for (int t = 0; t < 11; ++t) {
-      const float g = taps.g[t];
-      mx = fmaf(g, s_h[0][oy + t][ox], mx); my = fmaf(g, s_h[1][oy + t][ox], my);
-      exx = fmaf(g, s_h[2][oy + t][ox], exx); eyy = fmaf(g, s_h[3][oy + t][ox], eyy); exy = fmaf(g, s_h[4][oy + t][ox], exy);
+    for (int m = 0; m < 5; ++m) {
+      float v[14];
+#pragma unroll
+      for (int t = 0; t < 14; ++t) v[t] = s_h[m][oy0 + t][ox];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        float a = 0.f;
+#pragma unroll
+        for (int t = 0; t < 11; ++t) a = fmaf(taps.g[t], v[k + t], a);
+        bl[m][k] = a;
+      }
     }
-    const float sxx = exx - mx * mx, syy = eyy - my * my, sxy = exy - mx * my;
-    const float A1 = fmaf(2.0f * mx, my, 1e-4f), A2 = fmaf(2.0f, sxy, 9e-4f);
-    const float B1 = fmaf(mx, mx, fmaf(my, my, 1e-4f)), B2 = sxx + syy + 9e-4f;
-    const float iB1 = 1.0f / B1, iB2 = 1.0f / B2, iB = iB1 * iB2;
-    const float S = A1 * A2 * iB;
-    const size_t p = (size_t)c * HW + (size_t)iy * W + ix;
-    d_mu[p] = gS * (2.0f * my * (A2 - A1) * iB - 2.0f * mx * S * (iB1 - iB2));
-    d_xx[p] = gS * (-S * iB2);
-    d_xy[p] = gS * (2.0f * A1 * iB);
-    l1 += (double)fabsf(s_x[oy + kPH][ox + kPH] - s_y[oy + kPH][ox + kPH]);
-    ss += (double)S;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int oy = oy0 + k, ix = x0 + ox, iy = y0 + oy;
+      if (ix >= W || iy >= H) continue;
+      const float mx = bl[0][k], my = bl[1][k], exx = bl[2][k], eyy = bl[3][k], exy = bl[4][k];
+      const float sxx = exx - mx * mx, syy = eyy - my * my, sxy = exy - mx * my;
+      const float A1 = fmaf(2.0f * mx, my, 1e-4f), A2 = fmaf(2.0f, sxy, 9e-4f);
+      const float B1 = fmaf(mx, mx, fmaf(my, my, 1e-4f)), B2 = sxx + syy + 9e-4f;
+      const float iB1 = 1.0f / B1, iB2 = 1.0f / B2, iB = iB1 * iB2;
+      const float S = A1 * A2 * iB;
+      const size_t p = (size_t)c * HW + (size_t)iy * W + ix;
+      d_mu[p] = gS * (2.0f * my * (A2 - A1) * iB - 2.0f * mx * S * (iB1 - iB2));
+      d_xx[p] = gS * (-S * iB2);
+      d_xy[p] = gS * (2.0f * A1 * iB);
+      l1 += (double)fabsf(s_x[oy + kPH][ox + kPH] - s_y[oy + kPH][ox + kPH]);
+      ss += (double)S;
+    }
   }
   // block partials (fixed order -> deterministic totals)
 #pragma unroll
@@ -111,36 +132,53 @@ __global__ void __launch_bounds__(256) ssim_grad_kernel(const float* __restrict_
     for (int k = 0; k < 3; ++k) s_in[k][ry][rx] = in ? src[k][p] : 0.f;
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < kPR * kPT; i += 256) {
-    const int ry = i / kPT, ox = i - ry * kPT;
-    float a0 = 0.f, a1 = 0.f, a2 = 0.f;
+  for (int i = threadIdx.x; i < kPR * (kPT / 8); i += 256) {
+    const int ry = i / (kPT / 8), ox0 = (i - ry * (kPT / 8)) * 8;
 #pragma unroll
-    for (int t = 0; t < 11; ++t) {
-      const float g = taps.g[t];
-      a0 = fmaf(g, s_in[0][ry][ox + t], a0); a1 = fmaf(g, s_in[1][ry][ox + t], a1); a2 = fmaf(g, s_in[2][ry][ox + t], a2);
+    for (int m = 0; m < 3; ++m) {
+      float v[18];
+#pragma unroll
+      for (int t = 0; t < 18; ++t) v[t] = s_in[m][ry][ox0 + t];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        float a = 0.f;
+#pragma unroll
+        for (int t = 0; t < 11; ++t) a = fmaf(taps.g[t], v[k + t], a);
+        s_h[m][ry][ox0 + k] = a;
+      }
     }
-    s_h[0][ry][ox] = a0; s_h[1][ry][ox] = a1; s_h[2][ry][ox] = a2;
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < kPT * kPT; i += 256) {
-    const int oy = i / kPT, ox = i - oy * kPT;
-    const int ix = x0 + ox, iy = y0 + oy;
-    if (ix >= W || iy >= H) continue;
-    float b0 = 0.f, b1 = 0.f, b2 = 0.f;
+  for (int i = threadIdx.x; i < kPT * (kPT / 4); i += 256) {
+    const int ox = i % kPT, oy0 = (i / kPT) * 4;
+    float bl[3][4];
 #pragma unroll
-    for (int t = 0; t < 11; ++t) {
-      const float g = taps.g[t];
-      b0 = fmaf(g, s_h[0][oy + t][ox], b0); b1 = fmaf(g, s_h[1][oy + t][ox], b1); b2 = fmaf(g, s_h[2][oy + t][ox], b2);
+    for (int m = 0; m < 3; ++m) {
+      float v[14];
+#pragma unroll
+      for (int t = 0; t < 14; ++t) v[t] = s_h[m][oy0 + t][ox];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        float a = 0.f;
+#pragma unroll
+        for (int t = 0; t < 11; ++t) a = fmaf(taps.g[t], v[k + t], a);
+        bl[m][k] = a;
+      }
     }
-    const size_t pp = (size_t)iy * W + ix;
-    const bool m = mask == nullptr || mask[pp] != 0;
-    float out = 0.f;
-    if (m) {  // x = R M: no gradient reaches the render outside the mask
-      const float x = color[(size_t)c * HW + pp], y = target[(size_t)c * HW + pp];
-      const float d = x - y;
-      out = b0 + 2.0f * x * b1 + y * b2 + (d > 0.f ? l1_scale : (d < 0.f ? -l1_scale : 0.f));
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int ix = x0 + ox, iy = y0 + oy0 + k;
+      if (ix >= W || iy >= H) continue;
+      const size_t pp = (size_t)iy * W + ix;
+      const bool m = mask == nullptr || mask[pp] != 0;
+      float out = 0.f;
+      if (m) {  // x = R M: no gradient reaches the render outside the mask
+        const float x = color[(size_t)c * HW + pp], y = target[(size_t)c * HW + pp];
+        const float d = x - y;
+        out = bl[0][k] + 2.0f * x * bl[1][k] + y * bl[2][k] + (d > 0.f ? l1_scale : (d < 0.f ? -l1_scale : 0.f));
+      }
+      dL_dcolor[(size_t)c * HW + pp] = out;
     }
-    dL_dcolor[(size_t)c * HW + pp] = out;
   }
 }
 
