@@ -158,6 +158,21 @@ int ocgs_render_bwd(const ocgs_surfels* surfels, const ocgs_camera* cam, const o
                     const float* dL_dalpha, const float* dL_ddepth, const float* dL_dnormal, float* d_pos, float* d_scale,
                     float* d_quat, float* d_opacity, float* d_sh, float* d_center2d, void* stream);
 
+/* ---- (3b)/(4b) forward / backward with the squared-depth moment map (reading R-moments) -----
+ * The 2DGS regularisers the paper keeps unchanged (depth distortion L_d, normal consistency L_n) are
+ * image-space functions of the rendered maps once the renderer also accumulates depth2 = sum_i w_i z_i^2 (w_i = alpha_i T_i,
+ * z_i the pair's depth as written to `depth`): sum_{i<j} w_i w_j (z_i - z_j)^2 = alpha * depth2 - depth^2 per pixel.
+ * ocgs_render_fwd_reg = ocgs_render_fwd + depth2 (device f32 [H,W], nullable = plain forward).
+ * ocgs_render_bwd_reg = ocgs_render_bwd + dL_ddepth2 (device f32 [H,W], nullable), the upstream gradient of depth2.
+ * ocgs_regularizers (below) evaluates L_d, L_n and the upstream gradients these calls consume. */
+int ocgs_render_fwd_reg(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
+                        float* color, float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg,
+                        uint32_t* vis_count, float* contrib_sum, float* depth2, void* stream);
+int ocgs_render_bwd_reg(const ocgs_surfels* surfels, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
+                        const uint8_t* mask, const uint32_t* n_contrib, const float* dL_dcolor, const float* dL_dalpha,
+                        const float* dL_ddepth, const float* dL_dnormal, const float* dL_ddepth2, float* d_pos, float* d_scale,
+                        float* d_quat, float* d_opacity, float* d_sh, float* d_center2d, void* stream);
+
 /* ---- (5) prune statistics -> mask -> stream compaction ----------------------------------------------------------------
  * "We propose to assign both G_j and G_k with false" -- a surfel that was never blended in any render
  * of the interval is removed whether it was outside the frustum or occluded; PAPER.md:101 (opacity threshold), S17.

@@ -17,7 +17,7 @@ _LIB_PATH = os.path.join(_HERE, "csrc", "libocgs.so")
 
 OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
-           "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_prune_workspace_bytes",
+           "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_render_fwd_reg", "ocgs_render_bwd_reg", "ocgs_prune_workspace_bytes",
            "ocgs_prune_stats", "ocgs_step_host", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss",
            "ocgs_profile_begin", "ocgs_profile_end"]
 
@@ -165,6 +165,21 @@ def ocgs_render_fwd(n, cam, cfg, ws, key_capacity, mask, color, alpha, depth, no
     _ok("ocgs_render_fwd", lib().ocgs_render_fwd(C.c_int(n), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity), _ptr(mask),
                                                  _ptr(color), _ptr(alpha), _ptr(depth), _ptr(normal), _ptr(n_contrib), _ptr(loss_bg),
                                                  _ptr(vis_count), _ptr(contrib_sum), _stream(stream)))
+
+
+def ocgs_render_fwd_reg(n, cam, cfg, ws, key_capacity, mask, color, alpha, depth, normal, n_contrib, loss_bg, vis_count, contrib_sum,
+                        depth2, stream=None):
+    _ok("ocgs_render_fwd_reg", lib().ocgs_render_fwd_reg(C.c_int(n), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity),
+                                                         _ptr(mask), _ptr(color), _ptr(alpha), _ptr(depth), _ptr(normal), _ptr(n_contrib),
+                                                         _ptr(loss_bg), _ptr(vis_count), _ptr(contrib_sum), _ptr(depth2), _stream(stream)))
+
+
+def ocgs_render_bwd_reg(surfels, cam, cfg, ws, key_capacity, mask, n_contrib, dL_dcolor, dL_dalpha, dL_ddepth, dL_dnormal, dL_ddepth2,
+                        d_pos, d_scale, d_quat, d_opacity, d_sh, d_center2d=None, stream=None):
+    _ok("ocgs_render_bwd_reg", lib().ocgs_render_bwd_reg(C.byref(surfels), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity),
+                                                         _ptr(mask), _ptr(n_contrib), _ptr(dL_dcolor), _ptr(dL_dalpha), _ptr(dL_ddepth),
+                                                         _ptr(dL_dnormal), _ptr(dL_ddepth2), _ptr(d_pos), _ptr(d_scale), _ptr(d_quat),
+                                                         _ptr(d_opacity), _ptr(d_sh), _ptr(d_center2d), _stream(stream)))
 
 
 def ocgs_render_bwd(surfels, cam, cfg, ws, key_capacity, mask, n_contrib, dL_dcolor, dL_dalpha, dL_ddepth, dL_dnormal, d_pos, d_scale,

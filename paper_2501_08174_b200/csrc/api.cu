@@ -176,9 +176,9 @@ static int carve_for_render(void* ws, int n, const ocgs_camera* cam, size_t key_
   return carve_workspace(ws, n, cam->width, cam->height, key_capacity, w, nullptr) ? OCGS_OK : OCGS_ERR_UNSUPPORTED;
 }
 
-int ocgs_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
+int ocgs_render_fwd_reg(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
                         float* color, float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg,
-                        uint32_t* vis_count, float* contrib_sum, void* stream) {
+                        uint32_t* vis_count, float* contrib_sum, float* depth2, void* stream) {
   if (!cam || !ws || !color || !alpha || !depth || !normal || !n_contrib) return OCGS_ERR_INVALID_ARG;
   int rc = check_cfg(cfg);
   if (rc != OCGS_OK) return rc;
@@ -186,12 +186,19 @@ int ocgs_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void*
   Workspace w;
   if ((rc = carve_for_render(ws, n, cam, key_capacity, &w)) != OCGS_OK) return rc;
   return launch_render_fwd(make_cam(*cam), *cfg, w, mask, color, alpha, depth, normal, n_contrib, loss_bg, vis_count, contrib_sum,
-                           (cudaStream_t)stream);
+                           depth2, (cudaStream_t)stream);
 }
 
-int ocgs_render_bwd(const ocgs_surfels* s, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
+int ocgs_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
+                        float* color, float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg,
+                        uint32_t* vis_count, float* contrib_sum, void* stream) {
+  return ocgs_render_fwd_reg(n, cam, cfg, ws, key_capacity, mask, color, alpha, depth, normal, n_contrib, loss_bg, vis_count,
+                             contrib_sum, nullptr, stream);
+}
+
+int ocgs_render_bwd_reg(const ocgs_surfels* s, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
                         const uint8_t* mask, const uint32_t* n_contrib, const float* gC, const float* gA, const float* gD,
-                        const float* gN, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
+                        const float* gN, const float* gD2, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
                         float* d_center2d, void* stream) {
   if (!s || !cam || !ws || !n_contrib) return OCGS_ERR_INVALID_ARG;
   int rc = check_cfg(cfg);
@@ -199,8 +206,16 @@ int ocgs_render_bwd(const ocgs_surfels* s, const ocgs_camera* cam, const ocgs_co
   if (s->n > 0 && (!d_pos || !d_scale || !d_quat || !d_opacity || !d_sh)) return OCGS_ERR_INVALID_ARG;
   Workspace w;
   if ((rc = carve_for_render(ws, s->n, cam, key_capacity, &w)) != OCGS_OK) return rc;
-  return launch_render_bwd(*s, make_cam(*cam), *cfg, w, mask, w.final_T, n_contrib, gC, gA, gD, gN, d_pos, d_scale, d_quat, d_opacity,
-                           d_sh, d_center2d, (cudaStream_t)stream);
+  return launch_render_bwd(*s, make_cam(*cam), *cfg, w, mask, w.final_T, n_contrib, gC, gA, gD, gN, gD2, d_pos, d_scale, d_quat,
+                           d_opacity, d_sh, d_center2d, (cudaStream_t)stream);
+}
+
+int ocgs_render_bwd(const ocgs_surfels* s, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
+                        const uint8_t* mask, const uint32_t* n_contrib, const float* gC, const float* gA, const float* gD,
+                        const float* gN, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
+                        float* d_center2d, void* stream) {
+  return ocgs_render_bwd_reg(s, cam, cfg, ws, key_capacity, mask, n_contrib, gC, gA, gD, gN, nullptr, d_pos, d_scale, d_quat, d_opacity,
+                             d_sh, d_center2d, stream);
 }
 
 int ocgs_masked_l1(const float* color, const float* target, const uint8_t* mask, int width, int height, float* dL_dcolor, float* loss,

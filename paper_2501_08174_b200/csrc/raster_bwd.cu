@@ -64,6 +64,7 @@ struct BwdPixel {
   float T;                         // running transmittance T_i
   float GS;                        // sum_c g_c S_c - gA T_final: upstream gradients dotted with the suffix sums behind the pair
   float gc0, gc1, gc2, gd, gn0, gn1, gn2;
+  float gd2;                       // upstream of depth2 = sum w z^2 (kMoments only)
   uint32_t last;                   // n_contrib (0 for pixels outside the image)
 };
 
@@ -73,6 +74,7 @@ struct BwdConsts { float near_z, alpha_max, inv_sigma2; };
 // With Q_c the accumulated maps, q_c this pair's values (rgb, z, n), S_c the suffix sums behind it (O7):
 //   dL/dalpha_i = sum_c g_c (q_c T_i - S_c/(1-alpha_i)) + gA T_final/(1-alpha_i) = T_i (g.q) - (g.S - gA T_final)/(1-alpha_i),
 // and g.S advances by w_i (g.q): one running scalar GS replaces the seven suffix sums.
+template <bool kMoments>
 __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4 r0, const float4 r1, const float4 r2, const float4 r3,
                                          const float4* __restrict__ sr, const BwdConsts& k, float* v, float* ex) {
   const float dx = s.px - r2.z, dy = s.py - r2.w;
@@ -97,13 +99,15 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
     s.T *= inv1ma;  // T_i = T_{i+1} / (1 - alpha_i)
     const float T = s.T, w = a * T;
     float gq = s.gd * z;
+    if (kMoments) gq = fmaf(s.gd2 * z, z, gq);  // depth2 behaves like one more blended channel with value z^2
     gq = fmaf(s.gc0, r4.y, gq); gq = fmaf(s.gc1, r4.z, gq); gq = fmaf(s.gc2, r4.w, gq);
     gq = fmaf(s.gn0, r5.x, gq); gq = fmaf(s.gn1, r5.y, gq); gq = fmaf(s.gn2, r5.z, gq);
     const float galpha = fmaf(T, gq, -s.GS * inv1ma);
     s.GS = fmaf(w, gq, s.GS);
     v[10] = fmaf(w, s.gc0, v[10]); v[11] = fmaf(w, s.gc1, v[11]); v[12] = fmaf(w, s.gc2, v[12]);
     v[13] = fmaf(w, s.gn0, v[13]); v[14] = fmaf(w, s.gn1, v[14]); v[15] = fmaf(w, s.gn2, v[15]);
-    const float gz = w * s.gd;
+    float gz = w * s.gd;
+    if (kMoments) gz = fmaf(2.0f * z * w, s.gd2, gz);  // ... and depends on z directly
     float grho = 0.f;
     if (!capped) { v[9] = fmaf(G, galpha, v[9]); grho = -0.5f * G * r4.x * galpha; }  // S12: zero through the cap
     if (surf) {
@@ -132,12 +136,13 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
 #ifndef OCGS_BWD_MINB
 #define OCGS_BWD_MINB 5
 #endif
+template <bool kMoments>
 __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                             const float4* __restrict__ rec, const uint2* __restrict__ blist, const uint8_t* __restrict__ mask,
                                                             const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
                                                             const float* __restrict__ gC, const float* __restrict__ gA,
-                                                            const float* __restrict__ gD, const float* __restrict__ gN, int W, int H,
+                                                            const float* __restrict__ gD, const float* __restrict__ gN, const float* __restrict__ gD2, int W, int H,
                                                             int tiles_x, ocgs_config cfg, float gamma_over_hw, float* __restrict__ grad_rec) {
   __shared__ float4 s_rec[kBwdBatch * 6];
   __shared__ uint32_t s_rank[kBwdBatch];
@@ -167,7 +172,7 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
     s.px = (float)ix; s.py = (float)iy;
     s.last = 0;
     float Tfin = 1.0f, ga = 0.f;
-    s.gc0 = s.gc1 = s.gc2 = s.gd = s.gn0 = s.gn1 = s.gn2 = 0.f;
+    s.gc0 = s.gc1 = s.gc2 = s.gd = s.gn0 = s.gn1 = s.gn2 = s.gd2 = 0.f;
     if (ix < W && iy < H) {
       const size_t p = (size_t)iy * W + ix;
       s.last = n_contrib[p];
@@ -175,6 +180,7 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
       if (gC) { s.gc0 = gC[p]; s.gc1 = gC[HW + p]; s.gc2 = gC[2 * HW + p]; }
       if (gA) ga = gA[p];
       if (gD) s.gd = gD[p];
+      if (kMoments) s.gd2 = gD2[p];
       if (gN) { s.gn0 = gN[p]; s.gn1 = gN[HW + p]; s.gn2 = gN[2 * HW + p]; }
       if (mask && mask[p] == 0) ga += gamma_over_hw;  // d(gamma L_b)/dA = gamma (1-M)/(HW), Eq. 1 / Eq. 3
     }
@@ -218,8 +224,8 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
 #pragma unroll
         for (int i = 0; i < 16; ++i) v[i] = 0.f;
         float ex[4] = {0.f, 0.f, 0.f, 0.f};  // gD0, gzj, gcx, gcy
-        if ((m0 >> jb) & 1u) bwd_pair(ps[0], idx, r0, r1, r2, r3, sr, kc, v, ex);
-        if ((m1 >> jb) & 1u) bwd_pair(ps[1], idx, r0, r1, r2, r3, sr, kc, v, ex);
+        if ((m0 >> jb) & 1u) bwd_pair<kMoments>(ps[0], idx, r0, r1, r2, r3, sr, kc, v, ex);
+        if ((m1 >> jb) & 1u) bwd_pair<kMoments>(ps[1], idx, r0, r1, r2, r3, sr, kc, v, ex);
         float* dst = acc + j * kNG;
         warp_transpose_reduce16(v, lane);
         if ((lane & 1) == 0) dst[lane >> 1] = v[0];
@@ -403,7 +409,7 @@ __global__ void __launch_bounds__(128) project_bwd_kernel(const float* __restric
 
 int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, const uint8_t* mask,
                       const float* final_T, const uint32_t* n_contrib, const float* gC, const float* gA, const float* gD,
-                      const float* gN, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
+                      const float* gN, const float* gD2, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
                       float* d_center2d, cudaStream_t st) {
   if (s.n == 0) return OCGS_OK;
   clear_grad_rec_kernel<<<(unsigned)min(div_up((size_t)s.n * 6, 256), (size_t)148 * 16), 256, 0, st>>>(w.header, (float4*)w.grad_rec);
@@ -412,8 +418,12 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
     int rc = launch_order_tiles(w, /*from_ranges=*/false, st);  // tile_work = max n_contrib per tile, from the forward pass
     if (rc != OCGS_OK) return rc;
     const float goh = mask ? (float)((double)cfg.gamma_bg / ((double)cam.W * (double)cam.H)) : 0.f;
-    render_bwd_kernel<<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN,
-                                                 cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
+    if (gD2)
+      render_bwd_kernel<true><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, gD2,
+                                                         cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
+    else
+      render_bwd_kernel<false><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, nullptr,
+                                                          cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
     OCGS_LAUNCHED(st, "render_bwd_kernel");
   }
   project_bwd_kernel<<<(unsigned)div_up((size_t)s.n, 128), 128, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity,

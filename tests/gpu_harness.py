@@ -61,7 +61,7 @@ class GpuView:
             res["tile_keys"] = self.sec("tile_keys", torch.int32, max(K, 1)).view(np.uint32)[:K]
         return res
 
-    def render_fwd(self, mask=None, stats=True, vis_count=None, contrib_sum=None, want_loss=True):
+    def render_fwd(self, mask=None, stats=True, vis_count=None, contrib_sum=None, want_loss=True, moments=False):
         torch, B = self.torch, self.B
         self.out = B.alloc_outputs(self.W, self.H)
         self.mask_t = None if mask is None else torch.tensor(np.ascontiguousarray(mask, np.uint8), device="cuda")
@@ -71,8 +71,13 @@ class GpuView:
         else:
             self.vis = self.cs = None
         o = self.out
-        B.ocgs_render_fwd(self.n, self.cam, self.cfg, self.ws, self.cap, self.mask_t, o["color"], o["alpha"], o["depth"], o["normal"],
-                          o["n_contrib"], o["loss_bg"] if want_loss else None, self.vis, self.cs)
+        if moments:  # forward with the squared-depth moment map
+            o["depth2"] = torch.zeros_like(o["depth"])
+            B.ocgs_render_fwd_reg(self.n, self.cam, self.cfg, self.ws, self.cap, self.mask_t, o["color"], o["alpha"], o["depth"], o["normal"],
+                                  o["n_contrib"], o["loss_bg"] if want_loss else None, self.vis, self.cs, o["depth2"])
+        else:
+            B.ocgs_render_fwd(self.n, self.cam, self.cfg, self.ws, self.cap, self.mask_t, o["color"], o["alpha"], o["depth"], o["normal"],
+                              o["n_contrib"], o["loss_bg"] if want_loss else None, self.vis, self.cs)
         torch.cuda.synchronize()
         res = {k: v.cpu().numpy() for k, v in o.items()}
         res["n_contrib"] = res["n_contrib"].view(np.uint32)
@@ -82,15 +87,19 @@ class GpuView:
             res["contrib_sum"] = self.cs.cpu().numpy()
         return res
 
-    def render_bwd(self, gC=None, gA=None, gD=None, gN=None, mask="same"):
+    def render_bwd(self, gC=None, gA=None, gD=None, gN=None, mask="same", gD2=None):
         torch, B = self.torch, self.B
         g = B.alloc_grads(self.n)
 
         def dev(a):
             return None if a is None else torch.tensor(np.ascontiguousarray(a, np.float32), device="cuda")
         m = self.mask_t if isinstance(mask, str) else (None if mask is None else torch.tensor(np.ascontiguousarray(mask, np.uint8), device="cuda"))
-        B.ocgs_render_bwd(self.surfels, self.cam, self.cfg, self.ws, self.cap, m, self.out["n_contrib"], dev(gC), dev(gA), dev(gD), dev(gN),
-                          g["d_pos"], g["d_scale"], g["d_quat"], g["d_opacity"], g["d_sh"], g["d_center2d"])
+        if gD2 is not None:
+            B.ocgs_render_bwd_reg(self.surfels, self.cam, self.cfg, self.ws, self.cap, m, self.out["n_contrib"], dev(gC), dev(gA), dev(gD),
+                                  dev(gN), dev(gD2), g["d_pos"], g["d_scale"], g["d_quat"], g["d_opacity"], g["d_sh"], g["d_center2d"])
+        else:
+            B.ocgs_render_bwd(self.surfels, self.cam, self.cfg, self.ws, self.cap, m, self.out["n_contrib"], dev(gC), dev(gA), dev(gD), dev(gN),
+                              g["d_pos"], g["d_scale"], g["d_quat"], g["d_opacity"], g["d_sh"], g["d_center2d"])
         torch.cuda.synchronize()
         return {k: v.cpu().numpy() for k, v in g.items()}
 

@@ -122,6 +122,39 @@ def test_sh_degrees():
         full_parity(sc, 0, dict(sh_degree=deg))
 
 
+def test_depth_moment_map_and_its_gradient():
+    """SURVEY.md 8(f) f-2 / reading R-moments: ocgs_render_fwd_reg's depth2 = sum w z^2 and ocgs_render_bwd_reg's upstream
+    gradient of it, against the oracle; the other maps must be bit-identical to the plain forward."""
+    for sc, cfg_kw in ((sg.random_scene(300, 100, 70, 80.0, seed=3, sh_degree=3), dict(sh_degree=3)),
+                       (sg.make_scene("config2", n_obj=20_000, n_bg=20_000), dict(sh_degree=3))):
+        P = arrays(sc)
+        camn = sc.cameras[0]
+        m = sc.mask(0)
+        orc, cam, cfg, pre, srt, fw = oracle_view(P, camn, cfg_kw, mask=m)
+        g = GpuView(P, camn, cfg_kw)
+        g.preprocess(); g.bin_sort(want_ids=False)
+        plain = g.render_fwd(mask=m)
+        gf = g.render_fwd(mask=m, moments=True)
+        for k in ("color", "alpha", "depth", "normal", "n_contrib"):
+            assert np.array_equal(plain[k], gf[k]), k
+        ok = fw["fragile"] == 0
+        err = np.abs(gf["depth2"] - fw["depth2"]) / np.maximum(1.0, np.abs(fw["depth2"]))
+        assert (err * ok).max() <= IMG_TOL, (err * ok).max()
+        rng = np.random.default_rng(17)
+        H, W = camn.height, camn.width
+        okf = ok.astype(np.float64)
+        gC, gD, gD2 = rng.normal(size=(3, H, W)) * okf, rng.normal(size=(H, W)) * okf, rng.normal(size=(H, W)) * okf
+        mm = np.where(ok, m, 1).astype(np.uint8)
+        gg = g.render_bwd(gC=gC, gD=gD, gD2=gD2, mask=mm)
+        og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=gC.astype(np.float32), gD=gD.astype(np.float32), gD2=gD2.astype(np.float32))
+        check_grads(gg, og)
+        # the moment channel alone
+        gg2 = g.render_bwd(gD2=gD2, mask=None)
+        cfg0 = orc.default_config(sh_degree=3, gamma_bg=0.0)
+        og2 = orc.render_bwd(*P, pre, srt, cam, cfg0, mask=None, gD2=gD2.astype(np.float32))
+        check_grads(gg2, og2)
+
+
 def test_empty_and_all_culled_and_capacity():
     import torch
     from paper_2501_08174_b200 import binding as B
