@@ -173,6 +173,20 @@ int ocgs_render_bwd_reg(const ocgs_surfels* surfels, const ocgs_camera* cam, con
                         const float* dL_ddepth, const float* dL_dnormal, const float* dL_ddepth2, float* d_pos, float* d_scale,
                         float* d_quat, float* d_opacity, float* d_sh, float* d_center2d, void* stream);
 
+/* ---- regularisers of Eq. 3 (readings R-Ld, R-Ln) -------------------------
+ * L_d = 1/(HW) sum_p (alpha depth2 - depth^2) (depth distortion, squared pairwise form) and
+ * L_n = 1/(HW) sum_p (alpha - normal . Nhat) (normal consistency; Nhat = camera-facing unit normal of the expected-depth
+ * surface depth/alpha by central differences of the back-projected points, zero on the image border and next to pixels
+ * with alpha <= 1e-4), unmasked.  Inputs: the maps of ocgs_render_fwd_reg (device f32; normal [3,H,W]) and the camera.
+ * Outputs (device f32, OVERWRITTEN): dL_dalpha[H,W], dL_ddepth[H,W], dL_ddepth2[H,W], dL_dnormal[3,H,W] = gradients of
+ * w_d L_d + w_n L_n (pass them to ocgs_render_bwd_reg, adding other losses' gradients first if there are any);
+ * loss: device f32[2] or NULL <- (L_d, L_n), unweighted, deterministic.
+ * scratch: device memory of at least ocgs_regularizers_workspace_bytes(width, height), 256-B aligned. */
+size_t ocgs_regularizers_workspace_bytes(int width, int height);
+int ocgs_regularizers(const float* alpha, const float* depth, const float* depth2, const float* normal, const ocgs_camera* cam,
+                      float w_d, float w_n, float* dL_dalpha, float* dL_ddepth, float* dL_ddepth2, float* dL_dnormal, float* loss,
+                      void* scratch, void* stream);
+
 /* ---- (5) prune statistics -> mask -> stream compaction ----------------------------------------------------------------
  * "We propose to assign both G_j and G_k with false" -- a surfel that was never blended in any render
  * of the interval is removed whether it was outside the frustum or occluded; PAPER.md:101 (opacity threshold), S17.

@@ -153,7 +153,7 @@ def render_fwd(pre, srt, opacity, cam: OrcCamera, cfg: OrcConfig, mask=None, win
     opacity = _f32(opacity)
     x0, y0, x1, y1 = window if window is not None else (0, 0, W, H)
     out = dict(color=np.zeros((3, H, W)), alpha=np.zeros((H, W)), depth=np.zeros((H, W)), normal=np.zeros((3, H, W)),
-               n_contrib=np.zeros((H, W), np.uint32), depth2=np.zeros((H, W)))
+               n_contrib=np.zeros((H, W), np.uint32), origin=np.zeros((H, W)), m1=np.zeros((H, W)), m2=np.zeros((H, W)))
     if vis_count is None:
         vis_count = np.zeros(n, np.uint32)
     if contrib_sum is None:
@@ -169,13 +169,13 @@ def render_fwd(pre, srt, opacity, cam: OrcCamera, cfg: OrcConfig, mask=None, win
                               _p(pre["M"]), _p(pre["c2d"]), _p(pre["rho_cut"]), _p(opacity), _p(pre["normal"]), _p(pre["rgb"]),
                               _p(ids), _p(srt["ranges"]), _p(m), C.c_int(x0), C.c_int(y0), C.c_int(x1), C.c_int(y1),
                               _p(out["color"]), _p(out["alpha"]), _p(out["depth"]), _p(out["normal"]), _p(out["n_contrib"]),
-                              _p(vis_count), _p(contrib_sum), _p(fragile), _p(ftouch), _p(cond_rho), _p(out["depth2"]))
+                              _p(vis_count), _p(contrib_sum), _p(fragile), _p(ftouch), _p(cond_rho), _p(out["origin"]), _p(out["m1"]), _p(out["m2"]))
     out.update(loss_bg=float(Lb), vis_count=vis_count, contrib_sum=contrib_sum, fragile=fragile, fragile_touch=ftouch, cond_rho=cond_rho)
     return out
 
 
 def render_bwd(pos, scale, quat, opacity, sh, pre, srt, cam: OrcCamera, cfg: OrcConfig, mask=None, gC=None, gA=None, gD=None,
-               gN=None, window=None, gD2=None) -> Dict[str, np.ndarray]:
+               gN=None, window=None, gM1=None, gM2=None) -> Dict[str, np.ndarray]:
     pos, scale, quat, opacity, sh = _f32(pos), _f32(scale), _f32(quat), _f32(opacity), _f32(sh)
     n = pos.shape[0]
     W, H = cam.width, cam.height
@@ -185,12 +185,12 @@ def render_bwd(pos, scale, quat, opacity, sh, pre, srt, cam: OrcCamera, cfg: Orc
     oabs = np.zeros(n)
     ids = srt["ids"] if srt["K"] > 0 else np.zeros(1, np.uint32)
     m = None if mask is None else np.ascontiguousarray(mask, np.uint8)
-    gC, gA, gD, gN, gD2 = _f64(gC), _f64(gA), _f64(gD), _f64(gN), _f64(gD2)
+    gC, gA, gD, gN, gM1, gM2 = _f64(gC), _f64(gA), _f64(gD), _f64(gN), _f64(gM1), _f64(gM2)
     lib().orc_render_bwd(C.c_int(n), _p(pos), _p(scale), _p(quat), _p(opacity), _p(sh), C.byref(cam), C.byref(cfg),
                          _p(pre["visible"]), _p(pre["M"]), _p(pre["c2d"]), _p(pre["rho_cut"]), _p(pre["normal"]), _p(pre["rgb"]),
                          _p(pre["clamp"]), _p(ids), _p(srt["ranges"]), _p(m), _p(gC), _p(gA), _p(gD), _p(gN),
                          C.c_int(x0), C.c_int(y0), C.c_int(x1), C.c_int(y1), _p(out["d_pos"]), _p(out["d_scale"]),
-                         _p(out["d_quat"]), _p(out["d_opacity"]), _p(out["d_sh"]), _p(out["d_center2d"]), _p(oabs), _p(gD2))
+                         _p(out["d_quat"]), _p(out["d_opacity"]), _p(out["d_sh"]), _p(out["d_center2d"]), _p(oabs), _p(gM1), _p(gM2))
     out["_d_opacity_abs"] = oabs
     return out
 
@@ -230,13 +230,13 @@ def bf_render(pos, scale, quat, opacity, sh, cam: OrcCamera, cfg: OrcConfig, mas
     W, H = cam.width, cam.height
     x0, y0, x1, y1 = window if window is not None else (0, 0, W, H)
     out = dict(color=np.zeros((3, H, W)), alpha=np.zeros((H, W)), depth=np.zeros((H, W)), normal=np.zeros((3, H, W)),
-               n_blended=np.zeros((H, W), np.uint32), depth2=np.zeros((H, W)))
+               n_blended=np.zeros((H, W), np.uint32), origin=np.zeros((H, W)), m1=np.zeros((H, W)), m2=np.zeros((H, W)))
     vis = np.zeros(n, np.uint32) if want_stats else None
     cs = np.zeros(n, np.float64) if want_stats else None
     m = None if mask is None else np.ascontiguousarray(mask, np.uint8)
     Lb = lib().orc_bf_render(C.c_int(n), _p(pos), _p(scale), _p(quat), _p(opacity), _p(sh), C.byref(cam), C.byref(cfg), _p(m),
                              C.c_int(x0), C.c_int(y0), C.c_int(x1), C.c_int(y1), _p(out["color"]), _p(out["alpha"]),
-                             _p(out["depth"]), _p(out["normal"]), _p(out["n_blended"]), _p(vis), _p(cs), _p(out["depth2"]))
+                             _p(out["depth"]), _p(out["normal"]), _p(out["n_blended"]), _p(vis), _p(cs), _p(out["origin"]), _p(out["m1"]), _p(out["m2"]))
     out.update(loss_bg=float(Lb), vis_count=vis, contrib_sum=cs)
     return out
 

@@ -448,7 +448,8 @@ double orc_render_fwd(int n, const OrcCamera* cam, const OrcConfig* cfg, const O
                       const float* rho_cut, const float* opacity, const double* normal, const double* rgb, const uint32_t* ids,
                       const uint32_t* ranges, const uint8_t* mask, int wx0, int wy0, int wx1, int wy1, double* color,
                       double* alpha, double* depth, double* nrm, uint32_t* n_contrib, uint32_t* vis_count, double* contrib_sum,
-                      uint8_t* fragile, uint32_t* fragile_touch, double* cond_rho, double* depth2 /*nullable: sum w z^2 (reading R-moments)*/) {
+                      uint8_t* fragile, uint32_t* fragile_touch, double* cond_rho,
+                      double* origin, double* m1, double* m2 /*nullable together: depth moments about the first blended pair's depth (reading R-moments)*/) {
   (void)n;
   const int W = cam->width, H = cam->height, T = cfg->tile;
   const int tiles_x = (W + T - 1) / T, tiles_y = (H + T - 1) / T;
@@ -460,7 +461,7 @@ double orc_render_fwd(int n, const OrcCamera* cam, const OrcConfig* cfg, const O
     const uint32_t start = ranges[2 * t], end = ranges[2 * t + 1];
     for (int y = std::max(ty * T, wy0); y < std::min({(ty + 1) * T, H, wy1}); ++y)
       for (int x = std::max(tx * T, wx0); x < std::min({(tx + 1) * T, W, wx1}); ++x) {
-        double Tr = 1.0, C[3] = {0, 0, 0}, D = 0, D2 = 0, N[3] = {0, 0, 0};
+        double Tr = 1.0, C[3] = {0, 0, 0}, D = 0, M1 = 0, M2 = 0, c0 = 0, N[3] = {0, 0, 0};
         uint32_t last = 0;
         bool frag = false;
         double cerr = 0.0;
@@ -480,7 +481,9 @@ double orc_render_fwd(int n, const OrcCamera* cam, const OrcConfig* cfg, const O
           }
           for (int c = 0; c < 3; ++c) { C[c] += w * rgb[3 * j + c]; N[c] += w * normal[3 * j + c]; }
           D += w * e.z;
-          D2 += w * e.z * e.z;
+          if (last == 0) c0 = e.z;  // origin of the depth moments: depth of the first blended pair
+          M1 += w * (e.z - c0);
+          M2 += w * (e.z - c0) * (e.z - c0);
           if (vis_count) {
 #pragma omp atomic
             vis_count[j] += 1;
@@ -496,7 +499,7 @@ double orc_render_fwd(int n, const OrcCamera* cam, const OrcConfig* cfg, const O
         for (int c = 0; c < 3; ++c) { color[c * HW + p] = C[c] + Tr * (double)cfg->bg[c]; nrm[c * HW + p] = N[c]; }
         alpha[p] = 1.0 - Tr;
         depth[p] = D;
-        if (depth2) depth2[p] = D2;
+        if (origin) { origin[p] = c0; m1[p] = M1; m2[p] = M2; }
         n_contrib[p] = last;
         const bool illc = mg && cerr > mg->cond_abs;
         if (fragile) fragile[p] = (uint8_t)((frag ? 1 : 0) | (illc ? 2 : 0));  // bit 0: decision margin, bit 1: ill-conditioned
@@ -525,7 +528,8 @@ void orc_render_bwd(int n, const float* pos, const float* scale, const float* qu
                     const float* rho_cut, const double* normal, const double* rgb, const uint8_t* clamp, const uint32_t* ids,
                     const uint32_t* ranges, const uint8_t* mask, const double* gC, const double* gA, const double* gD,
                     const double* gN, int wx0, int wy0, int wx1, int wy1, double* d_pos, double* d_scale, double* d_quat,
-                    double* d_opacity, double* d_sh, double* d_center2d, double* d_opacity_abs, const double* gD2 /*nullable: upstream of depth2*/) {
+                    double* d_opacity, double* d_sh, double* d_center2d, double* d_opacity_abs,
+                    const double* gM1, const double* gM2 /*nullable: upstream of the depth moments m1, m2 (origin held fixed)*/) {
   const int W = cam->width, H = cam->height, T = cfg->tile;
   const int tiles_x = (W + T - 1) / T, tiles_y = (H + T - 1) / T;
   const size_t HW = (size_t)W * H;
@@ -549,7 +553,7 @@ void orc_render_bwd(int n, const float* pos, const float* scale, const float* qu
           if (gN) for (int c = 0; c < 3; ++c) gnn[c] = gN[c * HW + p];
           if (gA) ga = gA[p];
           if (gD) gd = gD[p];
-          const double gd2 = gD2 ? gD2[p] : 0.0;
+          const double gm1 = gM1 ? gM1[p] : 0.0, gm2 = gM2 ? gM2[p] : 0.0;
           if (mask && cfg->gamma_bg != 0.0f) ga += (double)cfg->gamma_bg * (mask[p] ? 0.0 : 1.0) / (double)HW;
           // forward replay
           seq.clear();
@@ -564,22 +568,25 @@ void orc_render_bwd(int n, const float* pos, const float* scale, const float* qu
             Tr = Tn;
           }
           const double Tfin = Tr;
-          double SC[3] = {Tfin * cfg->bg[0], Tfin * cfg->bg[1], Tfin * cfg->bg[2]}, SD = 0, SD2 = 0, SN[3] = {0, 0, 0};
+          double SC[3] = {Tfin * cfg->bg[0], Tfin * cfg->bg[1], Tfin * cfg->bg[2]}, SD = 0, SM1 = 0, SM2 = 0, SN[3] = {0, 0, 0};
+          const double c0 = seq.empty() ? 0.0 : seq[0].e.z;  // origin of the depth moments (a constant: the terms built on it do not depend on it)
           for (size_t i = seq.size(); i-- > 0;) {
             const uint32_t j = seq[i].j;
             const PairEval& e = seq[i].e;
             const double Ti = seq[i].Tr, w = e.alpha * Ti, inv1ma = 1.0 / (1.0 - e.alpha);
-            double galpha = ga * Tfin * inv1ma + gd * (e.z * Ti - SD * inv1ma) + gd2 * (e.z * e.z * Ti - SD2 * inv1ma);
+            const double dz = e.z - c0;
+            double galpha = ga * Tfin * inv1ma + gd * (e.z * Ti - SD * inv1ma) + gm1 * (dz * Ti - SM1 * inv1ma) + gm2 * (dz * dz * Ti - SM2 * inv1ma);
             for (int c = 0; c < 3; ++c) {
               galpha += gc[c] * (rgb[3 * j + c] * Ti - SC[c] * inv1ma);
               galpha += gnn[c] * (normal[3 * j + c] * Ti - SN[c] * inv1ma);
             }
             for (int c = 0; c < 3; ++c) { SC[c] += w * rgb[3 * j + c]; SN[c] += w * normal[3 * j + c]; }
             SD += w * e.z;
-            SD2 += w * e.z * e.z;
+            SM1 += w * dz;
+            SM2 += w * dz * dz;
             double a_rgb[3], a_n[3];
             for (int c = 0; c < 3; ++c) { a_rgb[c] = w * gc[c]; a_n[c] = w * gnn[c]; }
-            const double gz = w * gd + 2.0 * e.z * w * gd2;  // z enters D = sum w z and D2 = sum w z^2
+            const double gz = w * gd + w * gm1 + 2.0 * dz * w * gm2;  // z enters D = sum w z, m1 = sum w (z-c), m2 = sum w (z-c)^2
             double a_o = 0, grho = 0;
             if (!e.capped) {  // S12: zero gradient through the cap
               a_o = e.G * galpha;
@@ -742,7 +749,7 @@ int orc_prune(int n, const uint32_t* vis_count, const float* contrib_sum, const 
 double orc_bf_render(int n, const double* pos, const double* scale, const double* quat, const double* opacity, const double* sh,
                      const OrcCamera* cam, const OrcConfig* cfg, const uint8_t* mask, int wx0, int wy0, int wx1, int wy1,
                      double* color, double* alpha, double* depth, double* nrm, uint32_t* n_blended, uint32_t* vis_count,
-                     double* contrib_sum, double* depth2 /*nullable*/) {
+                     double* contrib_sum, double* origin, double* m1, double* m2 /*nullable together*/) {
   const int W = cam->width, H = cam->height;
   const size_t HW = (size_t)W * H;
   const float* V = cam->view;
@@ -824,7 +831,7 @@ double orc_bf_render(int n, const double* pos, const double* scale, const double
         cands.push_back({s.key, j, a, z});
       }
       std::sort(cands.begin(), cands.end(), [](const Cand& a, const Cand& b) { return a.key != b.key ? a.key < b.key : a.j < b.j; });
-      double Tr = 1.0, C[3] = {0, 0, 0}, D = 0, D2 = 0, N[3] = {0, 0, 0};
+      double Tr = 1.0, C[3] = {0, 0, 0}, D = 0, M1 = 0, M2 = 0, c0 = 0, N[3] = {0, 0, 0};
       uint32_t cnt = 0;
       for (const Cand& c : cands) {
         const double Tn = Tr * (1.0 - c.alpha);
@@ -833,7 +840,9 @@ double orc_bf_render(int n, const double* pos, const double* scale, const double
         const S& s = ss[(size_t)c.j];
         for (int k = 0; k < 3; ++k) { C[k] += w * s.rgb[k]; N[k] += w * s.facing[k]; }
         D += w * c.z;
-        D2 += w * c.z * c.z;
+        if (cnt == 0) c0 = c.z;
+        M1 += w * (c.z - c0);
+        M2 += w * (c.z - c0) * (c.z - c0);
         if (vis_count) {
 #pragma omp atomic
           vis_count[c.j] += 1;
@@ -849,7 +858,7 @@ double orc_bf_render(int n, const double* pos, const double* scale, const double
       for (int k = 0; k < 3; ++k) { color[k * HW + p] = C[k] + Tr * (double)cfg->bg[k]; nrm[k * HW + p] = N[k]; }
       alpha[p] = 1.0 - Tr;
       depth[p] = D;
-      if (depth2) depth2[p] = D2;
+      if (origin) { origin[p] = c0; m1[p] = M1; m2[p] = M2; }
       if (n_blended) n_blended[p] = cnt;
       const double m = mask ? (mask[p] ? 1.0 : 0.0) : 0.0;
       Lb += (1.0 - Tr) * (1.0 - m);

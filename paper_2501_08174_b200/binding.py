@@ -18,7 +18,7 @@ _LIB_PATH = os.path.join(_HERE, "csrc", "libocgs.so")
 OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
            "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_render_fwd_reg", "ocgs_render_bwd_reg", "ocgs_prune_workspace_bytes",
-           "ocgs_prune_stats", "ocgs_step_host", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss",
+           "ocgs_prune_stats", "ocgs_step_host", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
            "ocgs_profile_begin", "ocgs_profile_end"]
 
 
@@ -76,6 +76,7 @@ def lib():
         _lib.ocgs_workspace_bytes.restype = C.c_size_t
         _lib.ocgs_prune_workspace_bytes.restype = C.c_size_t
         _lib.ocgs_photometric_workspace_bytes.restype = C.c_size_t
+        _lib.ocgs_regularizers_workspace_bytes.restype = C.c_size_t
         for name in EXPORTS:
             getattr(_lib, name)  # raises AttributeError if a declared symbol is not exported
     return _lib
@@ -215,6 +216,16 @@ def ocgs_step_host(h_pos, h_scale, h_quat, h_opacity, h_sh, n, cam, cfg, h_mask,
 def ocgs_masked_l1(color, target, mask, width, height, dL_dcolor, loss, ws, n, key_capacity, stream=None):
     _ok("ocgs_masked_l1", lib().ocgs_masked_l1(_ptr(color), _ptr(target), _ptr(mask), C.c_int(width), C.c_int(height), _ptr(dL_dcolor),
                                                _ptr(loss), _ptr(ws), C.c_int(n), C.c_size_t(key_capacity), _stream(stream)))
+
+
+def ocgs_regularizers_workspace_bytes(width: int, height: int) -> int:
+    return int(lib().ocgs_regularizers_workspace_bytes(C.c_int(width), C.c_int(height)))
+
+
+def ocgs_regularizers(alpha, depth, depth2, normal, cam, w_d, w_n, dL_dalpha, dL_ddepth, dL_ddepth2, dL_dnormal, loss, scratch, stream=None):
+    _ok("ocgs_regularizers", lib().ocgs_regularizers(_ptr(alpha), _ptr(depth), _ptr(depth2), _ptr(normal), C.byref(cam), C.c_float(w_d),
+                                                     C.c_float(w_n), _ptr(dL_dalpha), _ptr(dL_ddepth), _ptr(dL_ddepth2), _ptr(dL_dnormal),
+                                                     _ptr(loss), _ptr(scratch), _stream(stream)))
 
 
 def ocgs_photometric_workspace_bytes(width: int, height: int) -> int:

@@ -226,6 +226,19 @@ int ocgs_masked_l1(const float* color, const float* target, const uint8_t* mask,
   return launch_masked_l1(color, target, mask, width, height, dL_dcolor, loss, w.loss_partial, w.n_tiles, (cudaStream_t)stream);
 }
 
+size_t ocgs_regularizers_workspace_bytes(int width, int height) { return regularizers_workspace_bytes(width, height); }
+
+int ocgs_regularizers(const float* alpha, const float* depth, const float* depth2, const float* normal, const ocgs_camera* cam, float w_d,
+                      float w_n, float* dL_dalpha, float* dL_ddepth, float* dL_ddepth2, float* dL_dnormal, float* loss, void* scratch,
+                      void* stream) {
+  if (!alpha || !depth || !depth2 || !normal || !cam || !dL_dalpha || !dL_ddepth || !dL_ddepth2 || !dL_dnormal || !scratch)
+    return OCGS_ERR_INVALID_ARG;
+  if (cam->width <= 0 || cam->height <= 0 || !(cam->fx > 0.f) || !(cam->fy > 0.f)) return OCGS_ERR_INVALID_ARG;
+  if (cam->width > OCGS_MAX_DIM || cam->height > OCGS_MAX_DIM) return OCGS_ERR_UNSUPPORTED;
+  return launch_regularizers(alpha, depth, depth2, normal, *cam, w_d, w_n, dL_dalpha, dL_ddepth, dL_ddepth2, dL_dnormal, loss, scratch,
+                             (cudaStream_t)stream);
+}
+
 size_t ocgs_photometric_workspace_bytes(int width, int height) { return photometric_workspace_bytes(width, height); }
 
 int ocgs_photometric_loss(const float* color, const float* target, const uint8_t* mask, int width, int height, float lambda_dssim,

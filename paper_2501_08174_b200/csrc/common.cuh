@@ -108,6 +108,9 @@ int launch_prune(const ocgs_surfels& in, uint32_t* vis_count, float* contrib_sum
 int launch_masked_l1(const float* color, const float* target, const uint8_t* mask, int W, int H, float* dL_dcolor, float* loss,
                      float* partial, int n_partial, cudaStream_t st);
 
+size_t regularizers_workspace_bytes(int W, int H);
+int launch_regularizers(const float* alpha, const float* depth, const float* depth2, const float* normal, const ocgs_camera& c, float w_d,
+                        float w_n, float* gA, float* gD, float* gD2, float* gN, float* loss, void* scratch, cudaStream_t st);
 size_t photometric_workspace_bytes(int W, int H);
 int launch_photometric(const float* color, const float* target, const uint8_t* mask, int W, int H, float lam, float* dL_dcolor,
                        float* loss, void* scratch, cudaStream_t st);

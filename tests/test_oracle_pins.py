@@ -160,10 +160,14 @@ def test_two_layer_closed_form_and_background():
     assert np.allclose(fwd["color"][:, py, px], expC, atol=1e-6)
     assert fwd["alpha"][py, px] == pytest.approx(1 - T, abs=1e-7)
     assert fwd["n_contrib"][py, px] == 2
-    # depth moments (reading R-moments): D = sum w z, D2 = sum w z^2 with fronto-parallel hit depths 1.5 and 3
+    # depth moments (reading R-moments) about the first blended pair's depth c = 1.5: m1 = sum w (z - c), m2 = sum w (z - c)^2
     w1, w2 = a[0], (1 - a[0]) * a[1]
     assert fwd["depth"][py, px] == pytest.approx(w1 * 1.5 + w2 * 3.0, abs=1e-6)
-    assert fwd["depth2"][py, px] == pytest.approx(w1 * 1.5 ** 2 + w2 * 3.0 ** 2, abs=1e-6)
+    assert fwd["origin"][py, px] == pytest.approx(1.5, abs=1e-6)
+    assert fwd["m1"][py, px] == pytest.approx(w2 * 1.5, abs=1e-6) and fwd["m2"][py, px] == pytest.approx(w2 * 1.5 ** 2, abs=1e-6)
+    # ... and the pairwise distortion sum_{i<j} w_i w_j (z_i - z_j)^2 = A m2 - m1^2
+    A_ = fwd["alpha"][py, px]
+    assert A_ * fwd["m2"][py, px] - fwd["m1"][py, px] ** 2 == pytest.approx(w1 * w2 * 1.5 ** 2, abs=1e-6)
     # sort order: the nearer surfel (id 1) first although its id is larger (S9)
     t = (py // 16) * 1 + px // 16
     assert list(srt["ids"][srt["ranges"][t, 0]:srt["ranges"][t, 1]]) == [1, 0]
@@ -411,11 +415,11 @@ def _compare_bf_tiled(sc, view, cfg, tol=5e-5):
     bf = orc.bf_render(*P, cam, cfg, mask=m)
     ok = fw["fragile"] == 0
     assert ok.mean() > 0.995
-    for k in ("color", "alpha", "depth", "normal", "depth2"):
-        scale = 1.0 if not k.startswith("depth") else np.maximum(1.0, np.abs(bf[k]))
+    for k in ("color", "alpha", "depth", "normal", "origin", "m1", "m2"):
+        scale = 1.0 if k not in ("depth", "origin") else np.maximum(1.0, np.abs(bf[k]))
         err = np.abs(fw[k] - bf[k]) / scale
         # M is an fp32 record (~1e-7 relative); the hit depth of oblique surfels amplifies that most
-        assert (err * ok).max() < (tol if not k.startswith("depth") else 10 * tol), (k, (err * ok).max())
+        assert (err * ok).max() < (tol if k not in ("depth", "origin", "m1", "m2") else 10 * tol), (k, (err * ok).max())
     untouched = fw["fragile_touch"] == 0
     assert np.array_equal(fw["vis_count"][untouched], bf["vis_count"][untouched])
     assert np.allclose(fw["contrib_sum"][untouched], bf["contrib_sum"][untouched], rtol=1e-4, atol=1e-6)
@@ -446,19 +450,22 @@ def _fd_check(seed, n, W, H, f, sh_degree, **kw):
     m = sc.mask(0)
     rng = np.random.default_rng(seed + 100)
     wC, wA, wD, wN = rng.normal(size=(3, H, W)), rng.normal(size=(H, W)), rng.normal(size=(H, W)), rng.normal(size=(3, H, W))
-    wD2 = rng.normal(size=(H, W))  # upstream of the squared-depth moment map (reading R-moments)
+    wX = rng.normal(size=(H, W))  # per-pixel weight of the pairwise depth distortion A m2 - m1^2 (reading R-moments)
     params = dict(pos=sc.pos.astype(np.float64), scale=sc.scale.astype(np.float64), quat=sc.quat.astype(np.float64),
                   opacity=sc.opacity.astype(np.float64), sh=sc.sh.astype(np.float64))
 
     def loss(p):
         r = orc.bf_render(p["pos"], p["scale"], p["quat"], p["opacity"], p["sh"], cam, cfg, mask=m, want_stats=False)
         L = (wC * r["color"]).sum() + (wA * r["alpha"]).sum() + (wD * r["depth"]).sum() + (wN * r["normal"]).sum()
-        L += (wD2 * r["depth2"]).sum()
+        L += (wX * (r["alpha"] * r["m2"] - r["m1"] ** 2)).sum()  # invariant to the moments' origin, so FD sees no kink from it
         return L + cfg.gamma_bg * r["loss_bg"], r["n_blended"]
 
     pre = orc.preprocess(sc.pos, sc.scale, sc.quat, sc.opacity, sc.sh, cam, cfg)
     srt = orc.bin_sort(pre, cam, cfg)
-    g = orc.render_bwd(sc.pos, sc.scale, sc.quat, sc.opacity, sc.sh, pre, srt, cam, cfg, mask=m, gC=wC, gA=wA, gD=wD, gN=wN, gD2=wD2)
+    fw0 = orc.render_fwd(pre, srt, sc.opacity, cam, cfg, mask=m, want_fragile=False)
+    # chain rule of the distortion term through the maps: d(A m2 - m1^2) = m2 dA - 2 m1 dm1 + A dm2
+    g = orc.render_bwd(sc.pos, sc.scale, sc.quat, sc.opacity, sc.sh, pre, srt, cam, cfg, mask=m, gC=wC, gA=wA + wX * fw0["m2"], gD=wD, gN=wN,
+                       gM1=-2.0 * wX * fw0["m1"], gM2=wX * fw0["alpha"])
     names = dict(pos="d_pos", scale="d_scale", quat="d_quat", opacity="d_opacity", sh="d_sh")
     nb = (sh_degree + 1) ** 2
     checked = skipped = 0

@@ -16,23 +16,25 @@ def smooth_maps(seed, H=18, W=24):
     A = 0.55 + 0.3 * np.sin(xs / 5.0) * np.cos(ys / 4.0)
     zbar = 2.0 + 0.2 * np.sin(xs / 3.0 + 0.3) + 0.15 * np.cos(ys / 2.5) + 0.01 * rng.normal(size=(H, W))
     D = A * zbar
-    D2 = A * (zbar ** 2 + 0.05 + 0.02 * rng.uniform(size=(H, W)))
+    m1 = A * (0.05 + 0.03 * np.sin(xs / 4.0))            # sum w (z - c)
+    m2 = A * (0.01 + 0.004 * rng.uniform(size=(H, W)))   # sum w (z - c)^2
     n = rng.normal(size=(3, H, W)) * 0.2 + np.array([0.1, -0.2, -0.9])[:, None, None]
     Nrm = A[None] * n
-    return A, D, D2, Nrm
+    return A, D, m1, m2, Nrm
 
 
 def test_distortion_identity_against_the_double_sum():
-    """R-Ld: sum_{i<j} w_i w_j (z_i - z_j)^2 == A D2 - D^2 with A = sum w, D = sum w z, D2 = sum w z^2."""
+    """R-Ld: sum_{i<j} w_i w_j (z_i - z_j)^2 == A m2 - m1^2 with A = sum w, m1 = sum w (z - c), m2 = sum w (z - c)^2, for any c."""
     rng = np.random.default_rng(0)
     for n in (1, 2, 5, 40):
         w = rng.uniform(0, 0.3, n)
         z = rng.uniform(0.5, 6.0, n)
-        A, D, D2 = w.sum(), (w * z).sum(), (w * z * z).sum()
-        assert rg.distortion_map(A, D, D2) == pytest.approx(rg.distortion_bruteforce(w, z), rel=1e-12, abs=1e-14)
+        for c in (0.0, z[0], 17.0):
+            A, m1, m2 = w.sum(), (w * (z - c)).sum(), (w * (z - c) ** 2).sum()
+            assert rg.distortion_map(A, m1, m2) == pytest.approx(rg.distortion_bruteforce(w, z), rel=1e-10, abs=1e-12)
     # one layer: no distortion; two layers: w1 w2 (z1 - z2)^2
-    assert rg.distortion_map(0.7, 0.7 * 3.0, 0.7 * 9.0) == pytest.approx(0.0, abs=1e-15)
-    assert rg.distortion_map(0.5 + 0.2, 0.5 * 1.0 + 0.2 * 4.0, 0.5 * 1.0 + 0.2 * 16.0) == pytest.approx(0.5 * 0.2 * 9.0, rel=1e-14)
+    assert rg.distortion_map(0.7, 0.0, 0.0) == 0.0  # origin = the layer's own depth
+    assert rg.distortion_map(0.5 + 0.2, 0.2 * 3.0, 0.2 * 9.0) == pytest.approx(0.5 * 0.2 * 9.0, rel=1e-14)  # z = 1, 4; c = 1
 
 
 def test_fronto_parallel_depth_gives_camera_facing_axis_normal():
@@ -54,15 +56,15 @@ def test_planar_depth_map_reproduces_the_plane_normal_and_zero_loss_inside():
     zbar = d / (n[:, None, None] * r).sum(0)
     A = np.full((H, W), 0.8)
     Nrm = A[None] * n[:, None, None]
-    out = rg.regularizers(A, A * zbar, A * zbar ** 2, Nrm, FX, FY, CX, CY)
+    out = rg.regularizers(A, A * zbar, np.zeros((H, W)), np.zeros((H, W)), Nrm, FX, FY, CX, CY)
     assert np.abs(out["Nhat"][:, 1:-1, 1:-1] - n[:, None, None]).max() < 1e-12
     border = H * W - (H - 2) * (W - 2)
     assert out["L_n"] == pytest.approx(0.8 * border / (H * W), abs=1e-12)  # border pixels have Nhat = 0: term = A
-    assert out["L_d"] == pytest.approx(0.0, abs=1e-13)  # D2 = A zbar^2: a single layer per pixel
+    assert out["L_d"] == 0.0  # a single layer per pixel: both centred moments vanish
 
 
 def test_pixels_without_surface_have_no_normal():
-    A, D, D2, Nrm = smooth_maps(1)
+    A, D, m1, m2, Nrm = smooth_maps(1)
     A2 = A.copy(); A2[5, 7] = 0.0
     Nhat, t = rg.depth_normal(A2, D, FX, FY, CX, CY)
     for (y, x) in ((5, 7), (5, 6), (5, 8), (4, 7), (6, 7)):
@@ -72,21 +74,21 @@ def test_pixels_without_surface_have_no_normal():
 
 @pytest.mark.parametrize("w_d,w_n", [(1.0, 0.0), (0.0, 1.0), (3.0, 0.5)])
 def test_gradients_match_central_finite_differences(w_d, w_n):
-    A, D, D2, Nrm = smooth_maps(2)
-    out = rg.regularizers(A, D, D2, Nrm, FX, FY, CX, CY, w_d=w_d, w_n=w_n)
+    A, D, m1, m2, Nrm = smooth_maps(2)
+    out = rg.regularizers(A, D, m1, m2, Nrm, FX, FY, CX, CY, w_d=w_d, w_n=w_n)
 
-    def L(A_, D_, D2_, N_):
-        o = rg.regularizers(A_, D_, D2_, N_, FX, FY, CX, CY)
+    def L(A_, D_, m1_, m2_, N_):
+        o = rg.regularizers(A_, D_, m1_, m2_, N_, FX, FY, CX, CY)
         return w_d * o["L_d"] + w_n * o["L_n"]
 
     rng = np.random.default_rng(3)
     h = 1e-6
-    scale = {k: np.abs(out[k]).max() + 1e-30 for k in ("gA", "gD", "gD2", "gN")}
+    scale = {k: np.abs(out[k]).max() + 1e-30 for k in ("gA", "gD", "gM1", "gM2", "gN")}
     for _ in range(30):
         y, x = int(rng.integers(0, A.shape[0])), int(rng.integers(0, A.shape[1]))
-        for name, arr, idx in (("gA", A, (y, x)), ("gD", D, (y, x)), ("gD2", D2, (y, x)), ("gN", Nrm, (int(rng.integers(0, 3)), y, x))):
-            maps = dict(gA=A, gD=D, gD2=D2, gN=Nrm)
+        for name, idx in (("gA", (y, x)), ("gD", (y, x)), ("gM1", (y, x)), ("gM2", (y, x)), ("gN", (int(rng.integers(0, 3)), y, x))):
+            maps = dict(gA=A, gD=D, gM1=m1, gM2=m2, gN=Nrm)
             p, m = {k: v.copy() for k, v in maps.items()}, {k: v.copy() for k, v in maps.items()}
             p[name][idx] += h; m[name][idx] -= h
-            fd = (L(p["gA"], p["gD"], p["gD2"], p["gN"]) - L(m["gA"], m["gD"], m["gD2"], m["gN"])) / (2 * h)
+            fd = (L(p["gA"], p["gD"], p["gM1"], p["gM2"], p["gN"]) - L(m["gA"], m["gD"], m["gM1"], m["gM2"], m["gN"])) / (2 * h)
             assert abs(out[name][idx] - fd) <= 1e-6 * scale[name] + 1e-5 * abs(fd), (name, idx, out[name][idx], fd)
