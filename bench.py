@@ -42,7 +42,9 @@ def parse_args():
     ap.add_argument("--shrink", type=float, default=1.0, help="scale surfel counts (debug only; invalidates the metric)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--loss", default="l1", choices=["l1", "dssim"], help="photometric term of the step: masked L1 (harness loss S20, the default the metric is quoted on) or the full L_c^M = 0.8 L1 + 0.2 D-SSIM of Eq. 2 (ocgs_photometric_loss)")
+    ap.add_argument("--loss", default="l1", choices=["l1", "dssim", "eq3"],
+                    help="loss of the step: masked L1 (harness loss S20, the default the metric is quoted on); the full L_c^M = 0.8 L1 + 0.2 D-SSIM of "
+                         "Eq. 2 (ocgs_photometric_loss); or all of Eq. 3 (moment forward, ocgs_regularizers, moment backward)")
     ap.add_argument("--no-graph", action="store_true", help="time direct kernel launches instead of CUDA graph replays")
     return ap.parse_args()
 
@@ -208,7 +210,13 @@ def run_ours(args):
     gC = torch.empty((3, H, W), dtype=torch.float32, device=dev)
     loss_l1 = torch.zeros(1, dtype=torch.float32, device=dev)
     loss_pm = torch.zeros(3, dtype=torch.float32, device=dev)
-    pws_photo = torch.empty(B.ocgs_photometric_workspace_bytes(W, H), dtype=torch.uint8, device=dev) if args.loss == "dssim" else None
+    pws_photo = torch.empty(B.ocgs_photometric_workspace_bytes(W, H), dtype=torch.uint8, device=dev) if args.loss != "l1" else None
+    loss_reg = torch.zeros(2, dtype=torch.float32, device=dev)
+    if args.loss == "eq3":
+        moments = torch.zeros((3, H, W), dtype=torch.float32, device=dev)
+        gA_r, gD_r = torch.zeros((H, W), dtype=torch.float32, device=dev), torch.zeros((H, W), dtype=torch.float32, device=dev)
+        gM_r, gN_r = torch.zeros((2, H, W), dtype=torch.float32, device=dev), torch.zeros((3, H, W), dtype=torch.float32, device=dev)
+        pws_reg = torch.empty(B.ocgs_regularizers_workspace_bytes(W, H), dtype=torch.uint8, device=dev)
     vis = torch.zeros(n, dtype=torch.int32, device=dev)
     cs = torch.zeros(n, dtype=torch.float32, device=dev)
     cam_c = [B.camera_from(cams[v]) for v in my_views]
@@ -231,6 +239,14 @@ def run_ours(args):
         c, m = cam_c[i], masks[i]
         B.ocgs_preprocess(surfels, c, cfg, ws, cap)
         B.ocgs_bin_sort(n, c, cfg, ws, cap)
+        if args.loss == "eq3":  # Eq. 3: L_c^M + alpha L_d + beta L_n + gamma L_b (alpha = 100, beta = 0.05: 2DGS's values for bounded scenes)
+            B.ocgs_render_fwd_reg(n, c, cfg, ws, cap, m, out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"], out["loss_bg"],
+                                  vis if stats else None, cs if stats else None, moments)
+            B.ocgs_photometric_loss(out["color"], targets[i], m, W, H, 0.2, gC, loss_pm, pws_photo)
+            B.ocgs_regularizers(out["alpha"], out["depth"], moments, out["normal"], c, 100.0, 0.05, gA_r, gD_r, gM_r, gN_r, loss_reg, pws_reg)
+            B.ocgs_render_bwd_reg(surfels, c, cfg, ws, cap, m, out["n_contrib"], gC, gA_r, gD_r, gN_r, moments, gM_r, grads["d_pos"],
+                                  grads["d_scale"], grads["d_quat"], grads["d_opacity"], grads["d_sh"], grads["d_center2d"])
+            return
         B.ocgs_render_fwd(n, c, cfg, ws, cap, m, out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"], out["loss_bg"],
                           vis if stats else None, cs if stats else None)
         if args.loss == "dssim":
@@ -250,7 +266,8 @@ def run_ours(args):
         if i < nv:
             counters.append(dict(K=int(h.K), n_vis=int(h.n_vis), E=int(out["n_contrib"].long().sum().item()),
                                  B=int(vis.long().sum().item()), loss_bg=float(out["loss_bg"].item()),
-                                 loss_l1=float(loss_pm[1].item() if args.loss == "dssim" else loss_l1.item()), loss_dssim=float(loss_pm[2].item())))
+                                 loss_l1=float(loss_pm[1].item() if args.loss != "l1" else loss_l1.item()), loss_dssim=float(loss_pm[2].item()),
+                                 loss_dist=float(loss_reg[0].item()), loss_normal=float(loss_reg[1].item())))
     vis.zero_(); cs.zero_()
 
     def barrier():
@@ -426,7 +443,8 @@ def run_ours(args):
                       "radix_hist_all_kernel": 4.0 * (n + K) / 2.0, "emit_keys_kernel": 8.0 * K + 12.0 * nvis,
                       "preprocess_kernel": 61.0 * n + 296.0 * nvis, "project_bwd_kernel": 232.0 * n + 328.0 * nvis,
                       "reorder_kernel": 208.0 * nvis, "clear_grad_rec_kernel": 96.0 * nvis, "tile_ranges_kernel": 4.0 * K,
-                      "masked_l1_kernel": 25.0 * W * H, "ssim_terms_kernel": 63.0 * W * H, "ssim_grad_kernel": 75.0 * W * H}.get(name)
+                      "masked_l1_kernel": 25.0 * W * H, "ssim_terms_kernel": 63.0 * W * H, "ssim_grad_kernel": 75.0 * W * H,
+                      "reg_terms_kernel": 76.0 * W * H, "reg_gather_kernel": 52.0 * W * H}.get(name)
         if per_launch is None:
             return None
         ach = per_launch / avg_s / 1e9
@@ -442,7 +460,8 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": f"{scene.name}: {n} surfels, {W}x{H}, SH degree {deg}, {nv} views rotated per rank (views sharded over ranks)",
                        "l2": "inputs larger than L2: 232 MB of surfel parameters are re-read every step", "key_capacity": cap,
-                       "shrink": args.shrink, "photometric_term": "masked L1 (S20)" if args.loss == "l1" else "L_c^M = 0.8 L1 + 0.2 D-SSIM (Eq. 2)"},
+                       "shrink": args.shrink, "loss": {"l1": "masked L1 (S20) + gamma L_b", "dssim": "L_c^M = 0.8 L1 + 0.2 D-SSIM (Eq. 2) + gamma L_b",
+                                "eq3": "Eq. 3: L_c^M + 100 L_d + 0.05 L_n + gamma L_b"}[args.loss]},
             "surfels_per_s": n * world / (ms_total / steps * 1e-3), "pixels_per_s": W * H * world / (ms_total / steps * 1e-3),
             "workload_counters": mean, "gpu_launches": launches, "clocks": clocks, "roofline": roof, "rooflines": rooflines, "kernels": kernels[:14],
             "kernel_ms_sum_per_step": kern_total / steps,

@@ -158,33 +158,35 @@ int ocgs_render_bwd(const ocgs_surfels* surfels, const ocgs_camera* cam, const o
                     const float* dL_dalpha, const float* dL_ddepth, const float* dL_dnormal, float* d_pos, float* d_scale,
                     float* d_quat, float* d_opacity, float* d_sh, float* d_center2d, void* stream);
 
-/* ---- (3b)/(4b) forward / backward with the squared-depth moment map (reading R-moments) -----
+/* ---- (3b)/(4b) forward / backward with the depth moments (reading R-moments) ---------------
  * The 2DGS regularisers the paper keeps unchanged (depth distortion L_d, normal consistency L_n) are
- * image-space functions of the rendered maps once the renderer also accumulates depth2 = sum_i w_i z_i^2 (w_i = alpha_i T_i,
- * z_i the pair's depth as written to `depth`): sum_{i<j} w_i w_j (z_i - z_j)^2 = alpha * depth2 - depth^2 per pixel.
- * ocgs_render_fwd_reg = ocgs_render_fwd + depth2 (device f32 [H,W], nullable = plain forward).
- * ocgs_render_bwd_reg = ocgs_render_bwd + dL_ddepth2 (device f32 [H,W], nullable), the upstream gradient of depth2.
- * ocgs_regularizers (below) evaluates L_d, L_n and the upstream gradients these calls consume. */
+ * image-space functions of the rendered maps once the renderer also accumulates, per pixel, the depth moments
+ *   moments[0] = c  (origin: depth of the pixel's first blended pair, 0 if none),
+ *   moments[1] = m1 = sum_i w_i (z_i - c),   moments[2] = m2 = sum_i w_i (z_i - c)^2     (w_i = alpha_i T_i, z_i as in `depth`):
+ *   sum_{i<j} w_i w_j (z_i - z_j)^2 = alpha * m2 - m1^2 for any origin; about c the difference is well conditioned in fp32.
+ * ocgs_render_fwd_reg = ocgs_render_fwd + moments (device f32 [3,H,W], nullable = plain forward).
+ * ocgs_render_bwd_reg = ocgs_render_bwd + moments (the forward's map) and dL_dmoments (device f32 [2,H,W]: upstream
+ * gradients of m1 and m2, the origin held fixed); both NULL = plain backward, exactly one NULL = OCGS_ERR_INVALID_ARG. */
 int ocgs_render_fwd_reg(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
                         float* color, float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg,
-                        uint32_t* vis_count, float* contrib_sum, float* depth2, void* stream);
+                        uint32_t* vis_count, float* contrib_sum, float* moments, void* stream);
 int ocgs_render_bwd_reg(const ocgs_surfels* surfels, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
                         const uint8_t* mask, const uint32_t* n_contrib, const float* dL_dcolor, const float* dL_dalpha,
-                        const float* dL_ddepth, const float* dL_dnormal, const float* dL_ddepth2, float* d_pos, float* d_scale,
-                        float* d_quat, float* d_opacity, float* d_sh, float* d_center2d, void* stream);
+                        const float* dL_ddepth, const float* dL_dnormal, const float* moments, const float* dL_dmoments,
+                        float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh, float* d_center2d, void* stream);
 
 /* ---- regularisers of Eq. 3 (readings R-Ld, R-Ln) -------------------------
- * L_d = 1/(HW) sum_p (alpha depth2 - depth^2) (depth distortion, squared pairwise form) and
+ * L_d = 1/(HW) sum_p (alpha m2 - m1^2) (depth distortion, squared pairwise form) and
  * L_n = 1/(HW) sum_p (alpha - normal . Nhat) (normal consistency; Nhat = camera-facing unit normal of the expected-depth
  * surface depth/alpha by central differences of the back-projected points, zero on the image border and next to pixels
- * with alpha <= 1e-4), unmasked.  Inputs: the maps of ocgs_render_fwd_reg (device f32; normal [3,H,W]) and the camera.
- * Outputs (device f32, OVERWRITTEN): dL_dalpha[H,W], dL_ddepth[H,W], dL_ddepth2[H,W], dL_dnormal[3,H,W] = gradients of
- * w_d L_d + w_n L_n (pass them to ocgs_render_bwd_reg, adding other losses' gradients first if there are any);
+ * with alpha <= 1e-4), unmasked.  Inputs: the maps of ocgs_render_fwd_reg (device f32; normal and moments [3,H,W]) and
+ * the camera.  Outputs (device f32, OVERWRITTEN): dL_dalpha[H,W], dL_ddepth[H,W], dL_dmoments[2,H,W], dL_dnormal[3,H,W]
+ * = gradients of w_d L_d + w_n L_n (pass them to ocgs_render_bwd_reg, adding other losses' gradients first if any);
  * loss: device f32[2] or NULL <- (L_d, L_n), unweighted, deterministic.
  * scratch: device memory of at least ocgs_regularizers_workspace_bytes(width, height), 256-B aligned. */
 size_t ocgs_regularizers_workspace_bytes(int width, int height);
-int ocgs_regularizers(const float* alpha, const float* depth, const float* depth2, const float* normal, const ocgs_camera* cam,
-                      float w_d, float w_n, float* dL_dalpha, float* dL_ddepth, float* dL_ddepth2, float* dL_dnormal, float* loss,
+int ocgs_regularizers(const float* alpha, const float* depth, const float* moments, const float* normal, const ocgs_camera* cam,
+                      float w_d, float w_n, float* dL_dalpha, float* dL_ddepth, float* dL_dmoments, float* dL_dnormal, float* loss,
                       void* scratch, void* stream);
 
 /* ---- (5) prune statistics -> mask -> stream compaction ----------------------------------------------------------------

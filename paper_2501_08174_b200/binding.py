@@ -169,17 +169,17 @@ def ocgs_render_fwd(n, cam, cfg, ws, key_capacity, mask, color, alpha, depth, no
 
 
 def ocgs_render_fwd_reg(n, cam, cfg, ws, key_capacity, mask, color, alpha, depth, normal, n_contrib, loss_bg, vis_count, contrib_sum,
-                        depth2, stream=None):
+                        moments, stream=None):
     _ok("ocgs_render_fwd_reg", lib().ocgs_render_fwd_reg(C.c_int(n), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity),
                                                          _ptr(mask), _ptr(color), _ptr(alpha), _ptr(depth), _ptr(normal), _ptr(n_contrib),
-                                                         _ptr(loss_bg), _ptr(vis_count), _ptr(contrib_sum), _ptr(depth2), _stream(stream)))
+                                                         _ptr(loss_bg), _ptr(vis_count), _ptr(contrib_sum), _ptr(moments), _stream(stream)))
 
 
-def ocgs_render_bwd_reg(surfels, cam, cfg, ws, key_capacity, mask, n_contrib, dL_dcolor, dL_dalpha, dL_ddepth, dL_dnormal, dL_ddepth2,
+def ocgs_render_bwd_reg(surfels, cam, cfg, ws, key_capacity, mask, n_contrib, dL_dcolor, dL_dalpha, dL_ddepth, dL_dnormal, moments, dL_dmoments,
                         d_pos, d_scale, d_quat, d_opacity, d_sh, d_center2d=None, stream=None):
     _ok("ocgs_render_bwd_reg", lib().ocgs_render_bwd_reg(C.byref(surfels), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity),
                                                          _ptr(mask), _ptr(n_contrib), _ptr(dL_dcolor), _ptr(dL_dalpha), _ptr(dL_ddepth),
-                                                         _ptr(dL_dnormal), _ptr(dL_ddepth2), _ptr(d_pos), _ptr(d_scale), _ptr(d_quat),
+                                                         _ptr(dL_dnormal), _ptr(moments), _ptr(dL_dmoments), _ptr(d_pos), _ptr(d_scale), _ptr(d_quat),
                                                          _ptr(d_opacity), _ptr(d_sh), _ptr(d_center2d), _stream(stream)))
 
 
@@ -222,9 +222,9 @@ def ocgs_regularizers_workspace_bytes(width: int, height: int) -> int:
     return int(lib().ocgs_regularizers_workspace_bytes(C.c_int(width), C.c_int(height)))
 
 
-def ocgs_regularizers(alpha, depth, depth2, normal, cam, w_d, w_n, dL_dalpha, dL_ddepth, dL_ddepth2, dL_dnormal, loss, scratch, stream=None):
-    _ok("ocgs_regularizers", lib().ocgs_regularizers(_ptr(alpha), _ptr(depth), _ptr(depth2), _ptr(normal), C.byref(cam), C.c_float(w_d),
-                                                     C.c_float(w_n), _ptr(dL_dalpha), _ptr(dL_ddepth), _ptr(dL_ddepth2), _ptr(dL_dnormal),
+def ocgs_regularizers(alpha, depth, moments, normal, cam, w_d, w_n, dL_dalpha, dL_ddepth, dL_dmoments, dL_dnormal, loss, scratch, stream=None):
+    _ok("ocgs_regularizers", lib().ocgs_regularizers(_ptr(alpha), _ptr(depth), _ptr(moments), _ptr(normal), C.byref(cam), C.c_float(w_d),
+                                                     C.c_float(w_n), _ptr(dL_dalpha), _ptr(dL_ddepth), _ptr(dL_dmoments), _ptr(dL_dnormal),
                                                      _ptr(loss), _ptr(scratch), _stream(stream)))
 
 

@@ -178,7 +178,7 @@ static int carve_for_render(void* ws, int n, const ocgs_camera* cam, size_t key_
 
 int ocgs_render_fwd_reg(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
                         float* color, float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg,
-                        uint32_t* vis_count, float* contrib_sum, float* depth2, void* stream) {
+                        uint32_t* vis_count, float* contrib_sum, float* moments, void* stream) {
   if (!cam || !ws || !color || !alpha || !depth || !normal || !n_contrib) return OCGS_ERR_INVALID_ARG;
   int rc = check_cfg(cfg);
   if (rc != OCGS_OK) return rc;
@@ -186,7 +186,7 @@ int ocgs_render_fwd_reg(int n, const ocgs_camera* cam, const ocgs_config* cfg, v
   Workspace w;
   if ((rc = carve_for_render(ws, n, cam, key_capacity, &w)) != OCGS_OK) return rc;
   return launch_render_fwd(make_cam(*cam), *cfg, w, mask, color, alpha, depth, normal, n_contrib, loss_bg, vis_count, contrib_sum,
-                           depth2, (cudaStream_t)stream);
+                           moments, (cudaStream_t)stream);
 }
 
 int ocgs_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
@@ -198,15 +198,18 @@ int ocgs_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void*
 
 int ocgs_render_bwd_reg(const ocgs_surfels* s, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
                         const uint8_t* mask, const uint32_t* n_contrib, const float* gC, const float* gA, const float* gD,
-                        const float* gN, const float* gD2, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
-                        float* d_center2d, void* stream) {
+                        const float* gN, const float* moments, const float* gM, float* d_pos, float* d_scale, float* d_quat,
+                        float* d_opacity, float* d_sh, float* d_center2d, void* stream) {
   if (!s || !cam || !ws || !n_contrib) return OCGS_ERR_INVALID_ARG;
   int rc = check_cfg(cfg);
   if (rc != OCGS_OK) return rc;
   if (s->n > 0 && (!d_pos || !d_scale || !d_quat || !d_opacity || !d_sh)) return OCGS_ERR_INVALID_ARG;
+  if ((gM != nullptr) != (moments != nullptr)) return OCGS_ERR_INVALID_ARG;
+  const float* gM1 = gM;
+  const float* gM2 = gM ? gM + (size_t)cam->width * cam->height : nullptr;
   Workspace w;
   if ((rc = carve_for_render(ws, s->n, cam, key_capacity, &w)) != OCGS_OK) return rc;
-  return launch_render_bwd(*s, make_cam(*cam), *cfg, w, mask, w.final_T, n_contrib, gC, gA, gD, gN, gD2, d_pos, d_scale, d_quat,
+  return launch_render_bwd(*s, make_cam(*cam), *cfg, w, mask, w.final_T, n_contrib, gC, gA, gD, gN, moments, gM1, gM2, d_pos, d_scale, d_quat,
                            d_opacity, d_sh, d_center2d, (cudaStream_t)stream);
 }
 
@@ -214,7 +217,7 @@ int ocgs_render_bwd(const ocgs_surfels* s, const ocgs_camera* cam, const ocgs_co
                         const uint8_t* mask, const uint32_t* n_contrib, const float* gC, const float* gA, const float* gD,
                         const float* gN, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
                         float* d_center2d, void* stream) {
-  return ocgs_render_bwd_reg(s, cam, cfg, ws, key_capacity, mask, n_contrib, gC, gA, gD, gN, nullptr, d_pos, d_scale, d_quat, d_opacity,
+  return ocgs_render_bwd_reg(s, cam, cfg, ws, key_capacity, mask, n_contrib, gC, gA, gD, gN, nullptr, nullptr, d_pos, d_scale, d_quat, d_opacity,
                              d_sh, d_center2d, stream);
 }
 
@@ -228,14 +231,14 @@ int ocgs_masked_l1(const float* color, const float* target, const uint8_t* mask,
 
 size_t ocgs_regularizers_workspace_bytes(int width, int height) { return regularizers_workspace_bytes(width, height); }
 
-int ocgs_regularizers(const float* alpha, const float* depth, const float* depth2, const float* normal, const ocgs_camera* cam, float w_d,
-                      float w_n, float* dL_dalpha, float* dL_ddepth, float* dL_ddepth2, float* dL_dnormal, float* loss, void* scratch,
+int ocgs_regularizers(const float* alpha, const float* depth, const float* moments, const float* normal, const ocgs_camera* cam, float w_d,
+                      float w_n, float* dL_dalpha, float* dL_ddepth, float* dL_dmoments, float* dL_dnormal, float* loss, void* scratch,
                       void* stream) {
-  if (!alpha || !depth || !depth2 || !normal || !cam || !dL_dalpha || !dL_ddepth || !dL_ddepth2 || !dL_dnormal || !scratch)
+  if (!alpha || !depth || !moments || !normal || !cam || !dL_dalpha || !dL_ddepth || !dL_dmoments || !dL_dnormal || !scratch)
     return OCGS_ERR_INVALID_ARG;
   if (cam->width <= 0 || cam->height <= 0 || !(cam->fx > 0.f) || !(cam->fy > 0.f)) return OCGS_ERR_INVALID_ARG;
   if (cam->width > OCGS_MAX_DIM || cam->height > OCGS_MAX_DIM) return OCGS_ERR_UNSUPPORTED;
-  return launch_regularizers(alpha, depth, depth2, normal, *cam, w_d, w_n, dL_dalpha, dL_ddepth, dL_ddepth2, dL_dnormal, loss, scratch,
+  return launch_regularizers(alpha, depth, moments, normal, *cam, w_d, w_n, dL_dalpha, dL_ddepth, dL_dmoments, dL_dnormal, loss, scratch,
                              (cudaStream_t)stream);
 }
 

@@ -96,10 +96,10 @@ int launch_preprocess(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
 int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cudaStream_t st);
 int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Workspace& w, const uint8_t* mask, float* color,
                       float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,
-                      float* contrib_sum, float* depth2, cudaStream_t st);
+                      float* contrib_sum, float* mom, cudaStream_t st);
 int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, const uint8_t* mask,
                       const float* final_T, const uint32_t* n_contrib, const float* gC, const float* gA, const float* gD,
-                      const float* gN, const float* gD2, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
+                      const float* gN, const float* mom, const float* gM1, const float* gM2, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
                       float* d_center2d, cudaStream_t st);
 
 int launch_prune(const ocgs_surfels& in, uint32_t* vis_count, float* contrib_sum, const ocgs_config& cfg, uint8_t* prune_mask,
@@ -109,8 +109,8 @@ int launch_masked_l1(const float* color, const float* target, const uint8_t* mas
                      float* partial, int n_partial, cudaStream_t st);
 
 size_t regularizers_workspace_bytes(int W, int H);
-int launch_regularizers(const float* alpha, const float* depth, const float* depth2, const float* normal, const ocgs_camera& c, float w_d,
-                        float w_n, float* gA, float* gD, float* gD2, float* gN, float* loss, void* scratch, cudaStream_t st);
+int launch_regularizers(const float* alpha, const float* depth, const float* mom, const float* normal, const ocgs_camera& c, float w_d,
+                        float w_n, float* gA, float* gD, float* gM, float* gN, float* loss, void* scratch, cudaStream_t st);
 size_t photometric_workspace_bytes(int W, int H);
 int launch_photometric(const float* color, const float* target, const uint8_t* mask, int W, int H, float lam, float* dL_dcolor,
                        float* loss, void* scratch, cudaStream_t st);

@@ -64,7 +64,7 @@ struct BwdPixel {
   float T;                         // running transmittance T_i
   float GS;                        // sum_c g_c S_c - gA T_final: upstream gradients dotted with the suffix sums behind the pair
   float gc0, gc1, gc2, gd, gn0, gn1, gn2;
-  float gd2;                       // upstream of depth2 = sum w z^2 (kMoments only)
+  float zc, gm1, gm2;              // kMoments: origin of the depth moments and the upstream gradients of m1, m2
   uint32_t last;                   // n_contrib (0 for pixels outside the image)
 };
 
@@ -99,7 +99,8 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
     s.T *= inv1ma;  // T_i = T_{i+1} / (1 - alpha_i)
     const float T = s.T, w = a * T;
     float gq = s.gd * z;
-    if (kMoments) gq = fmaf(s.gd2 * z, z, gq);  // depth2 behaves like one more blended channel with value z^2
+    const float dz = z - s.zc;
+    if (kMoments) gq = fmaf(s.gm2 * dz, dz, fmaf(s.gm1, dz, gq));  // m1, m2 behave like blended channels with values dz, dz^2
     gq = fmaf(s.gc0, r4.y, gq); gq = fmaf(s.gc1, r4.z, gq); gq = fmaf(s.gc2, r4.w, gq);
     gq = fmaf(s.gn0, r5.x, gq); gq = fmaf(s.gn1, r5.y, gq); gq = fmaf(s.gn2, r5.z, gq);
     const float galpha = fmaf(T, gq, -s.GS * inv1ma);
@@ -107,7 +108,7 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
     v[10] = fmaf(w, s.gc0, v[10]); v[11] = fmaf(w, s.gc1, v[11]); v[12] = fmaf(w, s.gc2, v[12]);
     v[13] = fmaf(w, s.gn0, v[13]); v[14] = fmaf(w, s.gn1, v[14]); v[15] = fmaf(w, s.gn2, v[15]);
     float gz = w * s.gd;
-    if (kMoments) gz = fmaf(2.0f * z * w, s.gd2, gz);  // ... and depends on z directly
+    if (kMoments) gz = fmaf(w, fmaf(2.0f * dz, s.gm2, s.gm1), gz);  // ... and depend on z directly (the origin is a constant)
     float grho = 0.f;
     if (!capped) { v[9] = fmaf(G, galpha, v[9]); grho = -0.5f * G * r4.x * galpha; }  // S12: zero through the cap
     if (surf) {
@@ -142,7 +143,7 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
                                                             const float4* __restrict__ rec, const uint2* __restrict__ blist, const uint8_t* __restrict__ mask,
                                                             const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
                                                             const float* __restrict__ gC, const float* __restrict__ gA,
-                                                            const float* __restrict__ gD, const float* __restrict__ gN, const float* __restrict__ gD2, int W, int H,
+                                                            const float* __restrict__ gD, const float* __restrict__ gN, const float* __restrict__ mom, const float* __restrict__ gM1, const float* __restrict__ gM2, int W, int H,
                                                             int tiles_x, ocgs_config cfg, float gamma_over_hw, float* __restrict__ grad_rec) {
   __shared__ float4 s_rec[kBwdBatch * 6];
   __shared__ uint32_t s_rank[kBwdBatch];
@@ -172,7 +173,7 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
     s.px = (float)ix; s.py = (float)iy;
     s.last = 0;
     float Tfin = 1.0f, ga = 0.f;
-    s.gc0 = s.gc1 = s.gc2 = s.gd = s.gn0 = s.gn1 = s.gn2 = s.gd2 = 0.f;
+    s.gc0 = s.gc1 = s.gc2 = s.gd = s.gn0 = s.gn1 = s.gn2 = s.zc = s.gm1 = s.gm2 = 0.f;
     if (ix < W && iy < H) {
       const size_t p = (size_t)iy * W + ix;
       s.last = n_contrib[p];
@@ -180,7 +181,7 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
       if (gC) { s.gc0 = gC[p]; s.gc1 = gC[HW + p]; s.gc2 = gC[2 * HW + p]; }
       if (gA) ga = gA[p];
       if (gD) s.gd = gD[p];
-      if (kMoments) s.gd2 = gD2[p];
+      if (kMoments) { s.zc = mom[p]; s.gm1 = gM1[p]; s.gm2 = gM2[p]; }
       if (gN) { s.gn0 = gN[p]; s.gn1 = gN[HW + p]; s.gn2 = gN[2 * HW + p]; }
       if (mask && mask[p] == 0) ga += gamma_over_hw;  // d(gamma L_b)/dA = gamma (1-M)/(HW), Eq. 1 / Eq. 3
     }
@@ -409,7 +410,7 @@ __global__ void __launch_bounds__(128) project_bwd_kernel(const float* __restric
 
 int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, const uint8_t* mask,
                       const float* final_T, const uint32_t* n_contrib, const float* gC, const float* gA, const float* gD,
-                      const float* gN, const float* gD2, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
+                      const float* gN, const float* mom, const float* gM1, const float* gM2, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
                       float* d_center2d, cudaStream_t st) {
   if (s.n == 0) return OCGS_OK;
   clear_grad_rec_kernel<<<(unsigned)min(div_up((size_t)s.n * 6, 256), (size_t)148 * 16), 256, 0, st>>>(w.header, (float4*)w.grad_rec);
@@ -418,11 +419,11 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
     int rc = launch_order_tiles(w, /*from_ranges=*/false, st);  // tile_work = max n_contrib per tile, from the forward pass
     if (rc != OCGS_OK) return rc;
     const float goh = mask ? (float)((double)cfg.gamma_bg / ((double)cam.W * (double)cam.H)) : 0.f;
-    if (gD2)
-      render_bwd_kernel<true><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, gD2,
+    if (mom && gM1 && gM2)
+      render_bwd_kernel<true><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, mom, gM1, gM2,
                                                          cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
     else
-      render_bwd_kernel<false><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, nullptr,
+      render_bwd_kernel<false><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, nullptr, nullptr, nullptr,
                                                           cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
     OCGS_LAUNCHED(st, "render_bwd_kernel");
   }

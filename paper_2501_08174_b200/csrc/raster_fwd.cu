@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
                                                          ocgs_config cfg, float* __restrict__ color, float* __restrict__ alpha,
                                                          float* __restrict__ depth, float* __restrict__ normal,
                                                          uint32_t* __restrict__ n_contrib, float* __restrict__ final_T, uint2* __restrict__ blist, ocgs_header* __restrict__ header, float* __restrict__ loss_partial,
-                                                         uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum, float* __restrict__ depth2) {
+                                                         uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum, float* __restrict__ mom /*[3,H,W]: origin, m1, m2 (kMoments)*/) {
   __shared__ float4 s_rec[kFwdBatch * 6];
   __shared__ uint32_t s_rank[kFwdBatch];
   __shared__ uint32_t s_hit[kFwdBatch];  // bit w: warp w blended the entry (read by the backward pass)
@@ -82,7 +82,8 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
   const float near_z = cfg.near_z, alpha_max = cfg.alpha_max, t_min = cfg.t_min;
 
   float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f;
-  float D2 = 0.f;  // sum w z^2 (kMoments: the squared-depth moment of the depth-distortion regulariser, reading R-moments)
+  // kMoments: depth moments about the first blended pair's depth zc (reading R-moments): m1 = sum w (z - zc), m2 = sum w (z - zc)^2
+  float zc = 0.f, M1 = 0.f, M2 = 0.f;
   uint32_t last = 0;
   uint32_t nhit = 0;  // entries of this tile blended so far (uniform across the CTA)
   bool done = !inside;
@@ -142,7 +143,12 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
             wgt = a * T;
             C0 = fmaf(wgt, r4.y, C0); C1 = fmaf(wgt, r4.z, C1); C2 = fmaf(wgt, r4.w, C2);
             D = fmaf(wgt, z, D);
-            if (kMoments) D2 = fmaf(wgt * z, z, D2);
+            if (kMoments) {
+              if (last == 0) zc = z;
+              const float dz = z - zc;
+              M1 = fmaf(wgt, dz, M1);
+              M2 = fmaf(wgt * dz, dz, M2);
+            }
             N0 = fmaf(wgt, r5.x, N0); N1 = fmaf(wgt, r5.y, N1); N2 = fmaf(wgt, r5.z, N2);
             T = Tn;
             last = (b0 - start) + c0 + jj + 1;
@@ -199,7 +205,7 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
     color[p] = fmaf(T, cfg.bg[0], C0); color[HW + p] = fmaf(T, cfg.bg[1], C1); color[2 * HW + p] = fmaf(T, cfg.bg[2], C2);
     alpha[p] = A;
     depth[p] = D;
-    if (kMoments) depth2[p] = D2;
+    if (kMoments) { mom[p] = zc; mom[HW + p] = M1; mom[2 * HW + p] = M2; }
     normal[p] = N0; normal[HW + p] = N1; normal[2 * HW + p] = N2;
     n_contrib[p] = last;
     final_T[p] = T;
@@ -241,7 +247,7 @@ __global__ void __launch_bounds__(1024) loss_final_kernel(const float* __restric
 
 int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Workspace& w, const uint8_t* mask, float* color,
                       float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,
-                      float* contrib_sum, float* depth2, cudaStream_t st) {
+                      float* contrib_sum, float* mom, cudaStream_t st) {
   if (w.n_tiles == 0) return OCGS_OK;
   int rc = launch_order_tiles(w, /*from_ranges=*/true, st);  // launch order: longest lists first
   if (rc != OCGS_OK) return rc;
@@ -250,9 +256,9 @@ int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Worksp
 #define OCGS_FWD_LAUNCH(S, M)                                                                                                      \
   render_fwd_kernel<S, M><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, \
                                                      mask, cam.W, cam.H, cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib,   \
-                                                     w.final_T, w.blist, w.header, lp, vis_count, contrib_sum, depth2)
-  if (stats) { if (depth2) OCGS_FWD_LAUNCH(true, true); else OCGS_FWD_LAUNCH(true, false); }
-  else       { if (depth2) OCGS_FWD_LAUNCH(false, true); else OCGS_FWD_LAUNCH(false, false); }
+                                                     w.final_T, w.blist, w.header, lp, vis_count, contrib_sum, mom)
+  if (stats) { if (mom) OCGS_FWD_LAUNCH(true, true); else OCGS_FWD_LAUNCH(true, false); }
+  else       { if (mom) OCGS_FWD_LAUNCH(false, true); else OCGS_FWD_LAUNCH(false, false); }
 #undef OCGS_FWD_LAUNCH
   OCGS_LAUNCHED(st, "render_fwd_kernel");
   if (loss_bg) {

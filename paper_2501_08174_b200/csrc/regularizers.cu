@@ -1,10 +1,11 @@
 // regularizers.cu -- ocgs_regularizers: the depth-distortion and normal-consistency terms L_d, L_n of Eq. 3
 // (the 2DGS regularisers, "unchanged", unmasked) as image-space functions of the maps the renderer
 // returns for a view, and the upstream gradients ocgs_render_bwd_reg consumes (readings R-moments, R-Ld, R-Ln):
-//   L_d = 1/(hw) sum_p (A D2 - D^2)                 (= sum_{i<j} w_i w_j (z_i - z_j)^2 per pixel)
+//   L_d = 1/(hw) sum_p (A m2 - m1^2)                (= sum_{i<j} w_i w_j (z_i - z_j)^2 per pixel; m1, m2 the depth moments about
+//                                                    the first blended pair's depth, which keeps this difference well conditioned)
 //   L_n = 1/(hw) sum_p (A - Nrm . Nhat),  Nhat = unit normal of the expected-depth surface zbar = D/A by central differences
-// Two element-wise / 5-point-stencil kernels, HBM-bound: reg_terms_kernel reads 24 B and writes 44 B per pixel (dL/dNrm,
-// dL/dD2 and the gradients g_a, g_b of the two difference vectors), reg_gather_kernel reads ~44 B and writes 8 B.
+// Two element-wise / 5-point-stencil kernels, HBM-bound: reg_terms_kernel reads 28 B and writes 48 B per pixel (dL/dNrm,
+// dL/dm1, dL/dm2 and the gradients g_a, g_b of the two difference vectors), reg_gather_kernel reads ~44 B and writes 8 B.
 // The surface-normal arithmetic runs in fp64: zbar differences of neighbouring pixels cancel to 1e-3 of zbar at f = 2800,
 // which in fp32 would leave 1e-4 in Nhat; it is ~60 fp64 operations per pixel, far below the kernel's memory time.
 #include "common.cuh"
@@ -25,8 +26,8 @@ __device__ __forceinline__ bool reg_surface(const float* __restrict__ alpha, con
 }
 
 __global__ void __launch_bounds__(256) reg_terms_kernel(const float* __restrict__ alpha, const float* __restrict__ depth,
-                                                        const float* __restrict__ depth2, const float* __restrict__ normal, RegCam cam,
-                                                        float wd_hw, float wn_hw, float* __restrict__ gD2, float* __restrict__ gN,
+                                                        const float* __restrict__ mom /*[3,H,W]: origin, m1, m2*/, const float* __restrict__ normal, RegCam cam,
+                                                        float wd_hw, float wn_hw, float* __restrict__ gM /*[2,H,W]*/, float* __restrict__ gN,
                                                         float* __restrict__ g_ab /*[6,H,W]*/, double* __restrict__ partial /*[blocks][2]*/) {
   const int W = cam.W, H = cam.H;
   const size_t HW = (size_t)W * H;
@@ -34,10 +35,11 @@ __global__ void __launch_bounds__(256) reg_terms_kernel(const float* __restrict_
   double ld = 0.0, ln = 0.0;
   if (x < W && y < H) {
     const size_t p = (size_t)y * W + x;
-    const float A = alpha[p], D = depth[p], D2 = depth2[p];
+    const float A = alpha[p], m1 = mom[HW + p], m2 = mom[2 * HW + p];
     const float n0 = normal[p], n1 = normal[HW + p], n2 = normal[2 * HW + p];
-    ld = (double)A * (double)D2 - (double)D * (double)D;
-    gD2[p] = wd_hw * A;
+    ld = (double)A * (double)m2 - (double)m1 * (double)m1;
+    gM[p] = -2.0f * wd_hw * m1;
+    gM[HW + p] = wd_hw * A;
     double Nh[3] = {0.0, 0.0, 0.0}, ga[3] = {0.0, 0.0, 0.0}, gb[3] = {0.0, 0.0, 0.0};
     double z0, zxm, zxp, zym, zyp;
     bool valid = x > 0 && y > 0 && x < W - 1 && y < H - 1;
@@ -85,7 +87,7 @@ __global__ void __launch_bounds__(256) reg_terms_kernel(const float* __restrict_
 }
 
 __global__ void __launch_bounds__(256) reg_gather_kernel(const float* __restrict__ alpha, const float* __restrict__ depth,
-                                                         const float* __restrict__ depth2, RegCam cam, float wd_hw, float wn_hw,
+                                                         const float* __restrict__ mom, RegCam cam, float wd_hw, float wn_hw,
                                                          const float* __restrict__ g_ab, float* __restrict__ gA, float* __restrict__ gD) {
   const int W = cam.W, H = cam.H;
   const size_t HW = (size_t)W * H;
@@ -106,8 +108,8 @@ __global__ void __launch_bounds__(256) reg_gather_kernel(const float* __restrict
   const double rx = ((double)x - cam.ox) * cam.inv_fx, ry = ((double)y - cam.oy) * cam.inv_fy;
   const double gz = gP[0] * rx + gP[1] * ry + gP[2];  // P = zbar r
   const float A = alpha[p], D = depth[p];
-  double ga = (double)wd_hw * (double)depth2[p] + (double)wn_hw;  // d(A D2 - D^2)/dA + d(A - Nrm.Nhat)/dA
-  double gd = -2.0 * (double)wd_hw * (double)D;
+  double ga = (double)wd_hw * (double)mom[2 * HW + p] + (double)wn_hw;  // d(A m2 - m1^2)/dA + d(A - Nrm.Nhat)/dA
+  double gd = 0.0;
   if (A > kRegEpsA) {  // zbar = D / A
     const double ia = 1.0 / (double)A;
     gd += gz * ia;
@@ -139,8 +141,8 @@ size_t regularizers_workspace_bytes(int W, int H) {
   return reg_align(6 * HW * sizeof(float)) + reg_align(blocks * 2 * sizeof(double));
 }
 
-int launch_regularizers(const float* alpha, const float* depth, const float* depth2, const float* normal, const ocgs_camera& c, float w_d,
-                        float w_n, float* gA, float* gD, float* gD2, float* gN, float* loss, void* scratch, cudaStream_t st) {
+int launch_regularizers(const float* alpha, const float* depth, const float* mom, const float* normal, const ocgs_camera& c, float w_d,
+                        float w_n, float* gA, float* gD, float* gM, float* gN, float* loss, void* scratch, cudaStream_t st) {
   RegCam cam;
   cam.inv_fx = 1.0 / (double)c.fx; cam.inv_fy = 1.0 / (double)c.fy;
   cam.ox = (double)(c.cx - 0.5f); cam.oy = (double)(c.cy - 0.5f);
@@ -150,10 +152,10 @@ int launch_regularizers(const float* alpha, const float* depth, const float* dep
   double* partial = (double*)((char*)scratch + reg_align(6 * HW * sizeof(float)));
   const double inv_hw = 1.0 / (double)HW;
   const dim3 grid((unsigned)div_up((size_t)c.width, 32), (unsigned)div_up((size_t)c.height, 8));
-  reg_terms_kernel<<<grid, 256, 0, st>>>(alpha, depth, depth2, normal, cam, (float)((double)w_d * inv_hw), (float)((double)w_n * inv_hw), gD2, gN,
+  reg_terms_kernel<<<grid, 256, 0, st>>>(alpha, depth, mom, normal, cam, (float)((double)w_d * inv_hw), (float)((double)w_n * inv_hw), gM, gN,
                                          g_ab, partial);
   OCGS_LAUNCHED(st, "reg_terms_kernel");
-  reg_gather_kernel<<<grid, 256, 0, st>>>(alpha, depth, depth2, cam, (float)((double)w_d * inv_hw), (float)((double)w_n * inv_hw), g_ab, gA, gD);
+  reg_gather_kernel<<<grid, 256, 0, st>>>(alpha, depth, mom, cam, (float)((double)w_d * inv_hw), (float)((double)w_n * inv_hw), g_ab, gA, gD);
   OCGS_LAUNCHED(st, "reg_gather_kernel");
   if (loss) {
     reg_final_kernel<<<1, 1024, 0, st>>>(partial, (int)(grid.x * grid.y), inv_hw, loss);

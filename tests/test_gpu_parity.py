@@ -122,9 +122,9 @@ def test_sh_degrees():
         full_parity(sc, 0, dict(sh_degree=deg))
 
 
-def test_depth_moment_map_and_its_gradient():
-    """SURVEY.md 8(f) f-2 / reading R-moments: ocgs_render_fwd_reg's depth2 = sum w z^2 and ocgs_render_bwd_reg's upstream
-    gradient of it, against the oracle; the other maps must be bit-identical to the plain forward."""
+def test_depth_moments_and_their_gradient():
+    """SURVEY.md 8(f) f-2 / reading R-moments: ocgs_render_fwd_reg's (origin, m1, m2) and ocgs_render_bwd_reg's upstream
+    gradients of m1, m2, against the oracle; the other maps must be bit-identical to the plain forward."""
     for sc, cfg_kw in ((sg.random_scene(300, 100, 70, 80.0, seed=3, sh_degree=3), dict(sh_degree=3)),
                        (sg.make_scene("config2", n_obj=20_000, n_bg=20_000), dict(sh_degree=3))):
         P = arrays(sc)
@@ -138,21 +138,20 @@ def test_depth_moment_map_and_its_gradient():
         for k in ("color", "alpha", "depth", "normal", "n_contrib"):
             assert np.array_equal(plain[k], gf[k]), k
         ok = fw["fragile"] == 0
-        err = np.abs(gf["depth2"] - fw["depth2"]) / np.maximum(1.0, np.abs(fw["depth2"]))
-        assert (err * ok).max() <= IMG_TOL, (err * ok).max()
+        for i, k in enumerate(("origin", "m1", "m2")):
+            err = np.abs(gf["moments"][i] - fw[k]) / np.maximum(1.0, np.abs(fw[k]))
+            assert (err * ok).max() <= IMG_TOL, (k, (err * ok).max())
         rng = np.random.default_rng(17)
         H, W = camn.height, camn.width
         okf = ok.astype(np.float64)
-        gC, gD, gD2 = rng.normal(size=(3, H, W)) * okf, rng.normal(size=(H, W)) * okf, rng.normal(size=(H, W)) * okf
+        gC, gD, gM = rng.normal(size=(3, H, W)) * okf, rng.normal(size=(H, W)) * okf, rng.normal(size=(2, H, W)) * okf
         mm = np.where(ok, m, 1).astype(np.uint8)
-        gg = g.render_bwd(gC=gC, gD=gD, gD2=gD2, mask=mm)
-        og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=gC.astype(np.float32), gD=gD.astype(np.float32), gD2=gD2.astype(np.float32))
-        check_grads(gg, og)
-        # the moment channel alone
-        gg2 = g.render_bwd(gD2=gD2, mask=None)
-        cfg0 = orc.default_config(sh_degree=3, gamma_bg=0.0)
-        og2 = orc.render_bwd(*P, pre, srt, cam, cfg0, mask=None, gD2=gD2.astype(np.float32))
-        check_grads(gg2, og2)
+        gg = g.render_bwd(gC=gC, gD=gD, gM=gM, mask=mm)
+        og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=gC.astype(np.float32), gD=gD.astype(np.float32),
+                            gM1=gM[0].astype(np.float32), gM2=gM[1].astype(np.float32))
+        # dz = z_i - z_first is a difference of fp32 depths (each good to ~3e-7 at z ~ 3): for thin surfaces the terms
+        # proportional to dz carry that absolute noise, so the floor is 1e-4 of each array's typical (99th percentile) scale
+        check_grads(gg, og, floor_frac=1e-4)
 
 
 def test_empty_and_all_culled_and_capacity():
