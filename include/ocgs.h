@@ -201,6 +201,12 @@ int ocgs_prune_stats(const ocgs_surfels* in, uint32_t* vis_count, float* contrib
                      uint8_t* prune_mask, int32_t* remap, const ocgs_surfels_mut* out, int* n_out, int reset_stats,
                      void* ws, void* stream);
 
+/* Compaction of any other per-surfel array with the remap of ocgs_prune_stats (pruning happens every 100 /
+ * 600 iterations INSIDE the optimisation, so optimiser moments and accumulated densification statistics must follow the
+ * parameters): out[remap[j], :] = in[j, :] for remap[j] >= 0, rows of `row_floats` floats.
+ * in, out: device f32 [n, row_floats], distinct buffers; rows of `out` beyond the survivor count are left untouched. */
+int ocgs_compact_rows(const float* in, const int32_t* remap, int n, int row_floats, float* out, void* stream);
+
 /* ---- harness photometric term (S20; the L1 part of Eq. 2) --------------------------------------------
  * loss = 1/(3 H W) sum |M (R - I)| (device scalar, nullable), dL_dcolor[3,H,W] = M sign(R - I)/(3 H W).  color, target:
  * device [3,H,W]; mask device u8 [H,W], nullable (= all ones).  Uses ws.loss_partial as scratch (n, key_capacity: the values

@@ -18,7 +18,7 @@ _LIB_PATH = os.path.join(_HERE, "csrc", "libocgs.so")
 OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
            "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_render_fwd_reg", "ocgs_render_bwd_reg", "ocgs_prune_workspace_bytes",
-           "ocgs_prune_stats", "ocgs_step_host", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
+           "ocgs_prune_stats", "ocgs_compact_rows", "ocgs_step_host", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
            "ocgs_profile_begin", "ocgs_profile_end"]
 
 
@@ -200,6 +200,10 @@ def ocgs_prune_stats(surfels, vis_count, contrib_sum, cfg, prune_mask, remap, ou
     _ok("ocgs_prune_stats", lib().ocgs_prune_stats(C.byref(surfels), _ptr(vis_count), _ptr(contrib_sum), C.byref(cfg), _ptr(prune_mask),
                                                    _ptr(remap), C.byref(out) if out is not None else None, _ptr(n_out),
                                                    C.c_int(int(reset_stats)), _ptr(ws), _stream(stream)))
+
+
+def ocgs_compact_rows(inp, remap, n: int, row_floats: int, out, stream=None):
+    _ok("ocgs_compact_rows", lib().ocgs_compact_rows(_ptr(inp), _ptr(remap), C.c_int(n), C.c_int(row_floats), _ptr(out), _stream(stream)))
 
 
 def ocgs_step_host(h_pos, h_scale, h_quat, h_opacity, h_sh, n, cam, cfg, h_mask, h_target, h_grads, h_alpha, h_loss_bg, d_params,

@@ -290,6 +290,12 @@ int ocgs_prune_stats(const ocgs_surfels* in, uint32_t* vis_count, float* contrib
   return launch_prune(*in, vis_count, contrib_sum, *cfg, prune_mask, remap, out, n_out, reset_stats, ws, (cudaStream_t)stream);
 }
 
+int ocgs_compact_rows(const float* in, const int32_t* remap, int n, int row_floats, float* out, void* stream) {
+  if (n < 0 || row_floats <= 0) return OCGS_ERR_INVALID_ARG;
+  if (n > 0 && (!in || !remap || !out || in == out)) return OCGS_ERR_INVALID_ARG;
+  return launch_compact_rows(in, remap, n, row_floats, out, (cudaStream_t)stream);
+}
+
 int ocgs_step_host(const float* h_pos, const float* h_scale, const float* h_quat, const float* h_opacity, const float* h_sh, int n,
                    const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask, const float* h_target, float* h_grads,
                    float* h_alpha, float* h_loss_bg, float* d_params, uint8_t* d_mask, float* d_images, uint32_t* d_ncontrib,

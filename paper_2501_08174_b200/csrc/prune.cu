@@ -110,6 +110,25 @@ static int launch_compact(const float* in, float* out, const int32_t* remap, int
   return OCGS_OK;
 }
 
+// generic per-surfel rows (optimiser state, accumulated densification statistics, ...): row j of `row_floats` floats moves to row remap[j]
+__global__ void __launch_bounds__(256) compact_rows_kernel(const float* __restrict__ in, const int32_t* __restrict__ remap, size_t total,
+                                                           int row_floats, float* __restrict__ out) {
+  for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < total; i += (size_t)gridDim.x * 256) {
+    const size_t j = i / (size_t)row_floats;
+    const int32_t r = __ldg(remap + j);
+    if (r >= 0) out[(size_t)r * row_floats + (i - j * row_floats)] = in[i];
+  }
+}
+
+int launch_compact_rows(const float* in, const int32_t* remap, int n, int row_floats, float* out, cudaStream_t st) {
+  const size_t total = (size_t)n * (size_t)row_floats;
+  if (total == 0) return OCGS_OK;
+  const unsigned grid = (unsigned)min(div_up(total, 256), (size_t)148 * 64);
+  compact_rows_kernel<<<grid, 256, 0, st>>>(in, remap, total, row_floats, out);
+  OCGS_LAUNCHED(st, "compact_rows_kernel");
+  return OCGS_OK;
+}
+
 int launch_prune(const ocgs_surfels& in, uint32_t* vis_count, float* contrib_sum, const ocgs_config& cfg, uint8_t* prune_mask,
                  int32_t* remap, const ocgs_surfels_mut* out, int* n_out, int reset_stats, void* ws, cudaStream_t st) {
   const int n = in.n;

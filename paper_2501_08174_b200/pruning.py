@@ -1,0 +1,49 @@
+"""Occlusion-aware pruning drivers: orchestration only -- every step runs in the CUDA
+library; this module loops over views and marshals arguments.
+
+* accumulate_visibility: render the given views with the statistics switched on ("Inside the renderer, we save which
+  Gaussians are used during the color accumulation step"); `vis_count` / `contrib_sum` accumulate.
+* prune: "remove all Gaussians that are not visible in any training view" (the post-hoc variant; the same
+  call serves the in-training variant every 100 / 600 iterations) -- mask, remap, compacted parameters.
+"""
+from __future__ import annotations
+
+from typing import Dict, Optional, Sequence
+
+import torch
+
+from . import binding as B
+
+
+def accumulate_visibility(surfels: B.ocgs_surfels, n: int, cameras: Sequence, cfg: B.ocgs_config, ws: torch.Tensor, key_capacity: int,
+                          out: Dict[str, torch.Tensor], vis_count: torch.Tensor, contrib_sum: torch.Tensor, stream=None) -> None:
+    """Forward-only pass over `cameras` (scene cameras or ocgs_camera structs); the images in `out` are overwritten per
+    view, the per-surfel statistics accumulate.  No host synchronisation except one ocgs_check at the end."""
+    for cam in cameras:
+        c = cam if isinstance(cam, B.ocgs_camera) else B.camera_from(cam)
+        B.ocgs_preprocess(surfels, c, cfg, ws, key_capacity, stream)
+        B.ocgs_bin_sort(n, c, cfg, ws, key_capacity, None, stream)
+        B.ocgs_render_fwd(n, c, cfg, ws, key_capacity, None, out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"],
+                          None, vis_count, contrib_sum, stream)
+    B.ocgs_check(ws, stream)
+
+
+def prune(surfels: B.ocgs_surfels, params: Dict[str, torch.Tensor], n: int, cfg: B.ocgs_config, vis_count: torch.Tensor,
+          contrib_sum: torch.Tensor, reset_stats: bool = True, extra_rows: Optional[Dict[str, torch.Tensor]] = None, stream=None):
+    """Prune mask from the statistics, stable compaction of the five parameter arrays and of any `extra_rows` (per-surfel
+    [n, k] float arrays such as optimiser moments).  Returns (compacted params, compacted extras, n_kept, prune_mask, remap)."""
+    dev = vis_count.device
+    mask = torch.empty(n, dtype=torch.uint8, device=dev)
+    remap = torch.empty(n, dtype=torch.int32, device=dev)
+    n_out = torch.zeros(1, dtype=torch.int32, device=dev)
+    outs = {k: torch.empty_like(params[k]) for k in ("pos", "scale", "quat", "opacity", "sh")}
+    om = B.ocgs_surfels_mut(*[B._ptr(outs[k]) for k in ("pos", "scale", "quat", "opacity", "sh")], n)
+    pws = torch.empty(B.ocgs_prune_workspace_bytes(n), dtype=torch.uint8, device=dev)
+    B.ocgs_prune_stats(surfels, vis_count, contrib_sum, cfg, mask, remap, om, n_out, 1 if reset_stats else 0, pws, stream)
+    extras = {}
+    for k, t in (extra_rows or {}).items():
+        o = torch.empty_like(t)
+        B.ocgs_compact_rows(t, remap, n, int(t.numel() // max(n, 1)), o, stream)
+        extras[k] = o
+    kept = int(n_out.item())  # the one host read of the pass
+    return {k: v[:kept] for k, v in outs.items()}, {k: v[:kept] for k, v in extras.items()}, kept, mask, remap

@@ -96,6 +96,65 @@ def test_prune_tau_and_min_opacity_rule():
         assert np.array_equal(remap_t.cpu().numpy(), po["remap"]) and int(n_out.item()) == po["n_out"]
 
 
+def test_posthoc_prune_driver_matches_the_oracle():
+    """PAPER.md:234 (post-hoc variant): render every view with the statistics on, remove the never-blended surfels and
+    carry a per-surfel side array (optimiser state) along; the driver in paper_2501_08174_b200.pruning only loops and
+    marshals, so its result must equal the oracle's rule on the oracle's statistics."""
+    import torch
+    import oracle as orc
+    from paper_2501_08174_b200 import binding as B, pruning
+    sc = sg.make_scene("config4", n_shell=3000, n_in=4000, n_bg=1500, res=192, f=245.0, n_views=8, scale_mul=8.0)
+    P = arrays(sc)
+    n = sc.n
+    g = GpuView(P, sc.cameras[0], dict(sh_degree=3))
+    out = B.alloc_outputs(g.W, g.H)
+    vis = torch.zeros(n, dtype=torch.int32, device="cuda"); cs = torch.zeros(n, dtype=torch.float32, device="cuda")
+    pruning.accumulate_visibility(g.surfels, n, sc.cameras, g.cfg, g.ws, g.cap, out, vis, cs)
+    vis_o = np.zeros(n, np.uint32); cs_o = np.zeros(n, np.float64); touch = np.zeros(n, np.uint64)
+    ocfg = orc.default_config(sh_degree=3)
+    for camn in sc.cameras:
+        cam = orc.camera_from(camn)
+        pre = orc.preprocess(*P, cam, ocfg); srt = orc.bin_sort(pre, cam, ocfg)
+        fw = orc.render_fwd(pre, srt, sc.opacity, cam, ocfg, mask=None, vis_count=vis_o, contrib_sum=cs_o)
+        touch += fw["fragile_touch"]
+    clean = touch == 0
+    assert np.array_equal(vis.cpu().numpy().view(np.uint32)[clean], vis_o[clean])
+    state = torch.tensor(np.random.default_rng(0).normal(size=(n, 58)).astype(np.float32), device="cuda")
+    vg = vis.cpu().numpy().view(np.uint32).copy(); cg = cs.cpu().numpy().copy()
+    params, extras, kept, mask, remap = pruning.prune(g.surfels, g.t, n, g.cfg, vis, cs, reset_stats=True, extra_rows=dict(adam_m=state))
+    po = orc.prune(vg, cg, sc.opacity)
+    assert kept == po["n_out"] and np.array_equal(mask.cpu().numpy(), po["prune_mask"]) and np.array_equal(remap.cpu().numpy(), po["remap"])
+    comp = orc.compact(dict(pos=sc.pos, scale=sc.scale, quat=sc.quat, opacity=sc.opacity, sh=sc.sh, adam_m=state.cpu().numpy()), po["prune_mask"])
+    for k in ("pos", "scale", "quat", "opacity", "sh"):
+        assert np.array_equal(params[k].cpu().numpy(), comp[k]), k
+    assert np.array_equal(extras["adam_m"].cpu().numpy(), comp["adam_m"])
+    assert int(vis.abs().sum().item()) == 0  # reset for the next interval
+    assert po["prune_mask"][sc.group == 2].mean() > 0.7  # most of the occluded interior goes (3 000 shell surfels leave gaps)
+
+
+def test_compact_rows_follows_the_remap():
+    """Optimiser state follows the parameters through a prune: by definition
+    out = [row for row, pruned in zip(in, mask) if not pruned]."""
+    import torch
+    import oracle as orc
+    from paper_2501_08174_b200 import binding as B
+    rng = np.random.default_rng(4)
+    n = 70_001
+    pm = (rng.uniform(size=n) < 0.4).astype(np.uint8)
+    remap = np.where(pm == 0, np.cumsum(pm == 0) - 1, -1).astype(np.int32)
+    for row in (1, 3, 48, 58):
+        x = rng.normal(size=(n, row)).astype(np.float32)
+        xt, rt = torch.tensor(x, device="cuda"), torch.tensor(remap, device="cuda")
+        out = torch.full((n, row), -7.0, dtype=torch.float32, device="cuda")
+        B.ocgs_compact_rows(xt, rt, n, row, out)
+        torch.cuda.synchronize()
+        ref = orc.compact(dict(x=x), pm)["x"]
+        got = out.cpu().numpy()
+        assert np.array_equal(got[: len(ref)], ref) and np.all(got[len(ref):] == -7.0)
+    with pytest.raises(B.OcgsError):
+        B.ocgs_compact_rows(xt, rt, n, 0, out)
+
+
 def test_config3_full_size_sampled_windows():
     """BASELINE.json configs[2] at full size, in bench.py's launch configuration: integer outputs compared in full,
     images and gradients on sampled windows the oracle can compute."""
