@@ -25,9 +25,9 @@ sys.path.insert(0, ROOT)
 METRIC = "ms per fwd+bwd raster step (1600x1200, 1M surfels)"
 FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 40.0, 22.0, 72.0  # DESIGN.md section 6 "algorithmic work per unit" (FMA = 2)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the raster kernels, from the `ncu --set full` capture of this
-# workload committed as profiles/r01d_raster_kernels_full.md (bytes)
-NCU_TRAFFIC = {"render_bwd_kernel": 95.6e6, "render_fwd_kernel": 85.5e6}
-NCU_TRAFFIC_SOURCE = "profiles/r01d_raster_kernels_full.md"
+# workload committed as profiles/r01e_raster_kernels_full.md (bytes)
+NCU_TRAFFIC = {"render_bwd_kernel": 89.5e6, "render_fwd_kernel": 92.3e6}
+NCU_TRAFFIC_SOURCE = "profiles/r01e_raster_kernels_full.md"
 ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 148 SMs x 128 FP32 lanes x 2 (FMA) x max SM clock (B200_PROFILING.md)
 
 
@@ -45,6 +45,7 @@ def parse_args():
     ap.add_argument("--loss", default="l1", choices=["l1", "dssim", "eq3"],
                     help="loss of the step: masked L1 (harness loss S20, the default the metric is quoted on); the full L_c^M = 0.8 L1 + 0.2 D-SSIM of "
                          "Eq. 2 (ocgs_photometric_loss); or all of Eq. 3 (moment forward, ocgs_regularizers, moment backward)")
+    ap.add_argument("--no-prune", action="store_true", help="skip the separately timed prune pass (profiling runs)")
     ap.add_argument("--no-graph", action="store_true", help="time direct kernel launches instead of CUDA graph replays")
     return ap.parse_args()
 
@@ -343,7 +344,7 @@ def run_ours(args):
     # ---- prune pass, timed separately: once per pruning interval, not per step -------------------
     # statistics of the nv views just rendered -> mask -> scan -> stable compaction of all five parameter arrays
     prune = None
-    if rank == 0:
+    if rank == 0 and not args.no_prune:
         vis.zero_(); cs.zero_()
         for i in range(nv):
             step(i)
