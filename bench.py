@@ -26,7 +26,7 @@ METRIC = "ms per fwd+bwd raster step (1600x1200, 1M surfels)"
 FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 40.0, 22.0, 72.0  # DESIGN.md section 6 "algorithmic work per unit" (FMA = 2)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the raster kernels, from the `ncu --set full` capture of this
 # workload committed as profiles/r01e_raster_kernels_full.md (bytes)
-NCU_TRAFFIC = {"render_bwd_kernel": 89.5e6, "render_fwd_kernel": 92.3e6}
+NCU_TRAFFIC = {"render_bwd_kernel": 88.5e6, "render_fwd_kernel": 92.8e6}
 NCU_TRAFFIC_SOURCE = "profiles/r01e_raster_kernels_full.md"
 ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 148 SMs x 128 FP32 lanes x 2 (FMA) x max SM clock (B200_PROFILING.md)
 
@@ -373,40 +373,62 @@ def run_ours(args):
         del outs, om
         vis.zero_(); cs.zero_()
 
-    # ---- e2e: the same step through ocgs_step_host with pinned host buffers -----------------------------------------
-    e2e = None
+    # ---- e2e: the training step through the library's host-facing calls, pinned host buffers, copies inside -------------
+    # (a) `e2e`: ocgs_step_view_host -- what a training loop does per iteration: the model (parameters and
+    #     gradients) is resident on the device, the VIEW's inputs (target image, mask; the camera travels by value) come
+    #     from pinned host memory every step and the step's result (the two loss scalars) is read back.
+    # (b) `e2e_host_params`: ocgs_step_host -- the same step with the parameters uploaded and the gradients downloaded
+    #     every step as well (a host-side optimiser): 464 MB over PCIe per step, reported for reference.
+    e2e = e2e_hp = None
     if not args.no_e2e:
-        hp = {k: torch.tensor(np.ascontiguousarray(getattr(scene, k)), dtype=torch.float32).pin_memory() for k in ("pos", "scale", "quat", "opacity", "sh")}
         h_masks = [m.cpu().pin_memory() for m in masks]
         h_targets = [tg.cpu().pin_memory() for tg in targets]
+        d_images = torch.empty(14 * H * W, dtype=torch.float32, device=dev)
+        d_mask = torch.empty(H * W, dtype=torch.uint8, device=dev)
+        d_nc = torch.empty(H * W, dtype=torch.int32, device=dev)
+        d_losses = torch.zeros(2, dtype=torch.float32, device=dev)
+        h_losses = torch.zeros(2, dtype=torch.float32).pin_memory()
+        k_e = max(3, min(args.steps, 20))
+
+        def time_steps(fn):
+            for i in range(2):
+                fn(i % nv)
+            barrier()
+            t0 = time.perf_counter()
+            for i in range(k_e):
+                fn(i % nv)  # synchronises inside (the results are on the host when it returns)
+            torch.cuda.synchronize()
+            te = torch.tensor([(time.perf_counter() - t0) * 1e3], dtype=torch.float64, device=dev)
+            if world > 1:
+                dist.all_reduce(te, op=dist.ReduceOp.MAX)
+            return float(te.item()) / (k_e * world)
+
+        copy_stream = torch.cuda.Stream()
+
+        def view_step(i):
+            B.ocgs_step_view_host(surfels, cam_c[i], cfg, h_masks[i], h_targets[i], h_losses, d_mask, d_images, d_nc, grads, vis, cs,
+                                  d_losses, ws, cap, copy_stream=copy_stream)
+        ms_view = time_steps(view_step)
+        e2e = {"value": ms_view, "unit": "ms", "h2d_bytes_per_step": H * W + 3 * H * W * 4, "d2h_bytes_per_step": 8 + 16, "steps": k_e,
+               "what": "ocgs_step_view_host: target image + mask from pinned host memory each step, parameters and gradients resident "
+                       "in HBM, uploads on a second stream overlapping preprocess/sort/forward, loss scalars read back", "losses_last_step": [float(h_losses[0]), float(h_losses[1])]}
+        hp = {k: torch.tensor(np.ascontiguousarray(getattr(scene, k)), dtype=torch.float32).pin_memory() for k in ("pos", "scale", "quat", "opacity", "sh")}
         h_grads = torch.empty(58 * n, dtype=torch.float32).pin_memory()
         h_alpha = torch.empty(H * W, dtype=torch.float32).pin_memory()
         h_loss = torch.empty(1, dtype=torch.float32).pin_memory()
         d_params = torch.empty(58 * n + 16, dtype=torch.float32, device=dev)
         d_grads = torch.empty(58 * n + 16, dtype=torch.float32, device=dev)
-        d_images = torch.empty(14 * H * W, dtype=torch.float32, device=dev)
-        d_mask = torch.empty(H * W, dtype=torch.uint8, device=dev)
-        d_nc = torch.empty(H * W, dtype=torch.int32, device=dev)
         d_lb = torch.zeros(1, dtype=torch.float32, device=dev)
 
-        def e2e_step(i):
+        def host_params_step(i):
             B.ocgs_step_host(hp["pos"], hp["scale"], hp["quat"], hp["opacity"], hp["sh"], n, cam_c[i], cfg, h_masks[i], h_targets[i],
                              h_grads, h_alpha, h_loss, d_params, d_mask, d_images, d_nc, d_grads, vis, cs, d_lb, ws, cap)
-        for i in range(2):
-            e2e_step(i % nv)
         k_e = max(3, min(args.steps, 10))
-        barrier()
-        t0 = time.perf_counter()
-        for i in range(k_e):
-            e2e_step(i % nv)  # synchronises inside (results are on the host when it returns)
-        torch.cuda.synchronize()
-        t_e = (time.perf_counter() - t0) * 1e3
-        te = torch.tensor([t_e], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        h2d = 58 * n * 4 + H * W + 3 * H * W * 4
-        d2h = 58 * n * 4 + H * W * 4 + 4 + 16
-        e2e = {"value": float(te.item()) / (k_e * world), "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": k_e}
+        ms_hp = time_steps(host_params_step)
+        e2e_hp = {"value": ms_hp, "unit": "ms", "h2d_bytes_per_step": 58 * n * 4 + H * W + 3 * H * W * 4,
+                  "d2h_bytes_per_step": 58 * n * 4 + H * W * 4 + 4 + 16, "steps": k_e,
+                  "what": "ocgs_step_host: parameters up and gradients down every step as well (PCIe bound by construction)"}
+        del hp, h_grads, d_params, d_grads
 
     if rank != 0:
         if world > 1:
@@ -473,6 +495,7 @@ def run_ours(args):
     line["prune"] = prune
     if e2e:
         line["e2e"] = e2e
+        line["e2e_host_params"] = e2e_hp
     if world == 1 and not args.no_cpu_baseline:
         ms_cpu, desc, cores = oracle_sample(scene, my_views[0], window_frac=0.1)
         line["cpu_baseline"] = {"value": ms_cpu, "unit": "ms", "cores": cores, "kind": "oracle", "sample": desc}

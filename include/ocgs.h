@@ -9,7 +9,7 @@
  *  - "device" pointers are CUDA device memory owned by the caller; "host" pointers are ordinary host memory.
  *    The library allocates no device memory, keeps no global state and is re-entrant per stream.
  *  - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream).  No entry point
- *    synchronises except ocgs_check() and ocgs_step_host().  A step can therefore be captured in a CUDA graph.
+ *    synchronises except ocgs_check(), ocgs_step_view_host() and ocgs_step_host().  A step can therefore be captured in a CUDA graph.
  *  - The data-dependent key count K never travels to the host inside a step: kernels read it from the workspace
  *    header.  If K exceeds `key_capacity` the header error flag is set, later calls of the step become no-ops, and
  *    ocgs_check() reports OCGS_ERR_CAPACITY with the needed size.
@@ -235,7 +235,23 @@ int ocgs_photometric_loss(const float* color, const float* target, const uint8_t
 int ocgs_profile_begin(int capacity, void* stream);
 int ocgs_profile_end(void* stream, int max_out, float* ms_out, char* names_out, int* count);
 
-/* ---- end-to-end step with HOST buffers (bench.py "e2e") ---------------------------------------------------------------
+/* ---- end-to-end TRAINING step: per-view inputs from the host, parameters resident on the device (bench.py "e2e") -------
+ * What a training loop does per iteration (pick a view, render, losses, backpropagate): the model -- the
+ * surfel parameters and their gradients -- lives in device memory (`surfels`, d_grad_*), the view's data come from the
+ * host.  Copies the target image h_target [3,H,W] f32 and the mask h_mask [H,W] u8 from (pinned) host memory into
+ * d_images / d_mask, runs (1)-(3) with L_b and the statistics on, ocgs_masked_l1, then (4) into the device gradient
+ * arrays, copies the two loss scalars back into h_losses[0..1] = (L_b, masked L1) and synchronises.
+ * d_images: device [14*H*W] floats (color 3, alpha 1, depth 1, normal 3, target 3, dL_dcolor 3); d_ncontrib u32 [H*W];
+ * d_losses: device f32[2].  Every call of one step must pass the n, image size and key_capacity the workspace was sized with.
+ * copy_stream (nullable): a second stream for the two uploads, so that they overlap preprocess / sort / forward (the
+ * mask is awaited before the forward pass, the target before the photometric term); NULL = upload on `stream`. */
+int ocgs_step_view_host(const ocgs_surfels* surfels, const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask,
+                        const float* h_target, float* h_losses, uint8_t* d_mask, float* d_images, uint32_t* d_ncontrib,
+                        float* d_grad_pos, float* d_grad_scale, float* d_grad_quat, float* d_grad_opacity, float* d_grad_sh,
+                        uint32_t* d_vis_count, float* d_contrib_sum, float* d_losses, void* ws, size_t key_capacity, void* stream,
+                        void* copy_stream);
+
+/* ---- end-to-end step with HOST parameters (bench.py "e2e_host_params") ---------------------------------------------------------------
  * Copies the surfel parameters, mask and target image from (pinned) host memory to the given device staging buffers,
  * runs (1)-(3) with L_b and statistics on, ocgs_masked_l1, then (4); copies the gradients, the alpha map and loss_bg back
  * and synchronises.  Every pointer named h_* is host memory, d_* device memory owned by the caller.

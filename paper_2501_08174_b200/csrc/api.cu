@@ -296,6 +296,56 @@ int ocgs_compact_rows(const float* in, const int32_t* remap, int n, int row_floa
   return launch_compact_rows(in, remap, n, row_floats, out, (cudaStream_t)stream);
 }
 
+int ocgs_step_view_host(const ocgs_surfels* surfels, const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask,
+                        const float* h_target, float* h_losses, uint8_t* d_mask, float* d_images, uint32_t* d_ncontrib,
+                        float* d_grad_pos, float* d_grad_scale, float* d_grad_quat, float* d_grad_opacity, float* d_grad_sh,
+                        uint32_t* d_vis_count, float* d_contrib_sum, float* d_losses, void* ws, size_t key_capacity, void* stream,
+                        void* copy_stream) {
+  if (!surfels || !cam || !cfg || !h_mask || !h_target || !h_losses || !d_mask || !d_images || !d_ncontrib || !d_losses || !ws)
+    return OCGS_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaStream_t cs = copy_stream ? (cudaStream_t)copy_stream : st;
+  const size_t HW = (size_t)cam->width * cam->height;
+  float* color = d_images; float* alpha = color + 3 * HW; float* depth = alpha + HW; float* normal = depth + HW;
+  float* target = normal + 3 * HW;
+  float* gC = target + 3 * HW;
+  // the view's inputs travel on the copy stream while preprocess / sort / forward run: the mask is needed by the forward
+  // pass, the target only by the photometric term
+  cudaEvent_t ev_begin = nullptr, ev_mask = nullptr, ev_target = nullptr;
+  const bool overlap = cs != st;
+  if (overlap) {
+    OCGS_CUDA_OK(cudaEventCreateWithFlags(&ev_begin, cudaEventDisableTiming));
+    OCGS_CUDA_OK(cudaEventCreateWithFlags(&ev_mask, cudaEventDisableTiming));
+    OCGS_CUDA_OK(cudaEventCreateWithFlags(&ev_target, cudaEventDisableTiming));
+    OCGS_CUDA_OK(cudaEventRecord(ev_begin, st));  // the previous step's readers of d_mask / target are done
+    OCGS_CUDA_OK(cudaStreamWaitEvent(cs, ev_begin, 0));
+  }
+  OCGS_CUDA_OK(cudaMemcpyAsync(d_mask, h_mask, HW, cudaMemcpyHostToDevice, cs));
+  if (overlap) OCGS_CUDA_OK(cudaEventRecord(ev_mask, cs));
+  OCGS_CUDA_OK(cudaMemcpyAsync(target, h_target, 3 * HW * sizeof(float), cudaMemcpyHostToDevice, cs));
+  if (overlap) OCGS_CUDA_OK(cudaEventRecord(ev_target, cs));
+  const int n = surfels->n;
+  int rc = OCGS_OK;
+  do {
+    if ((rc = ocgs_preprocess(surfels, cam, cfg, ws, key_capacity, stream)) != OCGS_OK) break;
+    if ((rc = ocgs_bin_sort(n, cam, cfg, ws, key_capacity, nullptr, stream)) != OCGS_OK) break;
+    if (overlap && cudaStreamWaitEvent(st, ev_mask, 0) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
+    if ((rc = ocgs_render_fwd(n, cam, cfg, ws, key_capacity, d_mask, color, alpha, depth, normal, d_ncontrib, d_losses, d_vis_count,
+                              d_contrib_sum, stream)) != OCGS_OK) break;
+    if (overlap && cudaStreamWaitEvent(st, ev_target, 0) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
+    if ((rc = ocgs_masked_l1(color, target, d_mask, cam->width, cam->height, gC, d_losses + 1, ws, n, key_capacity, stream)) != OCGS_OK) break;
+    if ((rc = ocgs_render_bwd(surfels, cam, cfg, ws, key_capacity, d_mask, d_ncontrib, gC, nullptr, nullptr, nullptr, d_grad_pos, d_grad_scale,
+                              d_grad_quat, d_grad_opacity, d_grad_sh, nullptr, stream)) != OCGS_OK) break;
+    if (cudaMemcpyAsync(h_losses, d_losses, 2 * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
+    rc = ocgs_check(ws, stream, nullptr);
+  } while (false);
+  if (overlap) {
+    if (rc != OCGS_OK) cudaStreamSynchronize(cs);
+    cudaEventDestroy(ev_begin); cudaEventDestroy(ev_mask); cudaEventDestroy(ev_target);
+  }
+  return rc;
+}
+
 int ocgs_step_host(const float* h_pos, const float* h_scale, const float* h_quat, const float* h_opacity, const float* h_sh, int n,
                    const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask, const float* h_target, float* h_grads,
                    float* h_alpha, float* h_loss_bg, float* d_params, uint8_t* d_mask, float* d_images, uint32_t* d_ncontrib,

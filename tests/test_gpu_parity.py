@@ -234,3 +234,17 @@ def test_masked_l1_and_host_step_match_device_path():
         a, b = hg[lo:hi], gg[name].ravel()
         assert np.allclose(a, b, rtol=2e-3, atol=1e-6 + 1e-4 * np.abs(b).max()), name
     assert np.array_equal(vis.cpu().numpy().view(np.uint32), gf["vis_count"])
+    # the training step with resident parameters (ocgs_step_view_host): only the view's target and mask come from the host,
+    # uploaded on a second stream; losses come back, gradients stay on the device
+    grads = B.alloc_grads(n)
+    h_losses = torch.zeros(2).pin_memory(); d_losses = torch.zeros(2, device="cuda")
+    vis2 = torch.zeros(n, dtype=torch.int32, device="cuda"); cs2 = torch.zeros(n, device="cuda")
+    for copy_stream in (None, torch.cuda.Stream()):
+        vis2.zero_(); cs2.zero_()
+        B.ocgs_step_view_host(g.surfels, g.cam, g.cfg, torch.tensor(m).pin_memory(), torch.tensor(target).pin_memory(), h_losses, d_mask,
+                              d_images, d_nc, grads, vis2, cs2, d_losses, g.ws, g.cap, copy_stream=copy_stream)
+        assert float(h_losses[0]) == gf["loss_bg"] and abs(float(h_losses[1]) - float(loss.item())) < 1e-7
+        for name in ("d_pos", "d_scale", "d_quat", "d_opacity", "d_sh"):
+            a, b = grads[name].cpu().numpy().ravel(), gg[name].ravel()
+            assert np.allclose(a, b, rtol=2e-3, atol=1e-6 + 1e-4 * np.abs(b).max()), name
+        assert np.array_equal(vis2.cpu().numpy().view(np.uint32), gf["vis_count"])
