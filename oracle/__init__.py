@@ -246,3 +246,64 @@ def sh_basis(direction) -> np.ndarray:
     Y = np.zeros(16)
     lib().orc_sh_basis(_p(d), _p(Y))
     return Y
+
+
+# --------------------------------------------------------------------------------------------------
+# 3D-Gaussian variant of the visibility statistics (Appendix B; reading R-3D)
+# --------------------------------------------------------------------------------------------------
+
+def preprocess3d(pos, scale3, quat, opacity, sh, cam: OrcCamera, cfg: OrcConfig) -> Dict[str, np.ndarray]:
+    pos, scale3, quat, opacity, sh = _f32(pos), _f32(scale3), _f32(quat), _f32(opacity), _f32(sh)
+    n = pos.shape[0]
+    assert scale3.shape == (n, 3)
+    out = dict(visible=np.zeros(n, np.uint8), depth_bits=np.zeros(n, np.uint32), rect=np.zeros((n, 4), np.int32),
+               tiles_touched=np.zeros(n, np.uint32), conic=np.zeros((n, 3), np.float32), c2d=np.zeros((n, 2), np.float32),
+               rho_cut=np.zeros(n, np.float32), rgb=np.zeros((n, 3), np.float64), clamp=np.zeros(n, np.uint8))
+    lib().orc3d_preprocess(C.c_int(n), _p(pos), _p(scale3), _p(quat), _p(opacity), _p(sh), C.byref(cam), C.byref(cfg),
+                           _p(out["visible"]), _p(out["depth_bits"]), _p(out["rect"]), _p(out["tiles_touched"]), _p(out["conic"]),
+                           _p(out["c2d"]), _p(out["rho_cut"]), _p(out["rgb"]), _p(out["clamp"]))
+    return out
+
+
+def render3d_fwd(pre, srt, opacity, cam: OrcCamera, cfg: OrcConfig, mask=None, window=None, vis_count=None, contrib_sum=None,
+                 want_fragile=True) -> Dict[str, np.ndarray]:
+    """bin_sort(pre, ...) serves both primitives: it only reads visible / depth_bits / rect."""
+    W, H = cam.width, cam.height
+    n = pre["visible"].shape[0]
+    opacity = _f32(opacity)
+    x0, y0, x1, y1 = window if window is not None else (0, 0, W, H)
+    out = dict(color=np.zeros((3, H, W)), alpha=np.zeros((H, W)), depth=np.zeros((H, W)), n_contrib=np.zeros((H, W), np.uint32))
+    if vis_count is None:
+        vis_count = np.zeros(n, np.uint32)
+    if contrib_sum is None:
+        contrib_sum = np.zeros(n, np.float64)
+    fragile = np.zeros((H, W), np.uint8) if want_fragile else None
+    ftouch = np.zeros(n, np.uint32) if want_fragile else None
+    margins = default_margins() if want_fragile else None
+    ids = srt["ids"] if srt["K"] > 0 else np.zeros(1, np.uint32)
+    m = None if mask is None else np.ascontiguousarray(mask, np.uint8)
+    lib().orc3d_render_fwd.restype = C.c_double
+    Lb = lib().orc3d_render_fwd(C.c_int(n), C.byref(cam), C.byref(cfg), C.byref(margins) if margins is not None else None,
+                                _p(pre["conic"]), _p(pre["c2d"]), _p(pre["rho_cut"]), _p(opacity), _p(pre["depth_bits"]), _p(pre["rgb"]),
+                                _p(ids), _p(srt["ranges"]), _p(m), C.c_int(x0), C.c_int(y0), C.c_int(x1), C.c_int(y1),
+                                _p(out["color"]), _p(out["alpha"]), _p(out["depth"]), _p(out["n_contrib"]), _p(vis_count),
+                                _p(contrib_sum), _p(fragile), _p(ftouch))
+    out.update(loss_bg=float(Lb), vis_count=vis_count, contrib_sum=contrib_sum, fragile=fragile, fragile_touch=ftouch)
+    return out
+
+
+def bf3d_render(pos, scale3, quat, opacity, sh, cam: OrcCamera, cfg: OrcConfig, mask=None, window=None, want_stats=True):
+    pos, scale3, quat, opacity, sh = _f64(pos), _f64(scale3), _f64(quat), _f64(opacity), _f64(sh)
+    n = pos.shape[0]
+    W, H = cam.width, cam.height
+    x0, y0, x1, y1 = window if window is not None else (0, 0, W, H)
+    out = dict(color=np.zeros((3, H, W)), alpha=np.zeros((H, W)), depth=np.zeros((H, W)), n_blended=np.zeros((H, W), np.uint32))
+    vis = np.zeros(n, np.uint32) if want_stats else None
+    cs = np.zeros(n, np.float64) if want_stats else None
+    m = None if mask is None else np.ascontiguousarray(mask, np.uint8)
+    lib().orc3d_bf_render.restype = C.c_double
+    Lb = lib().orc3d_bf_render(C.c_int(n), _p(pos), _p(scale3), _p(quat), _p(opacity), _p(sh), C.byref(cam), C.byref(cfg), _p(m),
+                               C.c_int(x0), C.c_int(y0), C.c_int(x1), C.c_int(y1), _p(out["color"]), _p(out["alpha"]),
+                               _p(out["depth"]), _p(out["n_blended"]), _p(vis), _p(cs))
+    out.update(loss_bg=float(Lb), vis_count=vis, contrib_sum=cs)
+    return out

@@ -867,6 +867,297 @@ double orc_bf_render(int n, const double* pos, const double* scale, const double
   return Lb / (double)HW;
 }
 
+// ================================================================================================
+// 3D-Gaussian variant of the visibility statistics (Appendix B: "We demonstrate the versatility of
+// our pruning strategy by implementing it in 3DGS").  Only the primitive changes: O1 (projection)
+// and O4 (per-pair evaluation); keys, order, compositing, termination, statistics and the prune rule are the ones above.
+// The paper gives no formulas for 3DGS (PAPER.md:63 defers to Kerbl et al. 2023); readings (R-3D):
+//   Gaussian j: mean p, covariance Sigma = R(q) diag(s^2) R(q)^T, opacity o, SH colour as for surfels.
+//   EWA projection: t = W p + t_wc, J = d(fx tx/tz, fy ty/tz)/dt, Sigma' = J W Sigma W^T J^T + 0.3 I (the published
+//   screen-space dilation), centre c = (fx tx/tz + cx - 1/2, fy ty/tz + cy - 1/2); rho(x) = (x - c)^T Sigma'^-1 (x - c);
+//   the pair contributes iff rho <= rho_cut = min(9, 2 ln(o/alpha_min)) (S6, same pixel-exact cut as for surfels, which
+//   keeps the image independent of the tiling), alpha = min(alpha_max, o exp(-rho/2)); depth of a pair = centre depth t_z.
+//   Box: exact AABB of the rho_cut ellipse, half extents sqrt(rho_cut Sigma'_xx), sqrt(rho_cut Sigma'_yy), padded like R-bbox.
+// Integer-deciding sequence (fp32, each operation rounded once, fma written explicitly; the GPU kernel repeats it):
+//   R columns as in Appendix A step 1 (plus t_w = (2(xz+wy), 2(yz-wx), 1-2(xx+yy))); t = view_point(p); cull !(t_z > near),
+//   o < alpha_min; m_k = view_dir(R column k), b_k = s_k m_k (k = 0..2); S_ij = fma(b_0i, b_0j, fma(b_1i, b_1j, b_2i b_2j));
+//   itz = 1/t_z; j00 = fx itz; j02 = -((j00 t_x) itz); j11 = fy itz; j12 = -((j11 t_y) itz);
+//   T0 = (fma(j00,S00, j02 S02), fma(j00,S01, j02 S12), fma(j00,S02, j02 S22)), T1 likewise with (j11, j12) and rows 1, 2;
+//   cxx = fma(T0x,j00, T0z j02) + 0.3; cxy = fma(T0y,j11, T0z j12); cyy = fma(T1y,j11, T1z j12) + 0.3;
+//   det = fma(cxx,cyy, -(cxy cxy)); cull !(det > 0); conic = (cyy/det, -cxy/det, cxx/det);
+//   c = (fma(j00,t_x, cx-1/2), fma(j11,t_y, cy-1/2)); rho_cut as Appendix A step 5;
+//   h_x = fma(sqrt(rho_cut cxx), 1+2^-16, 2^-7), h_y likewise; bounds ceil(c - h) .. floor(c + h), clamps as step 8.
+// ================================================================================================
+namespace {
+
+struct Pre3 {
+  bool visible;
+  float conic[3], cov[3], c2d[2], rho_cut, depth;
+  int rect[4];
+};
+
+Pre3 preprocess3d_one(const float* p, const float* s, const float* q, float o, const OrcCamera& cam, const OrcConfig& cfg) {
+  Pre3 r;
+  std::memset(&r, 0, sizeof(r));
+  const float* V = cam.view;
+  const float w = q[0], x = q[1], y = q[2], z = q[3];
+  const float xx = x * x, yy = y * y, zz = z * z, xy = x * y, xz = x * z, yz = y * z, wx = w * x, wy = w * y, wz = w * z;
+  const float col[3][3] = {{1.0f - 2.0f * (yy + zz), 2.0f * (xy + wz), 2.0f * (xz - wy)},
+                           {2.0f * (xy - wz), 1.0f - 2.0f * (xx + zz), 2.0f * (yz + wx)},
+                           {2.0f * (xz + wy), 2.0f * (yz - wx), 1.0f - 2.0f * (xx + yy)}};
+  float t[3];
+  view_point(V, p, t);
+  r.depth = t[2];
+  if (!(t[2] > cfg.near_z)) return r;
+  if (o < cfg.alpha_min) return r;
+  float b[3][3];  // b[k] = s_k * W R e_k
+  for (int k = 0; k < 3; ++k) {
+    float m[3];
+    view_dir(V, col[k], m);
+    for (int i = 0; i < 3; ++i) b[k][i] = s[k] * m[i];
+  }
+  auto S = [&](int i, int j) { return std::fmaf(b[0][i], b[0][j], std::fmaf(b[1][i], b[1][j], b[2][i] * b[2][j])); };
+  const float S00 = S(0, 0), S01 = S(0, 1), S02 = S(0, 2), S11 = S(1, 1), S12 = S(1, 2), S22 = S(2, 2);
+  const float itz = 1.0f / t[2];
+  const float j00 = cam.fx * itz, j02 = -((j00 * t[0]) * itz), j11 = cam.fy * itz, j12 = -((j11 * t[1]) * itz);
+  const float T0x = std::fmaf(j00, S00, j02 * S02), T0y = std::fmaf(j00, S01, j02 * S12), T0z = std::fmaf(j00, S02, j02 * S22);
+  const float T1y = std::fmaf(j11, S11, j12 * S12), T1z = std::fmaf(j11, S12, j12 * S22);
+  const float cxx = std::fmaf(T0x, j00, T0z * j02) + 0.3f;
+  const float cxy = std::fmaf(T0y, j11, T0z * j12);
+  const float cyy = std::fmaf(T1y, j11, T1z * j12) + 0.3f;
+  const float det = std::fmaf(cxx, cyy, -(cxy * cxy));
+  if (!(det > 0.0f)) return r;
+  r.cov[0] = cxx; r.cov[1] = cxy; r.cov[2] = cyy;
+  r.conic[0] = cyy / det; r.conic[1] = -cxy / det; r.conic[2] = cxx / det;
+  r.c2d[0] = std::fmaf(j00, t[0], cam.cx - 0.5f);
+  r.c2d[1] = std::fmaf(j11, t[1], cam.cy - 0.5f);
+  const double rr = 2.0 * std::log((double)o / (double)cfg.alpha_min);
+  const float rc = (float)std::fmin((double)cfg.rho_max, rr);
+  r.rho_cut = rc;
+  const float h[2] = {std::fmaf(std::sqrt(rc * cxx), 1.0000152587890625f, 0.0078125f),
+                      std::fmaf(std::sqrt(rc * cyy), 1.0000152587890625f, 0.0078125f)};
+  const float lim = 1073741824.0f;
+  const int WH[2] = {cam.width, cam.height};
+  int lo[2], hi[2];
+  for (int k = 0; k < 2; ++k) {
+    float mn = std::fmax(-lim, std::fmin(lim, r.c2d[k] - h[k]));
+    float mx = std::fmax(-lim, std::fmin(lim, r.c2d[k] + h[k]));
+    lo[k] = (int)std::ceil(mn);
+    hi[k] = (int)std::floor(mx);
+    if (hi[k] < 0 || lo[k] > WH[k] - 1 || lo[k] > hi[k]) return r;
+    lo[k] = std::max(lo[k], 0);
+    hi[k] = std::min(hi[k], WH[k] - 1);
+  }
+  r.rect[0] = lo[0]; r.rect[1] = lo[1]; r.rect[2] = hi[0]; r.rect[3] = hi[1];
+  r.visible = true;
+  return r;
+}
+
+}  // namespace
+
+extern "C" {
+
+void orc3d_preprocess(int n, const float* pos, const float* scale, const float* quat, const float* opacity, const float* sh,
+                      const OrcCamera* cam, const OrcConfig* cfg, uint8_t* visible, uint32_t* depth_bits, int32_t* rect,
+                      uint32_t* tiles_touched, float* conic, float* c2d, float* rho_cut, double* rgb, uint8_t* clamp) {
+  double campos[3];
+  cam_position(cam->view, campos);
+#pragma omp parallel for schedule(static)
+  for (int j = 0; j < n; ++j) {
+    const Pre3 r = preprocess3d_one(pos + 3 * j, scale + 3 * j, quat + 4 * j, opacity[j], *cam, *cfg);
+    visible[j] = r.visible ? 1 : 0;
+    depth_bits[j] = float_bits(r.depth);
+    for (int k = 0; k < 3; ++k) { conic[3 * j + k] = r.conic[k]; rgb[3 * j + k] = 0; }
+    c2d[2 * j] = r.c2d[0]; c2d[2 * j + 1] = r.c2d[1];
+    rho_cut[j] = r.rho_cut;
+    for (int k = 0; k < 4; ++k) rect[4 * j + k] = r.visible ? r.rect[k] : 0;
+    tiles_touched[j] = 0;
+    clamp[j] = 0;
+    if (!r.visible) continue;
+    const int T = cfg->tile;
+    tiles_touched[j] = (uint32_t)((r.rect[2] / T + 1 - r.rect[0] / T) * (r.rect[3] / T + 1 - r.rect[1] / T));
+    surfel_colour(pos + 3 * j, sh + 48 * j, cfg->sh_degree, campos, rgb + 3 * j, clamp + j);
+  }
+}
+
+}  // extern "C" (3D preprocess)
+
+extern "C" {
+
+// TILED forward for 3D Gaussians: same walk as orc_render_fwd (O5, O6, O8), per-pair evaluation of R-3D in fp64 from the
+// fp32 record (conic, c2d, rho_cut).  depth accumulates the CENTRE depth of each blended Gaussian.  A pixel is fragile when
+// a decision is within the margins (rho vs rho_cut, the stop test).
+double orc3d_render_fwd(int n, const OrcCamera* cam, const OrcConfig* cfg, const OrcMargins* mg, const float* conic, const float* c2d,
+                        const float* rho_cut, const float* opacity, const uint32_t* depth_bits, const double* rgb, const uint32_t* ids,
+                        const uint32_t* ranges, const uint8_t* mask, int wx0, int wy0, int wx1, int wy1, double* color, double* alpha,
+                        double* depth, uint32_t* n_contrib, uint32_t* vis_count, double* contrib_sum, uint8_t* fragile,
+                        uint32_t* fragile_touch) {
+  (void)n;
+  const int W = cam->width, H = cam->height, T = cfg->tile;
+  const int tiles_x = (W + T - 1) / T, tiles_y = (H + T - 1) / T;
+  const size_t HW = (size_t)W * H;
+  double Lb = 0.0;
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : Lb)
+  for (int t = 0; t < tiles_x * tiles_y; ++t) {
+    const int tx = t % tiles_x, ty = t / tiles_x;
+    const uint32_t start = ranges[2 * t], end = ranges[2 * t + 1];
+    for (int y = std::max(ty * T, wy0); y < std::min({(ty + 1) * T, H, wy1}); ++y)
+      for (int x = std::max(tx * T, wx0); x < std::min({(tx + 1) * T, W, wx1}); ++x) {
+        double Tr = 1.0, C[3] = {0, 0, 0}, D = 0;
+        uint32_t last = 0;
+        bool frag = false;
+        for (uint32_t pos = start; pos < end; ++pos) {
+          const uint32_t j = ids[pos];
+          const double dx = (double)x - (double)c2d[2 * j], dy = (double)y - (double)c2d[2 * j + 1];
+          const double rho = (double)conic[3 * j] * dx * dx + 2.0 * (double)conic[3 * j + 1] * dx * dy + (double)conic[3 * j + 2] * dy * dy;
+          const double rc = rho_cut[j];
+          if (mg && std::fabs(rho - rc) <= mg->rho_cut_abs) frag = true;
+          if (rho > rc) continue;
+          const double a = std::fmin((double)cfg->alpha_max, (double)opacity[j] * std::exp(-0.5 * rho));
+          const double Tn = Tr * (1.0 - a);
+          if (mg && std::fabs(Tn - (double)cfg->t_min) <= mg->tmin_rel * (double)cfg->t_min) frag = true;
+          if (Tn < (double)cfg->t_min) break;
+          const double w = a * Tr;
+          float zf; std::memcpy(&zf, &depth_bits[j], 4);
+          for (int c = 0; c < 3; ++c) C[c] += w * rgb[3 * j + c];
+          D += w * (double)zf;
+          if (vis_count) {
+#pragma omp atomic
+            vis_count[j] += 1;
+          }
+          if (contrib_sum) {
+#pragma omp atomic
+            contrib_sum[j] += w;
+          }
+          Tr = Tn;
+          last = pos - start + 1;
+        }
+        const size_t p = (size_t)y * W + x;
+        for (int c = 0; c < 3; ++c) color[c * HW + p] = C[c] + Tr * (double)cfg->bg[c];
+        alpha[p] = 1.0 - Tr;
+        depth[p] = D;
+        n_contrib[p] = last;
+        if (fragile) fragile[p] = frag ? 1 : 0;
+        if (frag && fragile_touch)
+          for (uint32_t pos = start; pos < end; ++pos) {
+#pragma omp atomic
+            fragile_touch[ids[pos]] += 1;
+          }
+        const double m = mask ? (mask[p] ? 1.0 : 0.0) : 0.0;
+        Lb += (1.0 - Tr) * (1.0 - m);
+      }
+  }
+  return Lb / (double)HW;
+}
+
+// Brute force for 3D Gaussians: fp64 from the raw parameters, every (pixel, Gaussian) pair, no boxes, no tiles, exhaustive
+// per-pixel sort by (fp32 centre-depth bits, id).  Knows nothing of the fp32 sequence above except the ordering key.
+double orc3d_bf_render(int n, const double* pos, const double* scale, const double* quat, const double* opacity, const double* sh,
+                       const OrcCamera* cam, const OrcConfig* cfg, const uint8_t* mask, int wx0, int wy0, int wx1, int wy1,
+                       double* color, double* alpha, double* depth, uint32_t* n_blended, uint32_t* vis_count, double* contrib_sum) {
+  const int W = cam->width, H = cam->height;
+  const size_t HW = (size_t)W * H;
+  const float* V = cam->view;
+  double campos[3];
+  cam_position(V, campos);
+  struct G { bool ok; double c[2], q[3], rho_cut, o, z, rgb[3]; uint32_t key; };
+  std::vector<G> gs((size_t)n);
+  const double fx = cam->fx, fy = cam->fy, ox = (double)(cam->cx - 0.5f), oy = (double)(cam->cy - 0.5f);
+  for (int j = 0; j < n; ++j) {
+    G& g = gs[(size_t)j];
+    const double* p = pos + 3 * j;
+    double t[3];
+    for (int k = 0; k < 3; ++k) t[k] = (double)V[4 * k] * p[0] + (double)V[4 * k + 1] * p[1] + (double)V[4 * k + 2] * p[2] + (double)V[4 * k + 3];
+    const float pf[3] = {(float)p[0], (float)p[1], (float)p[2]};
+    float tf[3];
+    view_point(V, pf, tf);
+    g.key = float_bits(tf[2]);
+    g.z = (double)tf[2];  // the depth map accumulates the fp32 centre depth (the key), as the tiled path does
+    g.o = opacity[j];
+    g.ok = t[2] > (double)cfg->near_z && g.o >= (double)cfg->alpha_min;
+    if (!g.ok) continue;
+    const Rot r = rot_from_quat(quat + 4 * j);
+    const double* cols[3] = {r.tu, r.tv, r.tw};
+    double B[3][3];  // B[k] = s_k W R e_k
+    for (int k = 0; k < 3; ++k) {
+      double m[3];
+      mat3_vec(V, cols[k], m);
+      for (int i = 0; i < 3; ++i) B[k][i] = scale[3 * j + k] * m[i];
+    }
+    double S[3][3];
+    for (int a = 0; a < 3; ++a)
+      for (int b2 = 0; b2 < 3; ++b2) S[a][b2] = B[0][a] * B[0][b2] + B[1][a] * B[1][b2] + B[2][a] * B[2][b2];
+    const double J[2][3] = {{fx / t[2], 0.0, -fx * t[0] / (t[2] * t[2])}, {0.0, fy / t[2], -fy * t[1] / (t[2] * t[2])}};
+    double cov[2][2];
+    for (int a = 0; a < 2; ++a)
+      for (int b2 = 0; b2 < 2; ++b2) {
+        double acc = 0;
+        for (int k = 0; k < 3; ++k)
+          for (int l = 0; l < 3; ++l) acc += J[a][k] * S[k][l] * J[b2][l];
+        cov[a][b2] = acc;
+      }
+    cov[0][0] += 0.3; cov[1][1] += 0.3;
+    const double det = cov[0][0] * cov[1][1] - cov[0][1] * cov[1][0];
+    if (!(det > 0)) { g.ok = false; continue; }
+    g.q[0] = cov[1][1] / det; g.q[1] = -cov[0][1] / det; g.q[2] = cov[0][0] / det;
+    g.c[0] = fx * t[0] / t[2] + ox; g.c[1] = fy * t[1] / t[2] + oy;
+    g.rho_cut = std::fmin((double)cfg->rho_max, 2.0 * std::log(g.o / (double)cfg->alpha_min));
+    const float pff[3] = {(float)p[0], (float)p[1], (float)p[2]};
+    std::vector<float> shf(48);
+    for (int k = 0; k < 48; ++k) shf[(size_t)k] = (float)sh[48 * (size_t)j + k];
+    uint8_t cl;
+    surfel_colour(pff, shf.data(), cfg->sh_degree, campos, g.rgb, &cl);
+  }
+  double Lb = 0.0;
+#pragma omp parallel for schedule(dynamic, 4) reduction(+ : Lb)
+  for (int y = wy0; y < wy1; ++y) {
+    struct Cand { uint32_t key; int j; double alpha; };
+    std::vector<Cand> cands;
+    for (int x = wx0; x < wx1; ++x) {
+      cands.clear();
+      for (int j = 0; j < n; ++j) {
+        const G& g = gs[(size_t)j];
+        if (!g.ok) continue;
+        const double dx = x - g.c[0], dy = y - g.c[1];
+        const double rho = g.q[0] * dx * dx + 2 * g.q[1] * dx * dy + g.q[2] * dy * dy;
+        if (rho > g.rho_cut) continue;
+        cands.push_back({g.key, j, std::fmin((double)cfg->alpha_max, g.o * std::exp(-0.5 * rho))});
+      }
+      std::sort(cands.begin(), cands.end(), [](const Cand& a, const Cand& b) { return a.key != b.key ? a.key < b.key : a.j < b.j; });
+      double Tr = 1.0, C[3] = {0, 0, 0}, D = 0;
+      uint32_t cnt = 0;
+      for (const Cand& c : cands) {
+        const double Tn = Tr * (1.0 - c.alpha);
+        if (Tn < (double)cfg->t_min) break;
+        const double w = c.alpha * Tr;
+        const G& g = gs[(size_t)c.j];
+        for (int k = 0; k < 3; ++k) C[k] += w * g.rgb[k];
+        D += w * g.z;
+        if (vis_count) {
+#pragma omp atomic
+          vis_count[c.j] += 1;
+        }
+        if (contrib_sum) {
+#pragma omp atomic
+          contrib_sum[c.j] += w;
+        }
+        Tr = Tn;
+        ++cnt;
+      }
+      const size_t p = (size_t)y * W + x;
+      for (int k = 0; k < 3; ++k) color[k * HW + p] = C[k] + Tr * (double)cfg->bg[k];
+      alpha[p] = 1.0 - Tr;
+      depth[p] = D;
+      if (n_blended) n_blended[p] = cnt;
+      const double m = mask ? (mask[p] ? 1.0 : 0.0) : 0.0;
+      Lb += (1.0 - Tr) * (1.0 - m);
+    }
+  }
+  return Lb / (double)HW;
+}
+
+}  // extern "C" (3D render)
+
 // SH basis exposed for the orthonormality pin (tests integrate Y_i Y_j over the sphere by quadrature).
 void orc_sh_basis(const double* dir, double* Y16) { sh_basis(dir, Y16, nullptr); }
 
