@@ -189,6 +189,28 @@ int ocgs_regularizers(const float* alpha, const float* depth, const float* momen
                       float w_d, float w_n, float* dL_dalpha, float* dL_ddepth, float* dL_dmoments, float* dL_dnormal, float* loss,
                       void* scratch, void* stream);
 
+/* ---- 3D-Gaussian variant of the visibility statistics (Appendix B; R-3D) ----
+ * "We demonstrate the versatility of our pruning strategy by implementing it in 3DGS": the same forward walk, statistics
+ * and prune rule on 3D Gaussians (mean, three scales, rotation, opacity, SH colour; EWA projection
+ * Sigma' = J W Sigma W^T J^T + 0.3 I; a pair contributes iff (x-c)^T Sigma'^-1 (x-c) <= rho_cut).  Forward only.
+ * ocgs3d_preprocess fills the same workspace sections as ocgs_preprocess; ocgs_bin_sort is then called unchanged;
+ * ocgs3d_render_fwd = ocgs_render_fwd without the normal map (depth accumulates the Gaussians' centre depths).
+ * Pruning: ocgs_prune_stats with a NULL `out` (only in->n and in->opacity are read) gives mask / remap / count, and
+ * ocgs_compact_rows moves each parameter array (row lengths 3, 3, 4, 1, 48). */
+typedef struct {
+  const float* pos;      /* [N,3] */
+  const float* scale;    /* [N,3] activated (> 0) standard deviations along the Gaussian's axes */
+  const float* quat;     /* [N,4] (w,x,y,z) */
+  const float* opacity;  /* [N] */
+  const float* sh;       /* [N,16,3] */
+  int n;
+} ocgs_gaussians3d;
+int ocgs3d_preprocess(const ocgs_gaussians3d* gaussians, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
+                      void* stream);
+int ocgs3d_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
+                      float* color, float* alpha, float* depth, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,
+                      float* contrib_sum, void* stream);
+
 /* ---- (5) prune statistics -> mask -> stream compaction ----------------------------------------------------------------
  * "We propose to assign both G_j and G_k with false" -- a surfel that was never blended in any render
  * of the interval is removed whether it was outside the frustum or occluded; PAPER.md:101 (opacity threshold), S17.

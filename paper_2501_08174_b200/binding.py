@@ -17,7 +17,7 @@ _LIB_PATH = os.path.join(_HERE, "csrc", "libocgs.so")
 
 OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
-           "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_render_fwd_reg", "ocgs_render_bwd_reg", "ocgs_prune_workspace_bytes",
+           "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_render_fwd_reg", "ocgs_render_bwd_reg", "ocgs3d_preprocess", "ocgs3d_render_fwd", "ocgs_prune_workspace_bytes",
            "ocgs_prune_stats", "ocgs_compact_rows", "ocgs_step_host", "ocgs_step_view_host", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
            "ocgs_profile_begin", "ocgs_profile_end"]
 
@@ -42,6 +42,11 @@ class ocgs_config(C.Structure):
 
 
 class ocgs_surfels(C.Structure):
+    _fields_ = [("pos", C.c_void_p), ("scale", C.c_void_p), ("quat", C.c_void_p), ("opacity", C.c_void_p), ("sh", C.c_void_p),
+                ("n", C.c_int)]
+
+
+class ocgs_gaussians3d(C.Structure):
     _fields_ = [("pos", C.c_void_p), ("scale", C.c_void_p), ("quat", C.c_void_p), ("opacity", C.c_void_p), ("sh", C.c_void_p),
                 ("n", C.c_int)]
 
@@ -166,6 +171,26 @@ def ocgs_render_fwd(n, cam, cfg, ws, key_capacity, mask, color, alpha, depth, no
     _ok("ocgs_render_fwd", lib().ocgs_render_fwd(C.c_int(n), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity), _ptr(mask),
                                                  _ptr(color), _ptr(alpha), _ptr(depth), _ptr(normal), _ptr(n_contrib), _ptr(loss_bg),
                                                  _ptr(vis_count), _ptr(contrib_sum), _stream(stream)))
+
+
+def make_gaussians3d(pos, scale3, quat, opacity, sh) -> ocgs_gaussians3d:
+    n = int(pos.shape[0])
+    for t, shape in ((pos, (n, 3)), (scale3, (n, 3)), (quat, (n, 4)), (opacity, (n,)), (sh, (n, 16, 3))):
+        if tuple(t.shape) != shape or t.dtype != torch.float32:
+            raise ValueError(f"expected float32 tensor of shape {shape}, got {tuple(t.shape)} {t.dtype}")
+    return ocgs_gaussians3d(_ptr(pos), _ptr(scale3), _ptr(quat), _ptr(opacity), _ptr(sh), n)
+
+
+def ocgs3d_preprocess(gaussians: ocgs_gaussians3d, cam, cfg, ws, key_capacity, stream=None):
+    _ok("ocgs3d_preprocess", lib().ocgs3d_preprocess(C.byref(gaussians), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity),
+                                                     _stream(stream)))
+
+
+def ocgs3d_render_fwd(n, cam, cfg, ws, key_capacity, mask, color, alpha, depth, n_contrib, loss_bg=None, vis_count=None, contrib_sum=None,
+                      stream=None):
+    _ok("ocgs3d_render_fwd", lib().ocgs3d_render_fwd(C.c_int(n), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity), _ptr(mask),
+                                                     _ptr(color), _ptr(alpha), _ptr(depth), _ptr(n_contrib), _ptr(loss_bg),
+                                                     _ptr(vis_count), _ptr(contrib_sum), _stream(stream)))
 
 
 def ocgs_render_fwd_reg(n, cam, cfg, ws, key_capacity, mask, color, alpha, depth, normal, n_contrib, loss_bg, vis_count, contrib_sum,

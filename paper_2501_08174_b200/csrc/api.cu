@@ -186,7 +186,30 @@ int ocgs_render_fwd_reg(int n, const ocgs_camera* cam, const ocgs_config* cfg, v
   Workspace w;
   if ((rc = carve_for_render(ws, n, cam, key_capacity, &w)) != OCGS_OK) return rc;
   return launch_render_fwd(make_cam(*cam), *cfg, w, mask, color, alpha, depth, normal, n_contrib, loss_bg, vis_count, contrib_sum,
-                           moments, (cudaStream_t)stream);
+                           moments, /*prim=*/0, (cudaStream_t)stream);
+}
+
+int ocgs3d_preprocess(const ocgs_gaussians3d* g, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, void* stream) {
+  if (!g || !cam || !ws) return OCGS_ERR_INVALID_ARG;
+  int rc = check_cfg(cfg);
+  if (rc != OCGS_OK) return rc;
+  if (g->n > 0 && (!g->pos || !g->scale || !g->quat || !g->opacity || !g->sh)) return OCGS_ERR_INVALID_ARG;
+  Workspace w;
+  if (!carve_workspace(ws, g->n, cam->width, cam->height, key_capacity, &w, nullptr)) return OCGS_ERR_UNSUPPORTED;
+  return launch_preprocess3d(*g, make_cam(*cam), *cfg, w, (cudaStream_t)stream);
+}
+
+int ocgs3d_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
+                      float* color, float* alpha, float* depth, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,
+                      float* contrib_sum, void* stream) {
+  if (!cam || !ws || !color || !alpha || !depth || !n_contrib) return OCGS_ERR_INVALID_ARG;
+  int rc = check_cfg(cfg);
+  if (rc != OCGS_OK) return rc;
+  if ((vis_count == nullptr) != (contrib_sum == nullptr)) return OCGS_ERR_INVALID_ARG;
+  Workspace w;
+  if ((rc = carve_for_render(ws, n, cam, key_capacity, &w)) != OCGS_OK) return rc;
+  return launch_render_fwd(make_cam(*cam), *cfg, w, mask, color, alpha, depth, /*normal=*/nullptr, n_contrib, loss_bg, vis_count, contrib_sum,
+                           nullptr, /*prim=*/1, (cudaStream_t)stream);
 }
 
 int ocgs_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,

@@ -46,10 +46,32 @@ __device__ __forceinline__ bool strip_may_contribute(const float4 r0, const floa
   return keep;
 }
 
+// The same conservative block test for the 3D-Gaussian variant (gaussian3d.cu): rho = a dx^2 + 2 b dx dy + c dy^2 <= rc,
+// per pixel row a quadratic in dx with roots (-b dy -+ sqrt((b dy)^2 - a (c dy^2 - rc))) / a.
+__device__ __forceinline__ bool block_may_contribute3d(const float4 r0, const float4 r2, const float4 r3, int x0, int y0) {
+  constexpr int kW = kSubW, kH = kSubH;
+  const uint32_t b0 = __float_as_uint(r3.z), b1 = __float_as_uint(r3.w);
+  const int ix0 = (int)(b0 & 0xFFFFu), iy0 = (int)(b0 >> 16), ix1 = (int)(b1 & 0xFFFFu), iy1 = (int)(b1 >> 16);
+  if (iy1 < y0 || iy0 > y0 + kH - 1 || ix1 < x0 || ix0 > x0 + kW - 1) return false;
+  const float rc = fmaf(r3.x, 1.0001f, 1e-4f);
+  const float dxa = ((float)x0 - r2.z) - 0.01f, dxb = ((float)(x0 + kW - 1) - r2.z) + 0.01f;
+  const float a = r0.x, b = r0.y, c = r0.z;
+  bool keep = !(a > 0.0f);
+#pragma unroll
+  for (int row = 0; row < kH; ++row) {
+    const float dy = (float)(y0 + row) - r2.w;
+    const float B = -b * dy, Cp = c * dy * dy;
+    const float disc = fmaf(B, B, -a * (Cp - rc)) + 1e-5f * a * (Cp + rc);
+    const float sq = sqrtf(fmaxf(disc, 0.0f));
+    keep |= disc >= 0.0f && (B - sq) <= a * dxb && (B + sq) >= a * dxa;
+  }
+  return keep;
+}
+
 #ifndef OCGS_FWD_MINB
 #define OCGS_FWD_MINB 6
 #endif
-template <bool kStats, bool kMoments>
+template <bool kStats, bool kMoments, int kPrim /*0 = 2D surfel, 1 = 3D Gaussian (EWA conic record)*/>
 __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                          const float4* __restrict__ rec, const uint32_t* __restrict__ rank_to_id,
@@ -109,7 +131,8 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
       bool keep = false;
       if (lane < ce) {
         const float4* se = s_rec + 6 * (c0 + lane);
-        keep = strip_may_contribute(se[0], se[1], se[2], se[3], tx * kTile + sub_x0, ty * kTile + sub_y0, inv_sigma2);
+        keep = kPrim == 0 ? strip_may_contribute(se[0], se[1], se[2], se[3], tx * kTile + sub_x0, ty * kTile + sub_y0, inv_sigma2)
+                          : block_may_contribute3d(se[0], se[2], se[3], tx * kTile + sub_x0, ty * kTile + sub_y0);
       }
       uint32_t todo = __ballot_sync(0xFFFFFFFFu, keep);
       if (__all_sync(0xFFFFFFFFu, done)) { all_done = true; break; }  // once per 32 entries: finished lanes are predicated off below
@@ -118,18 +141,26 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
         todo &= todo - 1;
         const float4* sr = s_rec + 6 * (c0 + jj);
         const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
-        // O4 from the record: q = R - dx P - dy Q, (u,v) = (qx,qy)/qz, hit depth D0/qz
         const float dx = px - r2.z, dy = py - r2.w;
-        const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
-        const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
-        const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
-        const float inv = rcp_approx(qz);
-        const float u = qx * inv, v = qy * inv;
-        const float rho3 = fmaf(u, u, v * v);
-        const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
-        const bool surf = rho3 <= rho2;
-        const float rho = surf ? rho3 : rho2;
-        const float z = surf ? r2.y * inv : r3.y;
+        float rho, z, qz;
+        if (kPrim == 0) {
+          // O4 from the record: q = R - dx P - dy Q, (u,v) = (qx,qy)/qz, hit depth D0/qz
+          const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
+          const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
+          qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
+          const float inv = rcp_approx(qz);
+          const float u = qx * inv, v = qy * inv;
+          const float rho3 = fmaf(u, u, v * v);
+          const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
+          const bool surf = rho3 <= rho2;
+          rho = surf ? rho3 : rho2;
+          z = surf ? r2.y * inv : r3.y;
+        } else {
+          // R-3D: rho = d^T Sigma'^-1 d, depth of the pair = centre depth
+          rho = fmaf(r0.x * dx, dx, fmaf(2.0f * r0.y * dx, dy, r0.z * dy * dy));
+          z = r3.y;
+          qz = 1.0f;
+        }
         bool blend = false;
         float wgt = 0.f;
         if (!done && qz != 0.0f && !(z < near_z) && !(rho > r3.x)) {
@@ -206,7 +237,7 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
     alpha[p] = A;
     depth[p] = D;
     if (kMoments) { mom[p] = zc; mom[HW + p] = M1; mom[2 * HW + p] = M2; }
-    normal[p] = N0; normal[HW + p] = N1; normal[2 * HW + p] = N2;
+    if (kPrim == 0) { normal[p] = N0; normal[HW + p] = N1; normal[2 * HW + p] = N2; }  // the 3D variant has no normal map
     n_contrib[p] = last;
     final_T[p] = T;
   }
@@ -247,18 +278,21 @@ __global__ void __launch_bounds__(1024) loss_final_kernel(const float* __restric
 
 int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Workspace& w, const uint8_t* mask, float* color,
                       float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,
-                      float* contrib_sum, float* mom, cudaStream_t st) {
+                      float* contrib_sum, float* mom, int prim, cudaStream_t st) {
   if (w.n_tiles == 0) return OCGS_OK;
   int rc = launch_order_tiles(w, /*from_ranges=*/true, st);  // launch order: longest lists first
   if (rc != OCGS_OK) return rc;
   const bool stats = vis_count != nullptr && contrib_sum != nullptr;
   float* lp = loss_bg ? w.loss_partial : nullptr;
-#define OCGS_FWD_LAUNCH(S, M)                                                                                                      \
-  render_fwd_kernel<S, M><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, \
+#define OCGS_FWD_LAUNCH(S, M, P)                                                                                                   \
+  render_fwd_kernel<S, M, P><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, \
                                                      mask, cam.W, cam.H, cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib,   \
                                                      w.final_T, w.blist, w.header, lp, vis_count, contrib_sum, mom)
-  if (stats) { if (mom) OCGS_FWD_LAUNCH(true, true); else OCGS_FWD_LAUNCH(true, false); }
-  else       { if (mom) OCGS_FWD_LAUNCH(false, true); else OCGS_FWD_LAUNCH(false, false); }
+  if (prim == 1) {  // 3D Gaussians: forward + statistics only (no moment maps)
+    if (mom) return OCGS_ERR_UNSUPPORTED;
+    if (stats) OCGS_FWD_LAUNCH(true, false, 1); else OCGS_FWD_LAUNCH(false, false, 1);
+  } else if (stats) { if (mom) OCGS_FWD_LAUNCH(true, true, 0); else OCGS_FWD_LAUNCH(true, false, 0); }
+  else              { if (mom) OCGS_FWD_LAUNCH(false, true, 0); else OCGS_FWD_LAUNCH(false, false, 0); }
 #undef OCGS_FWD_LAUNCH
   OCGS_LAUNCHED(st, "render_fwd_kernel");
   if (loss_bg) {

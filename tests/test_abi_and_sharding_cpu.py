@@ -21,7 +21,7 @@ def lib():
 def test_library_exports_every_declared_symbol(lib):
     hdr = open(os.path.join(ROOT, "include", "ocgs.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(ocgs_[a-z0-9_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(ocgs(?:3d)?_[a-z0-9_]+)\s*\(", hdr))
     assert {"ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_prune_stats"} <= declared
     for name in sorted(declared):
         assert hasattr(lib, name), name
