@@ -229,6 +229,22 @@ int ocgs_prune_stats(const ocgs_surfels* in, uint32_t* vis_count, float* contrib
  * in, out: device f32 [n, row_floats], distinct buffers; rows of `out` beyond the survivor count are left untouched. */
 int ocgs_compact_rows(const float* in, const int32_t* remap, int n, int row_floats, float* out, void* stream);
 
+/* ---- clone / split densification (reading R-densify) ---------------------
+ * ocgs_densify_accumulate: after ocgs_render_bwd of a view, grad_accum[j] += |d_center2d_j| and denom[j] += 1 for every
+ *   surfel that passed this view's frustum test (read from the workspace of that view's ocgs_preprocess / ocgs_bin_sort).
+ * ocgs_densify: avg = grad_accum / denom (0 if denom = 0); avg >= grad_threshold selects a surfel; selected surfels with
+ *   max(scale) <= scale_threshold are CLONED, the others SPLIT into two children at p + s_u xi[j,k,0] t_u + s_v xi[j,k,1] t_v
+ *   (xi: device f32 [N,2,2], standard normal numbers supplied by the caller) with scales / 1.6, the parent removed.
+ *   `out` (capacity >= N, ideally 2 N) receives, in this order: non-split surfels (ascending id), clones (ascending id),
+ *   children (ascending parent id, child 0 then 1); src (device i32 [capacity], nullable) the source id of each row;
+ *   counts (device i32[4]) = (n_out, n_keep, n_clone, n_split).  Rows beyond out->capacity are dropped: the caller
+ *   compares counts[0] with the capacity after synchronising.  ws: ocgs_densify_workspace_bytes(N) bytes of device scratch. */
+size_t ocgs_densify_workspace_bytes(int n);
+int ocgs_densify_accumulate(void* ws, int n, int width, int height, size_t key_capacity, const float* d_center2d, float* grad_accum,
+                            uint32_t* denom, void* stream);
+int ocgs_densify(const ocgs_surfels* in, const float* grad_accum, const uint32_t* denom, float grad_threshold, float scale_threshold,
+                 const float* xi, const ocgs_surfels_mut* out, int32_t* src, int* counts, void* ws, void* stream);
+
 /* ---- harness photometric term (S20; the L1 part of Eq. 2) --------------------------------------------
  * loss = 1/(3 H W) sum |M (R - I)| (device scalar, nullable), dL_dcolor[3,H,W] = M sign(R - I)/(3 H W).  color, target:
  * device [3,H,W]; mask device u8 [H,W], nullable (= all ones).  Uses ws.loss_partial as scratch (n, key_capacity: the values

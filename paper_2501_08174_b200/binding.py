@@ -18,7 +18,7 @@ _LIB_PATH = os.path.join(_HERE, "csrc", "libocgs.so")
 OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
            "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_render_fwd_reg", "ocgs_render_bwd_reg", "ocgs3d_preprocess", "ocgs3d_render_fwd", "ocgs_prune_workspace_bytes",
-           "ocgs_prune_stats", "ocgs_compact_rows", "ocgs_step_host", "ocgs_step_view_host", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
+           "ocgs_prune_stats", "ocgs_compact_rows", "ocgs_densify_workspace_bytes", "ocgs_densify_accumulate", "ocgs_densify", "ocgs_step_host", "ocgs_step_view_host", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
            "ocgs_profile_begin", "ocgs_profile_end"]
 
 
@@ -81,6 +81,7 @@ def lib():
         _lib.ocgs_workspace_bytes.restype = C.c_size_t
         _lib.ocgs_prune_workspace_bytes.restype = C.c_size_t
         _lib.ocgs_photometric_workspace_bytes.restype = C.c_size_t
+        _lib.ocgs_densify_workspace_bytes.restype = C.c_size_t
         _lib.ocgs_regularizers_workspace_bytes.restype = C.c_size_t
         for name in EXPORTS:
             getattr(_lib, name)  # raises AttributeError if a declared symbol is not exported
@@ -225,6 +226,20 @@ def ocgs_prune_stats(surfels, vis_count, contrib_sum, cfg, prune_mask, remap, ou
     _ok("ocgs_prune_stats", lib().ocgs_prune_stats(C.byref(surfels), _ptr(vis_count), _ptr(contrib_sum), C.byref(cfg), _ptr(prune_mask),
                                                    _ptr(remap), C.byref(out) if out is not None else None, _ptr(n_out),
                                                    C.c_int(int(reset_stats)), _ptr(ws), _stream(stream)))
+
+
+def ocgs_densify_workspace_bytes(n: int) -> int:
+    return int(lib().ocgs_densify_workspace_bytes(C.c_int(n)))
+
+
+def ocgs_densify_accumulate(ws, n, width, height, key_capacity, d_center2d, grad_accum, denom, stream=None):
+    _ok("ocgs_densify_accumulate", lib().ocgs_densify_accumulate(_ptr(ws), C.c_int(n), C.c_int(width), C.c_int(height), C.c_size_t(key_capacity),
+                                                                 _ptr(d_center2d), _ptr(grad_accum), _ptr(denom), _stream(stream)))
+
+
+def ocgs_densify(surfels, grad_accum, denom, grad_threshold, scale_threshold, xi, out: ocgs_surfels_mut, src, counts, scratch, stream=None):
+    _ok("ocgs_densify", lib().ocgs_densify(C.byref(surfels), _ptr(grad_accum), _ptr(denom), C.c_float(grad_threshold), C.c_float(scale_threshold),
+                                           _ptr(xi), C.byref(out), _ptr(src), _ptr(counts), _ptr(scratch), _stream(stream)))
 
 
 def ocgs_compact_rows(inp, remap, n: int, row_floats: int, out, stream=None):

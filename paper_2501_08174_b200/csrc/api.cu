@@ -313,6 +313,25 @@ int ocgs_prune_stats(const ocgs_surfels* in, uint32_t* vis_count, float* contrib
   return launch_prune(*in, vis_count, contrib_sum, *cfg, prune_mask, remap, out, n_out, reset_stats, ws, (cudaStream_t)stream);
 }
 
+size_t ocgs_densify_workspace_bytes(int n) { return densify_workspace_bytes(n); }
+
+int ocgs_densify_accumulate(void* ws, int n, int width, int height, size_t key_capacity, const float* d_center2d, float* grad_accum,
+                            uint32_t* denom, void* stream) {
+  if (!ws || (n > 0 && (!d_center2d || !grad_accum || !denom))) return OCGS_ERR_INVALID_ARG;
+  Workspace w;
+  if (!carve_workspace(ws, n, width, height, key_capacity, &w, nullptr)) return OCGS_ERR_UNSUPPORTED;
+  return launch_densify_accumulate(w, d_center2d, grad_accum, denom, (cudaStream_t)stream);
+}
+
+int ocgs_densify(const ocgs_surfels* in, const float* grad_accum, const uint32_t* denom, float grad_threshold, float scale_threshold,
+                 const float* xi, const ocgs_surfels_mut* out, int32_t* src, int* counts, void* ws, void* stream) {
+  if (!in || !out || !counts || !ws) return OCGS_ERR_INVALID_ARG;
+  if (in->n > 0 && (!grad_accum || !denom || !xi || !in->pos || !in->scale || !in->quat || !in->opacity || !in->sh || !out->pos ||
+                    !out->scale || !out->quat || !out->opacity || !out->sh)) return OCGS_ERR_INVALID_ARG;
+  if (out->capacity < in->n) return OCGS_ERR_CAPACITY;
+  return launch_densify(*in, grad_accum, denom, grad_threshold, scale_threshold, xi, *out, src, counts, ws, (cudaStream_t)stream);
+}
+
 int ocgs_compact_rows(const float* in, const int32_t* remap, int n, int row_floats, float* out, void* stream) {
   if (n < 0 || row_floats <= 0) return OCGS_ERR_INVALID_ARG;
   if (n > 0 && (!in || !remap || !out || in == out)) return OCGS_ERR_INVALID_ARG;

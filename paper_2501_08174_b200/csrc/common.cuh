@@ -106,6 +106,10 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
 int launch_prune(const ocgs_surfels& in, uint32_t* vis_count, float* contrib_sum, const ocgs_config& cfg, uint8_t* prune_mask,
                  int32_t* remap, const ocgs_surfels_mut* out, int* n_out, int reset_stats, void* ws, cudaStream_t st);
 
+size_t densify_workspace_bytes(int n);
+int launch_densify_accumulate(const Workspace& w, const float* d_center2d, float* grad_accum, uint32_t* denom, cudaStream_t st);
+int launch_densify(const ocgs_surfels& in, const float* grad_accum, const uint32_t* denom, float grad_threshold, float scale_threshold,
+                   const float* xi, const ocgs_surfels_mut& out, int32_t* src, int* counts, void* ws, cudaStream_t st);
 int launch_compact_rows(const float* in, const int32_t* remap, int n, int row_floats, float* out, cudaStream_t st);
 
 int launch_masked_l1(const float* color, const float* target, const uint8_t* mask, int W, int H, float* dL_dcolor, float* loss,
