@@ -2,9 +2,9 @@
 """bench.py -- ms per fwd+bwd raster step on the paper-shaped workload (BASELINE.json configs[2]: 1600x1200, 1 M surfels).
 
 A "step" is one pass of the whole hot path over one view: ocgs_preprocess -> ocgs_bin_sort -> ocgs_render_fwd (background
-loss L_b and visibility statistics on) -> ocgs_masked_l1 (harness photometric gradient, S20) -> ocgs_render_bwd, all
+loss L_b and visibility statistics on, with the harness masked-L1 term of S20 fused: ocgs_render_fwd_l1) -> ocgs_render_bwd, all
 through the C ABI.  Views rotate over a fixed set; inputs are resident in HBM before the timed region (`value`), or in
-pinned host memory with the copies inside the timed region (`e2e`, through ocgs_step_host).  `--impl reference` times the
+pinned host memory with the copies inside the timed region (`e2e`, through ocgs_step_view_host).  `--impl reference` times the
 CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -248,12 +248,13 @@ def run_ours(args):
             B.ocgs_render_bwd_reg(surfels, c, cfg, ws, cap, m, out["n_contrib"], gC, gA_r, gD_r, gN_r, moments, gM_r, grads["d_pos"],
                                   grads["d_scale"], grads["d_quat"], grads["d_opacity"], grads["d_sh"], grads["d_center2d"])
             return
-        B.ocgs_render_fwd(n, c, cfg, ws, cap, m, out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"], out["loss_bg"],
-                          vis if stats else None, cs if stats else None)
         if args.loss == "dssim":
+            B.ocgs_render_fwd(n, c, cfg, ws, cap, m, out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"], out["loss_bg"],
+                              vis if stats else None, cs if stats else None)
             B.ocgs_photometric_loss(out["color"], targets[i], m, W, H, 0.2, gC, loss_pm, pws_photo)
-        else:
-            B.ocgs_masked_l1(out["color"], targets[i], m, W, H, gC, loss_l1, ws, n, cap)
+        else:  # harness loss S20: masked L1 fused into the forward epilogue (dL/dcolor produced in-kernel)
+            B.ocgs_render_fwd_l1(n, c, cfg, ws, cap, m, targets[i], out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"],
+                                 out["loss_bg"], loss_l1, gC, vis if stats else None, cs if stats else None)
         B.ocgs_render_bwd(surfels, c, cfg, ws, cap, m, out["n_contrib"], gC, None, None, None, grads["d_pos"], grads["d_scale"],
                           grads["d_quat"], grads["d_opacity"], grads["d_sh"], grads["d_center2d"])
 

@@ -144,6 +144,15 @@ int ocgs_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void*
                     float* color, float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg,
                     uint32_t* vis_count, float* contrib_sum, void* stream);
 
+/* (3a) forward with the harness photometric term fused into the epilogue (S20; "M R vs M I L1 in the fwd
+ * epilogue and dL/dC produced in-kernel"): = ocgs_render_fwd followed by ocgs_masked_l1(color, target, mask, ...), without
+ * re-reading the colour map.  target: device f32 [3,H,W]; dL_dcolor: device f32 [3,H,W], OVERWRITTEN (bit-identical to
+ * ocgs_masked_l1's); loss_l1: device f32 scalar, nullable (deterministic; its summation order differs from
+ * ocgs_masked_l1's, so the two values agree to fp32 rounding, not bit for bit). */
+int ocgs_render_fwd_l1(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
+                       const float* target, float* color, float* alpha, float* depth, float* normal, uint32_t* n_contrib,
+                       float* loss_bg, float* loss_l1, float* dL_dcolor, uint32_t* vis_count, float* contrib_sum, void* stream);
+
 /* ---- (4) backward ---------------------------------------------------------------------------------------------------
  * "Through backpropagation, the position, shape, and appearance of all involved Gaussians are updated";
  * occluded Gaussians receive no gradient (exact zeros).  O7.  Inputs: the forward's n_contrib (and the

@@ -96,7 +96,7 @@ int launch_preprocess(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
 int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cudaStream_t st);
 int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Workspace& w, const uint8_t* mask, float* color,
                       float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,
-                      float* contrib_sum, float* mom, int prim, cudaStream_t st);
+                      float* contrib_sum, float* mom, int prim, const float* target, float* gC, float* loss_l1, cudaStream_t st);
 int launch_preprocess3d(const ocgs_gaussians3d& g, const CamParams& cam, const ocgs_config& cfg, Workspace& w, cudaStream_t st);
 int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, const uint8_t* mask,
                       const float* final_T, const uint32_t* n_contrib, const float* gC, const float* gA, const float* gD,

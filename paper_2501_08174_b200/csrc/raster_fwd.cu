@@ -71,7 +71,10 @@ __device__ __forceinline__ bool block_may_contribute3d(const float4 r0, const fl
 #ifndef OCGS_FWD_MINB
 #define OCGS_FWD_MINB 6
 #endif
-template <bool kStats, bool kMoments, int kPrim /*0 = 2D surfel, 1 = 3D Gaussian (EWA conic record)*/>
+// fused harness photometric term (S20): target image in, dL/dcolor and per-tile partial sums of |M (R - I)| out
+struct FwdL1 { const float* target; float* gC; float* partial; float inv_norm; };
+
+template <bool kStats, bool kMoments, int kPrim /*0 = 2D surfel, 1 = 3D Gaussian (EWA conic record)*/, bool kL1>
 __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                          const float4* __restrict__ rec, const uint32_t* __restrict__ rank_to_id,
@@ -79,7 +82,7 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
                                                          ocgs_config cfg, float* __restrict__ color, float* __restrict__ alpha,
                                                          float* __restrict__ depth, float* __restrict__ normal,
                                                          uint32_t* __restrict__ n_contrib, float* __restrict__ final_T, uint2* __restrict__ blist, ocgs_header* __restrict__ header, float* __restrict__ loss_partial,
-                                                         uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum, float* __restrict__ mom /*[3,H,W]: origin, m1, m2 (kMoments)*/) {
+                                                         uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum, float* __restrict__ mom /*[3,H,W]: origin, m1, m2 (kMoments)*/, FwdL1 l1) {
   __shared__ float4 s_rec[kFwdBatch * 6];
   __shared__ uint32_t s_rank[kFwdBatch];
   __shared__ uint32_t s_hit[kFwdBatch];  // bit w: warp w blended the entry (read by the backward pass)
@@ -231,6 +234,7 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
   }
 
   const float A = 1.0f - T;
+  float l1sum = 0.f;
   if (inside) {
     const size_t HW = (size_t)W * H, p = (size_t)iy * W + ix;
     color[p] = fmaf(T, cfg.bg[0], C0); color[HW + p] = fmaf(T, cfg.bg[1], C1); color[2 * HW + p] = fmaf(T, cfg.bg[2], C2);
@@ -240,6 +244,16 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
     if (kPrim == 0) { normal[p] = N0; normal[HW + p] = N1; normal[2 * HW + p] = N2; }  // the 3D variant has no normal map
     n_contrib[p] = last;
     final_T[p] = T;
+    if (kL1) {  // masked L1 against the target, straight from the registers that hold the pixel's colour
+      const bool m = mask == nullptr || mask[p] != 0;
+      const float col[3] = {fmaf(T, cfg.bg[0], C0), fmaf(T, cfg.bg[1], C1), fmaf(T, cfg.bg[2], C2)};
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const float d = m ? col[c] - l1.target[c * HW + p] : 0.f;
+        l1sum += fabsf(d);
+        l1.gC[c * HW + p] = d > 0.f ? l1.inv_norm : (d < 0.f ? -l1.inv_norm : 0.f);
+      }
+    }
   }
   if (threadIdx.x == 0) {
     tile_work[tile] = nhit;  // length of the blended list: the backward pass's loop bound and work estimate
@@ -260,43 +274,69 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
       loss_partial[tile] = s;
     }
   }
+  if (kL1) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) l1sum += __shfl_xor_sync(0xFFFFFFFFu, l1sum, o);
+    __syncthreads();
+    if (lane == 0) s_red[threadIdx.x >> 5] = l1sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      float s = 0.f;
+#pragma unroll
+      for (int w2 = 0; w2 < 8; ++w2) s += s_red[w2];
+      l1.partial[tile] = s;
+    }
+  }
 }
 
 __global__ void __launch_bounds__(1024) loss_final_kernel(const float* __restrict__ partial, int n_tiles, float inv_hw,
-                                                          float* __restrict__ loss_bg) {
-  __shared__ double s[1024];
-  double acc = 0.0;
-  for (int i = threadIdx.x; i < n_tiles; i += 1024) acc += (double)partial[i];
-  s[threadIdx.x] = acc;
+                                                          float* __restrict__ loss_bg, const float* __restrict__ partial2, float scale2,
+                                                          float* __restrict__ loss2) {
+  __shared__ double s[2][1024];
+  double acc = 0.0, acc2 = 0.0;
+  for (int i = threadIdx.x; i < n_tiles; i += 1024) {
+    if (loss_bg) acc += (double)partial[i];
+    if (loss2) acc2 += (double)partial2[i];
+  }
+  s[0][threadIdx.x] = acc; s[1][threadIdx.x] = acc2;
   __syncthreads();
   for (int o = 512; o > 0; o >>= 1) {
-    if ((int)threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
+    if ((int)threadIdx.x < o) { s[0][threadIdx.x] += s[0][threadIdx.x + o]; s[1][threadIdx.x] += s[1][threadIdx.x + o]; }
     __syncthreads();
   }
-  if (threadIdx.x == 0) *loss_bg = (float)(s[0] * (double)inv_hw);
+  if (threadIdx.x == 0) {
+    if (loss_bg) *loss_bg = (float)(s[0][0] * (double)inv_hw);
+    if (loss2) *loss2 = (float)(s[1][0] * (double)scale2);
+  }
 }
 
 int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Workspace& w, const uint8_t* mask, float* color,
                       float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,
-                      float* contrib_sum, float* mom, int prim, cudaStream_t st) {
+                      float* contrib_sum, float* mom, int prim, const float* target, float* gC, float* loss_l1, cudaStream_t st) {
   if (w.n_tiles == 0) return OCGS_OK;
   int rc = launch_order_tiles(w, /*from_ranges=*/true, st);  // launch order: longest lists first
   if (rc != OCGS_OK) return rc;
   const bool stats = vis_count != nullptr && contrib_sum != nullptr;
   float* lp = loss_bg ? w.loss_partial : nullptr;
-#define OCGS_FWD_LAUNCH(S, M, P)                                                                                                   \
-  render_fwd_kernel<S, M, P><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, \
+  FwdL1 l1 = {target, gC, w.loss_partial + w.n_tiles, (float)(1.0 / (3.0 * (double)cam.W * (double)cam.H))};
+#define OCGS_FWD_LAUNCH(S, M, P, L)                                                                                                \
+  render_fwd_kernel<S, M, P, L><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, \
                                                      mask, cam.W, cam.H, cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib,   \
-                                                     w.final_T, w.blist, w.header, lp, vis_count, contrib_sum, mom)
+                                                     w.final_T, w.blist, w.header, lp, vis_count, contrib_sum, mom, l1)
   if (prim == 1) {  // 3D Gaussians: forward + statistics only (no moment maps)
-    if (mom) return OCGS_ERR_UNSUPPORTED;
-    if (stats) OCGS_FWD_LAUNCH(true, false, 1); else OCGS_FWD_LAUNCH(false, false, 1);
-  } else if (stats) { if (mom) OCGS_FWD_LAUNCH(true, true, 0); else OCGS_FWD_LAUNCH(true, false, 0); }
-  else              { if (mom) OCGS_FWD_LAUNCH(false, true, 0); else OCGS_FWD_LAUNCH(false, false, 0); }
+    if (mom || target) return OCGS_ERR_UNSUPPORTED;
+    if (stats) OCGS_FWD_LAUNCH(true, false, 1, false); else OCGS_FWD_LAUNCH(false, false, 1, false);
+  } else if (target) {  // fused masked L1 (no moment maps in this variant)
+    if (mom || !gC) return OCGS_ERR_UNSUPPORTED;
+    if (stats) OCGS_FWD_LAUNCH(true, false, 0, true); else OCGS_FWD_LAUNCH(false, false, 0, true);
+  } else if (stats) { if (mom) OCGS_FWD_LAUNCH(true, true, 0, false); else OCGS_FWD_LAUNCH(true, false, 0, false); }
+  else              { if (mom) OCGS_FWD_LAUNCH(false, true, 0, false); else OCGS_FWD_LAUNCH(false, false, 0, false); }
 #undef OCGS_FWD_LAUNCH
   OCGS_LAUNCHED(st, "render_fwd_kernel");
-  if (loss_bg) {
-    loss_final_kernel<<<1, 1024, 0, st>>>(w.loss_partial, w.n_tiles, (float)(1.0 / ((double)cam.W * (double)cam.H)), loss_bg);
+  float* l1_out = target ? loss_l1 : nullptr;
+  if (loss_bg || l1_out) {
+    loss_final_kernel<<<1, 1024, 0, st>>>(w.loss_partial, w.n_tiles, (float)(1.0 / ((double)cam.W * (double)cam.H)), loss_bg,
+                                          w.loss_partial + w.n_tiles, l1.inv_norm, l1_out);
     OCGS_LAUNCHED(st, "loss_final_kernel");
   }
   return OCGS_OK;

@@ -216,6 +216,20 @@ def test_masked_l1_and_host_step_match_device_path():
     assert abs(float(loss.item()) - np.abs(d).sum() / (3 * 240 * 320)) < 1e-6
     assert np.array_equal(gC.cpu().numpy(), (np.sign(d) / np.float32(3 * 240 * 320)).astype(np.float32))
     gg = g.render_bwd(gC=gC.cpu().numpy())
+    # the fused forward (ocgs_render_fwd_l1) = forward + masked L1 without re-reading the colour map: maps and dL/dcolor
+    # bit-identical, the L1 scalar equal to fp32 rounding (different summation order)
+    o2 = B.alloc_outputs(320, 240)
+    gC2 = torch.full_like(tt, 9.0); l1f = torch.zeros(1, device="cuda")
+    vis_f = torch.zeros(g.n, dtype=torch.int32, device="cuda"); cs_f = torch.zeros(g.n, device="cuda")
+    B.ocgs_render_fwd_l1(g.n, g.cam, g.cfg, g.ws, g.cap, g.mask_t, tt, o2["color"], o2["alpha"], o2["depth"], o2["normal"], o2["n_contrib"],
+                         o2["loss_bg"], l1f, gC2, vis_f, cs_f)
+    torch.cuda.synchronize()
+    for k in ("color", "alpha", "depth", "normal"):
+        assert np.array_equal(o2[k].cpu().numpy(), gf[k]), k
+    assert np.array_equal(gC2.cpu().numpy(), gC.cpu().numpy()) and float(o2["loss_bg"].item()) == gf["loss_bg"]
+    assert abs(float(l1f.item()) - float(loss.item())) < 1e-7
+    assert np.array_equal(vis_f.cpu().numpy().view(np.uint32), gf["vis_count"])
+    g.render_fwd(mask=m)  # restore the workspace state (blended lists) the checks below rely on
     # the same step through ocgs_step_host (host buffers, copies inside)
     n, H, W = g.n, 240, 320
     hp = [torch.tensor(np.ascontiguousarray(a, np.float32)).pin_memory() for a in arrays(sc)]
