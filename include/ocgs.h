@@ -12,7 +12,9 @@
  *    synchronises except ocgs_check(), ocgs_step_view_host() and ocgs_step_host().  A step can therefore be captured in a CUDA graph.
  *  - The data-dependent key count K never travels to the host inside a step: kernels read it from the workspace
  *    header.  If K exceeds `key_capacity` the header error flag is set, later calls of the step become no-ops, and
- *    ocgs_check() reports OCGS_ERR_CAPACITY with the needed size.
+ *    ocgs_check() reports OCGS_ERR_CAPACITY with the needed size.  Limits: N and key_capacity below 2^30 (the radix
+ *    passes carry counts in 30-bit status words); a single tile's list below 2^24 entries (list positions are packed
+ *    with the hit bits handed to the backward pass), otherwise ocgs_check() reports OCGS_ERR_UNSUPPORTED.
  *  - Images are planar [C,H,W] fp32, row-major, origin top-left; integer pixel index (ix,iy) is the pixel centre,
  *    x_idx = fx X/Z + cx - 1/2 (S2).  Surfel parameters are ACTIVATED values: scale > 0, opacity in (0,1),
  *    quaternion (w,x,y,z) used through the polynomial R(q) without normalisation (S19).

@@ -26,7 +26,7 @@ static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 bool carve_workspace(void* ws, int n, int width, int height, size_t key_capacity, Workspace* out, ocgs_ws_layout* layout) {
   if (n < 0 || width <= 0 || height <= 0 || width > OCGS_MAX_DIM || height > OCGS_MAX_DIM) return false;
-  if (key_capacity > 0xFFFFFFF0ull || (size_t)n > 0x7FFFFFF0ull) return false;
+  if (key_capacity >= (1ull << 30) || (size_t)n >= (1ull << 30)) return false;  // 30-bit counts in the radix status words
   const int tiles_x = (width + kTile - 1) / kTile, tiles_y = (height + kTile - 1) / kTile;
   const size_t n_tiles = (size_t)tiles_x * tiles_y;
   const size_t N = (size_t)n, K = key_capacity;

@@ -10,10 +10,8 @@ namespace ocgs {
 constexpr int kTile = 16;
 // pixel block of one forward warp inside the tile (32 pixels); bit w of a list entry's `hit` byte refers to block w,
 // numbered row-major.  8x4 blocks are cut by fewer splat outlines than 16x2 strips, so fewer (warp, entry) pairs are walked.
-#ifndef OCGS_SUBW
-#define OCGS_SUBW 8
-#endif
-constexpr int kSubW = OCGS_SUBW, kSubH = 32 / kSubW;
+// (16x2 strips and 4x8 blocks measured slower: step 2.30 / 2.35 ms against 2.21 ms.)
+constexpr int kSubW = 8, kSubH = 32 / kSubW;
 constexpr int kRec = 24;  // floats per raster record (96 B = 6 x float4)
 // Record layout.  With c = c2d the projected centre, A0 = M0 - cx*M2, A1 = M1 - cy*M2 (third
 // components are the exact division residuals), the pixel ray (x, y) meets the surfel plane at (u,v) = (qx,qy)/qz with

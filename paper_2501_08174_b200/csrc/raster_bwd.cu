@@ -1,8 +1,8 @@
 // raster_bwd.cu -- ocgs_render_bwd (O7).
-//  (a) render_bwd_kernel: one CTA per tile, one thread per pixel, the tile list walked BACK to FRONT over
-//      [0, max n_contrib); per pair the chain rule through compositing and the ray-splat intersection gives 18 record
-//      gradients, reduced across the warp by a transposing butterfly (16 values, 16+8+4+2+1 shuffles) then combined
-//      across the CTA in shared memory and flushed with one global RED per (tile, entry, field).
+//  (a) render_bwd_kernel: one CTA per tile, two pixels per thread, the tile's compact list of BLENDED entries (written by
+//      the forward pass) walked BACK to FRONT; per pair the chain rule through compositing and the ray-splat intersection
+//      gives 16 + 4 record gradients, reduced across the warp by a transposing butterfly (16 values, 8+4+2+1+1 shuffles),
+//      stored per warp in shared memory, combined across the CTA and flushed with one global RED per (tile, entry, field).
 //  (b) project_bwd_kernel: one thread per surfel, record gradients -> (pos, scale, quat, opacity, sh) gradients.
 #include "projection.cuh"
 
@@ -128,17 +128,15 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
   return contributes;
 }
 
-// CTA = one 16x16 tile, 128 threads, TWO pixels per thread: warp w owns rows 4w..4w+3, lane l the pixels
-// (l & 15, 4w + (l >> 4)) and (l & 15, 4w + 2 + (l >> 4)), i.e. one pixel in each of the forward kernel's 16x2 strips
-// 2w and 2w+1.  The two pixels' gradient terms are added in registers (free: the adds fold into FMAs) before the
-// 32-lane transposing reduction, which is therefore paid once per 64 pixels (four pixels per thread, 64-thread CTAs, measured slower: 1.21 vs 1.13 ms).  Each warp owns a slice of the batch
-// accumulator and visits an entry at most once per batch, so its totals are plain stores (shared float atomics are
-// CAS loops); the flush adds the slices of the warps whose forward `hit` bits are set.
-#ifndef OCGS_BWD_MINB
-#define OCGS_BWD_MINB 5
-#endif
+// CTA = one 16x16 tile, 128 threads, TWO pixels per thread: warp w owns two vertically adjacent pixel blocks of the forward
+// kernel (kSubW x kSubH each, common.cuh), lane l one pixel in each.  The two pixels' gradient terms are added in registers
+// (free: the adds fold into FMAs) before the 32-lane transposing reduction, which is therefore paid once per 64 pixels
+// (four pixels per thread in 64-thread CTAs measured slower: 1.21 vs 1.13 ms).  Each warp owns a slice of the batch
+// accumulator and visits an entry at most once per batch, so its totals are plain stores (shared float atomics are CAS
+// loops); the flush adds the slices of the warps whose forward hit bits are set.
+constexpr int kBwdMinBlocks = 5;  // 4, 6, 7 measured slower
 template <bool kMoments>
-__global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
+__global__ void __launch_bounds__(128, kBwdMinBlocks) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                             const float4* __restrict__ rec, const uint2* __restrict__ blist, const uint8_t* __restrict__ mask,
                                                             const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
@@ -205,7 +203,7 @@ __global__ void __launch_bounds__(128, OCGS_BWD_MINB) render_bwd_kernel(const ui
       const int e = i / 6, part = i - 6 * e;
       s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
     }
-    // per warp: which entries of the batch did strips 2w / 2w+1 blend (bit e of lo: entry e, of hi: entry 32 + e)
+    // per warp: which entries of the batch did its two pixel blocks blend (bit e of lo: entry e, of hi: entry 32 + e)
     const uint32_t mlo = lane < cnt ? s_mask[lane] : 0u, mhi = lane + 32 < cnt ? s_mask[lane + 32] : 0u;
     const uint32_t lo0 = __ballot_sync(0xFFFFFFFFu, mlo & bit0), lo1 = __ballot_sync(0xFFFFFFFFu, mlo & bit1);
     const uint32_t hi0 = __ballot_sync(0xFFFFFFFFu, mhi & bit0), hi1 = __ballot_sync(0xFFFFFFFFu, mhi & bit1);

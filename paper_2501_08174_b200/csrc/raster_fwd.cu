@@ -1,26 +1,26 @@
-// raster_fwd.cu -- ocgs_render_fwd (O4-O6, O8): one CTA per 16x16 tile, one thread per pixel, the tile's depth-ordered
-// list walked front to back in shared-memory batches of records; early stop per pixel, per warp and per CTA.
-// Fused: background loss L_b (Eq. 1) and the visibility statistics.
+// raster_fwd.cu -- ocgs_render_fwd and its variants (O4-O6, O8): one CTA per 16x16 tile, one thread per pixel, warp w owns the
+// kSubW x kSubH pixel block w; the tile's depth-ordered list is walked front to back in shared-memory batches of records:
+// per 32 entries an entry-parallel conservative cull against the warp's block, then the pixel-parallel walk of the
+// survivors; early stop per pixel, per warp and per CTA.  Fused: background loss L_b (Eq. 1), the visibility
+// statistics, the compact list of blended entries handed to the backward pass, and optionally the depth
+// moments (kMoments, f-2), the harness masked-L1 term (kL1, f-1) or the 3D-Gaussian pair rule (kPrim = 1, f-3).
 #include "common.cuh"
 
 namespace ocgs {
 
-#ifndef OCGS_FWD_BATCH
-#define OCGS_FWD_BATCH 256
-#endif
-constexpr int kFwdBatch = OCGS_FWD_BATCH;     // list entries staged per batch
+constexpr int kFwdBatch = 256;                 // list entries staged per batch (= block size; 128 measured 2 % slower)
 constexpr float kContribFix = 134217728.0f;    // 2^27: alpha*T in fixed point for the warp-wide REDUX sum
 
-// Conservative test "can surfel (r0..r3) contribute to any pixel of the 16x2 strip with first pixel (x0, y0)?", run by ONE
+// Conservative test "can surfel (r0..r3) contribute to any pixel of the kSubW x kSubH block with first pixel (x0, y0)?", run by ONE
 // lane per list entry (32 entries per warp step) so that the pixel-parallel walk below only visits survivors.
 // A pair contributes iff rho = min(rho3, rho2) <= rho_cut (S6).  Per pixel row dy = y - cy:
 //   rho3 <= rc  <=>  F(dx) = |S - dx P|_W^2 <= 0,  S = R - dy Q,  W = diag(1, 1, -rc)   (q = R - dx P - dy Q, rho3 = (qx^2+qy^2)/qz^2)
 //   i.e. A dx^2 - 2 B dx + C <= 0 with A = P.WP, B = S.WP, C = S.WS: real roots (B -+ sqrt(B^2 - AC))/A must overlap the
-//   strip's dx range; rho2 <= rc is a disc of radius sqrt(rc sigma_f^2) about the centre.
+//   block's dx range; rho2 <= rc is a disc of radius sqrt(rc sigma_f^2) about the centre.
 // Every inequality is relaxed (rc by 1e-4 relative + 1e-4, the dx range by 0.01 px, the discriminant by 1e-5 of its
 // term magnitudes), far more than the fp32 error of either this test or the per-pixel evaluation, so a pair the walk
 // would blend is never culled: the images are bit-identical with and without the cull.
-__device__ __forceinline__ bool strip_may_contribute(const float4 r0, const float4 r1, const float4 r2, const float4 r3, int x0, int y0,
+__device__ __forceinline__ bool block_may_contribute(const float4 r0, const float4 r1, const float4 r2, const float4 r3, int x0, int y0,
                                                      float inv_sigma2) {
   constexpr int kW = kSubW, kH = kSubH;  // the warp's pixel block (common.cuh)
   const uint32_t b0 = __float_as_uint(r3.z), b1 = __float_as_uint(r3.w);
@@ -68,14 +68,12 @@ __device__ __forceinline__ bool block_may_contribute3d(const float4 r0, const fl
   return keep;
 }
 
-#ifndef OCGS_FWD_MINB
-#define OCGS_FWD_MINB 6
-#endif
+constexpr int kFwdMinBlocks = 6;               // CTAs per SM the register budget is held to (40 registers; 5 and 7 measured slower)
 // fused harness photometric term (S20): target image in, dL/dcolor and per-tile partial sums of |M (R - I)| out
 struct FwdL1 { const float* target; float* gC; float* partial; float inv_norm; };
 
 template <bool kStats, bool kMoments, int kPrim /*0 = 2D surfel, 1 = 3D Gaussian (EWA conic record)*/, bool kL1>
-__global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ tile_work,
+__global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                          const float4* __restrict__ rec, const uint32_t* __restrict__ rank_to_id,
                                                          const uint8_t* __restrict__ mask, int W, int H, int tiles_x,
@@ -130,11 +128,11 @@ __global__ void __launch_bounds__(256, OCGS_FWD_MINB) render_fwd_kernel(const ui
     for (int c0 = 0; c0 < cnt && !all_done; c0 += 32) {
       uint32_t cntr = 0, fixr = 0;
       const int ce = min(32, cnt - c0);
-      // entry-parallel cull: lane l tests entry c0 + l against this warp's strip; the walk visits the survivors
+      // entry-parallel cull: lane l tests entry c0 + l against this warp's pixel block; the walk visits the survivors
       bool keep = false;
       if (lane < ce) {
         const float4* se = s_rec + 6 * (c0 + lane);
-        keep = kPrim == 0 ? strip_may_contribute(se[0], se[1], se[2], se[3], tx * kTile + sub_x0, ty * kTile + sub_y0, inv_sigma2)
+        keep = kPrim == 0 ? block_may_contribute(se[0], se[1], se[2], se[3], tx * kTile + sub_x0, ty * kTile + sub_y0, inv_sigma2)
                           : block_may_contribute3d(se[0], se[2], se[3], tx * kTile + sub_x0, ty * kTile + sub_y0);
       }
       uint32_t todo = __ballot_sync(0xFFFFFFFFu, keep);
