@@ -68,6 +68,11 @@ __device__ __forceinline__ bool block_may_contribute3d(const float4 r0, const fl
   return keep;
 }
 
+// Tiles with long lists finish last, alone on their SM, where two warps per scheduler cannot hide the ~300-cycle dependent
+// chain of one survivor: above kFwdHeavyLen entries the walk takes kFwdIlp survivors per iteration (measured at config 5:
+// forward 2.34 -> 2.04 ms with 2, 2.07 with 4, 2.09 with 3; used for every tile it costs 3 % at config 3).
+constexpr int kFwdIlp = 2;
+constexpr uint32_t kFwdHeavyLen = 2048;
 constexpr int kFwdMinBlocks = 6;               // CTAs per SM the register budget is held to (40 registers; 5 and 7 measured slower)
 // fused harness photometric term (S20): target image in, dL/dcolor and per-tile partial sums of |M (R - I)| out
 struct FwdL1 { const float* target; float* gC; float* partial; float inv_norm; };
@@ -110,6 +115,7 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
   uint32_t last = 0;
   uint32_t nhit = 0;  // entries of this tile blended so far (uniform across the CTA)
   bool done = !inside;
+  const bool heavy = end - start > kFwdHeavyLen;
 
   for (uint32_t b0 = start; b0 < end; b0 += kFwdBatch) {
     const int cnt = (int)min((uint32_t)kFwdBatch, end - b0);
@@ -137,6 +143,62 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
       }
       uint32_t todo = __ballot_sync(0xFFFFFFFFu, keep);
       if (__all_sync(0xFFFFFFFFu, done)) { all_done = true; break; }  // once per 32 entries: finished lanes are predicated off below
+      if (kPrim == 0 && heavy) {
+        // long lists (a lone CTA on its SM at the kernel's tail): kFwdIlp survivors per iteration, evaluated without branches so
+        // that their latencies overlap; the blend itself stays in list order and keeps the arithmetic of the loop below
+        while (todo) {
+          int jj[kFwdIlp]; bool ok[kFwdIlp]; float a[kFwdIlp], z[kFwdIlp];
+#pragma unroll
+          for (int k = 0; k < kFwdIlp; ++k) {
+            const bool on = todo != 0;
+            jj[k] = on ? __ffs(todo) - 1 : (k ? jj[0] : 0);
+            todo &= todo - 1;
+            const float4* sr = s_rec + 6 * (c0 + jj[k]);
+            const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
+            const float dx = px - r2.z, dy = py - r2.w;
+            const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
+            const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
+            const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
+            const float inv = rcp_approx(qz);
+            const float u = qx * inv, v = qy * inv;
+            const float rho3 = fmaf(u, u, v * v);
+            const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
+            const bool surf = rho3 <= rho2;
+            const float rho = surf ? rho3 : rho2;
+            const float zz = surf ? r2.y * inv : r3.y;
+            ok[k] = on && qz != 0.0f && !(zz < near_z) && !(rho > r3.x);
+            z[k] = ok[k] ? zz : 0.0f;
+            a[k] = fminf(alpha_max, sr[4].x * ex2_approx(rho * kNegHalfLog2e));
+            if (!on) jj[k] = -1;
+          }
+#pragma unroll
+          for (int k = 0; k < kFwdIlp; ++k) {
+            const int j = jj[k] < 0 ? 0 : jj[k];
+            const float4* sr = s_rec + 6 * (c0 + j);
+            const float Tn = T * (1.0f - a[k]);
+            const bool live = ok[k] && !done;
+            const bool blend = live && !(Tn < t_min);
+            done = done || (live && Tn < t_min);  // S11: stop before blending this pair
+            const float wgt = blend ? a[k] * T : 0.0f;
+            const float4 r4 = sr[4], r5 = sr[5];
+            C0 = fmaf(wgt, r4.y, C0); C1 = fmaf(wgt, r4.z, C1); C2 = fmaf(wgt, r4.w, C2);
+            D = fmaf(wgt, z[k], D);
+            if (kMoments) {
+              zc = (blend && last == 0) ? z[k] : zc;
+              const float dz = blend ? z[k] - zc : 0.0f;
+              M1 = fmaf(wgt, dz, M1);
+              M2 = fmaf(wgt * dz, dz, M2);
+            }
+            N0 = fmaf(wgt, r5.x, N0); N1 = fmaf(wgt, r5.y, N1); N2 = fmaf(wgt, r5.z, N2);
+            T = blend ? Tn : T;
+            last = blend ? (b0 - start) + c0 + j + 1 : last;
+            const unsigned bal = __ballot_sync(0xFFFFFFFFu, blend);
+            unsigned fix = 0;
+            if (kStats) fix = __reduce_add_sync(0xFFFFFFFFu, (unsigned)__float2uint_rn(wgt * kContribFix));
+            if (lane == jj[k]) { fixr = fix; cntr = (uint32_t)__popc(bal); }
+          }
+        }
+      } else
       while (todo) {
         const int jj = __ffs(todo) - 1;
         todo &= todo - 1;

@@ -116,6 +116,25 @@ def test_config2_shrunk_two_views():
         assert r["K"] > 4096 * 3
 
 
+def test_long_tile_lists_take_the_heavy_walk():
+    """Tiles whose lists exceed kFwdHeavyLen (raster_fwd.cu) take the several-survivors-per-iteration walk: thousands of large,
+    nearly transparent surfels over a ragged 40x24 image, so that every pixel blends of the order of a thousand pairs."""
+    sc = sg.random_scene(6000, 40, 24, 40.0, seed=21, sh_degree=1, scale_lo=0.2, scale_hi=0.5, op_mu=-4.0, op_sigma=0.5)
+    r = full_parity(sc, 0, dict(sh_degree=1, bg=(0.1, 0.2, 0.3)), max_fragile=0.08)
+    assert r["K"] > 6 * 2048
+    # the same walk with the depth moments (kMoments instance)
+    P, m = arrays(sc), sc.mask(0)
+    orc, cam, cfg, pre, srt, fw = oracle_view(P, sc.cameras[0], dict(sh_degree=1), mask=m)
+    g = GpuView(P, sc.cameras[0], dict(sh_degree=1))
+    g.preprocess(); g.bin_sort(want_ids=False)
+    gf = g.render_fwd(mask=m, moments=True)
+    ok = fw["fragile"] == 0
+    assert np.array_equal(gf["n_contrib"][ok], fw["n_contrib"][ok])
+    for i, k in enumerate(("origin", "m1", "m2")):
+        err = np.abs(gf["moments"][i] - fw[k]) / np.maximum(1.0, np.abs(fw[k]))
+        assert (err * ok).max() <= IMG_TOL, (k, (err * ok).max())
+
+
 def test_sh_degrees():
     sc = sg.random_scene(120, 48, 48, 40.0, seed=13, sh_degree=3)
     for deg in (0, 1, 2, 3):
