@@ -127,7 +127,8 @@ int launch_order_tiles(const Workspace& w, bool from_ranges, cudaStream_t st);
 // u32 selected by n_is_u64) and bounded by n_max for grid sizing. Result lands in (keysA, valsA) when the number of
 // passes is even, else in (keysB, valsB); returns that through *result_in_B.
 int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t* valsB, const void* n_ptr, bool n_is_u64,
-                     size_t n_max, int key_bits, uint32_t* status, uint32_t* ghist, bool* result_in_B, cudaStream_t st);
+                     size_t n_max, int key_bits, uint32_t* status, uint32_t* ghist, bool* result_in_B, cudaStream_t st,
+                     bool prepared = false);
 
 #ifdef __CUDACC__
 // MUFU approximations (1-2 ulp, flush-to-zero): enough for the 1e-4 / 1e-3 tolerances, no denormal fix-up code

@@ -64,7 +64,8 @@ __global__ void __launch_bounds__(kSortThreads) radix_hist_all_kernel(const uint
   }
 }
 
-__global__ void __launch_bounds__(kSortThreads) radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
+constexpr int kSortCtas = 3;  // resident blocks per SM the register budget is held to (80 registers; six passes at config 3: 200 us with 2, 178 with 3, 199 with 4)
+__global__ void __launch_bounds__(kSortThreads, kSortCtas) radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
                                                                       uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
                                                                       const void* n_ptr, bool n_is_u64, size_t n_cap, int shift, uint32_t mask,
                                                                       const uint32_t* __restrict__ ghist, uint32_t* status,
@@ -182,8 +183,11 @@ __global__ void __launch_bounds__(kSortThreads) radix_onesweep_kernel(const uint
   }  // next ticket
 }
 
+// `prepared`: the producer of the keys has already built the digit histograms in `ghist` and cleared the look-back state
+// (emit_keys_kernel does, for the tile sort); otherwise radix_hist_all_kernel reads the keys once to do both.
 int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t* valsB, const void* n_ptr, bool n_is_u64,
-                     size_t n_max, int key_bits, uint32_t* status, uint32_t* ghist, bool* result_in_B, cudaStream_t st) {
+                     size_t n_max, int key_bits, uint32_t* status, uint32_t* ghist, bool* result_in_B, cudaStream_t st,
+                     bool prepared) {
   static_assert(kSortThreads == kRadix, "one thread per digit");
   const int passes = (key_bits + kRadixBits - 1) / kRadixBits;
   const unsigned tiles_max = (unsigned)div_up(n_max, kSortTile);
@@ -192,16 +196,18 @@ int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t
   if (grid == 0 || passes == 0) { *result_in_B = false; return OCGS_OK; }
   if (passes > kMaxPasses || n_max > (size_t)kValMask) return OCGS_ERR_UNSUPPORTED;
   uint32_t* tickets = ghist + kMaxPasses * kRadix;
-  OCGS_CUDA_OK(cudaMemsetAsync(ghist, 0, (kMaxPasses * kRadix + kMaxPasses) * sizeof(uint32_t), st));
   const size_t stride = (size_t)tiles_max * kRadix;
-  radix_hist_all_kernel<<<grid, kSortThreads, 0, st>>>(keysA, n_ptr, n_is_u64, n_max, key_bits, passes, ghist, status, stride);
-  OCGS_LAUNCHED(st, "radix_hist_all_kernel");
+  if (!prepared) {
+    OCGS_CUDA_OK(cudaMemsetAsync(ghist, 0, (kMaxPasses * kRadix + kMaxPasses) * sizeof(uint32_t), st));
+    radix_hist_all_kernel<<<grid, kSortThreads, 0, st>>>(keysA, n_ptr, n_is_u64, n_max, key_bits, passes, ghist, status, stride);
+    OCGS_LAUNCHED(st, "radix_hist_all_kernel");
+  }
   uint32_t *kin = keysA, *vin = valsA, *kout = keysB, *vout = valsB;
   for (int p = 0; p < passes; ++p) {
     const int shift = p * kRadixBits;
     const int bits = min(kRadixBits, key_bits - shift);
     const uint32_t mask = (1u << bits) - 1u;
-    radix_onesweep_kernel<<<min(tiles_max, 148u * 2u), kSortThreads, 0, st>>>(kin, vin, kout, vout, n_ptr, n_is_u64, n_max, shift, mask, ghist + p * kRadix,
+    radix_onesweep_kernel<<<min(tiles_max, 148u * (unsigned)kSortCtas), kSortThreads, 0, st>>>(kin, vin, kout, vout, n_ptr, n_is_u64, n_max, shift, mask, ghist + p * kRadix,
                                                          status + (size_t)p * stride, tickets + p);
     OCGS_LAUNCHED(st, "radix_onesweep_kernel");
     uint32_t* t = kin; kin = kout; kout = t;
@@ -336,12 +342,26 @@ constexpr int kEmitTile = kEmitThreads * kEmitPerThread;  // 2048 keys -> at mos
 
 __global__ void __launch_bounds__(kEmitThreads) emit_keys_kernel(const ocgs_header* __restrict__ header, const uint32_t* __restrict__ offsets,
                                                                  const uint32_t* __restrict__ rank_to_id, const ushort4* __restrict__ rect,
-                                                                 int tiles_x, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+                                                                 int tiles_x, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals,
+                                                                 int passes, int key_bits, size_t key_capacity, uint32_t* __restrict__ ghist,
+                                                                 uint32_t* __restrict__ status, size_t status_stride) {
+  // look-back state of the sort tiles the tile sort will run over (also when the capacity overflowed: the passes still run)
+  {
+    const unsigned long long kc = min((unsigned long long)header->K, (unsigned long long)key_capacity);
+    for (unsigned t = blockIdx.x; t < (unsigned)div_up((size_t)kc, kSortTile); t += gridDim.x)
+      for (int p = 0; p < passes; ++p) status[(size_t)p * status_stride + (size_t)t * kRadix + threadIdx.x] = 0;
+  }
   if (header->error) return;
   const unsigned K = (unsigned)header->K;
   const unsigned n_vis = header->n_vis;
   __shared__ uint32_t s_off[kEmitTile + 2];
   __shared__ unsigned s_r0, s_r1;
+  // the tile sort's digit histograms (radix_sort_pairs, `prepared`) are built while the keys are still in registers
+  __shared__ uint32_t s_h[2][kRadix];
+  static_assert(kEmitThreads == kRadix, "one thread per digit");
+  s_h[0][threadIdx.x] = 0; s_h[1][threadIdx.x] = 0;
+  const int lane = threadIdx.x & 31;
+  const uint32_t mask1 = passes > 1 ? (1u << min(kRadixBits, key_bits - kRadixBits)) - 1u : 0u;
   for (unsigned k0 = blockIdx.x * kEmitTile; k0 < K; k0 += gridDim.x * kEmitTile) {
   const unsigned k1 = min(k0 + kEmitTile, K);
   __syncthreads();  // previous tile's s_off fully consumed
@@ -366,18 +386,40 @@ __global__ void __launch_bounds__(kEmitThreads) emit_keys_kernel(const ocgs_head
   const unsigned r0 = s_r0, cnt = s_r1 - s_r0 + 1;  // surfels r0 .. r0+cnt-1 own the keys of this block (cnt <= kEmitTile)
   for (unsigned i = threadIdx.x; i <= cnt; i += kEmitThreads) s_off[i] = offsets[r0 + i];
   __syncthreads();
-  for (unsigned k = k0 + threadIdx.x; k < k1; k += kEmitThreads) {
-    unsigned lo = 0, hi = cnt;
-    while (hi - lo > 1) { const unsigned mid = (lo + hi) >> 1; if (s_off[mid] <= k) lo = mid; else hi = mid; }
-    // skip surfels with zero tiles cannot happen: visible surfels touch >= 1 tile, so s_off is strictly increasing
-    const unsigned r = r0 + lo;
-    const unsigned local = k - s_off[lo];
-    const ushort4 rc = rect[rank_to_id[r]];
-    const unsigned tx0 = rc.x >> 4, ty0 = rc.y >> 4, wdt = (rc.z >> 4) + 1 - tx0;
-    const unsigned ty = ty0 + local / wdt, tx = tx0 + local % wdt;
-    keys[k] = ty * (unsigned)tiles_x + tx;
-    vals[k] = r;
+  for (unsigned kb = k0 + (threadIdx.x & ~31u); kb < k1; kb += kEmitThreads) {  // warp-uniform trip count
+    const unsigned k = kb + lane;
+    const bool valid = k < k1;
+    uint32_t key = 0;
+    if (valid) {
+      unsigned lo = 0, hi = cnt;
+      while (hi - lo > 1) { const unsigned mid = (lo + hi) >> 1; if (s_off[mid] <= k) lo = mid; else hi = mid; }
+      // skip surfels with zero tiles cannot happen: visible surfels touch >= 1 tile, so s_off is strictly increasing
+      const unsigned r = r0 + lo;
+      const unsigned local = k - s_off[lo];
+      const ushort4 rc = rect[rank_to_id[r]];
+      const unsigned tx0 = rc.x >> 4, ty0 = rc.y >> 4, wdt = (rc.z >> 4) + 1 - tx0;
+      const unsigned ty = ty0 + local / wdt, tx = tx0 + local % wdt;
+      key = ty * (unsigned)tiles_x + tx;
+      keys[k] = key;
+      vals[k] = r;
+      if (passes > 0) atomicAdd(&s_h[0][key & (kRadix - 1)], 1u);
+    }
+    if (passes > 1) {
+      // the high digit (tile row) is nearly constant across 32 consecutive keys: one add of 32 instead of 32 colliding adds
+      const uint32_t dg = (key >> kRadixBits) & mask1;
+      const uint32_t d0 = __shfl_sync(0xFFFFFFFFu, dg, 0);
+      if (__all_sync(0xFFFFFFFFu, valid && dg == d0)) {
+        if (lane == 0) atomicAdd(&s_h[1][d0], 32u);
+      } else if (valid) {
+        atomicAdd(&s_h[1][dg], 1u);
+      }
+    }
   }
+  }
+  __syncthreads();
+  for (int p = 0; p < min(passes, 2); ++p) {
+    const uint32_t c = s_h[p][threadIdx.x];
+    if (c) atomicAdd(&ghist[p * kRadix + threadIdx.x], c);
   }
 }
 
@@ -439,13 +481,17 @@ int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cu
   }
   const size_t cap = w.key_capacity;
   if (cap > 0 && n > 0) {
-    emit_keys_kernel<<<(unsigned)min(div_up(cap, kEmitTile), (size_t)148 * 8), kEmitThreads, 0, st>>>(w.header, w.offsets, w.rank_to_id, w.rect, cam.tiles_x,
-                                                                                w.tile_keys, w.tile_vals);
-    OCGS_LAUNCHED(st, "emit_keys_kernel");
     int bits = 1;
     while ((1 << bits) < w.n_tiles) ++bits;
+    const int passes = (bits + kRadixBits - 1) / kRadixBits;
+    const bool fused_hist = passes <= 2;  // emit_keys_kernel keeps two histograms (n_tiles <= 65536)
+    if (fused_hist) OCGS_CUDA_OK(cudaMemsetAsync(w.digit_total, 0, (kMaxPasses * kRadix + kMaxPasses) * sizeof(uint32_t), st));
+    emit_keys_kernel<<<(unsigned)min(div_up(cap, kEmitTile), (size_t)148 * 8), kEmitThreads, 0, st>>>(
+        w.header, w.offsets, w.rank_to_id, w.rect, cam.tiles_x, w.tile_keys, w.tile_vals, fused_hist ? passes : 0, bits, cap, w.digit_total, w.hist,
+        div_up(cap, kSortTile) * kRadix);
+    OCGS_LAUNCHED(st, "emit_keys_kernel");
     bool inB = false;
-    int rc = radix_sort_pairs(w.tile_keys, w.tile_vals, w.tkeyB, w.tvalB, &w.header->K, true, cap, bits, w.hist, w.digit_total, &inB, st);
+    int rc = radix_sort_pairs(w.tile_keys, w.tile_vals, w.tkeyB, w.tvalB, &w.header->K, true, cap, bits, w.hist, w.digit_total, &inB, st, fused_hist);
     if (rc != OCGS_OK) return rc;
     if (inB) {  // odd number of passes: bring the result back to the documented sections
       const unsigned g = (unsigned)min(div_up(cap, 1024), (size_t)148 * 8);
