@@ -121,7 +121,7 @@ int launch_photometric(const float* color, const float* target, const uint8_t* m
                        float* loss, void* scratch, cudaStream_t st);
 
 // tile_order <- tiles sorted by descending tile_work (bucketed; launch order of the raster CTAs)
-int launch_order_tiles(const Workspace& w, bool from_ranges, cudaStream_t st);
+int launch_order_tiles(const Workspace& w, bool from_ranges, cudaStream_t st, bool clear_grad_rec = false);
 
 // stable LSD radix sort of (u32 key, u32 value) pairs on bits [0, key_bits); count is read from the device (*n_ptr, u64 or
 // u32 selected by n_is_u64) and bounded by n_max for grid sizing. Result lands in (keysA, valsA) when the number of

@@ -411,10 +411,12 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
                       const float* gN, const float* mom, const float* gM1, const float* gM2, float* d_pos, float* d_scale, float* d_quat, float* d_opacity, float* d_sh,
                       float* d_center2d, cudaStream_t st) {
   if (s.n == 0) return OCGS_OK;
-  clear_grad_rec_kernel<<<(unsigned)min(div_up((size_t)s.n * 6, 256), (size_t)148 * 16), 256, 0, st>>>(w.header, (float4*)w.grad_rec);
-  OCGS_LAUNCHED(st, "clear_grad_rec_kernel");
-  if (w.n_tiles > 0) {
-    int rc = launch_order_tiles(w, /*from_ranges=*/false, st);  // tile_work = max n_contrib per tile, from the forward pass
+  if (w.n_tiles == 0) {
+    clear_grad_rec_kernel<<<(unsigned)min(div_up((size_t)s.n * 6, 256), (size_t)148 * 16), 256, 0, st>>>(w.header, (float4*)w.grad_rec);
+    OCGS_LAUNCHED(st, "clear_grad_rec_kernel");
+  } else {
+    // tile_work = length of each tile's blended list, from the forward pass; the same launch clears grad_rec
+    int rc = launch_order_tiles(w, /*from_ranges=*/false, st, /*clear_grad_rec=*/true);
     if (rc != OCGS_OK) return rc;
     const float goh = mask ? (float)((double)cfg.gamma_bg / ((double)cam.W * (double)cam.H)) : 0.f;
     if (mom && gM1 && gM2)

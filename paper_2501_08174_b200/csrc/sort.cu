@@ -515,8 +515,16 @@ int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cu
 // ---- launch order of the raster CTAs: heavy tiles first (longest-processing-time-first keeps the tail short) -----------
 namespace ocgs {
 
+// Blocks 1.. of the grid (backward pass only) clear the record-gradient accumulator, which is indexed by depth rank: only
+// its first n_vis rows are ever touched.  One launch instead of two short dependent ones in front of render_bwd_kernel.
 __global__ void __launch_bounds__(1024) order_tiles_kernel(const uint32_t* __restrict__ ranges, uint32_t* __restrict__ work, int n_tiles,
-                                                           bool from_ranges, uint32_t* __restrict__ order) {
+                                                           bool from_ranges, uint32_t* __restrict__ order,
+                                                           const ocgs_header* __restrict__ header, float4* __restrict__ grad_rec) {
+  if (blockIdx.x > 0) {
+    const size_t n4 = (size_t)header->n_vis * (kRec / 4);
+    for (size_t i = (size_t)(blockIdx.x - 1) * 1024 + threadIdx.x; i < n4; i += (size_t)(gridDim.x - 1) * 1024) grad_rec[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    return;
+  }
   constexpr int kBuckets = 1024;
   __shared__ uint32_t s_cnt[kBuckets];
   __shared__ uint32_t s_warp[32];
@@ -539,10 +547,10 @@ __global__ void __launch_bounds__(1024) order_tiles_kernel(const uint32_t* __res
     s_maxw = m;
   }
   __syncthreads();
-  const unsigned long long maxw = (unsigned long long)s_maxw + 1ull;
-  // bucket 0 = heaviest
+  // bucket 0 = heaviest; any monotone map of the work onto the buckets will do (a float scale instead of a 64-bit division)
+  const float scale = (float)kBuckets / ((float)s_maxw + 1.0f);
   for (int t = tid; t < n_tiles; t += 1024) {
-    const uint32_t b = (kBuckets - 1) - (uint32_t)(((unsigned long long)work[t] * kBuckets) / maxw);
+    const uint32_t b = (kBuckets - 1) - min((uint32_t)(kBuckets - 1), (uint32_t)((float)work[t] * scale));
     atomicAdd(&s_cnt[b], 1u);
   }
   __syncthreads();
@@ -569,14 +577,15 @@ __global__ void __launch_bounds__(1024) order_tiles_kernel(const uint32_t* __res
   s_cnt[tid] = (wid ? s_warp[wid - 1] : 0) + inc - c;
   __syncthreads();
   for (int t = tid; t < n_tiles; t += 1024) {
-    const uint32_t b = (kBuckets - 1) - (uint32_t)(((unsigned long long)work[t] * kBuckets) / maxw);
+    const uint32_t b = (kBuckets - 1) - min((uint32_t)(kBuckets - 1), (uint32_t)((float)work[t] * scale));
     order[atomicAdd(&s_cnt[b], 1u)] = (uint32_t)t;
   }
 }
 
-int launch_order_tiles(const Workspace& w, bool from_ranges, cudaStream_t st) {
+int launch_order_tiles(const Workspace& w, bool from_ranges, cudaStream_t st, bool clear_grad_rec) {
   if (w.n_tiles == 0) return OCGS_OK;
-  order_tiles_kernel<<<1, 1024, 0, st>>>(w.ranges, w.tile_work, w.n_tiles, from_ranges, w.tile_order);
+  const unsigned clear_blocks = clear_grad_rec ? (unsigned)min(div_up((size_t)w.n * (kRec / 4), 1024), (size_t)148 * 2) : 0u;
+  order_tiles_kernel<<<1 + clear_blocks, 1024, 0, st>>>(w.ranges, w.tile_work, w.n_tiles, from_ranges, w.tile_order, w.header, (float4*)w.grad_rec);
   OCGS_LAUNCHED(st, "order_tiles_kernel");
   return OCGS_OK;
 }
