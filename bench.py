@@ -464,7 +464,7 @@ def run_ours(args):
                     "traffic": NCU_TRAFFIC.get(name), "traffic_source": NCU_TRAFFIC_SOURCE,
                     "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)", "algorithmic": what}
         per_launch = {"radix_onesweep_kernel": 16.0 * (4 * n + 2 * K) / 6.0,  # 8 B read + 8 B written per key; 4 passes over N, 2 over K
-                      "radix_hist_all_kernel": 4.0 * (n + K) / 2.0, "emit_keys_kernel": 8.0 * K + 12.0 * nvis,
+                      "radix_hist_all_kernel": 4.0 * n, "emit_keys_kernel": 8.0 * K + 12.0 * nvis,  # the tile sort's histograms are built by emit_keys_kernel
                       "preprocess_kernel": 61.0 * n + 296.0 * nvis, "project_bwd_kernel": 232.0 * n + 328.0 * nvis,
                       "reorder_kernel": 208.0 * nvis, "clear_grad_rec_kernel": 96.0 * nvis, "tile_ranges_kernel": 4.0 * K,
                       "masked_l1_kernel": 25.0 * W * H, "ssim_terms_kernel": 63.0 * W * H, "ssim_grad_kernel": 75.0 * W * H,
