@@ -248,7 +248,11 @@ inline void cross3(const double* a, const double* b, double* o) {
 }
 inline uint32_t float_bits(float f) { uint32_t u; std::memcpy(&u, &f, 4); return u; }
 
-// colour (S14): rgb = max(0, 1/2 + sum_k Y_k(dir) sh_k), dir = normalise(p - cam_pos); clamp bit c set when channel c is clamped
+// colour (S14): rgb = max(0, 1/2 + sum_k Y_k(dir) sh_k), dir = normalise(p - cam_pos); clamp bit c set when channel c is clamped.
+// Bit 4 + c marks the decision of channel c as FRAGILE (S22, extended to the colour clamp): the unclamped value lies within
+// kClampMargin of zero, closer than an fp32 evaluation of the 16-term sum can resolve, so a kernel that takes the decision in
+// fp32 may take the other branch; tests compare the clamp bit and the gradients of such a surfel only where it is clear.
+constexpr double kClampMargin = 4e-6;
 void surfel_colour(const float* p, const float* sh, int degree, const double* campos, double* rgb, uint8_t* clamp) {
   double v[3] = {p[0] - campos[0], p[1] - campos[1], p[2] - campos[2]};
   const double len = std::sqrt(dot3(v, v));
@@ -260,6 +264,7 @@ void surfel_colour(const float* p, const float* sh, int degree, const double* ca
   for (int c = 0; c < 3; ++c) {
     double acc = 0.5;
     for (int k = 0; k < nb; ++k) acc += Y[k] * (double)sh[3 * k + c];
+    if (std::fabs(acc) <= kClampMargin) *clamp |= (uint8_t)(1u << (4 + c));
     if (acc < 0.0) { acc = 0.0; *clamp |= (uint8_t)(1u << c); }
     rgb[c] = acc;
   }

@@ -116,7 +116,7 @@ def oracle_view(scene_arrays, cam_np, cfg_kw, mask=None):
 GROUPS = ("d_pos", "d_scale", "d_quat", "d_opacity", "d_sh", "d_center2d")
 
 
-def check_grads(gpu, ora, rel=1e-3, floor=1e-6, sum_eps=1e-5, floor_frac=None):
+def check_grads(gpu, ora, rel=1e-3, floor=1e-6, sum_eps=1e-5, floor_frac=None, skip_rows=None):
     """Gradient parity rule (north_star: relative error 1e-3 on entries above 1e-6).
 
     An entry passes when |gpu - oracle| <= rel*|oracle| + floor, or -- for entries that are small because the fp32 sum
@@ -125,13 +125,17 @@ def check_grads(gpu, ora, rel=1e-3, floor=1e-6, sum_eps=1e-5, floor_frac=None):
     per array, the number of entries, the number passing the strict per-entry rule and the worst block-relative error;
     raises AssertionError naming the first failing array.  floor_frac (optional): the absolute floor of each array is
     raised to floor_frac x the 99th percentile of its per-surfel block scales (for upstream gradients whose per-pair terms
-    are differences of nearly equal fp32 depths: their absolute noise is set by the depth, not by the entry)."""
+    are differences of nearly equal fp32 depths: their absolute noise is set by the depth, not by the entry).
+    skip_rows (optional, bool per surfel): surfels left out of the comparison -- those whose colour clamp decision is fragile
+    (oracle preprocess 'clamp_fragile'): the two sides may legitimately sit on different sides of max(0, .)."""
     report = {}
     floor0 = floor
     for k in GROUPS:
         a = gpu[k].astype(np.float64).reshape(gpu[k].shape[0], -1)
         b = ora[k].reshape(a.shape)
         err = np.abs(a - b)
+        if skip_rows is not None:
+            err[np.asarray(skip_rows, bool)] = 0.0
         floor = floor0
         if floor_frac is not None and a.size:
             bs = np.abs(b).max(1)

@@ -34,7 +34,7 @@ def windows_parity(sc, view, windows, key_capacity, rng_seed=11):
     gp = g.preprocess()
     vis = pre["visible"] == 1
     assert np.array_equal(gp["tiles"], pre["tiles_touched"]) and np.array_equal(gp["depth_bits"], pre["depth_bits"])
-    assert np.array_equal(gp["rect"][vis], pre["rect"][vis]) and np.array_equal(gp["clamp"][vis], pre["clamp"][vis])
+    assert np.array_equal(gp["rect"][vis], pre["rect"][vis]) and orc.clamp_matches(gp["clamp"], pre, vis)
     gs = g.bin_sort()
     assert gs["error"] == 0 and gs["K"] == srt["K"] and gs["n_vis"] == int(vis.sum())
     assert np.array_equal(gs["ids"], srt["ids"]) and np.array_equal(gs["ranges"], srt["ranges"])
@@ -70,7 +70,7 @@ def windows_parity(sc, view, windows, key_capacity, rng_seed=11):
                               gD=gD.astype(np.float32), gN=gN.astype(np.float32), window=w)
         for k in og:
             og[k] += part[k]
-    rep = check_grads(gg, og)
+    rep = check_grads(gg, og, skip_rows=pre["clamp_fragile"] != 0)
     return dict(K=srt["K"], n_vis=int(vis.sum()), grads=rep, ranges=srt["ranges"])
 
 
@@ -146,3 +146,15 @@ def test_config4_full_size_all_views_prune():
           (pm[interior].mean(), pm[shell].mean(), pm[sc.group == 1].mean(), k, n))
     assert pm[interior].mean() > 0.97
     assert pm[shell].mean() < 0.5
+
+
+def test_more_than_2_pow_24_keys():
+    """Config 3's geometry with four times its surfels (4 M; one view): 19 M (tile, surfel) keys -- more than 2^24, so that no
+    index anywhere on the path can hide in 24 bits or in an fp32 mantissa -- and mean tile lists of ~2 500 entries, so that
+    most tiles take the long-list walk of the forward kernel.  Integer outputs in full, maps and gradients on three windows."""
+    sc = sg.make_scene("config3", n_obj=1_200_000, n_bg=2_800_000, n_views=2)
+    W, H = 1600, 1200
+    windows = [(776, 576, 808, 608), (0, 0, 32, 32), (W - 32, H - 32, W, H)]
+    r = windows_parity(sc, 1, windows, key_capacity=12 * sc.n)
+    L = r["ranges"][:, 1] - r["ranges"][:, 0]
+    assert r["K"] > (1 << 24) and np.median(L) > 2048

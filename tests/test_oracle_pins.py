@@ -56,6 +56,26 @@ def test_sh_sign_convention_degree1():
     assert Y[1] == pytest.approx(-c1)
 
 
+def test_colour_clamp_and_its_fragile_margin():
+    """S14 / S22: channel c is clamped iff 1/2 + sum Y sh < 0; the decision is marked fragile iff that value lies within 4e-6
+    of zero (what an fp32 evaluation cannot resolve).  Degree 0: the value is the requested rgb up to the fp32 rounding of sh."""
+    cam = ident_cam(32, 32, 50.0)
+    cfg = orc.default_config(sh_degree=0)
+    rgbs = [(-1e-3, 1e-3, 0.5), (-1e-6, 1e-6, -0.2), (0.0, -3e-6, 3e-6), (-1e-5, 1e-5, 2.0)]
+    s = stack(*[one_surfel((0, 0, 2.0), (0.1, 0.1), rgb=c) for c in rgbs])
+    pre = orc.preprocess(*s, cam, cfg)
+    assert list(pre["clamp"]) == [0b001, 0b101, int(pre["clamp"][2]) & 0b001 | 0b010, 0b001]
+    assert list(pre["clamp_fragile"]) == [0b000, 0b011, 0b111, 0b000]
+    assert np.all(pre["rgb"] >= 0.0) and np.allclose(pre["rgb"][0], [0.0, 1e-3, 0.5], atol=1e-7)
+    # clamp_matches: a disagreement counts only on channels whose decision is clear
+    other = pre["clamp"].copy(); other[1] ^= 0b011
+    assert orc.clamp_matches(other, pre)
+    other[1] ^= 0b100
+    assert not orc.clamp_matches(other, pre)
+    other = pre["clamp"].copy(); other[0] ^= 0b001
+    assert not orc.clamp_matches(other, pre) and orc.clamp_matches(other, pre, rows=np.array([False, True, True, True]))
+
+
 # ---------------------------------------------------------------------------------------------
 # north_star: "a single fronto-parallel surfel gives an analytic Gaussian footprint"
 # ---------------------------------------------------------------------------------------------
