@@ -158,3 +158,14 @@ def test_more_than_2_pow_24_keys():
     r = windows_parity(sc, 1, windows, key_capacity=12 * sc.n)
     L = r["ranges"][:, 1] - r["ranges"][:, 0]
     assert r["K"] > (1 << 24) and np.median(L) > 2048
+
+
+def test_more_than_2_pow_17_tiles_three_tile_sort_passes():
+    """8192 x 4112 pixels = 512 x 257 = 131 584 tiles: tile ids need 18 bits, so the tile sort takes three radix passes (an odd
+    number: the result is copied back from the alternate buffers) and its histograms come from radix_hist_all_kernel instead
+    of emit_keys_kernel's two; pixel coordinates up to 8191 in the packed rects.  Integers in full, maps on windows."""
+    W, H = 8192, 4112
+    sc = sg.random_scene(60_000, W, H, 6000.0, seed=31, sh_degree=1, scale_lo=0.003, scale_hi=0.03)
+    windows = [(0, 0, 32, 32), (W - 32, H - 32, W, H), (4080, 2040, 4112, 2072), (W - 40, 0, W, 24)]
+    r = windows_parity(sc, 0, windows, key_capacity=12_000_000)
+    assert r["ranges"].shape[0] == 512 * 257 and r["K"] > 5_000_000
