@@ -260,60 +260,46 @@ __global__ void __launch_bounds__(kScanBlock) reorder_kernel(const uint32_t* __r
   }
 }
 
-// single block: exclusive scan of the block sums (64-bit running total), K, capacity check
-__global__ void __launch_bounds__(1024) scan_blocksums_kernel(uint32_t* __restrict__ blocksum, ocgs_header* __restrict__ header,
-                                                              size_t key_capacity, uint32_t* __restrict__ offsets) {
+// Offsets = exclusive scan of tiles-touched in rank order.  Every block sums the block sums in front of it itself (at most
+// n_vis / 1024 values: one load per thread), so no separate scan of the block sums is launched; block 0 also totals all of
+// them: K (64-bit), the capacity check and the closing entry offsets[n_vis].
+__global__ void __launch_bounds__(kScanBlock) scan_apply_kernel(const uint32_t* __restrict__ tcount, const uint32_t* __restrict__ blocksum,
+                                                                ocgs_header* __restrict__ header, size_t key_capacity,
+                                                                uint32_t* __restrict__ offsets) {
   const unsigned n_vis = header->n_vis;
   const unsigned nb = (unsigned)div_up((size_t)n_vis, kScanBlock);
-  __shared__ unsigned long long warp_sums[32];
-  __shared__ unsigned long long carry;
-  if (threadIdx.x == 0) carry = 0;
-  __syncthreads();
+  if (blockIdx.x > 0 && blockIdx.x >= nb) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  for (unsigned base = 0; base < nb; base += 1024) {
-    const unsigned i = base + threadIdx.x;
-    const unsigned long long v = i < nb ? blocksum[i] : 0;
-    unsigned long long inc = v;
+  __shared__ unsigned long long wsum[32];
+  __shared__ uint32_t ws[32];
+  __shared__ unsigned long long s_pre;
+  unsigned long long part = 0;
+  const unsigned upto = blockIdx.x == 0 ? nb : blockIdx.x;  // block 0: the total; block b: the sums in front of it
+  for (unsigned i = threadIdx.x; i < upto; i += kScanBlock) part += blocksum[i];
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
-      if (lane >= o) inc += t;
-    }
-    if (lane == 31) warp_sums[wid] = inc;
-    __syncthreads();
-    if (wid == 0) {
-      unsigned long long w = warp_sums[lane];
+  for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xFFFFFFFFu, part, o);
+  if (lane == 0) wsum[wid] = part;
+  __syncthreads();
+  if (wid == 0) {
+    unsigned long long w = wsum[lane];
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, w, o);
-        if (lane >= o) w += t;
-      }
-      warp_sums[lane] = w;
+    for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xFFFFFFFFu, w, o);
+    if (lane == 0) s_pre = w;
+  }
+  __syncthreads();
+  unsigned long long pre = s_pre;
+  if (blockIdx.x == 0) {
+    if (threadIdx.x == 0) {
+      const unsigned long long K = pre;
+      header->K = K;
+      if (K > (unsigned long long)key_capacity || K > 0xFFFFFFF0ull) header->error |= 1u;
+      offsets[n_vis] = (uint32_t)min(K, 0xFFFFFFFFull);
     }
-    __syncthreads();
-    const unsigned long long c = carry;
-    const unsigned long long ex = c + (wid ? warp_sums[wid - 1] : 0) + inc - v;
-    if (i < nb) blocksum[i] = (uint32_t)min(ex, 0xFFFFFFFFull);
-    __syncthreads();
-    if (threadIdx.x == 0) carry = c + warp_sums[31];
-    __syncthreads();
+    pre = 0;
+    if (nb == 0) return;
   }
-  if (threadIdx.x == 0) {
-    const unsigned long long K = carry;
-    header->K = K;
-    if (K > (unsigned long long)key_capacity || K > 0xFFFFFFF0ull) header->error |= 1u;
-    offsets[n_vis] = (uint32_t)min(K, 0xFFFFFFFFull);
-  }
-}
-
-__global__ void __launch_bounds__(kScanBlock) scan_apply_kernel(const uint32_t* __restrict__ tcount, const uint32_t* __restrict__ blocksum,
-                                                                const ocgs_header* __restrict__ header, uint32_t* __restrict__ offsets) {
-  const unsigned n_vis = header->n_vis;
-  if (blockIdx.x * kScanBlock >= n_vis) return;
   const unsigned r = blockIdx.x * kScanBlock + threadIdx.x;
   const uint32_t v = r < n_vis ? tcount[r] : 0;
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  __shared__ uint32_t ws[32];
   uint32_t inc = v;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
@@ -332,7 +318,7 @@ __global__ void __launch_bounds__(kScanBlock) scan_apply_kernel(const uint32_t* 
     ws[lane] = w;
   }
   __syncthreads();
-  if (r < n_vis) offsets[r] = blocksum[blockIdx.x] + (wid ? ws[wid - 1] : 0) + inc - v;
+  if (r < n_vis) offsets[r] = (uint32_t)min(pre, 0xFFFFFFFFull) + (wid ? ws[wid - 1] : 0) + inc - v;
 }
 
 // ---- key emission: one thread per key, the owning surfel found by binary search in a shared slice of `offsets` -----
@@ -473,12 +459,8 @@ int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cu
                                                 w.tcount, w.blocksum);
     OCGS_LAUNCHED(st, "reorder_kernel");
   }
-  scan_blocksums_kernel<<<1, 1024, 0, st>>>(w.blocksum, w.header, w.key_capacity, w.offsets);
-  OCGS_LAUNCHED(st, "scan_blocksums_kernel");
-  if (n > 0) {
-    scan_apply_kernel<<<nblk, kScanBlock, 0, st>>>(w.tcount, w.blocksum, w.header, w.offsets);
-    OCGS_LAUNCHED(st, "scan_apply_kernel");
-  }
+  scan_apply_kernel<<<nblk, kScanBlock, 0, st>>>(w.tcount, w.blocksum, w.header, w.key_capacity, w.offsets);
+  OCGS_LAUNCHED(st, "scan_apply_kernel");
   const size_t cap = w.key_capacity;
   if (cap > 0 && n > 0) {
     int bits = 1;
