@@ -9,7 +9,7 @@
  *  - "device" pointers are CUDA device memory owned by the caller; "host" pointers are ordinary host memory.
  *    The library allocates no device memory, keeps no global state and is re-entrant per stream.
  *  - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream).  No entry point
- *    synchronises except ocgs_check(), ocgs_step_view_host() and ocgs_step_host().  A step can therefore be captured in a CUDA graph.
+ *    synchronises except ocgs_check(), ocgs_profile_end(), ocgs_step_view_host() and ocgs_step_host().  A step can therefore be captured in a CUDA graph.
  *  - The data-dependent key count K never travels to the host inside a step: kernels read it from the workspace
  *    header.  If K exceeds `key_capacity` the header error flag is set, later calls of the step become no-ops, and
  *    ocgs_check() reports OCGS_ERR_CAPACITY with the needed size.  Limits: N and key_capacity below 2^30 (the radix
@@ -299,6 +299,17 @@ int ocgs_step_view_host(const ocgs_surfels* surfels, const ocgs_camera* cam, con
                         float* d_grad_pos, float* d_grad_scale, float* d_grad_quat, float* d_grad_opacity, float* d_grad_sh,
                         uint32_t* d_vis_count, float* d_contrib_sum, float* d_losses, void* ws, size_t key_capacity, void* stream,
                         void* copy_stream);
+/* The same step WITHOUT the closing synchronisation: everything, including the copy of the two loss scalars into h_losses and
+ * (if h_header is not NULL) of the workspace header into *h_header, is only enqueued; the caller synchronises `stream` and
+ * then reads h_losses and checks h_header->error (bit 0: K > key_capacity, bit 1: a tile list over 2^24 entries).  h_mask,
+ * h_target, h_losses and h_header must be page-locked.  The call contains no synchronising operation, so it can be
+ * captured into a CUDA graph (cudaStreamBeginCapture on `stream`; copy_stream joins the capture through events) and the
+ * graph replayed once per iteration for the same view: the uploads are memcpy nodes and happen on every replay. */
+int ocgs_step_view_host_enqueue(const ocgs_surfels* surfels, const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask,
+                                const float* h_target, float* h_losses, ocgs_header* h_header, uint8_t* d_mask, float* d_images,
+                                uint32_t* d_ncontrib, float* d_grad_pos, float* d_grad_scale, float* d_grad_quat, float* d_grad_opacity,
+                                float* d_grad_sh, uint32_t* d_vis_count, float* d_contrib_sum, float* d_losses, void* ws,
+                                size_t key_capacity, void* stream, void* copy_stream);
 
 /* ---- end-to-end step with HOST parameters (bench.py "e2e_host_params") ---------------------------------------------------------------
  * Copies the surfel parameters, mask and target image from (pinned) host memory to the given device staging buffers,

@@ -360,6 +360,18 @@ int ocgs_step_view_host(const ocgs_surfels* surfels, const ocgs_camera* cam, con
                         float* d_grad_pos, float* d_grad_scale, float* d_grad_quat, float* d_grad_opacity, float* d_grad_sh,
                         uint32_t* d_vis_count, float* d_contrib_sum, float* d_losses, void* ws, size_t key_capacity, void* stream,
                         void* copy_stream) {
+  int rc = ocgs_step_view_host_enqueue(surfels, cam, cfg, h_mask, h_target, h_losses, nullptr, d_mask, d_images, d_ncontrib, d_grad_pos,
+                                       d_grad_scale, d_grad_quat, d_grad_opacity, d_grad_sh, d_vis_count, d_contrib_sum, d_losses, ws,
+                                       key_capacity, stream, copy_stream);
+  if (rc != OCGS_OK) { cudaStreamSynchronize((cudaStream_t)stream); return rc; }
+  return ocgs_check(ws, stream, nullptr);
+}
+
+int ocgs_step_view_host_enqueue(const ocgs_surfels* surfels, const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask,
+                                const float* h_target, float* h_losses, ocgs_header* h_header, uint8_t* d_mask, float* d_images,
+                                uint32_t* d_ncontrib, float* d_grad_pos, float* d_grad_scale, float* d_grad_quat, float* d_grad_opacity,
+                                float* d_grad_sh, uint32_t* d_vis_count, float* d_contrib_sum, float* d_losses, void* ws,
+                                size_t key_capacity, void* stream, void* copy_stream) {
   if (!surfels || !cam || !cfg || !h_mask || !h_target || !h_losses || !d_mask || !d_images || !d_ncontrib || !d_losses || !ws)
     return OCGS_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
@@ -398,10 +410,11 @@ int ocgs_step_view_host(const ocgs_surfels* surfels, const ocgs_camera* cam, con
     if ((rc = ocgs_render_bwd(surfels, cam, cfg, ws, key_capacity, d_mask, d_ncontrib, gC, nullptr, nullptr, nullptr, d_grad_pos, d_grad_scale,
                               d_grad_quat, d_grad_opacity, d_grad_sh, nullptr, stream)) != OCGS_OK) break;
     if (cudaMemcpyAsync(h_losses, d_losses, 2 * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
-    rc = ocgs_check(ws, stream, nullptr);
+    if (h_header && cudaMemcpyAsync(h_header, ws, sizeof(ocgs_header), cudaMemcpyDeviceToHost, st) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
   } while (false);
   if (overlap) {
-    if (rc != OCGS_OK) cudaStreamSynchronize(cs);
+    // a failed call must not leave the copy stream dangling off a capture or racing the caller's buffers: join it
+    if (rc != OCGS_OK) cudaStreamWaitEvent(st, ev_target, 0);
     cudaEventDestroy(ev_begin); cudaEventDestroy(ev_mask); cudaEventDestroy(ev_target);
   }
   return rc;

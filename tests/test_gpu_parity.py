@@ -223,7 +223,8 @@ def test_masked_l1_and_host_step_match_device_path():
     camn = sc.cameras[1]
     m = sc.mask(1)
     g = GpuView(arrays(sc), camn, dict(sh_degree=3))
-    g.preprocess(); g.bin_sort()
+    g.preprocess()
+    gs_nvis = g.bin_sort()["n_vis"]
     gf = g.render_fwd(mask=m)
     rng = np.random.default_rng(0)
     target = rng.uniform(0, 1, (3, 240, 320)).astype(np.float32)
@@ -281,3 +282,31 @@ def test_masked_l1_and_host_step_match_device_path():
             a, b = grads[name].cpu().numpy().ravel(), gg[name].ravel()
             assert np.allclose(a, b, rtol=2e-3, atol=1e-6 + 1e-4 * np.abs(b).max()), name
         assert np.array_equal(vis2.cpu().numpy().view(np.uint32), gf["vis_count"])
+    # the same step enqueued without synchronisation and captured into a CUDA graph (ocgs_step_view_host_enqueue): every
+    # replay uploads the view's data again, so changing the pinned target between replays must change the result
+    h_mask, h_target = torch.tensor(m).pin_memory(), torch.tensor(target).pin_memory()
+    h_header = torch.zeros(4, dtype=torch.int32).pin_memory()
+    main, side = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=main):
+        B.ocgs_step_view_host_enqueue(g.surfels, g.cam, g.cfg, h_mask, h_target, h_losses, h_header, d_mask, d_images, d_nc, grads, vis2,
+                                      cs2, d_losses, g.ws, g.cap, stream=main, copy_stream=side)
+    for rep in range(2):
+        vis2.zero_(); cs2.zero_(); h_losses.zero_(); h_header.fill_(-1)
+        for name in grads:
+            grads[name].fill_(7.0)
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert int(h_header[3]) == 0 and int(h_header[2]) == gs_nvis
+        assert float(h_losses[0]) == gf["loss_bg"]
+        if rep == 0:
+            assert abs(float(h_losses[1]) - float(loss.item())) < 1e-7
+            for name in ("d_pos", "d_scale", "d_quat", "d_opacity", "d_sh"):
+                a, b = grads[name].cpu().numpy().ravel(), gg[name].ravel()
+                assert np.allclose(a, b, rtol=2e-3, atol=1e-6 + 1e-4 * np.abs(b).max()), name
+            assert np.array_equal(vis2.cpu().numpy().view(np.uint32), gf["vis_count"])
+            h_target.add_(0.25)  # the next replay must see the new host data
+        else:
+            assert float(h_losses[1]) > float(loss.item()) + 0.01
