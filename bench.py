@@ -279,7 +279,7 @@ def run_ours(args):
 
     # ---- timed region 1 (`value`): K steps, CUDA events on the launching stream -------------------------------------
     # The step keeps every count on the device (no host sync), so it is captured once per view into a CUDA graph and
-    # replayed (--no-graph launches the ~28 kernels directly).  Per-launch events are NOT recorded here: an event after
+    # replayed (--no-graph launches the 18 kernels directly).  Per-launch events are NOT recorded here: an event after
     # every kernel costs ~0.17 ms per step of idle gaps; the per-kernel breakdown comes from region 2 below.
     graphs = None
     if not args.no_graph:
