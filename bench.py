@@ -360,6 +360,55 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_total = float(t.item())
 
+    # ---- visibility pass ("rendering all training views" for the pruning statistics), timed separately ------
+    # (a) through the full forward pass (preprocess + bin_sort + render_fwd with the statistics on), (b) through
+    # ocgs_visibility_pass (no SH colour, no maps, no blended lists); direct launches, CUDA events, nv views x reps
+    vis_pass = None
+    if rank == 0 and not args.no_prune:
+        vis_b = torch.zeros_like(vis); cs_b = torch.zeros_like(cs)
+        reps = max(1, min(args.steps, 20) // nv)
+
+        def full_fwd(i):
+            B.ocgs_preprocess(surfels, cam_c[i], cfg, ws, cap)
+            B.ocgs_bin_sort(n, cam_c[i], cfg, ws, cap)
+            B.ocgs_render_fwd(n, cam_c[i], cfg, ws, cap, None, out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"],
+                              None, vis_b, cs_b)
+
+        def stats_only(i):
+            B.ocgs_visibility_pass(surfels, cam_c[i], cfg, ws, cap, vis_b, cs_b)
+        res = {}
+        for name, fn in (("full_forward", full_fwd), ("visibility_pass", stats_only)):
+            for i in range(nv):
+                fn(i)
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a0.record()
+            for _ in range(reps):
+                for i in range(nv):
+                    fn(i)
+            a1.record()
+            torch.cuda.synchronize()
+            res[name] = a0.elapsed_time(a1) / (reps * nv)
+        B.ocgs_check(ws)
+        # (c) the same pass with two views in flight (two workspaces, two streams): pruning.accumulate_visibility(ws2=...)
+        from paper_2501_08174_b200 import pruning
+        ws_b = B.alloc_workspace(n, W, H, cap, device=dev)
+        cams_rep = [cam_c[i] for _ in range(reps) for i in range(nv)]
+        pruning.accumulate_visibility(surfels, n, cams_rep[:nv], cfg, ws, cap, None, vis_b, cs_b, ws2=ws_b)
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a0.record()
+        pruning.accumulate_visibility(surfels, n, cams_rep, cfg, ws, cap, None, vis_b, cs_b, ws2=ws_b)
+        a1.record()
+        torch.cuda.synchronize()
+        res["two_streams"] = a0.elapsed_time(a1) / len(cams_rep)
+        del ws_b
+        vis_pass = {"ms_per_view_full_forward": res["full_forward"], "ms_per_view": res["visibility_pass"],
+                    "ms_per_view_two_streams": res["two_streams"], "views": nv, "reps": reps,
+                    "what": "statistics of one view: preprocess + bin_sort + forward walk; ocgs_visibility_pass skips the SH colour, "
+                            "the maps and the blended lists"}
+        del vis_b, cs_b
+
     # ---- prune pass, timed separately: once per pruning interval, not per step -------------------
     # statistics of the nv views just rendered -> mask -> scan -> stable compaction of all five parameter arrays
     prune = None
@@ -539,6 +588,7 @@ def run_ours(args):
                                      "(those events cost idle gaps, so `value` comes from the region without them)",
                               "ms_per_step_with_events": ms_marked / steps}}
     line["prune"] = prune
+    line["visibility_pass"] = vis_pass
     if e2e:
         line["e2e"] = e2e
         line["e2e_host_params"] = e2e_hp

@@ -222,6 +222,21 @@ int ocgs3d_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, voi
                       float* color, float* alpha, float* depth, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,
                       float* contrib_sum, void* stream);
 
+/* ---- the visibility pass: statistics of one view, nothing else --------------------------------------------------------
+ * PAPER.md:129 / :219 / :234: the pruning statistics come from "rendering all training views"; PAPER.md:119 defines what
+ * is counted (a pair counts iff G_j is actually blended into the pixel, in front-to-back order, before the pixel stops).
+ * ocgs_visibility_pass = (1) without the SH colour and the normal (surfels->sh is not read and may be NULL), (2), and the
+ * walk of (3) without the colour / depth / normal blends, the maps, L_b and the blended lists: for every surfel j
+ *   vis_count[j]   += number of pixels that blended it,      contrib_sum[j] += sum over those pixels of alpha_ij T_ij
+ * exactly as ocgs_render_fwd accumulates them (vis_count bit-identical; contrib_sum up to the order of float atomics).
+ * The workspace afterwards holds this view's lists but NO blended lists: do not call ocgs_render_bwd on it.
+ * ocgs3d_visibility_pass: the same for 3D Gaussians (Appendix B).
+ * vis_count u32[N], contrib_sum f32[N]: device, ACCUMULATED into.  Asynchronous on `stream`; errors as (1)-(3). */
+int ocgs_visibility_pass(const ocgs_surfels* surfels, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
+                         uint32_t* vis_count, float* contrib_sum, void* stream);
+int ocgs3d_visibility_pass(const ocgs_gaussians3d* gaussians, const ocgs_camera* cam, const ocgs_config* cfg, void* ws,
+                           size_t key_capacity, uint32_t* vis_count, float* contrib_sum, void* stream);
+
 /* ---- (5) prune statistics -> mask -> stream compaction ----------------------------------------------------------------
  * "We propose to assign both G_j and G_k with false" -- a surfel that was never blended in any render
  * of the interval is removed whether it was outside the frustum or occluded; PAPER.md:101 (opacity threshold), S17.

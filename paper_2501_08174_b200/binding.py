@@ -18,7 +18,7 @@ _LIB_PATH = os.path.join(_HERE, "csrc", "libocgs.so")
 OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
            "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_render_fwd_l1", "ocgs_render_fwd_reg", "ocgs_render_bwd_reg", "ocgs3d_preprocess", "ocgs3d_render_fwd", "ocgs_prune_workspace_bytes",
-           "ocgs_prune_stats", "ocgs_compact_rows", "ocgs_densify_workspace_bytes", "ocgs_densify_accumulate", "ocgs_densify", "ocgs_step_host", "ocgs_step_view_host", "ocgs_step_view_host_enqueue", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
+           "ocgs_prune_stats", "ocgs_compact_rows", "ocgs_densify_workspace_bytes", "ocgs_densify_accumulate", "ocgs_densify", "ocgs_step_host", "ocgs_step_view_host", "ocgs_step_view_host_enqueue", "ocgs_visibility_pass", "ocgs3d_visibility_pass", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
            "ocgs_profile_begin", "ocgs_profile_end"]
 
 
@@ -200,6 +200,16 @@ def ocgs3d_render_fwd(n, cam, cfg, ws, key_capacity, mask, color, alpha, depth, 
     _ok("ocgs3d_render_fwd", lib().ocgs3d_render_fwd(C.c_int(n), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity), _ptr(mask),
                                                      _ptr(color), _ptr(alpha), _ptr(depth), _ptr(n_contrib), _ptr(loss_bg),
                                                      _ptr(vis_count), _ptr(contrib_sum), _stream(stream)))
+
+
+def ocgs_visibility_pass(surfels, cam, cfg, ws, key_capacity, vis_count, contrib_sum, stream=None):
+    _ok("ocgs_visibility_pass", lib().ocgs_visibility_pass(C.byref(surfels), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity),
+                                                           _ptr(vis_count), _ptr(contrib_sum), _stream(stream)))
+
+
+def ocgs3d_visibility_pass(gaussians, cam, cfg, ws, key_capacity, vis_count, contrib_sum, stream=None):
+    _ok("ocgs3d_visibility_pass", lib().ocgs3d_visibility_pass(C.byref(gaussians), C.byref(cam), C.byref(cfg), _ptr(ws), C.c_size_t(key_capacity),
+                                                               _ptr(vis_count), _ptr(contrib_sum), _stream(stream)))
 
 
 def ocgs_render_fwd_reg(n, cam, cfg, ws, key_capacity, mask, color, alpha, depth, normal, n_contrib, loss_bg, vis_count, contrib_sum,

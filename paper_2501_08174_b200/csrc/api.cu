@@ -212,6 +212,34 @@ int ocgs3d_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, voi
                            nullptr, /*prim=*/1, nullptr, nullptr, nullptr, (cudaStream_t)stream);
 }
 
+int ocgs_visibility_pass(const ocgs_surfels* s, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
+                         uint32_t* vis_count, float* contrib_sum, void* stream) {
+  if (!s || !cam || !ws || !vis_count || !contrib_sum) return OCGS_ERR_INVALID_ARG;
+  int rc = check_cfg(cfg);
+  if (rc != OCGS_OK) return rc;
+  if (s->n > 0 && (!s->pos || !s->scale || !s->quat || !s->opacity)) return OCGS_ERR_INVALID_ARG;
+  Workspace w;
+  if (!carve_workspace(ws, s->n, cam->width, cam->height, key_capacity, &w, nullptr)) return OCGS_ERR_UNSUPPORTED;
+  const CamParams cp = make_cam(*cam);
+  if ((rc = launch_preprocess(*s, cp, *cfg, w, (cudaStream_t)stream, /*colour=*/false)) != OCGS_OK) return rc;
+  if ((rc = launch_bin_sort(cp, w, nullptr, (cudaStream_t)stream)) != OCGS_OK) return rc;
+  return launch_render_stats(cp, *cfg, w, vis_count, contrib_sum, /*prim=*/0, (cudaStream_t)stream);
+}
+
+int ocgs3d_visibility_pass(const ocgs_gaussians3d* g, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity,
+                           uint32_t* vis_count, float* contrib_sum, void* stream) {
+  if (!g || !cam || !ws || !vis_count || !contrib_sum) return OCGS_ERR_INVALID_ARG;
+  int rc = check_cfg(cfg);
+  if (rc != OCGS_OK) return rc;
+  if (g->n > 0 && (!g->pos || !g->scale || !g->quat || !g->opacity || !g->sh)) return OCGS_ERR_INVALID_ARG;
+  Workspace w;
+  if (!carve_workspace(ws, g->n, cam->width, cam->height, key_capacity, &w, nullptr)) return OCGS_ERR_UNSUPPORTED;
+  const CamParams cp = make_cam(*cam);
+  if ((rc = launch_preprocess3d(*g, cp, *cfg, w, (cudaStream_t)stream)) != OCGS_OK) return rc;
+  if ((rc = launch_bin_sort(cp, w, nullptr, (cudaStream_t)stream)) != OCGS_OK) return rc;
+  return launch_render_stats(cp, *cfg, w, vis_count, contrib_sum, /*prim=*/1, (cudaStream_t)stream);
+}
+
 int ocgs_render_fwd_l1(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
                        const float* target, float* color, float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg,
                        float* loss_l1, float* dL_dcolor, uint32_t* vis_count, float* contrib_sum, void* stream) {

@@ -90,7 +90,9 @@ struct CamParams {
 CamParams make_cam(const ocgs_camera& c);
 
 // stage launchers (each returns an OCGS_* code)
-int launch_preprocess(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, cudaStream_t st);
+int launch_preprocess(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, cudaStream_t st, bool colour = true);
+int launch_render_stats(const CamParams& cam, const ocgs_config& cfg, const Workspace& w, uint32_t* vis_count, float* contrib_sum,
+                        int prim, cudaStream_t st);
 int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cudaStream_t st);
 int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Workspace& w, const uint8_t* mask, float* color,
                       float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg, uint32_t* vis_count,

@@ -8,6 +8,9 @@ namespace ocgs {
 // the per-id integers; the visible ones (29 % at config 3, scattered) are compacted into a block-local list.  (2) the
 // list is processed densely, one visible surfel per thread: normal, SH colour (192 B read), the 96-byte raster record.
 // Without the compaction every warp runs the long second part with a third of its lanes.
+// kColour = false (the visibility pass): the facing normal and the SH colour are not needed -- the 192 B of SH per visible
+// surfel are not read, the record's colour and normal slots stay zero.
+template <bool kColour>
 __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict__ pos, const float2* __restrict__ scale,
                                                          const float4* __restrict__ quat, const float* __restrict__ opacity,
                                                          const float4* __restrict__ sh, int n, CamParams cam, ocgs_config cfg,
@@ -64,13 +67,15 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
     Projected pr;
     project_surfel(p, scale[id].x, scale[id].y, q, o, cam, cfg, pr);  // same inputs, same fp32 sequence: same result as phase 1
     uint8_t cl = 0;
-    {
+    float nx = 0.f, ny = 0.f, nz = 0.f;
+    float col[3] = {0.f, 0.f, 0.f};
+    if (kColour) {
       // facing normal (view space): n = R_wc t_w, flipped when n . p_c > 0
       const float w = q.x, x = q.y, y = q.z, z = q.w;
       const float tw0 = 2.0f * (x * z + w * y), tw1 = 2.0f * (y * z - w * x), tw2 = 1.0f - 2.0f * (x * x + y * y);
-      float nx = cam.V[0] * tw0 + cam.V[1] * tw1 + cam.V[2] * tw2;
-      float ny = cam.V[4] * tw0 + cam.V[5] * tw1 + cam.V[6] * tw2;
-      float nz = cam.V[8] * tw0 + cam.V[9] * tw1 + cam.V[10] * tw2;
+      nx = cam.V[0] * tw0 + cam.V[1] * tw1 + cam.V[2] * tw2;
+      ny = cam.V[4] * tw0 + cam.V[5] * tw1 + cam.V[6] * tw2;
+      nz = cam.V[8] * tw0 + cam.V[9] * tw1 + cam.V[10] * tw2;
       if (nx * pr.pc[0] + ny * pr.pc[1] + nz * pr.pc[2] > 0.0f) { nx = -nx; ny = -ny; nz = -nz; }
       // SH colour (S14)
       float dx = p[0] - cam.campos[0], dy = p[1] - cam.campos[1], dz = p[2] - cam.campos[2];
@@ -79,7 +84,7 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
       float Y[16];
       sh_basis(dx, dy, dz, cfg.sh_degree, Y);
       const int nb = (cfg.sh_degree + 1) * (cfg.sh_degree + 1);
-      float col[3] = {0.5f, 0.5f, 0.5f};
+      col[0] = col[1] = col[2] = 0.5f;
       const float4* shj = sh + (size_t)id * 12;
       const int nvec = (3 * nb + 3) / 4;
 #pragma unroll
@@ -99,6 +104,8 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
 #pragma unroll
       for (int c = 0; c < 3; ++c)
         if (col[c] < 0.0f) { col[c] = 0.0f; cl |= (uint8_t)(1u << c); }
+    }
+    {
       // centred record (common.cuh): P, Q, R, D0 in fp64 from the fp32 M, rounded once
       const float* M = pr.M;
       const double cxd = pr.cx, cyd = pr.cy;
@@ -122,14 +129,19 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
   }
 }
 
-int launch_preprocess(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, cudaStream_t st) {
+int launch_preprocess(const ocgs_surfels& s, const CamParams& cam, const ocgs_config& cfg, Workspace& w, cudaStream_t st, bool colour) {
   OCGS_CUDA_OK(cudaMemsetAsync(w.header, 0, sizeof(ocgs_header), st));
   if (g_prof_on) prof_mark(st, "memset_header");
   if (s.n == 0) return OCGS_OK;
   const int blocks = (int)div_up((size_t)s.n, 256);
-  preprocess_kernel<<<blocks, 256, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity, (const float4*)s.sh,
-                                            s.n, cam, cfg, w.depth_bits, w.rect, w.tiles, w.clamp, (float4*)w.rec_id,
-                                            w.id_to_rank, w.dkeyA, w.rank_to_id, w.header);
+  if (colour)
+    preprocess_kernel<true><<<blocks, 256, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity, (const float4*)s.sh,
+                                                    s.n, cam, cfg, w.depth_bits, w.rect, w.tiles, w.clamp, (float4*)w.rec_id,
+                                                    w.id_to_rank, w.dkeyA, w.rank_to_id, w.header);
+  else
+    preprocess_kernel<false><<<blocks, 256, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity, (const float4*)s.sh,
+                                                     s.n, cam, cfg, w.depth_bits, w.rect, w.tiles, w.clamp, (float4*)w.rec_id,
+                                                     w.id_to_rank, w.dkeyA, w.rank_to_id, w.header);
   OCGS_LAUNCHED(st, "preprocess_kernel");
   return OCGS_OK;
 }

@@ -77,7 +77,8 @@ constexpr int kFwdMinBlocks = 6;               // CTAs per SM the register budge
 // fused harness photometric term (S20): target image in, dL/dcolor and per-tile partial sums of |M (R - I)| out
 struct FwdL1 { const float* target; float* gC; float* partial; float inv_norm; };
 
-template <bool kStats, bool kMoments, int kPrim /*0 = 2D surfel, 1 = 3D Gaussian (EWA conic record)*/, bool kL1>
+// kMaps = false: the visibility pass (ocgs_visibility_pass): only the statistics are produced -- no maps, no blended lists, no loss
+template <bool kStats, bool kMoments, int kPrim /*0 = 2D surfel, 1 = 3D Gaussian (EWA conic record)*/, bool kL1, bool kMaps = true>
 __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                          const float4* __restrict__ rec, const uint32_t* __restrict__ rank_to_id,
@@ -121,7 +122,7 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
     const int cnt = (int)min((uint32_t)kFwdBatch, end - b0);
     if (__syncthreads_and(done)) break;
     if ((int)threadIdx.x < cnt) s_rank[threadIdx.x] = list[b0 + threadIdx.x];
-    if (threadIdx.x < kFwdBatch) s_hit[threadIdx.x] = 0;
+    if (kMaps && threadIdx.x < kFwdBatch) s_hit[threadIdx.x] = 0;
     if (kStats && threadIdx.x < kFwdBatch) { s_cnt[threadIdx.x] = 0; s_fix[threadIdx.x] = 0ull; }
     __syncthreads();
     for (int i = threadIdx.x; i < cnt * 6; i += 256) {
@@ -180,18 +181,20 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
             const bool blend = live && !(Tn < t_min);
             done = done || (live && Tn < t_min);  // S11: stop before blending this pair
             const float wgt = blend ? a[k] * T : 0.0f;
-            const float4 r4 = sr[4], r5 = sr[5];
-            C0 = fmaf(wgt, r4.y, C0); C1 = fmaf(wgt, r4.z, C1); C2 = fmaf(wgt, r4.w, C2);
-            D = fmaf(wgt, z[k], D);
-            if (kMoments) {
-              zc = (blend && last == 0) ? z[k] : zc;
-              const float dz = blend ? z[k] - zc : 0.0f;
-              M1 = fmaf(wgt, dz, M1);
-              M2 = fmaf(wgt * dz, dz, M2);
+            if (kMaps) {
+              const float4 r4 = sr[4], r5 = sr[5];
+              C0 = fmaf(wgt, r4.y, C0); C1 = fmaf(wgt, r4.z, C1); C2 = fmaf(wgt, r4.w, C2);
+              D = fmaf(wgt, z[k], D);
+              if (kMoments) {
+                zc = (blend && last == 0) ? z[k] : zc;
+                const float dz = blend ? z[k] - zc : 0.0f;
+                M1 = fmaf(wgt, dz, M1);
+                M2 = fmaf(wgt * dz, dz, M2);
+              }
+              N0 = fmaf(wgt, r5.x, N0); N1 = fmaf(wgt, r5.y, N1); N2 = fmaf(wgt, r5.z, N2);
+              last = blend ? (b0 - start) + c0 + j + 1 : last;
             }
-            N0 = fmaf(wgt, r5.x, N0); N1 = fmaf(wgt, r5.y, N1); N2 = fmaf(wgt, r5.z, N2);
             T = blend ? Tn : T;
-            last = blend ? (b0 - start) + c0 + j + 1 : last;
             const unsigned bal = __ballot_sync(0xFFFFFFFFu, blend);
             unsigned fix = 0;
             if (kStats) fix = __reduce_add_sync(0xFFFFFFFFu, (unsigned)__float2uint_rn(wgt * kContribFix));
@@ -233,19 +236,21 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
           if (Tn < t_min) {
             done = true;  // S11: stop before blending this pair
           } else {
-            const float4 r5 = sr[5];
             wgt = a * T;
-            C0 = fmaf(wgt, r4.y, C0); C1 = fmaf(wgt, r4.z, C1); C2 = fmaf(wgt, r4.w, C2);
-            D = fmaf(wgt, z, D);
-            if (kMoments) {
-              if (last == 0) zc = z;
-              const float dz = z - zc;
-              M1 = fmaf(wgt, dz, M1);
-              M2 = fmaf(wgt * dz, dz, M2);
+            if (kMaps) {
+              const float4 r5 = sr[5];
+              C0 = fmaf(wgt, r4.y, C0); C1 = fmaf(wgt, r4.z, C1); C2 = fmaf(wgt, r4.w, C2);
+              D = fmaf(wgt, z, D);
+              if (kMoments) {
+                if (last == 0) zc = z;
+                const float dz = z - zc;
+                M1 = fmaf(wgt, dz, M1);
+                M2 = fmaf(wgt * dz, dz, M2);
+              }
+              N0 = fmaf(wgt, r5.x, N0); N1 = fmaf(wgt, r5.y, N1); N2 = fmaf(wgt, r5.z, N2);
+              last = (b0 - start) + c0 + jj + 1;
             }
-            N0 = fmaf(wgt, r5.x, N0); N1 = fmaf(wgt, r5.y, N1); N2 = fmaf(wgt, r5.z, N2);
             T = Tn;
-            last = (b0 - start) + c0 + jj + 1;
             blend = true;
           }
         }
@@ -259,7 +264,7 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
         }
       }
       if (cntr) {
-        atomicOr(&s_hit[c0 + lane], wbit);
+        if (kMaps) atomicOr(&s_hit[c0 + lane], wbit);
         if (kStats) {
           atomicAdd(&s_cnt[c0 + lane], cntr);
           atomicAdd(&s_fix[c0 + lane], (unsigned long long)fixr);
@@ -267,7 +272,7 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
       }
     }
     __syncthreads();
-    {  // append the entries some warp blended to the tile's blended list (walked back to front by render_bwd)
+    if (kMaps) {  // append the entries some warp blended to the tile's blended list (walked back to front by render_bwd)
       const bool hitme = (int)threadIdx.x < cnt && s_hit[threadIdx.x] != 0;
       const unsigned bal = __ballot_sync(0xFFFFFFFFu, hitme);
       if (lane == 0) s_wcnt[threadIdx.x >> 5] = (uint32_t)__popc(bal);
@@ -293,6 +298,7 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
     }
   }
 
+  if (!kMaps) return;
   const float A = 1.0f - T;
   float l1sum = 0.f;
   if (inside) {
@@ -368,6 +374,27 @@ __global__ void __launch_bounds__(1024) loss_final_kernel(const float* __restric
     if (loss_bg) *loss_bg = (float)(s[0][0] * (double)inv_hw);
     if (loss2) *loss2 = (float)(s[1][0] * (double)scale2);
   }
+}
+
+// The visibility pass: statistics only ("rendering all training views"): same pair rule, same transmittance
+// chain and stop rule as the forward pass -- vis_count is bit-identical -- without the colour / depth / normal blends, the
+// maps, L_b and the blended lists.
+int launch_render_stats(const CamParams& cam, const ocgs_config& cfg, const Workspace& w, uint32_t* vis_count, float* contrib_sum,
+                        int prim, cudaStream_t st) {
+  if (w.n_tiles == 0) return OCGS_OK;
+  int rc = launch_order_tiles(w, /*from_ranges=*/true, st);
+  if (rc != OCGS_OK) return rc;
+  FwdL1 l1 = {nullptr, nullptr, nullptr, 0.f};
+  if (prim == 1)
+    render_fwd_kernel<true, false, 1, false, false><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec,
+        w.rank_to_id, nullptr, cam.W, cam.H, cam.tiles_x, cfg, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, w.header, nullptr,
+        vis_count, contrib_sum, nullptr, l1);
+  else
+    render_fwd_kernel<true, false, 0, false, false><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec,
+        w.rank_to_id, nullptr, cam.W, cam.H, cam.tiles_x, cfg, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, w.header, nullptr,
+        vis_count, contrib_sum, nullptr, l1);
+  OCGS_LAUNCHED(st, "render_stats_kernel");
+  return OCGS_OK;
 }
 
 int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Workspace& w, const uint8_t* mask, float* color,

@@ -16,11 +16,33 @@ from . import binding as B
 
 
 def accumulate_visibility(surfels: B.ocgs_surfels, n: int, cameras: Sequence, cfg: B.ocgs_config, ws: torch.Tensor, key_capacity: int,
-                          out: Dict[str, torch.Tensor], vis_count: torch.Tensor, contrib_sum: torch.Tensor, stream=None) -> None:
-    """Forward-only pass over `cameras` (scene cameras or ocgs_camera structs); the images in `out` are overwritten per
-    view, the per-surfel statistics accumulate.  No host synchronisation except one ocgs_check at the end."""
+                          out: Optional[Dict[str, torch.Tensor]], vis_count: torch.Tensor, contrib_sum: torch.Tensor, stream=None,
+                          ws2: Optional[torch.Tensor] = None) -> None:
+    """Forward-only pass over `cameras` (scene cameras or ocgs_camera structs); the per-surfel statistics accumulate.
+    out = None: the statistics-only pass (ocgs_visibility_pass: no images, no SH colour); otherwise the full forward pass,
+    the images in `out` overwritten per view.  ws2 (statistics-only pass): a second workspace of the same size; views then
+    alternate between two streams.  No host synchronisation except the ocgs_check at the end."""
+    if out is None and ws2 is not None:
+        # two views in flight: the short sort kernels and the tail of one view's walk (a few long tile lists on a few SMs)
+        # overlap the other view's work; both streams add into the same statistics with atomics
+        cur = torch.cuda.current_stream() if stream is None else stream
+        lanes = [(ws, torch.cuda.Stream()), (ws2, torch.cuda.Stream())]
+        for _, st in lanes:
+            st.wait_stream(cur)
+        for i, cam in enumerate(cameras):
+            c = cam if isinstance(cam, B.ocgs_camera) else B.camera_from(cam)
+            w, st = lanes[i % 2]
+            B.ocgs_visibility_pass(surfels, c, cfg, w, key_capacity, vis_count, contrib_sum, st)
+        for w, st in lanes:
+            cur.wait_stream(st)
+        B.ocgs_check(ws, stream)
+        B.ocgs_check(ws2, stream)
+        return
     for cam in cameras:
         c = cam if isinstance(cam, B.ocgs_camera) else B.camera_from(cam)
+        if out is None:
+            B.ocgs_visibility_pass(surfels, c, cfg, ws, key_capacity, vis_count, contrib_sum, stream)
+            continue
         B.ocgs_preprocess(surfels, c, cfg, ws, key_capacity, stream)
         B.ocgs_bin_sort(n, c, cfg, ws, key_capacity, None, stream)
         B.ocgs_render_fwd(n, c, cfg, ws, key_capacity, None, out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"],

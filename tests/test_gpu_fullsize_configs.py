@@ -98,6 +98,7 @@ def test_config4_full_size_all_views_prune():
     vis_o = np.zeros(n, np.uint32); cs_o = np.zeros(n, np.float64); touch = np.zeros(n, np.uint64)
     g = GpuView(P, sc.cameras[0], dict(sh_degree=3), key_capacity=24 * n)
     vis_g = torch.zeros(n, dtype=torch.int32, device="cuda"); cs_g = torch.zeros(n, dtype=torch.float32, device="cuda")
+    vis_s = torch.zeros_like(vis_g); cs_s = torch.zeros_like(cs_g)  # the same statistics through ocgs_visibility_pass
     ocfg = orc.default_config(sh_degree=3)
     for v in range(len(sc.cameras)):
         cam = orc.camera_from(sc.cameras[v])
@@ -116,6 +117,9 @@ def test_config4_full_size_all_views_prune():
             ok = fw["fragile"] == 0
             assert (np.abs(gf["alpha"] - fw["alpha"]) * ok).max() <= 1e-4
             assert (np.abs(gf["color"] - fw["color"]) * ok).max() <= 1e-4
+        B.ocgs_visibility_pass(g.surfels, g.cam, g.cfg, g.ws, g.cap, vis_s, cs_s)
+    assert torch.equal(vis_s, vis_g)
+    assert np.allclose(cs_s.cpu().numpy(), cs_g.cpu().numpy(), rtol=1e-5, atol=1e-7)
     vg = vis_g.cpu().numpy().view(np.uint32)
     clean = touch == 0
     assert np.array_equal(vg[clean], vis_o[clean])

@@ -100,6 +100,12 @@ def run_scene(sc, s3, views, sh_degree, with_masks=True):
     vis_g = torch.zeros(n, dtype=torch.int32, device="cuda"); cs_g = torch.zeros(n, dtype=torch.float32, device="cuda")
     vis_o = np.zeros(n, np.uint32); cs_o = np.zeros(n, np.float64); touch = np.zeros(n, np.uint64)
     Ks = [view_parity(g, P, sc.cameras[v], sc.mask(v) if with_masks else None, vis_g, cs_g, vis_o, cs_o, touch) for v in views]
+    # the statistics-only pass (ocgs3d_visibility_pass) counts exactly the same pairs as the forward pass
+    vis_s = torch.zeros_like(vis_g); cs_s = torch.zeros_like(cs_g)
+    for v in views:
+        B.ocgs3d_visibility_pass(g.g, B.camera_from(sc.cameras[v]), g.cfg, g.ws, g.cap, vis_s, cs_s)
+    assert torch.equal(vis_s, vis_g)
+    assert np.allclose(cs_s.cpu().numpy(), cs_g.cpu().numpy(), rtol=1e-5, atol=1e-7)
     vg = vis_g.cpu().numpy().view(np.uint32)
     clean = touch == 0
     assert np.array_equal(vg[clean], vis_o[clean])

@@ -110,6 +110,18 @@ def test_posthoc_prune_driver_matches_the_oracle():
     out = B.alloc_outputs(g.W, g.H)
     vis = torch.zeros(n, dtype=torch.int32, device="cuda"); cs = torch.zeros(n, dtype=torch.float32, device="cuda")
     pruning.accumulate_visibility(g.surfels, n, sc.cameras, g.cfg, g.ws, g.cap, out, vis, cs)
+    # the statistics-only pass (ocgs_visibility_pass: no SH colour, no maps, no blended lists) counts exactly the same pairs
+    vis_s = torch.zeros_like(vis); cs_s = torch.zeros_like(cs)
+    pruning.accumulate_visibility(g.surfels, n, sc.cameras, g.cfg, g.ws, g.cap, None, vis_s, cs_s)
+    assert torch.equal(vis_s, vis) and int(vis.sum().item()) > 10_000
+    assert np.allclose(cs_s.cpu().numpy(), cs.cpu().numpy(), rtol=1e-5, atol=1e-7)
+    # ... also with two views in flight on two streams and two workspaces
+    vis_s.zero_(); cs_s.zero_()
+    ws2 = B.alloc_workspace(n, g.W, g.H, g.cap)
+    pruning.accumulate_visibility(g.surfels, n, sc.cameras, g.cfg, g.ws, g.cap, None, vis_s, cs_s, ws2=ws2)
+    torch.cuda.synchronize()
+    assert torch.equal(vis_s, vis)
+    assert np.allclose(cs_s.cpu().numpy(), cs.cpu().numpy(), rtol=1e-5, atol=1e-7)
     vis_o = np.zeros(n, np.uint32); cs_o = np.zeros(n, np.float64); touch = np.zeros(n, np.uint64)
     ocfg = orc.default_config(sh_degree=3)
     for camn in sc.cameras:
