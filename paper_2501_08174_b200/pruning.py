@@ -21,33 +21,47 @@ def accumulate_visibility(surfels: B.ocgs_surfels, n: int, cameras: Sequence, cf
     """Forward-only pass over `cameras` (scene cameras or ocgs_camera structs); the per-surfel statistics accumulate.
     out = None: the statistics-only pass (ocgs_visibility_pass: no images, no SH colour); otherwise the full forward pass,
     the images in `out` overwritten per view.  ws2 (statistics-only pass): a second workspace of the same size; views then
-    alternate between two streams.  No host synchronisation except the ocgs_check at the end."""
+    alternate between two streams.  One host synchronisation, at the end; raises OcgsError if any view overflowed the key capacity."""
+    cams = [cam if isinstance(cam, B.ocgs_camera) else B.camera_from(cam) for cam in cameras]
+    cur = torch.cuda.current_stream() if stream is None else stream
+    # every view's workspace header (K, n_vis, error word; the next view's preprocess clears it) is kept on the device and
+    # checked once at the end, so that a key-capacity overflow in ANY view is reported without a per-view synchronisation
+    headers = torch.zeros((max(len(cams), 1), 4), dtype=torch.int32, device=ws.device)
+
+    def keep_header(i, w, st):
+        with torch.cuda.stream(st):
+            headers[i].copy_(w[:16].view(torch.int32), non_blocking=True)
+
     if out is None and ws2 is not None:
         # two views in flight: the short sort kernels and the tail of one view's walk (a few long tile lists on a few SMs)
         # overlap the other view's work; both streams add into the same statistics with atomics
-        cur = torch.cuda.current_stream() if stream is None else stream
         lanes = [(ws, torch.cuda.Stream()), (ws2, torch.cuda.Stream())]
         for _, st in lanes:
             st.wait_stream(cur)
-        for i, cam in enumerate(cameras):
-            c = cam if isinstance(cam, B.ocgs_camera) else B.camera_from(cam)
+        for i, c in enumerate(cams):
             w, st = lanes[i % 2]
             B.ocgs_visibility_pass(surfels, c, cfg, w, key_capacity, vis_count, contrib_sum, st)
-        for w, st in lanes:
+            keep_header(i, w, st)
+        for _, st in lanes:
             cur.wait_stream(st)
-        B.ocgs_check(ws, stream)
-        B.ocgs_check(ws2, stream)
-        return
-    for cam in cameras:
-        c = cam if isinstance(cam, B.ocgs_camera) else B.camera_from(cam)
-        if out is None:
-            B.ocgs_visibility_pass(surfels, c, cfg, ws, key_capacity, vis_count, contrib_sum, stream)
-            continue
-        B.ocgs_preprocess(surfels, c, cfg, ws, key_capacity, stream)
-        B.ocgs_bin_sort(n, c, cfg, ws, key_capacity, None, stream)
-        B.ocgs_render_fwd(n, c, cfg, ws, key_capacity, None, out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"],
-                          None, vis_count, contrib_sum, stream)
-    B.ocgs_check(ws, stream)
+    else:
+        for i, c in enumerate(cams):
+            if out is None:
+                B.ocgs_visibility_pass(surfels, c, cfg, ws, key_capacity, vis_count, contrib_sum, cur)
+            else:
+                B.ocgs_preprocess(surfels, c, cfg, ws, key_capacity, cur)
+                B.ocgs_bin_sort(n, c, cfg, ws, key_capacity, None, cur)
+                B.ocgs_render_fwd(n, c, cfg, ws, key_capacity, None, out["color"], out["alpha"], out["depth"], out["normal"], out["n_contrib"],
+                                  None, vis_count, contrib_sum, cur)
+            keep_header(i, ws, cur)
+    cur.synchronize()
+    err = headers[:, 3].cpu()
+    if int((err & 1).sum()) > 0:
+        bad = int(torch.nonzero(err & 1)[0])
+        need = int(headers[bad, :2].cpu().numpy().view("uint64")[0])
+        raise B.OcgsError(f"accumulate_visibility: view {bad} needs key_capacity >= {need}", B.OCGS_ERR_CAPACITY)
+    if int((err & 2).sum()) > 0:
+        raise B.OcgsError("accumulate_visibility: a tile list exceeds 2^24 entries", B.OCGS_ERR_UNSUPPORTED)
 
 
 def prune(surfels: B.ocgs_surfels, params: Dict[str, torch.Tensor], n: int, cfg: B.ocgs_config, vis_count: torch.Tensor,

@@ -122,6 +122,12 @@ def test_posthoc_prune_driver_matches_the_oracle():
     torch.cuda.synchronize()
     assert torch.equal(vis_s, vis)
     assert np.allclose(cs_s.cpu().numpy(), cs.cpu().numpy(), rtol=1e-5, atol=1e-7)
+    # a key capacity that only the first views exceed is still reported (the driver keeps every view's header)
+    cams_mixed = list(sc.cameras[:2]) + [sc.cameras[0]] * 2
+    small = B.alloc_workspace(n, g.W, g.H, 64)
+    with pytest.raises(B.OcgsError) as e:
+        pruning.accumulate_visibility(g.surfels, n, cams_mixed, g.cfg, small, 64, None, torch.zeros_like(vis), torch.zeros_like(cs))
+    assert e.value.code == B.OCGS_ERR_CAPACITY and "key_capacity >=" in str(e.value)
     vis_o = np.zeros(n, np.uint32); cs_o = np.zeros(n, np.float64); touch = np.zeros(n, np.uint64)
     ocfg = orc.default_config(sh_degree=3)
     for camn in sc.cameras:
