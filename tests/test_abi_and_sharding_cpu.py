@@ -114,3 +114,19 @@ def test_statistics_merge_over_gloo_world2_matches_single_process():
     m0 = orc.prune(res[0][1].astype(np.uint32), res[0][2].astype(np.float32), sc.opacity)["prune_mask"]
     m1 = orc.prune(res[1][1].astype(np.uint32), res[1][2].astype(np.float32), sc.opacity)["prune_mask"]
     assert np.array_equal(m0, m1)
+
+
+def test_defaults_match_the_constants_the_paper_states():
+    """tests/golden/paper_constants.txt: gamma = 0.5 in the library's default config (through the C ABI: the
+    helper is host-only) and in the oracle's; the pruning intervals are the training loop's business and only recorded."""
+    import os
+    import oracle as orc
+    from paper_2501_08174_b200 import binding as B
+    vals = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")):
+        if line.strip() and not line.startswith("#"):
+            name, value = line.split()[:2]
+            vals[name] = float(value)
+            assert "PAPER.md:" in line
+    assert B.ocgs_default_config().gamma_bg == vals["gamma_bg"] == orc.default_config().gamma_bg
+    assert (vals["prune_interval_dtu"], vals["prune_interval_mipnerf360"], vals["iterations"]) == (100, 600, 30000)
