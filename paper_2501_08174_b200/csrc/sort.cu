@@ -326,7 +326,8 @@ constexpr int kEmitThreads = 256;
 constexpr int kEmitPerThread = 8;
 constexpr int kEmitTile = kEmitThreads * kEmitPerThread;  // 2048 keys -> at most 2049 offsets entries
 
-__global__ void __launch_bounds__(kEmitThreads) emit_keys_kernel(const ocgs_header* __restrict__ header, const uint32_t* __restrict__ offsets,
+constexpr int kEmitBlocks = 6;  // resident blocks per SM = grid size / 148: one wave (1184 blocks of 40 registers ran as 1.33 waves: 42 us against 35)
+__global__ void __launch_bounds__(kEmitThreads, kEmitBlocks) emit_keys_kernel(const ocgs_header* __restrict__ header, const uint32_t* __restrict__ offsets,
                                                                  const uint32_t* __restrict__ rank_to_id, const ushort4* __restrict__ rect,
                                                                  int tiles_x, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals,
                                                                  int passes, int key_bits, size_t key_capacity, uint32_t* __restrict__ ghist,
@@ -346,7 +347,6 @@ __global__ void __launch_bounds__(kEmitThreads) emit_keys_kernel(const ocgs_head
   __shared__ uint32_t s_h[2][kRadix];
   static_assert(kEmitThreads == kRadix, "one thread per digit");
   s_h[0][threadIdx.x] = 0; s_h[1][threadIdx.x] = 0;
-  const int lane = threadIdx.x & 31;
   const uint32_t mask1 = passes > 1 ? (1u << min(kRadixBits, key_bits - kRadixBits)) - 1u : 0u;
   for (unsigned k0 = blockIdx.x * kEmitTile; k0 < K; k0 += gridDim.x * kEmitTile) {
   const unsigned k1 = min(k0 + kEmitTile, K);
@@ -372,32 +372,53 @@ __global__ void __launch_bounds__(kEmitThreads) emit_keys_kernel(const ocgs_head
   const unsigned r0 = s_r0, cnt = s_r1 - s_r0 + 1;  // surfels r0 .. r0+cnt-1 own the keys of this block (cnt <= kEmitTile)
   for (unsigned i = threadIdx.x; i <= cnt; i += kEmitThreads) s_off[i] = offsets[r0 + i];
   __syncthreads();
-  for (unsigned kb = k0 + (threadIdx.x & ~31u); kb < k1; kb += kEmitThreads) {  // warp-uniform trip count
-    const unsigned k = kb + lane;
-    const bool valid = k < k1;
-    uint32_t key = 0;
-    if (valid) {
+  // thread t emits the kEmitPerThread consecutive keys k0 + 8 t ..: one binary search for the first, then a walk along the
+  // surfel's rect (x fastest) and on to the next surfels -- no search and no division for the other seven
+  {
+    const unsigned kk = k0 + threadIdx.x * kEmitPerThread;
+    if (kk < k1) {
       unsigned lo = 0, hi = cnt;
-      while (hi - lo > 1) { const unsigned mid = (lo + hi) >> 1; if (s_off[mid] <= k) lo = mid; else hi = mid; }
-      // skip surfels with zero tiles cannot happen: visible surfels touch >= 1 tile, so s_off is strictly increasing
-      const unsigned r = r0 + lo;
-      const unsigned local = k - s_off[lo];
-      const ushort4 rc = rect[rank_to_id[r]];
-      const unsigned tx0 = rc.x >> 4, ty0 = rc.y >> 4, wdt = (rc.z >> 4) + 1 - tx0;
-      const unsigned ty = ty0 + local / wdt, tx = tx0 + local % wdt;
-      key = ty * (unsigned)tiles_x + tx;
-      keys[k] = key;
-      vals[k] = r;
-      if (passes > 0) atomicAdd(&s_h[0][key & (kRadix - 1)], 1u);
-    }
-    if (passes > 1) {
-      // the high digit (tile row) is nearly constant across 32 consecutive keys: one add of 32 instead of 32 colliding adds
-      const uint32_t dg = (key >> kRadixBits) & mask1;
-      const uint32_t d0 = __shfl_sync(0xFFFFFFFFu, dg, 0);
-      if (__all_sync(0xFFFFFFFFu, valid && dg == d0)) {
-        if (lane == 0) atomicAdd(&s_h[1][d0], 32u);
-      } else if (valid) {
-        atomicAdd(&s_h[1][dg], 1u);
+      while (hi - lo > 1) { const unsigned mid = (lo + hi) >> 1; if (s_off[mid] <= kk) lo = mid; else hi = mid; }
+      // (visible surfels touch >= 1 tile, so s_off is strictly increasing and every step below lands on a surfel with keys)
+      unsigned r = r0 + lo, next_off = s_off[lo + 1];
+      ushort4 rc = rect[rank_to_id[r]];
+      unsigned tx0 = rc.x >> 4, wdt = (rc.z >> 4) + 1 - tx0;
+      const unsigned local = kk - s_off[lo];
+      unsigned ty = (rc.y >> 4) + local / wdt, tx = tx0 + local % wdt;
+      uint32_t kbuf[kEmitPerThread], vbuf[kEmitPerThread];
+      uint32_t run_digit = 0xFFFFFFFFu, run_len = 0;
+      const int nk = (int)min((unsigned)kEmitPerThread, k1 - kk);
+#pragma unroll
+      for (int i = 0; i < kEmitPerThread; ++i) {
+        if (i < nk) {
+          if (kk + i >= next_off) {
+            ++lo; r = r0 + lo; next_off = s_off[lo + 1];
+            rc = rect[rank_to_id[r]];
+            tx0 = rc.x >> 4; wdt = (rc.z >> 4) + 1 - tx0; tx = tx0; ty = rc.y >> 4;
+          }
+          const uint32_t key = ty * (unsigned)tiles_x + tx;
+          kbuf[i] = key; vbuf[i] = r;
+          if (++tx == tx0 + wdt) { tx = tx0; ++ty; }
+          if (passes > 0) atomicAdd(&s_h[0][key & (kRadix - 1)], 1u);
+          if (passes > 1) {  // the high digit (tile row) changes rarely along the walk: one add per run
+            const uint32_t dg = (key >> kRadixBits) & mask1;
+            if (dg != run_digit) {
+              if (run_len) atomicAdd(&s_h[1][run_digit], run_len);
+              run_digit = dg; run_len = 0;
+            }
+            ++run_len;
+          }
+        }
+      }
+      if (passes > 1 && run_len) atomicAdd(&s_h[1][run_digit], run_len);
+      if (nk == kEmitPerThread) {  // k0 and 8 t are multiples of 8: 32-byte aligned
+        uint4* kd = (uint4*)(keys + kk); uint4* vd = (uint4*)(vals + kk);
+        kd[0] = make_uint4(kbuf[0], kbuf[1], kbuf[2], kbuf[3]); kd[1] = make_uint4(kbuf[4], kbuf[5], kbuf[6], kbuf[7]);
+        vd[0] = make_uint4(vbuf[0], vbuf[1], vbuf[2], vbuf[3]); vd[1] = make_uint4(vbuf[4], vbuf[5], vbuf[6], vbuf[7]);
+      } else {
+#pragma unroll
+        for (int i = 0; i < kEmitPerThread; ++i)
+          if (i < nk) { keys[kk + i] = kbuf[i]; vals[kk + i] = vbuf[i]; }
       }
     }
   }
@@ -468,7 +489,7 @@ int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cu
     const int passes = (bits + kRadixBits - 1) / kRadixBits;
     const bool fused_hist = passes <= 2;  // emit_keys_kernel keeps two histograms (n_tiles <= 65536)
     if (fused_hist) OCGS_CUDA_OK(cudaMemsetAsync(w.digit_total, 0, (kMaxPasses * kRadix + kMaxPasses) * sizeof(uint32_t), st));
-    emit_keys_kernel<<<(unsigned)min(div_up(cap, kEmitTile), (size_t)148 * 8), kEmitThreads, 0, st>>>(
+    emit_keys_kernel<<<(unsigned)min(div_up(cap, kEmitTile), (size_t)148 * kEmitBlocks), kEmitThreads, 0, st>>>(
         w.header, w.offsets, w.rank_to_id, w.rect, cam.tiles_x, w.tile_keys, w.tile_vals, fused_hist ? passes : 0, bits, cap, w.digit_total, w.hist,
         div_up(cap, kSortTile) * kRadix);
     OCGS_LAUNCHED(st, "emit_keys_kernel");
