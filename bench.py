@@ -503,10 +503,61 @@ def run_ours(args):
             how = "ocgs_step_view_host_enqueue captured into one CUDA graph per view, replay + stream synchronise + header check per step"
             # same view as the last direct step -> same forward loss, bit for bit (L_b is a fixed-order reduction)
             assert float(h_losses[0]) == direct_losses[0], (float(h_losses[0]), direct_losses)
+        ms_sameview = None
+        if not args.no_graph:
+            # the prefetching form (ocgs_step_view_prefetch_enqueue), what a data loader does: step k runs on view k's mask and
+            # target, which step k-1 uploaded from pinned host memory while it was computing, and uploads view k+1's meanwhile;
+            # every step's timed region therefore contains exactly one view's upload (its successor's) and the read-back of
+            # its own losses and header.  The resident target lets the forward pass fuse the masked L1.
+            ms_sameview = ms_view
+            d_img11 = torch.empty(11 * H * W, dtype=torch.float32, device=dev)
+            bufs = [(torch.empty(H * W, dtype=torch.uint8, device=dev), torch.empty(3 * H * W, dtype=torch.float32, device=dev)) for _ in range(2)]
+            pgraphs = {}
+
+            def pgraph(v, par):
+                if (v, par) not in pgraphs:
+                    nx = (v + 1) % nv
+                    torch.cuda.synchronize()
+                    gr = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(gr, stream=main):
+                        B.ocgs_step_view_prefetch_enqueue(surfels, cam_c[v], cfg, h_masks[nx], h_targets[nx], h_losses, h_header, bufs[par][0],
+                                                          bufs[par][1], bufs[1 - par][0], bufs[1 - par][1], d_img11, d_nc, grads, vis, cs,
+                                                          d_losses, ws, cap, stream=main, copy_stream=copy_stream)
+                    pgraphs[(v, par)] = gr
+                return pgraphs[(v, par)]
+            for k in range(2 * nv):
+                pgraph(k % nv, k % 2)
+            state = {"k": 0}
+
+            def prime():  # view 0 into buffer 0, outside the timed region (once per run)
+                bufs[0][0].copy_(h_masks[0].view(-1), non_blocking=True)
+                bufs[0][1].copy_(h_targets[0].view(-1), non_blocking=True)
+                torch.cuda.synchronize()
+                state["k"] = 0
+
+            def view_step_prefetch(_):
+                k = state["k"]
+                gr = pgraph(k % nv, k % 2)
+                with torch.cuda.stream(main):
+                    gr.replay()
+                main.synchronize()
+                if int(h_header[3]) != 0:
+                    raise RuntimeError("step reported error bits %d" % int(h_header[3]))
+                state["k"] = k + 1
+            prime()
+            ms_view = time_steps(view_step_prefetch)
+            how = ("ocgs_step_view_prefetch_enqueue captured into CUDA graphs (one per view and buffer parity), replay + stream synchronise + "
+                   "header check per step; the step's own inputs were uploaded by the previous step's prefetch, the next view's are uploaded "
+                   "during this step")
+            # the pipelined steps really ran on their own view's data: same forward losses as a direct step on that view
+            v_last, got = (state["k"] - 1) % nv, (float(h_losses[0]), float(h_losses[1]))
+            view_step(v_last)
+            assert got[0] == float(h_losses[0]) and abs(got[1] - float(h_losses[1])) < 1e-6, (got, float(h_losses[0]), float(h_losses[1]))
         e2e = {"value": ms_view, "unit": "ms", "h2d_bytes_per_step": H * W + 3 * H * W * 4, "d2h_bytes_per_step": 8 + 16, "steps": k_e,
                "what": how + ": target image + mask from pinned host memory each step, parameters and gradients resident "
                        "in HBM, uploads on a second stream overlapping preprocess/sort/forward, loss scalars read back",
-               "direct_launch_ms": ms_direct, "losses_last_step": [float(h_losses[0]), float(h_losses[1])]}
+               "direct_launch_ms": ms_direct, "graph_upload_inside_step_ms": ms_sameview,
+               "losses_last_step": [float(h_losses[0]), float(h_losses[1])]}
         hp = {k: torch.tensor(np.ascontiguousarray(getattr(scene, k)), dtype=torch.float32).pin_memory() for k in ("pos", "scale", "quat", "opacity", "sh")}
         h_grads = torch.empty(58 * n, dtype=torch.float32).pin_memory()
         h_alpha = torch.empty(H * W, dtype=torch.float32).pin_memory()

@@ -326,6 +326,20 @@ int ocgs_step_view_host_enqueue(const ocgs_surfels* surfels, const ocgs_camera* 
                                 float* d_grad_sh, uint32_t* d_vis_count, float* d_contrib_sum, float* d_losses, void* ws,
                                 size_t key_capacity, void* stream, void* copy_stream);
 
+/* The step with the NEXT view's inputs prefetched (what a data loader does): this view's mask and target are already in
+ * device memory (d_mask_cur, d_target_cur: put there by the previous call's prefetch, or by the caller for the first step);
+ * while the step runs, h_next_mask / h_next_target (page-locked host, NULL = nothing to prefetch) are uploaded on
+ * copy_stream into d_mask_next / d_target_next, off the critical path.  Because the target is resident when the forward
+ * pass starts, the masked L1 is fused into it (ocgs_render_fwd_l1).  Otherwise as ocgs_step_view_host_enqueue: nothing
+ * synchronises, losses and header come back through h_losses / h_header, the call is capturable into a CUDA graph.
+ * d_images: device [11*H*W] floats (color 3, alpha 1, depth 1, normal 3, dL_dcolor 3); d_target_*: device [3*H*W] floats. */
+int ocgs_step_view_prefetch_enqueue(const ocgs_surfels* surfels, const ocgs_camera* cam, const ocgs_config* cfg,
+                                    const uint8_t* h_next_mask, const float* h_next_target, float* h_losses, ocgs_header* h_header,
+                                    const uint8_t* d_mask_cur, const float* d_target_cur, uint8_t* d_mask_next, float* d_target_next,
+                                    float* d_images, uint32_t* d_ncontrib, float* d_grad_pos, float* d_grad_scale, float* d_grad_quat,
+                                    float* d_grad_opacity, float* d_grad_sh, uint32_t* d_vis_count, float* d_contrib_sum,
+                                    float* d_losses, void* ws, size_t key_capacity, void* stream, void* copy_stream);
+
 /* ---- end-to-end step with HOST parameters (bench.py "e2e_host_params") ---------------------------------------------------------------
  * Copies the surfel parameters, mask and target image from (pinned) host memory to the given device staging buffers,
  * runs (1)-(3) with L_b and statistics on, ocgs_masked_l1, then (4); copies the gradients, the alpha map and loss_bg back

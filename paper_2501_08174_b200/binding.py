@@ -18,7 +18,7 @@ _LIB_PATH = os.path.join(_HERE, "csrc", "libocgs.so")
 OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
            "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_render_fwd_l1", "ocgs_render_fwd_reg", "ocgs_render_bwd_reg", "ocgs3d_preprocess", "ocgs3d_render_fwd", "ocgs_prune_workspace_bytes",
-           "ocgs_prune_stats", "ocgs_compact_rows", "ocgs_densify_workspace_bytes", "ocgs_densify_accumulate", "ocgs_densify", "ocgs_step_host", "ocgs_step_view_host", "ocgs_step_view_host_enqueue", "ocgs_visibility_pass", "ocgs3d_visibility_pass", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
+           "ocgs_prune_stats", "ocgs_compact_rows", "ocgs_densify_workspace_bytes", "ocgs_densify_accumulate", "ocgs_densify", "ocgs_step_host", "ocgs_step_view_host", "ocgs_step_view_host_enqueue", "ocgs_step_view_prefetch_enqueue", "ocgs_visibility_pass", "ocgs3d_visibility_pass", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
            "ocgs_profile_begin", "ocgs_profile_end"]
 
 
@@ -295,6 +295,26 @@ def ocgs_step_view_host_enqueue(surfels, cam, cfg, h_mask, h_target, h_losses, h
                                           _ptr(d_grads["d_quat"]), _ptr(d_grads["d_opacity"]), _ptr(d_grads["d_sh"]), _ptr(d_vis_count),
                                           _ptr(d_contrib_sum), _ptr(d_losses), _ptr(ws), C.c_size_t(key_capacity), _stream(stream),
                                           C.c_void_p(copy_stream.cuda_stream) if copy_stream is not None else None))
+
+
+def ocgs_step_view_prefetch_enqueue(surfels, cam, cfg, h_next_mask, h_next_target, h_losses, h_header, d_mask_cur, d_target_cur, d_mask_next,
+                                    d_target_next, d_images, d_ncontrib, d_grads, d_vis_count, d_contrib_sum, d_losses, ws, key_capacity,
+                                    stream=None, copy_stream=None):
+    """The step on a view whose mask / target are already on the device, while the next view's are uploaded from pinned host
+    memory on copy_stream (h_next_* = None: no prefetch).  Enqueue only; capturable."""
+    def hp(t):
+        if t is None:
+            return None
+        if t.is_cuda or not t.is_contiguous() or not t.is_pinned():
+            raise ValueError("expected a contiguous page-locked host tensor")
+        return C.c_void_p(t.data_ptr())
+    _ok("ocgs_step_view_prefetch_enqueue",
+        lib().ocgs_step_view_prefetch_enqueue(C.byref(surfels), C.byref(cam), C.byref(cfg), hp(h_next_mask), hp(h_next_target), hp(h_losses),
+                                              hp(h_header), _ptr(d_mask_cur), _ptr(d_target_cur), _ptr(d_mask_next), _ptr(d_target_next),
+                                              _ptr(d_images), _ptr(d_ncontrib), _ptr(d_grads["d_pos"]), _ptr(d_grads["d_scale"]),
+                                              _ptr(d_grads["d_quat"]), _ptr(d_grads["d_opacity"]), _ptr(d_grads["d_sh"]), _ptr(d_vis_count),
+                                              _ptr(d_contrib_sum), _ptr(d_losses), _ptr(ws), C.c_size_t(key_capacity), _stream(stream),
+                                              C.c_void_p(copy_stream.cuda_stream) if copy_stream is not None else None))
 
 
 def ocgs_step_host(h_pos, h_scale, h_quat, h_opacity, h_sh, n, cam, cfg, h_mask, h_target, h_grads, h_alpha, h_loss_bg, d_params,

@@ -448,6 +448,53 @@ int ocgs_step_view_host_enqueue(const ocgs_surfels* surfels, const ocgs_camera* 
   return rc;
 }
 
+int ocgs_step_view_prefetch_enqueue(const ocgs_surfels* surfels, const ocgs_camera* cam, const ocgs_config* cfg,
+                                    const uint8_t* h_next_mask, const float* h_next_target, float* h_losses, ocgs_header* h_header,
+                                    const uint8_t* d_mask_cur, const float* d_target_cur, uint8_t* d_mask_next, float* d_target_next,
+                                    float* d_images, uint32_t* d_ncontrib, float* d_grad_pos, float* d_grad_scale, float* d_grad_quat,
+                                    float* d_grad_opacity, float* d_grad_sh, uint32_t* d_vis_count, float* d_contrib_sum,
+                                    float* d_losses, void* ws, size_t key_capacity, void* stream, void* copy_stream) {
+  if (!surfels || !cam || !cfg || !h_losses || !d_mask_cur || !d_target_cur || !d_images || !d_ncontrib || !d_losses || !ws)
+    return OCGS_ERR_INVALID_ARG;
+  const bool prefetch = h_next_mask != nullptr || h_next_target != nullptr;
+  if (prefetch && (!h_next_mask || !h_next_target || !d_mask_next || !d_target_next)) return OCGS_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaStream_t cs = copy_stream ? (cudaStream_t)copy_stream : st;
+  const size_t HW = (size_t)cam->width * cam->height;
+  float* color = d_images; float* alpha = color + 3 * HW; float* depth = alpha + HW; float* normal = depth + HW;
+  float* gC = normal + 3 * HW;
+  cudaEvent_t ev_begin = nullptr, ev_done = nullptr;
+  const bool fork = prefetch && cs != st;
+  if (prefetch) {
+    if (fork) {
+      OCGS_CUDA_OK(cudaEventCreateWithFlags(&ev_begin, cudaEventDisableTiming));
+      OCGS_CUDA_OK(cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming));
+      OCGS_CUDA_OK(cudaEventRecord(ev_begin, st));  // the step that last read d_*_next has finished
+      OCGS_CUDA_OK(cudaStreamWaitEvent(cs, ev_begin, 0));
+    }
+    OCGS_CUDA_OK(cudaMemcpyAsync(d_mask_next, h_next_mask, HW, cudaMemcpyHostToDevice, cs));
+    OCGS_CUDA_OK(cudaMemcpyAsync(d_target_next, h_next_target, 3 * HW * sizeof(float), cudaMemcpyHostToDevice, cs));
+    if (fork) OCGS_CUDA_OK(cudaEventRecord(ev_done, cs));
+  }
+  const int n = surfels->n;
+  int rc = OCGS_OK;
+  do {
+    if ((rc = ocgs_preprocess(surfels, cam, cfg, ws, key_capacity, stream)) != OCGS_OK) break;
+    if ((rc = ocgs_bin_sort(n, cam, cfg, ws, key_capacity, nullptr, stream)) != OCGS_OK) break;
+    if ((rc = ocgs_render_fwd_l1(n, cam, cfg, ws, key_capacity, d_mask_cur, d_target_cur, color, alpha, depth, normal, d_ncontrib, d_losses,
+                                 d_losses + 1, gC, d_vis_count, d_contrib_sum, stream)) != OCGS_OK) break;
+    if ((rc = ocgs_render_bwd(surfels, cam, cfg, ws, key_capacity, d_mask_cur, d_ncontrib, gC, nullptr, nullptr, nullptr, d_grad_pos, d_grad_scale,
+                              d_grad_quat, d_grad_opacity, d_grad_sh, nullptr, stream)) != OCGS_OK) break;
+    if (cudaMemcpyAsync(h_losses, d_losses, 2 * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
+    if (h_header && cudaMemcpyAsync(h_header, ws, sizeof(ocgs_header), cudaMemcpyDeviceToHost, st) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
+  } while (false);
+  if (fork) {
+    cudaStreamWaitEvent(st, ev_done, 0);  // join: the next call (and the end of a capture) sees the prefetch finished
+    cudaEventDestroy(ev_begin); cudaEventDestroy(ev_done);
+  }
+  return rc;
+}
+
 int ocgs_step_host(const float* h_pos, const float* h_scale, const float* h_quat, const float* h_opacity, const float* h_sh, int n,
                    const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask, const float* h_target, float* h_grads,
                    float* h_alpha, float* h_loss_bg, float* d_params, uint8_t* d_mask, float* d_images, uint32_t* d_ncontrib,

@@ -310,3 +310,27 @@ def test_masked_l1_and_host_step_match_device_path():
             h_target.add_(0.25)  # the next replay must see the new host data
         else:
             assert float(h_losses[1]) > float(loss.item()) + 0.01
+    # the prefetching form (ocgs_step_view_prefetch_enqueue): this view's inputs already resident, the NEXT view's uploaded
+    # meanwhile on the copy stream; fused L1.  Step A prefetches (mask, target) into the second buffers, step B runs on them.
+    h_target.copy_(torch.tensor(target))
+    HW = H * W
+    d_img11 = torch.empty(11 * HW, device="cuda")
+    bufs = [(torch.tensor(m, device="cuda"), torch.tensor(target, device="cuda") + 0.5),      # view data of step A (shifted target)
+            (torch.zeros(HW, dtype=torch.uint8, device="cuda"), torch.zeros(3 * HW, device="cuda"))]  # filled by A's prefetch
+    for step_i, (cur, nxt, hm, ht) in enumerate(((0, 1, h_mask, h_target), (1, 0, None, None))):
+        vis2.zero_(); cs2.zero_(); h_header.fill_(-1)
+        B.ocgs_step_view_prefetch_enqueue(g.surfels, g.cam, g.cfg, hm, ht, h_losses, h_header, bufs[cur][0], bufs[cur][1],
+                                          bufs[nxt][0] if hm is not None else None, bufs[nxt][1] if hm is not None else None,
+                                          d_img11, d_nc, grads, vis2, cs2, d_losses, g.ws, g.cap, stream=main, copy_stream=side)
+        main.synchronize()
+        assert int(h_header[3]) == 0 and float(h_losses[0]) == gf["loss_bg"]
+        if step_i == 0:
+            assert float(h_losses[1]) > float(loss.item()) + 0.01   # ran on the shifted target
+            side.synchronize()
+            assert torch.equal(bufs[1][0].cpu(), h_mask.view(-1)) and torch.equal(bufs[1][1].cpu(), h_target.view(-1))
+        else:
+            assert abs(float(h_losses[1]) - float(loss.item())) < 1e-7
+            for name in ("d_pos", "d_scale", "d_quat", "d_opacity", "d_sh"):
+                a, b = grads[name].cpu().numpy().ravel(), gg[name].ravel()
+                assert np.allclose(a, b, rtol=2e-3, atol=1e-6 + 1e-4 * np.abs(b).max()), name
+            assert np.array_equal(vis2.cpu().numpy().view(np.uint32), gf["vis_count"])
