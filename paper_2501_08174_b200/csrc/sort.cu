@@ -25,21 +25,24 @@ __device__ __forceinline__ unsigned long long load_count(const void* n_ptr, bool
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kFlagMask = 3u << 30, kValMask = (1u << 30) - 1u;
 constexpr int kMaxPasses = 4;
 
+constexpr int kHistItems = 4;  // keys per thread and unit of work of the histogram kernel (finer than a sort tile: more blocks in flight)
 __global__ void __launch_bounds__(kSortThreads) radix_hist_all_kernel(const uint32_t* __restrict__ keys, const void* n_ptr, bool n_is_u64,
                                                                       size_t n_cap, int key_bits, int passes, uint32_t* __restrict__ ghist,
                                                                       uint32_t* __restrict__ status, size_t status_stride) {
   const unsigned long long n = min(load_count(n_ptr, n_is_u64), (unsigned long long)n_cap);
   const unsigned nblk = (unsigned)div_up((size_t)n, kSortTile);
-  if (blockIdx.x >= nblk) return;
+  const unsigned nunit = (unsigned)div_up((size_t)n, (size_t)kHistItems * kSortThreads);
+  if (blockIdx.x >= nunit) return;
   __shared__ uint32_t h[kMaxPasses][kRadix];
   for (int p = 0; p < passes; ++p) h[p][threadIdx.x] = 0;
   __syncthreads();
   const int lane = threadIdx.x & 31;
-  for (unsigned tile = blockIdx.x; tile < nblk; tile += gridDim.x) {
-  for (int p = 0; p < passes; ++p) status[(size_t)p * status_stride + (size_t)tile * kRadix + threadIdx.x] = 0;  // look-back state of the tile
-  const size_t base = (size_t)tile * kSortTile;
-#pragma unroll 4
-  for (int r = 0; r < kSortItems; ++r) {
+  for (unsigned tile = blockIdx.x; tile < nblk; tile += gridDim.x)  // look-back state of the sort tiles
+    for (int p = 0; p < passes; ++p) status[(size_t)p * status_stride + (size_t)tile * kRadix + threadIdx.x] = 0;
+  for (unsigned unit = blockIdx.x; unit < nunit; unit += gridDim.x) {
+  const size_t base = (size_t)unit * kHistItems * kSortThreads;
+#pragma unroll
+  for (int r = 0; r < kHistItems; ++r) {
     const size_t i = base + (size_t)r * kSortThreads + threadIdx.x;
     const bool valid = i < n;
     const uint32_t k = valid ? keys[i] : 0u;
@@ -191,7 +194,7 @@ int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t
   static_assert(kSortThreads == kRadix, "one thread per digit");
   const int passes = (key_bits + kRadixBits - 1) / kRadixBits;
   const unsigned tiles_max = (unsigned)div_up(n_max, kSortTile);
-  const unsigned grid = min(tiles_max, 148u * 4u);
+  const unsigned grid = (unsigned)min(div_up(n_max, (size_t)kHistItems * kSortThreads), (size_t)148 * 4);
   *result_in_B = (passes & 1) != 0;
   if (grid == 0 || passes == 0) { *result_in_B = false; return OCGS_OK; }
   if (passes > kMaxPasses || n_max > (size_t)kValMask) return OCGS_ERR_UNSUPPORTED;
