@@ -24,6 +24,7 @@ sys.path.insert(0, ROOT)
 
 METRIC = "ms per fwd+bwd raster step (1600x1200, 1M surfels)"
 FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 40.0, 22.0, 72.0  # DESIGN.md section 6 "algorithmic work per unit" (FMA = 2)
+FLOP_BLEND_BWD_COLOUR_ONLY = 54.0  # no upstream gradient on depth / normal maps (masked L1 + L_b): those terms are not evaluated
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the raster kernels, from the `ncu --set full` capture of this
 # workload committed as profiles/r01j_raster_kernels_full.md (bytes)
 NCU_TRAFFIC = {"render_bwd_kernel": 88.7e6, "render_fwd_kernel": 139.3e6}
@@ -603,7 +604,8 @@ def run_ours(args):
             if name == "render_fwd_kernel":
                 fl, what = FLOP_EVAL * E + FLOP_BLEND_FWD * Bp, f"{FLOP_EVAL:.0f} flop x E evaluated pairs + {FLOP_BLEND_FWD:.0f} flop x B blended pairs"
             else:
-                fl, what = (FLOP_EVAL + FLOP_BLEND_BWD) * Bp, f"({FLOP_EVAL:.0f} + {FLOP_BLEND_BWD:.0f}) flop x B blended pairs"
+                fb = FLOP_BLEND_BWD_COLOUR_ONLY if args.loss in ("l1", "dssim") else FLOP_BLEND_BWD
+                fl, what = (FLOP_EVAL + fb) * Bp, f"({FLOP_EVAL:.0f} + {fb:.0f}) flop x B blended pairs"
             ach = fl / avg_s / 1e12
             return {"kernel": name, "bound": "alu", "achieved": ach, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / ALU_PEAK_TFLOPS,
                     "traffic": NCU_TRAFFIC.get(name), "traffic_source": NCU_TRAFFIC_SOURCE,

@@ -74,7 +74,9 @@ struct BwdConsts { float near_z, alpha_max, inv_sigma2; };
 // With Q_c the accumulated maps, q_c this pair's values (rgb, z, n), S_c the suffix sums behind it (O7):
 //   dL/dalpha_i = sum_c g_c (q_c T_i - S_c/(1-alpha_i)) + gA T_final/(1-alpha_i) = T_i (g.q) - (g.S - gA T_final)/(1-alpha_i),
 // and g.S advances by w_i (g.q): one running scalar GS replaces the seven suffix sums.
-template <bool kMoments>
+// kGeo = false: no upstream gradient on the depth / normal / moment maps (gD, gN null: the masked-L1 + L_b step), so the
+// terms they multiply are identically zero and are not evaluated.
+template <bool kMoments, bool kGeo>
 __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4 r0, const float4 r1, const float4 r2, const float4 r3,
                                          const float4* __restrict__ sr, const BwdConsts& k, float* v, float* ex) {
   const float dx = s.px - r2.z, dy = s.py - r2.w;
@@ -90,7 +92,7 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
   const float z = surf ? r2.y * inv : r3.y;
   const bool contributes = idx < s.last && qz != 0.0f && !(z < k.near_z) && !(rho > r3.x);
   if (contributes) {
-    const float4 r4 = sr[4], r5 = sr[5];
+    const float4 r4 = sr[4], r5 = kGeo ? sr[5] : make_float4(0.f, 0.f, 0.f, 0.f);
     const float G = ex2_approx(rho * kNegHalfLog2e);
     const float araw = r4.x * G;
     const bool capped = araw > k.alpha_max;
@@ -98,29 +100,29 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
     const float inv1ma = rcp_approx(1.0f - a);
     s.T *= inv1ma;  // T_i = T_{i+1} / (1 - alpha_i)
     const float T = s.T, w = a * T;
-    float gq = s.gd * z;
+    float gq = kGeo ? s.gd * z : 0.f;
     const float dz = z - s.zc;
     if (kMoments) gq = fmaf(s.gm2 * dz, dz, fmaf(s.gm1, dz, gq));  // m1, m2 behave like blended channels with values dz, dz^2
     gq = fmaf(s.gc0, r4.y, gq); gq = fmaf(s.gc1, r4.z, gq); gq = fmaf(s.gc2, r4.w, gq);
-    gq = fmaf(s.gn0, r5.x, gq); gq = fmaf(s.gn1, r5.y, gq); gq = fmaf(s.gn2, r5.z, gq);
+    if (kGeo) { gq = fmaf(s.gn0, r5.x, gq); gq = fmaf(s.gn1, r5.y, gq); gq = fmaf(s.gn2, r5.z, gq); }
     const float galpha = fmaf(T, gq, -s.GS * inv1ma);
     s.GS = fmaf(w, gq, s.GS);
     v[10] = fmaf(w, s.gc0, v[10]); v[11] = fmaf(w, s.gc1, v[11]); v[12] = fmaf(w, s.gc2, v[12]);
-    v[13] = fmaf(w, s.gn0, v[13]); v[14] = fmaf(w, s.gn1, v[14]); v[15] = fmaf(w, s.gn2, v[15]);
-    float gz = w * s.gd;
+    if (kGeo) { v[13] = fmaf(w, s.gn0, v[13]); v[14] = fmaf(w, s.gn1, v[14]); v[15] = fmaf(w, s.gn2, v[15]); }
+    float gz = kGeo ? w * s.gd : 0.f;
     if (kMoments) gz = fmaf(w, fmaf(2.0f * dz, s.gm2, s.gm1), gz);  // ... and depend on z directly (the origin is a constant)
     float grho = 0.f;
     if (!capped) { v[9] = fmaf(G, galpha, v[9]); grho = -0.5f * G * r4.x * galpha; }  // S12: zero through the cap
     if (surf) {
       // rho = u^2+v^2, z = D0/qz, (u,v) = (qx,qy)/qz, q = R - dx P - dy Q
       const float gu = 2.0f * u * grho, gv = 2.0f * vv * grho;
-      const float gq0 = gu * inv, gq1 = gv * inv, gq2 = -(fmaf(gu, u, fmaf(gv, vv, gz * z))) * inv;
+      const float gq0 = gu * inv, gq1 = gv * inv, gq2 = -(fmaf(gu, u, fmaf(gv, vv, kGeo ? gz * z : 0.f))) * inv;
       v[0] = fmaf(-dx, gq0, v[0]); v[1] = fmaf(-dx, gq1, v[1]); v[2] = fmaf(-dx, gq2, v[2]);
       v[3] = fmaf(-dy, gq0, v[3]); v[4] = fmaf(-dy, gq1, v[4]); v[5] = fmaf(-dy, gq2, v[5]);
       v[6] += gq0; v[7] += gq1; v[8] += gq2;
-      ex[0] = fmaf(gz, inv, ex[0]);
+      if (kGeo) ex[0] = fmaf(gz, inv, ex[0]);
     } else {
-      ex[1] += gz;  // z = z_j
+      if (kGeo) ex[1] += gz;  // z = z_j
       ex[2] = fmaf(-2.0f * dx * k.inv_sigma2, grho, ex[2]);
       ex[3] = fmaf(-2.0f * dy * k.inv_sigma2, grho, ex[3]);
     }
@@ -135,7 +137,7 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
 // accumulator and visits an entry at most once per batch, so its totals are plain stores (shared float atomics are CAS
 // loops); the flush adds the slices of the warps whose forward hit bits are set.
 constexpr int kBwdMinBlocks = 5;  // 4, 6, 7 measured slower
-template <bool kMoments>
+template <bool kMoments, bool kGeo>
 __global__ void __launch_bounds__(128, kBwdMinBlocks) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                             const float4* __restrict__ rec, const uint2* __restrict__ blist, const uint8_t* __restrict__ mask,
@@ -178,9 +180,9 @@ __global__ void __launch_bounds__(128, kBwdMinBlocks) render_bwd_kernel(const ui
       Tfin = final_T[p];
       if (gC) { s.gc0 = gC[p]; s.gc1 = gC[HW + p]; s.gc2 = gC[2 * HW + p]; }
       if (gA) ga = gA[p];
-      if (gD) s.gd = gD[p];
+      if (kGeo && gD) s.gd = gD[p];
       if (kMoments) { s.zc = mom[p]; s.gm1 = gM1[p]; s.gm2 = gM2[p]; }
-      if (gN) { s.gn0 = gN[p]; s.gn1 = gN[HW + p]; s.gn2 = gN[2 * HW + p]; }
+      if (kGeo && gN) { s.gn0 = gN[p]; s.gn1 = gN[HW + p]; s.gn2 = gN[2 * HW + p]; }
       if (mask && mask[p] == 0) ga += gamma_over_hw;  // d(gamma L_b)/dA = gamma (1-M)/(HW), Eq. 1 / Eq. 3
     }
     s.T = Tfin;
@@ -223,12 +225,13 @@ __global__ void __launch_bounds__(128, kBwdMinBlocks) render_bwd_kernel(const ui
 #pragma unroll
         for (int i = 0; i < 16; ++i) v[i] = 0.f;
         float ex[4] = {0.f, 0.f, 0.f, 0.f};  // gD0, gzj, gcx, gcy
-        if ((m0 >> jb) & 1u) bwd_pair<kMoments>(ps[0], idx, r0, r1, r2, r3, sr, kc, v, ex);
-        if ((m1 >> jb) & 1u) bwd_pair<kMoments>(ps[1], idx, r0, r1, r2, r3, sr, kc, v, ex);
+        if ((m0 >> jb) & 1u) bwd_pair<kMoments, kGeo>(ps[0], idx, r0, r1, r2, r3, sr, kc, v, ex);
+        if ((m1 >> jb) & 1u) bwd_pair<kMoments, kGeo>(ps[1], idx, r0, r1, r2, r3, sr, kc, v, ex);
         float* dst = acc + j * kNG;
         warp_transpose_reduce16(v, lane);
         if ((lane & 1) == 0) dst[lane >> 1] = v[0];
-        if (__any_sync(0xFFFFFFFFu, (ex[0] != 0.f) | (ex[1] != 0.f) | (ex[2] != 0.f) | (ex[3] != 0.f))) warp_transpose_reduce4(ex, lane);
+        if (__any_sync(0xFFFFFFFFu, kGeo ? (ex[0] != 0.f) | (ex[1] != 0.f) | (ex[2] != 0.f) | (ex[3] != 0.f) : (ex[2] != 0.f) | (ex[3] != 0.f)))
+          warp_transpose_reduce4(ex, lane);
         if ((lane & 7) == 0) dst[16 + (lane >> 3)] = ex[0];  // without the reduction every lane's ex[0] is zero
       }
     }
@@ -434,11 +437,14 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
     if (rc != OCGS_OK) return rc;
     const float goh = mask ? (float)((double)cfg.gamma_bg / ((double)cam.W * (double)cam.H)) : 0.f;
     if (mom && gM1 && gM2)
-      render_bwd_kernel<true><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, mom, gM1, gM2,
+      render_bwd_kernel<true, true><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, mom, gM1, gM2,
                                                          cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
-    else
-      render_bwd_kernel<false><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, nullptr, nullptr, nullptr,
-                                                          cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
+    else if (gD || gN)
+      render_bwd_kernel<false, true><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, nullptr, nullptr, nullptr,
+                                                                cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
+    else  // colour / alpha gradients only (masked L1 + L_b): the depth and normal terms are identically zero
+      render_bwd_kernel<false, false><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, nullptr, nullptr, nullptr, nullptr, nullptr,
+                                                                 cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
     OCGS_LAUNCHED(st, "render_bwd_kernel");
   }
   project_bwd_kernel<<<(unsigned)div_up((size_t)s.n, 128), 128, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity,
