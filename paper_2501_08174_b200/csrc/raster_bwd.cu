@@ -137,30 +137,49 @@ __device__ __forceinline__ bool bwd_pair(BwdPixel& s, uint32_t idx, const float4
 // accumulator and visits an entry at most once per batch, so its totals are plain stores (shared float atomics are CAS
 // loops); the flush adds the slices of the warps whose forward hit bits are set.
 constexpr int kBwdMinBlocks = 5;  // 4, 6, 7 measured slower
+// A tile's blended list is walked by one CTA, each warp's part of it strictly in order: when lists are long and never
+// saturate (config 5) the kernel's time is the chain of its heaviest tiles.  Tiles among the first kBwdSplitMax of the launch
+// order whose blended list is longer than kBwdHeavyLen are therefore walked by TWO CTAs, one pixel per thread, each warp
+// owning one forward block: a warp then visits only the entries its single block blended (about half as many).
+constexpr int kBwdSplitMax = 512;
+constexpr uint32_t kBwdHeavyLen = 2048;
+#ifndef OCGS_BWD_LEAN_BLOCKS
+#define OCGS_BWD_LEAN_BLOCKS 6
+#endif
+constexpr int kBwdLeanMinBlocks = OCGS_BWD_LEAN_BLOCKS;  // the colour / alpha-only instance (72 registers: 7 resident blocks)
 template <bool kMoments, bool kGeo>
-__global__ void __launch_bounds__(128, kBwdMinBlocks) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
+__global__ void __launch_bounds__(128, kGeo ? kBwdMinBlocks : kBwdLeanMinBlocks) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                             const float4* __restrict__ rec, const uint2* __restrict__ blist, const uint8_t* __restrict__ mask,
                                                             const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
                                                             const float* __restrict__ gC, const float* __restrict__ gA,
                                                             const float* __restrict__ gD, const float* __restrict__ gN, const float* __restrict__ mom, const float* __restrict__ gM1, const float* __restrict__ gM2, int W, int H,
-                                                            int tiles_x, ocgs_config cfg, float gamma_over_hw, float* __restrict__ grad_rec) {
+                                                            int tiles_x, int n_tiles, ocgs_config cfg, float gamma_over_hw, float* __restrict__ grad_rec) {
   __shared__ float4 s_rec[kBwdBatch * 6];
   __shared__ uint32_t s_rank[kBwdBatch];
   __shared__ uint8_t s_mask[kBwdBatch];
   __shared__ uint32_t s_idx[kBwdBatch];   // position of the entry in the tile's full list (n_contrib counts those)
   __shared__ float s_acc[4][kBwdBatch * kNG];
   static_assert(kBwdBatch == 64, "the per-warp entry masks below cover two 32-entry halves");
-  const int tile = (int)tile_order[blockIdx.x];  // heavy tiles are launched first
+  // launch order: heavy tiles first (tile_order); the first `n_split` positions own two consecutive blocks each, so that a
+  // tile with a long blended list can be walked by two CTAs (see kBwdHeavyLen)
+  const int n_split = min(n_tiles, kBwdSplitMax);
+  const int pos = (int)blockIdx.x < 2 * n_split ? (int)(blockIdx.x >> 1) : (int)blockIdx.x - n_split;
+  const int part = (int)blockIdx.x < 2 * n_split ? (int)(blockIdx.x & 1u) : 0;
+  const int tile = (int)tile_order[pos];
   const uint32_t mx = tile_work[tile];           // length of the tile's blended list (written by the forward pass)
-  if (mx == 0) return;
+  const bool split = pos < n_split && mx > kBwdHeavyLen;
+  if (mx == 0 || (part && !split)) return;
   const int tx = tile % tiles_x, ty = tile / tiles_x;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t start = ranges[2 * tile];
-  // this warp's two forward blocks: vertically adjacent, block ids differ by the number of blocks per tile row
+  // this warp's two forward blocks: vertically adjacent, block ids differ by the number of blocks per tile row; in a split
+  // tile the warp owns ONE forward block (CTA `part` takes blocks 4 part .. 4 part + 3) and the second pixel is switched off
   constexpr int kBX = kTile / kSubW;  // forward blocks per tile row
-  const int bcol = warp % kBX, brow = 2 * (warp / kBX);
-  const uint32_t bit0 = 1u << (brow * kBX + bcol), bit1 = bit0 << kBX;
+  static_assert((kTile / kSubW) * (kTile / kSubH) == 8, "a split tile gives four of its eight forward blocks to each CTA");
+  const int fb = split ? 4 * part + warp : 2 * (warp / kBX) * kBX + warp % kBX;  // the warp's (first) forward block
+  const int bcol = fb % kBX, brow = fb / kBX;
+  const uint32_t bit0 = 1u << fb, bit1 = split ? 0u : bit0 << kBX;
   const size_t HW = (size_t)W * H;
   BwdConsts kc = {cfg.near_z, cfg.alpha_max, 1.0f / cfg.filter_sigma2};
   float* acc = s_acc[warp];
@@ -174,7 +193,7 @@ __global__ void __launch_bounds__(128, kBwdMinBlocks) render_bwd_kernel(const ui
     s.last = 0;
     float Tfin = 1.0f, ga = 0.f;
     s.gc0 = s.gc1 = s.gc2 = s.gd = s.gn0 = s.gn1 = s.gn2 = s.zc = s.gm1 = s.gm2 = 0.f;
-    if (ix < W && iy < H) {
+    if (ix < W && iy < H && !(split && q)) {
       const size_t p = (size_t)iy * W + ix;
       s.last = n_contrib[p];
       Tfin = final_T[p];
@@ -242,7 +261,7 @@ __global__ void __launch_bounds__(128, kBwdMinBlocks) render_bwd_kernel(const ui
       float val = 0.f;
 #pragma unroll
       for (int w2 = 0; w2 < 4; ++w2)
-        if (m & (((1u << kBX) | 1u) << ((2 * (w2 / kBX)) * kBX + w2 % kBX))) val += s_acc[w2][i];
+        if (m & (split ? 1u << (4 * part + w2) : ((1u << kBX) | 1u) << ((2 * (w2 / kBX)) * kBX + w2 % kBX))) val += s_acc[w2][i];
       if (val != 0.f) atomicAdd(grad_rec + (size_t)s_rank[e] * kRec + (i - kNG * e), val);
     }
   }
@@ -437,14 +456,14 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
     if (rc != OCGS_OK) return rc;
     const float goh = mask ? (float)((double)cfg.gamma_bg / ((double)cam.W * (double)cam.H)) : 0.f;
     if (mom && gM1 && gM2)
-      render_bwd_kernel<true, true><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, mom, gM1, gM2,
-                                                         cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
+      render_bwd_kernel<true, true><<<w.n_tiles + min(w.n_tiles, kBwdSplitMax), 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, mom, gM1, gM2,
+                                                         cam.W, cam.H, cam.tiles_x, w.n_tiles, cfg, goh, w.grad_rec);
     else if (gD || gN)
-      render_bwd_kernel<false, true><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, nullptr, nullptr, nullptr,
-                                                                cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
+      render_bwd_kernel<false, true><<<w.n_tiles + min(w.n_tiles, kBwdSplitMax), 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, nullptr, nullptr, nullptr,
+                                                                cam.W, cam.H, cam.tiles_x, w.n_tiles, cfg, goh, w.grad_rec);
     else  // colour / alpha gradients only (masked L1 + L_b): the depth and normal terms are identically zero
-      render_bwd_kernel<false, false><<<w.n_tiles, 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, nullptr, nullptr, nullptr, nullptr, nullptr,
-                                                                 cam.W, cam.H, cam.tiles_x, cfg, goh, w.grad_rec);
+      render_bwd_kernel<false, false><<<w.n_tiles + min(w.n_tiles, kBwdSplitMax), 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, nullptr, nullptr, nullptr, nullptr, nullptr,
+                                                                 cam.W, cam.H, cam.tiles_x, w.n_tiles, cfg, goh, w.grad_rec);
     OCGS_LAUNCHED(st, "render_bwd_kernel");
   }
   project_bwd_kernel<<<(unsigned)div_up((size_t)s.n, 128), 128, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity,
