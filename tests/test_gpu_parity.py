@@ -83,6 +83,10 @@ def full_parity(sc, view, cfg_kw, rng_seed=5, max_fragile=2e-3, with_bwd=True):
         og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=gC.astype(np.float32), gA=gA.astype(np.float32),
                             gD=gD.astype(np.float32), gN=gN.astype(np.float32))
         rep = check_grads(gg, og, skip_rows=pre["clamp_fragile"] != 0)
+        # the colour / alpha-only instance of the kernel (no upstream gradient on the depth and normal maps)
+        gg2 = g.render_bwd(gC=gC, gA=gA, mask=mm)
+        og2 = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=gC.astype(np.float32), gA=gA.astype(np.float32))
+        check_grads(gg2, og2, skip_rows=pre["clamp_fragile"] != 0)
         # surfels never blended receive exactly zero gradient
         never = gf["vis_count"] == 0
         for k in ("d_pos", "d_scale", "d_quat", "d_opacity", "d_sh"):
@@ -133,6 +137,36 @@ def test_long_tile_lists_take_the_heavy_walk():
     for i, k in enumerate(("origin", "m1", "m2")):
         err = np.abs(gf["moments"][i] - fw[k]) / np.maximum(1.0, np.abs(fw[k]))
         assert (err * ok).max() <= IMG_TOL, (k, (err * ok).max())
+
+
+def test_split_heavy_tile_backward_both_instances():
+    """ONE 16x16 tile whose blended list (= the surfels with vis_count > 0, by the oracle) is longer than kBwdHeavyLen = 2048
+    (raster_bwd.cu): the backward pass walks it with two CTAs, one pixel per thread.  Checked for both instances of the kernel:
+    upstream gradients on all four maps, and on colour + alpha only (the masked-L1 + L_b step; depth / normal terms left out)."""
+    sc = sg.random_scene(6000, 16, 16, 40.0, seed=33, sh_degree=0, scale_lo=0.2, scale_hi=0.5, op_mu=-4.5, op_sigma=0.5)
+    P, m = arrays(sc), sc.mask(0)
+    orc, cam, cfg, pre, srt, fw = oracle_view(P, sc.cameras[0], dict(sh_degree=0), mask=m)
+    assert int((fw["vis_count"] > 0).sum()) > 2048
+    g = GpuView(P, sc.cameras[0], dict(sh_degree=0))
+    g.preprocess(); g.bin_sort(want_ids=False)
+    gf = g.render_fwd(mask=m)
+    ok = fw["fragile"] == 0
+    assert np.array_equal(gf["n_contrib"][ok], fw["n_contrib"][ok])
+    rng = np.random.default_rng(12)
+    okf = ok.astype(np.float64)
+    gC, gA = rng.normal(size=(3, 16, 16)) * okf, rng.normal(size=(16, 16)) * okf
+    gD, gN = rng.normal(size=(16, 16)) * okf, rng.normal(size=(3, 16, 16)) * okf
+    mm = np.where(ok, m, 1).astype(np.uint8)
+    f32 = lambda a: a.astype(np.float32)
+    gg = g.render_bwd(gC=gC, gA=gA, gD=gD, gN=gN, mask=mm)
+    og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=f32(gC), gA=f32(gA), gD=f32(gD), gN=f32(gN))
+    check_grads(gg, og, skip_rows=pre["clamp_fragile"] != 0)
+    gg = g.render_bwd(gC=gC, gA=gA, mask=mm)
+    og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=f32(gC), gA=f32(gA))
+    check_grads(gg, og, skip_rows=pre["clamp_fragile"] != 0)
+    never = gf["vis_count"] == 0
+    for k in ("d_pos", "d_scale", "d_quat", "d_opacity", "d_sh"):
+        assert np.all(gg[k][never] == 0.0), k
 
 
 def test_sh_degrees():
