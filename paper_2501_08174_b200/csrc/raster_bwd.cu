@@ -13,10 +13,15 @@ constexpr int kNG = G_COUNT;  // 20 accumulated fields per list entry
 
 // sum of v[0..15] over the 32 lanes (16 shuffles); afterwards v[0] of lane L holds the total of value index
 // 8*bit4(L) + 4*bit3(L) + 2*bit2(L) + bit1(L), i.e. index L >> 1
+// kLast3Zero: v[13..15] are identically zero and their totals are not wanted (the colour / alpha-only backward instance): the
+// first step then needs no selects for the pairs (5,13), (6,14), (7,15) -- the upper half-warp ends up with copies of the
+// totals of 5..7 in the slots of 13..15, which the caller does not store.
+template <bool kLast3Zero = false>
 __device__ __forceinline__ void warp_transpose_reduce16(float* v, int lane) {
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     const bool up = lane & 16;
+    if (kLast3Zero && i >= 5) { v[i] += __shfl_xor_sync(0xFFFFFFFFu, v[i], 16); continue; }
     const float send = up ? v[i] : v[i + 8], keep = up ? v[i + 8] : v[i];
     v[i] = keep + __shfl_xor_sync(0xFFFFFFFFu, send, 16);
   }
@@ -247,22 +252,26 @@ __global__ void __launch_bounds__(128, kGeo ? kBwdMinBlocks : kBwdLeanMinBlocks)
         if ((m0 >> jb) & 1u) bwd_pair<kMoments, kGeo>(ps[0], idx, r0, r1, r2, r3, sr, kc, v, ex);
         if ((m1 >> jb) & 1u) bwd_pair<kMoments, kGeo>(ps[1], idx, r0, r1, r2, r3, sr, kc, v, ex);
         float* dst = acc + j * kNG;
-        warp_transpose_reduce16(v, lane);
-        if ((lane & 1) == 0) dst[lane >> 1] = v[0];
+        warp_transpose_reduce16<!kGeo>(v, lane);
+        if ((lane & 1) == 0 && (kGeo || lane < 26)) dst[lane >> 1] = v[0];  // !kGeo: fields 13..15 are zero and never read
         if (__any_sync(0xFFFFFFFFu, kGeo ? (ex[0] != 0.f) | (ex[1] != 0.f) | (ex[2] != 0.f) | (ex[3] != 0.f) : (ex[2] != 0.f) | (ex[3] != 0.f)))
           warp_transpose_reduce4(ex, lane);
-        if ((lane & 7) == 0) dst[16 + (lane >> 3)] = ex[0];  // without the reduction every lane's ex[0] is zero
+        if ((lane & 7) == 0 && (kGeo || lane >= 16)) dst[16 + (lane >> 3)] = ex[0];  // without the reduction every lane's ex[0] is zero
       }
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < cnt * kNG; i += 128) {
-      const int e = i / kNG;
+    // !kGeo: fields 13..17 (normal, D0, z_j) are identically zero: 15 of the 20 fields are flushed
+    constexpr int kNF = kGeo ? kNG : kNG - 5;
+    for (int i = threadIdx.x; i < cnt * kNF; i += 128) {
+      const int e = i / kNF;
+      int f = i - kNF * e;
+      if (!kGeo && f >= 13) f += 5;
       const uint32_t m = s_mask[e];
       float val = 0.f;
 #pragma unroll
       for (int w2 = 0; w2 < 4; ++w2)
-        if (m & (split ? 1u << (4 * part + w2) : ((1u << kBX) | 1u) << ((2 * (w2 / kBX)) * kBX + w2 % kBX))) val += s_acc[w2][i];
-      if (val != 0.f) atomicAdd(grad_rec + (size_t)s_rank[e] * kRec + (i - kNG * e), val);
+        if (m & (split ? 1u << (4 * part + w2) : ((1u << kBX) | 1u) << ((2 * (w2 / kBX)) * kBX + w2 % kBX))) val += s_acc[w2][e * kNG + f];
+      if (val != 0.f) atomicAdd(grad_rec + (size_t)s_rank[e] * kRec + f, val);
     }
   }
 }
