@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(128, kGeo ? kBwdMinBlocks : kBwdLeanMinBlocks)
   __shared__ uint32_t s_rank[kBwdBatch];
   __shared__ uint8_t s_mask[kBwdBatch];
   __shared__ uint32_t s_idx[kBwdBatch];   // position of the entry in the tile's full list (n_contrib counts those)
-  __shared__ float s_acc[4][kBwdBatch * kNG];
+  __shared__ __align__(16) float s_acc[4][kBwdBatch * kNG];
   static_assert(kBwdBatch == 64, "the per-warp entry masks below cover two 32-entry halves");
   // launch order: heavy tiles first (tile_order); the first `n_split` positions own two consecutive blocks each, so that a
   // tile with a long blended list can be walked by two CTAs (see kBwdHeavyLen)
@@ -260,18 +260,26 @@ __global__ void __launch_bounds__(128, kGeo ? kBwdMinBlocks : kBwdLeanMinBlocks)
       }
     }
     __syncthreads();
-    // !kGeo: fields 13..17 (normal, D0, z_j) are identically zero: 15 of the 20 fields are flushed
-    constexpr int kNF = kGeo ? kNG : kNG - 5;
-    for (int i = threadIdx.x; i < cnt * kNF; i += 128) {
-      const int e = i / kNF;
-      int f = i - kNF * e;
-      if (!kGeo && f >= 13) f += 5;
+    // flush: one 16-byte vector RED per (tile, entry, group of four fields); !kGeo: fields 13..17 (normal, D0, z_j) are
+    // identically zero and were never stored, so they are blanked here
+    static_assert(kNG % 4 == 0, "fields are flushed in groups of four");
+    constexpr int kNV = kNG / 4;
+    for (int i = threadIdx.x; i < cnt * kNV; i += 128) {
+      const int e = i / kNV, g4 = i - kNV * e;
       const uint32_t m = s_mask[e];
-      float val = 0.f;
+      float4 val = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
       for (int w2 = 0; w2 < 4; ++w2)
-        if (m & (split ? 1u << (4 * part + w2) : ((1u << kBX) | 1u) << ((2 * (w2 / kBX)) * kBX + w2 % kBX))) val += s_acc[w2][e * kNG + f];
-      if (val != 0.f) atomicAdd(grad_rec + (size_t)s_rank[e] * kRec + f, val);
+        if (m & (split ? 1u << (4 * part + w2) : ((1u << kBX) | 1u) << ((2 * (w2 / kBX)) * kBX + w2 % kBX))) {
+          const float4 a = *reinterpret_cast<const float4*>(&s_acc[w2][e * kNG + 4 * g4]);
+          val.x += a.x; val.y += a.y; val.z += a.z; val.w += a.w;
+        }
+      if (!kGeo) {
+        if (g4 == 3) val.y = val.z = val.w = 0.f;
+        if (g4 == 4) val.x = val.y = 0.f;
+      }
+      if (val.x != 0.f || val.y != 0.f || val.z != 0.f || val.w != 0.f)
+        atomicAdd(reinterpret_cast<float4*>(grad_rec + (size_t)s_rank[e] * kRec + 4 * g4), val);
     }
   }
 }
