@@ -27,8 +27,8 @@ FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 40.0, 22.0, 72.0  # DESIGN.md sectio
 FLOP_BLEND_BWD_COLOUR_ONLY = 54.0  # no upstream gradient on depth / normal maps (masked L1 + L_b): those terms are not evaluated
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the raster kernels, from the `ncu --set full` capture of this
 # workload committed as profiles/r01j_raster_kernels_full.md (bytes)
-NCU_TRAFFIC = {"render_bwd_kernel": 88.5e6, "render_fwd_kernel": 139.2e6}
-NCU_TRAFFIC_SOURCE = "profiles/r01l_raster_kernels_full.md"
+NCU_TRAFFIC = {"render_bwd_kernel": 90.0e6, "render_fwd_kernel": 139.2e6}
+NCU_TRAFFIC_SOURCE = "profiles/r01m_raster_kernels_full.md"
 ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 148 SMs x 128 FP32 lanes x 2 (FMA) x max SM clock (B200_PROFILING.md)
 
 

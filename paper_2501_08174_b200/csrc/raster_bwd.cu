@@ -225,9 +225,10 @@ __global__ void __launch_bounds__(128, kGeo ? kBwdMinBlocks : kBwdLeanMinBlocks)
       s_idx[threadIdx.x] = be.y >> 8;
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < cnt * 6; i += 128) {
-      const int e = i / 6, part = i - 6 * e;
-      s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
+    constexpr int kParts = kGeo ? 6 : 5;  // the last 16 bytes of a record hold the normal: not read without dL/dnormal
+    for (int i = threadIdx.x; i < cnt * kParts; i += 128) {
+      const int e = i / kParts, part = i - kParts * e;
+      s_rec[6 * e + part] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
     }
     // per warp: which entries of the batch did its two pixel blocks blend (bit e of lo: entry e, of hi: entry 32 + e)
     const uint32_t mlo = lane < cnt ? s_mask[lane] : 0u, mhi = lane + 32 < cnt ? s_mask[lane + 32] : 0u;
