@@ -125,9 +125,10 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
     if (kMaps && threadIdx.x < kFwdBatch) s_hit[threadIdx.x] = 0;
     if (kStats && threadIdx.x < kFwdBatch) { s_cnt[threadIdx.x] = 0; s_fix[threadIdx.x] = 0ull; }
     __syncthreads();
-    for (int i = threadIdx.x; i < cnt * 6; i += 256) {
-      const int e = i / 6, part = i - 6 * e;
-      s_rec[i] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
+    constexpr int kParts = kMaps ? 6 : 5;  // the last 16 bytes of a record hold the normal: not read by the statistics-only walk
+    for (int i = threadIdx.x; i < cnt * kParts; i += 256) {
+      const int e = i / kParts, part = i - kParts * e;
+      s_rec[6 * e + part] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
     }
     __syncthreads();
     // the batch in chunks of 32 entries: lane jj keeps the statistics of entry c0 + jj in registers
