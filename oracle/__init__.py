@@ -116,18 +116,12 @@ def _f64(a):
 # TILED path
 # --------------------------------------------------------------------------------------------------
 
-def _split_clamp(out):
-    """clamp: bits 0-2 = channel clamped at zero (S14); clamp_fragile: bits 0-2 = that decision is within the margin of an fp32
-    evaluation (S22 extended to the colour clamp; ocgs_oracle.cpp surfel_colour)."""
-    out["clamp_fragile"] = (out["clamp"] >> 4) & 7
-    out["clamp"] &= 7
-
-
-def clamp_matches(clamp_other, pre, rows=None) -> bool:
-    """Clamp bits of another implementation against the oracle's, on the channels whose decision is not fragile."""
-    rows = slice(None) if rows is None else rows
-    clear = (~pre["clamp_fragile"][rows]) & 7
-    return bool(np.array_equal(np.asarray(clamp_other)[rows] & clear, pre["clamp"][rows] & clear))
+def colour_probe(p, sh, degree: int, cam: OrcCamera):
+    """R-clamp: (fp32 decision values, fp64 values before the clamp, clamp bits) of one surfel's colour."""
+    p, sh = _f32(p).reshape(3), _f32(sh).reshape(16, 3)
+    a32, a64, cl = np.zeros(3, np.float32), np.zeros(3, np.float64), np.zeros(1, np.uint8)
+    lib().orc_colour_probe(_p(p), _p(sh), C.c_int(degree), C.byref(cam), _p(a32), _p(a64), _p(cl))
+    return a32, a64, int(cl[0])
 
 
 def preprocess(pos, scale, quat, opacity, sh, cam: OrcCamera, cfg: OrcConfig) -> Dict[str, np.ndarray]:
@@ -140,7 +134,6 @@ def preprocess(pos, scale, quat, opacity, sh, cam: OrcCamera, cfg: OrcConfig) ->
     lib().orc_preprocess(C.c_int(n), _p(pos), _p(scale), _p(quat), _p(opacity), _p(sh), C.byref(cam), C.byref(cfg),
                          _p(out["visible"]), _p(out["depth_bits"]), _p(out["rect"]), _p(out["tiles_touched"]), _p(out["M"]),
                          _p(out["c2d"]), _p(out["rho_cut"]), _p(out["normal"]), _p(out["rgb"]), _p(out["clamp"]))
-    _split_clamp(out)
     return out
 
 
@@ -277,7 +270,6 @@ def preprocess3d(pos, scale3, quat, opacity, sh, cam: OrcCamera, cfg: OrcConfig)
     lib().orc3d_preprocess(C.c_int(n), _p(pos), _p(scale3), _p(quat), _p(opacity), _p(sh), C.byref(cam), C.byref(cfg),
                            _p(out["visible"]), _p(out["depth_bits"]), _p(out["rect"]), _p(out["tiles_touched"]), _p(out["conic"]),
                            _p(out["c2d"]), _p(out["rho_cut"]), _p(out["rgb"]), _p(out["clamp"]))
-    _split_clamp(out)
     return out
 
 

@@ -249,24 +249,55 @@ inline void cross3(const double* a, const double* b, double* o) {
 inline uint32_t float_bits(float f) { uint32_t u; std::memcpy(&u, &f, 4); return u; }
 
 // colour (S14): rgb = max(0, 1/2 + sum_k Y_k(dir) sh_k), dir = normalise(p - cam_pos); clamp bit c set when channel c is clamped.
-// Bit 4 + c marks the decision of channel c as FRAGILE (S22, extended to the colour clamp): the unclamped value lies within
-// kClampMargin of zero, closer than an fp32 evaluation of the 16-term sum can resolve, so a kernel that takes the decision in
-// fp32 may take the other branch; tests compare the clamp bit and the gradients of such a surfel only where it is clear.
-constexpr double kClampMargin = 4e-6;
-void surfel_colour(const float* p, const float* sh, int degree, const double* campos, double* rgb, uint8_t* clamp) {
+// The clamp is a DECISION (zero gradient on clamped channels, S12), and where floating point decides a bit both sides take
+// the decision in the same precision: DESIGN.md reading R-clamp fixes the fp32 sequence below (IEEE-exact single operations
+// only: +, -, x, /, sqrt, fma; this file compiles with -ffp-contract=off).  The colour VALUE stays fp64 (surfel_colour).
+//   d = p - campos (campos: fp64 -R^T t of the fp32 view entries, rounded once);  n2 = fma(dx,dx, fma(dy,dy, dz*dz));
+//   len = sqrt(n2);  (x,y,z) = d / len;  xx = x*x, yy = y*y, zz = z*z;  K* = fp32 roundings of the closed forms of S14;
+//   Y0 = K0;  Y1 = (-K1)*y;  Y2 = K1*z;  Y3 = (-K1)*x;
+//   Y4 = (K2A*x)*y;  Y5 = ((-K2A)*y)*z;  Y6 = K2B*(fma(2,zz,-xx) - yy);  Y7 = ((-K2A)*x)*z;  Y8 = K2C*(xx - yy);
+//   Y9 = ((-K3A)*y)*fma(3,xx,-yy);  Y10 = ((K3B*x)*y)*z;  b = fma(4,zz,-xx) - yy;  Y11 = ((-K3C)*y)*b;
+//   Y12 = (K3D*z)*fma(-3,yy, fma(-3,xx, 2*zz));  Y13 = ((-K3C)*x)*b;  Y14 = (K3E*z)*(xx - yy);  Y15 = ((-K3A)*x)*fma(-3,yy,xx);
+//   acc_c = 1/2;  for k = 0 .. (degree+1)^2 - 1 in order: acc_c = fma(Y_k, sh[k][c], acc_c);   channel c clamped  <=>  acc_c < 0.
+void colour_f32(const float* p, const float* sh, int degree, const double* campos, float acc[3]) {
+  const float k0 = (float)SHC.c0, k1 = (float)SHC.c1, k2a = (float)SHC.c2a, k2b = (float)SHC.c2b, k2c = (float)SHC.c2c,
+              k3a = (float)SHC.c3a, k3b = (float)SHC.c3b, k3c = (float)SHC.c3c, k3d = (float)SHC.c3d, k3e = (float)SHC.c3e;
+  const float d0 = p[0] - (float)campos[0], d1 = p[1] - (float)campos[1], d2 = p[2] - (float)campos[2];
+  const float len = std::sqrt(std::fmaf(d0, d0, std::fmaf(d1, d1, d2 * d2)));
+  const float x = d0 / len, y = d1 / len, z = d2 / len;
+  const float xx = x * x, yy = y * y, zz = z * z;
+  float Y[16];
+  Y[0] = k0;
+  Y[1] = (-k1) * y; Y[2] = k1 * z; Y[3] = (-k1) * x;
+  Y[4] = (k2a * x) * y; Y[5] = ((-k2a) * y) * z; Y[6] = k2b * (std::fmaf(2.0f, zz, -xx) - yy); Y[7] = ((-k2a) * x) * z; Y[8] = k2c * (xx - yy);
+  const float b = std::fmaf(4.0f, zz, -xx) - yy;
+  Y[9] = ((-k3a) * y) * std::fmaf(3.0f, xx, -yy); Y[10] = ((k3b * x) * y) * z; Y[11] = ((-k3c) * y) * b;
+  Y[12] = (k3d * z) * std::fmaf(-3.0f, yy, std::fmaf(-3.0f, xx, 2.0f * zz)); Y[13] = ((-k3c) * x) * b; Y[14] = (k3e * z) * (xx - yy);
+  Y[15] = ((-k3a) * x) * std::fmaf(-3.0f, yy, xx);
+  const int nb = (degree + 1) * (degree + 1);
+  for (int c = 0; c < 3; ++c) {
+    float a = 0.5f;
+    for (int k = 0; k < nb; ++k) a = std::fmaf(Y[k], sh[3 * k + c], a);
+    acc[c] = a;
+  }
+}
+
+void surfel_colour(const float* p, const float* sh, int degree, const double* campos, double* rgb, uint8_t* clamp, double* unclamped = nullptr) {
   double v[3] = {p[0] - campos[0], p[1] - campos[1], p[2] - campos[2]};
   const double len = std::sqrt(dot3(v, v));
   double d[3] = {v[0] / len, v[1] / len, v[2] / len};
   double Y[16];
   sh_basis(d, Y, nullptr);
   const int nb = (degree + 1) * (degree + 1);
+  float dec[3];
+  colour_f32(p, sh, degree, campos, dec);
   *clamp = 0;
   for (int c = 0; c < 3; ++c) {
     double acc = 0.5;
     for (int k = 0; k < nb; ++k) acc += Y[k] * (double)sh[3 * k + c];
-    if (std::fabs(acc) <= kClampMargin) *clamp |= (uint8_t)(1u << (4 + c));
-    if (acc < 0.0) { acc = 0.0; *clamp |= (uint8_t)(1u << c); }
-    rgb[c] = acc;
+    if (unclamped) unclamped[c] = acc;
+    if (dec[c] < 0.0f) { acc = 0.0; *clamp |= (uint8_t)(1u << c); }  // the decision: R-clamp (fp32 sequence)
+    rgb[c] = acc < 0.0 ? 0.0 : acc;  // a channel the fp32 decision left open while the fp64 value is (by < 4e-6) negative
   }
 }
 
@@ -397,6 +428,14 @@ void orc_preprocess(int n, const float* pos, const float* scale, const float* qu
     surfel_normal(quat + 4 * j, V, pcd, normal + 3 * j);
     surfel_colour(pos + 3 * j, sh + 48 * j, cfg->sh_degree, campos, rgb + 3 * j, clamp + j);
   }
+}
+
+// pin access (tests/test_oracle_pins.py): the fp32 decision values of R-clamp beside the fp64 colour values before the clamp
+void orc_colour_probe(const float* p, const float* sh, int degree, const OrcCamera* cam, float* acc32, double* acc64, uint8_t* clamp) {
+  double campos[3], rgb[3];
+  cam_position(cam->view, campos);
+  colour_f32(p, sh, degree, campos, acc32);
+  surfel_colour(p, sh, degree, campos, rgb, clamp, acc64);
 }
 
 // ------------------------------------------------------------------------------------------------

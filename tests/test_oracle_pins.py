@@ -4,6 +4,7 @@ Each test names the passage / reading it pins.  Closed forms, invariants, specia
 results, brute force with an exhaustive per-pixel sort, and central finite differences.
 """
 import math
+from fractions import Fraction
 
 import numpy as np
 import pytest
@@ -56,24 +57,41 @@ def test_sh_sign_convention_degree1():
     assert Y[1] == pytest.approx(-c1)
 
 
-def test_colour_clamp_and_its_fragile_margin():
-    """S14 / S22: channel c is clamped iff 1/2 + sum Y sh < 0; the decision is marked fragile iff that value lies within 4e-6
-    of zero (what an fp32 evaluation cannot resolve).  Degree 0: the value is the requested rgb up to the fp32 rounding of sh."""
-    cam = ident_cam(32, 32, 50.0)
+def test_colour_clamp_decision_fp32_sequence():
+    """S14 / DESIGN.md reading R-clamp: channel c is clamped iff the fp32 sequence acc_c = fma(Y_k, sh_kc, acc_c) (k in order,
+    from 1/2) is negative.  Pins: (i) the fp32 values track the fp64 colour (whose basis the quadrature test above pins) to the
+    error of a 16-term fp32 sum, on random directions and coefficients and for every degree -- a wrong constant, sign or
+    polynomial in the fp32 basis moves them by 1e-2; (ii) wherever the fp64 value is clear of zero the decision is its
+    sign; (iii) degree 0 is exact: acc = fma(fl(Y0), sh_0, 1/2), so the requested colours below clamp exactly the channels
+    that are negative after the fp32 rounding of sh_0; (iv) a clamped channel's value is exactly 0, an open one's the fp64 value."""
+    rng = np.random.default_rng(7)
+    cam = orc.camera_from(sg.random_scene(4, 32, 32, 30.0, seed=1, sh_degree=0).cameras[0])  # a generic pose
+    worst = 0.0
+    for deg in (0, 1, 2, 3):
+        for _ in range(1500):
+            p = rng.normal(size=3) * 2.0
+            sh = rng.normal(size=(16, 3)) * 0.6
+            a32, a64, cl = orc.colour_probe(p, sh, deg, cam)
+            worst = max(worst, float(np.abs(a32 - a64).max()))
+            for c in range(3):
+                if abs(a64[c]) > 4e-6:
+                    assert bool(cl >> c & 1) == (a64[c] < 0)
+                assert bool(cl >> c & 1) == (a32[c] < 0)
+    assert worst < 4e-6
+    # degree 0, by hand
+    y0f = np.float32(Y0)
+    for rgb in ((-1e-3, 1e-3, 0.5), (-1e-6, 1e-6, -0.2), (0.0, -3e-7, 3e-7), (-1e-5, 1e-5, 2.0)):
+        s = one_surfel((0.3, -0.2, 2.0), (0.1, 0.1), rgb=rgb)
+        a32, a64, cl = orc.colour_probe(s[0][0], s[4][0], 0, ident_cam(32, 32, 50.0))
+        expect = [float(Fraction(float(y0f)) * Fraction(float(s[4][0, 0, c])) + Fraction(1, 2)) for c in range(3)]  # one rounding of the exact value
+        assert [float(v) for v in a32] == [float(np.float32(e)) for e in expect]
+        assert cl == sum(1 << c for c in range(3) if np.float32(expect[c]) < 0)
     cfg = orc.default_config(sh_degree=0)
-    rgbs = [(-1e-3, 1e-3, 0.5), (-1e-6, 1e-6, -0.2), (0.0, -3e-6, 3e-6), (-1e-5, 1e-5, 2.0)]
-    s = stack(*[one_surfel((0, 0, 2.0), (0.1, 0.1), rgb=c) for c in rgbs])
-    pre = orc.preprocess(*s, cam, cfg)
-    assert list(pre["clamp"]) == [0b001, 0b101, int(pre["clamp"][2]) & 0b001 | 0b010, 0b001]
-    assert list(pre["clamp_fragile"]) == [0b000, 0b011, 0b111, 0b000]
-    assert np.all(pre["rgb"] >= 0.0) and np.allclose(pre["rgb"][0], [0.0, 1e-3, 0.5], atol=1e-7)
-    # clamp_matches: a disagreement counts only on channels whose decision is clear
-    other = pre["clamp"].copy(); other[1] ^= 0b011
-    assert orc.clamp_matches(other, pre)
-    other[1] ^= 0b100
-    assert not orc.clamp_matches(other, pre)
-    other = pre["clamp"].copy(); other[0] ^= 0b001
-    assert not orc.clamp_matches(other, pre) and orc.clamp_matches(other, pre, rows=np.array([False, True, True, True]))
+    s = stack(*[one_surfel((0, 0, 2.0), (0.1, 0.1), rgb=c) for c in ((-1e-3, 1e-3, 0.5), (0.25, -0.5, 0.0))])
+    pre = orc.preprocess(*s, ident_cam(32, 32, 50.0), cfg)
+    assert list(pre["clamp"][:2]) == [0b001, 0b010 | (int(pre["clamp"][1]) & 0b100)]
+    assert pre["rgb"][0, 0] == 0.0 and pre["rgb"][1, 1] == 0.0 and np.all(pre["rgb"] >= 0.0)
+    assert np.allclose(pre["rgb"][0], [0.0, 1e-3, 0.5], atol=1e-7)
 
 
 # ---------------------------------------------------------------------------------------------
@@ -527,6 +545,73 @@ def test_backward_matches_finite_differences_sh3():
 def test_backward_matches_finite_differences_small_surfels_filter_active():
     # sub-pixel surfels: the screen-space filter branch (S8) and its gradient to the centre are exercised
     _fd_check(seed=22, n=8, W=16, H=16, f=18.0, sh_degree=1, scale_lo=0.01, scale_hi=0.08)
+
+
+def test_d_center2d_reading_r_c2d():
+    """DESIGN.md reading R-c2d (the densification statistic): d_center2d = dL/d(projected centre) at fixed view
+    depth = M22 (dL/dM02, dL/dM12).  Pins: (i) central differences on the BF forward of a shift of the surfel centre by
+    delta pixels in the image plane at fixed depth (p_c += (delta z/fx, 0, 0) resp. (0, delta z/fy, 0), mapped back to the
+    world) on a scene of sub-pixel surfels, where the filter branch (S8) and its -4 d g_rho term are active; SH degree 0,
+    so the colour does not move with the position; (ii) identity camera: p_c = p, M02 = fx p_x + ox p_z, so
+    d_center2d = (z/fx, z/fy) * d_pos[:, :2] exactly -- d_pos itself is pinned by the finite-difference tests above."""
+    n, W, H, f = 8, 16, 16, 18.0
+    sc = sg.random_scene(n, W, H, f, seed=22, sh_degree=0, scale_lo=0.01, scale_hi=0.08)
+    camn = sc.cameras[0]
+    cam = orc.camera_from(camn)
+    cfg = orc.default_config(sh_degree=0, bg=(0.2, 0.4, 0.1))
+    m = sc.mask(0)
+    rng = np.random.default_rng(5)
+    wC, wA, wD, wN = rng.normal(size=(3, H, W)), rng.normal(size=(H, W)), rng.normal(size=(H, W)), rng.normal(size=(3, H, W))
+    pos64 = sc.pos.astype(np.float64)
+    others = [a.astype(np.float64) for a in (sc.scale, sc.quat, sc.opacity, sc.sh)]
+
+    def loss(pos):
+        r = orc.bf_render(pos, *others, cam, cfg, mask=m, want_stats=False)
+        return ((wC * r["color"]).sum() + (wA * r["alpha"]).sum() + (wD * r["depth"]).sum() + (wN * r["normal"]).sum()
+                + cfg.gamma_bg * r["loss_bg"]), r["n_blended"]
+
+    pre = orc.preprocess(sc.pos, sc.scale, sc.quat, sc.opacity, sc.sh, cam, cfg)
+    srt = orc.bin_sort(pre, cam, cfg)
+    fw = orc.render_fwd(pre, srt, sc.opacity, cam, cfg, mask=m, want_fragile=False)
+    g = orc.render_bwd(sc.pos, sc.scale, sc.quat, sc.opacity, sc.sh, pre, srt, cam, cfg, mask=m, gC=wC, gA=wA, gD=wD, gN=wN)
+    V = np.asarray(camn.view, np.float64).reshape(4, 4)
+    Rwc = V[:3, :3]
+    checked = 0
+    filter_seen = False
+    for j in range(n):
+        if not pre["visible"][j] or fw["vis_count"][j] == 0:
+            assert np.all(g["d_center2d"][j] == 0.0)
+            continue
+        z = float((V[:3, :3] @ pos64[j] + V[:3, 3])[2])
+        for ax, fl in ((0, camn.fx), (1, camn.fy)):
+            h = 1e-5
+            e = np.zeros(3); e[ax] = z / fl          # one pixel along the image axis at depth z, in camera coordinates
+            dw = Rwc.T @ e                            # ... in world coordinates
+            pp, pm = pos64.copy(), pos64.copy()
+            pp[j] += h * dw; pm[j] -= h * dw
+            Lp, np_ = loss(pp); Lm, nm_ = loss(pm)
+            if not np.array_equal(np_, nm_):
+                continue
+            fd = (Lp - Lm) / (2 * h)
+            an = g["d_center2d"][j, ax]
+            assert abs(fd - an) <= 2e-4 * max(1e-3, abs(fd), np.abs(g["d_center2d"][j]).max()), (j, ax, fd, an)
+            checked += 1
+        # the filter term was active for this surfel somewhere: sigma_px = f s / z below sigma_f for the small ones
+        filter_seen |= bool(f * sc.scale[j].min() / z < 0.7)
+    assert checked >= 8 and filter_seen
+    # (ii) identity camera
+    s = stack(one_surfel((0.13, -0.07, 2.0), (0.1, 0.06), quat=(0.9, 0.1, 0.3, 0.2)), one_surfel((-0.2, 0.1, 2.5), (0.004, 0.004)))
+    s = (s[0], s[1], s[2] / np.linalg.norm(s[2], axis=1, keepdims=True).astype(np.float32), s[3], s[4])
+    cam = ident_cam(24, 20, 30.0)
+    cfg = orc.default_config(sh_degree=0)
+    pre = orc.preprocess(*s, cam, cfg)
+    srt = orc.bin_sort(pre, cam, cfg)
+    rng = np.random.default_rng(6)
+    g = orc.render_bwd(*s, pre, srt, cam, cfg, gC=rng.normal(size=(3, 20, 24)), gA=rng.normal(size=(20, 24)), gD=rng.normal(size=(20, 24)))
+    assert np.abs(g["d_center2d"]).min() > 0
+    for j in range(2):
+        z = float(s[0][j, 2])
+        assert np.allclose(g["d_center2d"][j], z / 30.0 * g["d_pos"][j, :2], rtol=1e-12, atol=0)
 
 
 def test_prune_and_compaction_definition():
