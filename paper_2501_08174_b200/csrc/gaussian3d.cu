@@ -107,34 +107,8 @@ __global__ void __launch_bounds__(256) preprocess3d_kernel(const float* __restri
       const int tx0 = pr.ix0 >> 4, tx1 = (pr.ix1 >> 4) + 1, ty0 = pr.iy0 >> 4, ty1 = (pr.iy1 >> 4) + 1;
       nt = (uint32_t)((tx1 - tx0) * (ty1 - ty0));
       rect[j] = make_ushort4((unsigned short)pr.ix0, (unsigned short)pr.iy0, (unsigned short)pr.ix1, (unsigned short)pr.iy1);
-      float dx = p[0] - cam.campos[0], dy = p[1] - cam.campos[1], dz = p[2] - cam.campos[2];
-      const float inv = rsqrtf(dx * dx + dy * dy + dz * dz);
-      dx *= inv; dy *= inv; dz *= inv;
-      float Y[16];
-#pragma unroll
-      for (int k = 0; k < 16; ++k) Y[k] = 0.f;
-      sh_basis(dx, dy, dz, cfg.sh_degree, Y);
-      const int nb = (cfg.sh_degree + 1) * (cfg.sh_degree + 1);
-      float colr[3] = {0.5f, 0.5f, 0.5f};
-      const float4* shj = sh + (size_t)j * 12;
-      const int nvec = (3 * nb + 3) / 4;
-#pragma unroll
-      for (int v4 = 0; v4 < 12; ++v4) {
-        if (v4 >= nvec) break;
-        const float4 f = __ldg(shj + v4);
-        const float ff[4] = {f.x, f.y, f.z, f.w};
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const int idx = 4 * v4 + e;
-          if (idx < 3 * nb) {
-            const int k = idx / 3, c = idx - 3 * k;
-            colr[c] = fmaf(Y[k], ff[e], colr[c]);
-          }
-        }
-      }
-#pragma unroll
-      for (int c = 0; c < 3; ++c)
-        if (colr[c] < 0.0f) { colr[c] = 0.0f; cl |= (uint8_t)(1u << c); }
+      float colr[3];
+      cl = sh_colour_rn(p, sh + (size_t)j * 12, cam, cfg.sh_degree, colr);  // reading R-clamp: the fixed fp32 colour sequence
       float4* out = rec_id + (size_t)j * 6;
       out[0] = make_float4(pr.conic[0], pr.conic[1], pr.conic[2], 0.f);
       out[1] = make_float4(0.f, 0.f, 0.f, 0.f);

@@ -77,33 +77,8 @@ __global__ void __launch_bounds__(256) preprocess_kernel(const float* __restrict
       ny = cam.V[4] * tw0 + cam.V[5] * tw1 + cam.V[6] * tw2;
       nz = cam.V[8] * tw0 + cam.V[9] * tw1 + cam.V[10] * tw2;
       if (nx * pr.pc[0] + ny * pr.pc[1] + nz * pr.pc[2] > 0.0f) { nx = -nx; ny = -ny; nz = -nz; }
-      // SH colour (S14)
-      float dx = p[0] - cam.campos[0], dy = p[1] - cam.campos[1], dz = p[2] - cam.campos[2];
-      const float inv = rsqrtf(dx * dx + dy * dy + dz * dz);
-      dx *= inv; dy *= inv; dz *= inv;
-      float Y[16];
-      sh_basis(dx, dy, dz, cfg.sh_degree, Y);
-      const int nb = (cfg.sh_degree + 1) * (cfg.sh_degree + 1);
-      col[0] = col[1] = col[2] = 0.5f;
-      const float4* shj = sh + (size_t)id * 12;
-      const int nvec = (3 * nb + 3) / 4;
-#pragma unroll
-      for (int v4 = 0; v4 < 12; ++v4) {
-        if (v4 >= nvec) break;
-        const float4 f = __ldg(shj + v4);
-        const float ff[4] = {f.x, f.y, f.z, f.w};
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const int idx = 4 * v4 + e;
-          if (idx < 3 * nb) {
-            const int k = idx / 3, c = idx - 3 * k;
-            col[c] = fmaf(Y[k], ff[e], col[c]);
-          }
-        }
-      }
-#pragma unroll
-      for (int c = 0; c < 3; ++c)
-        if (col[c] < 0.0f) { col[c] = 0.0f; cl |= (uint8_t)(1u << c); }
+      // SH colour (S14); the clamp decision follows the fixed fp32 sequence of reading R-clamp
+      cl = sh_colour_rn(p, sh + (size_t)id * 12, cam, cfg.sh_degree, col);
     }
     {
       // centred record (common.cuh): P, Q, R, D0 in fp64 from the fp32 M, rounded once

@@ -120,6 +120,63 @@ __device__ __forceinline__ void sh_basis(float x, float y, float z, int degree, 
   Y[14] = SH_K3E * z * (xx - yy); Y[15] = -SH_K3A * x * (xx - 3.0f * yy);
 }
 
+// DESIGN.md reading R-clamp: the colour sum whose sign decides the clamp bit is a FIXED fp32 sequence (round-to-nearest
+// intrinsics only, so nvcc can neither contract nor re-associate it): dir = (p - campos) / sqrt(fma(dx,dx, fma(dy,dy, dz dz))),
+// the basis below with the multiplication order written out, then acc_c = fma(Y_k, sh[k][c], acc_c) for k in order from 1/2.
+__device__ __forceinline__ void sh_basis_rn(float x, float y, float z, int degree, float* Y) {
+  Y[0] = SH_K0;
+  if (degree < 1) return;
+  Y[1] = __fmul_rn(-SH_K1, y); Y[2] = __fmul_rn(SH_K1, z); Y[3] = __fmul_rn(-SH_K1, x);
+  if (degree < 2) return;
+  const float xx = __fmul_rn(x, x), yy = __fmul_rn(y, y), zz = __fmul_rn(z, z);
+  const float xx_yy = __fsub_rn(xx, yy);
+  Y[4] = __fmul_rn(__fmul_rn(SH_K2A, x), y);
+  Y[5] = __fmul_rn(__fmul_rn(-SH_K2A, y), z);
+  Y[6] = __fmul_rn(SH_K2B, __fsub_rn(__fmaf_rn(2.0f, zz, -xx), yy));
+  Y[7] = __fmul_rn(__fmul_rn(-SH_K2A, x), z);
+  Y[8] = __fmul_rn(SH_K2C, xx_yy);
+  if (degree < 3) return;
+  const float b = __fsub_rn(__fmaf_rn(4.0f, zz, -xx), yy);
+  Y[9] = __fmul_rn(__fmul_rn(-SH_K3A, y), __fmaf_rn(3.0f, xx, -yy));
+  Y[10] = __fmul_rn(__fmul_rn(__fmul_rn(SH_K3B, x), y), z);
+  Y[11] = __fmul_rn(__fmul_rn(-SH_K3C, y), b);
+  Y[12] = __fmul_rn(__fmul_rn(SH_K3D, z), __fmaf_rn(-3.0f, yy, __fmaf_rn(-3.0f, xx, __fmul_rn(2.0f, zz))));
+  Y[13] = __fmul_rn(__fmul_rn(-SH_K3C, x), b);
+  Y[14] = __fmul_rn(__fmul_rn(SH_K3E, z), xx_yy);
+  Y[15] = __fmul_rn(__fmul_rn(-SH_K3A, x), __fmaf_rn(-3.0f, yy, xx));
+}
+
+// SH colour of one surfel (S14) by the R-clamp sequence: col[c] = max(0, acc_c), bit c of the result set iff acc_c < 0
+__device__ __forceinline__ uint8_t sh_colour_rn(const float p[3], const float4* __restrict__ shj, const CamParams& cam, int degree, float col[3]) {
+  const float d0 = __fsub_rn(p[0], cam.campos[0]), d1 = __fsub_rn(p[1], cam.campos[1]), d2 = __fsub_rn(p[2], cam.campos[2]);
+  const float len = __fsqrt_rn(__fmaf_rn(d0, d0, __fmaf_rn(d1, d1, __fmul_rn(d2, d2))));
+  const float x = __fdiv_rn(d0, len), y = __fdiv_rn(d1, len), z = __fdiv_rn(d2, len);
+  float Y[16];
+  sh_basis_rn(x, y, z, degree, Y);
+  const int nb = (degree + 1) * (degree + 1);
+  col[0] = col[1] = col[2] = 0.5f;
+  const int nvec = (3 * nb + 3) / 4;
+#pragma unroll
+  for (int v4 = 0; v4 < 12; ++v4) {
+    if (v4 >= nvec) break;
+    const float4 f = __ldg(shj + v4);
+    const float ff[4] = {f.x, f.y, f.z, f.w};
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const int idx = 4 * v4 + e;
+      if (idx < 3 * nb) {
+        const int k = idx / 3, c = idx - 3 * k;  // per channel the terms arrive in ascending k
+        col[c] = __fmaf_rn(Y[k], ff[e], col[c]);
+      }
+    }
+  }
+  uint8_t cl = 0;
+#pragma unroll
+  for (int c = 0; c < 3; ++c)
+    if (col[c] < 0.0f) { col[c] = 0.0f; cl |= (uint8_t)(1u << c); }
+  return cl;
+}
+
 // gradient of sum_k a_k Y_k(x,y,z) w.r.t. (x,y,z), the polynomials taken with x,y,z independent
 __device__ __forceinline__ void sh_basis_grad(float x, float y, float z, int degree, const float* a, float* g) {
   g[0] = g[1] = g[2] = 0.0f;

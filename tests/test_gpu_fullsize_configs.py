@@ -74,15 +74,23 @@ def windows_parity(sc, view, windows, key_capacity, rng_seed=11):
     return dict(K=srt["K"], n_vis=int(vis.sum()), grads=rep, ranges=srt["ranges"])
 
 
-def test_config5_full_size_sampled_windows():
-    """4 M surfels, 1920x1080: 1080 = 67.5 x 16, so the last tile row is half empty (ragged tail), tile lists up to
-    ~15 k entries (many 128-entry batches per tile), 4.3 M keys through both radix stages."""
+def test_config5_full_size_full_image():
+    """4 M surfels, 1920x1080: 1080 = 67.5 x 16, so the last tile row is half empty (ragged tail), tile lists of thousands of
+    entries (many batches per tile), 4.3 M keys through both radix stages.  Every pixel of a view, every output (see
+    full_parity), the prune mask from its statistics and the step bench.py times."""
     sc = sg.make_scene("config5")
-    W, H = 1920, 1080
-    windows = [(0, 0, 48, 48), (936, 516, 984, 564), (W - 48, H - 40, W, H), (608, H - 24, 656, H), (1300, 300, 1332, 332)]
-    r = windows_parity(sc, 0, windows, key_capacity=16 * sc.n)
+    r = full_parity(sc, 0, dict(sh_degree=3), key_capacity=16 * sc.n, max_fragile=3e-3, check_prune=True, bench_step=True, label="config5")
     L = r["ranges"][:, 1] - r["ranges"][:, 0]
     assert r["K"] > 2_000_000 and L.max() > 4096
+
+
+def test_config5_heaviest_view_forward_and_colour_backward():
+    """The view of config 5 with the longest tile list (view 7: one tile of 25 338 entries, the heavy-tile walk of both raster
+    kernels): every pixel of the forward outputs and the colour / alpha-only backward instance."""
+    sc = sg.make_scene("config5")
+    r = full_parity(sc, 7, dict(sh_degree=3), key_capacity=16 * sc.n, max_fragile=3e-3, label="config5-heaviest")
+    L = r["ranges"][:, 1] - r["ranges"][:, 0]
+    assert L.max() > 20_000
 
 
 def test_config4_full_size_all_views_prune():
@@ -138,7 +146,10 @@ def test_config4_full_size_all_views_prune():
     po2 = orc.prune(vis_o, cs_o.astype(np.float32), sc.opacity)
     assert np.array_equal(pm[clean], po2["prune_mask"][clean])
     # surfels whose only blends fell on fragile pixels may legitimately differ (S22); there must be almost none
-    assert (pm != po2["prune_mask"]).sum() <= 8
+    n_diff = int((pm != po2["prune_mask"]).sum())
+    print("PARITY config4: prune mask differs from the mask of the oracle's own statistics on %d of %d surfels; %d surfels touch a fragile pixel in some view"
+          % (n_diff, n, int((~clean).sum())))
+    assert n_diff <= 8
     comp = orc.compact(dict(pos=sc.pos, scale=sc.scale, quat=sc.quat, opacity=sc.opacity, sh=sc.sh), pm)
     k = po["n_out"]
     for t, name in zip(outs, ("pos", "scale", "quat", "opacity", "sh")):

@@ -18,12 +18,20 @@ def arrays(sc):
     return (sc.pos, sc.scale, sc.quat, sc.opacity, sc.sh)
 
 
-def full_parity(sc, view, cfg_kw, rng_seed=5, max_fragile=2e-3, with_bwd=True):
+def full_parity(sc, view, cfg_kw, rng_seed=5, max_fragile=2e-3, with_bwd=True, key_capacity=None, check_prune=False, bench_step=False,
+                max_illcond_err=1e-3, label=None):
+    """One view through the five C-ABI calls against the oracle, EVERY output, every pixel, every surfel.
+
+    check_prune: the prune mask, remap and compaction from this view's statistics (a5) against the oracle's rule.
+    bench_step:  additionally the step bench.py times -- ocgs_render_fwd_l1 (masked L1 fused, dL/dcolor made in-kernel) + the
+                 colour / alpha-only backward instance -- against the oracle fed with ITS OWN dL/dC = M sign(R - I)/(3HW),
+                 target I = the oracle's render of the perturbed copy.
+    Prints one line of measured numbers (fragile fraction, worst errors, strict-rule misses); pytest -s shows it."""
     P = arrays(sc)
     camn = sc.cameras[view]
     m = sc.mask(view)
     orc, cam, cfg, pre, srt, fw = oracle_view(P, camn, cfg_kw, mask=m)
-    g = GpuView(P, camn, cfg_kw)
+    g = GpuView(P, camn, cfg_kw, key_capacity=key_capacity)
     # (1) preprocess: integer outputs bit-exact
     gp = g.preprocess()
     vis = pre["visible"] == 1
@@ -46,7 +54,7 @@ def full_parity(sc, view, cfg_kw, rng_seed=5, max_fragile=2e-3, with_bwd=True):
         ref = np.concatenate([Pq, Qq, Rq, (m2 * Rq).sum(1, keepdims=True)], 1)
         # (the kernel forms them in fp64 with fused multiply-adds, numpy without: equal to an fp32 ulp of the row scale)
         assert np.all(np.abs(rec[:, 0:10] - ref) <= 2e-7 * np.abs(ref).max(1, keepdims=True))
-        assert np.abs(rec[:, 17:20] - pre["rgb"][vis]).max() < 2e-5
+        assert np.abs(rec[:, 17:20] - pre["rgb"][vis]).max() < 4e-6  # fp32 colour sum against the fp64 value (R-clamp bound)
         assert np.abs(rec[:, 20:23] - pre["normal"][vis]).max() < 2e-6
     # (2) bin_sort: keys, order, ranges bit-exact
     gs = g.bin_sort()
@@ -54,14 +62,21 @@ def full_parity(sc, view, cfg_kw, rng_seed=5, max_fragile=2e-3, with_bwd=True):
     assert np.array_equal(gs["ids"], srt["ids"])
     assert np.array_equal(gs["tile_keys"], (srt["keys"] >> np.uint64(32)).astype(np.uint32))
     assert np.array_equal(gs["ranges"], srt["ranges"])
-    # (3) forward
+    # (3) forward: every pixel.  fragile bit 0 = a decision within its margin (the two sides may take different branches:
+    # bounded by the discontinuity jump 0.02); bit 1 only = ill-conditioned pair evaluation, nothing discontinuous: 10 x tolerance
     gf = g.render_fwd(mask=m)
     ok = fw["fragile"] == 0
-    assert 1.0 - ok.mean() <= max_fragile, f"fragile fraction {1 - ok.mean()}"
+    illc = fw["fragile"] == 2
+    frag_frac = float(1.0 - ok.mean())
+    assert frag_frac <= max_fragile, f"fragile fraction {frag_frac}"
+    worst = {}
     for k in ("color", "alpha", "depth", "normal"):
         scale = np.maximum(1.0, np.abs(fw[k])) if k == "depth" else 1.0
         err = np.abs(gf[k] - fw[k]) / scale
-        assert (err * ok).max() <= IMG_TOL, (k, (err * ok).max())
+        worst[k] = float((err * ok).max())
+        worst[k + "_illcond"] = float((err * illc).max())
+        assert worst[k] <= IMG_TOL, (k, worst[k])
+        assert worst[k + "_illcond"] <= max_illcond_err, (k, "ill-conditioned pixel", worst[k + "_illcond"])
         assert err.max() <= 0.02, (k, "fragile pixel beyond the discontinuity bound", err.max())
     assert np.array_equal(gf["n_contrib"][ok], fw["n_contrib"][ok])
     assert abs(gf["loss_bg"] - fw["loss_bg"]) <= IMG_TOL
@@ -70,6 +85,34 @@ def full_parity(sc, view, cfg_kw, rng_seed=5, max_fragile=2e-3, with_bwd=True):
     clean = fw["fragile_touch"] == 0
     assert np.array_equal(gf["vis_count"][clean], fw["vis_count"][clean])
     assert np.allclose(gf["contrib_sum"][clean], fw["contrib_sum"][clean], rtol=1e-4, atol=2e-6)
+    info = dict(fragile=frag_frac, K=srt["K"], worst=worst, loss_bg_err=abs(gf["loss_bg"] - fw["loss_bg"]),
+                vis_count_diff_surfels=int((dv != 0).sum()))
+    if check_prune:
+        # (3b) a5 from this view's statistics: mask / remap / count bit-exact against the oracle's rule on the same statistics,
+        # and against the oracle's OWN statistics wherever no fragile pixel was involved; compaction by its definition
+        import torch
+        B = g.B
+        n = g.n
+        mask_t = torch.empty(n, dtype=torch.uint8, device="cuda"); remap_t = torch.empty(n, dtype=torch.int32, device="cuda")
+        n_out = torch.zeros(1, dtype=torch.int32, device="cuda")
+        outs = [torch.full_like(t, -7.0) for t in (g.t["pos"], g.t["scale"], g.t["quat"], g.t["opacity"], g.t["sh"])]
+        om = B.ocgs_surfels_mut(*[B._ptr(t) for t in outs], n)
+        pws = torch.empty(B.ocgs_prune_workspace_bytes(n), dtype=torch.uint8, device="cuda")
+        B.ocgs_prune_stats(g.surfels, g.vis, g.cs, g.cfg, mask_t, remap_t, om, n_out, 0, pws)
+        torch.cuda.synchronize()
+        pm = mask_t.cpu().numpy()
+        po = orc.prune(gf["vis_count"], gf["contrib_sum"], sc.opacity)
+        assert np.array_equal(pm, po["prune_mask"]) and np.array_equal(remap_t.cpu().numpy(), po["remap"]) and int(n_out.item()) == po["n_out"]
+        po2 = orc.prune(fw["vis_count"], fw["contrib_sum"].astype(np.float32), sc.opacity)
+        assert np.array_equal(pm[clean], po2["prune_mask"][clean])
+        info["prune_mask_diff"] = int((pm != po2["prune_mask"]).sum())
+        assert info["prune_mask_diff"] <= max(2, int(1e-5 * n))
+        comp = orc.compact(dict(pos=sc.pos, scale=sc.scale, quat=sc.quat, opacity=sc.opacity, sh=sc.sh), pm)
+        for t, name in zip(outs, ("pos", "scale", "quat", "opacity", "sh")):
+            got = t.cpu().numpy()
+            assert np.array_equal(got[:po["n_out"]], comp[name]), name
+            assert np.all(got[po["n_out"]:] == -7.0), name
+        del outs, om
     rep = None
     if with_bwd:
         # (4) backward: seeded N(0,1) upstream on all four maps, zero on fragile pixels (both sides see the same inputs)
@@ -86,12 +129,70 @@ def full_parity(sc, view, cfg_kw, rng_seed=5, max_fragile=2e-3, with_bwd=True):
         # the colour / alpha-only instance of the kernel (no upstream gradient on the depth and normal maps)
         gg2 = g.render_bwd(gC=gC, gA=gA, mask=mm)
         og2 = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=gC.astype(np.float32), gA=gA.astype(np.float32))
-        check_grads(gg2, og2)
+        rep2 = check_grads(gg2, og2)
         # surfels never blended receive exactly zero gradient
         never = gf["vis_count"] == 0
         for k in ("d_pos", "d_scale", "d_quat", "d_opacity", "d_sh"):
             assert np.all(gg[k][never] == 0.0), k
-    return dict(fragile=float(1 - ok.mean()), grads=rep, K=srt["K"])
+        info["grads"] = {k: (v["strict_fail_frac"], v["worst_strict_rel"], v["worst_block_rel"]) for k, v in rep.items()}
+        info["grads_colour_alpha"] = {k: (v["strict_fail_frac"], v["worst_strict_rel"], v["worst_block_rel"]) for k, v in rep2.items()}
+    if bench_step:
+        info["bench_step"] = bench_step_parity(sc, view, g, orc, cam, cfg, pre, srt, fw, gf, m)
+    print(f"PARITY {label or sc.name} n={sc.n} {camn.width}x{camn.height} view {view}: {info}")
+    return dict(fragile=frag_frac, grads=rep, K=srt["K"], info=info, ranges=srt["ranges"])
+
+
+def bench_step_parity(sc, view, g, orc, cam, cfg, pre, srt, fw, gf, m):
+    """The step bench.py times: ocgs_render_fwd_l1 + ocgs_render_bwd with dL/dcolor only (render_bwd_kernel<false,false>)."""
+    import torch
+    B = g.B
+    P = arrays(sc)
+    H, W = g.H, g.W
+    HW3 = 3.0 * H * W
+    # target image (Appendix B): the oracle's render of the perturbed copy
+    pt = sc.perturbed()
+    _, _, _, _, _, tw = oracle_view(arrays(pt), sc.cameras[view], dict(sh_degree=sc.sh_degree), mask=m)
+    target = tw["color"].astype(np.float32)
+    tt = torch.tensor(target, device="cuda")
+    o2 = B.alloc_outputs(W, H)
+    gC_t = torch.full_like(tt, 9.0); l1 = torch.zeros(1, device="cuda")
+    vis_f = torch.zeros(g.n, dtype=torch.int32, device="cuda"); cs_f = torch.zeros(g.n, device="cuda")
+    B.ocgs_render_fwd_l1(g.n, g.cam, g.cfg, g.ws, g.cap, g.mask_t, tt, o2["color"], o2["alpha"], o2["depth"], o2["normal"], o2["n_contrib"],
+                         o2["loss_bg"], l1, gC_t, vis_f, cs_f)
+    grads = B.alloc_grads(g.n)
+    B.ocgs_render_bwd(g.surfels, g.cam, g.cfg, g.ws, g.cap, g.mask_t, o2["n_contrib"], gC_t, None, None, None, grads["d_pos"], grads["d_scale"],
+                      grads["d_quat"], grads["d_opacity"], grads["d_sh"], grads["d_center2d"])
+    torch.cuda.synchronize()
+    # the fused forward writes the same maps, statistics and L_b as the plain forward
+    for k in ("color", "alpha", "depth", "normal"):
+        assert np.array_equal(o2[k].cpu().numpy(), gf[k]), k
+    assert float(o2["loss_bg"].item()) == gf["loss_bg"] and np.array_equal(vis_f.cpu().numpy().view(np.uint32), gf["vis_count"])
+    # masked L1 (S20) against the oracle's own maps
+    ok = fw["fragile"] == 0
+    diff = (fw["color"] - target.astype(np.float64)) * (m[None] > 0)
+    l1_o = np.abs(diff).sum() / HW3
+    assert abs(float(l1.item()) - l1_o) <= 1e-4 * max(1.0, l1_o)
+    gC_o = np.sign(diff) / HW3
+    gC_g = gC_t.cpu().numpy().astype(np.float64)
+    clear = ok[None] & (np.abs(diff) > 2e-4)  # the sign of R - I is a decision: compared where it is clear on both sides
+    assert np.array_equal(np.sign(gC_g)[clear], np.sign(gC_o)[clear])
+    assert np.all(np.isin(np.round(np.abs(gC_g) * HW3, 3), (0.0, 1.0)))
+    # (a) the whole step: GPU-made dL/dC -> GPU backward against oracle-made dL/dC -> oracle backward.  The few pixels whose sign
+    # differs (|R - I| below fp32 resolution) and the fragile pixels move an entry by O(1/(3HW)) x w, far below the 1e-6 floor
+    og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=m, gC=gC_o.astype(np.float32))
+    gg = {k: v.cpu().numpy() for k, v in grads.items()}
+    rep = check_grads(gg, og)
+    # (b) every entry of this step is O(pixels / (3HW)), mostly below north_star's floor, so the colour / alpha-only instance is
+    # also run on the oracle's dL/dC (zero on fragile pixels, both sides the same input) and compared with the floor at 1e-9:
+    # block-relative rule asserted, strict-rule misses reported
+    gC_in = (gC_o * ok[None]).astype(np.float32)
+    mm = np.where(ok, m, 1).astype(np.uint8)
+    gg_b = g.render_bwd(gC=gC_in, mask=mm)
+    og_b = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=gC_in)
+    rep9 = check_grads(gg_b, og_b, floor=1e-9, max_strict_fail=1.0)
+    return dict(l1_err=abs(float(l1.item()) - l1_o), sign_unclear=int((~clear).sum()),
+                strict={k: (v["strict_fail_frac"], v["worst_strict_rel"]) for k, v in rep.items()},
+                floor1e9={k: (v["strict_fail_frac"], v["worst_block_rel"]) for k, v in rep9.items()})
 
 
 def test_config1_all_views():
@@ -151,6 +252,8 @@ def test_split_heavy_tile_backward_both_instances():
     g.preprocess(); g.bin_sort(want_ids=False)
     gf = g.render_fwd(mask=m)
     ok = fw["fragile"] == 0
+    print("PARITY split-tile scene: fragile fraction %.4f" % (1 - ok.mean()))
+    assert 1 - ok.mean() <= 0.2  # thousands of nearly transparent surfels over one tile: measured 0.09
     assert np.array_equal(gf["n_contrib"][ok], fw["n_contrib"][ok])
     rng = np.random.default_rng(12)
     okf = ok.astype(np.float64)
