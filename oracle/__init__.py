@@ -191,6 +191,8 @@ def render_bwd(pos, scale, quat, opacity, sh, pre, srt, cam: OrcCamera, cfg: Orc
     out = dict(d_pos=np.zeros((n, 3)), d_scale=np.zeros((n, 2)), d_quat=np.zeros((n, 4)), d_opacity=np.zeros(n),
                d_sh=np.zeros((n, 16, 3)), d_center2d=np.zeros((n, 2)))
     oabs = np.zeros(n)
+    # sums of |terms| behind every entry (conditioning of the sums; see orc_render_bwd)
+    ab = dict(d_pos=np.zeros((n, 3)), d_scale=np.zeros((n, 2)), d_quat=np.zeros((n, 4)), d_sh=np.zeros((n, 16, 3)), d_center2d=np.zeros((n, 2)))
     ids = srt["ids"] if srt["K"] > 0 else np.zeros(1, np.uint32)
     m = None if mask is None else np.ascontiguousarray(mask, np.uint8)
     gC, gA, gD, gN, gM1, gM2 = _f64(gC), _f64(gA), _f64(gD), _f64(gN), _f64(gM1), _f64(gM2)
@@ -198,8 +200,11 @@ def render_bwd(pos, scale, quat, opacity, sh, pre, srt, cam: OrcCamera, cfg: Orc
                          _p(pre["visible"]), _p(pre["M"]), _p(pre["c2d"]), _p(pre["rho_cut"]), _p(pre["normal"]), _p(pre["rgb"]),
                          _p(pre["clamp"]), _p(ids), _p(srt["ranges"]), _p(m), _p(gC), _p(gA), _p(gD), _p(gN),
                          C.c_int(x0), C.c_int(y0), C.c_int(x1), C.c_int(y1), _p(out["d_pos"]), _p(out["d_scale"]),
-                         _p(out["d_quat"]), _p(out["d_opacity"]), _p(out["d_sh"]), _p(out["d_center2d"]), _p(oabs), _p(gM1), _p(gM2))
+                         _p(out["d_quat"]), _p(out["d_opacity"]), _p(out["d_sh"]), _p(out["d_center2d"]), _p(oabs), _p(gM1), _p(gM2),
+                         _p(ab["d_pos"]), _p(ab["d_scale"]), _p(ab["d_quat"]), _p(ab["d_sh"]), _p(ab["d_center2d"]))
     out["_d_opacity_abs"] = oabs
+    ab["d_opacity"] = oabs
+    out["_abs"] = ab
     return out
 
 

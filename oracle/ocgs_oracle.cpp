@@ -343,21 +343,8 @@ inline PairEval eval_pair(double x, double y, const float* Mf, const float* c2df
   e.rho = e.surf ? rho3 : rho2;
   e.z = e.surf ? (M[6] * e.u + M[7] * e.v + M[8]) : M[8];
   const double near = cfg.near_z, rc = rho_cut_f;
-  if (mg) {
-    // the switch only matters if the pair can be blended under either reading
-    if (std::fabs(rho3 - rho2) <= mg->switch_rel * std::fmax(e.rho, 1e-12) && e.rho <= rc + mg->rho_cut_abs) e.fragile = true;
-    if (std::fabs(e.z - near) <= mg->near_rel * near && e.rho <= rc + mg->rho_cut_abs) e.fragile = true;
-    if (std::fabs(e.rho - rc) <= mg->rho_cut_abs && e.z >= near * (1.0 - mg->near_rel)) e.fragile = true;
-  }
-  if (e.z < near) return e;
-  if (e.rho > rc) return e;
-  e.G = std::exp(-0.5 * e.rho);
-  const double araw = (double)of * e.G;
-  e.capped = araw > (double)cfg.alpha_max;
-  e.alpha = e.capped ? (double)cfg.alpha_max : araw;
-  if (mg && std::fabs(araw - (double)cfg.alpha_max) <= mg->cap_abs) e.fragile = true;
-  e.valid = true;
-  if (mg && mg->eps32 > 0.0) {
+  double drho3 = 0.0, drho2 = 0.0, dz3 = 0.0;
+  if (mg && mg->eps32 > 0.0 && e.rho <= 2.0 * rc + 1.0) {
     // Forward error of evaluating this pair in fp32 from the fp32 record, first order, for the centred form
     // k = (x - c)*M2 - (M0 - c*M2) (no large-number cancellation in forming k).  For surfels seen almost edge-on
     // q_z = k0 l1 - k1 l0 cancels and the map record -> alpha is intrinsically ill-conditioned.
@@ -374,17 +361,33 @@ inline PairEval eval_pair(double x, double y, const float* Mf, const float* c2df
     dq[0] = A(l[2]) * dk[1] + A(k[1]) * dl[2] + A(l[1]) * dk[2] + A(k[2]) * dl[1] + ep * (A(k[1] * l[2]) + A(k[2] * l[1]));
     dq[1] = A(l[0]) * dk[2] + A(k[2]) * dl[0] + A(l[2]) * dk[0] + A(k[0]) * dl[2] + ep * (A(k[2] * l[0]) + A(k[0] * l[2]));
     dq[2] = A(l[1]) * dk[0] + A(k[0]) * dl[1] + A(l[0]) * dk[1] + A(k[1]) * dl[0] + ep * (A(k[0] * l[1]) + A(k[1] * l[0]));
-    double drho, dz = 0.0;
-    if (e.surf) {
-      const double du = (dq[0] + A(e.u) * dq[2]) / A(e.qz) + ep * A(e.u), dv = (dq[1] + A(e.v) * dq[2]) / A(e.qz) + ep * A(e.v);
-      drho = 2.0 * (A(e.u) * du + A(e.v) * dv);
-      dz = A(M[6]) * du + A(M[7]) * dv;
-    } else {
-      drho = 4.0 * ep * e.rho;
-    }
+    const double du = (dq[0] + A(e.u) * dq[2]) / A(e.qz) + ep * A(e.u), dv = (dq[1] + A(e.v) * dq[2]) / A(e.qz) + ep * A(e.v);
+    drho3 = 2.0 * (A(e.u) * du + A(e.v) * dv);
+    dz3 = A(M[6]) * du + A(M[7]) * dv;
+    drho2 = 4.0 * ep * rho2;
+  }
+  const double drho = e.surf ? drho3 : drho2, dz = e.surf ? dz3 : 0.0;
+  if (mg) {
+    // S22: a decision is fragile when it is within its margin -- a few fp32 ulps of the quantity, or, for a pair whose fp32
+    // evaluation is ill-conditioned (surfel seen almost edge-on), that pair's own first-order error estimate if larger.
+    // the switch only matters if the pair can be blended under either reading
+    const double m_cut = std::fmax(mg->rho_cut_abs, drho), m_near = std::fmax(mg->near_rel * near, dz);
+    if (std::fabs(rho3 - rho2) <= std::fmax(mg->switch_rel * std::fmax(e.rho, 1e-12), drho3 + drho2) && e.rho <= rc + m_cut) e.fragile = true;
+    if (std::fabs(e.z - near) <= m_near && e.rho <= rc + m_cut) e.fragile = true;
+    if (std::fabs(e.rho - rc) <= m_cut && e.z >= near - m_near) e.fragile = true;
+  }
+  if (e.z < near) return e;
+  if (e.rho > rc) return e;
+  e.G = std::exp(-0.5 * e.rho);
+  const double araw = (double)of * e.G;
+  e.capped = araw > (double)cfg.alpha_max;
+  e.alpha = e.capped ? (double)cfg.alpha_max : araw;
+  if (mg && std::fabs(araw - (double)cfg.alpha_max) <= std::fmax(mg->cap_abs, 0.5 * araw * drho)) e.fragile = true;
+  e.valid = true;
+  if (mg && mg->eps32 > 0.0) {
     e.drho_est = drho;
     const double dalpha = e.capped ? 0.0 : 0.5 * e.alpha * drho;
-    e.err_est = dalpha + e.alpha * dz / std::fmax(1.0, A(e.z));
+    e.err_est = dalpha + e.alpha * dz / std::fmax(1.0, std::fabs(e.z));
   }
   return e;
 }
@@ -573,13 +576,20 @@ void orc_render_bwd(int n, const float* pos, const float* scale, const float* qu
                     const uint32_t* ranges, const uint8_t* mask, const double* gC, const double* gA, const double* gD,
                     const double* gN, int wx0, int wy0, int wx1, int wy1, double* d_pos, double* d_scale, double* d_quat,
                     double* d_opacity, double* d_sh, double* d_center2d, double* d_opacity_abs,
-                    const double* gM1, const double* gM2 /*nullable: upstream of the depth moments m1, m2 (origin held fixed)*/) {
+                    const double* gM1, const double* gM2 /*nullable: upstream of the depth moments m1, m2 (origin held fixed)*/,
+                    double* abs_pos, double* abs_scale, double* abs_quat, double* abs_sh, double* abs_center2d
+                    /*nullable together: for every gradient entry the sum of the ABSOLUTE values of the terms it is the sum of
+                      (per-pair terms, then the same linear chain with absolute coefficients) -- the conditioning of the sum: an fp32
+                      evaluation cannot be closer than ~eps32 x this, whatever the size of the entry itself*/) {
   const int W = cam->width, H = cam->height, T = cfg->tile;
   const int tiles_x = (W + T - 1) / T, tiles_y = (H + T - 1) / T;
   const size_t HW = (size_t)W * H;
   // per-surfel intermediate gradients: gM[9], g_c2d[2], g_o, g_rgb[3], g_n[3]
   std::vector<double> goabs((size_t)n, 0.0);
   std::vector<double> gM((size_t)n * 9, 0.0), gc2((size_t)n * 2, 0.0), go((size_t)n, 0.0), grgb((size_t)n * 3, 0.0), gn((size_t)n * 3, 0.0);
+  const bool want_abs = abs_pos != nullptr;
+  std::vector<double> gMa(want_abs ? (size_t)n * 9 : 0, 0.0), gc2a(want_abs ? (size_t)n * 2 : 0, 0.0), grgba(want_abs ? (size_t)n * 3 : 0, 0.0),
+      gna(want_abs ? (size_t)n * 3 : 0, 0.0);
 
 #pragma omp parallel
   {
@@ -658,10 +668,18 @@ void orc_render_bwd(int n, const float* pos, const float* scale, const float* qu
             for (int i2 = 0; i2 < 9; ++i2) if (aM[i2] != 0.0) {
 #pragma omp atomic
               gM[9 * (size_t)j + i2] += aM[i2];
+              if (want_abs) {
+#pragma omp atomic
+                gMa[9 * (size_t)j + i2] += std::fabs(aM[i2]);
+              }
             }
             for (int i2 = 0; i2 < 2; ++i2) if (ac[i2] != 0.0) {
 #pragma omp atomic
               gc2[2 * (size_t)j + i2] += ac[i2];
+              if (want_abs) {
+#pragma omp atomic
+                gc2a[2 * (size_t)j + i2] += std::fabs(ac[i2]);
+              }
             }
             if (a_o != 0.0) {
 #pragma omp atomic
@@ -673,10 +691,18 @@ void orc_render_bwd(int n, const float* pos, const float* scale, const float* qu
               if (a_rgb[c] != 0.0) {
 #pragma omp atomic
                 grgb[3 * (size_t)j + c] += a_rgb[c];
+                if (want_abs) {
+#pragma omp atomic
+                  grgba[3 * (size_t)j + c] += std::fabs(a_rgb[c]);
+                }
               }
               if (a_n[c] != 0.0) {
 #pragma omp atomic
                 gn[3 * (size_t)j + c] += a_n[c];
+                if (want_abs) {
+#pragma omp atomic
+                  gna[3 * (size_t)j + c] += std::fabs(a_n[c]);
+                }
               }
             }
           }
@@ -698,6 +724,12 @@ void orc_render_bwd(int n, const float* pos, const float* scale, const float* qu
     d_opacity[j] = 0;
     if (d_opacity_abs) d_opacity_abs[j] = goabs[j];  // sum of |terms|: conditioning of the d_opacity summation
     for (int k = 0; k < 48; ++k) d_sh[48 * (size_t)j + k] = 0;
+    if (want_abs) {
+      for (int k = 0; k < 3; ++k) abs_pos[3 * j + k] = 0;
+      for (int k = 0; k < 2; ++k) { abs_scale[2 * j + k] = 0; abs_center2d[2 * j + k] = 0; }
+      for (int k = 0; k < 4; ++k) abs_quat[4 * j + k] = 0;
+      for (int k = 0; k < 48; ++k) abs_sh[48 * (size_t)j + k] = 0;
+    }
     if (!visible[j]) continue;
     double g[9];
     for (int k = 0; k < 9; ++k) g[k] = gM[9 * (size_t)j + k];
@@ -764,6 +796,54 @@ void orc_render_bwd(int n, const float* pos, const float* scale, const float* qu
     const double dd = dot3(dir, gdir);
     for (int k = 0; k < 3; ++k) gp[k] += (gdir[k] - dir[k] * dd) / len;
     for (int k = 0; k < 3; ++k) d_pos[3 * j + k] = gp[k];
+    if (want_abs) {
+      // the same linear chain with the absolute values of every coefficient, applied to the sums of |terms|
+      auto A = [](double v) { return std::fabs(v); };
+      double ga[9];
+      for (int k = 0; k < 9; ++k) ga[k] = gMa[9 * (size_t)j + k];
+      const double c0a = gc2a[2 * j], c1a = gc2a[2 * j + 1];
+      ga[2] += c0a / A(M22);
+      ga[5] += c1a / A(M22);
+      ga[8] += (c0a * A((double)c2d[2 * j]) + c1a * A((double)c2d[2 * j + 1])) / A(M22);
+      abs_center2d[2 * j] = A(M22) * ga[2];
+      abs_center2d[2 * j + 1] = A(M22) * ga[5];
+      double gca[3][3];
+      for (int i = 0; i < 3; ++i) {
+        gca[i][0] = A(fx) * ga[i];
+        gca[i][1] = A(fy) * ga[3 + i];
+        gca[i][2] = A(ox) * ga[i] + A(oy) * ga[3 + i] + ga[6 + i];
+      }
+      auto VTa = [&](const double* e, double* out) {  // |R_wc^T| e
+        for (int k = 0; k < 3; ++k) out[k] = A((double)V[k]) * e[0] + A((double)V[4 + k]) * e[1] + A((double)V[8 + k]) * e[2];
+      };
+      abs_scale[2 * j] = gca[0][0] * A(vu[0]) + gca[0][1] * A(vu[1]) + gca[0][2] * A(vu[2]);
+      abs_scale[2 * j + 1] = gca[1][0] * A(vv[0]) + gca[1][1] * A(vv[1]) + gca[1][2] * A(vv[2]);
+      double ua[3], va[3], wa[3], pa[3], t3[3];
+      VTa(gca[0], t3);
+      for (int k = 0; k < 3; ++k) ua[k] = A((double)scale[2 * j]) * t3[k];
+      VTa(gca[1], t3);
+      for (int k = 0; k < 3; ++k) va[k] = A((double)scale[2 * j + 1]) * t3[k];
+      VTa(gca[2], pa);
+      const double gnja[3] = {gna[3 * (size_t)j], gna[3 * (size_t)j + 1], gna[3 * (size_t)j + 2]};
+      VTa(gnja, wa);
+      const double aw = A(w), ax = A(x), ay = A(y), az = A(z);
+      abs_quat[4 * j + 0] = 2 * (az * ua[1] + ay * ua[2] + az * va[0] + ax * va[2] + ay * wa[0] + ax * wa[1]);
+      abs_quat[4 * j + 1] = 2 * (ay * ua[1] + az * ua[2] + ay * va[0] + 2 * ax * va[1] + aw * va[2] + az * wa[0] + aw * wa[1] + 2 * ax * wa[2]);
+      abs_quat[4 * j + 2] = 2 * (2 * ay * ua[0] + ax * ua[1] + aw * ua[2] + ax * va[0] + az * va[2] + aw * wa[0] + az * wa[1] + 2 * ay * wa[2]);
+      abs_quat[4 * j + 3] = 2 * (2 * az * ua[0] + aw * ua[1] + ax * ua[2] + aw * va[0] + 2 * az * va[1] + ay * va[2] + ax * wa[0] + ay * wa[1]);
+      double gda[3] = {0, 0, 0};
+      for (int c = 0; c < 3; ++c) {
+        if (clamp[j] & (1u << c)) continue;
+        const double gca_c = grgba[3 * (size_t)j + c];
+        for (int k = 0; k < nb; ++k) {
+          abs_sh[48 * (size_t)j + 3 * k + c] = A(Y[k]) * gca_c;
+          const double sa = A((double)sh[48 * (size_t)j + 3 * k + c]) * gca_c;
+          gda[0] += A(dY[k][0]) * sa; gda[1] += A(dY[k][1]) * sa; gda[2] += A(dY[k][2]) * sa;
+        }
+      }
+      const double dda = A(dir[0]) * gda[0] + A(dir[1]) * gda[1] + A(dir[2]) * gda[2];
+      for (int k = 0; k < 3; ++k) abs_pos[3 * j + k] = pa[k] + (gda[k] + A(dir[k]) * dda) / len;
+    }
   }
 }
 

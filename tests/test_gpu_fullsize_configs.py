@@ -15,7 +15,7 @@ pytestmark = pytest.mark.gpu
 def test_config2_full_size_full_image():
     """200 k surfels, 800x600 (DTU's training resolution), SH degree 3: every pixel, every gradient."""
     sc = sg.make_scene("config2")
-    r = full_parity(sc, 3, dict(sh_degree=3), max_fragile=4e-3)
+    r = full_parity(sc, 3, dict(sh_degree=3), max_fragile=3e-3)  # measured 1.06e-3
     assert r["K"] > 100_000
 
 
@@ -43,8 +43,10 @@ def windows_parity(sc, view, windows, key_capacity, rng_seed=11):
     gC = np.zeros((3, H, W)); gA = np.zeros((H, W)); gD = np.zeros((H, W)); gN = np.zeros((3, H, W))
     rng = np.random.default_rng(rng_seed)
     frag_total = npix = 0
+    cond_rho = np.zeros(sc.n)
     for (x0, y0, x1, y1) in windows:
         fw = orc.render_fwd(pre, srt, sc.opacity, cam, cfg, mask=m, window=(x0, y0, x1, y1))
+        cond_rho = np.maximum(cond_rho, fw["cond_rho"])
         ok = fw["fragile"][y0:y1, x0:x1] == 0
         frag_total += int((~ok).sum()); npix += ok.size
         for k in ("color", "alpha", "depth", "normal"):
@@ -64,13 +66,14 @@ def windows_parity(sc, view, windows, key_capacity, rng_seed=11):
     g.cfg.gamma_bg = 0.0
     gg = g.render_bwd(gC=gC, gA=gA, gD=gD, gN=gN, mask=m)
     og = {k: np.zeros_like(v, dtype=np.float64) for k, v in gg.items()}
-    og["_d_opacity_abs"] = np.zeros(sc.n)
-    for w in windows:
+    og["_abs"] = {k: np.zeros_like(v, dtype=np.float64) for k, v in gg.items()}
+    for w in windows:  # gradients and their sums of |terms| are additive over disjoint sets of pixels
         part = orc.render_bwd(*P, pre, srt, cam, cfg0, mask=m, gC=gC.astype(np.float32), gA=gA.astype(np.float32),
                               gD=gD.astype(np.float32), gN=gN.astype(np.float32), window=w)
-        for k in og:
+        for k in gg:
             og[k] += part[k]
-    rep = check_grads(gg, og)
+            og["_abs"][k] += part["_abs"][k].reshape(og["_abs"][k].shape)
+    rep = check_grads(gg, og, cond_rho=cond_rho)
     return dict(K=srt["K"], n_vis=int(vis.sum()), grads=rep, ranges=srt["ranges"])
 
 
@@ -79,7 +82,7 @@ def test_config5_full_size_full_image():
     entries (many batches per tile), 4.3 M keys through both radix stages.  Every pixel of a view, every output (see
     full_parity), the prune mask from its statistics and the step bench.py times."""
     sc = sg.make_scene("config5")
-    r = full_parity(sc, 0, dict(sh_degree=3), key_capacity=16 * sc.n, max_fragile=3e-3, check_prune=True, bench_step=True, label="config5")
+    r = full_parity(sc, 0, dict(sh_degree=3), key_capacity=16 * sc.n, max_fragile=2.7e-3, check_prune=True, bench_step=True, label="config5")  # measured 9.2e-4
     L = r["ranges"][:, 1] - r["ranges"][:, 0]
     assert r["K"] > 2_000_000 and L.max() > 4096
 
@@ -88,7 +91,7 @@ def test_config5_heaviest_view_forward_and_colour_backward():
     """The view of config 5 with the longest tile list (view 7: one tile of 25 338 entries, the heavy-tile walk of both raster
     kernels): every pixel of the forward outputs and the colour / alpha-only backward instance."""
     sc = sg.make_scene("config5")
-    r = full_parity(sc, 7, dict(sh_degree=3), key_capacity=16 * sc.n, max_fragile=3e-3, label="config5-heaviest")
+    r = full_parity(sc, 7, dict(sh_degree=3), key_capacity=16 * sc.n, max_fragile=2.4e-3, label="config5-heaviest")  # measured 7.7e-4
     L = r["ranges"][:, 1] - r["ranges"][:, 0]
     assert L.max() > 20_000
 
@@ -149,7 +152,7 @@ def test_config4_full_size_all_views_prune():
     n_diff = int((pm != po2["prune_mask"]).sum())
     print("PARITY config4: prune mask differs from the mask of the oracle's own statistics on %d of %d surfels; %d surfels touch a fragile pixel in some view"
           % (n_diff, n, int((~clean).sum())))
-    assert n_diff <= 8
+    assert n_diff <= 2  # measured: 0
     comp = orc.compact(dict(pos=sc.pos, scale=sc.scale, quat=sc.quat, opacity=sc.opacity, sh=sc.sh), pm)
     k = po["n_out"]
     for t, name in zip(outs, ("pos", "scale", "quat", "opacity", "sh")):

@@ -19,7 +19,7 @@ def arrays(sc):
 
 
 def full_parity(sc, view, cfg_kw, rng_seed=5, max_fragile=2e-3, with_bwd=True, key_capacity=None, check_prune=False, bench_step=False,
-                max_illcond_err=1e-3, label=None):
+                max_illcond_err=IMG_TOL, label=None):
     """One view through the five C-ABI calls against the oracle, EVERY output, every pixel, every surfel.
 
     check_prune: the prune mask, remap and compaction from this view's statistics (a5) against the oracle's rule.
@@ -63,7 +63,8 @@ def full_parity(sc, view, cfg_kw, rng_seed=5, max_fragile=2e-3, with_bwd=True, k
     assert np.array_equal(gs["tile_keys"], (srt["keys"] >> np.uint64(32)).astype(np.uint32))
     assert np.array_equal(gs["ranges"], srt["ranges"])
     # (3) forward: every pixel.  fragile bit 0 = a decision within its margin (the two sides may take different branches:
-    # bounded by the discontinuity jump 0.02); bit 1 only = ill-conditioned pair evaluation, nothing discontinuous: 10 x tolerance
+    # bounded by the discontinuity jump 0.02); bit 1 only = ill-conditioned pair evaluation, nothing discontinuous: the same 1e-4
+    # (measured: 7e-6 at config 3); such pixels are only left out of the upstream gradients of the backward comparison
     gf = g.render_fwd(mask=m)
     ok = fw["fragile"] == 0
     illc = fw["fragile"] == 2
@@ -125,17 +126,17 @@ def full_parity(sc, view, cfg_kw, rng_seed=5, max_fragile=2e-3, with_bwd=True, k
         gg = g.render_bwd(gC=gC, gA=gA, gD=gD, gN=gN, mask=mm)
         og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=gC.astype(np.float32), gA=gA.astype(np.float32),
                             gD=gD.astype(np.float32), gN=gN.astype(np.float32))
-        rep = check_grads(gg, og)
+        rep = check_grads(gg, og, cond_rho=fw["cond_rho"])
         # the colour / alpha-only instance of the kernel (no upstream gradient on the depth and normal maps)
         gg2 = g.render_bwd(gC=gC, gA=gA, mask=mm)
         og2 = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=gC.astype(np.float32), gA=gA.astype(np.float32))
-        rep2 = check_grads(gg2, og2)
+        rep2 = check_grads(gg2, og2, cond_rho=fw["cond_rho"])
         # surfels never blended receive exactly zero gradient
         never = gf["vis_count"] == 0
         for k in ("d_pos", "d_scale", "d_quat", "d_opacity", "d_sh"):
             assert np.all(gg[k][never] == 0.0), k
-        info["grads"] = {k: (v["strict_fail_frac"], v["worst_strict_rel"], v["worst_block_rel"]) for k, v in rep.items()}
-        info["grads_colour_alpha"] = {k: (v["strict_fail_frac"], v["worst_strict_rel"], v["worst_block_rel"]) for k, v in rep2.items()}
+        info["grads"] = {k: (v["strict_fail_frac"], v["worst_strict_rel"], v["worst_cond_units"]) for k, v in rep.items()}
+        info["grads_colour_alpha"] = {k: (v["strict_fail_frac"], v["worst_strict_rel"], v["worst_cond_units"]) for k, v in rep2.items()}
     if bench_step:
         info["bench_step"] = bench_step_parity(sc, view, g, orc, cam, cfg, pre, srt, fw, gf, m)
     print(f"PARITY {label or sc.name} n={sc.n} {camn.width}x{camn.height} view {view}: {info}")
@@ -181,18 +182,18 @@ def bench_step_parity(sc, view, g, orc, cam, cfg, pre, srt, fw, gf, m):
     # differs (|R - I| below fp32 resolution) and the fragile pixels move an entry by O(1/(3HW)) x w, far below the 1e-6 floor
     og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=m, gC=gC_o.astype(np.float32))
     gg = {k: v.cpu().numpy() for k, v in grads.items()}
-    rep = check_grads(gg, og)
+    rep = check_grads(gg, og, cond_rho=fw["cond_rho"])
     # (b) every entry of this step is O(pixels / (3HW)), mostly below north_star's floor, so the colour / alpha-only instance is
     # also run on the oracle's dL/dC (zero on fragile pixels, both sides the same input) and compared with the floor at 1e-9:
-    # block-relative rule asserted, strict-rule misses reported
+    # conditioning rule asserted, strict-rule misses reported
     gC_in = (gC_o * ok[None]).astype(np.float32)
     mm = np.where(ok, m, 1).astype(np.uint8)
     gg_b = g.render_bwd(gC=gC_in, mask=mm)
     og_b = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=gC_in)
-    rep9 = check_grads(gg_b, og_b, floor=1e-9, max_strict_fail=1.0)
+    rep9 = check_grads(gg_b, og_b, floor=1e-9, max_strict_fail=1.0, cond_rho=fw["cond_rho"])
     return dict(l1_err=abs(float(l1.item()) - l1_o), sign_unclear=int((~clear).sum()),
                 strict={k: (v["strict_fail_frac"], v["worst_strict_rel"]) for k, v in rep.items()},
-                floor1e9={k: (v["strict_fail_frac"], v["worst_block_rel"]) for k, v in rep9.items()})
+                floor1e9={k: (v["strict_fail_frac"], v["worst_cond_units"]) for k, v in rep9.items()})
 
 
 def test_config1_all_views():
@@ -263,10 +264,10 @@ def test_split_heavy_tile_backward_both_instances():
     f32 = lambda a: a.astype(np.float32)
     gg = g.render_bwd(gC=gC, gA=gA, gD=gD, gN=gN, mask=mm)
     og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=f32(gC), gA=f32(gA), gD=f32(gD), gN=f32(gN))
-    check_grads(gg, og)
+    check_grads(gg, og, cond_rho=fw["cond_rho"])
     gg = g.render_bwd(gC=gC, gA=gA, mask=mm)
     og = orc.render_bwd(*P, pre, srt, cam, cfg, mask=mm, gC=f32(gC), gA=f32(gA))
-    check_grads(gg, og)
+    check_grads(gg, og, cond_rho=fw["cond_rho"])
     never = gf["vis_count"] == 0
     for k in ("d_pos", "d_scale", "d_quat", "d_opacity", "d_sh"):
         assert np.all(gg[k][never] == 0.0), k
@@ -307,7 +308,7 @@ def test_depth_moments_and_their_gradient():
                             gM1=gM[0].astype(np.float32), gM2=gM[1].astype(np.float32))
         # dz = z_i - z_first is a difference of fp32 depths (each good to ~3e-7 at z ~ 3): for thin surfaces the terms
         # proportional to dz carry that absolute noise, so the floor is 1e-4 of each array's typical (99th percentile) scale
-        check_grads(gg, og, floor_frac=1e-4)
+        check_grads(gg, og, floor_frac=1e-4, cond_rho=fw["cond_rho"])
 
 
 def test_empty_and_all_culled_and_capacity():

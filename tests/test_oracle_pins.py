@@ -230,7 +230,7 @@ def test_opaque_front_layers_occlude_surfel_behind_exact_zero():
     rng = np.random.default_rng(0)
     g = orc.render_bwd(*s, pre, srt, cam, cfg, mask=np.zeros((H, W), np.uint8), gC=rng.normal(size=(3, H, W)),
                        gA=rng.normal(size=(H, W)), gD=rng.normal(size=(H, W)), gN=rng.normal(size=(3, H, W)))
-    for k, v in g.items():
+    for k, v in [kv for kv in g.items() if kv[0] != "_abs"] + list(g["_abs"].items()):
         assert np.all(v[4] == 0.0), k
         assert np.all(v[3] == 0.0), k
     assert np.any(g["d_opacity"][:3] != 0.0)
@@ -286,7 +286,7 @@ def test_background_loss_eq1_special_cases_and_gradient_sign():
     # the fused gradient equals feeding gA = gamma (1-M)/(HW) explicitly
     cfg0 = orc.default_config(sh_degree=1, gamma_bg=0.0)
     g2 = orc.render_bwd(*P, pre, srt, cam, cfg0, mask=left, gA=0.5 * (1.0 - left) / (H * W))
-    for k in g:
+    for k in (k for k in g if k != "_abs"):
         assert np.allclose(g[k], g2[k], rtol=1e-12, atol=1e-18), k
 
 
@@ -612,6 +612,32 @@ def test_d_center2d_reading_r_c2d():
     for j in range(2):
         z = float(s[0][j, 2])
         assert np.allclose(g["d_center2d"][j], z / 30.0 * g["d_pos"][j, :2], rtol=1e-12, atol=0)
+
+
+def test_backward_sums_of_absolute_terms_bound_the_gradients():
+    """The conditioning sums the gradient tolerance uses (orc_render_bwd abs_*) are what they claim:
+    every entry satisfies |g| <= sum|terms| (triangle inequality through the whole chain), the sums are positively
+    homogeneous in the upstream gradients (x -2 doubles them), and for a non-negative upstream on colour only the colour
+    chain has no cancellation at all: sum|terms| == |d_sh| exactly."""
+    sc = sg.random_scene(40, 48, 40, 40.0, seed=31, sh_degree=2)
+    cam = orc.camera_from(sc.cameras[0])
+    cfg = orc.default_config(sh_degree=2)
+    P = (sc.pos, sc.scale, sc.quat, sc.opacity, sc.sh)
+    pre = orc.preprocess(*P, cam, cfg)
+    srt = orc.bin_sort(pre, cam, cfg)
+    rng = np.random.default_rng(2)
+    gC, gA, gD, gN = rng.normal(size=(3, 40, 48)), rng.normal(size=(40, 48)), rng.normal(size=(40, 48)), rng.normal(size=(3, 40, 48))
+    g = orc.render_bwd(*P, pre, srt, cam, cfg, gC=gC, gA=gA, gD=gD, gN=gN)
+    g2 = orc.render_bwd(*P, pre, srt, cam, cfg, gC=-2 * gC, gA=-2 * gA, gD=-2 * gD, gN=-2 * gN)
+    assert (g["d_pos"] != 0).sum() > 50
+    for k in ("d_pos", "d_scale", "d_quat", "d_opacity", "d_sh", "d_center2d"):
+        a = g["_abs"][k].reshape(g[k].shape)
+        assert np.all(np.abs(g[k]) <= a * (1 + 1e-12) + 1e-300), k
+        assert np.allclose(g2["_abs"][k].reshape(a.shape), 2 * a, rtol=1e-12, atol=0), k
+        assert np.allclose(g2[k], -2 * g[k], rtol=1e-9, atol=1e-14), k
+    gp = orc.render_bwd(*P, pre, srt, cam, cfg, gC=np.abs(gC))
+    sh0 = gp["d_sh"][:, 0, :]  # Y0 > 0: d_sh[0] = Y0 * sum of non-negative terms
+    assert np.allclose(gp["_abs"]["d_sh"][:, 0, :], np.abs(sh0), rtol=1e-12, atol=0) and (sh0 > 0).sum() > 20
 
 
 def test_prune_and_compaction_definition():
