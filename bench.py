@@ -25,11 +25,12 @@ sys.path.insert(0, ROOT)
 METRIC = "ms per fwd+bwd raster step (1600x1200, 1M surfels)"
 FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 40.0, 22.0, 72.0  # DESIGN.md section 6 "algorithmic work per unit" (FMA = 2)
 FLOP_BLEND_BWD_COLOUR_ONLY = 54.0  # no upstream gradient on depth / normal maps (masked L1 + L_b): those terms are not evaluated
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the raster kernels, from the `ncu --set full` capture of this
-# workload committed as profiles/r01j_raster_kernels_full.md (bytes)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the raster kernels (bytes), from the `ncu --set full` capture of
+# this workload committed under profiles/ (NCU_TRAFFIC_SOURCE)
 NCU_TRAFFIC = {"render_bwd_kernel": 90.0e6, "render_fwd_kernel": 139.2e6}
 NCU_TRAFFIC_SOURCE = "profiles/r01m_raster_kernels_full.md"
-ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 148 SMs x 128 FP32 lanes x 2 (FMA) x max SM clock (B200_PROFILING.md)
+# fallback only (used when the microbenchmark of ocgs_peak_probe cannot run): 148 SMs x 128 FP32 lanes x 2 (FMA) x max SM clock
+ALU_PEAK_TFLOPS_DERIVED = 148 * 128 * 2 * 1.965e9 / 1e12
 
 
 def parse_args():
@@ -39,7 +40,10 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="config3")
-    ap.add_argument("--views", type=int, default=4, help="distinct views rotated over per rank")
+    ap.add_argument("--views", type=int, default=8, help="distinct views rotated over per rank (0 = the rank's whole shard of the config's views)")
+    ap.add_argument("--batch-views", action="store_true",
+                    help="N > 1 only: the N views of a step form one optimiser batch -- every step ends with the all-reduce (sum) of the gradient "
+                         "arrays over ranks (SURVEY.md 8(e)); direct launches, the collective is inside the timed region")
     ap.add_argument("--shrink", type=float, default=1.0, help="scale surfel counts (debug only; invalidates the metric)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -49,6 +53,12 @@ def parse_args():
     ap.add_argument("--no-prune", action="store_true", help="skip the separately timed prune pass (profiling runs)")
     ap.add_argument("--no-graph", action="store_true", help="time direct kernel launches instead of CUDA graph replays")
     return ap.parse_args()
+
+
+def workload_name(scene):
+    """The same string in both arms, so that the driver sees one config."""
+    c = scene.cameras[0]
+    return f"{scene.name}: {scene.n} surfels, {c.width}x{c.height}, SH degree {scene.sh_degree}, {len(scene.cameras)} views"
 
 
 def make_scene(args):
@@ -150,6 +160,42 @@ def oracle_sample(scene, view, window_frac=0.2):
     return ms, desc, orc.num_threads(), t2 - t1
 
 
+def alu_peaks(B, torch, dev):
+    """FP32-FMA and MUFU.EX2 rates of this device, measured with the library's microbenchmark (ocgs_peak_probe): best of five
+    launches of ~1 ms, CUDA events on the launching stream.  SURVEY.md 8(d): the rooflines of the raster kernels are quoted
+    against THESE, not against unit counts x clock."""
+    props = torch.cuda.get_device_properties(dev)
+    out = torch.empty(props.multi_processor_count * 8 * 256, dtype=torch.float32, device=dev)
+    res = {}
+    for kind, key in ((0, "fp32_tflops_measured"), (1, "ex2_tops_measured")):
+        iters = 2048 if kind == 0 else 256
+        best = 0.0
+        for rep_i in range(6):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ops = B.ocgs_peak_probe(kind, iters, out)
+            e1.record()
+            torch.cuda.synchronize()
+            if rep_i:  # the first launch warms up
+                best = max(best, ops / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+        res[key] = best
+    res["how"] = ("ocgs_peak_probe: 8 independent chains per thread of a <- fma(a,b,c) (2 flop) / a <- -ex2(a), 8 blocks x 256 threads per SM, "
+                  "best of 5 launches, CUDA events")
+    res["sm_count"] = props.multi_processor_count
+    res["fp32_tflops_derived"] = ALU_PEAK_TFLOPS_DERIVED
+    return res
+
+
+def oracle_cores():
+    """(threads the oracle uses, affinity mask of this process as a sorted list of CPU ids, os.cpu_count())"""
+    import oracle as orc
+    try:
+        aff = sorted(os.sched_getaffinity(0))
+    except AttributeError:
+        aff = []
+    return orc.num_threads(), aff, os.cpu_count()
+
+
 def pick_window_frac(scene, view, budget_s):
     """Largest centred window (up to the whole image) whose forward + backward stays near budget_s of CPU work: the less is
     extrapolated the better -- a small window has too few tiles to keep all cores busy and sits on the object, which
@@ -181,11 +227,12 @@ def run_reference(args):
         if i >= args.warmup:
             vals.append(ms)
     v = float(np.mean(vals))
+    _, aff, ncpu = oracle_cores()
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{scene.name}: {scene.n} surfels, {cam0.width}x{cam0.height}, views rotated"},
-            "cpu_baseline": {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": desc},
+            "config": {"workload": workload_name(scene)},
+            "cpu_baseline": {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": desc, "affinity": aff, "cpu_count": ncpu},
             "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
 
@@ -199,23 +246,27 @@ def run_ours(args):
     import torch.distributed as dist
     from paper_2501_08174_b200 import binding as B
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2501_08174_b200 import sharding
+    rank, world, local = sharding.env_rank()
+    if world != args.gpus:
+        raise RuntimeError(f"--gpus {args.gpus} but the launch has WORLD_SIZE={world}: the number printed must be the number measured")
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    if torch.cuda.device_count() <= local:
+        raise RuntimeError(f"rank {rank} needs CUDA device {local}, the node has {torch.cuda.device_count()}")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     B.lib()
+    peaks = alu_peaks(B, torch, dev)
 
     scene = make_scene(args)
     n, deg = scene.n, scene.sh_degree
     cams = scene.cameras
     W, H = cams[0].width, cams[0].height
-    # views are sharded over ranks: rank r owns views r, r+world, ...; no data-path collective
-    my_views = [v for v in range(len(cams)) if v % world == rank][: args.views] or [rank % len(cams)]
+    # views are sharded over ranks: rank r owns views r, r+world, ...; no data-path collective in the step
+    my_views = sharding.rotation_for_rank(len(cams), rank, world, args.views)
     cfg = B.ocgs_default_config(sh_degree=deg)
     cap = int(os.environ.get("OCGS_KEY_CAPACITY", 48 * n if n < 2_000_000 else 16 * n))
 
@@ -276,7 +327,10 @@ def run_ours(args):
                                  out["loss_bg"], loss_l1, gC, vis if stats else None, cs if stats else None)
         B.ocgs_render_bwd(surfels, c, cfg, ws, cap, m, out["n_contrib"], gC, None, None, None, grads["d_pos"], grads["d_scale"],
                           grads["d_quat"], grads["d_opacity"], grads["d_sh"], grads["d_center2d"])
+        if batch_views:  # the world's views of this step are one optimiser batch: sum their gradients over NVLink
+            sharding.allreduce_grads(grads)
 
+    batch_views = bool(args.batch_views and world > 1)
     # warm-up + workload counters (outside the timed region)
     nv = len(my_views)
     counters = []
@@ -301,7 +355,7 @@ def run_ours(args):
     # replayed (--no-graph launches the 18 kernels directly).  Per-launch events are NOT recorded here: an event after
     # every kernel costs ~0.17 ms per step of idle gaps; the per-kernel breakdown comes from region 2 below.
     graphs = None
-    if not args.no_graph:
+    if not args.no_graph and not batch_views:
         try:
             graphs = []
             side = torch.cuda.Stream()
@@ -356,10 +410,19 @@ def run_ours(args):
     ms_marked = ev2.elapsed_time(ev3)
     clocks = sampler.stop() if rank == 0 else None
     B.ocgs_check(ws)
-    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    ms_total = sharding.max_over_ranks(ms_total, dev)
+    # the one exchange step of the un-batched method: the merge of the visibility statistics at the end of a pruning
+    # interval -- once per rotation, not per step; timed beside the step (device time, max over ranks)
+    stats_allreduce_ms = None
     if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
+        sharding.allreduce_stats(vis, cs)  # warm-up (communicator set-up)
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        a0.record()
+        sharding.allreduce_stats(vis, cs)
+        a1.record()
+        barrier()
+        stats_allreduce_ms = sharding.max_over_ranks(a0.elapsed_time(a1), dev)
 
     # ---- visibility pass ("rendering all training views" for the pruning statistics), timed separately ------
     # (a) through the full forward pass (preprocess + bin_sort + render_fwd with the statistics on), (b) through
@@ -485,17 +548,17 @@ def run_ours(args):
             h_header = torch.zeros(4, dtype=torch.int32).pin_memory()
             main = torch.cuda.Stream()
             torch.cuda.synchronize()
-            graphs = []
+            e2e_graphs = []
             for i in range(nv):
                 gr = torch.cuda.CUDAGraph()
                 with torch.cuda.graph(gr, stream=main):
                     B.ocgs_step_view_host_enqueue(surfels, cam_c[i], cfg, h_masks[i], h_targets[i], h_losses, h_header, d_mask, d_images, d_nc,
                                                   grads, vis, cs, d_losses, ws, cap, stream=main, copy_stream=copy_stream)
-                graphs.append(gr)
+                e2e_graphs.append(gr)
 
             def view_step_graph(i):
                 with torch.cuda.stream(main):
-                    graphs[i].replay()
+                    e2e_graphs[i].replay()
                 main.synchronize()
                 if int(h_header[3]) != 0:
                     raise RuntimeError("step reported error bits %d" % int(h_header[3]))
@@ -555,8 +618,10 @@ def run_ours(args):
             view_step(v_last)
             assert got[0] == float(h_losses[0]) and abs(got[1] - float(h_losses[1])) < 1e-6, (got, float(h_losses[0]), float(h_losses[1]))
         e2e = {"value": ms_view, "unit": "ms", "h2d_bytes_per_step": H * W + 3 * H * W * 4, "d2h_bytes_per_step": 8 + 16, "steps": k_e,
-               "what": how + ": target image + mask from pinned host memory each step, parameters and gradients resident "
-                       "in HBM, uploads on a second stream overlapping preprocess/sort/forward, loss scalars read back",
+               "what": ("step k runs on inputs uploaded during step k-1 (data-loader prefetch): " if not args.no_graph else "") + how +
+                       ": target image + mask from pinned host memory each step, parameters and gradients resident "
+                       "in HBM, uploads on a second stream overlapping preprocess/sort/forward, loss scalars read back; the form that uploads "
+                       "the step's OWN view inside the step is graph_upload_inside_step_ms",
                "direct_launch_ms": ms_direct, "graph_upload_inside_step_ms": ms_sameview,
                "losses_last_step": [float(h_losses[0]), float(h_losses[1])]}
         hp = {k: torch.tensor(np.ascontiguousarray(getattr(scene, k)), dtype=torch.float32).pin_memory() for k in ("pos", "scale", "quat", "opacity", "sh")}
@@ -607,9 +672,10 @@ def run_ours(args):
                 fb = FLOP_BLEND_BWD_COLOUR_ONLY if args.loss in ("l1", "dssim") else FLOP_BLEND_BWD
                 fl, what = (FLOP_EVAL + fb) * Bp, f"({FLOP_EVAL:.0f} + {fb:.0f}) flop x B blended pairs"
             ach = fl / avg_s / 1e12
-            return {"kernel": name, "bound": "alu", "achieved": ach, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / ALU_PEAK_TFLOPS,
+            pk = peaks["fp32_tflops_measured"]
+            return {"kernel": name, "bound": "alu", "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": ach / pk,
                     "traffic": NCU_TRAFFIC.get(name), "traffic_source": NCU_TRAFFIC_SOURCE,
-                    "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)", "algorithmic": what}
+                    "peak_source": "measured: FP32 FMA microbenchmark of this run (ocgs_peak_probe, peaks.fp32_tflops_measured)", "algorithmic": what}
         per_launch = {"radix_onesweep_kernel": 16.0 * (4 * n + 2 * K) / 6.0,  # 8 B read + 8 B written per key; 4 passes over N, 2 over K
                       "radix_hist_all_kernel": 4.0 * n, "emit_keys_kernel": 8.0 * K + 12.0 * nvis,  # the tile sort's histograms are built by emit_keys_kernel
                       "preprocess_kernel": 61.0 * n + 296.0 * nvis, "project_bwd_kernel": 232.0 * n + 328.0 * nvis,
@@ -629,14 +695,15 @@ def run_ours(args):
     line = {"metric": METRIC, "value": ms_per_step, "unit": "ms", "n_gpus": world, "steps": steps, "warmup": max(args.warmup, nv),
             "ms_per_step": ms_total / steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
-            "config": {"workload": f"{scene.name}: {n} surfels, {W}x{H}, SH degree {deg}, {nv} views rotated per rank (views sharded over ranks)",
+            "config": {"workload": workload_name(scene), "views_rotated_per_rank": nv, "views": my_views, "sharding": "views r, r+N, ... to rank r",
+                       "batch_views": batch_views,
                        "l2": "inputs larger than L2: 232 MB of surfel parameters are re-read every step", "key_capacity": cap,
                        "shrink": args.shrink, "loss": {"l1": "masked L1 (S20) + gamma L_b", "dssim": "L_c^M = 0.8 L1 + 0.2 D-SSIM (Eq. 2) + gamma L_b",
                                 "eq3": "Eq. 3: L_c^M + 100 L_d + 0.05 L_n + gamma L_b"}[args.loss]},
             "surfels_per_s": n * world / (ms_total / steps * 1e-3), "pixels_per_s": W * H * world / (ms_total / steps * 1e-3),
             "workload_counters": mean, "gpu_launches": launches, "clocks": clocks, "roofline": roof, "rooflines": rooflines, "kernels": kernels[:14],
             "kernel_ms_sum_per_step": kern_total / steps,
-            "launch": "cuda_graph_replay" if graphs is not None else "direct",
+            "launch": "cuda_graph_replay" if graphs is not None else "direct", "peaks": peaks, "stats_allreduce_ms": stats_allreduce_ms,
             "kernel_timing": {"how": "second timed region of the same K steps, direct launches, one CUDA event after every launch "
                                      "(those events cost idle gaps, so `value` comes from the region without them)",
                               "ms_per_step_with_events": ms_marked / steps}}
@@ -646,8 +713,15 @@ def run_ours(args):
         line["e2e"] = e2e
         line["e2e_host_params"] = e2e_hp
     if world == 1 and not args.no_cpu_baseline:
-        _, (ms_cpu, desc, cores, _) = pick_window_frac(scene, my_views[0], budget_s=15.0)
-        line["cpu_baseline"] = {"value": ms_cpu, "unit": "ms", "cores": cores, "kind": "oracle", "sample": desc}
+        import oracle as orc
+        frac, (ms_cpu, desc, cores, _) = pick_window_frac(scene, my_views[0], budget_s=12.0)
+        _, aff, ncpu = oracle_cores()
+        # the same oracle on ONE core: a smaller centred window, so that it stays within ~10 s
+        orc.set_num_threads(1)
+        ms_1, desc_1, _, _ = oracle_sample(scene, my_views[0], window_frac=max(0.1, frac / max(1.0, cores) ** 0.5))
+        orc.set_num_threads(cores)
+        line["cpu_baseline"] = {"value": ms_cpu, "unit": "ms", "cores": cores, "kind": "oracle", "sample": desc, "affinity": aff, "cpu_count": ncpu,
+                                "one_core": {"value": ms_1, "unit": "ms", "cores": 1, "sample": desc_1}}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -658,4 +732,9 @@ if __name__ == "__main__":
     if a.impl == "reference":
         run_reference(a)
     else:
+        # `--gpus N` outside torchrun starts the N ranks itself (and refuses when the node has fewer than N CUDA devices)
+        from paper_2501_08174_b200 import sharding as _sh
+        rc = _sh.relaunch_under_torchrun(a.gpus, [os.path.abspath(__file__)] + sys.argv[1:])
+        if rc is not None:
+            sys.exit(rc)
         run_ours(a)

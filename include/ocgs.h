@@ -141,7 +141,9 @@ int ocgs_bin_sort(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* w
  * position after the last blended pair; ws.final_T[H,W] = T.  loss_bg (device scalar, nullable; needs mask): Eq. 1, PAPER.md:99,
  * L_b = 1/(H W) sum A (1-M), deterministic reduction.  vis_count[N] / contrib_sum[N] (device, nullable): ACCUMULATE
  * (+=) the number of pixels that blended surfel j and sum of alpha*T ("we save which Gaussians are used
- * during the color accumulation step"; O8).  mask: device u8 [H,W], non-zero = object, nullable (= all background). */
+ * during the color accumulation step"; O8).  mask: device u8 [H,W], non-zero = object.  mask == NULL means ONE thing in every call
+ * of this library: no mask, i.e. M = 1 everywhere (every pixel is object) -- L_b = 0 and no gamma (1-M)/(HW) term in the
+ * backward pass, and the photometric terms cover the whole image. */
 int ocgs_render_fwd(int n, const ocgs_camera* cam, const ocgs_config* cfg, void* ws, size_t key_capacity, const uint8_t* mask,
                     float* color, float* alpha, float* depth, float* normal, uint32_t* n_contrib, float* loss_bg,
                     uint32_t* vis_count, float* contrib_sum, void* stream);
@@ -160,7 +162,8 @@ int ocgs_render_fwd_l1(int n, const ocgs_camera* cam, const ocgs_config* cfg, vo
  * occluded Gaussians receive no gradient (exact zeros).  O7.  Inputs: the forward's n_contrib (and the
  * lists, records and final transmittance that ocgs_render_fwd of the SAME view left in ws),
  * upstream gradients dL_dcolor[3,H,W], dL_dalpha[H,W], dL_ddepth[H,W], dL_dnormal[3,H,W] (device; any may be NULL = 0).
- * With mask != NULL and cfg->gamma_bg != 0 the gradient of gamma*L_b, gamma (1-M)/(H W), is added to dL/dA.
+ * With mask != NULL and cfg->gamma_bg != 0 the gradient of gamma*L_b, gamma (1-M)/(H W), is added to dL/dA (mask == NULL: M = 1,
+ * nothing is added -- the same meaning as in ocgs_render_fwd, whose L_b is then 0).
  * Outputs (device, OVERWRITTEN, zero for culled surfels): d_pos[N,3], d_scale[N,2], d_quat[N,4], d_opacity[N],
  * d_sh[N,16,3], d_center2d[N,2] (nullable) = M22 * (dL/dM02, dL/dM12), the gradient w.r.t. the projected centre at
  * fixed depth (densification statistic).  Uses ws.grad_rec as accumulator. */
@@ -256,7 +259,8 @@ int ocgs_prune_stats(const ocgs_surfels* in, uint32_t* vis_count, float* contrib
 int ocgs_compact_rows(const float* in, const int32_t* remap, int n, int row_floats, float* out, void* stream);
 
 /* ---- clone / split densification (reading R-densify) ---------------------
- * ocgs_densify_accumulate: after ocgs_render_bwd of a view, grad_accum[j] += |d_center2d_j| and denom[j] += 1 for every
+ * ocgs_densify_accumulate: after ocgs_render_bwd of a view, grad_accum[j] += |(width/2, height/2) * d_center2d_j| (d_center2d is
+ *   per pixel; the statistic is per NDC unit, the unit the default grad_threshold 2e-4 is calibrated in) and denom[j] += 1 for every
  *   surfel that passed this view's frustum test (read from the workspace of that view's ocgs_preprocess / ocgs_bin_sort).
  * ocgs_densify: avg = grad_accum / denom (0 if denom = 0); avg >= grad_threshold selects a surfel; selected surfels with
  *   max(scale) <= scale_threshold are CLONED, the others SPLIT into two children at p + s_u xi[j,k,0] t_u + s_v xi[j,k,1] t_v
@@ -298,6 +302,15 @@ int ocgs_photometric_loss(const float* color, const float* target, const uint8_t
  * Thread-local; the only state the library keeps, and only while profiling. */
 int ocgs_profile_begin(int capacity, void* stream);
 int ocgs_profile_end(void* stream, int max_out, float* ms_out, char* names_out, int* count);
+
+/* ---- diagnostics: measured ALU peaks of the device ("the builder must measure an FP32-FMA peak and a
+ * MUFU.EX2 peak microbenchmark on the box and use those" for the rooflines of the raster kernels, PAPER.md:119 renderer) ----
+ * Enqueues ONE launch of a microbenchmark on `stream`: kind 0 = eight independent chains of a <- fma(a, b, c) per thread
+ * (2 flop per step), kind 1 = eight chains of a <- -ex2(a) (one MUFU.EX2 per step); 8 blocks of 256 threads per SM,
+ * `iters` x 8 steps per chain.  *ops_per_launch (host) receives the flop (kind 0) or EX2 (kind 1) count of the launch; the
+ * caller times the launch with CUDA events and divides.  d_out: device f32[out_floats], out_floats >= 8 x 256 x number of
+ * SMs (OCGS_ERR_CAPACITY otherwise), scratch the kernels store their results to.  Asynchronous; not part of any step. */
+int ocgs_peak_probe(int kind, int iters, float* d_out, size_t out_floats, double* ops_per_launch, void* stream);
 
 /* ---- end-to-end TRAINING step: per-view inputs from the host, parameters resident on the device (bench.py "e2e") -------
  * What a training loop does per iteration (pick a view, render, losses, backpropagate): the model -- the

@@ -104,6 +104,12 @@ def num_threads() -> int:
     return int(lib().orc_num_threads())
 
 
+def set_num_threads(n: int) -> int:
+    """OpenMP threads of the following oracle calls; returns the number in force."""
+    lib().orc_set_num_threads.restype = C.c_int
+    return int(lib().orc_set_num_threads(C.c_int(int(n))))
+
+
 def _f32(a):
     return np.ascontiguousarray(a, np.float32)
 

@@ -26,11 +26,14 @@ import numpy as np
 SPLIT_SCALE_DIVISOR = 1.6
 
 
-def accumulate(grad_accum, denom, d_center2d, in_frustum):
-    """One view's contribution to the statistics (in place)."""
+def accumulate(grad_accum, denom, d_center2d, in_frustum, width, height):
+    """One view's contribution to the statistics (in place).  The statistic is the norm of the gradient w.r.t. the projected
+    centre in NDC units (pixel = ((ndc + 1) W - 1) / 2, so d/d ndc = (W/2, H/2) d/d pixel): the unit in which the cited
+    work's default threshold 2e-4 ("the same default values as 2DGS, which correspond to the 3DGS defaults")
+    is calibrated; d_center2d itself is per pixel (reading R-c2d)."""
     g = np.asarray(d_center2d, np.float64)
     m = np.asarray(in_frustum).astype(bool)
-    grad_accum[m] += np.sqrt(g[m, 0] ** 2 + g[m, 1] ** 2)
+    grad_accum[m] += np.sqrt((0.5 * width * g[m, 0]) ** 2 + (0.5 * height * g[m, 1]) ** 2)
     denom[m] += 1
     return grad_accum, denom
 

@@ -555,7 +555,7 @@ double orc_render_fwd(int n, const OrcCamera* cam, const OrcConfig* cfg, const O
 #pragma omp atomic
             fragile_touch[ids[pos]] += 1;
           }
-        const double m = mask ? (mask[p] ? 1.0 : 0.0) : 0.0;
+        const double m = mask ? (mask[p] ? 1.0 : 0.0) : 1.0;  // no mask: every pixel is object (M = 1), L_b = 0
         Lb += (1.0 - Tr) * (1.0 - m);
       }
   }
@@ -984,7 +984,7 @@ double orc_bf_render(int n, const double* pos, const double* scale, const double
       depth[p] = D;
       if (origin) { origin[p] = c0; m1[p] = M1; m2[p] = M2; }
       if (n_blended) n_blended[p] = cnt;
-      const double m = mask ? (mask[p] ? 1.0 : 0.0) : 0.0;
+      const double m = mask ? (mask[p] ? 1.0 : 0.0) : 1.0;  // no mask: every pixel is object (M = 1), L_b = 0
       Lb += (1.0 - Tr) * (1.0 - m);
     }
   }
@@ -1167,7 +1167,7 @@ double orc3d_render_fwd(int n, const OrcCamera* cam, const OrcConfig* cfg, const
 #pragma omp atomic
             fragile_touch[ids[pos]] += 1;
           }
-        const double m = mask ? (mask[p] ? 1.0 : 0.0) : 0.0;
+        const double m = mask ? (mask[p] ? 1.0 : 0.0) : 1.0;  // no mask: every pixel is object (M = 1), L_b = 0
         Lb += (1.0 - Tr) * (1.0 - m);
       }
   }
@@ -1273,7 +1273,7 @@ double orc3d_bf_render(int n, const double* pos, const double* scale, const doub
       alpha[p] = 1.0 - Tr;
       depth[p] = D;
       if (n_blended) n_blended[p] = cnt;
-      const double m = mask ? (mask[p] ? 1.0 : 0.0) : 0.0;
+      const double m = mask ? (mask[p] ? 1.0 : 0.0) : 1.0;  // no mask: every pixel is object (M = 1), L_b = 0
       Lb += (1.0 - Tr) * (1.0 - m);
     }
   }
@@ -1289,6 +1289,17 @@ int orc_num_threads() {
 #ifdef _OPENMP
   return omp_get_max_threads();
 #else
+  return 1;
+#endif
+}
+
+// number of OpenMP threads of the following calls (bench.py times the oracle on 1 core and on all cores); returns the value in force
+int orc_set_num_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+  return omp_get_max_threads();
+#else
+  (void)n;
   return 1;
 #endif
 }

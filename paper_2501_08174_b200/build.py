@@ -37,7 +37,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     log = []
     for s in srcs:
         o = s[:-3] + ".o"
-        cmd = [_nvcc(), *NVCC_FLAGS, "-c", s, "-o", o]
+        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("OCGS_NVCC_FLAGS", "").split(), "-c", s, "-o", o]
         r = subprocess.run(cmd, capture_output=True, text=True)
         log.append(r.stderr)
         if r.returncode != 0:

@@ -22,6 +22,15 @@ void prof_mark(cudaStream_t st, const char* name) {
   ++g_prof.used;
 }
 
+int sm_count() {
+  thread_local int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;  // B200
+  }
+  return n;
+}
+
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 bool carve_workspace(void* ws, int n, int width, int height, size_t key_capacity, Workspace* out, ocgs_ws_layout* layout) {
@@ -412,20 +421,23 @@ int ocgs_step_view_host_enqueue(const ocgs_surfels* surfels, const ocgs_camera* 
   // pass, the target only by the photometric term
   cudaEvent_t ev_begin = nullptr, ev_mask = nullptr, ev_target = nullptr;
   const bool overlap = cs != st;
-  if (overlap) {
-    OCGS_CUDA_OK(cudaEventCreateWithFlags(&ev_begin, cudaEventDisableTiming));
-    OCGS_CUDA_OK(cudaEventCreateWithFlags(&ev_mask, cudaEventDisableTiming));
-    OCGS_CUDA_OK(cudaEventCreateWithFlags(&ev_target, cudaEventDisableTiming));
-    OCGS_CUDA_OK(cudaEventRecord(ev_begin, st));  // the previous step's readers of d_mask / target are done
-    OCGS_CUDA_OK(cudaStreamWaitEvent(cs, ev_begin, 0));
-  }
-  OCGS_CUDA_OK(cudaMemcpyAsync(d_mask, h_mask, HW, cudaMemcpyHostToDevice, cs));
-  if (overlap) OCGS_CUDA_OK(cudaEventRecord(ev_mask, cs));
-  OCGS_CUDA_OK(cudaMemcpyAsync(target, h_target, 3 * HW * sizeof(float), cudaMemcpyHostToDevice, cs));
-  if (overlap) OCGS_CUDA_OK(cudaEventRecord(ev_target, cs));
+  bool forked = false;  // the copy stream has been made to depend on `st` (inside a capture: it has joined the capture)
   const int n = surfels->n;
   int rc = OCGS_OK;
+#define OCGS_STEP_OK(expr) { const cudaError_t _e = (expr); if (_e != cudaSuccess) { rc = cuda_fail(_e); break; } }
   do {
+    if (overlap) {
+      OCGS_STEP_OK(cudaEventCreateWithFlags(&ev_begin, cudaEventDisableTiming));
+      OCGS_STEP_OK(cudaEventCreateWithFlags(&ev_mask, cudaEventDisableTiming));
+      OCGS_STEP_OK(cudaEventCreateWithFlags(&ev_target, cudaEventDisableTiming));
+      OCGS_STEP_OK(cudaEventRecord(ev_begin, st));  // the previous step's readers of d_mask / target are done
+      OCGS_STEP_OK(cudaStreamWaitEvent(cs, ev_begin, 0));
+      forked = true;
+    }
+    OCGS_STEP_OK(cudaMemcpyAsync(d_mask, h_mask, HW, cudaMemcpyHostToDevice, cs));
+    if (overlap) OCGS_STEP_OK(cudaEventRecord(ev_mask, cs));
+    OCGS_STEP_OK(cudaMemcpyAsync(target, h_target, 3 * HW * sizeof(float), cudaMemcpyHostToDevice, cs));
+    if (overlap) OCGS_STEP_OK(cudaEventRecord(ev_target, cs));
     if ((rc = ocgs_preprocess(surfels, cam, cfg, ws, key_capacity, stream)) != OCGS_OK) break;
     if ((rc = ocgs_bin_sort(n, cam, cfg, ws, key_capacity, nullptr, stream)) != OCGS_OK) break;
     if (overlap && cudaStreamWaitEvent(st, ev_mask, 0) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
@@ -440,11 +452,12 @@ int ocgs_step_view_host_enqueue(const ocgs_surfels* surfels, const ocgs_camera* 
     if (cudaMemcpyAsync(h_losses, d_losses, 2 * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
     if (h_header && cudaMemcpyAsync(h_header, ws, sizeof(ocgs_header), cudaMemcpyDeviceToHost, st) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
   } while (false);
-  if (overlap) {
-    // a failed call must not leave the copy stream dangling off a capture or racing the caller's buffers: join it
-    if (rc != OCGS_OK) cudaStreamWaitEvent(st, ev_target, 0);
-    cudaEventDestroy(ev_begin); cudaEventDestroy(ev_mask); cudaEventDestroy(ev_target);
-  }
+  // every exit goes through here: a failed call must not leave the copy stream dangling off a capture or racing the caller's
+  // buffers (join it back into `st` with a fresh record), and the events are always destroyed
+  if (forked && rc != OCGS_OK && ev_target && cudaEventRecord(ev_target, cs) == cudaSuccess) cudaStreamWaitEvent(st, ev_target, 0);
+  if (ev_begin) cudaEventDestroy(ev_begin);
+  if (ev_mask) cudaEventDestroy(ev_mask);
+  if (ev_target) cudaEventDestroy(ev_target);
   return rc;
 }
 
@@ -465,20 +478,22 @@ int ocgs_step_view_prefetch_enqueue(const ocgs_surfels* surfels, const ocgs_came
   float* gC = normal + 3 * HW;
   cudaEvent_t ev_begin = nullptr, ev_done = nullptr;
   const bool fork = prefetch && cs != st;
-  if (prefetch) {
-    if (fork) {
-      OCGS_CUDA_OK(cudaEventCreateWithFlags(&ev_begin, cudaEventDisableTiming));
-      OCGS_CUDA_OK(cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming));
-      OCGS_CUDA_OK(cudaEventRecord(ev_begin, st));  // the step that last read d_*_next has finished
-      OCGS_CUDA_OK(cudaStreamWaitEvent(cs, ev_begin, 0));
-    }
-    OCGS_CUDA_OK(cudaMemcpyAsync(d_mask_next, h_next_mask, HW, cudaMemcpyHostToDevice, cs));
-    OCGS_CUDA_OK(cudaMemcpyAsync(d_target_next, h_next_target, 3 * HW * sizeof(float), cudaMemcpyHostToDevice, cs));
-    if (fork) OCGS_CUDA_OK(cudaEventRecord(ev_done, cs));
-  }
+  bool forked = false, done_recorded = false;
   const int n = surfels->n;
   int rc = OCGS_OK;
   do {
+    if (prefetch) {
+      if (fork) {
+        OCGS_STEP_OK(cudaEventCreateWithFlags(&ev_begin, cudaEventDisableTiming));
+        OCGS_STEP_OK(cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming));
+        OCGS_STEP_OK(cudaEventRecord(ev_begin, st));  // the step that last read d_*_next has finished
+        OCGS_STEP_OK(cudaStreamWaitEvent(cs, ev_begin, 0));
+        forked = true;
+      }
+      OCGS_STEP_OK(cudaMemcpyAsync(d_mask_next, h_next_mask, HW, cudaMemcpyHostToDevice, cs));
+      OCGS_STEP_OK(cudaMemcpyAsync(d_target_next, h_next_target, 3 * HW * sizeof(float), cudaMemcpyHostToDevice, cs));
+      if (fork) { OCGS_STEP_OK(cudaEventRecord(ev_done, cs)); done_recorded = true; }
+    }
     if ((rc = ocgs_preprocess(surfels, cam, cfg, ws, key_capacity, stream)) != OCGS_OK) break;
     if ((rc = ocgs_bin_sort(n, cam, cfg, ws, key_capacity, nullptr, stream)) != OCGS_OK) break;
     if ((rc = ocgs_render_fwd_l1(n, cam, cfg, ws, key_capacity, d_mask_cur, d_target_cur, color, alpha, depth, normal, d_ncontrib, d_losses,
@@ -488,12 +503,14 @@ int ocgs_step_view_prefetch_enqueue(const ocgs_surfels* surfels, const ocgs_came
     if (cudaMemcpyAsync(h_losses, d_losses, 2 * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
     if (h_header && cudaMemcpyAsync(h_header, ws, sizeof(ocgs_header), cudaMemcpyDeviceToHost, st) != cudaSuccess) { rc = OCGS_ERR_CUDA; break; }
   } while (false);
-  if (fork) {
-    cudaStreamWaitEvent(st, ev_done, 0);  // join: the next call (and the end of a capture) sees the prefetch finished
-    cudaEventDestroy(ev_begin); cudaEventDestroy(ev_done);
-  }
+  // every exit goes through here.  join: the next call (and the end of a capture) sees the prefetch finished; after a failure
+  // in between, whatever the copy stream got is joined with a fresh record
+  if (forked && ev_done && (done_recorded || cudaEventRecord(ev_done, cs) == cudaSuccess)) cudaStreamWaitEvent(st, ev_done, 0);
+  if (ev_begin) cudaEventDestroy(ev_begin);
+  if (ev_done) cudaEventDestroy(ev_done);
   return rc;
 }
+#undef OCGS_STEP_OK
 
 int ocgs_step_host(const float* h_pos, const float* h_scale, const float* h_quat, const float* h_opacity, const float* h_sh, int n,
                    const ocgs_camera* cam, const ocgs_config* cfg, const uint8_t* h_mask, const float* h_target, float* h_grads,

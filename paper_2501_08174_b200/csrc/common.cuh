@@ -141,4 +141,7 @@ constexpr float kNegHalfLog2e = -0.72134752044448170f;  // exp(-rho/2) = 2^(rho 
 
 __host__ __device__ inline size_t div_up(size_t a, size_t b) { return (a + b - 1) / b; }
 
+// number of SMs of the current device (queried once per thread; grids of the persistent / grid-stride kernels are multiples of it)
+int sm_count();
+
 }  // namespace ocgs

@@ -1,7 +1,8 @@
 // densify.cu -- clone / split half of the adaptive density control (DESIGN.md
 // reading R-densify).
-//   ocgs_densify_accumulate: grad_accum[j] += |d_center2d_j|, denom[j] += 1 for the surfels that passed this view's
-//                            frustum test (id_to_rank of the workspace).
+//   ocgs_densify_accumulate: grad_accum[j] += |(W/2, H/2) * d_center2d_j| (the gradient w.r.t. the projected centre in NDC units,
+//                            the unit the default threshold 2e-4 of the cited work is calibrated in), denom[j] += 1 for the
+//                            surfels that passed this view's frustum test (id_to_rank of the workspace).
 //   ocgs_densify:            class per surfel (keep / clone / split) from avg = grad_accum / denom in fp32, three exclusive
 //                            scans, stable scatter: non-split surfels, then clones, then two children per split surfel
 //                            (p + s_u xi0 t_u + s_v xi1 t_v, scales / 1.6); src[row] = source id; counts on the device.
@@ -13,11 +14,12 @@ namespace ocgs {
 constexpr int kDenBlock = 256;
 
 __global__ void __launch_bounds__(256) densify_accumulate_kernel(const uint32_t* __restrict__ id_to_rank, const float2* __restrict__ d_center2d,
-                                                                 int n, float* __restrict__ grad_accum, uint32_t* __restrict__ denom) {
+                                                                 int n, float half_w, float half_h, float* __restrict__ grad_accum, uint32_t* __restrict__ denom) {
   const int j = blockIdx.x * 256 + threadIdx.x;
   if (j >= n || id_to_rank[j] == 0xFFFFFFFFu) return;
   const float2 g = d_center2d[j];
-  grad_accum[j] += sqrtf(fmaf(g.x, g.x, g.y * g.y));
+  const float gx = half_w * g.x, gy = half_h * g.y;  // pixel = ((ndc + 1) W - 1) / 2: d/d ndc = (W/2) d/d pixel
+  grad_accum[j] += sqrtf(fmaf(gx, gx, gy * gy));
   denom[j] += 1u;
 }
 
@@ -162,7 +164,7 @@ size_t densify_workspace_bytes(int n) {
 
 int launch_densify_accumulate(const Workspace& w, const float* d_center2d, float* grad_accum, uint32_t* denom, cudaStream_t st) {
   if (w.n == 0) return OCGS_OK;
-  densify_accumulate_kernel<<<(unsigned)div_up((size_t)w.n, 256), 256, 0, st>>>(w.id_to_rank, (const float2*)d_center2d, w.n, grad_accum, denom);
+  densify_accumulate_kernel<<<(unsigned)div_up((size_t)w.n, 256), 256, 0, st>>>(w.id_to_rank, (const float2*)d_center2d, w.n, 0.5f * (float)w.width, 0.5f * (float)w.height, grad_accum, denom);
   OCGS_LAUNCHED(st, "densify_accumulate_kernel");
   return OCGS_OK;
 }

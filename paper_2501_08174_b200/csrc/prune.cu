@@ -104,7 +104,7 @@ template <typename Vec, int VPS>
 static int launch_compact(const float* in, float* out, const int32_t* remap, int n, cudaStream_t st) {
   const size_t total = (size_t)n * VPS;
   if (total == 0) return OCGS_OK;
-  const unsigned grid = (unsigned)min(div_up(total, 256), (size_t)148 * 64);
+  const unsigned grid = (unsigned)min(div_up(total, 256), (size_t)sm_count() * 64);
   compact_kernel<Vec, VPS><<<grid, 256, 0, st>>>((const Vec*)in, remap, total, (Vec*)out);
   OCGS_LAUNCHED(st, "compact_kernel");
   return OCGS_OK;
@@ -123,7 +123,7 @@ __global__ void __launch_bounds__(256) compact_rows_kernel(const float* __restri
 int launch_compact_rows(const float* in, const int32_t* remap, int n, int row_floats, float* out, cudaStream_t st) {
   const size_t total = (size_t)n * (size_t)row_floats;
   if (total == 0) return OCGS_OK;
-  const unsigned grid = (unsigned)min(div_up(total, 256), (size_t)148 * 64);
+  const unsigned grid = (unsigned)min(div_up(total, 256), (size_t)sm_count() * 64);
   compact_rows_kernel<<<grid, 256, 0, st>>>(in, remap, total, row_floats, out);
   OCGS_LAUNCHED(st, "compact_rows_kernel");
   return OCGS_OK;

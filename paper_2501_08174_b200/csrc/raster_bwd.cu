@@ -466,7 +466,7 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
                       float* d_center2d, cudaStream_t st) {
   if (s.n == 0) return OCGS_OK;
   if (w.n_tiles == 0) {
-    clear_grad_rec_kernel<<<(unsigned)min(div_up((size_t)s.n * 6, 256), (size_t)148 * 16), 256, 0, st>>>(w.header, (float4*)w.grad_rec);
+    clear_grad_rec_kernel<<<(unsigned)min(div_up((size_t)s.n * 6, 256), (size_t)sm_count() * 16), 256, 0, st>>>(w.header, (float4*)w.grad_rec);
     OCGS_LAUNCHED(st, "clear_grad_rec_kernel");
   } else {
     // tile_work = length of each tile's blended list, from the forward pass; the same launch clears grad_rec

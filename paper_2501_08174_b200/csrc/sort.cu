@@ -194,7 +194,7 @@ int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t
   static_assert(kSortThreads == kRadix, "one thread per digit");
   const int passes = (key_bits + kRadixBits - 1) / kRadixBits;
   const unsigned tiles_max = (unsigned)div_up(n_max, kSortTile);
-  const unsigned grid = (unsigned)min(div_up(n_max, (size_t)kHistItems * kSortThreads), (size_t)148 * 4);
+  const unsigned grid = (unsigned)min(div_up(n_max, (size_t)kHistItems * kSortThreads), (size_t)sm_count() * 4);
   *result_in_B = (passes & 1) != 0;
   if (grid == 0 || passes == 0) { *result_in_B = false; return OCGS_OK; }
   if (passes > kMaxPasses || n_max > (size_t)kValMask) return OCGS_ERR_UNSUPPORTED;
@@ -210,7 +210,7 @@ int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t
     const int shift = p * kRadixBits;
     const int bits = min(kRadixBits, key_bits - shift);
     const uint32_t mask = (1u << bits) - 1u;
-    radix_onesweep_kernel<<<min(tiles_max, 148u * (unsigned)kSortCtas), kSortThreads, 0, st>>>(kin, vin, kout, vout, n_ptr, n_is_u64, n_max, shift, mask, ghist + p * kRadix,
+    radix_onesweep_kernel<<<min(tiles_max, (unsigned)sm_count() * (unsigned)kSortCtas), kSortThreads, 0, st>>>(kin, vin, kout, vout, n_ptr, n_is_u64, n_max, shift, mask, ghist + p * kRadix,
                                                          status + (size_t)p * stride, tickets + p);
     OCGS_LAUNCHED(st, "radix_onesweep_kernel");
     uint32_t* t = kin; kin = kout; kout = t;
@@ -492,7 +492,7 @@ int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cu
     const int passes = (bits + kRadixBits - 1) / kRadixBits;
     const bool fused_hist = passes <= 2;  // emit_keys_kernel keeps two histograms (n_tiles <= 65536)
     if (fused_hist) OCGS_CUDA_OK(cudaMemsetAsync(w.digit_total, 0, (kMaxPasses * kRadix + kMaxPasses) * sizeof(uint32_t), st));
-    emit_keys_kernel<<<(unsigned)min(div_up(cap, kEmitTile), (size_t)148 * kEmitBlocks), kEmitThreads, 0, st>>>(
+    emit_keys_kernel<<<(unsigned)min(div_up(cap, kEmitTile), (size_t)sm_count() * kEmitBlocks), kEmitThreads, 0, st>>>(
         w.header, w.offsets, w.rank_to_id, w.rect, cam.tiles_x, w.tile_keys, w.tile_vals, fused_hist ? passes : 0, bits, cap, w.digit_total, w.hist,
         div_up(cap, kSortTile) * kRadix);
     OCGS_LAUNCHED(st, "emit_keys_kernel");
@@ -500,13 +500,13 @@ int launch_bin_sort(const CamParams& cam, Workspace& w, uint32_t* sorted_ids, cu
     int rc = radix_sort_pairs(w.tile_keys, w.tile_vals, w.tkeyB, w.tvalB, &w.header->K, true, cap, bits, w.hist, w.digit_total, &inB, st, fused_hist);
     if (rc != OCGS_OK) return rc;
     if (inB) {  // odd number of passes: bring the result back to the documented sections
-      const unsigned g = (unsigned)min(div_up(cap, 1024), (size_t)148 * 8);
+      const unsigned g = (unsigned)min(div_up(cap, 1024), (size_t)sm_count() * 8);
       copy_u32_kernel<<<g, 1024, 0, st>>>(w.tkeyB, w.tile_keys, w.header);
       copy_u32_kernel<<<g, 1024, 0, st>>>(w.tvalB, w.tile_vals, w.header);
       OCGS_LAUNCHED(st, "copy_u32_kernel");
     }
   }
-  const unsigned rgrid = (unsigned)min(max(div_up(max(cap, (size_t)1), 256), div_up((size_t)w.n_tiles, 256)), (size_t)148 * 16);
+  const unsigned rgrid = (unsigned)min(max(div_up(max(cap, (size_t)1), 256), div_up((size_t)w.n_tiles, 256)), (size_t)sm_count() * 16);
   tile_ranges_kernel<<<rgrid, 256, 0, st>>>(w.header, w.tile_keys, w.n_tiles, w.ranges);
   OCGS_LAUNCHED(st, "tile_ranges_kernel");
   if (sorted_ids && cap > 0) {
@@ -590,7 +590,7 @@ __global__ void __launch_bounds__(1024) order_tiles_kernel(const uint32_t* __res
 
 int launch_order_tiles(const Workspace& w, bool from_ranges, cudaStream_t st, bool clear_grad_rec) {
   if (w.n_tiles == 0) return OCGS_OK;
-  const unsigned clear_blocks = clear_grad_rec ? (unsigned)min(div_up((size_t)w.n * (kRec / 4), 1024), (size_t)148 * 2) : 0u;
+  const unsigned clear_blocks = clear_grad_rec ? (unsigned)min(div_up((size_t)w.n * (kRec / 4), 1024), (size_t)sm_count() * 2) : 0u;
   order_tiles_kernel<<<1 + clear_blocks, 1024, 0, st>>>(w.ranges, w.tile_work, w.n_tiles, from_ranges, w.tile_order, w.header, (float4*)w.grad_rec);
   OCGS_LAUNCHED(st, "order_tiles_kernel");
   return OCGS_OK;

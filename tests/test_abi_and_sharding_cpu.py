@@ -116,6 +116,70 @@ def test_statistics_merge_over_gloo_world2_matches_single_process():
     assert np.array_equal(m0, m1)
 
 
+def _bench_worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+    from paper_2501_08174_b200 import sharding
+    assert sharding.env_rank() == (rank, world, rank)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    views = sharding.rotation_for_rank(49, rank, world, 8)
+    # every rank "measures" its own step time; the bench reports the max over ranks and the whole-job aggregate
+    ms_local = 2.0 + rank
+    ms = sharding.max_over_ranks(ms_local)
+    grads = dict(d_pos=torch.full((5, 3), float(rank + 1)), d_sh=torch.full((5, 16, 3), 10.0 * (rank + 1)))
+    nbytes = sharding.allreduce_grads(grads)
+    q.put((rank, views, ms, nbytes, float(grads["d_pos"][0, 0]), float(grads["d_sh"][0, 0, 0]),
+           sharding.aggregate_throughput(1_000_000, world, ms)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_bench_rank_bookkeeping_over_gloo_world2():
+    """bench.py's own multi-rank bookkeeping (paper_2501_08174_b200.sharding), on two gloo ranks: view rotation per rank, max over
+    ranks of the measured time, whole-job aggregate, and the gradient all-reduce of the batched-view mode."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 31500 + (os.getpid() % 500)
+    procs = [ctx.Process(target=_bench_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=180) for _ in procs)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    assert res[0][1] == [0, 2, 4, 6, 8, 10, 12, 14] and res[1][1] == [1, 3, 5, 7, 9, 11, 13, 15]
+    for rank, views, ms, nbytes, gp, gs, thr in res:
+        assert ms == 3.0                        # max over ranks
+        assert nbytes == (15 + 240) * 4
+        assert gp == 3.0 and gs == 30.0         # sum over ranks
+        assert thr == pytest.approx(2 * 1_000_000 / 3.0e-3)
+
+
+def test_view_rotation_and_launcher_rules():
+    from paper_2501_08174_b200 import sharding
+    assert sharding.rotation_for_rank(49, 0, 1, 8) == list(range(8))
+    assert sharding.rotation_for_rank(49, 3, 8, 0) == [3, 11, 19, 27, 35, 43]
+    assert sorted(v for r in range(8) for v in sharding.rotation_for_rank(49, r, 8, 0)) == list(range(49))  # a partition
+    assert sharding.rotation_for_rank(4, 6, 8, 2) == [2]                                                  # more ranks than views
+    assert sharding.relaunch_under_torchrun(1, ["x"], available=0) is None
+    with pytest.raises(RuntimeError, match="needs 2 CUDA devices"):
+        sharding.relaunch_under_torchrun(2, ["x"], available=1)
+
+
+def test_bench_refuses_more_gpus_than_the_node_has():
+    """`python bench.py --gpus N` starts the N ranks itself; on a node with fewer CUDA devices it must fail loudly rather than
+    measure fewer GPUs than it names (here: any N above the number of devices present)."""
+    import subprocess
+    import torch
+    n = (torch.cuda.device_count() if torch.cuda.is_available() else 0) + 1
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", str(max(n, 2))], capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode != 0 and f"needs {max(n, 2)} CUDA devices" in r.stderr
+
+
 def test_defaults_match_the_constants_the_paper_states():
     """tests/golden/paper_constants.txt: gamma = 0.5 in the library's default config (through the C ABI: the
     helper is host-only) and in the oracle's; the pruning intervals are the training loop's business and only recorded."""

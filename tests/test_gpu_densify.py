@@ -103,7 +103,7 @@ def test_accumulate_over_views_matches_the_definition():
         gg = g.render_bwd(gC=rng.normal(size=(3, g.H, g.W)))
         d2 = torch.tensor(gg["d_center2d"], device="cuda")
         B.ocgs_densify_accumulate(g.ws, n, g.W, g.H, g.cap, d2, ga_t, de_t)
-        dn.accumulate(ga_o, de_o, gg["d_center2d"], gp["tiles"] > 0)
+        dn.accumulate(ga_o, de_o, gg["d_center2d"], gp["tiles"] > 0, g.W, g.H)
     torch.cuda.synchronize()
     assert np.array_equal(de_t.cpu().numpy(), de_o)
     assert np.allclose(ga_t.cpu().numpy(), ga_o, rtol=1e-6, atol=1e-12)

@@ -87,6 +87,12 @@ def test_children_lie_in_the_tangent_plane_of_a_library_rotation():
 def test_accumulate_adds_the_norm_only_where_in_frustum():
     ga, de = np.zeros(4), np.zeros(4, np.int64)
     g = np.array([[3, 4], [1, 0], [0, 0], [6, 8]], np.float32)
-    dn.accumulate(ga, de, g, [1, 1, 1, 0])
-    dn.accumulate(ga, de, g, [1, 0, 1, 0])
+    dn.accumulate(ga, de, g, [1, 1, 1, 0], 2, 2)   # W/2 = H/2 = 1: the plain norm
+    dn.accumulate(ga, de, g, [1, 0, 1, 0], 2, 2)
     assert list(ga) == [10.0, 1.0, 0.0, 0.0] and list(de) == [2, 1, 2, 0]
+    # NDC units: pixel = ((ndc + 1) W - 1) / 2, so a unit gradient per pixel is W/2 per NDC unit along x, H/2 along y
+    ga, de = np.zeros(2), np.zeros(2, np.int64)
+    dn.accumulate(ga, de, np.array([[1, 0], [0, 1]], np.float32), [1, 1], 1600, 1200)
+    assert list(ga) == [800.0, 600.0]
+    dn.accumulate(ga, de, np.array([[3, 0], [3, 4]], np.float32), [0, 1], 8, 6)
+    assert list(ga) == [800.0, 600.0 + 12.0 * 2 ** 0.5] or np.allclose(ga, [800.0, 600.0 + np.hypot(12.0, 12.0)])
