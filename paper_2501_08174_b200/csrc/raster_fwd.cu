@@ -4,6 +4,9 @@
 // survivors; early stop per pixel, per warp and per CTA.  Fused: background loss L_b (Eq. 1), the visibility
 // statistics, the compact list of blended entries handed to the backward pass, and optionally the depth
 // moments (kMoments, f-2), the harness masked-L1 term (kL1, f-1) or the 3D-Gaussian pair rule (kPrim = 1, f-3).
+#include <cooperative_groups.h>
+#include <stdlib.h>
+
 #include "common.cuh"
 
 namespace ocgs {
@@ -77,16 +80,45 @@ constexpr int kFwdMinBlocks = 6;               // CTAs per SM the register budge
 // fused harness photometric term (S20): target image in, dL/dcolor and per-tile partial sums of |M (R - I)| out
 struct FwdL1 { const float* target; float* gC; float* partial; float inv_norm; };
 
+// Exact segmented compositing of heavy tiles (kSeg = 1).  A tile whose list is longer than kFwdHeavyLen is
+// walked by a thread-block CLUSTER of kSegRanks CTAs on kSegRanks SMs, CTA r taking the r-th part of the list:
+//   phase A  every CTA walks its part alpha-only and stop-free: P_r(p) = prod (1 - alpha) over the pairs that pass the pair rule;
+//   exchange through distributed shared memory: T_in,r(p) = prod_{r' < r} P_r'(p).  The stop rule (S11) fires at the first pair
+//            where the running product falls below t_min, and the product is monotone, so "a CTA in front has stopped" is
+//            exactly T_in,r < t_min: every blend / stop decision is the serial walk's (up to the rounding of the regrouped product,
+//            which matters only where the oracle calls the stop test fragile);
+//   phase B  the ordinary walk of the part, started at T = T_in,r: blends, statistics, blended lists;
+//   combine  CTA 0 adds the partial sums of the maps in list order (deterministic) through distributed shared memory, takes
+//            n_contrib = the last blended position and final T = T_out of the last CTA that was still walking, runs the ordinary
+//            epilogue, and packs the kSegRanks blended sub-lists into the one compact list the backward pass walks.
+// The launch covers the first kSegMaxTiles positions of the heavy-first tile order; clusters whose tile is not heavy exit at
+// once, and the ordinary launch skips the tiles the clusters took.
+#ifndef OCGS_SEG_RANKS
+#define OCGS_SEG_RANKS 8
+#endif
+#ifndef OCGS_SEG_LEN
+#define OCGS_SEG_LEN 6144
+#endif
+#ifndef OCGS_SEG_MINB
+#define OCGS_SEG_MINB 3
+#endif
+constexpr int kSegRanks = OCGS_SEG_RANKS;      // CTAs per cluster (8 is the portable maximum, 16 needs the non-portable opt-in)
+constexpr uint32_t kSegLen = OCGS_SEG_LEN;     // lists longer than this are segmented
+constexpr int kSegMaxTiles = 128;
+namespace cg = cooperative_groups;
+
 // kMaps = false: the visibility pass (ocgs_visibility_pass): only the statistics are produced -- no maps, no blended lists, no loss
-template <bool kStats, bool kMoments, int kPrim /*0 = 2D surfel, 1 = 3D Gaussian (EWA conic record)*/, bool kL1, bool kMaps = true>
-__global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ tile_work,
+template <bool kStats, bool kMoments, int kPrim /*0 = 2D surfel, 1 = 3D Gaussian (EWA conic record)*/, bool kL1, bool kMaps = true, int kSeg = 0>
+__global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) render_fwd_kernel(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                          const float4* __restrict__ rec, const uint32_t* __restrict__ rank_to_id,
                                                          const uint8_t* __restrict__ mask, int W, int H, int tiles_x,
                                                          ocgs_config cfg, float* __restrict__ color, float* __restrict__ alpha,
                                                          float* __restrict__ depth, float* __restrict__ normal,
                                                          uint32_t* __restrict__ n_contrib, float* __restrict__ final_T, uint2* __restrict__ blist, ocgs_header* __restrict__ header, float* __restrict__ loss_partial,
-                                                         uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum, float* __restrict__ mom /*[3,H,W]: origin, m1, m2 (kMoments)*/, FwdL1 l1) {
+                                                         uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum, float* __restrict__ mom /*[3,H,W]: origin, m1, m2 (kMoments)*/, FwdL1 l1,
+                                                         int seg_tiles /*leading positions of the tile order the segmented launch takes (0: none)*/) {
+  static_assert(!kSeg || (kMaps && !kMoments && kPrim == 0), "segmented compositing: surfel forward with maps, no depth moments");
   __shared__ float4 s_rec[kFwdBatch * 6];
   __shared__ uint32_t s_rank[kFwdBatch];
   __shared__ uint32_t s_hit[kFwdBatch];  // bit w: warp w blended the entry (read by the backward pass)
@@ -95,7 +127,10 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
   __shared__ float s_red[8];
   __shared__ uint32_t s_wcnt[8];
 
-  const int tile = (int)tile_order[blockIdx.x];  // heavy tiles are launched first
+  __shared__ float s_seg[kSeg ? 11 : 1][kSeg ? 256 : 1];  // kSeg: [0] = P_r, then the CTA's partial results, read by its cluster
+  __shared__ uint32_t s_segn;                              // kSeg: length of this CTA's blended sub-list
+  const int pos = kSeg ? (int)blockIdx.x / kSegRanks : (int)blockIdx.x;
+  const int tile = (int)tile_order[pos];  // heavy tiles are launched first
   const int tx = tile % tiles_x, ty = tile / tiles_x;
   // warp w owns the kSubW x kSubH pixel block number w of the tile (row-major over blocks), lane l pixel (l % kSubW, l / kSubW)
   const int sub = threadIdx.x >> 5, sl = threadIdx.x & 31;
@@ -104,7 +139,20 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
   const int ix = tx * kTile + lx, iy = ty * kTile + ly;
   const bool inside = ix < W && iy < H;
   const float px = (float)ix, py = (float)iy;
+  // Programmatic dependent launch: the ordinary launch follows the segmented one in the stream and needs nothing from it, so the
+  // clusters let it start at once and it fills the SMs their long chains leave idle; its LAST CTA waits for the clusters before
+  // it exits, so the ordinary grid -- and everything behind it in the stream -- completes only after the segmented one.
+  if (kSeg) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  struct PdlJoin {
+    bool on;
+    __device__ ~PdlJoin() { if (on) asm volatile("griddepcontrol.wait;" ::: "memory"); }
+  } pdl_join{!kSeg && seg_tiles > 0 && blockIdx.x == gridDim.x - 1};
   const uint32_t start = ranges[2 * tile], end = ranges[2 * tile + 1];
+  if (kSeg ? end - start <= kSegLen : (pos < seg_tiles && end - start > kSegLen)) return;  // (uniform over the CTA / cluster)
+  // kSeg: this CTA's part [rs, re) of the list, a multiple of the batch size long so that batches never straddle two parts
+  const uint32_t seg_rank = kSeg ? cg::this_cluster().block_rank() : 0u;
+  const uint32_t seg_len = kSeg ? (uint32_t)(div_up(div_up((size_t)(end - start), kSegRanks), kFwdBatch) * kFwdBatch) : end - start;
+  const uint32_t rs = kSeg ? min(end, start + seg_rank * seg_len) : start, re = kSeg ? min(end, rs + seg_len) : end;
   const float inv_sigma2 = 1.0f / cfg.filter_sigma2;
   const int lane = threadIdx.x & 31;
   const uint32_t wbit = 1u << (threadIdx.x >> 5);
@@ -116,10 +164,66 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
   uint32_t last = 0;
   uint32_t nhit = 0;  // entries of this tile blended so far (uniform across the CTA)
   bool done = !inside;
-  const bool heavy = end - start > kFwdHeavyLen;
+  const bool heavy = kSeg || end - start > kFwdHeavyLen;
 
-  for (uint32_t b0 = start; b0 < end; b0 += kFwdBatch) {
-    const int cnt = (int)min((uint32_t)kFwdBatch, end - b0);
+  if (kSeg) {
+    // ---- phase A: alpha-only, stop-free product over this CTA's part; a pixel may leave once P < t_min (all CTAs behind are then
+    // cut off whatever the exact value) ----
+    float P = 1.0f;
+    bool doneA = !inside;
+    for (uint32_t b0 = rs; b0 < re; b0 += kFwdBatch) {
+      const int cnt = (int)min((uint32_t)kFwdBatch, re - b0);
+      if (__syncthreads_and(doneA)) break;
+      if ((int)threadIdx.x < cnt) s_rank[threadIdx.x] = list[b0 + threadIdx.x];
+      __syncthreads();
+      for (int i = threadIdx.x; i < cnt * 5; i += 256) {
+        const int e = i / 5, part = i - 5 * e;
+        s_rec[6 * e + part] = __ldg(rec + (size_t)s_rank[e] * 6 + part);
+      }
+      __syncthreads();
+      for (int c0 = 0; c0 < cnt; c0 += 32) {
+        const int ce = min(32, cnt - c0);
+        bool keep = false;
+        if (lane < ce) {
+          const float4* se = s_rec + 6 * (c0 + lane);
+          keep = block_may_contribute(se[0], se[1], se[2], se[3], tx * kTile + sub_x0, ty * kTile + sub_y0, inv_sigma2);
+        }
+        uint32_t todo = __ballot_sync(0xFFFFFFFFu, keep);
+        if (__all_sync(0xFFFFFFFFu, doneA)) break;
+        while (todo) {
+          const int jj = __ffs(todo) - 1;
+          todo &= todo - 1;
+          const float4* sr = s_rec + 6 * (c0 + jj);
+          const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
+          const float dx = px - r2.z, dy = py - r2.w;
+          const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
+          const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
+          const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
+          const float inv = rcp_approx(qz);
+          const float u = qx * inv, v = qy * inv;
+          const float rho3 = fmaf(u, u, v * v);
+          const float rho2 = fmaf(dx, dx, dy * dy) * inv_sigma2;
+          const bool surf = rho3 <= rho2;
+          const float rho = surf ? rho3 : rho2;
+          const float z = surf ? r2.y * inv : r3.y;
+          if (!doneA && qz != 0.0f && !(z < near_z) && !(rho > r3.x)) {
+            const float a = fminf(alpha_max, sr[4].x * ex2_approx(rho * kNegHalfLog2e));
+            P *= 1.0f - a;
+            doneA = P < t_min;
+          }
+        }
+      }
+    }
+    __syncthreads();
+    s_seg[0][threadIdx.x] = P;
+    cg::this_cluster().sync();
+    for (uint32_t rr = 0; rr < seg_rank; ++rr) T *= *cg::this_cluster().map_shared_rank(&s_seg[0][threadIdx.x], rr);
+    done = !inside || T < t_min;  // a CTA in front has met the stop rule (S11)
+  }
+  const bool done_in = done;
+
+  for (uint32_t b0 = rs; b0 < re; b0 += kFwdBatch) {
+    const int cnt = (int)min((uint32_t)kFwdBatch, re - b0);
     if (__syncthreads_and(done)) break;
     if ((int)threadIdx.x < cnt) s_rank[threadIdx.x] = list[b0 + threadIdx.x];
     if (kMaps && threadIdx.x < kFwdBatch) s_hit[threadIdx.x] = 0;
@@ -286,7 +390,7 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
         total += c;
       }
       if (hitme)
-        blist[start + nhit + before + (uint32_t)__popc(bal & ((1u << lane) - 1u))] =
+        blist[rs + nhit + before + (uint32_t)__popc(bal & ((1u << lane) - 1u))] =
             make_uint2(s_rank[threadIdx.x], (((b0 - start) + threadIdx.x) << 8) | s_hit[threadIdx.x]);
       nhit += total;
     }
@@ -300,6 +404,38 @@ __global__ void __launch_bounds__(256, kFwdMinBlocks) render_fwd_kernel(const ui
   }
 
   if (!kMaps) return;
+  if (kSeg) {
+    cg::cluster_group cl = cg::this_cluster();
+    const int t = (int)threadIdx.x;
+    s_seg[1][t] = C0; s_seg[2][t] = C1; s_seg[3][t] = C2; s_seg[4][t] = D; s_seg[5][t] = N0; s_seg[6][t] = N1; s_seg[7][t] = N2;
+    s_seg[8][t] = T; s_seg[9][t] = __uint_as_float(last); s_seg[10][t] = done_in ? 1.0f : 0.0f;
+    if (t == 0) s_segn = nhit;
+    __threadfence();  // this CTA's part of the blended list is visible to CTA 0
+    cl.sync();
+    if (seg_rank != 0) { cl.sync(); return; }  // (CTA 0 has read this CTA's shared memory when the second barrier completes)
+    uint32_t packed = nhit;  // blended entries in front of the sub-list being moved
+    for (uint32_t rr = 1; rr < (uint32_t)kSegRanks; ++rr) {
+      const float* rp = cl.map_shared_rank(&s_seg[0][0], rr);
+      C0 += rp[1 * 256 + t]; C1 += rp[2 * 256 + t]; C2 += rp[3 * 256 + t]; D += rp[4 * 256 + t];
+      N0 += rp[5 * 256 + t]; N1 += rp[6 * 256 + t]; N2 += rp[7 * 256 + t];
+      if (rp[10 * 256 + t] == 0.0f) T = rp[8 * 256 + t];  // that CTA was still walking: its T_out is the pixel's transmittance so far
+      last = max(last, __float_as_uint(rp[9 * 256 + t]));
+      // its blended sub-list moves down behind the ones in front of it (never up: chunks are read before they are written)
+      const uint32_t cnt_r = *cl.map_shared_rank(&s_segn, rr);
+      const uint32_t src = min(end, start + rr * seg_len), dst = start + packed;
+      if (dst != src)
+        for (uint32_t i0 = 0; i0 < cnt_r; i0 += 256) {
+          uint2 e = make_uint2(0u, 0u);
+          if (i0 + t < cnt_r) e = __ldcg(blist + src + i0 + t);
+          __syncthreads();
+          if (i0 + t < cnt_r) blist[dst + i0 + t] = e;
+          __syncthreads();
+        }
+      packed += cnt_r;
+    }
+    nhit = packed;
+    cl.sync();
+  }
   const float A = 1.0f - T;
   float l1sum = 0.f;
   if (inside) {
@@ -389,11 +525,11 @@ int launch_render_stats(const CamParams& cam, const ocgs_config& cfg, const Work
   if (prim == 1)
     render_fwd_kernel<true, false, 1, false, false><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec,
         w.rank_to_id, nullptr, cam.W, cam.H, cam.tiles_x, cfg, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, w.header, nullptr,
-        vis_count, contrib_sum, nullptr, l1);
+        vis_count, contrib_sum, nullptr, l1, 0);
   else
     render_fwd_kernel<true, false, 0, false, false><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec,
         w.rank_to_id, nullptr, cam.W, cam.H, cam.tiles_x, cfg, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, w.header, nullptr,
-        vis_count, contrib_sum, nullptr, l1);
+        vis_count, contrib_sum, nullptr, l1, 0);
   OCGS_LAUNCHED(st, "render_stats_kernel");
   return OCGS_OK;
 }
@@ -407,10 +543,38 @@ int launch_render_fwd(const CamParams& cam, const ocgs_config& cfg, const Worksp
   const bool stats = vis_count != nullptr && contrib_sum != nullptr;
   float* lp = loss_bg ? w.loss_partial : nullptr;
   FwdL1 l1 = {target, gC, w.loss_partial + w.n_tiles, (float)(1.0 / (3.0 * (double)cam.W * (double)cam.H))};
+  // heavy tiles of the surfel forward (no depth moments): clusters of kSegRanks CTAs over the first positions of the tile order
+  static const bool seg_on = [] { const char* e = getenv("OCGS_FWD_SEGMENTED"); return !e || atoi(e) != 0; }();
+  const int seg_tiles = (prim == 0 && !mom && seg_on) ? min(w.n_tiles, kSegMaxTiles) : 0;
 #define OCGS_FWD_LAUNCH(S, M, P, L)                                                                                                \
-  render_fwd_kernel<S, M, P, L><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.rank_to_id, \
-                                                     mask, cam.W, cam.H, cam.tiles_x, cfg, color, alpha, depth, normal, n_contrib,   \
-                                                     w.final_T, w.blist, w.header, lp, vis_count, contrib_sum, mom, l1)
+  do {                                                                                                                             \
+    cudaLaunchConfig_t lc = {};                                                                                                    \
+    lc.gridDim = dim3((unsigned)w.n_tiles); lc.blockDim = dim3(256); lc.dynamicSmemBytes = 0; lc.stream = st;                     \
+    cudaLaunchAttribute at[1];                                                                                                     \
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;          \
+    lc.attrs = at; lc.numAttrs = seg_tiles > 0 ? 1 : 0;  /* overlap with the segmented launch in front (see the kernel) */      \
+    OCGS_CUDA_OK(cudaLaunchKernelEx(&lc, render_fwd_kernel<S, M, P, L>, (const uint32_t*)w.tile_order, w.tile_work, (const uint32_t*)w.ranges, \
+                                    (const uint32_t*)w.tile_vals, (const float4*)w.rec, (const uint32_t*)w.rank_to_id, mask, cam.W, cam.H, cam.tiles_x, cfg, \
+                                    color, alpha, depth, normal, n_contrib, w.final_T, w.blist, w.header, lp, vis_count, contrib_sum, mom, l1, seg_tiles)); \
+  } while (0)
+#define OCGS_FWD_LAUNCH_SEG(S, L)                                                                                                  \
+  do {                                                                                                                             \
+    cudaLaunchConfig_t lc = {};                                                                                                    \
+    lc.gridDim = dim3((unsigned)(seg_tiles * kSegRanks)); lc.blockDim = dim3(256); lc.dynamicSmemBytes = 0; lc.stream = st;       \
+    cudaLaunchAttribute at[1];                                                                                                     \
+    at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = kSegRanks; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1; \
+    lc.attrs = at; lc.numAttrs = 1;                                                                                                \
+    if (kSegRanks > 8) OCGS_CUDA_OK(cudaFuncSetAttribute(render_fwd_kernel<S, false, 0, L, true, 1>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1)); \
+    OCGS_CUDA_OK(cudaLaunchKernelEx(&lc, render_fwd_kernel<S, false, 0, L, true, 1>, (const uint32_t*)w.tile_order, w.tile_work, (const uint32_t*)w.ranges, \
+                                    (const uint32_t*)w.tile_vals, (const float4*)w.rec, (const uint32_t*)w.rank_to_id, mask, cam.W, cam.H, cam.tiles_x, cfg, \
+                                    color, alpha, depth, normal, n_contrib, w.final_T, w.blist, w.header, lp, vis_count, contrib_sum, mom, l1, seg_tiles)); \
+    OCGS_LAUNCHED(st, "render_fwd_seg_kernel");                                                                                    \
+  } while (0)
+  if (seg_tiles > 0) {
+    if (target) { if (stats) OCGS_FWD_LAUNCH_SEG(true, true); else OCGS_FWD_LAUNCH_SEG(false, true); }
+    else        { if (stats) OCGS_FWD_LAUNCH_SEG(true, false); else OCGS_FWD_LAUNCH_SEG(false, false); }
+  }
+#undef OCGS_FWD_LAUNCH_SEG
   if (prim == 1) {  // 3D Gaussians: forward + statistics only (no moment maps)
     if (mom || target) return OCGS_ERR_UNSUPPORTED;
     if (stats) OCGS_FWD_LAUNCH(true, false, 1, false); else OCGS_FWD_LAUNCH(false, false, 1, false);
