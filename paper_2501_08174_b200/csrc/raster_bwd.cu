@@ -4,6 +4,9 @@
 //      gives 16 + 4 record gradients, reduced across the warp by a transposing butterfly (16 values, 8+4+2+1+1 shuffles),
 //      stored per warp in shared memory, combined across the CTA and flushed with one global RED per (tile, entry, field).
 //  (b) project_bwd_kernel: one thread per surfel, record gradients -> (pos, scale, quat, opacity, sh) gradients.
+#include <cooperative_groups.h>
+#include <stdlib.h>
+
 #include "projection.cuh"
 
 namespace ocgs {
@@ -152,14 +155,29 @@ constexpr uint32_t kBwdHeavyLen = 2048;
 #define OCGS_BWD_LEAN_BLOCKS 6
 #endif
 constexpr int kBwdLeanMinBlocks = OCGS_BWD_LEAN_BLOCKS;  // the colour / alpha-only instance (72 registers: 7 resident blocks)
-template <bool kMoments, bool kGeo>
+// Segmented walk of heavy tiles (kSegB; the backward half of DESIGN.md "heavy tiles").  A tile whose BLENDED list is longer
+// than kBwdSegLen is walked by a cluster of 8 CTAs = kBwdSegParts parts of the list x the two pixel halves of the split walk.
+// The back-to-front chain needs, at the back of part r, the transmittance there and the running dot product g.S of everything
+// behind it.  Both follow from one cheap pre-pass over the part (no gradient terms, no reduction): with the part's own
+//   P_r = prod (1 - alpha_i),   G'_r = sum_i alpha_i T'_i (g.q_i),  T'_i = the product inside the part in front of pair i
+// (Horner from the back: G' <- alpha (g.q) + (1 - alpha) G'), the true values are linear in the transmittance in front of the
+// part, T_front,r = prod_{r' < r} P_r':   g.S at the back of part r = g.S_tail + sum_{r' > r} T_front,r' G'_r', T there = T_front,r+1.
+// P and G' travel through distributed shared memory; then every CTA runs the ordinary walk of its part.
+constexpr int kBwdSegParts = 4;
+constexpr uint32_t kBwdSegLen = 4096;
+constexpr int kBwdSegMaxTiles = 128;
+namespace cg = cooperative_groups;
+
+template <bool kMoments, bool kGeo, bool kSegB = false>
 __global__ void __launch_bounds__(128, kGeo ? kBwdMinBlocks : kBwdLeanMinBlocks) render_bwd_kernel(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ tile_work,
                                                             const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ list,
                                                             const float4* __restrict__ rec, const uint2* __restrict__ blist, const uint8_t* __restrict__ mask,
                                                             const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
                                                             const float* __restrict__ gC, const float* __restrict__ gA,
                                                             const float* __restrict__ gD, const float* __restrict__ gN, const float* __restrict__ mom, const float* __restrict__ gM1, const float* __restrict__ gM2, int W, int H,
-                                                            int tiles_x, int n_tiles, ocgs_config cfg, float gamma_over_hw, float* __restrict__ grad_rec) {
+                                                            int tiles_x, int n_tiles, ocgs_config cfg, float gamma_over_hw, float* __restrict__ grad_rec,
+                                                            int seg_tiles /*leading positions of the tile order the segmented launch takes (0: none)*/) {
+  __shared__ float s_seg[kSegB ? 2 : 1][kSegB ? 128 : 1];  // kSegB: P_r and G'_r of this CTA's pixels, read by its cluster
   __shared__ float4 s_rec[kBwdBatch * 6];
   __shared__ uint32_t s_rank[kBwdBatch];
   __shared__ uint8_t s_mask[kBwdBatch];
@@ -168,12 +186,21 @@ __global__ void __launch_bounds__(128, kGeo ? kBwdMinBlocks : kBwdLeanMinBlocks)
   static_assert(kBwdBatch == 64, "the per-warp entry masks below cover two 32-entry halves");
   // launch order: heavy tiles first (tile_order); the first `n_split` positions own two consecutive blocks each, so that a
   // tile with a long blended list can be walked by two CTAs (see kBwdHeavyLen)
+  // programmatic dependent launch, as in the forward pass: the ordinary launch overlaps the clusters and its last CTA joins them
+  if (kSegB) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  struct PdlJoin {
+    bool on;
+    __device__ ~PdlJoin() { if (on) asm volatile("griddepcontrol.wait;" ::: "memory"); }
+  } pdl_join{!kSegB && seg_tiles > 0 && blockIdx.x == gridDim.x - 1};
   const int n_split = min(n_tiles, kBwdSplitMax);
-  const int pos = (int)blockIdx.x < 2 * n_split ? (int)(blockIdx.x >> 1) : (int)blockIdx.x - n_split;
-  const int part = (int)blockIdx.x < 2 * n_split ? (int)(blockIdx.x & 1u) : 0;
+  const int crank = kSegB ? (int)cg::this_cluster().block_rank() : 0;  // kSegB: cluster rank = 2 * list part + pixel half
+  const int pos = kSegB ? (int)blockIdx.x / (2 * kBwdSegParts) : ((int)blockIdx.x < 2 * n_split ? (int)(blockIdx.x >> 1) : (int)blockIdx.x - n_split);
+  const int part = kSegB ? (crank & 1) : ((int)blockIdx.x < 2 * n_split ? (int)(blockIdx.x & 1u) : 0);
+  const int lpart = crank >> 1;
   const int tile = (int)tile_order[pos];
   const uint32_t mx = tile_work[tile];           // length of the tile's blended list (written by the forward pass)
-  const bool split = pos < n_split && mx > kBwdHeavyLen;
+  const bool split = kSegB || (pos < n_split && mx > kBwdHeavyLen);
+  if (kSegB ? mx <= kBwdSegLen : (pos < seg_tiles && mx > kBwdSegLen)) return;  // (uniform over the CTA / cluster)
   if (mx == 0 || (part && !split)) return;
   const int tx = tile % tiles_x, ty = tile / tiles_x;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -214,7 +241,12 @@ __global__ void __launch_bounds__(128, kGeo ? kBwdMinBlocks : kBwdLeanMinBlocks)
     s.GS = Tfin * (fmaf(s.gc0, cfg.bg[0], fmaf(s.gc1, cfg.bg[1], s.gc2 * cfg.bg[2])) - ga);
   }
   const int nbatch = (int)((mx + kBwdBatch - 1) / kBwdBatch);
-  for (int bi = nbatch - 1; bi >= 0; --bi) {
+  // kSegB: this CTA's part of the list, in whole batches
+  const int per = kSegB ? (nbatch + kBwdSegParts - 1) / kBwdSegParts : nbatch;
+  const int b_lo = kSegB ? min(nbatch, lpart * per) : 0, b_hi = kSegB ? min(nbatch, b_lo + per) : nbatch;
+  uint32_t lo0 = 0, lo1 = 0, hi0 = 0, hi1 = 0;
+  // stage batch bi: its entries of the blended list, their records, and the warp's hit masks (two barriers inside, one in front)
+  auto stage = [&](int bi) -> int {
     const uint32_t b0 = (uint32_t)bi * kBwdBatch;
     const int cnt = (int)min((uint32_t)kBwdBatch, mx - b0);
     __syncthreads();  // previous batch fully flushed before s_rank / s_mask / s_acc are reused
@@ -232,9 +264,70 @@ __global__ void __launch_bounds__(128, kGeo ? kBwdMinBlocks : kBwdLeanMinBlocks)
     }
     // per warp: which entries of the batch did its two pixel blocks blend (bit e of lo: entry e, of hi: entry 32 + e)
     const uint32_t mlo = lane < cnt ? s_mask[lane] : 0u, mhi = lane + 32 < cnt ? s_mask[lane + 32] : 0u;
-    const uint32_t lo0 = __ballot_sync(0xFFFFFFFFu, mlo & bit0), lo1 = __ballot_sync(0xFFFFFFFFu, mlo & bit1);
-    const uint32_t hi0 = __ballot_sync(0xFFFFFFFFu, mhi & bit0), hi1 = __ballot_sync(0xFFFFFFFFu, mhi & bit1);
+    lo0 = __ballot_sync(0xFFFFFFFFu, mlo & bit0); lo1 = __ballot_sync(0xFFFFFFFFu, mlo & bit1);
+    hi0 = __ballot_sync(0xFFFFFFFFu, mhi & bit0); hi1 = __ballot_sync(0xFFFFFFFFu, mhi & bit1);
     __syncthreads();
+    return cnt;
+  };
+  if (kSegB) {
+    // ---- pre-pass over this CTA's part (one pixel per thread: the split walk), back to front ----
+    BwdPixel& s = ps[0];
+    float P = 1.0f, Gp = 0.0f;
+    for (int bi = b_hi - 1; bi >= b_lo; --bi) {
+      stage(bi);
+#pragma unroll 1
+      for (int half = 1; half >= 0; --half) {
+        uint32_t todo = half ? hi0 : lo0;
+        while (todo) {
+          const int jb = 31 - __clz(todo);
+          todo &= ~(1u << jb);
+          const int j = 32 * half + jb;
+          const float4* sr = s_rec + 6 * j;
+          const float4 r0 = sr[0], r1 = sr[1], r2 = sr[2], r3 = sr[3];
+          const float dx = s.px - r2.z, dy = s.py - r2.w;
+          const float qx = fmaf(-dy, r0.w, fmaf(-dx, r0.x, r1.z));
+          const float qy = fmaf(-dy, r1.x, fmaf(-dx, r0.y, r1.w));
+          const float qz = fmaf(-dy, r1.y, fmaf(-dx, r0.z, r2.x));
+          const float inv = rcp_approx(qz);
+          const float u = qx * inv, vv = qy * inv;
+          const float rho3 = fmaf(u, u, vv * vv);
+          const float rho2 = fmaf(dx, dx, dy * dy) * kc.inv_sigma2;
+          const bool surf = rho3 <= rho2;
+          const float rho = surf ? rho3 : rho2;
+          const float z = surf ? r2.y * inv : r3.y;
+          if (s_idx[j] < s.last && qz != 0.0f && !(z < kc.near_z) && !(rho > r3.x)) {
+            const float4 r4 = sr[4], r5 = kGeo ? sr[5] : make_float4(0.f, 0.f, 0.f, 0.f);
+            const float a = fminf(kc.alpha_max, r4.x * ex2_approx(rho * kNegHalfLog2e));
+            float gq = kGeo ? s.gd * z : 0.f;
+            const float dz = z - s.zc;
+            if (kMoments) gq = fmaf(s.gm2 * dz, dz, fmaf(s.gm1, dz, gq));
+            gq = fmaf(s.gc0, r4.y, gq); gq = fmaf(s.gc1, r4.z, gq); gq = fmaf(s.gc2, r4.w, gq);
+            if (kGeo) { gq = fmaf(s.gn0, r5.x, gq); gq = fmaf(s.gn1, r5.y, gq); gq = fmaf(s.gn2, r5.z, gq); }
+            Gp = fmaf(1.0f - a, Gp, a * gq);
+            P *= 1.0f - a;
+          }
+        }
+      }
+    }
+    __syncthreads();
+    s_seg[0][threadIdx.x] = P; s_seg[1][threadIdx.x] = Gp;
+    cg::cluster_group cl = cg::this_cluster();
+    cl.sync();
+    // T_front of every part, then this part's state at its back: T = T_front of the next part (the forward pass's exact T_final for
+    // the last one), g.S = the tail term + the parts behind
+    float Tf = 1.0f, Tback = s.T, GS = s.GS;
+    for (int r = 0; r < kBwdSegParts; ++r) {
+      const float* rp = cl.map_shared_rank(&s_seg[0][0], (unsigned)(2 * r + part));
+      const float Pr = rp[threadIdx.x], Gr = rp[128 + threadIdx.x];
+      if (r > lpart) GS = fmaf(Tf, Gr, GS);
+      Tf *= Pr;
+      if (r == lpart && lpart < kBwdSegParts - 1) Tback = Tf;
+    }
+    s.T = Tback; s.GS = GS;
+    cl.sync();  // nobody leaves (or restages) while its shared memory may still be read
+  }
+  for (int bi = b_hi - 1; bi >= b_lo; --bi) {
+    const int cnt = stage(bi);
 #pragma unroll 1
     for (int half = 1; half >= 0; --half) {
       const uint32_t m0 = half ? hi0 : lo0, m1 = half ? hi1 : lo1;
@@ -473,15 +566,31 @@ int launch_render_bwd(const ocgs_surfels& s, const CamParams& cam, const ocgs_co
     int rc = launch_order_tiles(w, /*from_ranges=*/false, st, /*clear_grad_rec=*/true);
     if (rc != OCGS_OK) return rc;
     const float goh = mask ? (float)((double)cfg.gamma_bg / ((double)cam.W * (double)cam.H)) : 0.f;
-    if (mom && gM1 && gM2)
-      render_bwd_kernel<true, true><<<w.n_tiles + min(w.n_tiles, kBwdSplitMax), 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, mom, gM1, gM2,
-                                                         cam.W, cam.H, cam.tiles_x, w.n_tiles, cfg, goh, w.grad_rec);
-    else if (gD || gN)
-      render_bwd_kernel<false, true><<<w.n_tiles + min(w.n_tiles, kBwdSplitMax), 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, gD, gN, nullptr, nullptr, nullptr,
-                                                                cam.W, cam.H, cam.tiles_x, w.n_tiles, cfg, goh, w.grad_rec);
-    else  // colour / alpha gradients only (masked L1 + L_b): the depth and normal terms are identically zero
-      render_bwd_kernel<false, false><<<w.n_tiles + min(w.n_tiles, kBwdSplitMax), 128, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec, w.blist, mask, final_T, n_contrib, gC, gA, nullptr, nullptr, nullptr, nullptr, nullptr,
-                                                                 cam.W, cam.H, cam.tiles_x, w.n_tiles, cfg, goh, w.grad_rec);
+    static const bool seg_on = [] { const char* e = getenv("OCGS_BWD_SEGMENTED"); return !e || atoi(e) != 0; }();
+    const int seg_tiles = seg_on ? min(w.n_tiles, kBwdSegMaxTiles) : 0;
+    const float* momp = (mom && gM1 && gM2) ? mom : nullptr;
+    const bool geo = momp || gD || gN;  // colour / alpha gradients only (masked L1 + L_b): the depth and normal terms are identically zero
+#define OCGS_BWD_LAUNCH(M, G, SEG)                                                                                                 \
+  do {                                                                                                                             \
+    cudaLaunchConfig_t lc = {};                                                                                                    \
+    lc.gridDim = dim3(SEG ? (unsigned)(seg_tiles * 2 * kBwdSegParts) : (unsigned)(w.n_tiles + min(w.n_tiles, kBwdSplitMax)));      \
+    lc.blockDim = dim3(128); lc.dynamicSmemBytes = 0; lc.stream = st;                                                              \
+    cudaLaunchAttribute at[1];                                                                                                     \
+    if (SEG) { at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = 2 * kBwdSegParts; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1; } \
+    else { at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1; }  \
+    lc.attrs = at; lc.numAttrs = (SEG || seg_tiles > 0) ? 1 : 0;                                                                   \
+    OCGS_CUDA_OK(cudaLaunchKernelEx(&lc, render_bwd_kernel<M, G, SEG>, (const uint32_t*)w.tile_order, (const uint32_t*)w.tile_work, (const uint32_t*)w.ranges, \
+                                    (const uint32_t*)w.tile_vals, (const float4*)w.rec, (const uint2*)w.blist, mask, final_T, n_contrib, gC, gA, \
+                                    geo ? gD : (const float*)nullptr, geo ? gN : (const float*)nullptr, momp, momp ? gM1 : (const float*)nullptr, \
+                                    momp ? gM2 : (const float*)nullptr, cam.W, cam.H, cam.tiles_x, w.n_tiles, cfg, goh, w.grad_rec, seg_tiles)); \
+  } while (0)
+    for (int seg = seg_tiles > 0 ? 1 : 0; seg >= 0; --seg) {  // the clusters first, then the ordinary launch
+      if (momp) { if (seg) OCGS_BWD_LAUNCH(true, true, true); else OCGS_BWD_LAUNCH(true, true, false); }
+      else if (geo) { if (seg) OCGS_BWD_LAUNCH(false, true, true); else OCGS_BWD_LAUNCH(false, true, false); }
+      else { if (seg) OCGS_BWD_LAUNCH(false, false, true); else OCGS_BWD_LAUNCH(false, false, false); }
+      if (seg) OCGS_LAUNCHED(st, "render_bwd_seg_kernel");
+    }
+#undef OCGS_BWD_LAUNCH
     OCGS_LAUNCHED(st, "render_bwd_kernel");
   }
   project_bwd_kernel<<<(unsigned)div_up((size_t)s.n, 128), 128, 0, st>>>(s.pos, (const float2*)s.scale, (const float4*)s.quat, s.opacity,
