@@ -464,7 +464,7 @@ __global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) ren
   }
   if (loss_partial) {  // Eq. 1: A (1 - M), fixed-order reduction -> deterministic
     float lb = 0.f;
-    if (inside) lb = (mask == nullptr || mask[(size_t)iy * W + ix] == 0) ? A : 0.f;
+    if (inside) lb = (mask != nullptr && mask[(size_t)iy * W + ix] == 0) ? A : 0.f;  // mask == NULL: M = 1 everywhere, L_b = 0 (ocgs.h)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) lb += __shfl_xor_sync(0xFFFFFFFFu, lb, o);
     __syncthreads();
