@@ -282,6 +282,19 @@ int ocgs_densify(const ocgs_surfels* in, const float* grad_accum, const uint32_t
 int ocgs_masked_l1(const float* color, const float* target, const uint8_t* mask, int width, int height, float* dL_dcolor,
                    float* loss, void* ws, int n, size_t key_capacity, void* stream);
 
+/* The same term for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): no workspace argument -- the per-block partial sums live in a 32 KB static device array inside the library (held by
+ * every GPU that loads it until the process exits), and the call itself calls no cudaMalloc / cudaFree / allocating routine.
+ * Arguments as ocgs_masked_l1 (color, target, dL_dcolor device f32 [3,H,W]; mask device u8 [H,W], nullable = all ones; loss device
+ * f32 scalar, nullable); results bit-identical to ocgs_masked_l1's.  Limit: width * height <= OCGS_MASKED_L1_STATIC_MAX_PIXELS
+ * (2 097 152, e.g. 1920x1080), beyond it OCGS_ERR_CAPACITY and nothing is launched.  The first call on a device looks the array's
+ * address up (cudaGetSymbolAddress): make it before a capture starts.  All calls share the array: nothing in it has to start at
+ * zero (a call writes every slot it reads), but calls that OVERLAP on the GPU -- different streams, parallel graph branches -- race
+ * on it: serialise them.  Asynchronous on `stream`. */
+#define OCGS_MASKED_L1_STATIC_MAX_PIXELS 2097152
+int ocgs_masked_l1_static(const float* color, const float* target, const uint8_t* mask, int width, int height, float* dL_dcolor,
+                          float* loss, void* stream);
+
 /* ---- masked photometric loss L_c^M (Eq. 2) ---------------------------------------
  * L_c^M = L_c(I M, R M) with L_c = (1 - lambda) mean|x - y| + lambda (1 - mean SSIM(x, y)): the loss the paper takes from
  * "Equation 7 in the 3DGS paper" (reading S20b of DESIGN.md: SSIM of Wang et al. 2004 per channel over an

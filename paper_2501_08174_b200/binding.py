@@ -19,7 +19,7 @@ OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPP
 EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
            "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_render_fwd_l1", "ocgs_render_fwd_reg", "ocgs_render_bwd_reg", "ocgs3d_preprocess", "ocgs3d_render_fwd", "ocgs_prune_workspace_bytes",
            "ocgs_prune_stats", "ocgs_compact_rows", "ocgs_densify_workspace_bytes", "ocgs_densify_accumulate", "ocgs_densify", "ocgs_step_host", "ocgs_step_view_host", "ocgs_step_view_host_enqueue", "ocgs_step_view_prefetch_enqueue", "ocgs_visibility_pass", "ocgs3d_visibility_pass", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
-           "ocgs_profile_begin", "ocgs_profile_end", "ocgs_peak_probe"]
+           "ocgs_profile_begin", "ocgs_profile_end", "ocgs_peak_probe", "ocgs_masked_l1_static"]
 
 
 class OcgsError(RuntimeError):
@@ -331,6 +331,19 @@ def ocgs_step_host(h_pos, h_scale, h_quat, h_opacity, h_sh, n, cam, cfg, h_mask,
 def ocgs_masked_l1(color, target, mask, width, height, dL_dcolor, loss, ws, n, key_capacity, stream=None):
     _ok("ocgs_masked_l1", lib().ocgs_masked_l1(_ptr(color), _ptr(target), _ptr(mask), C.c_int(width), C.c_int(height), _ptr(dL_dcolor),
                                                _ptr(loss), _ptr(ws), C.c_int(n), C.c_size_t(key_capacity), _stream(stream)))
+
+
+OCGS_MASKED_L1_STATIC_MAX_PIXELS = 2097152
+
+
+def ocgs_masked_l1_static(color, target, mask, width, height, dL_dcolor, loss, stream=None):
+    """ocgs_masked_l1 without a workspace: scratch in a static device array of the library, no allocation in the call."""
+    code = lib().ocgs_masked_l1_static(_ptr(color), _ptr(target), _ptr(mask), C.c_int(width), C.c_int(height), _ptr(dL_dcolor), _ptr(loss),
+                                       _stream(stream))
+    if code == OCGS_ERR_CAPACITY:
+        raise OcgsError(f"ocgs_masked_l1_static ({width}x{height} = {width * height} pixels exceed the static scratch: at most "
+                        f"{OCGS_MASKED_L1_STATIC_MAX_PIXELS}; use ocgs_masked_l1 with a workspace)", code)
+    _ok("ocgs_masked_l1_static", code)
 
 
 def ocgs_regularizers_workspace_bytes(width: int, height: int) -> int:

@@ -60,3 +60,47 @@ int launch_masked_l1(const float* color, const float* target, const uint8_t* mas
 }
 
 }  // namespace ocgs
+
+// ---- ocgs_masked_l1_static: the same term for callers that may not allocate -------------------------------------------------
+// (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  The per-block partial sums, the only
+// scratch of this term, live in a file-scope device array instead of the caller's workspace: kStaticL1Partials floats = 32 KB,
+// held by every GPU that loads the library until the process exits.  One block per 256 pixels, so the limit is
+// OCGS_MASKED_L1_STATIC_MAX_PIXELS = 8192 * 256 = 2 097 152 pixels (every BASELINE.json config fits: 1920x1080 = 2 073 600),
+// and the launch geometry -- hence the loss, bit for bit -- is that of ocgs_masked_l1.
+// In HOST code the array's name is a host-side stand-in, not a device address: the kernels get the address that
+// cudaGetSymbolAddress returns, looked up once per device with that device current.  All calls share the array: every slot a
+// call reads it has written first (nothing has to start at zero, stale contents of the last call are never read), but two calls
+// that overlap on the GPU (different streams, or concurrent graph branches) race on it.
+namespace ocgs {
+constexpr int kStaticL1Partials = 8192;
+static __device__ __align__(256) float g_static_l1_partial[kStaticL1Partials];
+static_assert((size_t)kStaticL1Partials * 256 == OCGS_MASKED_L1_STATIC_MAX_PIXELS, "limit stated in ocgs.h");
+}  // namespace ocgs
+
+#include <mutex>
+
+extern "C" int ocgs_masked_l1_static(const float* color, const float* target, const uint8_t* mask, int width, int height, float* dL_dcolor,
+                                     float* loss, void* stream) {
+  using namespace ocgs;
+  if (!color || !target || !dL_dcolor || width <= 0 || height <= 0) return OCGS_ERR_INVALID_ARG;
+  if ((size_t)width * (size_t)height > (size_t)OCGS_MASKED_L1_STATIC_MAX_PIXELS) return OCGS_ERR_CAPACITY;  // beyond the static scratch
+  // set-up, once per device: the device address of the scratch array on the CURRENT device
+  constexpr int kMaxDevices = 64;
+  static float* s_ptr[kMaxDevices] = {};
+  static std::mutex s_mu;
+  int dev = 0;
+  OCGS_CUDA_OK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return OCGS_ERR_UNSUPPORTED;
+  float* partial = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(s_mu);
+    if (!s_ptr[dev]) {
+      void* p = nullptr;
+      OCGS_CUDA_OK(cudaGetSymbolAddress(&p, g_static_l1_partial));
+      if (!p) return OCGS_ERR_CUDA;
+      s_ptr[dev] = (float*)p;
+    }
+    partial = s_ptr[dev];
+  }
+  return launch_masked_l1(color, target, mask, width, height, dL_dcolor, loss, partial, kStaticL1Partials, (cudaStream_t)stream);
+}
