@@ -319,10 +319,13 @@ int ocgs_profile_end(void* stream, int max_out, float* ms_out, char* names_out, 
 /* ---- diagnostics: measured ALU peaks of the device ("the builder must measure an FP32-FMA peak and a
  * MUFU.EX2 peak microbenchmark on the box and use those" for the rooflines of the raster kernels, PAPER.md:119 renderer) ----
  * Enqueues ONE launch of a microbenchmark on `stream`: kind 0 = eight independent chains of a <- fma(a, b, c) per thread
- * (2 flop per step), kind 1 = eight chains of a <- -ex2(a) (one MUFU.EX2 per step); 8 blocks of 256 threads per SM,
- * `iters` x 8 steps per chain.  *ops_per_launch (host) receives the flop (kind 0) or EX2 (kind 1) count of the launch; the
- * caller times the launch with CUDA events and divides.  d_out: device f32[out_floats], out_floats >= 8 x 256 x number of
- * SMs (OCGS_ERR_CAPACITY otherwise), scratch the kernels store their results to.  Asynchronous; not part of any step. */
+ * (2 flop per step; b, c uniform operands), kind 1 = eight chains of a <- -ex2(a) (one MUFU.EX2 per step), kind 2 = kind 0 with
+ * b, c in registers (the three-register FFMA real kernels issue), kind 3 = packed fma.rn.f32x2 chains (FFMA2, 4 flop per step,
+ * register operands); 8 blocks of 256 threads per SM, `iters` x 8 steps per chain.  *ops_per_launch (host) receives the flop
+ * (kinds 0, 2, 3) or EX2 (kind 1) count of the launch; the caller times the launch with CUDA events and divides.
+ * d_out: device f32[out_floats], out_floats >= 8 x 256 x number of SMs (+ 16 for kinds 2, 3; OCGS_ERR_CAPACITY otherwise),
+ * scratch the kernels store their results to.  Kinds 0, 1 are asynchronous; kinds 2, 3 upload their 16 operands and synchronise
+ * `stream` once before the launch.  Not part of any step. */
 int ocgs_peak_probe(int kind, int iters, float* d_out, size_t out_floats, double* ops_per_launch, void* stream);
 
 /* ---- end-to-end TRAINING step: per-view inputs from the host, parameters resident on the device (bench.py "e2e") -------

@@ -44,11 +44,57 @@ __global__ void __launch_bounds__(256) ex2_peak_kernel(float* __restrict__ out, 
   out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+// kind 2: the same chains with b and c in REGISTERS (loaded from memory, so that they cannot become constant-bank operands):
+// the three-register form real kernels issue
+__global__ void __launch_bounds__(256) fma3_peak_kernel(float* __restrict__ out, int iters, const float* __restrict__ bc) {
+  float a[kPeakChains], b[kPeakChains], c[kPeakChains];
+#pragma unroll
+  for (int k = 0; k < kPeakChains; ++k) { a[k] = (float)(threadIdx.x + k) * 1e-3f; b[k] = bc[k]; c[k] = bc[kPeakChains + k]; }
+#pragma unroll 1
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+      for (int k = 0; k < kPeakChains; ++k) a[k] = fmaf(a[k], b[k], c[k]);
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int k = 0; k < kPeakChains; ++k) s += a[k];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+// kind 3: packed fp32 (fma.rn.f32x2, sm_100): kPeakChains chains of TWO fused multiply-adds per instruction, operands in registers
+__global__ void __launch_bounds__(256) fma2_peak_kernel(float* __restrict__ out, int iters, const float* __restrict__ bc) {
+  unsigned long long a[kPeakChains], b[kPeakChains], c[kPeakChains];
+#pragma unroll
+  for (int k = 0; k < kPeakChains; ++k) {
+    const float a0 = (float)(threadIdx.x + k) * 1e-3f, a1 = a0 + 0.5f;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(a[k]) : "f"(a0), "f"(a1));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b[k]) : "f"(bc[k]), "f"(bc[k]));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(c[k]) : "f"(bc[kPeakChains + k]), "f"(bc[kPeakChains + k]));
+  }
+#pragma unroll 1
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+      for (int k = 0; k < kPeakChains; ++k) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(a[k]) : "l"(b[k]), "l"(c[k]));
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int k = 0; k < kPeakChains; ++k) {
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a[k]));
+    s += lo + hi;
+  }
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace ocgs
 
 extern "C" int ocgs_peak_probe(int kind, int iters, float* d_out, size_t out_floats, double* ops_per_launch, void* stream) {
   using namespace ocgs;
-  if (!d_out || !ops_per_launch || iters <= 0 || (kind != 0 && kind != 1)) return OCGS_ERR_INVALID_ARG;
+  if (!d_out || !ops_per_launch || iters <= 0 || kind < 0 || kind > 3) return OCGS_ERR_INVALID_ARG;
   int dev = 0, sms = 0;
   OCGS_CUDA_OK(cudaGetDevice(&dev));
   OCGS_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -56,7 +102,17 @@ extern "C" int ocgs_peak_probe(int kind, int iters, float* d_out, size_t out_flo
   if (out_floats < (size_t)blocks * 256) return OCGS_ERR_CAPACITY;
   const double steps = (double)blocks * 256.0 * (double)iters * 8.0 * (double)kPeakChains;
   cudaStream_t st = (cudaStream_t)stream;
-  if (kind == 0) {
+  if (kind == 2 || kind == 3) {
+    // b, c of the register-operand forms are 16 floats BEHIND the kernels' result slots (d_out[blocks * 256 ...]), uploaded here
+    float h[2 * kPeakChains];
+    for (int k = 0; k < kPeakChains; ++k) { h[k] = 0.999f; h[kPeakChains + k] = 1e-3f; }
+    if (out_floats < (size_t)blocks * 256 + 2 * kPeakChains) return OCGS_ERR_CAPACITY;
+    float* bc = d_out + (size_t)blocks * 256;
+    OCGS_CUDA_OK(cudaMemcpyAsync(bc, h, sizeof(h), cudaMemcpyHostToDevice, st));
+    OCGS_CUDA_OK(cudaStreamSynchronize(st));  // (h is a stack buffer; diagnostic call, not part of any step)
+    if (kind == 2) { fma3_peak_kernel<<<blocks, 256, 0, st>>>(d_out, iters, bc); *ops_per_launch = 2.0 * steps; }
+    else { fma2_peak_kernel<<<blocks, 256, 0, st>>>(d_out, iters, bc); *ops_per_launch = 4.0 * steps; }
+  } else if (kind == 0) {
     fma_peak_kernel<<<blocks, 256, 0, st>>>(d_out, iters, 0.999f, 1e-3f);
     *ops_per_launch = 2.0 * steps;  // flop
   } else {
