@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) ren
                                                          uint32_t* __restrict__ n_contrib, float* __restrict__ final_T, uint2* __restrict__ blist, ocgs_header* __restrict__ header, float* __restrict__ loss_partial,
                                                          uint32_t* __restrict__ vis_count, float* __restrict__ contrib_sum, float* __restrict__ mom /*[3,H,W]: origin, m1, m2 (kMoments)*/, FwdL1 l1,
                                                          int seg_tiles /*leading positions of the tile order the segmented launch takes (0: none)*/) {
-  static_assert(!kSeg || (kMaps && !kMoments && kPrim == 0), "segmented compositing: surfel forward with maps, no depth moments");
+  static_assert(!kSeg || (!kMoments && kPrim == 0), "segmented compositing: surfel forward (with maps or statistics only), no depth moments");
   __shared__ float4 s_rec[kFwdBatch * 6];
   __shared__ uint32_t s_rank[kFwdBatch];
   __shared__ uint32_t s_hit[kFwdBatch];  // bit w: warp w blended the entry (read by the backward pass)
@@ -403,7 +403,12 @@ __global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) ren
     }
   }
 
-  if (!kMaps) return;
+  if (!kMaps) {
+    // statistics only: nothing to combine (every CTA has flushed its own counts); a cluster CTA stays until its cluster has read
+    // its P_r through distributed shared memory
+    if (kSeg) cg::this_cluster().sync();
+    return;
+  }
   if (kSeg) {
     cg::cluster_group cl = cg::this_cluster();
     const int t = (int)threadIdx.x;
@@ -522,14 +527,37 @@ int launch_render_stats(const CamParams& cam, const ocgs_config& cfg, const Work
   int rc = launch_order_tiles(w, /*from_ranges=*/true, st);
   if (rc != OCGS_OK) return rc;
   FwdL1 l1 = {nullptr, nullptr, nullptr, 0.f};
+  // heavy tiles (surfels): the same clusters as the full forward pass, transmittance exchange only; the ordinary launch overlaps them
+  static const bool seg_on = [] { const char* e = getenv("OCGS_FWD_SEGMENTED"); return !e || atoi(e) != 0; }();
+  const int seg_tiles = (prim == 0 && seg_on) ? min(w.n_tiles, kSegMaxTiles) : 0;
+  if (seg_tiles > 0) {
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3((unsigned)(seg_tiles * kSegRanks)); lc.blockDim = dim3(256); lc.dynamicSmemBytes = 0; lc.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = kSegRanks; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    lc.attrs = at; lc.numAttrs = 1;
+    if (kSegRanks > 8) OCGS_CUDA_OK(cudaFuncSetAttribute(render_fwd_kernel<true, false, 0, false, false, 1>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    OCGS_CUDA_OK(cudaLaunchKernelEx(&lc, render_fwd_kernel<true, false, 0, false, false, 1>, (const uint32_t*)w.tile_order, w.tile_work, (const uint32_t*)w.ranges,
+                                    (const uint32_t*)w.tile_vals, (const float4*)w.rec, (const uint32_t*)w.rank_to_id, (const uint8_t*)nullptr, cam.W, cam.H, cam.tiles_x, cfg,
+                                    (float*)nullptr, (float*)nullptr, (float*)nullptr, (float*)nullptr, (uint32_t*)nullptr, (float*)nullptr, (uint2*)nullptr, w.header,
+                                    (float*)nullptr, vis_count, contrib_sum, (float*)nullptr, l1, seg_tiles));
+    OCGS_LAUNCHED(st, "render_stats_seg_kernel");
+  }
   if (prim == 1)
     render_fwd_kernel<true, false, 1, false, false><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec,
         w.rank_to_id, nullptr, cam.W, cam.H, cam.tiles_x, cfg, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, w.header, nullptr,
         vis_count, contrib_sum, nullptr, l1, 0);
-  else
-    render_fwd_kernel<true, false, 0, false, false><<<w.n_tiles, 256, 0, st>>>(w.tile_order, w.tile_work, w.ranges, w.tile_vals, (const float4*)w.rec,
-        w.rank_to_id, nullptr, cam.W, cam.H, cam.tiles_x, cfg, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, w.header, nullptr,
-        vis_count, contrib_sum, nullptr, l1, 0);
+  else {
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3((unsigned)w.n_tiles); lc.blockDim = dim3(256); lc.dynamicSmemBytes = 0; lc.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
+    lc.attrs = at; lc.numAttrs = seg_tiles > 0 ? 1 : 0;
+    OCGS_CUDA_OK(cudaLaunchKernelEx(&lc, render_fwd_kernel<true, false, 0, false, false>, (const uint32_t*)w.tile_order, w.tile_work, (const uint32_t*)w.ranges,
+                                    (const uint32_t*)w.tile_vals, (const float4*)w.rec, (const uint32_t*)w.rank_to_id, (const uint8_t*)nullptr, cam.W, cam.H, cam.tiles_x, cfg,
+                                    (float*)nullptr, (float*)nullptr, (float*)nullptr, (float*)nullptr, (uint32_t*)nullptr, (float*)nullptr, (uint2*)nullptr, w.header,
+                                    (float*)nullptr, vis_count, contrib_sum, (float*)nullptr, l1, seg_tiles));
+  }
   OCGS_LAUNCHED(st, "render_stats_kernel");
   return OCGS_OK;
 }

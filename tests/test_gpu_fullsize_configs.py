@@ -94,6 +94,17 @@ def test_config5_heaviest_view_forward_and_colour_backward():
     r = full_parity(sc, 7, dict(sh_degree=3), key_capacity=16 * sc.n, max_fragile=2.4e-3, label="config5-heaviest")  # measured 7.7e-4
     L = r["ranges"][:, 1] - r["ranges"][:, 0]
     assert L.max() > 20_000
+    # the statistics-only pass takes the same clusters: identical counts
+    import torch
+    from paper_2501_08174_b200 import binding as B
+    g = GpuView(arrays(sc), sc.cameras[7], dict(sh_degree=3), key_capacity=16 * sc.n)
+    g.preprocess(); g.bin_sort(want_ids=False)
+    gf = g.render_fwd(mask=None, want_loss=False)
+    vis_s = torch.zeros(g.n, dtype=torch.int32, device="cuda"); cs_s = torch.zeros(g.n, device="cuda")
+    B.ocgs_visibility_pass(g.surfels, g.cam, g.cfg, g.ws, g.cap, vis_s, cs_s)
+    torch.cuda.synchronize()
+    assert np.array_equal(vis_s.cpu().numpy().view(np.uint32), gf["vis_count"])
+    assert np.allclose(cs_s.cpu().numpy(), gf["contrib_sum"], rtol=1e-5, atol=1e-7)
 
 
 def test_config4_full_size_all_views_prune():

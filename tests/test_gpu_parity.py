@@ -273,6 +273,29 @@ def test_split_heavy_tile_backward_both_instances():
         assert np.all(gg[k][never] == 0.0), k
 
 
+def test_segmented_heavy_tile_clusters_forward_backward_and_visibility_pass():
+    """ONE 16x16 tile under 9 000 near-transparent surfels: its list is longer than kSegLen = 6144 (raster_fwd.cu) and its blended
+    list longer than kBwdSegLen = 4096 (raster_bwd.cu), so the forward pass, the backward pass AND the statistics-only visibility
+    pass all take the thread-block clusters (exact segmented compositing).  Everything against the oracle
+    (full_parity), then the visibility pass against the forward pass: same pairs, same stop decisions, so vis_count is identical."""
+    import torch
+    from paper_2501_08174_b200 import binding as B
+    sc = sg.random_scene(9000, 16, 16, 40.0, seed=41, sh_degree=0, scale_lo=0.2, scale_hi=0.5, op_mu=-5.0, op_sigma=0.5)
+    r = full_parity(sc, 0, dict(sh_degree=0, bg=(0.2, 0.1, 0.3)), max_fragile=0.25, check_prune=True, label="one-tile-9000")
+    L = r["ranges"][:, 1] - r["ranges"][:, 0]
+    assert L.max() > 6144
+    P, m = arrays(sc), sc.mask(0)
+    g = GpuView(P, sc.cameras[0], dict(sh_degree=0))
+    g.preprocess(); g.bin_sort(want_ids=False)
+    gf = g.render_fwd(mask=m)
+    assert int((gf["vis_count"] > 0).sum()) > 4096  # the blended list is long enough for the backward clusters
+    vis_s = torch.zeros(g.n, dtype=torch.int32, device="cuda"); cs_s = torch.zeros(g.n, device="cuda")
+    B.ocgs_visibility_pass(g.surfels, g.cam, g.cfg, g.ws, g.cap, vis_s, cs_s)
+    torch.cuda.synchronize()
+    assert np.array_equal(vis_s.cpu().numpy().view(np.uint32), gf["vis_count"])
+    assert np.allclose(cs_s.cpu().numpy(), gf["contrib_sum"], rtol=1e-5, atol=1e-7)
+
+
 def test_sh_degrees():
     sc = sg.random_scene(120, 48, 48, 40.0, seed=13, sh_degree=3)
     for deg in (0, 1, 2, 3):
