@@ -328,6 +328,19 @@ int ocgs_profile_end(void* stream, int max_out, float* ms_out, char* names_out, 
  * `stream` once before the launch.  Not part of any step. */
 int ocgs_peak_probe(int kind, int iters, float* d_out, size_t out_floats, double* ops_per_launch, void* stream);
 
+/* ---- diagnostics: the staging step of the raster kernels in isolation, three ways ("TMA where the layout
+ * allows ... cp.async.bulk.tensor.2d ... tile::gather4 ... probe it, fall back to LDG.128 / cp.async"; the renderer is PAPER.md:119) ----
+ * Enqueues ONE launch: 6 persistent CTAs of 256 threads per SM, each gathering `iters` batches of records (rows of `rec`, 24 floats =
+ * 96 bytes each, selected by consecutive windows of `ranks`) into shared memory and reading a sixth of every batch back.
+ * kind 0: __ldg + st.shared + __syncthreads, batches of 256 (what the raster kernels do); kind 1: cp.async 16 B, double-buffered
+ * batches of 128; kind 2: TMA cp.async.bulk.tensor.2d tile::gather4 over a [n_rec, 24] fp32 tensor map + mbarrier, double-buffered
+ * batches of 128 (needs a driver that exports cuTensorMapEncodeTiled, else OCGS_ERR_UNSUPPORTED).
+ * rec: device f32 [n_rec, 24], 128-byte aligned; ranks: device u32 [n_ranks], every value < n_rec, n_ranks >= 256;
+ * d_out: device f32 [out_floats], out_floats >= 6 x 256 x number of SMs: per-thread sums of what was read (the test's evidence that
+ * the right rows arrived); *bytes_per_launch (host): record bytes gathered by the launch.  Asynchronous; not part of any step. */
+int ocgs_staging_probe(int kind, const float* rec, const uint32_t* ranks, uint32_t n_rec, uint32_t n_ranks, int iters, float* d_out,
+                       size_t out_floats, double* bytes_per_launch, void* stream);
+
 /* ---- end-to-end TRAINING step: per-view inputs from the host, parameters resident on the device (bench.py "e2e") -------
  * What a training loop does per iteration (pick a view, render, losses, backpropagate): the model -- the
  * surfel parameters and their gradients -- lives in device memory (`surfels`, d_grad_*), the view's data come from the

@@ -19,7 +19,7 @@ OCGS_OK, OCGS_ERR_INVALID_ARG, OCGS_ERR_CAPACITY, OCGS_ERR_CUDA, OCGS_ERR_UNSUPP
 EXPORTS = ["ocgs_default_config", "ocgs_workspace_layout", "ocgs_workspace_bytes", "ocgs_last_cuda_error", "ocgs_check",
            "ocgs_preprocess", "ocgs_bin_sort", "ocgs_render_fwd", "ocgs_render_bwd", "ocgs_render_fwd_l1", "ocgs_render_fwd_reg", "ocgs_render_bwd_reg", "ocgs3d_preprocess", "ocgs3d_render_fwd", "ocgs_prune_workspace_bytes",
            "ocgs_prune_stats", "ocgs_compact_rows", "ocgs_densify_workspace_bytes", "ocgs_densify_accumulate", "ocgs_densify", "ocgs_step_host", "ocgs_step_view_host", "ocgs_step_view_host_enqueue", "ocgs_step_view_prefetch_enqueue", "ocgs_visibility_pass", "ocgs3d_visibility_pass", "ocgs_masked_l1", "ocgs_photometric_workspace_bytes", "ocgs_photometric_loss", "ocgs_regularizers_workspace_bytes", "ocgs_regularizers",
-           "ocgs_profile_begin", "ocgs_profile_end", "ocgs_peak_probe", "ocgs_masked_l1_static"]
+           "ocgs_profile_begin", "ocgs_profile_end", "ocgs_peak_probe", "ocgs_masked_l1_static", "ocgs_staging_probe"]
 
 
 class OcgsError(RuntimeError):
@@ -385,6 +385,14 @@ def ocgs_peak_probe(kind: int, iters: int, out, stream=None) -> float:
     ops = C.c_double(0.0)
     _ok("ocgs_peak_probe", lib().ocgs_peak_probe(C.c_int(kind), C.c_int(iters), _ptr(out), C.c_size_t(out.numel()), C.byref(ops), _stream(stream)))
     return float(ops.value)
+
+
+def ocgs_staging_probe(kind: int, rec, ranks, n_rec: int, n_ranks: int, iters: int, out, stream=None) -> float:
+    """Enqueue one launch of the staging microbenchmark (0: __ldg, 1: cp.async, 2: TMA gather4); -> record bytes it gathers."""
+    nbytes = C.c_double(0.0)
+    _ok("ocgs_staging_probe", lib().ocgs_staging_probe(C.c_int(kind), _ptr(rec), _ptr(ranks), C.c_uint(n_rec), C.c_uint(n_ranks), C.c_int(iters),
+                                                        _ptr(out), C.c_size_t(out.numel()), C.byref(nbytes), _stream(stream)))
+    return float(nbytes.value)
 
 
 # ---- allocation helpers (device memory only; no arithmetic) --------------------------------------------------------
