@@ -163,9 +163,15 @@ constexpr int kBwdLeanMinBlocks = OCGS_BWD_LEAN_BLOCKS;  // the colour / alpha-o
 // (Horner from the back: G' <- alpha (g.q) + (1 - alpha) G'), the true values are linear in the transmittance in front of the
 // part, T_front,r = prod_{r' < r} P_r':   g.S at the back of part r = g.S_tail + sum_{r' > r} T_front,r' G'_r', T there = T_front,r+1.
 // P and G' travel through distributed shared memory; then every CTA runs the ordinary walk of its part.
+#ifndef OCGS_BWD_SEG_LEN
+#define OCGS_BWD_SEG_LEN 3072
+#endif
+#ifndef OCGS_BWD_SEG_TILES
+#define OCGS_BWD_SEG_TILES 128
+#endif
 constexpr int kBwdSegParts = 4;
-constexpr uint32_t kBwdSegLen = 4096;
-constexpr int kBwdSegMaxTiles = 128;
+constexpr uint32_t kBwdSegLen = OCGS_BWD_SEG_LEN;
+constexpr int kBwdSegMaxTiles = OCGS_BWD_SEG_TILES;
 namespace cg = cooperative_groups;
 
 template <bool kMoments, bool kGeo, bool kSegB = false>
