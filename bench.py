@@ -165,26 +165,27 @@ def alu_peaks(B, torch, dev):
     launches of ~1 ms, CUDA events on the launching stream.  SURVEY.md 8(d): the rooflines of the raster kernels are quoted
     against THESE, not against unit counts x clock."""
     props = torch.cuda.get_device_properties(dev)
-    out = torch.empty(props.multi_processor_count * 8 * 256 + 64, dtype=torch.float32, device=dev)
+    out = torch.empty(props.multi_processor_count * 8 * 256, dtype=torch.float32, device=dev)
     res = {}
     # kind 0: scalar FFMA with uniform (constant) b, c -- THE peak the rooflines are quoted against; 2: scalar FFMA with three register
-    # operands, the form real kernels issue (register-file bound: measured 48 TFLOP/s); 3: packed fma.rn.f32x2 (FFMA2), register operands
-    for kind, key in ((0, "fp32_tflops_measured"), (1, "ex2_tops_measured"), (2, "fp32_tflops_3reg_measured"), (3, "fp32x2_tflops_measured")):
-        iters = 2048 if kind == 0 else 256
+    # operands, the form real kernels issue (register-file bound: measured 48 TFLOP/s); 3 / 4: packed fma.rn.f32x2 (FFMA2) with b, c
+    # as broadcast scalars / as full register pairs
+    for kind, key in ((0, "fp32_tflops_measured"), (1, "ex2_tops_measured"), (2, "fp32_tflops_3reg_measured"), (3, "fp32x2_bcast_tflops_measured"),
+                      (4, "fp32x2_pairs_tflops_measured")):
+        iters = 256 if kind == 1 else 2048  # ~1 ms per launch for every kind (EX2 issues at 1/16 of the FMA rate)
         best = 0.0
-        for rep_i in range(6):
+        for rep_i in range(13):
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize()
             e0.record()
             ops = B.ocgs_peak_probe(kind, iters, out)
             e1.record()
             torch.cuda.synchronize()
-            if rep_i:  # the first launch warms up
+            if rep_i >= 3:  # the first launches warm up (clocks, instruction cache)
                 best = max(best, ops / (e0.elapsed_time(e1) * 1e-3) / 1e12)
         res[key] = best
     res["how"] = ("ocgs_peak_probe: 8 independent chains per thread of a <- fma(a,b,c) (2 flop; b, c uniform = fp32_tflops_measured, the roofline "
-                  "peak; b, c in registers = fp32_tflops_3reg_measured; packed fma.rn.f32x2 = fp32x2_tflops_measured) / a <- -ex2(a), "
-                  "8 blocks x 256 threads per SM, best of 5 launches, CUDA events")
+                  "peak; b, c in registers = fp32_tflops_3reg_measured; packed fma.rn.f32x2 with b, c broadcast scalars / full pairs = fp32x2_bcast_ / fp32x2_pairs_tflops_measured) / a <- -ex2(a), "
+                  "8 blocks x 256 threads per SM, best of 10 launches after 3 warm-up launches, CUDA events")
     res["sm_count"] = props.multi_processor_count
     res["fp32_tflops_derived"] = ALU_PEAK_TFLOPS_DERIVED
     return res

@@ -320,12 +320,12 @@ int ocgs_profile_end(void* stream, int max_out, float* ms_out, char* names_out, 
  * MUFU.EX2 peak microbenchmark on the box and use those" for the rooflines of the raster kernels, PAPER.md:119 renderer) ----
  * Enqueues ONE launch of a microbenchmark on `stream`: kind 0 = eight independent chains of a <- fma(a, b, c) per thread
  * (2 flop per step; b, c uniform operands), kind 1 = eight chains of a <- -ex2(a) (one MUFU.EX2 per step), kind 2 = kind 0 with
- * b, c in registers (the three-register FFMA real kernels issue), kind 3 = packed fma.rn.f32x2 chains (FFMA2, 4 flop per step,
- * register operands); 8 blocks of 256 threads per SM, `iters` x 8 steps per chain.  *ops_per_launch (host) receives the flop
- * (kinds 0, 2, 3) or EX2 (kind 1) count of the launch; the caller times the launch with CUDA events and divides.
- * d_out: device f32[out_floats], out_floats >= 8 x 256 x number of SMs (+ 16 for kinds 2, 3; OCGS_ERR_CAPACITY otherwise),
- * scratch the kernels store their results to.  Kinds 0, 1 are asynchronous; kinds 2, 3 upload their 16 operands and synchronise
- * `stream` once before the launch.  Not part of any step. */
+ * b, c in registers (the three-register FFMA real kernels issue), kinds 3 / 4 = packed fma.rn.f32x2 chains (SASS FFMA2, 4 flop per
+ * step) with b, c as scalars broadcast to both halves (kind 3) or as full pairs (kind 4); 8 blocks of 256 threads per SM,
+ * `iters` x 8 steps per chain.  *ops_per_launch (host) receives the flop (kinds 0, 2, 3, 4) or EX2 (kind 1) count of the launch;
+ * the caller times the launch with CUDA events and divides.
+ * d_out: device f32[out_floats], out_floats >= 8 x 256 x number of SMs (OCGS_ERR_CAPACITY otherwise), scratch the kernels store
+ * their results to.  Asynchronous; not part of any step. */
 int ocgs_peak_probe(int kind, int iters, float* d_out, size_t out_floats, double* ops_per_launch, void* stream);
 
 /* ---- diagnostics: the staging step of the raster kernels in isolation, three ways ("TMA where the layout

@@ -44,12 +44,18 @@ __global__ void __launch_bounds__(256) ex2_peak_kernel(float* __restrict__ out, 
   out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
-// kind 2: the same chains with b and c in REGISTERS (loaded from memory, so that they cannot become constant-bank operands):
-// the three-register form real kernels issue
-__global__ void __launch_bounds__(256) fma3_peak_kernel(float* __restrict__ out, int iters, const float* __restrict__ bc) {
+// kind 2: the same chains with b and c in REGISTERS: the values arrive as kernel arguments and take a round trip through volatile
+// shared memory, after which they are per-thread values to the compiler -- it can neither fold them into uniform / constant-bank
+// operands nor share one register between the chains: the three-register form real kernels issue
+__global__ void __launch_bounds__(256) fma3_peak_kernel(float* __restrict__ out, int iters, float b_in, float c_in) {
+  __shared__ volatile float s_bc[2][256];
+  s_bc[0][threadIdx.x] = b_in; s_bc[1][threadIdx.x] = c_in;
+  __syncthreads();
   float a[kPeakChains], b[kPeakChains], c[kPeakChains];
 #pragma unroll
-  for (int k = 0; k < kPeakChains; ++k) { a[k] = (float)(threadIdx.x + k) * 1e-3f; b[k] = bc[k]; c[k] = bc[kPeakChains + k]; }
+  for (int k = 0; k < kPeakChains; ++k) {
+    a[k] = (float)(threadIdx.x + k) * 1e-3f; b[k] = s_bc[0][(threadIdx.x + k) & 255]; c[k] = s_bc[1][(threadIdx.x + 2 * k) & 255];
+  }
 #pragma unroll 1
   for (int i = 0; i < iters; ++i) {
 #pragma unroll
@@ -63,15 +69,24 @@ __global__ void __launch_bounds__(256) fma3_peak_kernel(float* __restrict__ out,
   out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
-// kind 3: packed fp32 (fma.rn.f32x2, sm_100): kPeakChains chains of TWO fused multiply-adds per instruction, operands in registers
-__global__ void __launch_bounds__(256) fma2_peak_kernel(float* __restrict__ out, int iters, const float* __restrict__ bc) {
+// kinds 3, 4: packed fp32 (fma.rn.f32x2, sm_100; SASS FFMA2): kPeakChains chains of TWO fused multiply-adds per instruction, operands
+// in registers.  kBroadcast (kind 3): b and c are pairs {x, x} -- ptxas turns them into FFMA2's scalar-broadcast operand form
+// (`FFMA2 Rd, Ra.F32x2.HI_LO, Rb.F32, Rc.F32`: four registers read); kind 4: b and c are pairs of two different values (`...,
+// Rb.F32x2.HI_LO, Rc.F32x2.HI_LO`: six registers read, register-file bound like the three-register scalar FFMA)
+template <bool kBroadcast>
+__global__ void __launch_bounds__(256) fma2_peak_kernel(float* __restrict__ out, int iters, float b_in, float c_in) {
+  __shared__ volatile float s_bc[2][256];
+  s_bc[0][threadIdx.x] = b_in; s_bc[1][threadIdx.x] = c_in;
+  __syncthreads();
   unsigned long long a[kPeakChains], b[kPeakChains], c[kPeakChains];
 #pragma unroll
   for (int k = 0; k < kPeakChains; ++k) {
     const float a0 = (float)(threadIdx.x + k) * 1e-3f, a1 = a0 + 0.5f;
+    const float b0 = s_bc[0][(threadIdx.x + k) & 255], b1 = kBroadcast ? b0 : s_bc[0][(threadIdx.x + k + 8) & 255];
+    const float c0 = s_bc[1][(threadIdx.x + 2 * k) & 255], c1 = kBroadcast ? c0 : s_bc[1][(threadIdx.x + 2 * k + 1) & 255];
     asm("mov.b64 %0, {%1, %2};" : "=l"(a[k]) : "f"(a0), "f"(a1));
-    asm("mov.b64 %0, {%1, %2};" : "=l"(b[k]) : "f"(bc[k]), "f"(bc[k]));
-    asm("mov.b64 %0, {%1, %2};" : "=l"(c[k]) : "f"(bc[kPeakChains + k]), "f"(bc[kPeakChains + k]));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b[k]) : "f"(b0), "f"(b1));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(c[k]) : "f"(c0), "f"(c1));
   }
 #pragma unroll 1
   for (int i = 0; i < iters; ++i) {
@@ -94,7 +109,7 @@ __global__ void __launch_bounds__(256) fma2_peak_kernel(float* __restrict__ out,
 
 extern "C" int ocgs_peak_probe(int kind, int iters, float* d_out, size_t out_floats, double* ops_per_launch, void* stream) {
   using namespace ocgs;
-  if (!d_out || !ops_per_launch || iters <= 0 || kind < 0 || kind > 3) return OCGS_ERR_INVALID_ARG;
+  if (!d_out || !ops_per_launch || iters <= 0 || kind < 0 || kind > 4) return OCGS_ERR_INVALID_ARG;
   int dev = 0, sms = 0;
   OCGS_CUDA_OK(cudaGetDevice(&dev));
   OCGS_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -102,16 +117,13 @@ extern "C" int ocgs_peak_probe(int kind, int iters, float* d_out, size_t out_flo
   if (out_floats < (size_t)blocks * 256) return OCGS_ERR_CAPACITY;
   const double steps = (double)blocks * 256.0 * (double)iters * 8.0 * (double)kPeakChains;
   cudaStream_t st = (cudaStream_t)stream;
-  if (kind == 2 || kind == 3) {
-    // b, c of the register-operand forms are 16 floats BEHIND the kernels' result slots (d_out[blocks * 256 ...]), uploaded here
-    float h[2 * kPeakChains];
-    for (int k = 0; k < kPeakChains; ++k) { h[k] = 0.999f; h[kPeakChains + k] = 1e-3f; }
-    if (out_floats < (size_t)blocks * 256 + 2 * kPeakChains) return OCGS_ERR_CAPACITY;
-    float* bc = d_out + (size_t)blocks * 256;
-    OCGS_CUDA_OK(cudaMemcpyAsync(bc, h, sizeof(h), cudaMemcpyHostToDevice, st));
-    OCGS_CUDA_OK(cudaStreamSynchronize(st));  // (h is a stack buffer; diagnostic call, not part of any step)
-    if (kind == 2) { fma3_peak_kernel<<<blocks, 256, 0, st>>>(d_out, iters, bc); *ops_per_launch = 2.0 * steps; }
-    else { fma2_peak_kernel<<<blocks, 256, 0, st>>>(d_out, iters, bc); *ops_per_launch = 4.0 * steps; }
+  if (kind == 2) {
+    fma3_peak_kernel<<<blocks, 256, 0, st>>>(d_out, iters, 0.999f, 1e-3f);
+    *ops_per_launch = 2.0 * steps;
+  } else if (kind == 3 || kind == 4) {
+    if (kind == 3) fma2_peak_kernel<true><<<blocks, 256, 0, st>>>(d_out, iters, 0.999f, 1e-3f);
+    else fma2_peak_kernel<false><<<blocks, 256, 0, st>>>(d_out, iters, 0.999f, 1e-3f);
+    *ops_per_launch = 4.0 * steps;
   } else if (kind == 0) {
     fma_peak_kernel<<<blocks, 256, 0, st>>>(d_out, iters, 0.999f, 1e-3f);
     *ops_per_launch = 2.0 * steps;  // flop
