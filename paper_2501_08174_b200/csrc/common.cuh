@@ -31,7 +31,10 @@ enum GradField {
   G_D0, G_ZJ, G_CX, G_CY, G_COUNT
 };
 
-constexpr int kSortItems = 16;                       // keys per thread in a radix pass
+#ifndef OCGS_SORT_ITEMS
+#define OCGS_SORT_ITEMS 16
+#endif
+constexpr int kSortItems = OCGS_SORT_ITEMS;           // keys per thread in a radix pass
 constexpr int kSortThreads = 256;
 constexpr int kSortTile = kSortItems * kSortThreads;  // 4096 keys per block
 constexpr int kRadixBits = 8;

@@ -24,7 +24,13 @@ __device__ __forceinline__ unsigned long long load_count(const void* n_ptr, bool
 // Status word = 2 flag bits | 30-bit count, so a plain 32-bit store/load carries flag and value together.
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kFlagMask = 3u << 30, kValMask = (1u << 30) - 1u;
 constexpr int kMaxPasses = 4;
-
+#ifndef OCGS_SORT_LOOKBACK_WIDTH
+#define OCGS_SORT_LOOKBACK_WIDTH 4
+#endif
+// Predecessors whose status words one step of the look-back loads at once (independent, coalesced loads): the look-back is a chain
+// of dependent L2 round trips and a pass, one wave of blocks at these sizes, is as long as that chain
+// (profiles/r02_config3_radix_passes_full.md); width 1 is the textbook walk.
+constexpr int kLookbackWidth = OCGS_SORT_LOOKBACK_WIDTH;
 constexpr int kHistItems = 4;  // keys per thread and unit of work of the histogram kernel (finer than a sort tile: more blocks in flight)
 __global__ void __launch_bounds__(kSortThreads) radix_hist_all_kernel(const uint32_t* __restrict__ keys, const void* n_ptr, bool n_is_u64,
                                                                       size_t n_cap, int key_bits, int passes, uint32_t* __restrict__ ghist,
@@ -67,7 +73,11 @@ __global__ void __launch_bounds__(kSortThreads) radix_hist_all_kernel(const uint
   }
 }
 
-constexpr int kSortCtas = 3;  // resident blocks per SM the register budget is held to (80 registers; six passes at config 3: 200 us with 2, 178 with 3, 199 with 4)
+#ifndef OCGS_SORT_CTAS
+#define OCGS_SORT_CTAS 3
+#endif
+constexpr int kSortCtas = OCGS_SORT_CTAS;  // resident blocks per SM the register budget is held to (80 registers; six passes at config 3: 200 us with 2, 178 with 3, 199 with 4;
+                                           // with the 4-wide look-back: 161 us; 2048-key tiles (OCGS_SORT_ITEMS=8) 179 / 166 / 172 us with 3 / 4 / 6)
 __global__ void __launch_bounds__(kSortThreads, kSortCtas) radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
                                                                       uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
                                                                       const void* n_ptr, bool n_is_u64, size_t n_cap, int shift, uint32_t mask,
@@ -161,14 +171,22 @@ __global__ void __launch_bounds__(kSortThreads, kSortCtas) radix_onesweep_kernel
   // ---- decoupled look-back: keys of digit d in preceding tiles --------------------------------------------------
   uint32_t excl = 0;
   if (tile > 0) {
-    int p = (int)tile - 1;
-    while (true) {
-      const uint32_t sv = *(volatile uint32_t*)(status + (size_t)p * kRadix + d);
-      const uint32_t fl = sv & kFlagMask;
-      if (fl == 0) continue;  // predecessor has not published yet (it is running: tickets are taken in order)
-      excl += sv & kValMask;
-      if (fl == kFlagIncl) break;
-      --p;  // p >= 0 always: tile 0 publishes inclusive
+    int p = (int)tile - 1;  // the next predecessor to account for; tile 0 publishes inclusive, so the walk ends at or before it
+    while (p >= 0) {
+      uint32_t w[kLookbackWidth];
+#pragma unroll
+      for (int k = 0; k < kLookbackWidth; ++k)
+        w[k] = p - k >= 0 ? *(volatile uint32_t*)(status + (size_t)(p - k) * kRadix + d) : (uint32_t)(2u << 30);  // before tile 0: kFlagIncl | 0
+      bool stop = false;
+#pragma unroll
+      for (int k = 0; k < kLookbackWidth; ++k) {
+        if (stop) continue;
+        const uint32_t fl = w[k] & kFlagMask;
+        if (fl == 0) { stop = true; continue; }  // not published yet (it is running: tickets are taken in order): load again from p
+        excl += w[k] & kValMask;
+        --p;
+        if (fl == kFlagIncl) { p = -1; stop = true; }
+      }
     }
     *st = kFlagIncl | (excl + total);
   }
