@@ -139,6 +139,7 @@ int radix_sort_pairs(uint32_t* keysA, uint32_t* valsA, uint32_t* keysB, uint32_t
 // MUFU approximations (1-2 ulp, flush-to-zero): enough for the 1e-4 / 1e-3 tolerances, no denormal fix-up code
 __device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float ex2_approx(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float sqrt_approx(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 constexpr float kNegHalfLog2e = -0.72134752044448170f;  // exp(-rho/2) = 2^(rho * -0.5 log2 e)
 #endif
 

@@ -21,7 +21,8 @@ constexpr float kContribFix = 134217728.0f;    // 2^27: alpha*T in fixed point f
 //   i.e. A dx^2 - 2 B dx + C <= 0 with A = P.WP, B = S.WP, C = S.WS: real roots (B -+ sqrt(B^2 - AC))/A must overlap the
 //   block's dx range; rho2 <= rc is a disc of radius sqrt(rc sigma_f^2) about the centre.
 // Every inequality is relaxed (rc by 1e-4 relative + 1e-4, the dx range by 0.01 px, the discriminant by 1e-5 of its
-// term magnitudes), far more than the fp32 error of either this test or the per-pixel evaluation, so a pair the walk
+// term magnitudes), far more than the fp32 error of either this test (approximate square root included: 2^-22 relative, < 1e-3 px
+// on a root interval 1000 px wide) or the per-pixel evaluation, so a pair the walk
 // would blend is never culled: the images are bit-identical with and without the cull.
 __device__ __forceinline__ bool block_may_contribute(const float4 r0, const float4 r1, const float4 r2, const float4 r3, int x0, int y0,
                                                      float inv_sigma2) {
@@ -43,7 +44,7 @@ __device__ __forceinline__ bool block_may_contribute(const float4 r0, const floa
     const float Cp = fmaf(Sx, Sx, Sy * Sy), Cn = rc * Sz * Sz;
     const float B = fmaf(Sx, Px, fmaf(Sy, Py, -rc * Sz * Pz));
     const float disc = fmaf(B, B, -A * (Cp - Cn)) + 1e-5f * (Ap + An) * (Cp + Cn);
-    const float sq = sqrtf(fmaxf(disc, 0.0f));
+    const float sq = sqrt_approx(fmaxf(disc, 0.0f));  // one MUFU: sqrtf takes its slow path (a call) at 0, i.e. on every row that misses
     keep |= disc >= 0.0f && (B - sq) <= A * dxb && (B + sq) >= A * dxa;
   }
   return keep;
@@ -65,7 +66,7 @@ __device__ __forceinline__ bool block_may_contribute3d(const float4 r0, const fl
     const float dy = (float)(y0 + row) - r2.w;
     const float B = -b * dy, Cp = c * dy * dy;
     const float disc = fmaf(B, B, -a * (Cp - rc)) + 1e-5f * a * (Cp + rc);
-    const float sq = sqrtf(fmaxf(disc, 0.0f));
+    const float sq = sqrt_approx(fmaxf(disc, 0.0f));  // one MUFU: sqrtf takes its slow path (a call) at 0, i.e. on every row that misses
     keep |= disc >= 0.0f && (B - sq) <= a * dxb && (B + sq) >= a * dxa;
   }
   return keep;
