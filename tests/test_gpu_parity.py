@@ -377,6 +377,25 @@ def test_empty_and_all_culled_and_capacity():
     torch.cuda.synchronize()
 
 
+def test_tile_ranges_key_counts_of_every_residue_mod_4():
+    # tile_ranges_kernel reads four keys per thread with one 16-byte load and the ragged end key by key: K = 1 .. and every residue of
+    # K mod 4, with a key capacity that is not a multiple of four either
+    seen = set()
+    for n, seed in [(1, 3), (2, 4), (3, 5), (5, 6), (9, 7), (14, 8), (23, 9), (37, 10)]:
+        sc = sg.random_scene(n, 48, 40, 30.0, seed=seed, sh_degree=0)
+        P, camn, kw = arrays(sc), sc.cameras[0], dict(sh_degree=0)
+        orc, cam, cfg, pre, srt, fw = oracle_view(P, camn, kw, mask=sc.mask(0))
+        for slack in (1, 2, 3):
+            g = GpuView(P, camn, kw, key_capacity=max(srt["K"], 1) + slack)
+            g.preprocess()
+            gs = g.bin_sort()
+            assert gs["error"] == 0 and gs["K"] == srt["K"]
+            assert np.array_equal(gs["tile_keys"], (srt["keys"] >> np.uint64(32)).astype(np.uint32))
+            assert np.array_equal(gs["ranges"], srt["ranges"])
+        seen.add(srt["K"] % 4)
+    assert seen == {0, 1, 2, 3}, seen
+
+
 def test_masked_l1_and_host_step_match_device_path():
     import torch
     from paper_2501_08174_b200 import binding as B
