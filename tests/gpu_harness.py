@@ -90,6 +90,8 @@ class GpuView:
     def render_bwd(self, gC=None, gA=None, gD=None, gN=None, mask="same", gM=None):
         torch, B = self.torch, self.B
         g = B.alloc_grads(self.n)
+        for v in g.values():  # every row must be WRITTEN by the call (culled surfels: zeros), not found clean
+            v.fill_(float("nan"))
 
         def dev(a):
             return None if a is None else torch.tensor(np.ascontiguousarray(a, np.float32), device="cuda")
