@@ -241,6 +241,7 @@ __global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) ren
     for (int c0 = 0; c0 < cnt && !all_done; c0 += 32) {
       uint32_t cntr = 0, fixr = 0;
       const int ce = min(32, cnt - c0);
+      if (__all_sync(0xFFFFFFFFu, done)) { all_done = true; break; }  // once per 32 entries (before their cull): finished lanes are predicated off below
       // entry-parallel cull: lane l tests entry c0 + l against this warp's pixel block; the walk visits the survivors
       bool keep = false;
       if (lane < ce) {
@@ -249,7 +250,6 @@ __global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) ren
                           : block_may_contribute3d(se[0], se[2], se[3], tx * kTile + sub_x0, ty * kTile + sub_y0);
       }
       uint32_t todo = __ballot_sync(0xFFFFFFFFu, keep);
-      if (__all_sync(0xFFFFFFFFu, done)) { all_done = true; break; }  // once per 32 entries: finished lanes are predicated off below
       if (kPrim == 0 && heavy) {
         // long lists (a lone CTA on its SM at the kernel's tail): kFwdIlp survivors per iteration, evaluated without branches so
         // that their latencies overlap; the blend itself stays in list order and keeps the arithmetic of the loop below
