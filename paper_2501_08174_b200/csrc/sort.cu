@@ -572,8 +572,25 @@ __global__ void __launch_bounds__(1024) order_tiles_kernel(const uint32_t* __res
   __shared__ uint32_t s_warp[32];
   __shared__ uint32_t s_maxw;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  // the first kPer x 1024 tiles (all of them up to 1920x1080) stay in registers: their loads are issued together and the two later
+  // passes do not read them again -- the kernel is ONE block on the step's critical path, twice per step, and a loop per pass was
+  // 3 x 8 dependent L2 round trips
+  constexpr int kPer = 8;
+  uint32_t wreg[kPer];
   uint32_t mx = 0;
-  for (int t = tid; t < n_tiles; t += 1024) {
+#pragma unroll
+  for (int i = 0; i < kPer; ++i) {
+    const int t = tid + i * 1024;
+    wreg[i] = 0;
+    if (t < n_tiles) wreg[i] = from_ranges ? ranges[2 * t + 1] - ranges[2 * t] : work[t];
+  }
+#pragma unroll
+  for (int i = 0; i < kPer; ++i) {
+    const int t = tid + i * 1024;
+    if (from_ranges && t < n_tiles) work[t] = wreg[i];
+    mx = max(mx, wreg[i]);
+  }
+  for (int t = tid + kPer * 1024; t < n_tiles; t += 1024) {
     uint32_t wk = from_ranges ? ranges[2 * t + 1] - ranges[2 * t] : work[t];
     if (from_ranges) work[t] = wk;
     mx = max(mx, wk);
@@ -591,7 +608,14 @@ __global__ void __launch_bounds__(1024) order_tiles_kernel(const uint32_t* __res
   __syncthreads();
   // bucket 0 = heaviest; any monotone map of the work onto the buckets will do (a float scale instead of a 64-bit division)
   const float scale = (float)kBuckets / ((float)s_maxw + 1.0f);
-  for (int t = tid; t < n_tiles; t += 1024) {
+#pragma unroll
+  for (int i = 0; i < kPer; ++i) {
+    if (tid + i * 1024 < n_tiles) {
+      const uint32_t b = (kBuckets - 1) - min((uint32_t)(kBuckets - 1), (uint32_t)((float)wreg[i] * scale));
+      atomicAdd(&s_cnt[b], 1u);
+    }
+  }
+  for (int t = tid + kPer * 1024; t < n_tiles; t += 1024) {
     const uint32_t b = (kBuckets - 1) - min((uint32_t)(kBuckets - 1), (uint32_t)((float)work[t] * scale));
     atomicAdd(&s_cnt[b], 1u);
   }
@@ -618,7 +642,15 @@ __global__ void __launch_bounds__(1024) order_tiles_kernel(const uint32_t* __res
   __syncthreads();
   s_cnt[tid] = (wid ? s_warp[wid - 1] : 0) + inc - c;
   __syncthreads();
-  for (int t = tid; t < n_tiles; t += 1024) {
+#pragma unroll
+  for (int i = 0; i < kPer; ++i) {
+    const int t = tid + i * 1024;
+    if (t < n_tiles) {
+      const uint32_t b = (kBuckets - 1) - min((uint32_t)(kBuckets - 1), (uint32_t)((float)wreg[i] * scale));
+      order[atomicAdd(&s_cnt[b], 1u)] = (uint32_t)t;
+    }
+  }
+  for (int t = tid + kPer * 1024; t < n_tiles; t += 1024) {
     const uint32_t b = (kBuckets - 1) - min((uint32_t)(kBuckets - 1), (uint32_t)((float)work[t] * scale));
     order[atomicAdd(&s_cnt[b], 1u)] = (uint32_t)t;
   }

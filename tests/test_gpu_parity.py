@@ -377,6 +377,13 @@ def test_empty_and_all_culled_and_capacity():
     torch.cuda.synchronize()
 
 
+def test_more_than_8192_tiles():
+    # order_tiles_kernel keeps the work of the first 8 x 1024 tiles in registers and loops over the rest: 2320x1040 = 145 x 65 = 9425
+    # tiles (ragged on both axes), a sparse scene so that the oracle finishes in seconds; forward and backward launch orders both
+    sc = sg.random_scene(500, 2320, 1040, 1500.0, seed=11, sh_degree=0, scale_lo=0.01, scale_hi=0.1)
+    full_parity(sc, 0, dict(sh_degree=0))
+
+
 def test_tile_ranges_key_counts_of_every_residue_mod_4():
     # tile_ranges_kernel reads four keys per thread with one 16-byte load and the ragged end key by key: K = 1 .. and every residue of
     # K mod 4, with a key capacity that is not a multiple of four either
