@@ -27,7 +27,7 @@ FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 40.0, 22.0, 72.0  # DESIGN.md sectio
 FLOP_BLEND_BWD_COLOUR_ONLY = 54.0  # no upstream gradient on depth / normal maps (masked L1 + L_b): those terms are not evaluated
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the raster kernels (bytes), from the `ncu --set full` capture of
 # this workload committed under profiles/ (NCU_TRAFFIC_SOURCE)
-NCU_TRAFFIC = {"render_bwd_kernel": 86.53e6, "render_fwd_kernel": 134.20e6}  # 82.28 + 4.24 MB; 65.67 + 68.53 MB (ordinary launches)
+NCU_TRAFFIC = {"render_bwd_kernel": 86.28e6, "render_fwd_kernel": 133.83e6}  # dram read + write of the two ordinary launches
 NCU_TRAFFIC_SOURCE = "profiles/r02b_config3_raster_kernels_full.md"
 # fallback only (used when the microbenchmark of ocgs_peak_probe cannot run): 148 SMs x 128 FP32 lanes x 2 (FMA) x max SM clock
 ALU_PEAK_TFLOPS_DERIVED = 148 * 128 * 2 * 1.965e9 / 1e12
