@@ -124,7 +124,8 @@ __global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) ren
   __shared__ uint32_t s_rank[kFwdBatch];
   __shared__ uint32_t s_hit[kFwdBatch];  // bit w: warp w blended the entry (read by the backward pass)
   __shared__ uint32_t s_cnt[kStats ? kFwdBatch : 1];
-  __shared__ unsigned long long s_fix[kStats ? kFwdBatch : 1];  // sum of alpha*T in 2^-27 fixed point
+  __shared__ uint2 s_fix[kStats ? kFwdBatch : 1];  // sum of alpha*T in 2^-27 fixed point, as (sum of the low 16 bits, sum of the high 16 bits) of
+                                                   // the warps' 32-bit terms: two native 32-bit shared atomics instead of a 64-bit CAS loop
   __shared__ float s_red[8];
   __shared__ uint32_t s_wcnt[8];
 
@@ -228,7 +229,7 @@ __global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) ren
     if (__syncthreads_and(done)) break;
     if ((int)threadIdx.x < cnt) s_rank[threadIdx.x] = list[b0 + threadIdx.x];
     if (kMaps && threadIdx.x < kFwdBatch) s_hit[threadIdx.x] = 0;
-    if (kStats && threadIdx.x < kFwdBatch) { s_cnt[threadIdx.x] = 0; s_fix[threadIdx.x] = 0ull; }
+    if (kStats && threadIdx.x < kFwdBatch) { s_cnt[threadIdx.x] = 0; s_fix[threadIdx.x] = make_uint2(0u, 0u); }
     __syncthreads();
     constexpr int kParts = kMaps ? 6 : 5;  // the last 16 bytes of a record hold the normal: not read by the statistics-only walk
     for (int i = threadIdx.x; i < cnt * kParts; i += 256) {
@@ -374,7 +375,8 @@ __global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) ren
         if (kMaps) atomicOr(&s_hit[c0 + lane], wbit);
         if (kStats) {
           atomicAdd(&s_cnt[c0 + lane], cntr);
-          atomicAdd(&s_fix[c0 + lane], (unsigned long long)fixr);
+          atomicAdd(&s_fix[c0 + lane].x, fixr & 0xFFFFu);
+          atomicAdd(&s_fix[c0 + lane].y, fixr >> 16);
         }
       }
     }
@@ -400,7 +402,7 @@ __global__ void __launch_bounds__(256, kSeg ? OCGS_SEG_MINB : kFwdMinBlocks) ren
       if ((int)threadIdx.x < cnt && s_cnt[threadIdx.x] > 0) {
         const uint32_t id = rank_to_id[s_rank[threadIdx.x]];
         atomicAdd(&vis_count[id], s_cnt[threadIdx.x]);
-        atomicAdd(&contrib_sum[id], (float)s_fix[threadIdx.x] * (1.0f / kContribFix));
+        atomicAdd(&contrib_sum[id], (float)(((unsigned long long)s_fix[threadIdx.x].y << 16) + s_fix[threadIdx.x].x) * (1.0f / kContribFix));
       }
     }
   }
