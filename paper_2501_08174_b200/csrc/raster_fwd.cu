@@ -77,7 +77,11 @@ __device__ __forceinline__ bool block_may_contribute3d(const float4 r0, const fl
 // forward 2.34 -> 2.04 ms with 2, 2.07 with 4, 2.09 with 3; used for every tile it costs 3 % at config 3).
 constexpr int kFwdIlp = 2;
 constexpr uint32_t kFwdHeavyLen = 2048;
-constexpr int kFwdMinBlocks = 6;               // CTAs per SM the register budget is held to (40 registers; 5 and 7 measured slower)
+#ifndef OCGS_FWD_MIN_BLOCKS
+#define OCGS_FWD_MIN_BLOCKS 6
+#endif
+constexpr int kFwdMinBlocks = OCGS_FWD_MIN_BLOCKS;  // CTAs per SM the register budget is held to (40 registers; 5 (48 registers, no spill) and 7 (32) measured
+                                                    // slower at the end of round 2 too: 0.677 / 0.680 vs 0.643 ms at config 3)
 // fused harness photometric term (S20): target image in, dL/dcolor and per-tile partial sums of |M (R - I)| out
 struct FwdL1 { const float* target; float* gC; float* partial; float inv_norm; };
 
